@@ -1,0 +1,110 @@
+"""Seeded synthetic workloads shared by tests, bench.py and smoke() -- inputs only.
+
+This module holds NO arithmetic of the method (no RNG of the method, no update rule, no
+reduction): it only names the run parameters of BASELINE.json's five configurations and
+produces seeded synthetic spin configurations for the upload / restart tests.  Both the oracle
+side and the CUDA side of a parity test take their inputs from here; neither side's code is
+imported here.
+
+The paper's workloads are self-generated lattices (ordered or random start, temperatures near
+T_c), so these parameter sets *are* the workload; nothing stands in
+for an external dataset.  Temperatures follow DESIGN.md reading S12:
+``Tc = 1.0 / log(1.0 + sqrt(q))`` (Eq. 2) and ``T = f * Tc`` in double.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field
+from typing import List
+
+import numpy as np
+
+INIT_ORDERED = 0
+INIT_RANDOM = 1
+
+
+def t_c(q: int) -> float:
+    """Exact transition temperature of the square-lattice Potts model, Eq. 2."""
+    return 1.0 / math.log(1.0 + math.sqrt(float(q)))
+
+
+@dataclass(frozen=True)
+class Workload:
+    name: str
+    q: int
+    L: int
+    init: int
+    seed: int
+    t_factors: List[float]        # temperatures as multiples of T_c, in the order they are run
+    sweeps_per_t: int
+    every: int                    # measure after every `every`-th sweep
+    hist: bool                    # record the q-bin histogram with the energy
+    packed: bool = False          # sub-byte packed spin layout
+    note: str = ""
+    temperatures: List[float] = field(default_factory=list, compare=False)
+
+    def __post_init__(self):
+        object.__setattr__(self, "temperatures", [f * t_c(self.q) for f in self.t_factors])
+
+    @property
+    def total_sweeps(self) -> int:
+        return self.sweeps_per_t * len(self.t_factors)
+
+    @property
+    def updates(self) -> int:
+        return self.total_sweeps * self.L * self.L
+
+
+def _scan16() -> List[float]:
+    # S11: 16 points uniformly in [0.98, 1.02] T_c, endpoints inclusive, run as a cooling
+    # ladder (k = 15 -> 0) on one lattice, configuration carried over.
+    return [0.98 + 0.04 * k / 15.0 for k in range(15, -1, -1)]
+
+
+# BASELINE.json configs[0..4]; seeds of cfg3..5 are this build's choice.
+CONFIGS = {
+    1: Workload("cfg1_q9_L64", q=9, L=64, init=INIT_RANDOM, seed=1, t_factors=[0.99],
+                sweeps_per_t=1000, every=1, hist=True,
+                note="small case the oracle finishes in seconds"),
+    2: Workload("cfg2_q6_L1024", q=6, L=1024, init=INIT_ORDERED, seed=7, t_factors=[1.005],
+                sweeps_per_t=10_000, every=1, hist=False,
+                note="heating run from the ordered state; headline bench workload"),
+    3: Workload("cfg3_q9_L4096", q=9, L=4096, init=INIT_RANDOM, seed=3, t_factors=_scan16(),
+                sweeps_per_t=2000, every=1, hist=True,
+                note="16-point temperature scan, cooling, state carried over"),
+    4: Workload("cfg4_q24_L8192", q=24, L=8192, init=INIT_ORDERED, seed=4, t_factors=[1.002],
+                sweeps_per_t=5000, every=1, hist=False, packed=True,
+                note="sub-byte packed layout"),
+    5: Workload("cfg5_q9_L32768", q=9, L=32768, init=INIT_RANDOM, seed=5, t_factors=[0.995],
+                sweeps_per_t=1000, every=10, hist=True,
+                note="1.07e9 spins, streams from HBM"),
+}
+
+
+def synthetic_spins(L: int, q: int, seed: int, kind: str = "domains") -> np.ndarray:
+    """Seeded L x L uint8 configuration for upload / restart tests.
+
+    kind: "uniform"  i.i.d. states (the disordered start),
+          "ordered"  all zero,
+          "domains"  a few large single-state patches with sparse i.i.d. defects -- the
+                     coarsening / nucleating states the paper's runs pass through near T_c,
+          "stripes"  horizontal bands (the metastable stripe states of cooling runs).
+    """
+    rng = np.random.default_rng(seed)
+    if kind == "uniform":
+        return rng.integers(0, q, size=(L, L), dtype=np.uint8)
+    if kind == "ordered":
+        return np.zeros((L, L), dtype=np.uint8)
+    if kind == "stripes":
+        band = max(1, L // 4)
+        rows = (np.arange(L) // band) % q
+        return np.repeat(rows[:, None], L, axis=1).astype(np.uint8)
+    if kind == "domains":
+        blk = max(2, L // 4)
+        nb = (L + blk - 1) // blk
+        coarse = rng.integers(0, q, size=(nb, nb), dtype=np.uint8)
+        s = np.kron(coarse, np.ones((blk, blk), dtype=np.uint8))[:L, :L]
+        defects = rng.random((L, L)) < 0.1
+        noise = rng.integers(0, q, size=(L, L), dtype=np.uint8)
+        return np.where(defects, noise, s).astype(np.uint8)
+    raise ValueError(kind)
