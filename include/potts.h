@@ -1,0 +1,149 @@
+/*
+ * potts.h -- C-ABI boundary of the B200-native checkerboard Metropolis sweep of the 2D q-state
+ * Potts model (arXiv 1101.0876; citations are PAPER.md:<line>, section/equation).
+ *
+ * The library implements, entirely in hand-written CUDA for sm_100a, the one data-parallel hot
+ * path of the paper: the red/black single-spin-flip Metropolis sweep (sec. 3,
+ * :141 sec. 3.1) of  H = -J sum_<ij> delta(s_i,s_j)  (Eq. 1) on an L x L periodic
+ * square lattice, and the per-sweep energy and q-state occupancy reduction (PAPER.md:175
+ * sec. 3.4) that feeds the metastability analysis (sec. 6).
+ *
+ * Conventions
+ *   - Every function returns a POTTS_* code and never throws.  On any error the out-parameters
+ *     are left untouched and potts_last_error() describes the failure (thread-local string).
+ *   - "host" / "device" is stated for every pointer.  Host buffers are caller-owned; the handle
+ *     owns its device memory until potts_destroy (or borrows the caller's workspace, see
+ *     potts_create_ex).
+ *   - All device work is enqueued on the handle's CUDA stream (default: the legacy default
+ *     stream; the Python binding installs torch's current stream).  potts_sweep may return
+ *     before the GPU finishes; every function that fills a host buffer synchronises the stream.
+ *   - One handle = one lattice.  Handles are independent.  A handle is not thread-safe.
+ *   - There is no CPU fallback: without a usable CUDA device every call fails with
+ *     POTTS_ERR_CUDA.
+ *
+ * The simulated chain (what the bits are), see DESIGN.md section 3 for the readings:
+ *   spins s in {0..q-1}; J = k_B = 1; sweep t = all sites with (i+j) even, then all with (i+j)
+ *   odd; per site (w0,w1,..) = Philox4x32-10(counter (j, i, t, colour), key seed); proposal
+ *   s' = floor(w0 q / 2^32); d = n_old - n_new over the 4 neighbours; accept iff d <= 0 or
+ *   w1 < floor(2^32 exp(-d/T)).  No floating point is used on the device.
+ */
+#ifndef POTTS_B200_H
+#define POTTS_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct potts_s potts_t; /* opaque */
+
+enum {
+    POTTS_OK = 0,
+    POTTS_ERR_ARG = 1,         /* null pointer, L < 2 or odd, q outside [2,256], T not finite or <= 0,
+                                  nsweeps < 0, every < 1 or not dividing nsweeps, bad init/layout,
+                                  spin value >= q in an upload, sweep counter would pass 2^32 - 1 */
+    POTTS_ERR_UNSUPPORTED = 2, /* L not a multiple of 32 (vector width of the kernels), or q too large
+                                  for the packed layout */
+    POTTS_ERR_NOMEM = 3,       /* device or host allocation failed / workspace too small */
+    POTTS_ERR_CUDA = 4         /* CUDA runtime error (no device, launch failure, ...) */
+};
+
+enum { POTTS_INIT_ORDERED = 0 /* all s = 0 */, POTTS_INIT_RANDOM = 1 /* uniform {0..q-1} from seed */ };
+
+enum {
+    POTTS_LAYOUT_U8 = 0,    /* one byte per spin, split by colour */
+    POTTS_LAYOUT_PACKED = 1 /* sub-byte: 4 bits per spin for q <= 16, 5 bits packed 6-per-word..
+                               see DESIGN.md section 5; results are bit-identical to U8 */
+};
+
+/* ---- lifetime ------------------------------------------------------------------------------
+ * potts_create: allocate an L x L lattice with q states (byte spins, q <= 256,
+ * PAPER.md:161), Philox key `seed`, start state `init` (ordered / random), sweep
+ * counter t = 0, layout U8, on the current CUDA device.  *out (host) receives the handle. */
+int potts_create(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t init);
+
+/* potts_create_ex: as potts_create, with a layout and optionally caller-provided device memory
+ * and stream.  If dev_workspace (device) is non-null it must hold at least
+ * potts_workspace_bytes(...) bytes, be 256-byte aligned, and outlive the handle (the handle
+ * does not free it); if null the library allocates.  cuda_stream is a cudaStream_t (may be
+ * null = legacy default stream). */
+int potts_create_ex(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t init, int32_t layout,
+                    void *dev_workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Bytes of device memory a handle needs (spin planes + accumulators).  *bytes is host. */
+int potts_workspace_bytes(int32_t L, int32_t q, int32_t layout, size_t *bytes);
+
+/* Install the cudaStream_t all later work of this handle is enqueued on. */
+int potts_set_stream(potts_t *h, void *cuda_stream);
+
+void potts_destroy(potts_t *h);
+
+/* ---- the hot path --------------------------------------------------------------------------
+ * potts_sweep: nsweeps checkerboard Metropolis sweeps at temperature T (PAPER.md:94, :141,
+ * :145).  The four acceptance thresholds floor(2^32 exp(-d/T)) are built on the host in double
+ * at every call.  Enqueues and returns; advances the sweep counter by nsweeps.
+ * potts_sweep(h,T,a); potts_sweep(h,T,b) is the same chain as potts_sweep(h,T,a+b). */
+int potts_sweep(potts_t *h, double T, int64_t nsweeps);
+
+/* potts_sweep_measured: as potts_sweep, and after every `every`-th sweep of this call record
+ * the energy E (Eq. 1, int64) and, if hist_series is non-null, the occupancies N_0..N_{q-1}
+ * ("one measure each delta-t steps").  E_series (host) has
+ * nsweeps/every entries, hist_series (host) nsweeps/every rows of q.  Synchronises. */
+int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every,
+                         int64_t *E_series, int64_t *hist_series);
+
+/* Same, with E_series / hist_series in DEVICE memory; enqueues and returns without a sync. */
+int potts_sweep_measured_dev(potts_t *h, double T, int64_t nsweeps, int64_t every,
+                             int64_t *E_series_dev, int64_t *hist_series_dev);
+
+/* ---- measurements (sec. 3.4) ---------------------------------------------------
+ * potts_energy: E = -(number of satisfied nearest-neighbour bonds), range [-2 L^2, 0].  *E host. */
+int potts_energy(potts_t *h, int64_t *E);
+
+/* potts_histogram: counts[k] = #{sites with s = k}, k = 0..q-1 (host, q entries, caller-owned). */
+int potts_histogram(potts_t *h, int64_t *counts);
+
+/* ---- state transfer --------------------------------------------------------------------------
+ * potts_download: spins (host, L*L bytes, row-major s[i*L + j]) <- current configuration.
+ * Together with potts_sweep_count this is a complete checkpoint (the RNG is stateless). */
+int potts_download(potts_t *h, uint8_t *spins);
+
+/* potts_upload: replace the configuration (host, L*L bytes, every value < q). */
+int potts_upload(potts_t *h, const uint8_t *spins);
+
+int potts_sweep_count(potts_t *h, uint64_t *t);
+int potts_set_sweep_count(potts_t *h, uint64_t t); /* checkpoint restore; t < 2^32 */
+
+/* ---- host-side derived observables in double (PAPER.md:73 Eq. 7, :209 Eq. 9) ----------------
+ * From an energy series of n samples of a lattice with N = L^2 sites at temperature T:
+ *   *mean_e = <E>/N,  *cv = (<E^2> - <E>^2)/(N T^2),  *binder = 1 - <E^4>/(3 <E^2>^2).
+ * Sums of E and E^2 are exact (128-bit integers), E^4 is summed compensated in long double.
+ * All pointers host; any out-pointer may be null. */
+int potts_observables(const int64_t *E_series, int64_t n, int64_t N, double T,
+                      double *mean_e, double *cv, double *binder);
+
+/* *m = (q N_max/N - 1)/(q - 1) from a histogram (host, q entries). */
+int potts_magnetisation(const int64_t *counts, int32_t q, double *m);
+
+/* ---- introspection / tuning -------------------------------------------------------------------
+ * potts_launch_count: kernels launched by this handle since creation (bench.py's gpu_launches). */
+int potts_launch_count(potts_t *h, uint64_t *n);
+
+/* potts_set_option: tuning knobs that change HOW the sweep is launched, never WHAT it computes
+ * (tests assert bit-identity across them).  Unknown key -> POTTS_ERR_ARG.  Keys: see DESIGN.md
+ * section 6 ("variant", "sweeps_per_launch", "use_graph"). */
+int potts_set_option(potts_t *h, const char *key, int64_t value);
+int potts_get_option(potts_t *h, const char *key, int64_t *value);
+
+/* Description of the last failure on this thread ("" if none). */
+const char *potts_last_error(void);
+
+/* Library version string, e.g. "potts-b200 0.1 (sm_100a)". */
+const char *potts_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* POTTS_B200_H */

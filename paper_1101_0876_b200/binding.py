@@ -1,0 +1,228 @@
+"""Thin Python binding of the C-ABI in include/potts.h (same names, argument marshalling only).
+
+Every step of the hot path runs in the CUDA kernels of ``csrc/``; this module only converts
+arguments.  PyTorch supplies device memory (the lattice workspace is a ``torch.uint8`` CUDA
+tensor handed to ``potts_create_ex``) and the stream (torch's current stream).  There is no CPU
+fallback: if the shared library is missing or no CUDA device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpotts_b200.so")
+
+OK, ERR_ARG, ERR_UNSUPPORTED, ERR_NOMEM, ERR_CUDA = 0, 1, 2, 3, 4
+INIT_ORDERED, INIT_RANDOM = 0, 1
+LAYOUT_U8, LAYOUT_PACKED = 0, 1
+
+_lib = None
+
+
+class PottsError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"potts error {code}: {msg}")
+        self.code = code
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen the in-tree library; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_1101_0876_b200.build` "
+            "(or __graft_entry__.build()); there is no CPU fallback")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i32, i64, u64, dbl = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_uint64, ctypes.c_double
+    P = ctypes.POINTER
+    sigs = {
+        "potts_create": ([P(vp), i32, i32, u64, i32], ctypes.c_int),
+        "potts_create_ex": ([P(vp), i32, i32, u64, i32, i32, vp, ctypes.c_size_t, vp], ctypes.c_int),
+        "potts_workspace_bytes": ([i32, i32, i32, P(ctypes.c_size_t)], ctypes.c_int),
+        "potts_set_stream": ([vp, vp], ctypes.c_int),
+        "potts_destroy": ([vp], None),
+        "potts_sweep": ([vp, dbl, i64], ctypes.c_int),
+        "potts_sweep_measured": ([vp, dbl, i64, i64, vp, vp], ctypes.c_int),
+        "potts_sweep_measured_dev": ([vp, dbl, i64, i64, vp, vp], ctypes.c_int),
+        "potts_energy": ([vp, P(i64)], ctypes.c_int),
+        "potts_histogram": ([vp, vp], ctypes.c_int),
+        "potts_download": ([vp, vp], ctypes.c_int),
+        "potts_upload": ([vp, vp], ctypes.c_int),
+        "potts_sweep_count": ([vp, P(u64)], ctypes.c_int),
+        "potts_set_sweep_count": ([vp, u64], ctypes.c_int),
+        "potts_observables": ([vp, i64, i64, dbl, P(dbl), P(dbl), P(dbl)], ctypes.c_int),
+        "potts_magnetisation": ([vp, i32, P(dbl)], ctypes.c_int),
+        "potts_launch_count": ([vp, P(u64)], ctypes.c_int),
+        "potts_set_option": ([vp, ctypes.c_char_p, i64], ctypes.c_int),
+        "potts_get_option": ([vp, ctypes.c_char_p, P(i64)], ctypes.c_int),
+        "potts_last_error": ([], ctypes.c_char_p),
+        "potts_version": ([], ctypes.c_char_p),
+    }
+    for name, (argtypes, restype) in sigs.items():
+        fn = getattr(lib, name)          # AttributeError if the symbol is not exported
+        fn.argtypes = argtypes
+        fn.restype = restype
+    _lib = lib
+    return lib
+
+
+EXPORTED_SYMBOLS = [
+    "potts_create", "potts_create_ex", "potts_workspace_bytes", "potts_set_stream", "potts_destroy",
+    "potts_sweep", "potts_sweep_measured", "potts_sweep_measured_dev", "potts_energy", "potts_histogram",
+    "potts_download", "potts_upload", "potts_sweep_count", "potts_set_sweep_count", "potts_observables",
+    "potts_magnetisation", "potts_launch_count", "potts_set_option", "potts_get_option", "potts_last_error",
+    "potts_version",
+]
+
+
+def _check(rc: int):
+    if rc != OK:
+        raise PottsError(rc, load_library().potts_last_error().decode())
+
+
+def potts_version() -> str:
+    return load_library().potts_version().decode()
+
+
+def potts_workspace_bytes(L: int, q: int, layout: int = LAYOUT_U8) -> int:
+    n = ctypes.c_size_t(0)
+    _check(load_library().potts_workspace_bytes(L, q, layout, ctypes.byref(n)))
+    return int(n.value)
+
+
+def potts_observables(E_series, N: int, T: float):
+    """-> (mean_e, c_v, binder) in double, computed by the library on the host."""
+    E = np.ascontiguousarray(E_series, dtype=np.int64)
+    a, b, c = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    _check(load_library().potts_observables(E.ctypes.data, E.size, int(N), float(T),
+                                            ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
+    return a.value, b.value, c.value
+
+
+def potts_magnetisation(counts, q: int) -> float:
+    H = np.ascontiguousarray(counts, dtype=np.int64)
+    m = ctypes.c_double()
+    _check(load_library().potts_magnetisation(H.ctypes.data, int(q), ctypes.byref(m)))
+    return m.value
+
+
+class Potts:
+    """One lattice on the current CUDA device.  Methods mirror the C entry points one to one."""
+
+    def __init__(self, L: int, q: int, seed: int, init: int = INIT_ORDERED, layout: int = LAYOUT_U8,
+                 device: Optional[int] = None):
+        import torch
+
+        self._lib = load_library()
+        if not torch.cuda.is_available():
+            raise PottsError(ERR_CUDA, "no CUDA device: the Potts sweep has no CPU fallback")
+        self._torch = torch
+        self.device = torch.device("cuda", torch.cuda.current_device() if device is None else device)
+        self.L, self.q, self.seed, self.layout = int(L), int(q), int(seed), int(layout)
+        nbytes = potts_workspace_bytes(self.L, self.q, self.layout)
+        with torch.cuda.device(self.device):
+            # device memory from torch's caching allocator; the handle borrows it
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = self._ws.data_ptr()
+            off = (-base) % 256
+            h = ctypes.c_void_p()
+            _check(self._lib.potts_create_ex(ctypes.byref(h), self.L, self.q, self.seed, int(init), self.layout,
+                                             ctypes.c_void_p(base + off), nbytes, self._stream_ptr()))
+        self._h = h
+
+    # -- plumbing ---------------------------------------------------------------------------
+    def _stream_ptr(self):
+        return ctypes.c_void_p(self._torch.cuda.current_stream(self.device).cuda_stream)
+
+    def _sync_stream(self):
+        _check(self._lib.potts_set_stream(self._h, self._stream_ptr()))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._torch.cuda.synchronize(self.device)
+            self._lib.potts_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C-ABI, name for name -------------------------------------------------------------
+    def potts_sweep(self, T: float, nsweeps: int):
+        self._sync_stream()
+        _check(self._lib.potts_sweep(self._h, float(T), int(nsweeps)))
+
+    def potts_sweep_measured(self, T: float, nsweeps: int, every: int = 1, hist: bool = True):
+        """-> (E_series int64[n/every], hist_series int64[n/every, q] or None) on the host."""
+        self._sync_stream()
+        ns = int(nsweeps) // int(every) if every >= 1 and nsweeps >= 0 else 0
+        E = np.zeros(ns, dtype=np.int64)
+        H = np.zeros((ns, self.q), dtype=np.int64) if hist else None
+        _check(self._lib.potts_sweep_measured(self._h, float(T), int(nsweeps), int(every), E.ctypes.data,
+                                              H.ctypes.data if hist else None))
+        return E, H
+
+    def potts_sweep_measured_dev(self, T: float, nsweeps: int, every: int, E_dev, hist_dev=None):
+        """E_dev / hist_dev: torch.int64 CUDA tensors of nsweeps/every (x q) entries; no sync."""
+        self._sync_stream()
+        _check(self._lib.potts_sweep_measured_dev(
+            self._h, float(T), int(nsweeps), int(every),
+            ctypes.c_void_p(E_dev.data_ptr()) if E_dev is not None else None,
+            ctypes.c_void_p(hist_dev.data_ptr()) if hist_dev is not None else None))
+
+    def potts_energy(self) -> int:
+        self._sync_stream()
+        E = ctypes.c_int64()
+        _check(self._lib.potts_energy(self._h, ctypes.byref(E)))
+        return int(E.value)
+
+    def potts_histogram(self) -> np.ndarray:
+        self._sync_stream()
+        H = np.zeros(self.q, dtype=np.int64)
+        _check(self._lib.potts_histogram(self._h, H.ctypes.data))
+        return H
+
+    def potts_download(self, out: Optional[np.ndarray] = None) -> np.ndarray:
+        self._sync_stream()
+        if out is None:
+            out = np.empty((self.L, self.L), dtype=np.uint8)
+        assert out.dtype == np.uint8 and out.size == self.L * self.L and out.flags.c_contiguous
+        _check(self._lib.potts_download(self._h, out.ctypes.data))
+        return out
+
+    def potts_upload(self, spins: np.ndarray):
+        self._sync_stream()
+        a = np.ascontiguousarray(spins, dtype=np.uint8)
+        if a.size != self.L * self.L:
+            raise PottsError(ERR_ARG, "upload needs L*L spins")
+        _check(self._lib.potts_upload(self._h, a.ctypes.data))
+
+    def potts_sweep_count(self) -> int:
+        t = ctypes.c_uint64()
+        _check(self._lib.potts_sweep_count(self._h, ctypes.byref(t)))
+        return int(t.value)
+
+    def potts_set_sweep_count(self, t: int):
+        _check(self._lib.potts_set_sweep_count(self._h, int(t)))
+
+    def potts_launch_count(self) -> int:
+        n = ctypes.c_uint64()
+        _check(self._lib.potts_launch_count(self._h, ctypes.byref(n)))
+        return int(n.value)
+
+    def potts_set_option(self, key: str, value: int):
+        _check(self._lib.potts_set_option(self._h, key.encode(), int(value)))
+
+    def potts_get_option(self, key: str) -> int:
+        v = ctypes.c_int64()
+        _check(self._lib.potts_get_option(self._h, key.encode(), ctypes.byref(v)))
+        return int(v.value)

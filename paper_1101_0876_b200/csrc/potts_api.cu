@@ -1,0 +1,493 @@
+// potts_api.cu -- the C-ABI of include/potts.h: argument checking, device memory, launches.
+// Every step of the hot path runs in the kernels of potts_kernels.cuh; this file only marshals.
+#include "../../include/potts.h"
+#include "potts_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                          \
+    do {                                                                                        \
+        cudaError_t e_ = (expr);                                                                \
+        if (e_ != cudaSuccess)                                                                  \
+            return fail(e_ == cudaErrorMemoryAllocation ? POTTS_ERR_NOMEM : POTTS_ERR_CUDA,     \
+                        "%s failed: %s", #expr, cudaGetErrorString(e_));                        \
+    } while (0)
+
+constexpr size_t ALIGN = 256;
+constexpr size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+constexpr int ACC_WORDS = 1 + 256 + 1;   // E, hist[256], spare
+
+}  // namespace
+
+struct potts_s {
+    int32_t L = 0, q = 0, layout = 0;
+    uint64_t seed = 0, t = 0;
+    uint8_t *ws = nullptr;
+    bool owns_ws = false;
+    size_t plane_bytes = 0;
+    uint8_t *plane[2] = {nullptr, nullptr};
+    unsigned long long *acc = nullptr;   // device scratch: [0] = E, [1..q] = histogram
+    int *flag = nullptr;                 // device scratch flag (upload validation)
+    cudaStream_t stream = nullptr;
+    uint64_t launches = 0;
+    // options (how to launch, never what is computed)
+    int64_t opt_variant = 0;
+    int64_t opt_sweeps_per_launch = 1;
+    int64_t opt_use_graph = 0;
+};
+
+namespace {
+
+int check_shape(int32_t L, int32_t q, int32_t layout)
+{
+    if (L < 2 || (L & 1)) return fail(POTTS_ERR_ARG, "L = %d must be even and >= 2", L);
+    if (q < 2 || q > 256) return fail(POTTS_ERR_ARG, "q = %d outside [2, 256]", q);
+    if (layout != POTTS_LAYOUT_U8 && layout != POTTS_LAYOUT_PACKED)
+        return fail(POTTS_ERR_ARG, "unknown layout %d", layout);
+    if (L % 32 != 0)
+        return fail(POTTS_ERR_UNSUPPORTED, "L = %d is not a multiple of 32 (kernel vector width)", L);
+    if (layout == POTTS_LAYOUT_PACKED)
+        return fail(POTTS_ERR_UNSUPPORTED, "packed layout not built yet");
+    return POTTS_OK;
+}
+
+size_t plane_bytes_of(int32_t L, int32_t /*layout*/) { return align_up((size_t)L * (size_t)(L / 2)); }
+
+size_t workspace_bytes_of(int32_t L, int32_t layout)
+{
+    return 2 * plane_bytes_of(L, layout) + align_up(ACC_WORDS * sizeof(unsigned long long)) + ALIGN;
+}
+
+void thresholds(double T, uint32_t thr[4])
+{
+    // reading R6: exactly floor(ldexp(exp(-d/T), 32)) in double
+    for (int d = 1; d <= 4; ++d) thr[d - 1] = (uint32_t)std::floor(std::ldexp(std::exp(-(double)d / T), 32));
+}
+
+int check_launch(potts_t *h, const char *what)
+{
+    h->launches += 1;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(POTTS_ERR_CUDA, "launch of %s failed: %s", what, cudaGetErrorString(e));
+    return POTTS_OK;
+}
+
+potts::SweepParams sweep_params(const potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *E_out)
+{
+    potts::SweepParams P;
+    P.plane_own = h->plane[colour];
+    P.plane_oth = h->plane[1 - colour];
+    P.L = h->L;
+    P.pitch = h->L / 2;
+    P.q = (uint32_t)h->q;
+    P.colour = colour;
+    P.t = (uint32_t)h->t;
+    P.key0 = (uint32_t)(h->seed & 0xFFFFFFFFull);
+    P.key1 = (uint32_t)(h->seed >> 32);
+    for (int d = 0; d < 4; ++d) P.thr[d] = thr[d];
+    P.E_out = E_out;
+    return P;
+}
+
+int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *E_out)
+{
+    const potts::SweepParams P = sweep_params(h, colour, thr, E_out);
+    const long long threads = (long long)h->L * (h->L / 32);
+    const int block = 128;
+    const unsigned grid = (unsigned)((threads + block - 1) / block);
+    const bool wide = h->q > 128;
+    if (E_out) {
+        if (wide) potts::k_half_sweep_u8<true, true><<<grid, block, 0, h->stream>>>(P);
+        else potts::k_half_sweep_u8<false, true><<<grid, block, 0, h->stream>>>(P);
+    } else {
+        if (wide) potts::k_half_sweep_u8<true, false><<<grid, block, 0, h->stream>>>(P);
+        else potts::k_half_sweep_u8<false, false><<<grid, block, 0, h->stream>>>(P);
+    }
+    return check_launch(h, "k_half_sweep_u8");
+}
+
+int launch_measure(potts_t *h, unsigned long long *E_out, unsigned long long *hist_out)
+{
+    potts::MeasureParams M;
+    M.plane0 = h->plane[0];
+    M.plane1 = h->plane[1];
+    M.L = h->L;
+    M.pitch = h->L / 2;
+    M.q = (uint32_t)h->q;
+    M.E_out = E_out;
+    M.hist_out = hist_out;
+    const long long threads = (long long)h->L * (h->L / 32);
+    const int block = 256;
+    long long blocks = (threads + block - 1) / block;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    const size_t smem = hist_out ? (size_t)(block / 32) * h->q * sizeof(uint32_t) : 0;
+    if (h->q > 128) potts::k_measure_u8<true><<<(unsigned)blocks, block, smem, h->stream>>>(M);
+    else potts::k_measure_u8<false><<<(unsigned)blocks, block, smem, h->stream>>>(M);
+    return check_launch(h, "k_measure_u8");
+}
+
+int check_sweep_args(potts_t *h, double T, int64_t nsweeps)
+{
+    if (!h) return fail(POTTS_ERR_ARG, "null handle");
+    if (!(T > 0.0) || !std::isfinite(T)) return fail(POTTS_ERR_ARG, "T = %g must be finite and > 0", T);
+    if (nsweeps < 0) return fail(POTTS_ERR_ARG, "nsweeps = %lld < 0", (long long)nsweeps);
+    if (h->t + (uint64_t)nsweeps > 0xFFFFFFFFull)
+        return fail(POTTS_ERR_ARG, "sweep counter would pass 2^32 - 1 (Philox counter word)");
+    return POTTS_OK;
+}
+
+// the sweep loop shared by potts_sweep and potts_sweep_measured_dev
+int run_sweeps(potts_t *h, double T, int64_t nsweeps, int64_t every, unsigned long long *E_series_dev,
+               unsigned long long *hist_series_dev)
+{
+    uint32_t thr[4];
+    thresholds(T, thr);
+    for (int64_t n = 0; n < nsweeps; ++n) {
+        const bool sample = every > 0 && ((n + 1) % every == 0);
+        const int64_t idx = sample ? (n + 1) / every - 1 : 0;
+        int rc = launch_half_sweep(h, 0u, thr, nullptr);
+        if (rc) return rc;
+        rc = launch_half_sweep(h, 1u, thr, (sample && E_series_dev) ? E_series_dev + idx : nullptr);
+        if (rc) return rc;
+        h->t += 1;
+        if (sample && hist_series_dev) {
+            rc = launch_measure(h, nullptr, hist_series_dev + idx * h->q);
+            if (rc) return rc;
+        }
+    }
+    return POTTS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *potts_last_error(void) { return g_err.c_str(); }
+const char *potts_version(void) { return "potts-b200 0.1 (sm_100a)"; }
+
+int potts_workspace_bytes(int32_t L, int32_t q, int32_t layout, size_t *bytes)
+{
+    if (!bytes) return fail(POTTS_ERR_ARG, "null bytes pointer");
+    int rc = check_shape(L, q, layout);
+    if (rc) return rc;
+    *bytes = workspace_bytes_of(L, layout);
+    return POTTS_OK;
+}
+
+int potts_create_ex(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t init, int32_t layout,
+                    void *dev_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!out) return fail(POTTS_ERR_ARG, "null out pointer");
+    if (init != POTTS_INIT_ORDERED && init != POTTS_INIT_RANDOM) return fail(POTTS_ERR_ARG, "bad init %d", init);
+    int rc = check_shape(L, q, layout);
+    if (rc) return rc;
+    const size_t need = workspace_bytes_of(L, layout);
+    if (dev_workspace) {
+        if (workspace_bytes < need)
+            return fail(POTTS_ERR_NOMEM, "workspace of %zu bytes < %zu needed", workspace_bytes, need);
+        if ((uintptr_t)dev_workspace % ALIGN) return fail(POTTS_ERR_ARG, "workspace not %zu-byte aligned", ALIGN);
+    }
+    int ndev = 0;
+    CUDA_TRY(cudaGetDeviceCount(&ndev));
+    if (ndev < 1) return fail(POTTS_ERR_CUDA, "no CUDA device");
+    potts_t *h = new (std::nothrow) potts_s;
+    if (!h) return fail(POTTS_ERR_NOMEM, "host allocation failed");
+    h->L = L; h->q = q; h->layout = layout; h->seed = seed; h->t = 0;
+    h->stream = (cudaStream_t)cuda_stream;
+    if (dev_workspace) {
+        h->ws = (uint8_t *)dev_workspace;
+    } else {
+        cudaError_t e = cudaMalloc(&h->ws, need);
+        if (e != cudaSuccess) {
+            delete h;
+            return fail(e == cudaErrorMemoryAllocation ? POTTS_ERR_NOMEM : POTTS_ERR_CUDA,
+                        "cudaMalloc(%zu) failed: %s", need, cudaGetErrorString(e));
+        }
+        h->owns_ws = true;
+    }
+    h->plane_bytes = plane_bytes_of(L, layout);
+    h->plane[0] = h->ws;
+    h->plane[1] = h->ws + h->plane_bytes;
+    h->acc = (unsigned long long *)(h->ws + 2 * h->plane_bytes);
+    h->flag = (int *)(h->acc + ACC_WORDS - 1);
+
+    cudaError_t e = cudaSuccess;
+    if (init == POTTS_INIT_ORDERED) {
+        e = cudaMemsetAsync(h->ws, 0, 2 * h->plane_bytes, h->stream);
+    } else {
+        const long long words = 2ll * L * (L / 8);
+        const int block = 256;
+        potts::k_init_random_u8<<<(unsigned)((words + block - 1) / block), block, 0, h->stream>>>(
+            h->plane[0], h->plane[1], L, L / 2, (uint32_t)q, (uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32));
+        h->launches += 1;
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) {
+        potts_destroy(h);
+        return fail(POTTS_ERR_CUDA, "initialisation failed: %s", cudaGetErrorString(e));
+    }
+    *out = h;
+    return POTTS_OK;
+}
+
+int potts_create(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t init)
+{
+    return potts_create_ex(out, L, q, seed, init, POTTS_LAYOUT_U8, nullptr, 0, nullptr);
+}
+
+void potts_destroy(potts_t *h)
+{
+    if (!h) return;
+    if (h->owns_ws && h->ws) {
+        cudaStreamSynchronize(h->stream);
+        cudaFree(h->ws);
+    }
+    delete h;
+}
+
+int potts_set_stream(potts_t *h, void *cuda_stream)
+{
+    if (!h) return fail(POTTS_ERR_ARG, "null handle");
+    h->stream = (cudaStream_t)cuda_stream;
+    return POTTS_OK;
+}
+
+int potts_sweep(potts_t *h, double T, int64_t nsweeps)
+{
+    int rc = check_sweep_args(h, T, nsweeps);
+    if (rc) return rc;
+    return run_sweeps(h, T, nsweeps, 0, nullptr, nullptr);
+}
+
+int potts_sweep_measured_dev(potts_t *h, double T, int64_t nsweeps, int64_t every, int64_t *E_series_dev,
+                             int64_t *hist_series_dev)
+{
+    int rc = check_sweep_args(h, T, nsweeps);
+    if (rc) return rc;
+    if (every < 1 || nsweeps % every != 0)
+        return fail(POTTS_ERR_ARG, "every = %lld must be >= 1 and divide nsweeps = %lld", (long long)every,
+                    (long long)nsweeps);
+    const int64_t ns = nsweeps / every;
+    if (ns == 0) return POTTS_OK;
+    if (E_series_dev) CUDA_TRY(cudaMemsetAsync(E_series_dev, 0, (size_t)ns * 8, h->stream));
+    if (hist_series_dev) CUDA_TRY(cudaMemsetAsync(hist_series_dev, 0, (size_t)ns * h->q * 8, h->stream));
+    return run_sweeps(h, T, nsweeps, every, (unsigned long long *)E_series_dev,
+                      (unsigned long long *)hist_series_dev);
+}
+
+int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every, int64_t *E_series,
+                         int64_t *hist_series)
+{
+    int rc = check_sweep_args(h, T, nsweeps);
+    if (rc) return rc;
+    if (every < 1 || nsweeps % every != 0)
+        return fail(POTTS_ERR_ARG, "every = %lld must be >= 1 and divide nsweeps = %lld", (long long)every,
+                    (long long)nsweeps);
+    const int64_t ns = nsweeps / every;
+    if (ns == 0) return POTTS_OK;
+    const size_t eb = E_series ? (size_t)ns * 8 : 0, hb = hist_series ? (size_t)ns * h->q * 8 : 0;
+    uint8_t *dev = nullptr;
+    if (eb + hb) CUDA_TRY(cudaMalloc(&dev, eb + hb));
+    int64_t *dE = E_series ? (int64_t *)dev : nullptr;
+    int64_t *dH = hist_series ? (int64_t *)(dev + eb) : nullptr;
+    rc = potts_sweep_measured_dev(h, T, nsweeps, every, dE, dH);
+    cudaError_t e = cudaSuccess;
+    if (rc == POTTS_OK && eb) e = cudaMemcpyAsync(E_series, dE, eb, cudaMemcpyDeviceToHost, h->stream);
+    if (rc == POTTS_OK && e == cudaSuccess && hb)
+        e = cudaMemcpyAsync(hist_series, dH, hb, cudaMemcpyDeviceToHost, h->stream);
+    cudaError_t e2 = cudaStreamSynchronize(h->stream);
+    if (dev) cudaFree(dev);
+    if (rc) return rc;
+    if (e != cudaSuccess || e2 != cudaSuccess)
+        return fail(POTTS_ERR_CUDA, "series copy/sync failed: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
+    return POTTS_OK;
+}
+
+int potts_energy(potts_t *h, int64_t *E)
+{
+    if (!h || !E) return fail(POTTS_ERR_ARG, "null argument");
+    CUDA_TRY(cudaMemsetAsync(h->acc, 0, 8, h->stream));
+    int rc = launch_measure(h, h->acc, nullptr);
+    if (rc) return rc;
+    int64_t v = 0;
+    CUDA_TRY(cudaMemcpyAsync(&v, h->acc, 8, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    *E = v;
+    return POTTS_OK;
+}
+
+int potts_histogram(potts_t *h, int64_t *counts)
+{
+    if (!h || !counts) return fail(POTTS_ERR_ARG, "null argument");
+    CUDA_TRY(cudaMemsetAsync(h->acc + 1, 0, 8 * (size_t)h->q, h->stream));
+    int rc = launch_measure(h, nullptr, h->acc + 1);
+    if (rc) return rc;
+    int64_t tmp[256];
+    CUDA_TRY(cudaMemcpyAsync(tmp, h->acc + 1, 8 * (size_t)h->q, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    std::memcpy(counts, tmp, 8 * (size_t)h->q);
+    return POTTS_OK;
+}
+
+// rows per staging chunk: keeps the device staging buffer <= 64 MiB
+static int chunk_rows(int L) { long long r = (64ll << 20) / L; return (int)(r < 1 ? 1 : (r > L ? L : r)); }
+
+int potts_download(potts_t *h, uint8_t *spins)
+{
+    if (!h || !spins) return fail(POTTS_ERR_ARG, "null argument");
+    const int L = h->L, rows = chunk_rows(L);
+    uint8_t *stage = nullptr;
+    CUDA_TRY(cudaMalloc(&stage, (size_t)rows * L));
+    int rc = POTTS_OK;
+    for (int i0 = 0; i0 < L && rc == POTTS_OK; i0 += rows) {
+        const int r = (L - i0 < rows) ? L - i0 : rows;
+        const long long threads = (long long)r * (L / 8);
+        potts::k_planes_to_rowmajor<<<(unsigned)((threads + 255) / 256), 256, 0, h->stream>>>(
+            h->plane[0], h->plane[1], stage, L, L / 2, i0, r);
+        rc = check_launch(h, "k_planes_to_rowmajor");
+        if (rc == POTTS_OK) {
+            cudaError_t e = cudaMemcpyAsync(spins + (size_t)i0 * L, stage, (size_t)r * L, cudaMemcpyDeviceToHost, h->stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+            if (e != cudaSuccess) rc = fail(POTTS_ERR_CUDA, "download copy failed: %s", cudaGetErrorString(e));
+        }
+    }
+    cudaFree(stage);
+    return rc;
+}
+
+int potts_upload(potts_t *h, const uint8_t *spins)
+{
+    if (!h || !spins) return fail(POTTS_ERR_ARG, "null argument");
+    const int L = h->L, rows = chunk_rows(L);
+    // validate on the host first so that a rejected upload leaves the lattice untouched
+    if (h->q < 256)
+        for (size_t n = 0; n < (size_t)L * L; ++n)
+            if (spins[n] >= h->q) return fail(POTTS_ERR_ARG, "spin value %d >= q at offset %zu", (int)spins[n], n);
+    uint8_t *stage = nullptr;
+    CUDA_TRY(cudaMalloc(&stage, (size_t)rows * L));
+    int rc = POTTS_OK;
+    cudaMemsetAsync(h->flag, 0, sizeof(int), h->stream);
+    for (int i0 = 0; i0 < L && rc == POTTS_OK; i0 += rows) {
+        const int r = (L - i0 < rows) ? L - i0 : rows;
+        cudaError_t e = cudaMemcpyAsync(stage, spins + (size_t)i0 * L, (size_t)r * L, cudaMemcpyHostToDevice, h->stream);
+        if (e != cudaSuccess) { rc = fail(POTTS_ERR_CUDA, "upload copy failed: %s", cudaGetErrorString(e)); break; }
+        const long long threads = (long long)r * (L / 8);
+        potts::k_rowmajor_to_planes<<<(unsigned)((threads + 255) / 256), 256, 0, h->stream>>>(
+            stage, h->plane[0], h->plane[1], L, L / 2, i0, r, (uint32_t)h->q, h->flag);
+        rc = check_launch(h, "k_rowmajor_to_planes");
+        if (rc == POTTS_OK && cudaStreamSynchronize(h->stream) != cudaSuccess)
+            rc = fail(POTTS_ERR_CUDA, "upload sync failed");
+    }
+    cudaFree(stage);
+    return rc;
+}
+
+int potts_sweep_count(potts_t *h, uint64_t *t)
+{
+    if (!h || !t) return fail(POTTS_ERR_ARG, "null argument");
+    *t = h->t;
+    return POTTS_OK;
+}
+
+int potts_set_sweep_count(potts_t *h, uint64_t t)
+{
+    if (!h) return fail(POTTS_ERR_ARG, "null handle");
+    if (t > 0xFFFFFFFFull) return fail(POTTS_ERR_ARG, "t must be < 2^32");
+    h->t = t;
+    return POTTS_OK;
+}
+
+int potts_launch_count(potts_t *h, uint64_t *n)
+{
+    if (!h || !n) return fail(POTTS_ERR_ARG, "null argument");
+    *n = h->launches;
+    return POTTS_OK;
+}
+
+int potts_set_option(potts_t *h, const char *key, int64_t value)
+{
+    if (!h || !key) return fail(POTTS_ERR_ARG, "null argument");
+    if (!std::strcmp(key, "variant")) { h->opt_variant = value; return POTTS_OK; }
+    if (!std::strcmp(key, "sweeps_per_launch")) {
+        if (value < 1) return fail(POTTS_ERR_ARG, "sweeps_per_launch must be >= 1");
+        h->opt_sweeps_per_launch = value; return POTTS_OK;
+    }
+    if (!std::strcmp(key, "use_graph")) { h->opt_use_graph = value != 0; return POTTS_OK; }
+    return fail(POTTS_ERR_ARG, "unknown option '%s'", key);
+}
+
+int potts_get_option(potts_t *h, const char *key, int64_t *value)
+{
+    if (!h || !key || !value) return fail(POTTS_ERR_ARG, "null argument");
+    if (!std::strcmp(key, "variant")) { *value = h->opt_variant; return POTTS_OK; }
+    if (!std::strcmp(key, "sweeps_per_launch")) { *value = h->opt_sweeps_per_launch; return POTTS_OK; }
+    if (!std::strcmp(key, "use_graph")) { *value = h->opt_use_graph; return POTTS_OK; }
+    return fail(POTTS_ERR_ARG, "unknown option '%s'", key);
+}
+
+// ---- host-side derived observables (R10) -------------------------------------------------------
+int potts_observables(const int64_t *E_series, int64_t n, int64_t N, double T, double *mean_e, double *cv,
+                      double *binder)
+{
+    if (!E_series || n < 1 || N < 1 || !(T > 0.0) || !std::isfinite(T))
+        return fail(POTTS_ERR_ARG, "bad arguments to potts_observables");
+    typedef __int128 i128;
+    i128 s1 = 0, s2 = 0;
+    long double s4 = 0.0L, comp = 0.0L;            // Kahan-compensated sum of E^4
+    for (int64_t k = 0; k < n; ++k) {
+        const i128 e = (i128)E_series[k];
+        const i128 e2 = e * e;                      // < 2^63 for |E| <= 2^31.5: exact
+        s1 += e;
+        s2 += e2;
+        const long double e4 = (long double)e2 * (long double)e2;
+        const long double y = e4 - comp;
+        const long double tsum = s4 + y;
+        comp = (tsum - s4) - y;
+        s4 = tsum;
+    }
+    // <E^2> - <E>^2 = (n s2 - s1^2) / n^2, formed exactly in 128-bit integers
+    const i128 num = (i128)n * s2 - s1 * s1;
+    if (mean_e) *mean_e = (double)((long double)s1 / ((long double)n * (long double)N));
+    if (cv) *cv = (double)((long double)num / ((long double)n * (long double)n) / ((long double)N * (long double)T * (long double)T));
+    if (binder) {
+        if (s2 == 0) return fail(POTTS_ERR_ARG, "Binder cumulant undefined: all energies are zero");
+        *binder = (double)(1.0L - ((long double)n * s4) / (3.0L * (long double)s2 * (long double)s2));
+    }
+    return POTTS_OK;
+}
+
+int potts_magnetisation(const int64_t *counts, int32_t q, double *m)
+{
+    if (!counts || !m || q < 2 || q > 256) return fail(POTTS_ERR_ARG, "bad arguments to potts_magnetisation");
+    int64_t N = 0, mx = 0;
+    for (int k = 0; k < q; ++k) {
+        if (counts[k] < 0) return fail(POTTS_ERR_ARG, "negative count");
+        N += counts[k];
+        if (counts[k] > mx) mx = counts[k];
+    }
+    if (N == 0) return fail(POTTS_ERR_ARG, "empty histogram");
+    *m = (double)((((long double)q * (long double)mx) / (long double)N - 1.0L) / (long double)(q - 1));
+    return POTTS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,144 @@
+"""GPU parity: the CUDA path through the C-ABI against the CPU oracle, bit for bit (-m gpu).
+
+Same seeded inputs on both sides (workloads.py); spins, energy series and histograms must be
+identical after every sweep (north_star: "bit-exactly, with identical spin configurations,
+energy series and histograms after every sweep").  Integer work, so the bar is equality.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pb():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests selected but no CUDA device is visible")
+    import paper_1101_0876_b200 as pb
+    pb.load_library()
+    return pb
+
+
+def _pair(pb, L, q, seed, init, layout=0):
+    g = pb.Potts(L, q, seed, init, layout=layout)
+    o = oracle.OraclePotts(L, q, seed, init)
+    return g, o
+
+
+def test_cfg1_full_run_series_and_spins(pb):
+    """BASELINE configs[0] in full: q=9, L=64, random start, 0.99 T_c, 1000 sweeps, E+hist every sweep."""
+    w = workloads.CONFIGS[1]
+    g, o = _pair(pb, w.L, w.q, w.seed, w.init)
+    assert g.potts_energy() == o.energy()
+    assert (g.potts_histogram() == o.histogram()).all()
+    assert (g.potts_download() == o.spins()).all()
+    T = w.temperatures[0]
+    Eg, Hg = g.potts_sweep_measured(T, w.sweeps_per_t, w.every, hist=True)
+    Eo, Ho = o.sweep_measured(T, w.sweeps_per_t, w.every, hist=True)
+    assert (Eg == Eo).all()
+    assert (Hg == Ho).all()
+    assert (g.potts_download() == o.spins()).all()
+    assert g.potts_sweep_count() == o.t == 1000
+    # derived observables, host double, 1e-12 relative (north_star)
+    from oracle import observables as obs
+    me, cv, bl = pb.potts_observables(Eg, w.L * w.L, T)
+    for got, want in ((me, obs.mean_energy_per_spin(Eo, w.L * w.L)), (cv, obs.specific_heat(Eo, w.L * w.L, T)),
+                      (bl, obs.binder_cumulant(Eo))):
+        assert abs(got - want) <= 1e-12 * abs(want)
+    assert abs(pb.potts_magnetisation(Hg[-1], w.q) - obs.magnetisation(Ho[-1], w.q)) <= 1e-12
+
+
+@pytest.mark.parametrize("L,q,init,f,seed", [
+    (32, 2, workloads.INIT_RANDOM, 1.0, 11),        # smallest supported L, Ising limit
+    (64, 6, workloads.INIT_ORDERED, 1.005, 7),      # cfg2's parameters at small L
+    (96, 24, workloads.INIT_ORDERED, 1.002, 4),     # L not a power of two, several blocks + ragged tail
+    (160, 9, workloads.INIT_RANDOM, 0.98, 3),
+    (224, 128, workloads.INIT_RANDOM, 1.0, 5),      # largest q on the 7-bit compare path
+    (64, 129, workloads.INIT_RANDOM, 1.0, 6),       # first q on the 8-bit compare path
+    (96, 256, workloads.INIT_RANDOM, 1.1, 8),       # maximum q
+    (64, 3, workloads.INIT_RANDOM, 50.0, 9),        # hot: nearly every proposal accepted
+    (64, 5, workloads.INIT_RANDOM, 0.05, 10),       # cold: thresholds ~ 0
+    (512, 9, workloads.INIT_RANDOM, 0.995, 5),      # many blocks
+])
+def test_every_sweep_spins_energy_histogram(pb, L, q, init, f, seed):
+    g, o = _pair(pb, L, q, seed, init)
+    T = f * workloads.t_c(q)
+    assert (g.potts_download() == o.spins()).all()
+    for _ in range(6):
+        g.potts_sweep(T, 1)
+        o.sweep(T, 1)
+        assert (g.potts_download() == o.spins()).all()
+        assert g.potts_energy() == o.energy()
+        assert (g.potts_histogram() == o.histogram()).all()
+    Eg, Hg = g.potts_sweep_measured(T, 24, 3, hist=True)
+    Eo, Ho = o.sweep_measured(T, 24, 3, hist=True)
+    assert (Eg == Eo).all() and (Hg == Ho).all()
+    assert (g.potts_download() == o.spins()).all()
+
+
+def test_sweep_split_equals_single_call_and_seed_high_bits(pb):
+    L, q, seed = 128, 9, (0xDEADBEEF << 32) | 12345       # key1 != 0
+    T = 0.99 * workloads.t_c(q)
+    a, o = _pair(pb, L, q, seed, workloads.INIT_RANDOM)
+    b = pb.Potts(L, q, seed, workloads.INIT_RANDOM)
+    a.potts_sweep(T, 20)
+    b.potts_sweep(T, 7)
+    b.potts_sweep(T, 13)
+    o.sweep(T, 20)
+    sa = a.potts_download()
+    assert (sa == b.potts_download()).all() and (sa == o.spins()).all()
+
+
+@pytest.mark.parametrize("kind", ["domains", "stripes", "uniform"])
+def test_upload_restart_matches_oracle(pb, kind):
+    L, q = 96, 7
+    s0 = workloads.synthetic_spins(L, q, 123, kind)
+    g = pb.Potts(L, q, 99, workloads.INIT_ORDERED)
+    o = oracle.OraclePotts(L, q, 99, workloads.INIT_ORDERED)
+    g.potts_upload(s0)
+    g.potts_set_sweep_count(1000)
+    o.set_state(s0, 1000)
+    assert (g.potts_download() == s0).all()
+    assert g.potts_energy() == o.energy()
+    T = 1.0 * workloads.t_c(q)
+    Eg, Hg = g.potts_sweep_measured(T, 10, 1, hist=True)
+    Eo, Ho = o.sweep_measured(T, 10, 1, hist=True)
+    assert (Eg == Eo).all() and (Hg == Ho).all() and (g.potts_download() == o.spins()).all()
+
+
+def test_degenerate_temperatures(pb):
+    L, q = 64, 6
+    g = pb.Potts(L, q, 1, workloads.INIT_ORDERED)
+    E, H = g.potts_sweep_measured(0.01, 20, 1, hist=True)
+    assert (E == -2 * L * L).all() and (H[:, 0] == L * L).all()
+    g, o = _pair(pb, L, q, 2, workloads.INIT_RANDOM)
+    Eg, _ = g.potts_sweep_measured(1e12, 10, 1, hist=False)
+    Eo, _ = o.sweep_measured(1e12, 10, 1, hist=False)
+    assert (Eg == Eo).all()
+
+
+def test_errors_on_device(pb):
+    g = pb.Potts(64, 4, 1)
+    with pytest.raises(pb.PottsError) as e:
+        g.potts_sweep(-1.0, 1)
+    assert e.value.code == pb.ERR_ARG
+    with pytest.raises(pb.PottsError):
+        g.potts_sweep(float("nan"), 1)
+    with pytest.raises(pb.PottsError):
+        g.potts_sweep_measured(1.0, 10, 3)            # every does not divide nsweeps
+    bad = np.zeros((64, 64), dtype=np.uint8)
+    bad[5, 7] = 4                                      # >= q
+    before = g.potts_download()
+    with pytest.raises(pb.PottsError):
+        g.potts_upload(bad)
+    assert (g.potts_download() == before).all()        # rejected upload leaves the lattice untouched
+    g.potts_set_sweep_count(2 ** 32 - 2)
+    g.potts_sweep(1.0, 1)
+    with pytest.raises(pb.PottsError):
+        g.potts_sweep(1.0, 1)                          # counter would pass 2^32 - 1
+    E, _ = g.potts_sweep_measured(1.0, 0, 1)           # empty run is fine
+    assert E.size == 0
