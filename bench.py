@@ -1,0 +1,425 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the checkerboard Potts sweep on B200 (driver contract).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload cfgN] [--no-per-config] [--no-cpu-baseline]
+
+A "step" is one pass of the whole hot path over one workload of BASELINE.json: create the
+start state, then `sweeps` checkerboard Metropolis sweeps at the workload's temperature(s) with
+the workload's measurement cadence (energy / histogram series recorded on the device).  The
+default workload is BASELINE.json configs[1] (q=6, L=1024, ordered start, 1.005 T_c, 10^4
+sweeps, energy every sweep).  `value` = spin-flip attempts per second (= 1e9 / ns-per-flip),
+inputs resident in HBM; `e2e` = the same through the C-ABI with HOST buffers (upload of the
+start configuration from pinned host memory, series + final configuration copied back).
+
+N > 1 (torchrun): the paper averages over independent samples ("repeat over
+samples"), so rank r runs sample r (seed + r) of the same workload: no data-path collective,
+weak scaling; the time is the max over ranks.
+
+Rank 0 prints ONE JSON line.  See DESIGN.md section 8 for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads  # noqa: E402
+
+# ---- roofline constants -------------------------------------------------
+SM_COUNT = 148
+ISSUE_LANES_PER_SM_CLK = 128          # 4 SMSPs x 1 warp-instruction (32 lanes) per clock
+I_ALG_PER_UPDATE = 39                 # Philox4x32-10 (w0,w1): 17 IMAD.WIDE + 2 IMAD.HI + 19 LOP3, + 1 IMAD.HI proposal
+BYTES_ALG_PER_UPDATE_U8 = 3.0         # read own + read other (once) + write own, uint8 planes
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the
+# `ncu --set full` capture summarised in profiles/ (None until a capture exists for the workload)
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+# ---- clocks during the timed region -----------------------------------------------------------
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML every 20 ms while running."""
+
+    REASONS = {
+        0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+        0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+        0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting",
+    }
+
+    def __init__(self, index: int):
+        self.index, self.samples, self.mask, self.max_mhz = index, [], 0, None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._dev = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._dev, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _run(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._dev, nv.NVML_CLOCK_SM)))
+                self.mask |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._dev))
+            except Exception:
+                pass
+            self._stop.wait(0.02)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        reasons = [n for b, n in self.REASONS.items() if self.mask & b and n != "gpu_idle"]
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "samples": len(self.samples), "reasons": reasons}
+
+
+# ---- one workload on one GPU ------------------------------------------------------------------
+def slice_of(w: workloads.Workload, max_sweeps: int | None):
+    """(temperatures, sweeps per temperature) of the whole workload or of a bounded slice of it."""
+    if max_sweeps is None or max_sweeps >= w.total_sweeps:
+        return list(w.temperatures), w.sweeps_per_t
+    per_t = max(w.every, (max_sweeps // len(w.temperatures)) // w.every * w.every)
+    return list(w.temperatures), per_t
+
+
+class GpuRun:
+    """Drives the product through the Python binding of the C-ABI (argument marshalling only)."""
+
+    def __init__(self, pb, torch, w: workloads.Workload, seed: int, max_sweeps: int | None, options=None):
+        self.pb, self.torch, self.w, self.seed = pb, torch, w, seed
+        self.temps, self.per_t = slice_of(w, max_sweeps)
+        self.sweeps = self.per_t * len(self.temps)
+        self.updates = self.sweeps * w.L * w.L
+        self.ns = self.sweeps // w.every
+        self.layout = pb.LAYOUT_PACKED if w.packed and getattr(pb, "PACKED_AVAILABLE", False) else pb.LAYOUT_U8
+        self.options = dict(options or {})
+        dev = torch.device("cuda", torch.cuda.current_device())
+        self.E_dev = torch.zeros(max(self.ns, 1), dtype=torch.int64, device=dev)
+        self.H_dev = torch.zeros((max(self.ns, 1), w.q), dtype=torch.int64, device=dev) if w.hist else None
+        self.g = None
+
+    def fresh(self):
+        """New handle in the workload's start state, t = 0 (untimed)."""
+        if self.g is not None:
+            self.g.close()
+        self.g = self.pb.Potts(self.w.L, self.w.q, self.seed, self.w.init, layout=self.layout)
+        for k, v in self.options.items():
+            self.g.potts_set_option(k, v)
+        return self.g
+
+    def enqueue(self):
+        """The step: all sweeps with the device-resident series; returns without a sync."""
+        per_s = self.per_t // self.w.every
+        for n, T in enumerate(self.temps):
+            E = self.E_dev[n * per_s:(n + 1) * per_s]
+            H = self.H_dev[n * per_s:(n + 1) * per_s] if self.H_dev is not None else None
+            self.g.potts_sweep_measured_dev(T, self.per_t, self.w.every, E, H)
+
+    # -- end to end through host buffers ----------------------------------------------------
+    def e2e_prepare(self):
+        torch, w = self.torch, self.w
+        g = self.fresh()
+        self.h_start = torch.empty((w.L, w.L), dtype=torch.uint8, pin_memory=True)
+        g.potts_download(self.h_start.numpy())
+        self.h_final = torch.empty((w.L, w.L), dtype=torch.uint8, pin_memory=True)
+        self.h2d = w.L * w.L
+        self.d2h = w.L * w.L + self.ns * 8 * (1 + (w.q if w.hist else 0))
+
+    def e2e_step(self):
+        g, w = self.g, self.w
+        g.potts_upload(self.h_start.numpy())
+        g.potts_set_sweep_count(0)
+        last = None
+        for T in self.temps:
+            last = g.potts_sweep_measured(T, self.per_t, w.every, hist=w.hist)
+        g.potts_download(self.h_final.numpy())
+        return last
+
+
+def time_steps(torch, run: GpuRun, steps: int, warmup: int, flush, e2e: bool = False):
+    """-> (list of per-step ms, kernels launched in the timed steps)."""
+    if e2e:
+        run.e2e_prepare()
+    ms, launches = [], 0
+    for it in range(warmup + steps):
+        if not e2e:
+            run.fresh()
+        flush()
+        torch.cuda.synchronize()
+        n0 = run.g.potts_launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        if e2e:
+            run.e2e_step()
+        else:
+            run.enqueue()
+        e1.record()
+        torch.cuda.synchronize()
+        if it >= warmup:
+            ms.append(e0.elapsed_time(e1))
+            launches += run.g.potts_launch_count() - n0
+    return ms, launches
+
+
+def make_flusher(torch):
+    buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # 2x the 126 MB L2
+
+    def flush():
+        buf.fill_(1)
+    return flush
+
+
+# ---- the oracle timed on the host cores (cpu_baseline and --impl reference) --------------------
+def host_threads() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def oracle_time(w: workloads.Workload, sweeps: int, threads: int):
+    """Seconds the oracle, as it stands, needs for `sweeps` sweeps of workload w (with its cadence)."""
+    import oracle
+    o = oracle.OraclePotts(w.L, w.q, w.seed, w.init, threads=threads)
+    sweeps = max(w.every, sweeps // w.every * w.every)
+    t0 = time.perf_counter()
+    o.sweep_measured(w.temperatures[0], sweeps, w.every, hist=w.hist)
+    dt = time.perf_counter() - t0
+    used = o.threads
+    o.close()
+    return dt, sweeps, used
+
+
+def cpu_baseline(w: workloads.Workload, budget_s: float = 12.0):
+    """The oracle on a bounded sample of the workload: all host threads (row-parallel mode, same
+    bits) and one thread.  Returns the cpu_baseline object of the JSON line."""
+    threads = host_threads()
+    dt, n, _ = oracle_time(w, w.every, threads)                      # calibration (and page-in)
+    per_sweep = max(dt / n, 1e-6)
+    sweeps = int(min(w.total_sweeps, max(w.every, budget_s / per_sweep)))
+    dt, n, used = oracle_time(w, sweeps, threads)
+    multi = n * w.L * w.L / dt
+    n1 = max(w.every, int(n / max(threads, 1) / 2))
+    dt1, n1, _ = oracle_time(w, n1, 1)
+    single = n1 * w.L * w.L / dt1
+    return {"value": multi, "unit": "spin updates/s", "cores": used, "kind": "oracle",
+            "sample": f"{n} sweeps of {w.name} (L={w.L}, q={w.q}) with its measurement cadence, {dt:.1f} s",
+            "ns_per_spin_flip": 1e9 / multi,
+            "single_thread": {"value": single, "ns_per_spin_flip": 1e9 / single,
+                              "sample": f"{n1} sweeps, {dt1:.1f} s"}}
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle on the host cores, same metric / config; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    threads = host_threads()
+    dt, n, _ = oracle_time(w, w.every, threads)
+    per_sweep = max(dt / n, 1e-6)
+    total = args.steps + args.warmup
+    sweeps = int(min(w.total_sweeps, max(w.every, (90.0 / total) / per_sweep)))   # whole run ~1.5 min
+    times = []
+    for it in range(total):
+        dt, n, used = oracle_time(w, sweeps, threads)
+        if it >= args.warmup:
+            times.append(dt)
+    sec = sum(times) / len(times)
+    val = n * w.L * w.L / sec
+    sample = f"each step = {n} sweeps of {w.name} by the oracle (OpenMP rows, {used} threads)"
+    line = {
+        "impl": "reference", "metric": "spin_updates_per_s", "value": val, "unit": "spin updates/s",
+        "ns_per_spin_flip": 1e9 / val, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u8", "data": "synthetic", "gpu_launches": 0,
+        "config": {"workload": w.name, "q": w.q, "L": w.L, "init": "random" if w.init else "ordered",
+                   "T_over_Tc": w.t_factors[0], "sweeps_per_step": n, "measure_every": w.every, "hist": w.hist},
+        "cpu_baseline": {"value": val, "unit": "spin updates/s", "cores": used, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "spin updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---- roofline -----------------------------------------------------------------------------------
+def roofline(w, updates_per_launch: float, ms_per_launch: float, sm_mhz_max: float, hbm_gbs: float, which: str,
+             bytes_per_update: float):
+    """ALU/issue roofline of the half-sweep kernel: algorithmic thread-instructions
+    (39 per update: the Philox block and the proposal the stream definition fixes) over the average
+    launch duration, against 148 SMs x 128 lanes x max SM clock; the HBM view is reported beside it."""
+    sec = ms_per_launch * 1e-3
+    ach = I_ALG_PER_UPDATE * updates_per_launch / sec / 1e12
+    peak = SM_COUNT * ISSUE_LANES_PER_SM_CLK * sm_mhz_max * 1e6 / 1e12
+    gbs = bytes_per_update * updates_per_launch / sec / 1e9
+    return {"bound": "alu", "kernel": "k_half_sweep", "achieved": ach, "peak": peak, "unit": "Tinstr/s (thread-level)",
+            "frac": ach / peak, "peak_source": f"148 SMs x 128 lanes/clk x {sm_mhz_max:.0f} MHz ({which} max SM clock)",
+            "instr_per_update_algorithmic": I_ALG_PER_UPDATE,
+            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(w.name),
+            "hbm": {"achieved": gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": gbs / hbm_gbs,
+                    "bytes_per_update_algorithmic": bytes_per_update, "peak_source": f"{which} copy bandwidth"}}
+
+
+PER_CONFIG_SLICE = {1: None, 2: 2000, 3: 1600, 4: 200, 5: 100}       # sweeps timed per step (None = all)
+
+
+def per_config_table(pb, torch, flush, sm_max, hbm_gbs, which, skip=()):
+    out = {}
+    for k, w in workloads.CONFIGS.items():
+        if k in skip:
+            continue
+        run = GpuRun(pb, torch, w, w.seed, PER_CONFIG_SLICE[k])
+        ms, launches = time_steps(torch, run, steps=3, warmup=1, flush=flush)
+        sec = statistics.median(ms) * 1e-3
+        ups = run.updates / sec
+        half_sweeps = 2 * run.sweeps
+        r = roofline(w, w.L * w.L / 2, sec * 1e3 / half_sweeps, sm_max, hbm_gbs, which,
+                     bytes_per_update=run.g.bytes_per_update() if hasattr(run.g, "bytes_per_update") else BYTES_ALG_PER_UPDATE_U8)
+        out[w.name] = {"q": w.q, "L": w.L, "sweeps_timed": run.sweeps, "of_sweeps": w.total_sweeps,
+                       "ns_per_spin_flip": 1e9 / ups, "spin_updates_per_s": ups, "ms": sec * 1e3,
+                       "launches": launches // 3, "alu_frac": r["frac"], "hbm_frac": r["hbm"]["frac"],
+                       "layout": "packed" if run.layout == pb.LAYOUT_PACKED else "u8"}
+        run.g.close()
+        del run
+        torch.cuda.empty_cache()
+    return out
+
+
+# ---- main -----------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2", help="cfg1..cfg5 (BASELINE.json configs[0..4])")
+    ap.add_argument("--max-sweeps", type=int, default=None, help="time a bounded slice of the workload per step")
+    ap.add_argument("--no-per-config", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--option", action="append", default=[], help="key=value passed to potts_set_option")
+    args = ap.parse_args()
+    w = workloads.CONFIGS[int(args.workload.replace("cfg", ""))]
+
+    if args.impl == "reference":
+        run_reference(args, w)
+        return
+
+    import torch
+    import paper_1101_0876_b200 as pb
+    pb.load_library()                                    # raises if the CUDA library is not built: no fallback
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    hbm_gbs, sm_max, which = _peaks()
+    flush = make_flusher(torch)
+    options = {kv.split("=")[0]: int(kv.split("=")[1]) for kv in args.option}
+
+    # rank r runs sample r of the workload (independent lattice, seed + r): weak scaling, no collective
+    run = GpuRun(pb, torch, w, w.seed + rank, args.max_sweeps, options)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    barrier()
+    t_wall0 = time.perf_counter()
+    with ClockSampler(local) as clk:
+        ms, launches = time_steps(torch, run, args.steps, args.warmup, flush)
+    barrier()
+    wall = time.perf_counter() - t_wall0
+    total_ms = torch.tensor([sum(ms)], dtype=torch.float64, device="cuda")
+    counts = torch.tensor([run.updates * args.steps, launches], dtype=torch.int64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+        dist.all_reduce(counts, op=dist.ReduceOp.SUM)
+    total_s = float(total_ms.item()) * 1e-3
+    updates_all, launches_all = int(counts[0].item()), int(counts[1].item())
+    value = updates_all / total_s
+    bpu = BYTES_ALG_PER_UPDATE_U8 if run.layout == pb.LAYOUT_U8 else run.g.bytes_per_update()
+    half_sweeps = 2 * run.sweeps
+    roof = roofline(w, w.L * w.L / 2, (sum(ms) / len(ms)) / half_sweeps, sm_max, hbm_gbs, which, bpu)
+
+    e2e = None
+    if not args.no_e2e:
+        barrier()
+        ms_e, _ = time_steps(torch, run, args.steps, max(1, args.warmup), flush, e2e=True)
+        tot_e = torch.tensor([sum(ms_e)], dtype=torch.float64, device="cuda")
+        if dist is not None:
+            dist.all_reduce(tot_e, op=dist.ReduceOp.MAX)
+        e2e = {"value": run.updates * args.steps * world / (float(tot_e.item()) * 1e-3), "unit": "spin updates/s",
+               "h2d_bytes_per_step": run.h2d, "d2h_bytes_per_step": run.d2h, "ms_per_step": float(tot_e.item()) / args.steps,
+               "path": "potts_upload (pinned host) + potts_sweep_measured (host series) + potts_download (pinned host)"}
+    layout = "packed" if run.layout == pb.LAYOUT_PACKED else "u8"
+    run.g.close()
+
+    per_cfg, cpu = None, None
+    if rank == 0 and world == 1 and not args.no_per_config:
+        per_cfg = per_config_table(pb, torch, flush, sm_max, hbm_gbs, which)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(w)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+    line = {
+        "metric": "spin_updates_per_s", "value": value, "unit": "spin updates/s", "ns_per_spin_flip": 1e9 / value * world,
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_s * 1e3 / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+        "gpu_launches": launches_all,
+        "config": {"workload": w.name, "q": w.q, "L": w.L, "init": "random" if w.init else "ordered",
+                   "T_over_Tc": w.t_factors if len(w.t_factors) > 1 else w.t_factors[0],
+                   "sweeps_per_step": run.sweeps, "of_sweeps": w.total_sweeps, "measure_every": w.every,
+                   "hist": w.hist, "layout": layout, "seed": w.seed, "options": options,
+                   "parallelism": f"{world} independent sample(s), one per GPU" if world > 1 else "1 GPU",
+                   "l2": "each step starts from a fresh lattice after a 256 MiB L2 flush; within a step the "
+                         "lattice is re-swept in place, so L2 residency for L <= 8192 is the workload's own"},
+        "clocks": clk.summary(), "roofline": roof, "e2e": e2e, "cpu_baseline": cpu, "per_config": per_cfg,
+        "wall_s_timed_region": wall,
+        "paper_context": {"ns_per_spin_flip_gtx480": 0.147, "note": "other hardware and RNG; context, not a target"},
+    }
+    print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    main()
