@@ -2,6 +2,7 @@
 // Every step of the hot path runs in the kernels of potts_kernels.cuh; this file only marshals.
 #include "../../include/potts.h"
 #include "potts_kernels.cuh"
+#include "potts_resident.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -35,7 +36,8 @@ int fail(int code, const char *fmt, ...)
 
 constexpr size_t ALIGN = 256;
 constexpr size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
-constexpr int ACC_WORDS = 1 + 256 + 1;   // E, hist[256], spare
+constexpr int MAX_CTAS = 512;             // upper bound on the resident kernel's grid (SM count)
+constexpr int ACC_WORDS = 1 + 256 + 1 + MAX_CTAS;   // E, hist[256], flag/error word, resident flags
 
 }  // namespace
 
@@ -48,12 +50,15 @@ struct potts_s {
     uint8_t *plane[2] = {nullptr, nullptr};
     unsigned long long *acc = nullptr;   // device scratch: [0] = E, [1..q] = histogram
     int *flag = nullptr;                 // device scratch flag (upload validation)
+    int *error = nullptr;                // device: set by the resident kernel if a neighbour wait gave up
+    unsigned long long *cta_flags = nullptr;   // device: resident kernel's per-CTA progress counters
     cudaStream_t stream = nullptr;
     uint64_t launches = 0;
+    int num_sms = 0;
+    size_t smem_optin = 0;
     // options (how to launch, never what is computed)
-    int64_t opt_variant = 0;
-    int64_t opt_sweeps_per_launch = 1;
-    int64_t opt_use_graph = 0;
+    int64_t opt_variant = 0;             // 0 auto, 1 streaming (one launch per half-sweep), 2 resident
+    int64_t opt_resident_ctas = 0;       // 0 auto, else the resident kernel's grid size
 };
 
 namespace {
@@ -101,27 +106,36 @@ potts::SweepParams sweep_params(const potts_t *h, uint32_t colour, const uint32_
     P.pitch = h->L / 2;
     P.q = (uint32_t)h->q;
     P.colour = colour;
-    P.t = (uint32_t)h->t;
-    P.key0 = (uint32_t)(h->seed & 0xFFFFFFFFull);
-    P.key1 = (uint32_t)(h->seed >> 32);
+    P.K = potts::half_sweep_keys((uint32_t)(h->seed & 0xFFFFFFFFull), (uint32_t)(h->seed >> 32), (uint32_t)h->t, colour);
     for (int d = 0; d < 4; ++d) P.thr[d] = thr[d];
     P.E_out = E_out;
     return P;
 }
 
-int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *E_out)
+template <bool WIDE, bool MEASURE, bool HIST>
+void launch_hs(const potts::SweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
 {
-    const potts::SweepParams P = sweep_params(h, colour, thr, E_out);
-    const long long threads = (long long)h->L * (h->L / 32);
-    const int block = 128;
-    const unsigned grid = (unsigned)((threads + block - 1) / block);
-    const bool wide = h->q > 128;
-    if (E_out) {
-        if (wide) potts::k_half_sweep_u8<true, true><<<grid, block, 0, h->stream>>>(P);
-        else potts::k_half_sweep_u8<false, true><<<grid, block, 0, h->stream>>>(P);
-    } else {
-        if (wide) potts::k_half_sweep_u8<true, false><<<grid, block, 0, h->stream>>>(P);
-        else potts::k_half_sweep_u8<false, false><<<grid, block, 0, h->stream>>>(P);
+    potts::k_half_sweep_u8<WIDE, MEASURE, HIST><<<grid, dim3(32, potts::HS_ROWS), smem, st>>>(P);
+}
+
+int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *E_out,
+                      unsigned long long *hist_out)
+{
+    potts::SweepParams P = sweep_params(h, colour, thr, E_out);
+    P.hist_out = hist_out;
+    const int chunks = h->L / 32;
+    const dim3 grid((unsigned)((chunks + 31) / 32), (unsigned)(h->L / potts::HS_ROWS));
+    const size_t smem = hist_out ? (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4 : 0;
+    const int sel = (h->q > 128 ? 4 : 0) | (E_out ? 2 : 0) | (hist_out ? 1 : 0);
+    switch (sel) {
+    case 0: launch_hs<false, false, false>(P, grid, smem, h->stream); break;
+    case 1: launch_hs<false, false, true>(P, grid, smem, h->stream); break;
+    case 2: launch_hs<false, true, false>(P, grid, smem, h->stream); break;
+    case 3: launch_hs<false, true, true>(P, grid, smem, h->stream); break;
+    case 4: launch_hs<true, false, false>(P, grid, smem, h->stream); break;
+    case 5: launch_hs<true, false, true>(P, grid, smem, h->stream); break;
+    case 6: launch_hs<true, true, false>(P, grid, smem, h->stream); break;
+    default: launch_hs<true, true, true>(P, grid, smem, h->stream); break;
     }
     return check_launch(h, "k_half_sweep_u8");
 }
@@ -140,7 +154,7 @@ int launch_measure(potts_t *h, unsigned long long *E_out, unsigned long long *hi
     const int block = 256;
     long long blocks = (threads + block - 1) / block;
     if (blocks > 148 * 8) blocks = 148 * 8;
-    const size_t smem = hist_out ? (size_t)(block / 32) * h->q * sizeof(uint32_t) : 0;
+    const size_t smem = hist_out ? (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4 : 0;
     if (h->q > 128) potts::k_measure_u8<true><<<(unsigned)blocks, block, smem, h->stream>>>(M);
     else potts::k_measure_u8<false><<<(unsigned)blocks, block, smem, h->stream>>>(M);
     return check_launch(h, "k_measure_u8");
@@ -156,25 +170,126 @@ int check_sweep_args(potts_t *h, double T, int64_t nsweeps)
     return POTTS_OK;
 }
 
+// ---- resident (persistent, shared-memory) path ------------------------------------------------
+struct ResidentPlan {
+    bool ok = false;
+    int G = 0, ty = 0, wpr = 0, rows_max = 0;
+    size_t smem = 0;
+    const char *why = "";
+};
+
+int gcd_int(int a, int b) { return b ? gcd_int(b, a % b) : a; }
+
+ResidentPlan plan_resident(const potts_t *h)
+{
+    ResidentPlan R;
+    const int L = h->L;
+    R.wpr = L / 8;
+    if (R.wpr > 1024) { R.why = "L/8 words per row exceed 1024 threads"; return R; }
+    const long long words = (long long)L * R.wpr;                   // 4-site words per half-sweep
+    long long G = h->opt_resident_ctas > 0 ? h->opt_resident_ctas : words / 512;
+    if (G < 1) G = 1;
+    if (G > h->num_sms) G = h->num_sms;
+    if (G > L) G = L;
+    if (G > MAX_CTAS) G = MAX_CTAS;
+    R.G = (int)G;
+    R.rows_max = (L + R.G - 1) / R.G;
+    // block = (wpr, ty) threads, a multiple of 32 in total
+    const int mult = 32 / gcd_int(R.wpr, 32);
+    int ty = R.rows_max < 1024 / R.wpr ? R.rows_max : 1024 / R.wpr;
+    ty = (ty + mult - 1) / mult * mult;
+    if (R.wpr * ty > 1024) ty = (1024 / R.wpr) / mult * mult;
+    if (ty < 1) { R.why = "no block shape with a multiple of 32 threads"; return R; }
+    R.ty = ty;
+    if ((R.rows_max + ty - 1) / ty > 60) { R.why = "too many rows per thread"; return R; }
+    const size_t hist = (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4;
+    R.smem = 2 * (size_t)(R.rows_max + 2) * (L / 2) + hist;
+    if (R.smem + 1024 > h->smem_optin) { R.why = "lattice does not fit the shared memory of the grid"; return R; }
+    R.ok = true;
+    return R;
+}
+
+int launch_resident(potts_t *h, const ResidentPlan &R, const uint32_t thr[4], int64_t nsweeps, int64_t every,
+                    unsigned long long *E_series_dev, unsigned long long *hist_series_dev)
+{
+    potts::ResidentParams P;
+    P.plane[0] = h->plane[0];
+    P.plane[1] = h->plane[1];
+    P.L = h->L;
+    P.pitch = h->L / 2;
+    P.q = (uint32_t)h->q;
+    P.key0 = (uint32_t)(h->seed & 0xFFFFFFFFull);
+    P.key1 = (uint32_t)(h->seed >> 32);
+    for (int d = 0; d < 4; ++d) P.thr[d] = thr[d];
+    P.t0 = (uint32_t)h->t;
+    P.nsweeps = (uint32_t)nsweeps;
+    P.every = (uint32_t)every;
+    P.E_series = E_series_dev;
+    P.hist_series = hist_series_dev;
+    P.flags = h->cta_flags;
+    P.error = h->error;
+    P.rows_max = R.rows_max;
+    const void *fn = h->q > 128 ? (const void *)potts::k_resident_u8<true> : (const void *)potts::k_resident_u8<false>;
+    CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
+    int per_sm = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, R.wpr * R.ty, R.smem));
+    if (per_sm < 1 || (long long)per_sm * h->num_sms < R.G)
+        return fail(POTTS_ERR_UNSUPPORTED, "resident kernel: %d CTAs cannot be co-resident", R.G);
+    // the progress counters are absolute half-sweep indices; a restored sweep counter may be lower
+    CUDA_TRY(cudaMemsetAsync(h->cta_flags, 0, sizeof(unsigned long long) * MAX_CTAS, h->stream));
+    void *args[] = {(void *)&P};
+    CUDA_TRY(cudaLaunchCooperativeKernel(fn, dim3((unsigned)R.G), dim3((unsigned)R.wpr, (unsigned)R.ty), args, R.smem,
+                                         h->stream));
+    h->launches += 1;
+    return POTTS_OK;
+}
+
 // the sweep loop shared by potts_sweep and potts_sweep_measured_dev
 int run_sweeps(potts_t *h, double T, int64_t nsweeps, int64_t every, unsigned long long *E_series_dev,
                unsigned long long *hist_series_dev)
 {
     uint32_t thr[4];
     thresholds(T, thr);
+    if (nsweeps == 0) return POTTS_OK;
+    if (h->opt_variant != 1) {
+        const ResidentPlan R = plan_resident(h);
+        if (R.ok) {
+            // the kernel's sweep and sample counters are 32-bit: split very long calls
+            const int64_t piece = every > 0 ? (int64_t)((1ll << 30) / every) * every : (1ll << 30);
+            for (int64_t done = 0; done < nsweeps;) {
+                const int64_t n = nsweeps - done < piece ? nsweeps - done : piece;
+                const int64_t s0 = every > 0 ? done / every : 0;
+                int rc = launch_resident(h, R, thr, n, every > 0 ? every : 0,
+                                         E_series_dev ? E_series_dev + s0 : nullptr,
+                                         hist_series_dev ? hist_series_dev + s0 * h->q : nullptr);
+                if (rc) return rc;
+                h->t += (uint64_t)n;
+                done += n;
+            }
+            return POTTS_OK;
+        }
+        if (h->opt_variant == 2) return fail(POTTS_ERR_UNSUPPORTED, "resident variant unavailable: %s", R.why);
+    }
     for (int64_t n = 0; n < nsweeps; ++n) {
         const bool sample = every > 0 && ((n + 1) % every == 0);
         const int64_t idx = sample ? (n + 1) / every - 1 : 0;
-        int rc = launch_half_sweep(h, 0u, thr, nullptr);
+        unsigned long long *Hs = (sample && hist_series_dev) ? hist_series_dev + idx * h->q : nullptr;
+        int rc = launch_half_sweep(h, 0u, thr, nullptr, Hs);
         if (rc) return rc;
-        rc = launch_half_sweep(h, 1u, thr, (sample && E_series_dev) ? E_series_dev + idx : nullptr);
+        rc = launch_half_sweep(h, 1u, thr, (sample && E_series_dev) ? E_series_dev + idx : nullptr, Hs);
         if (rc) return rc;
         h->t += 1;
-        if (sample && hist_series_dev) {
-            rc = launch_measure(h, nullptr, hist_series_dev + idx * h->q);
-            if (rc) return rc;
-        }
     }
+    return POTTS_OK;
+}
+
+// after a stream sync: did a resident launch give up waiting for a neighbour?
+int check_device_error(potts_t *h)
+{
+    int e = 0;
+    CUDA_TRY(cudaMemcpyAsync(&e, h->error, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    if (e) return fail(POTTS_ERR_CUDA, "resident kernel: a neighbour wait timed out (results are invalid)");
     return POTTS_OK;
 }
 
@@ -229,7 +344,18 @@ int potts_create_ex(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t 
     h->plane[0] = h->ws;
     h->plane[1] = h->ws + h->plane_bytes;
     h->acc = (unsigned long long *)(h->ws + 2 * h->plane_bytes);
-    h->flag = (int *)(h->acc + ACC_WORDS - 1);
+    h->flag = (int *)(h->acc + 257);
+    h->error = h->flag + 1;
+    h->cta_flags = h->acc + 258;
+    {
+        int dev = 0, v = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+        h->num_sms = v;
+        cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        h->smem_optin = (size_t)v;
+        cudaMemsetAsync(h->acc, 0, ACC_WORDS * sizeof(unsigned long long), h->stream);
+    }
 
     cudaError_t e = cudaSuccess;
     if (init == POTTS_INIT_ORDERED) {
@@ -320,7 +446,7 @@ int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every, i
     if (rc) return rc;
     if (e != cudaSuccess || e2 != cudaSuccess)
         return fail(POTTS_ERR_CUDA, "series copy/sync failed: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
-    return POTTS_OK;
+    return check_device_error(h);
 }
 
 int potts_energy(potts_t *h, int64_t *E)
@@ -331,7 +457,8 @@ int potts_energy(potts_t *h, int64_t *E)
     if (rc) return rc;
     int64_t v = 0;
     CUDA_TRY(cudaMemcpyAsync(&v, h->acc, 8, cudaMemcpyDeviceToHost, h->stream));
-    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    rc = check_device_error(h);
+    if (rc) return rc;
     *E = v;
     return POTTS_OK;
 }
@@ -344,7 +471,8 @@ int potts_histogram(potts_t *h, int64_t *counts)
     if (rc) return rc;
     int64_t tmp[256];
     CUDA_TRY(cudaMemcpyAsync(tmp, h->acc + 1, 8 * (size_t)h->q, cudaMemcpyDeviceToHost, h->stream));
-    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    rc = check_device_error(h);
+    if (rc) return rc;
     std::memcpy(counts, tmp, 8 * (size_t)h->q);
     return POTTS_OK;
 }
@@ -372,7 +500,7 @@ int potts_download(potts_t *h, uint8_t *spins)
         }
     }
     cudaFree(stage);
-    return rc;
+    return rc ? rc : check_device_error(h);
 }
 
 int potts_upload(potts_t *h, const uint8_t *spins)
@@ -427,12 +555,14 @@ int potts_launch_count(potts_t *h, uint64_t *n)
 int potts_set_option(potts_t *h, const char *key, int64_t value)
 {
     if (!h || !key) return fail(POTTS_ERR_ARG, "null argument");
-    if (!std::strcmp(key, "variant")) { h->opt_variant = value; return POTTS_OK; }
-    if (!std::strcmp(key, "sweeps_per_launch")) {
-        if (value < 1) return fail(POTTS_ERR_ARG, "sweeps_per_launch must be >= 1");
-        h->opt_sweeps_per_launch = value; return POTTS_OK;
+    if (!std::strcmp(key, "variant")) {
+        if (value < 0 || value > 2) return fail(POTTS_ERR_ARG, "variant must be 0 (auto), 1 (streaming) or 2 (resident)");
+        h->opt_variant = value; return POTTS_OK;
     }
-    if (!std::strcmp(key, "use_graph")) { h->opt_use_graph = value != 0; return POTTS_OK; }
+    if (!std::strcmp(key, "resident_ctas")) {
+        if (value < 0 || value > MAX_CTAS) return fail(POTTS_ERR_ARG, "resident_ctas must be in [0, %d]", MAX_CTAS);
+        h->opt_resident_ctas = value; return POTTS_OK;
+    }
     return fail(POTTS_ERR_ARG, "unknown option '%s'", key);
 }
 
@@ -440,8 +570,10 @@ int potts_get_option(potts_t *h, const char *key, int64_t *value)
 {
     if (!h || !key || !value) return fail(POTTS_ERR_ARG, "null argument");
     if (!std::strcmp(key, "variant")) { *value = h->opt_variant; return POTTS_OK; }
-    if (!std::strcmp(key, "sweeps_per_launch")) { *value = h->opt_sweeps_per_launch; return POTTS_OK; }
-    if (!std::strcmp(key, "use_graph")) { *value = h->opt_use_graph; return POTTS_OK; }
+    if (!std::strcmp(key, "resident_ctas")) { *value = h->opt_resident_ctas; return POTTS_OK; }
+    if (!std::strcmp(key, "resident_active")) {            // read-only: would the next sweep call run resident?
+        *value = (h->opt_variant != 1 && plan_resident(h).ok) ? plan_resident(h).G : 0; return POTTS_OK;
+    }
     return fail(POTTS_ERR_ARG, "unknown option '%s'", key);
 }
 

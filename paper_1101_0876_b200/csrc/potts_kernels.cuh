@@ -1,9 +1,6 @@
-// potts_kernels.cuh -- device code of the checkerboard Potts sweep for sm_100a.
-//
-// Everything on the device is integer arithmetic: Philox4x32-10 keyed by
-// (seed; j, i, t, colour), multiply-high proposal, byte-parallel neighbour comparison, integer
-// threshold acceptance (PAPER.md:94 sec. 3, :145 sec. 3.2), and integer energy / histogram
-// reductions (sec. 3.4).  Not shared with oracle/ in any way.
+// potts_kernels.cuh -- streaming kernels of the checkerboard Potts sweep for sm_100a (U8 layout):
+// one half-sweep per launch reading the planes through L2/HBM, the standalone measurement, the
+// random start and the layout converters.  The per-site arithmetic is in potts_core.cuh.
 //
 // Spin layout "U8 split planes" (PAPER.md:159 packs whites then blacks; the exact map is ours):
 //   plane[c][i][k], c = (i+j)&1, k = j>>1, one byte per spin, row pitch L/2 bytes.
@@ -11,15 +8,9 @@
 // plane 1-c:  up [i-1][k], down [i+1][k], and horizontally [i][k],[i][k+1] if p = 1 or
 // [i][k-1],[i][k] if p = 0 (indices periodic).
 #pragma once
-#include <cstdint>
-#include <cuda_runtime.h>
+#include "potts_core.cuh"
 
 namespace potts {
-
-constexpr uint32_t PHILOX_M0 = 0xD2511F53u;
-constexpr uint32_t PHILOX_M1 = 0xCD9E8D57u;
-constexpr uint32_t PHILOX_W0 = 0x9E3779B9u;
-constexpr uint32_t PHILOX_W1 = 0xBB67AE85u;
 
 struct SweepParams {
     uint8_t *plane_own;         // plane of the colour being updated
@@ -28,134 +19,35 @@ struct SweepParams {
     int32_t pitch;              // L/2, bytes per plane row
     uint32_t q;
     uint32_t colour;            // 0 = white ((i+j) even), 1 = black
-    uint32_t t;                 // sweep counter (Philox counter word 2)
-    uint32_t key0, key1;        // seed low / high
+    HalfSweepKeys K;            // Philox key material of (seed, t, colour), built on the host
     uint32_t thr[4];            // floor(2^32 exp(-d/T)), d = 1..4
     unsigned long long *E_out;  // MEASURE: -= satisfied bonds seen from this colour's sites
+    unsigned long long *hist_out;  // HIST: += occupancies of this colour's sites after the update
 };
 
 // ---------------------------------------------------------------------------------------------
-// Philox4x32-10, words 0 and 1 only (the update rule uses w0 for the proposal and w1 for the
-// acceptance).  The last round therefore needs only the M1*c2 product.
-__device__ __forceinline__ void philox4x32_10_w01(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
-                                                  uint32_t k0, uint32_t k1, uint32_t &w0, uint32_t &w1)
-{
-#pragma unroll
-    for (int r = 0; r < 9; ++r) {
-        const uint32_t hi0 = __umulhi(PHILOX_M0, c0), lo0 = PHILOX_M0 * c0;
-        const uint32_t hi1 = __umulhi(PHILOX_M1, c2), lo1 = PHILOX_M1 * c2;
-        c0 = hi1 ^ c1 ^ k0;
-        c1 = lo1;
-        c2 = hi0 ^ c3 ^ k1;
-        c3 = lo0;
-        k0 += PHILOX_W0;
-        k1 += PHILOX_W1;
-    }
-    w0 = __umulhi(PHILOX_M1, c2) ^ c1 ^ k0;
-    w1 = PHILOX_M1 * c2;
-}
-
-// full 4-word version (init kernel, tests)
-__device__ __forceinline__ void philox4x32_10(uint32_t c[4], uint32_t k0, uint32_t k1)
-{
-#pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        const uint32_t hi0 = __umulhi(PHILOX_M0, c[0]), lo0 = PHILOX_M0 * c[0];
-        const uint32_t hi1 = __umulhi(PHILOX_M1, c[2]), lo1 = PHILOX_M1 * c[2];
-        c[0] = hi1 ^ c[1] ^ k0;
-        c[1] = lo1;
-        c[2] = hi0 ^ c[3] ^ k1;
-        c[3] = lo0;
-        k0 += PHILOX_W0;
-        k1 += PHILOX_W1;
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// Byte-parallel "not equal" flags: bit 7 of every byte of the result is set iff the bytes of a
-// and b differ.  WIDE = false assumes all spin values < 128 (q <= 128), so a^b has bit 7 clear
-// in every byte and adding 0x7f cannot carry across bytes.
-template <bool WIDE>
-__device__ __forceinline__ uint32_t ne_flags(uint32_t a, uint32_t b)
-{
-    const uint32_t x = a ^ b;
-    if (!WIDE) return (x + 0x7f7f7f7fu) & 0x80808080u;
-    return (((x & 0x7f7f7f7fu) + 0x7f7f7f7fu) | x) & 0x80808080u;
-}
-
-// per-byte count (0..4) of neighbours that differ from the bytes of s
-template <bool WIDE>
-__device__ __forceinline__ uint32_t ne_count4(uint32_t s, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt)
-{
-    return (ne_flags<WIDE>(s, up) >> 7) + (ne_flags<WIDE>(s, dn) >> 7) +
-           (ne_flags<WIDE>(s, lf) >> 7) + (ne_flags<WIDE>(s, rt) >> 7);
-}
-
-__device__ __forceinline__ uint32_t byte_sum(uint32_t v)   // sum of the 4 bytes (each <= 63)
-{
-    return (v * 0x01010101u) >> 24;
-}
-
-__device__ __forceinline__ int wrap(int x, int n) { return x < 0 ? x + n : (x >= n ? x - n : x); }
-
-// ---------------------------------------------------------------------------------------------
-// One word (4 same-colour sites, consecutive k) of the Metropolis update.
-//   own      current spins of the 4 sites
-//   up,dn,lf,rt  the 4 neighbour words, byte b = that neighbour of site b
-//   j0       column of byte 0 (columns advance by 2 per byte), i = row
-// Returns the new word; *ne_final receives the per-byte count of unequal neighbours of the
-// final spins (for the fused energy).
-template <bool WIDE>
-__device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t lf,
-                                                uint32_t rt, uint32_t j0, uint32_t i,
-                                                const SweepParams &P, const uint32_t *lut,
-                                                uint32_t *ne_final)
-{
-    uint32_t w0[4], w1[4];
-#pragma unroll
-    for (int b = 0; b < 4; ++b)
-        philox4x32_10_w01(j0 + 2u * b, i, P.t, P.colour, P.key0, P.key1, w0[b], w1[b]);
-    uint32_t prop = 0;
-#pragma unroll
-    for (int b = 0; b < 4; ++b) prop |= __umulhi(w0[b], P.q) << (8 * b);
-
-    const uint32_t c_old = ne_count4<WIDE>(own, up, dn, lf, rt);
-    const uint32_t c_new = ne_count4<WIDE>(prop, up, dn, lf, rt);
-    // d = n_old - n_new = ne_new - ne_old; biased by 4 per byte so that bytes stay in 0..8
-    const uint32_t dw = c_new + 0x04040404u - c_old;
-    uint32_t mask = 0;
-#pragma unroll
-    for (int b = 0; b < 4; ++b) {
-        const uint32_t dd = (dw >> (8 * b)) & 0xffu;       // d + 4
-        const bool acc = (dd <= 4u) || (w1[b] < lut[dd]);
-        mask |= acc ? (0xffu << (8 * b)) : 0u;
-    }
-    *ne_final = (c_new & mask) | (c_old & ~mask);
-    return (prop & mask) | (own & ~mask);
-}
-
-// ---------------------------------------------------------------------------------------------
 // Half-sweep, U8 layout, one thread per 16 consecutive same-colour sites of one row.
-// Requires L % 32 == 0.  grid = ceil(L * (L/32) / blockDim).
-template <bool WIDE, bool MEASURE>
-__global__ void __launch_bounds__(128) k_half_sweep_u8(const SweepParams P)
+// Block = (32 chunks, 4 rows); grid = (ceil(L/32 / 32), L/4).  Requires L % 32 == 0.
+constexpr int HS_ROWS = 4;
+
+template <bool WIDE, bool MEASURE, bool HIST>
+__global__ void __launch_bounds__(32 * HS_ROWS) k_half_sweep_u8(const __grid_constant__ SweepParams P)
 {
-    __shared__ uint32_t lut[16];
+    extern __shared__ uint32_t s_dyn[];             // HIST: the block's histogram table
+    __shared__ uint32_t lut[12];
     __shared__ unsigned long long blockE;
-    if (threadIdx.x < 16) {
-        const int dd = threadIdx.x;
-        lut[dd] = (dd >= 5 && dd <= 8) ? P.thr[dd - 5] : 0xFFFFFFFFu;
-    }
-    if (MEASURE && threadIdx.x == 0) blockE = 0ull;
+    const uint32_t tid = threadIdx.y * 32u + threadIdx.x;
+    if (tid < 9) lut[tid] = tid >= 5 ? P.thr[tid - 5] : 0u;
+    if (MEASURE && tid == 0) blockE = 0ull;
+    if (HIST)
+        for (uint32_t n = tid; n < hist_words(P.q); n += 32 * HS_ROWS) s_dyn[n] = 0u;
     __syncthreads();
 
     const int chunks = P.pitch >> 4;                                  // 16-byte chunks per row
-    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long total = (long long)P.L * chunks;
-    uint32_t satisfied = 0;
-    if (gid < total) {
-        const int i = (int)(gid / chunks);
-        const int x = (int)(gid - (long long)i * chunks);
+    const int x = (int)(blockIdx.x * 32u + threadIdx.x);
+    const int i = (int)(blockIdx.y * HS_ROWS + threadIdx.y);
+    uint32_t nef_sum = 0;
+    if (x < chunks) {
         const int k0 = x << 4;
         const uint32_t p = (uint32_t)(i + P.colour) & 1u;
         const int iu = wrap(i - 1, P.L), id = wrap(i + 1, P.L);
@@ -165,41 +57,40 @@ __global__ void __launch_bounds__(128) k_half_sweep_u8(const SweepParams P)
         const uint4 mid4 = *reinterpret_cast<const uint4 *>(P.plane_oth + row + k0);
         const uint4 up4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)iu * P.pitch + k0);
         const uint4 dn4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)id * P.pitch + k0);
-        // the one byte outside the chunk: [i][k0+16] if p = 1, [i][k0-1] if p = 0 (periodic)
-        const int ka = p ? wrap(k0 + 16, P.pitch) : wrap(k0 - 1, P.pitch);
-        const uint32_t adj = P.plane_oth[row + ka];
+        // the one word outside the chunk: [i][k0+16..] if p = 1, [i][..k0-1] if p = 0 (periodic)
+        const int ka = p ? wrap(k0 + 16, P.pitch) : wrap(k0 - 4, P.pitch);
+        const uint32_t adj = *reinterpret_cast<const uint32_t *>(P.plane_oth + row + ka);
 
+        const HalfSweepKeys &K = P.K;
+        const RowKeys R = row_keys(K, (uint32_t)i);
+        const uint32_t q = in_register(P.q);
         const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
-        const uint32_t mid[4] = {mid4.x, mid4.y, mid4.z, mid4.w};
+        const uint32_t mid[6] = {adj, mid4.x, mid4.y, mid4.z, mid4.w, adj};
         const uint32_t up[4] = {up4.x, up4.y, up4.z, up4.w};
         const uint32_t dn[4] = {dn4.x, dn4.y, dn4.z, dn4.w};
         uint32_t out[4];
 #pragma unroll
         for (int n = 0; n < 4; ++n) {
-            uint32_t lf, rt;
-            if (p) {   // neighbours at k and k+1
-                lf = mid[n];
-                const uint32_t nxt = (n < 3) ? mid[n < 3 ? n + 1 : 3] : adj;
-                rt = __funnelshift_r(mid[n], nxt, 8);
-            } else {   // neighbours at k-1 and k
-                const uint32_t prv = (n > 0) ? mid[n > 0 ? n - 1 : 0] : (adj << 24);
-                lf = __funnelshift_l(prv, mid[n], 8);
-                rt = mid[n];
-            }
-            uint32_t nef;
-            out[n] = update_word<WIDE>(own[n], up[n], dn[n], lf, rt, 2u * (uint32_t)(k0 + 4 * n) + p,
-                                       (uint32_t)i, P, lut, &nef);
-            if (MEASURE) satisfied += 16u - byte_sum(nef);
+            uint32_t lf, rt, nef;
+            horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
+            out[n] = update_word<WIDE>(own[n], up[n], dn[n], lf, rt, 2u * (uint32_t)(k0 + 4 * n) + p, q, K, R, lut, nef);
+            if (MEASURE) nef_sum += nef;                              // bytes stay <= 16
+            if (HIST) hist_add_word(s_dyn, P.q, out[n], threadIdx.x);
         }
         *reinterpret_cast<uint4 *>(P.plane_own + row + k0) = make_uint4(out[0], out[1], out[2], out[3]);
     }
     if (MEASURE) {
+        uint32_t satisfied = (x < chunks) ? 64u - byte_sum(nef_sum) : 0u;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
-        if ((threadIdx.x & 31) == 0) atomicAdd(&blockE, (unsigned long long)satisfied);
+        if (threadIdx.x == 0) atomicAdd(&blockE, (unsigned long long)satisfied);
         __syncthreads();
         // E = -(satisfied bonds): accumulate the two's-complement negative into the int64 slot
-        if (threadIdx.x == 0) atomicAdd(P.E_out, 0ull - blockE);
+        if (tid == 0) atomicAdd(P.E_out, 0ull - blockE);
+    }
+    if (HIST) {
+        __syncthreads();
+        hist_flush(s_dyn, P.q, P.hist_out, tid, 32 * HS_ROWS);
     }
 }
 
@@ -219,12 +110,11 @@ struct MeasureParams {
 template <bool WIDE>
 __global__ void __launch_bounds__(256) k_measure_u8(const MeasureParams P)
 {
-    extern __shared__ uint32_t s_hist[];            // [warps][q]
+    extern __shared__ uint32_t s_hist[];            // hist_words(q) counters, see potts_core.cuh
     __shared__ unsigned long long blockE;
-    const int warps = blockDim.x >> 5, warp = threadIdx.x >> 5;
     const bool do_hist = P.hist_out != nullptr;
     if (do_hist)
-        for (int n = threadIdx.x; n < warps * (int)P.q; n += blockDim.x) s_hist[n] = 0;
+        for (uint32_t n = threadIdx.x; n < hist_words(P.q); n += blockDim.x) s_hist[n] = 0;
     if (threadIdx.x == 0) blockE = 0ull;
     __syncthreads();
 
@@ -242,38 +132,30 @@ __global__ void __launch_bounds__(256) k_measure_u8(const MeasureParams P)
         const uint4 own4 = *reinterpret_cast<const uint4 *>(P.plane1 + row + k0);
         const uint4 mid4 = *reinterpret_cast<const uint4 *>(P.plane0 + row + k0);
         const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
-        const uint32_t mid[4] = {mid4.x, mid4.y, mid4.z, mid4.w};
         if (P.E_out) {
             const uint4 up4 = *reinterpret_cast<const uint4 *>(P.plane0 + (size_t)iu * P.pitch + k0);
             const uint4 dn4 = *reinterpret_cast<const uint4 *>(P.plane0 + (size_t)id * P.pitch + k0);
-            const int ka = p ? wrap(k0 + 16, P.pitch) : wrap(k0 - 1, P.pitch);
-            const uint32_t adj = P.plane0[row + ka];
+            const int ka = p ? wrap(k0 + 16, P.pitch) : wrap(k0 - 4, P.pitch);
+            const uint32_t adj = *reinterpret_cast<const uint32_t *>(P.plane0 + row + ka);
+            const uint32_t mid[6] = {adj, mid4.x, mid4.y, mid4.z, mid4.w, adj};
             const uint32_t up[4] = {up4.x, up4.y, up4.z, up4.w};
             const uint32_t dn[4] = {dn4.x, dn4.y, dn4.z, dn4.w};
+            uint32_t nef = 0;
 #pragma unroll
             for (int n = 0; n < 4; ++n) {
                 uint32_t lf, rt;
-                if (p) {
-                    lf = mid[n];
-                    const uint32_t nxt = (n < 3) ? mid[n < 3 ? n + 1 : 3] : adj;
-                    rt = __funnelshift_r(mid[n], nxt, 8);
-                } else {
-                    const uint32_t prv = (n > 0) ? mid[n > 0 ? n - 1 : 0] : (adj << 24);
-                    lf = __funnelshift_l(prv, mid[n], 8);
-                    rt = mid[n];
-                }
-                satisfied += 16u - byte_sum(ne_count4<WIDE>(own[n], up[n], dn[n], lf, rt));
+                horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
+                nef += ne_count4<WIDE>(own[n], up[n], dn[n], lf, rt);
             }
+            satisfied += 64u - byte_sum(nef);
         }
         if (do_hist) {
-            uint32_t *h = s_hist + warp * P.q;
+            const uint32_t oth[4] = {mid4.x, mid4.y, mid4.z, mid4.w};
 #pragma unroll
-            for (int n = 0; n < 4; ++n)
-#pragma unroll
-                for (int b = 0; b < 4; ++b) {
-                    atomicAdd(&h[(own[n] >> (8 * b)) & 0xffu], 1u);
-                    atomicAdd(&h[(mid[n] >> (8 * b)) & 0xffu], 1u);
-                }
+            for (int n = 0; n < 4; ++n) {
+                hist_add_word(s_hist, P.q, own[n], threadIdx.x & 31u);
+                hist_add_word(s_hist, P.q, oth[n], threadIdx.x & 31u);
+            }
         }
     }
     if (P.E_out) {
@@ -283,12 +165,7 @@ __global__ void __launch_bounds__(256) k_measure_u8(const MeasureParams P)
     }
     __syncthreads();
     if (P.E_out && threadIdx.x == 0) atomicAdd(P.E_out, 0ull - blockE);
-    if (do_hist)
-        for (int b = threadIdx.x; b < (int)P.q; b += blockDim.x) {
-            unsigned long long tot = 0;
-            for (int w = 0; w < warps; ++w) tot += s_hist[w * P.q + b];
-            if (tot) atomicAdd(&P.hist_out[b], tot);
-        }
+    if (do_hist) hist_flush(s_hist, P.q, P.hist_out, threadIdx.x, blockDim.x);
 }
 
 // ---------------------------------------------------------------------------------------------

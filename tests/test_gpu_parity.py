@@ -23,16 +23,38 @@ def pb():
     return pb
 
 
-def _pair(pb, L, q, seed, init, layout=0):
+# How the sweep is launched never changes what it computes (P6: "any GPU tile/launch shape ... same bits"):
+# streaming = one launch per half-sweep; resident = one persistent launch, lattice in shared memory,
+# split over `ctas` CTAs that exchange boundary rows (0 = the library's own choice).
+LAUNCH_SHAPES = {
+    "streaming": {"variant": 1},
+    "resident": {"variant": 2},
+    "resident1": {"variant": 2, "resident_ctas": 1},
+    "resident2": {"variant": 2, "resident_ctas": 2},
+    "resident3": {"variant": 2, "resident_ctas": 3},
+    "resident7": {"variant": 2, "resident_ctas": 7},
+    "resident148": {"variant": 2, "resident_ctas": 148},
+}
+
+
+def _pair(pb, L, q, seed, init, layout=0, shape=None):
     g = pb.Potts(L, q, seed, init, layout=layout)
+    for k, v in LAUNCH_SHAPES[shape or "streaming"].items():
+        g.potts_set_option(k, v)
+    if (shape or "streaming").startswith("resident") and g.potts_get_option("resident_active") == 0:
+        with pytest.raises(pb.PottsError) as e:          # a forced shape that cannot hold the lattice is refused
+            g.potts_sweep(1.0, 1)
+        assert e.value.code == pb.ERR_UNSUPPORTED
+        pytest.skip(f"L={L} does not fit the shared memory of shape {shape}")
     o = oracle.OraclePotts(L, q, seed, init)
     return g, o
 
 
-def test_cfg1_full_run_series_and_spins(pb):
+@pytest.mark.parametrize("shape", ["streaming", "resident", "resident2", "resident7"])
+def test_cfg1_full_run_series_and_spins(pb, shape):
     """BASELINE configs[0] in full: q=9, L=64, random start, 0.99 T_c, 1000 sweeps, E+hist every sweep."""
     w = workloads.CONFIGS[1]
-    g, o = _pair(pb, w.L, w.q, w.seed, w.init)
+    g, o = _pair(pb, w.L, w.q, w.seed, w.init, shape=shape)
     assert g.potts_energy() == o.energy()
     assert (g.potts_histogram() == o.histogram()).all()
     assert (g.potts_download() == o.spins()).all()
@@ -64,8 +86,9 @@ def test_cfg1_full_run_series_and_spins(pb):
     (64, 5, workloads.INIT_RANDOM, 0.05, 10),       # cold: thresholds ~ 0
     (512, 9, workloads.INIT_RANDOM, 0.995, 5),      # many blocks
 ])
-def test_every_sweep_spins_energy_histogram(pb, L, q, init, f, seed):
-    g, o = _pair(pb, L, q, seed, init)
+@pytest.mark.parametrize("shape", ["streaming", "resident", "resident1", "resident3", "resident148"])
+def test_every_sweep_spins_energy_histogram(pb, L, q, init, f, seed, shape):
+    g, o = _pair(pb, L, q, seed, init, shape=shape)
     T = f * workloads.t_c(q)
     assert (g.potts_download() == o.spins()).all()
     for _ in range(6):
