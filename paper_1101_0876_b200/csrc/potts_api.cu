@@ -36,8 +36,9 @@ int fail(int code, const char *fmt, ...)
 
 constexpr size_t ALIGN = 256;
 constexpr size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
-constexpr int MAX_CTAS = 512;             // upper bound on the resident kernel's grid (SM count)
-constexpr int ACC_WORDS = 1 + 256 + 1 + MAX_CTAS;   // E, hist[256], flag/error word, resident flags
+constexpr int MAX_CTAS = 160;             // upper bound on the resident kernel's grid (>= SM count of B200)
+constexpr int RESIDENT_L_MAX = 4096;      // largest lattice the resident kernel can hold (512 words per row)
+constexpr int ACC_WORDS = 1 + 256 + 1;    // E, hist[256], flag/error word
 
 }  // namespace
 
@@ -51,7 +52,7 @@ struct potts_s {
     unsigned long long *acc = nullptr;   // device scratch: [0] = E, [1..q] = histogram
     int *flag = nullptr;                 // device scratch flag (upload validation)
     int *error = nullptr;                // device: set by the resident kernel if a neighbour wait gave up
-    unsigned long long *cta_flags = nullptr;   // device: resident kernel's per-CTA progress counters
+    uint8_t *inbox = nullptr;            // device: resident kernel's boundary-row packets (null if L too large)
     cudaStream_t stream = nullptr;
     uint64_t launches = 0;
     int num_sms = 0;
@@ -78,9 +79,12 @@ int check_shape(int32_t L, int32_t q, int32_t layout)
 
 size_t plane_bytes_of(int32_t L, int32_t /*layout*/) { return align_up((size_t)L * (size_t)(L / 2)); }
 
+// resident kernel: per CTA 2 colours x 2 sides x L/8 packets of 8 bytes
+size_t inbox_bytes_of(int32_t L) { return L <= RESIDENT_L_MAX ? align_up((size_t)MAX_CTAS * 4 * (size_t)L) : 0; }
+
 size_t workspace_bytes_of(int32_t L, int32_t layout)
 {
-    return 2 * plane_bytes_of(L, layout) + align_up(ACC_WORDS * sizeof(unsigned long long)) + ALIGN;
+    return 2 * plane_bytes_of(L, layout) + align_up(ACC_WORDS * sizeof(unsigned long long)) + inbox_bytes_of(L) + ALIGN;
 }
 
 void thresholds(double T, uint32_t thr[4])
@@ -115,7 +119,7 @@ potts::SweepParams sweep_params(const potts_t *h, uint32_t colour, const uint32_
 template <bool WIDE, bool MEASURE, bool HIST>
 void launch_hs(const potts::SweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
 {
-    potts::k_half_sweep_u8<WIDE, MEASURE, HIST><<<grid, dim3(32, potts::HS_ROWS), smem, st>>>(P);
+    potts::k_half_sweep_u8<WIDE, MEASURE, HIST><<<grid, dim3(32, potts::HS_WARPS), smem, st>>>(P);
 }
 
 int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *E_out,
@@ -124,7 +128,7 @@ int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsign
     potts::SweepParams P = sweep_params(h, colour, thr, E_out);
     P.hist_out = hist_out;
     const int chunks = h->L / 32;
-    const dim3 grid((unsigned)((chunks + 31) / 32), (unsigned)(h->L / potts::HS_ROWS));
+    const dim3 grid((unsigned)((chunks + 31) / 32), (unsigned)(h->L / (potts::HS_WARPS * potts::HS_RPT)));
     const size_t smem = hist_out ? (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4 : 0;
     const int sel = (h->q > 128 ? 4 : 0) | (E_out ? 2 : 0) | (hist_out ? 1 : 0);
     switch (sel) {
@@ -173,19 +177,17 @@ int check_sweep_args(potts_t *h, double T, int64_t nsweeps)
 // ---- resident (persistent, shared-memory) path ------------------------------------------------
 struct ResidentPlan {
     bool ok = false;
-    int G = 0, ty = 0, wpr = 0, rows_max = 0;
+    int G = 0, tyc = 0, wpr = 0, rows_max = 0, nthreads = 0;
     size_t smem = 0;
     const char *why = "";
 };
-
-int gcd_int(int a, int b) { return b ? gcd_int(b, a % b) : a; }
 
 ResidentPlan plan_resident(const potts_t *h)
 {
     ResidentPlan R;
     const int L = h->L;
     R.wpr = L / 8;
-    if (R.wpr > 1024) { R.why = "L/8 words per row exceed 1024 threads"; return R; }
+    if (L > RESIDENT_L_MAX || !h->inbox) { R.why = "L exceeds the resident kernel's 512 words per row"; return R; }
     const long long words = (long long)L * R.wpr;                   // 4-site words per half-sweep
     long long G = h->opt_resident_ctas > 0 ? h->opt_resident_ctas : words / 512;
     if (G < 1) G = 1;
@@ -194,14 +196,14 @@ ResidentPlan plan_resident(const potts_t *h)
     if (G > MAX_CTAS) G = MAX_CTAS;
     R.G = (int)G;
     R.rows_max = (L + R.G - 1) / R.G;
-    // block = (wpr, ty) threads, a multiple of 32 in total
-    const int mult = 32 / gcd_int(R.wpr, 32);
-    int ty = R.rows_max < 1024 / R.wpr ? R.rows_max : 1024 / R.wpr;
-    ty = (ty + mult - 1) / mult * mult;
-    if (R.wpr * ty > 1024) ty = (1024 / R.wpr) / mult * mult;
-    if (ty < 1) { R.why = "no block shape with a multiple of 32 threads"; return R; }
-    R.ty = ty;
-    if ((R.rows_max + ty - 1) / ty > 60) { R.why = "too many rows per thread"; return R; }
+    // block = compute warps (wpr words x tyc rows at a time) + comm warps (wpr threads)
+    const int comm = (R.wpr + 31) / 32 * 32;
+    int tyc = (1024 - comm) / R.wpr;
+    if (tyc > R.rows_max) tyc = R.rows_max;
+    if (tyc < 1) { R.why = "no room for a compute row in a 1024-thread block"; return R; }
+    R.tyc = tyc;
+    R.nthreads = (R.wpr * tyc + 31) / 32 * 32 + comm;
+    if ((R.rows_max + tyc - 1) / tyc > 60) { R.why = "too many rows per thread"; return R; }
     const size_t hist = (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4;
     R.smem = 2 * (size_t)(R.rows_max + 2) * (L / 2) + hist;
     if (R.smem + 1024 > h->smem_optin) { R.why = "lattice does not fit the shared memory of the grid"; return R; }
@@ -226,20 +228,20 @@ int launch_resident(potts_t *h, const ResidentPlan &R, const uint32_t thr[4], in
     P.every = (uint32_t)every;
     P.E_series = E_series_dev;
     P.hist_series = hist_series_dev;
-    P.flags = h->cta_flags;
+    P.inbox = (uint2 *)h->inbox;
     P.error = h->error;
     P.rows_max = R.rows_max;
+    P.tyc = R.tyc;
     const void *fn = h->q > 128 ? (const void *)potts::k_resident_u8<true> : (const void *)potts::k_resident_u8<false>;
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
     int per_sm = 0;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, R.wpr * R.ty, R.smem));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, R.nthreads, R.smem));
     if (per_sm < 1 || (long long)per_sm * h->num_sms < R.G)
         return fail(POTTS_ERR_UNSUPPORTED, "resident kernel: %d CTAs cannot be co-resident", R.G);
-    // the progress counters are absolute half-sweep indices; a restored sweep counter may be lower
-    CUDA_TRY(cudaMemsetAsync(h->cta_flags, 0, sizeof(unsigned long long) * MAX_CTAS, h->stream));
+    // packet sequence numbers restart at 1 in every launch: clear what the previous launch left
+    if (R.G > 1) CUDA_TRY(cudaMemsetAsync(h->inbox, 0, (size_t)R.G * 4 * (size_t)h->L, h->stream));
     void *args[] = {(void *)&P};
-    CUDA_TRY(cudaLaunchCooperativeKernel(fn, dim3((unsigned)R.G), dim3((unsigned)R.wpr, (unsigned)R.ty), args, R.smem,
-                                         h->stream));
+    CUDA_TRY(cudaLaunchCooperativeKernel(fn, dim3((unsigned)R.G), dim3((unsigned)R.nthreads), args, R.smem, h->stream));
     h->launches += 1;
     return POTTS_OK;
 }
@@ -346,7 +348,7 @@ int potts_create_ex(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t 
     h->acc = (unsigned long long *)(h->ws + 2 * h->plane_bytes);
     h->flag = (int *)(h->acc + 257);
     h->error = h->flag + 1;
-    h->cta_flags = h->acc + 258;
+    h->inbox = inbox_bytes_of(L) ? h->ws + 2 * h->plane_bytes + align_up(ACC_WORDS * sizeof(unsigned long long)) : nullptr;
     {
         int dev = 0, v = 0;
         cudaGetDevice(&dev);

@@ -26,71 +26,76 @@ struct SweepParams {
 };
 
 // ---------------------------------------------------------------------------------------------
-// Half-sweep, U8 layout, one thread per 16 consecutive same-colour sites of one row.
-// Block = (32 chunks, 4 rows); grid = (ceil(L/32 / 32), L/4).  Requires L % 32 == 0.
-constexpr int HS_ROWS = 4;
+// Half-sweep, U8 layout.  A thread updates 16 consecutive same-colour sites (one 16-byte chunk) of
+// HS_RPT consecutive rows; a warp covers 32 chunks, a block HS_WARPS groups of rows.
+// grid = (ceil(L/32 / 32), L / (HS_WARPS * HS_RPT)).  Requires L % 32 == 0.
+constexpr int HS_WARPS = 4;
+constexpr int HS_RPT = 8;       // rows per thread: amortises the prologue and the block turnover
 
 template <bool WIDE, bool MEASURE, bool HIST>
-__global__ void __launch_bounds__(32 * HS_ROWS) k_half_sweep_u8(const __grid_constant__ SweepParams P)
+__global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_u8(const __grid_constant__ SweepParams P)
 {
     extern __shared__ uint32_t s_dyn[];             // HIST: the block's histogram table
     __shared__ uint32_t lut[12];
-    __shared__ unsigned long long blockE;
+    __shared__ uint32_t blockE;
     const uint32_t tid = threadIdx.y * 32u + threadIdx.x;
     if (tid < 9) lut[tid] = tid >= 5 ? P.thr[tid - 5] : 0u;
-    if (MEASURE && tid == 0) blockE = 0ull;
+    if (MEASURE && tid == 0) blockE = 0u;
     if (HIST)
-        for (uint32_t n = tid; n < hist_words(P.q); n += 32 * HS_ROWS) s_dyn[n] = 0u;
+        for (uint32_t n = tid; n < hist_words(P.q); n += 32 * HS_WARPS) s_dyn[n] = 0u;
     __syncthreads();
 
     const int chunks = P.pitch >> 4;                                  // 16-byte chunks per row
     const int x = (int)(blockIdx.x * 32u + threadIdx.x);
-    const int i = (int)(blockIdx.y * HS_ROWS + threadIdx.y);
-    uint32_t nef_sum = 0;
+    const int i0 = (int)(blockIdx.y * HS_WARPS + threadIdx.y) * HS_RPT;
+    uint32_t satisfied = 0;
     if (x < chunks) {
         const int k0 = x << 4;
-        const uint32_t p = (uint32_t)(i + P.colour) & 1u;
-        const int iu = wrap(i - 1, P.L), id = wrap(i + 1, P.L);
-        const size_t row = (size_t)i * P.pitch;
-
-        const uint4 own4 = *reinterpret_cast<const uint4 *>(P.plane_own + row + k0);
-        const uint4 mid4 = *reinterpret_cast<const uint4 *>(P.plane_oth + row + k0);
-        const uint4 up4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)iu * P.pitch + k0);
-        const uint4 dn4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)id * P.pitch + k0);
-        // the one word outside the chunk: [i][k0+16..] if p = 1, [i][..k0-1] if p = 0 (periodic)
-        const int ka = p ? wrap(k0 + 16, P.pitch) : wrap(k0 - 4, P.pitch);
-        const uint32_t adj = *reinterpret_cast<const uint32_t *>(P.plane_oth + row + ka);
-
         const HalfSweepKeys &K = P.K;
-        const RowKeys R = row_keys(K, (uint32_t)i);
         const uint32_t q = in_register(P.q);
-        const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
-        const uint32_t mid[6] = {adj, mid4.x, mid4.y, mid4.z, mid4.w, adj};
-        const uint32_t up[4] = {up4.x, up4.y, up4.z, up4.w};
-        const uint32_t dn[4] = {dn4.x, dn4.y, dn4.z, dn4.w};
-        uint32_t out[4];
+        const int kn = wrap(k0 + 16, P.pitch), kp = wrap(k0 - 4, P.pitch);
+#pragma unroll 1
+        for (int r = 0; r < HS_RPT; ++r) {
+            const int i = i0 + r;
+            const uint32_t p = (uint32_t)(i + P.colour) & 1u;
+            const int iu = wrap(i - 1, P.L), id = wrap(i + 1, P.L);
+            const size_t row = (size_t)i * P.pitch;
+            const uint4 own4 = *reinterpret_cast<const uint4 *>(P.plane_own + row + k0);
+            const uint4 mid4 = *reinterpret_cast<const uint4 *>(P.plane_oth + row + k0);
+            const uint4 up4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)iu * P.pitch + k0);
+            const uint4 dn4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)id * P.pitch + k0);
+            // the one word outside the chunk: [i][k0+16..] if p = 1, [i][..k0-1] if p = 0 (periodic)
+            const uint32_t adj = *reinterpret_cast<const uint32_t *>(P.plane_oth + row + (p ? kn : kp));
+
+            const RowKeys R = row_keys(K, (uint32_t)i);
+            const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
+            const uint32_t mid[6] = {adj, mid4.x, mid4.y, mid4.z, mid4.w, adj};
+            const uint32_t up[4] = {up4.x, up4.y, up4.z, up4.w};
+            const uint32_t dn[4] = {dn4.x, dn4.y, dn4.z, dn4.w};
+            uint32_t out[4], nef_sum = 0;
 #pragma unroll
-        for (int n = 0; n < 4; ++n) {
-            uint32_t lf, rt, nef;
-            horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
-            out[n] = update_word<WIDE>(own[n], up[n], dn[n], lf, rt, 2u * (uint32_t)(k0 + 4 * n) + p, q, K, R, lut, nef);
-            if (MEASURE) nef_sum += nef;                              // bytes stay <= 16
-            if (HIST) hist_add_word(s_dyn, P.q, out[n], threadIdx.x);
+            for (int n = 0; n < 4; ++n) {
+                uint32_t lf, rt, nef;
+                horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
+                out[n] = update_word<WIDE>(own[n], up[n], dn[n], lf, rt, 2u * (uint32_t)(k0 + 4 * n) + p, q, K, R, lut, nef);
+                if (MEASURE) nef_sum += nef;                          // bytes stay <= 16
+                if (HIST) hist_add_word(s_dyn, P.q, out[n], threadIdx.x);
+            }
+            *reinterpret_cast<uint4 *>(P.plane_own + row + k0) = make_uint4(out[0], out[1], out[2], out[3]);
+            if (MEASURE) satisfied += 64u - byte_sum(nef_sum);
         }
-        *reinterpret_cast<uint4 *>(P.plane_own + row + k0) = make_uint4(out[0], out[1], out[2], out[3]);
     }
     if (MEASURE) {
-        uint32_t satisfied = (x < chunks) ? 64u - byte_sum(nef_sum) : 0u;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
-        if (threadIdx.x == 0) atomicAdd(&blockE, (unsigned long long)satisfied);
+        if (threadIdx.x == 0) atomicAdd(&blockE, satisfied);
         __syncthreads();
         // E = -(satisfied bonds): accumulate the two's-complement negative into the int64 slot
-        if (tid == 0) atomicAdd(P.E_out, 0ull - blockE);
+        if (tid == 0) atomicAdd(P.E_out, 0ull - (unsigned long long)blockE);
     }
     if (HIST) {
         __syncthreads();
-        hist_flush(s_dyn, P.q, P.hist_out, tid, 32 * HS_ROWS);
+        hist_flush(s_dyn, P.q, P.hist_out, tid, 32 * HS_WARPS);
     }
 }
 

@@ -1,24 +1,30 @@
 // potts_resident.cuh -- persistent multi-sweep kernel: the lattice lives in shared memory.
 //
 // For lattices that fit the shared memory of the GPU (2 planes x L x L/2 bytes spread over up to 148
-// SMs: L <= ~4096) one cooperative launch runs ALL sweeps of a potts_sweep call.  CTA b owns the rows
+// SMs: L <= 4096) one cooperative launch runs ALL sweeps of a potts_sweep call.  CTA b owns the rows
 // [r0, r1) of both colour planes in its shared memory.  A half-sweep of colour c reads only the other
 // plane (sec. 3), so the only data that crosses CTAs are the two boundary rows of the
-// plane just written; they go through the global planes (L2) and a per-CTA counter:
+// plane just written.  They travel as 8-byte packets {4 spins, sequence number} written straight into
+// the neighbour's inbox in global memory (L2) by the thread that computed them; an aligned 8-byte
+// store is single-copy atomic, so the receiver just polls the packet until the sequence number is
+// the one it expects: no fence, no separate flag, one L2 round trip.
 //
-//   half-sweep hs (absolute index 2 t + c):
-//     W  wait until both neighbour CTAs have published half-sweep hs-1      (skipped for the first)
-//     H  copy their boundary rows of plane 1-c (global, L2) into the halo rows of shared memory
-//     B  update the CTA's first and last row, store them to shared AND global memory
-//     P  __syncthreads; one thread: fence, flags[b] = hs+1 (release)
-//     I  update the interior rows (hides the latency of P -> neighbour's W)
+//   Threads [0, ncw*32) compute: thread (tx = word in the row, ty) owns word tx of the row slots ty,
+//   ty + tyc, ...; slot 0 is the CTA's first row, slot 1 its last row, slots 2.. the interior rows.
+//   Threads [ncw*32, ncw*32 + wpr) only receive ("comm").  Per half-sweep of colour c:
+//     compute, boundary rows: update, store to shared memory, send packets
+//     compute, interior rows: warps without a boundary row start when the boundary warps are done
+//                             (named barrier 1), so the packets fly while the bulk of the work runs
+//     comm:    poll the inbox for the neighbours' packets of THIS half-sweep and write them into the
+//              halo rows of plane c (which only the next half-sweep reads)
+//     __syncthreads
 //
-// A neighbour overwrites a boundary row in global memory (its step B of hs+1) only after it has seen
-// flags[b] = hs+1, which CTA b sets after its step H of hs has consumed the previous version, so one
-// buffer per row is enough.  All rows are also written through to the global planes, so the global
-// state is complete when the kernel ends and every other entry point keeps working unchanged.
-// Energy and histogram of a sampled sweep are fused: per-thread sums, one block reduction, one
-// atomicAdd per CTA into the series slot (sec. 3.4).
+// Why one inbox slot per (CTA, colour, side) is enough: a sender overwrites a slot two half-sweeps
+// later, after it has received the receiver's packets of the half-sweep in between, and those were
+// sent after the barrier that ends the half-sweep in which the slot was consumed.
+// The global planes are written in the last sweep of the launch only, so every other entry point
+// (and the next launch) sees the complete state.  Energy and histogram of a sampled sweep are fused:
+// per-thread sums, one block reduction, one atomicAdd per CTA into the series slot.
 //
 // The random stream is a pure function of (seed, t, colour, i, j), so the result does not depend on
 // the number of CTAs or the row split; tests check that bit for bit.
@@ -38,40 +44,43 @@ struct ResidentParams {
     uint32_t every;                   // sample after every `every`-th sweep of this launch; 0 = never
     unsigned long long *E_series;     // device, nsweeps/every entries, may be null
     unsigned long long *hist_series;  // device, nsweeps/every rows of q, may be null
-    unsigned long long *flags;        // [gridDim.x] published half-sweeps, absolute (2 t + c + 1)
-    int *error;                       // set to 1 if a neighbour wait gave up
+    uint2 *inbox;                     // [gridDim.x][2 colours][2 sides][wpr] packets, zeroed before the launch
+    int *error;                       // set to 1 if a wait gave up
     int32_t rows_max;                 // rows of shared memory per plane = rows_max + 2
+    int32_t tyc;                      // thread rows that compute
 };
 
 constexpr long long RESIDENT_SPIN_LIMIT = 1ll << 24;   // polls before a wait gives up (seconds)
 
-__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long *p)
+__device__ __forceinline__ uint2 ld_packet(const uint2 *p)
 {
-    unsigned long long v;
-    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    uint2 v;
+    asm volatile("ld.relaxed.gpu.global.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p) : "memory");
     return v;
 }
 
-__device__ __forceinline__ void st_release_u64(unsigned long long *p, unsigned long long v)
+__device__ __forceinline__ void st_packet(uint2 *p, uint32_t data, uint32_t seq)
 {
-    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+    asm volatile("st.relaxed.gpu.global.v2.u32 [%0], {%1, %2};" ::"l"(p), "r"(data), "r"(seq) : "memory");
 }
 
-__device__ __forceinline__ uint4 ld_cg_u4(const void *p)   // L2 only: never a stale L1 line
+__device__ __forceinline__ void named_barrier_sync(int id, int nthreads)
 {
-    return __ldcg(reinterpret_cast<const uint4 *>(p));
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-// Block = (wpr_threads = L/8 words per plane row, ty rows); thread (tx, ty) owns word tx of the row
-// slots ty, ty + blockDim.y, ...  Slot 0 is the CTA's first row, slot 1 its last row, slots 2.. the
-// interior rows, so the boundary rows are finished (and published) first.
+__device__ __forceinline__ void named_barrier_arrive(int id, int nthreads)
+{
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
 template <bool WIDE>
 __global__ void __launch_bounds__(1024, 1) k_resident_u8(const __grid_constant__ ResidentParams P)
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
     __shared__ uint32_t lut[12];
-    __shared__ unsigned long long blockE;
-    __shared__ HalfSweepKeys s_keys[2];                             // double-buffered by colour
+    __shared__ uint32_t blockE;
+    __shared__ HalfSweepKeys s_keys[2];                             // one per colour
 
     const uint32_t G = gridDim.x, b = blockIdx.x;
     const int L = P.L, pitch = P.pitch;
@@ -79,121 +88,153 @@ __global__ void __launch_bounds__(1024, 1) k_resident_u8(const __grid_constant__
     const int rows = r1 - r0;
     const uint32_t up_cta = (b + G - 1) % G, dn_cta = (b + 1) % G;
     const int srows = P.rows_max + 2;                               // local row 0 / rows+1 = halos
-    const size_t plane_stride = (size_t)srows * pitch;
-    uint32_t *s_hist = reinterpret_cast<uint32_t *>(s_raw + 2 * (size_t)srows * pitch);
+    const uint32_t plane_stride = (uint32_t)srows * (uint32_t)pitch;
+    uint32_t *s_hist = reinterpret_cast<uint32_t *>(s_raw + 2 * plane_stride);
 
-    const uint32_t tx = threadIdx.x, ty = threadIdx.y;
-    const uint32_t nthreads = blockDim.x * blockDim.y, tid = ty * blockDim.x + tx;
-    const int wpr = pitch >> 2;
+    const uint32_t tid = threadIdx.x, nthreads = blockDim.x;
+    const int wpr = pitch >> 2;                                     // 4-site words per plane row
+    const int tyc = P.tyc;
+    const int ncompute = wpr * tyc;
+    const int nbar = (ncompute + 31) & ~31;                         // compute warps, in threads
+    const bool is_compute = (int)tid < ncompute;
+    const int ctx = (int)tid - nbar;                                // comm thread index
+    const bool is_comm = ctx >= 0 && ctx < wpr;
+    const int ty = is_compute ? (int)tid / wpr : 0;
+    const int tx = is_compute ? (int)tid - ty * wpr : (is_comm ? ctx : 0);
+    const int nb_rows = rows < 2 ? rows : 2;                        // boundary rows: local row 1 and local row `rows`
+    // a warp takes part in the boundary phase iff its first thread owns a boundary row
+    const bool warp_boundary = ((int)(tid & ~31u) / wpr) < (tyc < 2 ? tyc : 2);
+    // interior rows 2..rows-1 are dealt round-robin, starting with the thread rows that had no boundary row
+    const int ishift = tyc >= 3 ? 2 : 0;
+    const int lr_first = 2 + (ty - ishift + tyc) % tyc;
     const bool do_hist = P.hist_series != nullptr && P.every != 0;
     const bool do_E = P.E_series != nullptr && P.every != 0;
 
     if (tid < 9) lut[tid] = tid >= 5 ? P.thr[tid - 5] : 0u;
-    if (tid == 0) blockE = 0ull;
+    if (tid == 0) {
+        blockE = 0u;
+        s_keys[0] = half_sweep_keys(P.key0, P.key1, P.t0, 0u);
+    }
     if (do_hist)
         for (uint32_t n = tid; n < hist_words(P.q); n += nthreads) s_hist[n] = 0u;
-    // own rows of both planes: global -> shared (local row = global row - r0 + 1)
+    // own rows of both planes, and the halo rows of plane 1 (read by the first half-sweep, colour 0):
+    // global -> shared (local row = global row - r0 + 1)
     {
         const int vpr = pitch >> 4;                                 // uint4 per row
         for (int c = 0; c < 2; ++c)
-            for (int n = (int)tid; n < rows * vpr; n += (int)nthreads) {
+            for (int n = (int)tid; n < (rows + 2) * vpr; n += (int)nthreads) {
                 const int lr = n / vpr, v = n - lr * vpr;
-                *reinterpret_cast<uint4 *>(s_raw + c * plane_stride + (size_t)(lr + 1) * pitch + 16 * v) =
-                    ld_cg_u4(P.plane[c] + (size_t)(r0 + lr) * pitch + 16 * v);
+                if (c == 0 && (lr == 0 || lr == rows + 1)) continue;
+                const int gr = wrap(r0 + lr - 1, L);
+                *reinterpret_cast<uint4 *>(s_raw + c * plane_stride + (uint32_t)(lr * pitch + 16 * v)) =
+                    __ldcg(reinterpret_cast<const uint4 *>(P.plane[c] + (size_t)gr * pitch + 16 * v));
             }
     }
     __syncthreads();
 
-    const int nslots = rows;
-    const int iters = (nslots + (int)blockDim.y - 1) / (int)blockDim.y;
-    const int kb = ((rows < 2 ? rows : 2) - 1) / (int)blockDim.y;   // iteration that completes the boundary rows
-    const int kl = (int)tx == 0 ? wpr - 1 : (int)tx - 1, kr = (int)tx + 1 == wpr ? 0 : (int)tx + 1;
+    const uint32_t kl4 = 4u * (uint32_t)(tx == 0 ? wpr - 1 : tx - 1), kr4 = 4u * (uint32_t)(tx + 1 == wpr ? 0 : tx + 1);
+    const uint32_t q = in_register(P.q);
+    // inbox of CTA x, colour c, side s (0: the row above x's first row, 1: the row below x's last row)
+    auto inbox = [&](uint32_t x, uint32_t c, uint32_t s) { return P.inbox + ((size_t)(x * 2 + c) * 2 + s) * wpr + tx; };
+    uint2 *const send_up0 = inbox(up_cta, 0, 1);     // my first row -> the row below the last row of the CTA above
+    uint2 *const send_dn0 = inbox(dn_cta, 0, 0);     // my last row  -> the row above the first row of the CTA below
+    const uint2 *const recv0 = inbox(b, 0, 0);       // colour c: + c * 2 * wpr, side s: + s * wpr
+    const uint32_t cstride = 2u * (uint32_t)wpr;
 
     uint32_t until = P.every;                                       // sweeps until the next sample
     uint32_t sample_idx = 0;
+    uint32_t seq = 0;                                               // launch-local half-sweep number, from 1
     for (uint32_t n = 0; n < P.nsweeps; ++n) {
         const uint32_t t = P.t0 + n;
         const bool sample = P.every != 0 && --until == 0;
         if (sample) until = P.every;
+#pragma unroll
         for (uint32_t c = 0; c < 2; ++c) {
-            const unsigned long long hs = 2ull * t + c;
-            uint8_t *own_p = s_raw + c * plane_stride;
-            uint8_t *oth_p = s_raw + (1 - c) * plane_stride;
-            if (tid == 0) s_keys[c] = half_sweep_keys(P.key0, P.key1, t, c);   // visible after the barrier below
-            // ---- W: neighbours have published half-sweep hs-1
-            if (n != 0 || c != 0) {
-                if (tid < 2) {
-                    const unsigned long long *f = P.flags + (tid == 0 ? up_cta : dn_cta);
+            ++seq;
+            uint8_t *const own_col = s_raw + c * plane_stride + 4u * (uint32_t)tx;        // + lr*pitch: my word
+            const uint8_t *const oth_row = s_raw + (1u - c) * plane_stride;               // + lr*pitch: row start
+            // key material of the NEXT half-sweep (read after the barrier that ends this one)
+            if (tid == 0) s_keys[1 - c] = half_sweep_keys(P.key0, P.key1, t + c, 1u - c);
+            uint32_t nef_sum = 0, words_done = 0;
+            const bool count_E = sample && c == 1 && do_E, count_H = sample && do_hist;
+            if ((int)tid < nbar) {
+                const HalfSweepKeys K = s_keys[c];
+                // one word: local row lr, word tx
+                auto update = [&](int lr) -> uint32_t {
+                    const uint32_t ro = (uint32_t)(lr * pitch);
+                    const uint32_t i = (uint32_t)(r0 + lr - 1);
+                    const uint32_t p = (i + c) & 1u;
+                    const uint8_t *const orow = oth_row + ro;
+                    const uint32_t own = *reinterpret_cast<const uint32_t *>(own_col + ro);
+                    const uint32_t mid = *reinterpret_cast<const uint32_t *>(orow + 4u * (uint32_t)tx);
+                    const uint32_t up = *reinterpret_cast<const uint32_t *>(orow + 4u * (uint32_t)tx - pitch);
+                    const uint32_t dn = *reinterpret_cast<const uint32_t *>(orow + 4u * (uint32_t)tx + pitch);
+                    const uint32_t adj = *reinterpret_cast<const uint32_t *>(orow + (p ? kr4 : kl4));
+                    uint32_t lf, rt, nef;
+                    horizontal(p, mid, adj, lf, rt);
+                    const RowKeys R = row_keys(K, i);
+                    const uint32_t out = update_word<WIDE>(own, up, dn, lf, rt, 8u * (uint32_t)tx + p, q, K, R, lut, nef);
+                    *reinterpret_cast<uint32_t *>(own_col + ro) = out;
+                    if (count_E) { nef_sum += nef; ++words_done; }
+                    if (count_H) hist_add_word(s_hist, P.q, out, tid & 31u);
+                    return out;
+                };
+                if (warp_boundary) {
+                    // boundary rows first: the neighbours wait for them
+                    if (is_compute)
+                        for (int bs = ty; bs < nb_rows; bs += tyc) {
+                            const int lr = bs == 0 ? 1 : rows;
+                            const uint32_t out = update(lr);
+                            if (G > 1) {
+                                if (lr == 1) st_packet(send_up0 + c * cstride, out, seq);
+                                if (lr == rows) st_packet(send_dn0 + c * cstride, out, seq);
+                            }
+                        }
+                    named_barrier_arrive(1, nbar);
+                } else {
+                    named_barrier_sync(1, nbar);    // interior-only warps start when the boundary rows have been sent
+                }
+                if (is_compute)
+                    for (int lr = lr_first; lr < rows; lr += tyc) update(lr);
+            } else if (is_comm && G > 1) {
+                // receive the neighbours' boundary rows of plane c: halo rows for the NEXT half-sweep
+                uint8_t *const halo = s_raw + c * plane_stride + 4u * (uint32_t)tx;
+#pragma unroll 1
+                for (int s = 0; s < 2; ++s) {
+                    const uint2 *src = recv0 + c * cstride + (uint32_t)(s * wpr);
+                    uint2 v = ld_packet(src);
                     long long spins = 0;
-                    while (ld_acquire_u64(f) < hs)
+                    while (v.y != seq) {
                         if (++spins > RESIDENT_SPIN_LIMIT) { atomicExch(P.error, 1); break; }
+                        __nanosleep(40);
+                        v = ld_packet(src);
+                    }
+                    *reinterpret_cast<uint32_t *>(halo + (s == 0 ? 0u : (uint32_t)((rows + 1) * pitch))) = v.x;
+                }
+            }
+            __syncthreads();                                        // plane c complete in shared memory
+            if (G == 1) {
+                // a single CTA is its own neighbour: wrap the rows inside shared memory
+                if (is_comm) {
+                    uint8_t *const col = s_raw + c * plane_stride + 4u * (uint32_t)tx;
+                    *reinterpret_cast<uint32_t *>(col) = *reinterpret_cast<const uint32_t *>(col + (uint32_t)(rows * pitch));
+                    *reinterpret_cast<uint32_t *>(col + (uint32_t)((rows + 1) * pitch)) = *reinterpret_cast<const uint32_t *>(col + pitch);
                 }
                 __syncthreads();
             }
-            // ---- H: halo rows of the other plane
-            {
-                const int vpr = pitch >> 4;
-                const uint8_t *g = P.plane[1 - c];
-                const int gu = wrap(r0 - 1, L), gd = wrap(r1, L);
-                for (int v = (int)tid; v < 2 * vpr; v += (int)nthreads) {
-                    const bool lower = v >= vpr;
-                    const int vv = lower ? v - vpr : v;
-                    *reinterpret_cast<uint4 *>(oth_p + (size_t)(lower ? rows + 1 : 0) * pitch + 16 * vv) =
-                        ld_cg_u4(g + (size_t)(lower ? gd : gu) * pitch + 16 * vv);
-                }
-            }
-            __syncthreads();
-
-            const HalfSweepKeys K = s_keys[c];
-            const uint32_t q = in_register(P.q);
-            uint32_t nef_sum = 0, words_done = 0;
-            for (int k = 0; k < iters; ++k) {
-                const int slot = (int)ty + k * (int)blockDim.y;
-                if (slot < nslots) {
-                    const int lr = slot == 0 ? 1 : (slot == 1 ? rows : slot);        // local row 1..rows
-                    const int i = r0 + lr - 1;
-                    const uint32_t p = (uint32_t)(i + c) & 1u;
-                    const uint32_t *own_row = reinterpret_cast<const uint32_t *>(own_p + (size_t)lr * pitch);
-                    const uint32_t *mid_row = reinterpret_cast<const uint32_t *>(oth_p + (size_t)lr * pitch);
-                    const uint32_t own = own_row[tx];
-                    const uint32_t up = reinterpret_cast<const uint32_t *>(oth_p + (size_t)(lr - 1) * pitch)[tx];
-                    const uint32_t dn = reinterpret_cast<const uint32_t *>(oth_p + (size_t)(lr + 1) * pitch)[tx];
-                    const uint32_t mid = mid_row[tx];
-                    const uint32_t adj = mid_row[p ? kr : kl];
-                    uint32_t lf, rt, nef;
-                    horizontal(p, mid, adj, lf, rt);
-                    const RowKeys R = row_keys(K, (uint32_t)i);
-                    const uint32_t out = update_word<WIDE>(own, up, dn, lf, rt, 8u * tx + p, q, K, R, lut, nef);
-                    reinterpret_cast<uint32_t *>(own_p + (size_t)lr * pitch)[tx] = out;
-                    reinterpret_cast<uint32_t *>(P.plane[c] + (size_t)i * pitch)[tx] = out;
-                    if (sample) {
-                        if (c == 1 && do_E) { nef_sum += nef; ++words_done; }
-                        if (do_hist) hist_add_word(s_hist, P.q, out, tid & 31u);
-                    }
-                }
-                if (k == kb) {
-                    // ---- P: boundary rows are in global memory; publish half-sweep hs
-                    __syncthreads();
-                    if (tid == 0) {
-                        __threadfence();
-                        st_release_u64(P.flags + b, hs + 1ull);
-                    }
-                }
-            }
-            __syncthreads();                                        // own plane complete in shared memory
 
             if (sample && c == 1) {
                 if (do_E) {
                     // satisfied bonds seen from this thread's black sites = 4 per site - unequal neighbours
-                    // (nef_sum holds 4 byte counters, +<= 4 per word: the host keeps iters <= 60)
+                    // (nef_sum holds 4 byte counters, +<= 4 per word: the host keeps rows per thread <= 60)
                     uint32_t satisfied = 16u * words_done - byte_sum(nef_sum);
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
-                    if ((tid & 31u) == 0) atomicAdd(&blockE, (unsigned long long)satisfied);
+                    if ((tid & 31u) == 0 && satisfied) atomicAdd(&blockE, satisfied);
                     __syncthreads();
                     if (tid == 0) {
-                        atomicAdd(P.E_series + sample_idx, 0ull - blockE);
-                        blockE = 0ull;
+                        atomicAdd(P.E_series + sample_idx, 0ull - (unsigned long long)blockE);
+                        blockE = 0u;
                     }
                 }
                 if (do_hist) hist_flush(s_hist, P.q, P.hist_series + (size_t)sample_idx * P.q, tid, nthreads);
@@ -201,6 +242,16 @@ __global__ void __launch_bounds__(1024, 1) k_resident_u8(const __grid_constant__
                 __syncthreads();
             }
         }
+    }
+    // final state: shared -> global
+    {
+        const int vpr = pitch >> 4;
+        for (int c = 0; c < 2; ++c)
+            for (int n = (int)tid; n < rows * vpr; n += (int)nthreads) {
+                const int lr = n / vpr, v = n - lr * vpr;
+                *reinterpret_cast<uint4 *>(P.plane[c] + (size_t)(r0 + lr) * pitch + 16 * v) =
+                    *reinterpret_cast<const uint4 *>(s_raw + c * plane_stride + (uint32_t)((lr + 1) * pitch + 16 * v));
+            }
     }
 }
 
