@@ -128,7 +128,11 @@ int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsign
     potts::SweepParams P = sweep_params(h, colour, thr, E_out);
     P.hist_out = hist_out;
     const int chunks = h->L / 32;
-    const dim3 grid((unsigned)((chunks + 31) / 32), (unsigned)(h->L / (potts::HS_WARPS * potts::HS_RPT)));
+    const unsigned gx = (unsigned)((chunks + 31) / 32);
+    int rpt = 8;                                     // L % 32 == 0, so 8 divides L / HS_WARPS
+    while (rpt > 1 && (long long)gx * (h->L / (potts::HS_WARPS * rpt)) < 8ll * h->num_sms) rpt >>= 1;
+    P.rpt = rpt;
+    const dim3 grid(gx, (unsigned)(h->L / (potts::HS_WARPS * rpt)));
     const size_t smem = hist_out ? (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4 : 0;
     const int sel = (h->q > 128 ? 4 : 0) | (E_out ? 2 : 0) | (hist_out ? 1 : 0);
     switch (sel) {
@@ -196,14 +200,15 @@ ResidentPlan plan_resident(const potts_t *h)
     if (G > MAX_CTAS) G = MAX_CTAS;
     R.G = (int)G;
     R.rows_max = (L + R.G - 1) / R.G;
-    // block = compute warps (wpr words x tyc rows at a time) + comm warps (wpr threads)
-    const int comm = (R.wpr + 31) / 32 * 32;
-    int tyc = (1024 - comm) / R.wpr;
+    // block = compute warps (L/16 chunks x tyc rows at a time) + comm warps (L/16 threads)
+    const int cpr = L / 16;
+    const int comm = (cpr + 31) / 32 * 32;
+    int tyc = (1024 - comm) / cpr;
     if (tyc > R.rows_max) tyc = R.rows_max;
     if (tyc < 1) { R.why = "no room for a compute row in a 1024-thread block"; return R; }
     R.tyc = tyc;
-    R.nthreads = (R.wpr * tyc + 31) / 32 * 32 + comm;
-    if ((R.rows_max + tyc - 1) / tyc > 60) { R.why = "too many rows per thread"; return R; }
+    R.nthreads = (cpr * tyc + 31) / 32 * 32 + comm;
+    if ((R.rows_max + tyc - 1) / tyc > 30) { R.why = "too many rows per thread"; return R; }
     const size_t hist = (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4;
     R.smem = 2 * (size_t)(R.rows_max + 2) * (L / 2) + hist;
     if (R.smem + 1024 > h->smem_optin) { R.why = "lattice does not fit the shared memory of the grid"; return R; }
@@ -232,7 +237,9 @@ int launch_resident(potts_t *h, const ResidentPlan &R, const uint32_t thr[4], in
     P.error = h->error;
     P.rows_max = R.rows_max;
     P.tyc = R.tyc;
-    const void *fn = h->q > 128 ? (const void *)potts::k_resident_u8<true> : (const void *)potts::k_resident_u8<false>;
+    const bool small = R.nthreads <= 512;
+    const void *fn = h->q > 128 ? (small ? (const void *)potts::k_resident_u8<true, 512> : (const void *)potts::k_resident_u8<true, 1024>)
+                                : (small ? (const void *)potts::k_resident_u8<false, 512> : (const void *)potts::k_resident_u8<false, 1024>);
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
     int per_sm = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, R.nthreads, R.smem));

@@ -23,14 +23,15 @@ struct SweepParams {
     uint32_t thr[4];            // floor(2^32 exp(-d/T)), d = 1..4
     unsigned long long *E_out;  // MEASURE: -= satisfied bonds seen from this colour's sites
     unsigned long long *hist_out;  // HIST: += occupancies of this colour's sites after the update
+    int32_t rpt;                // rows per thread (divides L / HS_WARPS)
 };
 
 // ---------------------------------------------------------------------------------------------
 // Half-sweep, U8 layout.  A thread updates 16 consecutive same-colour sites (one 16-byte chunk) of
-// HS_RPT consecutive rows; a warp covers 32 chunks, a block HS_WARPS groups of rows.
-// grid = (ceil(L/32 / 32), L / (HS_WARPS * HS_RPT)).  Requires L % 32 == 0.
+// P.rpt consecutive rows; a warp covers 32 chunks, a block HS_WARPS groups of rows.
+// grid = (ceil(L/32 / 32), L / (HS_WARPS * rpt)).  Requires L % 32 == 0.  rpt up to 8 amortises the
+// prologue and the block turnover on large lattices; small ones keep rpt low to fill the GPU.
 constexpr int HS_WARPS = 4;
-constexpr int HS_RPT = 8;       // rows per thread: amortises the prologue and the block turnover
 
 template <bool WIDE, bool MEASURE, bool HIST>
 __global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_u8(const __grid_constant__ SweepParams P)
@@ -47,7 +48,7 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_u8(const __grid_co
 
     const int chunks = P.pitch >> 4;                                  // 16-byte chunks per row
     const int x = (int)(blockIdx.x * 32u + threadIdx.x);
-    const int i0 = (int)(blockIdx.y * HS_WARPS + threadIdx.y) * HS_RPT;
+    const int i0 = (int)(blockIdx.y * HS_WARPS + threadIdx.y) * P.rpt;
     uint32_t satisfied = 0;
     if (x < chunks) {
         const int k0 = x << 4;
@@ -55,7 +56,7 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_u8(const __grid_co
         const uint32_t q = in_register(P.q);
         const int kn = wrap(k0 + 16, P.pitch), kp = wrap(k0 - 4, P.pitch);
 #pragma unroll 1
-        for (int r = 0; r < HS_RPT; ++r) {
+        for (int r = 0; r < P.rpt; ++r) {
             const int i = i0 + r;
             const uint32_t p = (uint32_t)(i + P.colour) & 1u;
             const int iu = wrap(i - 1, P.L), id = wrap(i + 1, P.L);

@@ -9,9 +9,11 @@
 // store is single-copy atomic, so the receiver just polls the packet until the sequence number is
 // the one it expects: no fence, no separate flag, one L2 round trip.
 //
-//   Threads [0, ncw*32) compute: thread (tx = word in the row, ty) owns word tx of the row slots ty,
-//   ty + tyc, ...; slot 0 is the CTA's first row, slot 1 its last row, slots 2.. the interior rows.
-//   Threads [ncw*32, ncw*32 + wpr) only receive ("comm").  Per half-sweep of colour c:
+//   Threads [0, ncw*32) compute: thread (cx, ty) owns the 8-site chunk cx (two words) of some rows: in
+//   the boundary phase thread rows 0 / 1 take the CTA's first / last row, then the interior rows are
+//   dealt round-robin over all thread rows.  Threads [ncw*32, ncw*32 + L/16) only receive ("comm").
+//   Eight sites per thread (not four) halves the per-thread bookkeeping and leaves room for >64
+//   registers.  Per half-sweep of colour c:
 //     compute, boundary rows: update, store to shared memory, send packets
 //     compute, interior rows: warps without a boundary row start when the boundary warps are done
 //                             (named barrier 1), so the packets fly while the bulk of the work runs
@@ -64,6 +66,19 @@ __device__ __forceinline__ void st_packet(uint2 *p, uint32_t data, uint32_t seq)
     asm volatile("st.relaxed.gpu.global.v2.u32 [%0], {%1, %2};" ::"l"(p), "r"(data), "r"(seq) : "memory");
 }
 
+// two packets (an 8-site chunk) at once; each 8-byte half is still atomic on its own
+__device__ __forceinline__ uint4 ld_packet2(const uint2 *p)
+{
+    uint4 v;
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    return v;
+}
+
+__device__ __forceinline__ void st_packet2(uint2 *p, uint2 data, uint32_t seq)
+{
+    asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %2};" ::"l"(p), "r"(data.x), "r"(seq), "r"(data.y) : "memory");
+}
+
 __device__ __forceinline__ void named_barrier_sync(int id, int nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
@@ -74,13 +89,12 @@ __device__ __forceinline__ void named_barrier_arrive(int id, int nthreads)
     asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-template <bool WIDE>
-__global__ void __launch_bounds__(1024, 1) k_resident_u8(const __grid_constant__ ResidentParams P)
+template <bool WIDE, int MAXT>     // MAXT: block size the registers are budgeted for (512 -> up to 128 registers)
+__global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__ ResidentParams P)
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
     __shared__ uint32_t lut[12];
     __shared__ uint32_t blockE;
-    __shared__ HalfSweepKeys s_keys[2];                             // one per colour
 
     const uint32_t G = gridDim.x, b = blockIdx.x;
     const int L = P.L, pitch = P.pitch;
@@ -92,18 +106,19 @@ __global__ void __launch_bounds__(1024, 1) k_resident_u8(const __grid_constant__
     uint32_t *s_hist = reinterpret_cast<uint32_t *>(s_raw + 2 * plane_stride);
 
     const uint32_t tid = threadIdx.x, nthreads = blockDim.x;
-    const int wpr = pitch >> 2;                                     // 4-site words per plane row
+    const int cpr = pitch >> 3;                                     // 8-site chunks (2 words) per plane row
     const int tyc = P.tyc;
-    const int ncompute = wpr * tyc;
+    const int ncompute = cpr * tyc;
     const int nbar = (ncompute + 31) & ~31;                         // compute warps, in threads
     const bool is_compute = (int)tid < ncompute;
     const int ctx = (int)tid - nbar;                                // comm thread index
-    const bool is_comm = ctx >= 0 && ctx < wpr;
-    const int ty = is_compute ? (int)tid / wpr : 0;
-    const int tx = is_compute ? (int)tid - ty * wpr : (is_comm ? ctx : 0);
+    const bool is_comm = ctx >= 0 && ctx < cpr;
+    const int ty = is_compute ? (int)tid / cpr : 0;
+    const int cx = is_compute ? (int)tid - ty * cpr : (is_comm ? ctx : 0);
+    const uint32_t col = 8u * (uint32_t)cx;                         // byte offset of my chunk in a plane row
     const int nb_rows = rows < 2 ? rows : 2;                        // boundary rows: local row 1 and local row `rows`
     // a warp takes part in the boundary phase iff its first thread owns a boundary row
-    const bool warp_boundary = ((int)(tid & ~31u) / wpr) < (tyc < 2 ? tyc : 2);
+    const bool warp_boundary = ((int)(tid & ~31u) / cpr) < (tyc < 2 ? tyc : 2);
     // interior rows 2..rows-1 are dealt round-robin, starting with the thread rows that had no boundary row
     const int ishift = tyc >= 3 ? 2 : 0;
     const int lr_first = 2 + (ty - ishift + tyc) % tyc;
@@ -111,10 +126,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident_u8(const __grid_constant__
     const bool do_E = P.E_series != nullptr && P.every != 0;
 
     if (tid < 9) lut[tid] = tid >= 5 ? P.thr[tid - 5] : 0u;
-    if (tid == 0) {
-        blockE = 0u;
-        s_keys[0] = half_sweep_keys(P.key0, P.key1, P.t0, 0u);
-    }
+    if (tid == 0) blockE = 0u;
     if (do_hist)
         for (uint32_t n = tid; n < hist_words(P.q); n += nthreads) s_hist[n] = 0u;
     // own rows of both planes, and the halo rows of plane 1 (read by the first half-sweep, colour 0):
@@ -132,14 +144,18 @@ __global__ void __launch_bounds__(1024, 1) k_resident_u8(const __grid_constant__
     }
     __syncthreads();
 
-    const uint32_t kl4 = 4u * (uint32_t)(tx == 0 ? wpr - 1 : tx - 1), kr4 = 4u * (uint32_t)(tx + 1 == wpr ? 0 : tx + 1);
+    // the other-colour word left of my chunk (p = 0) / right of it (p = 1), periodic
+    const uint32_t col_prev = cx == 0 ? (uint32_t)pitch - 4u : col - 4u;
+    const uint32_t col_next = cx + 1 == cpr ? 0u : col + 8u;
     const uint32_t q = in_register(P.q);
-    // inbox of CTA x, colour c, side s (0: the row above x's first row, 1: the row below x's last row)
-    auto inbox = [&](uint32_t x, uint32_t c, uint32_t s) { return P.inbox + ((size_t)(x * 2 + c) * 2 + s) * wpr + tx; };
+    // inbox of CTA x, colour c, side s (0: the row above x's first row, 1: the row below x's last row);
+    // one packet {4 spins, seq} per word, so a chunk is two packets = 16 bytes
+    const uint32_t wpr = 2u * (uint32_t)cpr;
+    auto inbox = [&](uint32_t x, uint32_t c, uint32_t s) { return P.inbox + ((size_t)(x * 2 + c) * 2 + s) * wpr + 2u * (uint32_t)cx; };
     uint2 *const send_up0 = inbox(up_cta, 0, 1);     // my first row -> the row below the last row of the CTA above
     uint2 *const send_dn0 = inbox(dn_cta, 0, 0);     // my last row  -> the row above the first row of the CTA below
     const uint2 *const recv0 = inbox(b, 0, 0);       // colour c: + c * 2 * wpr, side s: + s * wpr
-    const uint32_t cstride = 2u * (uint32_t)wpr;
+    const uint32_t cstride = 2u * wpr;
 
     uint32_t until = P.every;                                       // sweeps until the next sample
     uint32_t sample_idx = 0;
@@ -151,32 +167,33 @@ __global__ void __launch_bounds__(1024, 1) k_resident_u8(const __grid_constant__
 #pragma unroll
         for (uint32_t c = 0; c < 2; ++c) {
             ++seq;
-            uint8_t *const own_col = s_raw + c * plane_stride + 4u * (uint32_t)tx;        // + lr*pitch: my word
+            uint8_t *const own_col = s_raw + c * plane_stride + col;                      // + lr*pitch: my chunk
             const uint8_t *const oth_row = s_raw + (1u - c) * plane_stride;               // + lr*pitch: row start
-            // key material of the NEXT half-sweep (read after the barrier that ends this one)
-            if (tid == 0) s_keys[1 - c] = half_sweep_keys(P.key0, P.key1, t + c, 1u - c);
             uint32_t nef_sum = 0, words_done = 0;
             const bool count_E = sample && c == 1 && do_E, count_H = sample && do_hist;
             if ((int)tid < nbar) {
-                const HalfSweepKeys K = s_keys[c];
-                // one word: local row lr, word tx
-                auto update = [&](int lr) -> uint32_t {
+                const HalfSweepKeys K = half_sweep_keys(P.key0, P.key1, t, c);             // uniform registers
+                // one chunk: local row lr, words 2cx and 2cx+1
+                auto update = [&](int lr) -> uint2 {
                     const uint32_t ro = (uint32_t)(lr * pitch);
                     const uint32_t i = (uint32_t)(r0 + lr - 1);
                     const uint32_t p = (i + c) & 1u;
                     const uint8_t *const orow = oth_row + ro;
-                    const uint32_t own = *reinterpret_cast<const uint32_t *>(own_col + ro);
-                    const uint32_t mid = *reinterpret_cast<const uint32_t *>(orow + 4u * (uint32_t)tx);
-                    const uint32_t up = *reinterpret_cast<const uint32_t *>(orow + 4u * (uint32_t)tx - pitch);
-                    const uint32_t dn = *reinterpret_cast<const uint32_t *>(orow + 4u * (uint32_t)tx + pitch);
-                    const uint32_t adj = *reinterpret_cast<const uint32_t *>(orow + (p ? kr4 : kl4));
-                    uint32_t lf, rt, nef;
-                    horizontal(p, mid, adj, lf, rt);
+                    const uint2 own = *reinterpret_cast<const uint2 *>(own_col + ro);
+                    const uint2 mid = *reinterpret_cast<const uint2 *>(orow + col);
+                    const uint2 up = *reinterpret_cast<const uint2 *>(orow + col - pitch);
+                    const uint2 dn = *reinterpret_cast<const uint2 *>(orow + col + pitch);
+                    const uint32_t adj = *reinterpret_cast<const uint32_t *>(orow + (p ? col_next : col_prev));
+                    uint32_t lf0, rt0, lf1, rt1, nef0, nef1;
+                    horizontal(p, mid.x, p ? mid.y : adj, lf0, rt0);
+                    horizontal(p, mid.y, p ? adj : mid.x, lf1, rt1);
                     const RowKeys R = row_keys(K, i);
-                    const uint32_t out = update_word<WIDE>(own, up, dn, lf, rt, 8u * (uint32_t)tx + p, q, K, R, lut, nef);
-                    *reinterpret_cast<uint32_t *>(own_col + ro) = out;
-                    if (count_E) { nef_sum += nef; ++words_done; }
-                    if (count_H) hist_add_word(s_hist, P.q, out, tid & 31u);
+                    uint2 out;
+                    out.x = update_word<WIDE>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, lut, nef0);
+                    out.y = update_word<WIDE>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, lut, nef1);
+                    *reinterpret_cast<uint2 *>(own_col + ro) = out;
+                    if (count_E) { nef_sum += nef0 + nef1; words_done += 2; }
+                    if (count_H) { hist_add_word(s_hist, P.q, out.x, tid & 31u); hist_add_word(s_hist, P.q, out.y, tid & 31u); }
                     return out;
                 };
                 if (warp_boundary) {
@@ -184,10 +201,10 @@ __global__ void __launch_bounds__(1024, 1) k_resident_u8(const __grid_constant__
                     if (is_compute)
                         for (int bs = ty; bs < nb_rows; bs += tyc) {
                             const int lr = bs == 0 ? 1 : rows;
-                            const uint32_t out = update(lr);
+                            const uint2 out = update(lr);
                             if (G > 1) {
-                                if (lr == 1) st_packet(send_up0 + c * cstride, out, seq);
-                                if (lr == rows) st_packet(send_dn0 + c * cstride, out, seq);
+                                if (lr == 1) st_packet2(send_up0 + c * cstride, out, seq);
+                                if (lr == rows) st_packet2(send_dn0 + c * cstride, out, seq);
                             }
                         }
                     named_barrier_arrive(1, nbar);
@@ -198,27 +215,27 @@ __global__ void __launch_bounds__(1024, 1) k_resident_u8(const __grid_constant__
                     for (int lr = lr_first; lr < rows; lr += tyc) update(lr);
             } else if (is_comm && G > 1) {
                 // receive the neighbours' boundary rows of plane c: halo rows for the NEXT half-sweep
-                uint8_t *const halo = s_raw + c * plane_stride + 4u * (uint32_t)tx;
+                uint8_t *const halo = s_raw + c * plane_stride + col;
 #pragma unroll 1
                 for (int s = 0; s < 2; ++s) {
-                    const uint2 *src = recv0 + c * cstride + (uint32_t)(s * wpr);
-                    uint2 v = ld_packet(src);
+                    const uint2 *src = recv0 + c * cstride + (uint32_t)s * wpr;
+                    uint4 v = ld_packet2(src);
                     long long spins = 0;
-                    while (v.y != seq) {
+                    while (v.y != seq || v.w != seq) {
                         if (++spins > RESIDENT_SPIN_LIMIT) { atomicExch(P.error, 1); break; }
                         __nanosleep(40);
-                        v = ld_packet(src);
+                        v = ld_packet2(src);
                     }
-                    *reinterpret_cast<uint32_t *>(halo + (s == 0 ? 0u : (uint32_t)((rows + 1) * pitch))) = v.x;
+                    *reinterpret_cast<uint2 *>(halo + (s == 0 ? 0u : (uint32_t)((rows + 1) * pitch))) = make_uint2(v.x, v.z);
                 }
             }
             __syncthreads();                                        // plane c complete in shared memory
             if (G == 1) {
                 // a single CTA is its own neighbour: wrap the rows inside shared memory
                 if (is_comm) {
-                    uint8_t *const col = s_raw + c * plane_stride + 4u * (uint32_t)tx;
-                    *reinterpret_cast<uint32_t *>(col) = *reinterpret_cast<const uint32_t *>(col + (uint32_t)(rows * pitch));
-                    *reinterpret_cast<uint32_t *>(col + (uint32_t)((rows + 1) * pitch)) = *reinterpret_cast<const uint32_t *>(col + pitch);
+                    uint8_t *const mine = s_raw + c * plane_stride + col;
+                    *reinterpret_cast<uint2 *>(mine) = *reinterpret_cast<const uint2 *>(mine + (uint32_t)(rows * pitch));
+                    *reinterpret_cast<uint2 *>(mine + (uint32_t)((rows + 1) * pitch)) = *reinterpret_cast<const uint2 *>(mine + pitch);
                 }
                 __syncthreads();
             }
@@ -226,7 +243,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident_u8(const __grid_constant__
             if (sample && c == 1) {
                 if (do_E) {
                     // satisfied bonds seen from this thread's black sites = 4 per site - unequal neighbours
-                    // (nef_sum holds 4 byte counters, +<= 4 per word: the host keeps rows per thread <= 60)
+                    // (nef_sum holds 4 byte counters, +<= 8 per chunk: the host keeps rows per thread <= 30)
                     uint32_t satisfied = 16u * words_done - byte_sum(nef_sum);
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
