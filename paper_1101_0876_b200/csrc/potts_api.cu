@@ -3,6 +3,7 @@
 #include "../../include/potts.h"
 #include "potts_kernels.cuh"
 #include "potts_resident.cuh"
+#include "potts_packed.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -49,6 +50,7 @@ struct potts_s {
     bool owns_ws = false;
     size_t plane_bytes = 0;
     uint8_t *plane[2] = {nullptr, nullptr};
+    potts::PackedPlanes pk = {};          // PACKED layout: nibble / high-bit planes inside plane[c]
     unsigned long long *acc = nullptr;   // device scratch: [0] = E, [1..q] = histogram
     int *flag = nullptr;                 // device scratch flag (upload validation)
     int *error = nullptr;                // device: set by the resident kernel if a neighbour wait gave up
@@ -72,19 +74,27 @@ int check_shape(int32_t L, int32_t q, int32_t layout)
         return fail(POTTS_ERR_ARG, "unknown layout %d", layout);
     if (L % 32 != 0)
         return fail(POTTS_ERR_UNSUPPORTED, "L = %d is not a multiple of 32 (kernel vector width)", L);
-    if (layout == POTTS_LAYOUT_PACKED)
-        return fail(POTTS_ERR_UNSUPPORTED, "packed layout not built yet");
+    if (layout == POTTS_LAYOUT_PACKED) {
+        if (q > 32) return fail(POTTS_ERR_UNSUPPORTED, "packed layout holds at most 5 bits per spin: q = %d > 32", q);
+        if (L % 64 != 0) return fail(POTTS_ERR_UNSUPPORTED, "packed layout needs L %% 64 == 0, L = %d", L);
+    }
     return POTTS_OK;
 }
 
-size_t plane_bytes_of(int32_t L, int32_t /*layout*/) { return align_up((size_t)L * (size_t)(L / 2)); }
+// bytes of ONE colour plane: U8 L*L/2; packed L*L/4 of nibbles (+ L*L/16 of high bits when q > 16)
+size_t nib_bytes_of(int32_t L) { return align_up((size_t)L * (size_t)(L / 4)); }
+size_t hb_bytes_of(int32_t L, int32_t q) { return q > 16 ? align_up((size_t)L * (size_t)(L / 16)) : 0; }
+size_t plane_bytes_of(int32_t L, int32_t q, int32_t layout)
+{
+    return layout == POTTS_LAYOUT_PACKED ? nib_bytes_of(L) + hb_bytes_of(L, q) : align_up((size_t)L * (size_t)(L / 2));
+}
 
 // resident kernel: per CTA 2 colours x 2 sides x L/8 packets of 8 bytes
 size_t inbox_bytes_of(int32_t L) { return L <= RESIDENT_L_MAX ? align_up((size_t)MAX_CTAS * 4 * (size_t)L) : 0; }
 
-size_t workspace_bytes_of(int32_t L, int32_t layout)
+size_t workspace_bytes_of(int32_t L, int32_t q, int32_t layout)
 {
-    return 2 * plane_bytes_of(L, layout) + align_up(ACC_WORDS * sizeof(unsigned long long)) + inbox_bytes_of(L) + ALIGN;
+    return 2 * plane_bytes_of(L, q, layout) + align_up(ACC_WORDS * sizeof(unsigned long long)) + inbox_bytes_of(L) + ALIGN;
 }
 
 void thresholds(double T, uint32_t thr[4])
@@ -148,8 +158,59 @@ int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsign
     return check_launch(h, "k_half_sweep_u8");
 }
 
+template <bool FIVE, bool MEASURE, bool HIST>
+void launch_pk(const potts::PackedSweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
+{
+    potts::k_half_sweep_packed<FIVE, MEASURE, HIST><<<grid, dim3(32, potts::PK_WARPS), smem, st>>>(P);
+}
+
+int launch_half_sweep_packed(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *E_out,
+                             unsigned long long *hist_out)
+{
+    potts::PackedSweepParams P;
+    P.S = h->pk;
+    P.q = (uint32_t)h->q;
+    P.colour = colour;
+    P.K = potts::half_sweep_keys((uint32_t)(h->seed & 0xFFFFFFFFull), (uint32_t)(h->seed >> 32), (uint32_t)h->t, colour);
+    for (int d = 0; d < 4; ++d) P.thr[d] = thr[d];
+    P.E_out = E_out;
+    P.hist_out = hist_out;
+    const int chunks = h->L / 64;
+    const unsigned gx = (unsigned)((chunks + 31) / 32);
+    int rpt = 4;                                     // L % 64 == 0, so 4 divides L / PK_WARPS
+    while (rpt > 1 && (long long)gx * (h->L / (potts::PK_WARPS * rpt)) < 8ll * h->num_sms) rpt >>= 1;
+    P.rpt = rpt;
+    const dim3 grid(gx, (unsigned)(h->L / (potts::PK_WARPS * rpt)));
+    const size_t smem = hist_out ? (size_t)h->q * 32 * 4 : 0;
+    const int sel = (h->q > 16 ? 4 : 0) | (E_out ? 2 : 0) | (hist_out ? 1 : 0);
+    switch (sel) {
+    case 0: launch_pk<false, false, false>(P, grid, smem, h->stream); break;
+    case 1: launch_pk<false, false, true>(P, grid, smem, h->stream); break;
+    case 2: launch_pk<false, true, false>(P, grid, smem, h->stream); break;
+    case 3: launch_pk<false, true, true>(P, grid, smem, h->stream); break;
+    case 4: launch_pk<true, false, false>(P, grid, smem, h->stream); break;
+    case 5: launch_pk<true, false, true>(P, grid, smem, h->stream); break;
+    case 6: launch_pk<true, true, false>(P, grid, smem, h->stream); break;
+    default: launch_pk<true, true, true>(P, grid, smem, h->stream); break;
+    }
+    return check_launch(h, "k_half_sweep_packed");
+}
+
 int launch_measure(potts_t *h, unsigned long long *E_out, unsigned long long *hist_out)
 {
+    if (h->layout == POTTS_LAYOUT_PACKED) {
+        potts::PackedMeasureParams M;
+        M.S = h->pk;
+        M.q = (uint32_t)h->q;
+        M.E_out = E_out;
+        M.hist_out = hist_out;
+        long long blocks = ((long long)h->L * (h->L / 64) + 255) / 256;
+        if (blocks > 148 * 8) blocks = 148 * 8;
+        const size_t smem = hist_out ? (size_t)h->q * 32 * 4 : 0;
+        if (h->q > 16) potts::k_measure_packed<true><<<(unsigned)blocks, 256, smem, h->stream>>>(M);
+        else potts::k_measure_packed<false><<<(unsigned)blocks, 256, smem, h->stream>>>(M);
+        return check_launch(h, "k_measure_packed");
+    }
     potts::MeasureParams M;
     M.plane0 = h->plane[0];
     M.plane1 = h->plane[1];
@@ -191,6 +252,7 @@ ResidentPlan plan_resident(const potts_t *h)
     ResidentPlan R;
     const int L = h->L;
     R.wpr = L / 8;
+    if (h->layout != POTTS_LAYOUT_U8) { R.why = "the resident kernel holds the U8 layout only"; return R; }
     if (L > RESIDENT_L_MAX || !h->inbox) { R.why = "L exceeds the resident kernel's 512 words per row"; return R; }
     const long long words = (long long)L * R.wpr;                   // 4-site words per half-sweep
     long long G = h->opt_resident_ctas > 0 ? h->opt_resident_ctas : words / 512;
@@ -283,9 +345,11 @@ int run_sweeps(potts_t *h, double T, int64_t nsweeps, int64_t every, unsigned lo
         const bool sample = every > 0 && ((n + 1) % every == 0);
         const int64_t idx = sample ? (n + 1) / every - 1 : 0;
         unsigned long long *Hs = (sample && hist_series_dev) ? hist_series_dev + idx * h->q : nullptr;
-        int rc = launch_half_sweep(h, 0u, thr, nullptr, Hs);
+        const bool pk = h->layout == POTTS_LAYOUT_PACKED;
+        unsigned long long *Es = (sample && E_series_dev) ? E_series_dev + idx : nullptr;
+        int rc = pk ? launch_half_sweep_packed(h, 0u, thr, nullptr, Hs) : launch_half_sweep(h, 0u, thr, nullptr, Hs);
         if (rc) return rc;
-        rc = launch_half_sweep(h, 1u, thr, (sample && E_series_dev) ? E_series_dev + idx : nullptr, Hs);
+        rc = pk ? launch_half_sweep_packed(h, 1u, thr, Es, Hs) : launch_half_sweep(h, 1u, thr, Es, Hs);
         if (rc) return rc;
         h->t += 1;
     }
@@ -314,7 +378,7 @@ int potts_workspace_bytes(int32_t L, int32_t q, int32_t layout, size_t *bytes)
     if (!bytes) return fail(POTTS_ERR_ARG, "null bytes pointer");
     int rc = check_shape(L, q, layout);
     if (rc) return rc;
-    *bytes = workspace_bytes_of(L, layout);
+    *bytes = workspace_bytes_of(L, q, layout);
     return POTTS_OK;
 }
 
@@ -325,7 +389,7 @@ int potts_create_ex(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t 
     if (init != POTTS_INIT_ORDERED && init != POTTS_INIT_RANDOM) return fail(POTTS_ERR_ARG, "bad init %d", init);
     int rc = check_shape(L, q, layout);
     if (rc) return rc;
-    const size_t need = workspace_bytes_of(L, layout);
+    const size_t need = workspace_bytes_of(L, q, layout);
     if (dev_workspace) {
         if (workspace_bytes < need)
             return fail(POTTS_ERR_NOMEM, "workspace of %zu bytes < %zu needed", workspace_bytes, need);
@@ -349,9 +413,18 @@ int potts_create_ex(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t 
         }
         h->owns_ws = true;
     }
-    h->plane_bytes = plane_bytes_of(L, layout);
+    h->plane_bytes = plane_bytes_of(L, q, layout);
     h->plane[0] = h->ws;
     h->plane[1] = h->ws + h->plane_bytes;
+    if (layout == POTTS_LAYOUT_PACKED) {
+        for (int c = 0; c < 2; ++c) {
+            h->pk.nib[c] = h->plane[c];
+            h->pk.hb[c] = q > 16 ? h->plane[c] + nib_bytes_of(L) : nullptr;
+        }
+        h->pk.L = L;
+        h->pk.pn = L / 4;
+        h->pk.ph = L / 16;
+    }
     h->acc = (unsigned long long *)(h->ws + 2 * h->plane_bytes);
     h->flag = (int *)(h->acc + 257);
     h->error = h->flag + 1;
@@ -369,6 +442,14 @@ int potts_create_ex(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t 
     cudaError_t e = cudaSuccess;
     if (init == POTTS_INIT_ORDERED) {
         e = cudaMemsetAsync(h->ws, 0, 2 * h->plane_bytes, h->stream);
+    } else if (layout == POTTS_LAYOUT_PACKED) {
+        const long long threads = 2ll * L * (L / 64);
+        const unsigned grid = (unsigned)((threads + 127) / 128);
+        const uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
+        if (q > 16) potts::k_init_random_packed<true><<<grid, 128, 0, h->stream>>>(h->pk, (uint32_t)q, k0, k1);
+        else potts::k_init_random_packed<false><<<grid, 128, 0, h->stream>>>(h->pk, (uint32_t)q, k0, k1);
+        h->launches += 1;
+        e = cudaGetLastError();
     } else {
         const long long words = 2ll * L * (L / 8);
         const int block = 256;
@@ -499,8 +580,14 @@ int potts_download(potts_t *h, uint8_t *spins)
     for (int i0 = 0; i0 < L && rc == POTTS_OK; i0 += rows) {
         const int r = (L - i0 < rows) ? L - i0 : rows;
         const long long threads = (long long)r * (L / 8);
-        potts::k_planes_to_rowmajor<<<(unsigned)((threads + 255) / 256), 256, 0, h->stream>>>(
-            h->plane[0], h->plane[1], stage, L, L / 2, i0, r);
+        if (h->layout == POTTS_LAYOUT_PACKED) {
+            const unsigned grid = (unsigned)(((long long)r * (L / 64) + 127) / 128);
+            if (h->q > 16) potts::k_packed_to_rowmajor<true><<<grid, 128, 0, h->stream>>>(h->pk, stage, i0, r);
+            else potts::k_packed_to_rowmajor<false><<<grid, 128, 0, h->stream>>>(h->pk, stage, i0, r);
+        } else {
+            potts::k_planes_to_rowmajor<<<(unsigned)((threads + 255) / 256), 256, 0, h->stream>>>(
+                h->plane[0], h->plane[1], stage, L, L / 2, i0, r);
+        }
         rc = check_launch(h, "k_planes_to_rowmajor");
         if (rc == POTTS_OK) {
             cudaError_t e = cudaMemcpyAsync(spins + (size_t)i0 * L, stage, (size_t)r * L, cudaMemcpyDeviceToHost, h->stream);
@@ -529,8 +616,13 @@ int potts_upload(potts_t *h, const uint8_t *spins)
         cudaError_t e = cudaMemcpyAsync(stage, spins + (size_t)i0 * L, (size_t)r * L, cudaMemcpyHostToDevice, h->stream);
         if (e != cudaSuccess) { rc = fail(POTTS_ERR_CUDA, "upload copy failed: %s", cudaGetErrorString(e)); break; }
         const long long threads = (long long)r * (L / 8);
-        potts::k_rowmajor_to_planes<<<(unsigned)((threads + 255) / 256), 256, 0, h->stream>>>(
-            stage, h->plane[0], h->plane[1], L, L / 2, i0, r, (uint32_t)h->q, h->flag);
+        if (h->layout == POTTS_LAYOUT_PACKED) {
+            const unsigned grid = (unsigned)(((long long)r * (L / 64) + 127) / 128);
+            if (h->q > 16) potts::k_rowmajor_to_packed<true><<<grid, 128, 0, h->stream>>>(stage, h->pk, i0, r, (uint32_t)h->q, h->flag);
+            else potts::k_rowmajor_to_packed<false><<<grid, 128, 0, h->stream>>>(stage, h->pk, i0, r, (uint32_t)h->q, h->flag);
+        } else
+            potts::k_rowmajor_to_planes<<<(unsigned)((threads + 255) / 256), 256, 0, h->stream>>>(
+                stage, h->plane[0], h->plane[1], L, L / 2, i0, r, (uint32_t)h->q, h->flag);
         rc = check_launch(h, "k_rowmajor_to_planes");
         if (rc == POTTS_OK && cudaStreamSynchronize(h->stream) != cudaSuccess)
             rc = fail(POTTS_ERR_CUDA, "upload sync failed");

@@ -165,3 +165,60 @@ def test_errors_on_device(pb):
         g.potts_sweep(1.0, 1)                          # counter would pass 2^32 - 1
     E, _ = g.potts_sweep_measured(1.0, 0, 1)           # empty run is fine
     assert E.size == 0
+
+
+# ---- sub-byte packed layout (BASELINE configs[3] is q=24 "sub-byte-packed ... (q<32)") ----------
+@pytest.mark.parametrize("L,q,init,f,seed", [
+    (64, 24, workloads.INIT_ORDERED, 1.002, 4),     # cfg4's parameters at the smallest packed L (5 bits)
+    (128, 24, workloads.INIT_RANDOM, 1.0, 4),
+    (192, 9, workloads.INIT_RANDOM, 0.99, 1),       # 4 bits, L not a power of two
+    (64, 16, workloads.INIT_RANDOM, 1.0, 2),        # largest q on 4 bits
+    (128, 17, workloads.INIT_RANDOM, 1.0, 3),       # first q on 5 bits
+    (64, 32, workloads.INIT_RANDOM, 1.05, 5),       # largest packed q
+    (64, 2, workloads.INIT_RANDOM, 1.0, 6),
+    (2048, 24, workloads.INIT_ORDERED, 1.002, 4),   # several blocks, more than one row per thread
+])
+def test_packed_layout_every_sweep(pb, L, q, init, f, seed):
+    g, o = _pair(pb, L, q, seed, init, layout=pb.LAYOUT_PACKED)
+    T = f * workloads.t_c(q)
+    assert (g.potts_download() == o.spins()).all()
+    assert g.potts_energy() == o.energy() and (g.potts_histogram() == o.histogram()).all()
+    nstep = 6 if L <= 256 else 2
+    for _ in range(nstep):
+        g.potts_sweep(T, 1)
+        o.sweep(T, 1)
+        assert (g.potts_download() == o.spins()).all()
+        assert g.potts_energy() == o.energy()
+        assert (g.potts_histogram() == o.histogram()).all()
+    n = 12 if L <= 256 else 3
+    Eg, Hg = g.potts_sweep_measured(T, n, 3, hist=True)
+    Eo, Ho = o.sweep_measured(T, n, 3, hist=True)
+    assert (Eg == Eo).all() and (Hg == Ho).all()
+    assert (g.potts_download() == o.spins()).all()
+
+
+def test_packed_upload_and_layout_invariance(pb):
+    L, q = 128, 24
+    s0 = workloads.synthetic_spins(L, q, 77, "domains")
+    T = 1.002 * workloads.t_c(q)
+    outs = []
+    for layout in (pb.LAYOUT_U8, pb.LAYOUT_PACKED):
+        g = pb.Potts(L, q, 4, workloads.INIT_ORDERED, layout=layout)
+        g.potts_upload(s0)
+        assert (g.potts_download() == s0).all()
+        E, H = g.potts_sweep_measured(T, 10, 1, hist=True)
+        outs.append((E, H, g.potts_download()))
+    for a, b in zip(outs[0], outs[1]):
+        assert (a == b).all()
+    o = oracle.OraclePotts(L, q, 4, workloads.INIT_ORDERED)
+    o.set_state(s0, 0)
+    Eo, Ho = o.sweep_measured(T, 10, 1, hist=True)
+    assert (outs[1][0] == Eo).all() and (outs[1][1] == Ho).all() and (outs[1][2] == o.spins()).all()
+
+
+def test_packed_limits(pb):
+    for L, q in ((64, 33), (96, 9)):
+        with pytest.raises(pb.PottsError) as e:
+            pb.Potts(L, q, 1, layout=pb.LAYOUT_PACKED)
+        assert e.value.code == pb.ERR_UNSUPPORTED
+    assert pb.potts_workspace_bytes(8192, 24, pb.LAYOUT_PACKED) < 0.7 * pb.potts_workspace_bytes(8192, 24, pb.LAYOUT_U8)
