@@ -39,8 +39,11 @@ import workloads  # noqa: E402
 # ---- roofline constants -------------------------------------------------
 SM_COUNT = 148
 ISSUE_LANES_PER_SM_CLK = 128          # 4 SMSPs x 1 warp-instruction (32 lanes) per clock
-I_ALG_PER_UPDATE = 39                 # Philox4x32-10 (w0,w1): 17 IMAD.WIDE + 2 IMAD.HI + 19 LOP3, + 1 IMAD.HI proposal
+I_ALG_PER_UPDATE = 36                 # Philox4x32-10 words 0,1 of counter (j,i,t,colour): 17 IMAD.WIDE + 18 LOP3, + 1 IMAD.HI proposal
 BYTES_ALG_PER_UPDATE_U8 = 3.0         # read own + read other (once) + write own, uint8 planes
+# Measured on B200 (profiles/r01b_pipe_model.md): for this integer mix (IMAD.WIDE / LOP3 / IADD3 / SHF / PRMT) an SM
+# sub-partition retires one warp instruction every 2 clocks, whichever pipe it goes to: half the nominal issue rate.
+MEASURED_INT_ISSUE_PER_CLK = 0.5
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for the workload)
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
@@ -123,7 +126,9 @@ class GpuRun:
         self.sweeps = self.per_t * len(self.temps)
         self.updates = self.sweeps * w.L * w.L
         self.ns = self.sweeps // w.every
-        self.layout = pb.LAYOUT_PACKED if w.packed and getattr(pb, "PACKED_AVAILABLE", False) else pb.LAYOUT_U8
+        self.layout = pb.LAYOUT_PACKED if w.packed else pb.LAYOUT_U8
+        bits = 8 if self.layout == pb.LAYOUT_U8 else (5 if w.q > 16 else 4)
+        self.bytes_per_update = 3.0 * bits / 8.0       # read own + read other (once) + write own
         self.options = dict(options or {})
         dev = torch.device("cuda", torch.cuda.current_device())
         self.E_dev = torch.zeros(max(self.ns, 1), dtype=torch.int64, device=dev)
@@ -137,7 +142,18 @@ class GpuRun:
         self.g = self.pb.Potts(self.w.L, self.w.q, self.seed, self.w.init, layout=self.layout)
         for k, v in self.options.items():
             self.g.potts_set_option(k, v)
+        self.resident_ctas = self.g.potts_get_option("resident_active")     # 0: one launch per half-sweep
         return self.g
+
+    @property
+    def kernel(self):
+        if self.layout != self.pb.LAYOUT_U8:
+            return "k_half_sweep_packed"
+        return "k_resident_u8" if self.resident_ctas else "k_half_sweep_u8"
+
+    @property
+    def kernel_launches_per_step(self):
+        return len(self.temps) if self.resident_ctas else 2 * self.sweeps
 
     def enqueue(self):
         """The step: all sweeps with the device-resident series; returns without a sync."""
@@ -271,19 +287,40 @@ def run_reference(args, w):
     print(json.dumps(line), flush=True)
 
 
+# ---- N > 1: independent samples, one per rank ------------------------------------------------------
+def rank_seed(w: workloads.Workload, rank: int) -> int:
+    """Rank r simulates sample r of the workload ("repeat over samples"): same parameters, seed + r."""
+    return w.seed + rank
+
+
+def reduce_over_ranks(dist, device, timed_ms: float, updates: int, launches: int):
+    """-> (max over ranks of the timed milliseconds, total updates, total launches).  `dist` is
+    torch.distributed (or None for one process); the path has no other collective (weak scaling)."""
+    import torch
+    t = torch.tensor([timed_ms], dtype=torch.float64, device=device)
+    c = torch.tensor([updates, launches], dtype=torch.int64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t.item()), int(c[0].item()), int(c[1].item())
+
+
 # ---- roofline -----------------------------------------------------------------------------------
-def roofline(w, updates_per_launch: float, ms_per_launch: float, sm_mhz_max: float, hbm_gbs: float, which: str,
-             bytes_per_update: float):
-    """ALU/issue roofline of the half-sweep kernel: algorithmic thread-instructions
-    (39 per update: the Philox block and the proposal the stream definition fixes) over the average
-    launch duration, against 148 SMs x 128 lanes x max SM clock; the HBM view is reported beside it."""
+def roofline(w, kernel: str, updates_per_launch: float, ms_per_launch: float, sm_mhz_max: float, hbm_gbs: float,
+             which: str, bytes_per_update: float):
+    """ALU/issue roofline of the dominant kernel: algorithmic thread-instructions (36 per
+    update: the Philox block and the proposal multiply the stream definition fixes) x updates per launch over the
+    average launch duration, against 148 SMs x 128 lanes/clk x max SM clock (one warp instruction per clock and
+    sub-partition, the guide's issue model); the HBM view and the measured integer issue ceiling go beside it."""
     sec = ms_per_launch * 1e-3
     ach = I_ALG_PER_UPDATE * updates_per_launch / sec / 1e12
     peak = SM_COUNT * ISSUE_LANES_PER_SM_CLK * sm_mhz_max * 1e6 / 1e12
     gbs = bytes_per_update * updates_per_launch / sec / 1e9
-    return {"bound": "alu", "kernel": "k_half_sweep", "achieved": ach, "peak": peak, "unit": "Tinstr/s (thread-level)",
+    return {"bound": "alu", "kernel": kernel, "achieved": ach, "peak": peak, "unit": "Tinstr/s (thread-level)",
             "frac": ach / peak, "peak_source": f"148 SMs x 128 lanes/clk x {sm_mhz_max:.0f} MHz ({which} max SM clock)",
-            "instr_per_update_algorithmic": I_ALG_PER_UPDATE,
+            "instr_per_update_algorithmic": I_ALG_PER_UPDATE, "ms_per_launch": ms_per_launch,
+            "updates_per_launch": updates_per_launch,
+            "frac_of_measured_int_issue": ach / (peak * MEASURED_INT_ISSUE_PER_CLK),
             "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(w.name),
             "hbm": {"achieved": gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": gbs / hbm_gbs,
                     "bytes_per_update_algorithmic": bytes_per_update, "peak_source": f"{which} copy bandwidth"}}
@@ -301,12 +338,13 @@ def per_config_table(pb, torch, flush, sm_max, hbm_gbs, which, skip=()):
         ms, launches = time_steps(torch, run, steps=3, warmup=1, flush=flush)
         sec = statistics.median(ms) * 1e-3
         ups = run.updates / sec
-        half_sweeps = 2 * run.sweeps
-        r = roofline(w, w.L * w.L / 2, sec * 1e3 / half_sweeps, sm_max, hbm_gbs, which,
-                     bytes_per_update=run.g.bytes_per_update() if hasattr(run.g, "bytes_per_update") else BYTES_ALG_PER_UPDATE_U8)
+        nl = run.kernel_launches_per_step
+        r = roofline(w, run.kernel, run.updates / nl, sec * 1e3 / nl, sm_max, hbm_gbs, which, run.bytes_per_update)
         out[w.name] = {"q": w.q, "L": w.L, "sweeps_timed": run.sweeps, "of_sweeps": w.total_sweeps,
                        "ns_per_spin_flip": 1e9 / ups, "spin_updates_per_s": ups, "ms": sec * 1e3,
-                       "launches": launches // 3, "alu_frac": r["frac"], "hbm_frac": r["hbm"]["frac"],
+                       "launches": launches // 3, "kernel": run.kernel, "resident_ctas": run.resident_ctas,
+                       "alu_frac": r["frac"], "alu_frac_of_measured_int_issue": r["frac_of_measured_int_issue"],
+                       "hbm_frac": r["hbm"]["frac"],
                        "layout": "packed" if run.layout == pb.LAYOUT_PACKED else "u8"}
         run.g.close()
         del run
@@ -353,7 +391,7 @@ def main():
     options = {kv.split("=")[0]: int(kv.split("=")[1]) for kv in args.option}
 
     # rank r runs sample r of the workload (independent lattice, seed + r): weak scaling, no collective
-    run = GpuRun(pb, torch, w, w.seed + rank, args.max_sweeps, options)
+    run = GpuRun(pb, torch, w, rank_seed(w, rank), args.max_sweeps, options)
 
     def barrier():
         torch.cuda.synchronize()
@@ -367,27 +405,19 @@ def main():
         ms, launches = time_steps(torch, run, args.steps, args.warmup, flush)
     barrier()
     wall = time.perf_counter() - t_wall0
-    total_ms = torch.tensor([sum(ms)], dtype=torch.float64, device="cuda")
-    counts = torch.tensor([run.updates * args.steps, launches], dtype=torch.int64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
-        dist.all_reduce(counts, op=dist.ReduceOp.SUM)
-    total_s = float(total_ms.item()) * 1e-3
-    updates_all, launches_all = int(counts[0].item()), int(counts[1].item())
+    total_ms, updates_all, launches_all = reduce_over_ranks(dist, "cuda", sum(ms), run.updates * args.steps, launches)
+    total_s = total_ms * 1e-3
     value = updates_all / total_s
-    bpu = BYTES_ALG_PER_UPDATE_U8 if run.layout == pb.LAYOUT_U8 else run.g.bytes_per_update()
-    half_sweeps = 2 * run.sweeps
-    roof = roofline(w, w.L * w.L / 2, (sum(ms) / len(ms)) / half_sweeps, sm_max, hbm_gbs, which, bpu)
+    nl = run.kernel_launches_per_step
+    roof = roofline(w, run.kernel, run.updates / nl, (sum(ms) / len(ms)) / nl, sm_max, hbm_gbs, which, run.bytes_per_update)
 
     e2e = None
     if not args.no_e2e:
         barrier()
         ms_e, _ = time_steps(torch, run, args.steps, max(1, args.warmup), flush, e2e=True)
-        tot_e = torch.tensor([sum(ms_e)], dtype=torch.float64, device="cuda")
-        if dist is not None:
-            dist.all_reduce(tot_e, op=dist.ReduceOp.MAX)
-        e2e = {"value": run.updates * args.steps * world / (float(tot_e.item()) * 1e-3), "unit": "spin updates/s",
-               "h2d_bytes_per_step": run.h2d, "d2h_bytes_per_step": run.d2h, "ms_per_step": float(tot_e.item()) / args.steps,
+        tot_e, upd_e, _ = reduce_over_ranks(dist, "cuda", sum(ms_e), run.updates * args.steps, 0)
+        e2e = {"value": upd_e / (tot_e * 1e-3), "unit": "spin updates/s",
+               "h2d_bytes_per_step": run.h2d, "d2h_bytes_per_step": run.d2h, "ms_per_step": tot_e / args.steps,
                "path": "potts_upload (pinned host) + potts_sweep_measured (host series) + potts_download (pinned host)"}
     layout = "packed" if run.layout == pb.LAYOUT_PACKED else "u8"
     run.g.close()

@@ -44,8 +44,9 @@ enum {
     POTTS_ERR_ARG = 1,         /* null pointer, L < 2 or odd, q outside [2,256], T not finite or <= 0,
                                   nsweeps < 0, every < 1 or not dividing nsweeps, bad init/layout,
                                   spin value >= q in an upload, sweep counter would pass 2^32 - 1 */
-    POTTS_ERR_UNSUPPORTED = 2, /* L not a multiple of 32 (vector width of the kernels), or q too large
-                                  for the packed layout */
+    POTTS_ERR_UNSUPPORTED = 2, /* L not a multiple of 32 (vector width of the kernels; 64 for the packed
+                                  layout), q > 32 with the packed layout, or a forced launch variant that
+                                  cannot hold this lattice */
     POTTS_ERR_NOMEM = 3,       /* device or host allocation failed / workspace too small */
     POTTS_ERR_CUDA = 4         /* CUDA runtime error (no device, launch failure, ...) */
 };
@@ -54,8 +55,9 @@ enum { POTTS_INIT_ORDERED = 0 /* all s = 0 */, POTTS_INIT_RANDOM = 1 /* uniform 
 
 enum {
     POTTS_LAYOUT_U8 = 0,    /* one byte per spin, split by colour */
-    POTTS_LAYOUT_PACKED = 1 /* sub-byte: 4 bits per spin for q <= 16, 5 bits packed 6-per-word..
-                               see DESIGN.md section 5; results are bit-identical to U8 */
+    POTTS_LAYOUT_PACKED = 1 /* sub-byte, q <= 32, L % 64 == 0: 4 bits per spin (nibble plane) for q <= 16,
+                               5 bits (nibble plane + high-bit plane) for 16 < q <= 32; DESIGN.md section 5.
+                               Results are bit-identical to U8 */
 };
 
 /* ---- lifetime ------------------------------------------------------------------------------
@@ -132,8 +134,12 @@ int potts_magnetisation(const int64_t *counts, int32_t q, double *m);
 int potts_launch_count(potts_t *h, uint64_t *n);
 
 /* potts_set_option: tuning knobs that change HOW the sweep is launched, never WHAT it computes
- * (tests assert bit-identity across them).  Unknown key -> POTTS_ERR_ARG.  Keys: see DESIGN.md
- * section 6 ("variant", "sweeps_per_launch", "use_graph"). */
+ * (tests assert bit-identity across them).  Unknown key -> POTTS_ERR_ARG.  Keys:
+ *   "variant"          0 = automatic, 1 = streaming (one kernel launch per half-sweep, planes read through
+ *                      L2/HBM), 2 = resident (one persistent cooperative launch per call, lattice in shared
+ *                      memory; U8 layout, L <= 4096; POTTS_ERR_UNSUPPORTED from the sweep call otherwise)
+ *   "resident_ctas"    0 = automatic, else the number of CTAs the resident kernel splits the rows over
+ *   "resident_active"  read-only: CTAs the next sweep call would run resident on (0 = streaming) */
 int potts_set_option(potts_t *h, const char *key, int64_t value);
 int potts_get_option(potts_t *h, const char *key, int64_t *value);
 
