@@ -55,5 +55,16 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_microbench() -> str:
+    """The issue-model microbenchmark (a measurement tool, see csrc/microbench_issue.cu)."""
+    out = os.path.join(HERE, "microbench_issue")
+    cmd = [_nvcc(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-o", out,
+           os.path.join(CSRC, "microbench_issue.cu")]
+    subprocess.check_call(cmd)
+    return out
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose=True))
+    if "--microbench" in sys.argv:
+        print(build_microbench())

@@ -4,12 +4,12 @@
 // (seed; j, i, t, colour), multiply-high proposal, byte-parallel neighbour comparison and integer
 // threshold acceptance (PAPER.md:94 sec. 3, :145 sec. 3.2).  Not shared with oracle/ in any way.
 //
-// Cost model this file is written against (profiles/r01a_first_path.md, measured on B200): a
-// 32x32->64 multiply (IMAD.WIDE) occupies the multiplier pipe of an SM sub-partition for 4 cycles
-// per warp, every other integer instruction (LOP3 / IADD3 / SHF / PRMT / ISETP) its ALU pipe for 2.
-// One update needs 17 wide multiplies of Philox (the stream definition fixes them) + 1 for the
-// proposal, so the multiplier pipe gives a floor of ~72 cycles per warp of updates and the ALU
-// instructions must stay under ~35 per update to hide beneath it.
+// Cost model this file is written against (profiles/r01b_pipe_model.md, measured on B200): for this
+// integer mix an SM sub-partition retires one warp instruction every 2 clocks whichever pipe it goes to
+// (IMAD.WIDE, IMAD, LOP3, IADD3, SHF, PRMT alike; IMAD.HI and POPC take 4), so the time of an update is
+// its instruction count.  One update needs 17 IMAD.WIDE + 18 LOP3 of Philox (fixed by the stream
+// definition) + 1 multiply for the proposal; everything else (neighbour compare, acceptance, packing,
+// loads and stores: ~22 instructions per update at 16 sites per thread) is overhead to keep small.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -23,16 +23,16 @@ constexpr uint32_t PHILOX_W1 = 0xBB67AE85u;
 
 __device__ __forceinline__ void mul_wide(uint32_t a, uint32_t b, uint32_t &hi, uint32_t &lo)
 {
-    // one IMAD.WIDE (4 multiplier-pipe cycles per warp); written in PTX so that the compiler does not
-    // split it into IMAD.HI + IMAD (4 + 2 cycles) where only part of the product looks live
+    // one IMAD.WIDE; written in PTX so that the compiler does not split it into IMAD.HI + IMAD
+    // (twice the issue cost) where only part of the product looks live
     unsigned long long p;
     asm("mul.wide.u32 %0, %1, %2;" : "=l"(p) : "r"(a), "r"(b));
     asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(p));
 }
 
 // Copy of a kernel-uniform value held in an ordinary register.  Multiplies cannot take a uniform-
-// register operand, and the compiler otherwise re-materialises the copy (an IMAD.U32 on the
-// multiplier pipe) before every use.
+// register operand, and the compiler otherwise re-materialises the copy (one more instruction)
+// before every use.
 __device__ __forceinline__ uint32_t in_register(uint32_t v)
 {
     uint32_t r;
@@ -72,10 +72,10 @@ struct HalfSweepKeys {
     uint32_t k0, k1;  // the key itself (round r uses k + r*W)
 };
 
-// Host and device: the streaming kernels get the keys as launch parameters, the resident kernel
-// computes them once per half-sweep in one thread and broadcasts them through shared memory.  (If
-// every thread derived xb from two uniform operands the compiler would fold the XOR into each use
-// and re-copy a uniform register through the multiplier pipe every time.)
+// Host and device: the streaming kernels get the keys as launch parameters (if every thread derived
+// xb from two uniform operands the compiler would fold the XOR into each use and re-copy a uniform
+// register for every site); the resident kernel unrolls the colour loop, so there the colour is a
+// literal and the keys stay in uniform registers.
 __host__ __device__ inline HalfSweepKeys half_sweep_keys(uint32_t key0, uint32_t key1, uint32_t t, uint32_t colour)
 {
     HalfSweepKeys K;

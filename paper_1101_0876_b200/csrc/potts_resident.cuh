@@ -9,22 +9,22 @@
 // store is single-copy atomic, so the receiver just polls the packet until the sequence number is
 // the one it expects: no fence, no separate flag, one L2 round trip.
 //
-//   Threads [0, ncw*32) compute: thread (cx, ty) owns the 8-site chunk cx (two words) of some rows: in
-//   the boundary phase thread rows 0 / 1 take the CTA's first / last row, then the interior rows are
-//   dealt round-robin over all thread rows.  Threads [ncw*32, ncw*32 + L/16) only receive ("comm").
-//   Eight sites per thread (not four) halves the per-thread bookkeeping and leaves room for >64
-//   registers.  Per half-sweep of colour c:
-//     compute, boundary rows: update, store to shared memory, send packets
-//     compute, interior rows: warps without a boundary row start when the boundary warps are done
-//                             (named barrier 1), so the packets fly while the bulk of the work runs
-//     comm:    poll the inbox for the neighbours' packets of THIS half-sweep and write them into the
-//              halo rows of plane c (which only the next half-sweep reads)
+//   Threads [0, ncw*32) compute: thread (cx, ty) owns the 8-site chunk cx (two words) of the rows dealt to
+//   thread row ty (round-robin, interior rows first, the CTA's first and last row at the very end).
+//   Threads [ncw*32, ncw*32 + L/16) only receive ("comm").  Eight sites per thread (not four) halves the
+//   per-thread bookkeeping and leaves room for >64 registers.  Per half-sweep number s of colour c:
+//     compute: interior rows (they read no halo row), then -- after named barrier 1 -- the two boundary
+//              rows; each boundary chunk goes straight into the neighbour's inbox with tag s
+//     comm:    poll the inbox for the packets tagged s-1 (plane 1-c, sent at the END of the previous
+//              half-sweep), write them into the halo rows of plane 1-c, arrive at named barrier 1
 //     __syncthreads
+//   Boundary rows LAST means the packets have a whole interior phase to cross the chip, and every warp
+//   has work from the first cycle of the half-sweep.
 //
-// Why one inbox slot per (CTA, colour, side) is enough: a sender overwrites a slot two half-sweeps
-// later, after it has received the receiver's packets of the half-sweep in between, and those were
-// sent after the barrier that ends the half-sweep in which the slot was consumed.
-// The global planes are written in the last sweep of the launch only, so every other entry point
+// Why one inbox slot per (CTA, colour, side) is enough: a sender overwrites the slot of colour c two
+// half-sweeps later, after its boundary phase has consumed the receiver's packets of the half-sweep in
+// between, and the receiver sent those after its own comm warps had consumed the slot.
+// The global planes are written at the end of the launch only, so every other entry point
 // (and the next launch) sees the complete state.  Energy and histogram of a sampled sweep are fused:
 // per-thread sums, one block reduction, one atomicAdd per CTA into the series slot.
 //
@@ -116,12 +116,21 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
     const int ty = is_compute ? (int)tid / cpr : 0;
     const int cx = is_compute ? (int)tid - ty * cpr : (is_comm ? ctx : 0);
     const uint32_t col = 8u * (uint32_t)cx;                         // byte offset of my chunk in a plane row
-    const int nb_rows = rows < 2 ? rows : 2;                        // boundary rows: local row 1 and local row `rows`
-    // a warp takes part in the boundary phase iff its first thread owns a boundary row
-    const bool warp_boundary = ((int)(tid & ~31u) / cpr) < (tyc < 2 ? tyc : 2);
-    // interior rows 2..rows-1 are dealt round-robin, starting with the thread rows that had no boundary row
-    const int ishift = tyc >= 3 ? 2 : 0;
-    const int lr_first = 2 + (ty - ishift + tyc) % tyc;
+    // Rows are dealt round-robin over the thread rows, interior rows (local 2..rows-1) first, the two
+    // boundary rows (local 1 and `rows`) last: they are the only ones that read a halo row.
+    const int ni = rows > 2 ? rows - 2 : 0;
+    const int tb0 = ni % tyc, tb1 = (ni + 1) % tyc;                 // thread rows that own local row 1 / local row `rows`
+    const bool two = rows >= 2;
+    // warps that hold a thread of those thread rows wait for the halo (named barrier 1) before the boundary phase
+    const int wid = (int)(tid >> 5);
+    const int w0lo = (tb0 * cpr) >> 5, w0hi = ((tb0 + 1) * cpr - 1) >> 5;
+    const int w1lo = (tb1 * cpr) >> 5, w1hi = ((tb1 + 1) * cpr - 1) >> 5;
+    const bool warp_boundary = (wid >= w0lo && wid <= w0hi) || (two && wid >= w1lo && wid <= w1hi);
+    int nbw = w0hi - w0lo + 1;
+    if (two) {
+        const int lo = w1lo > w0lo ? w1lo : w0lo, hi = w1hi < w0hi ? w1hi : w0hi;
+        nbw += (w1hi - w1lo + 1) - (hi >= lo ? hi - lo + 1 : 0);
+    }
     const bool do_hist = P.hist_series != nullptr && P.every != 0;
     const bool do_E = P.E_series != nullptr && P.every != 0;
 
@@ -156,6 +165,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
     uint2 *const send_dn0 = inbox(dn_cta, 0, 0);     // my last row  -> the row above the first row of the CTA below
     const uint2 *const recv0 = inbox(b, 0, 0);       // colour c: + c * 2 * wpr, side s: + s * wpr
     const uint32_t cstride = 2u * wpr;
+    const int halo_bar = 32 * nbw + ((int)nthreads - nbar);         // boundary warps + comm warps, in threads
 
     uint32_t until = P.every;                                       // sweeps until the next sample
     uint32_t sample_idx = 0;
@@ -196,38 +206,43 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
                     if (count_H) { hist_add_word(s_hist, P.q, out.x, tid & 31u); hist_add_word(s_hist, P.q, out.y, tid & 31u); }
                     return out;
                 };
+                if (is_compute)
+                    for (int lr = 2 + ty; lr < rows; lr += tyc) update(lr);
+                // boundary rows last: by now the neighbours' rows of the previous half-sweep have had a whole
+                // interior phase to arrive
                 if (warp_boundary) {
-                    // boundary rows first: the neighbours wait for them
-                    if (is_compute)
-                        for (int bs = ty; bs < nb_rows; bs += tyc) {
-                            const int lr = bs == 0 ? 1 : rows;
+                    if (G > 1) named_barrier_sync(1, halo_bar);      // comm warps have filled the halo rows of plane 1-c
+#pragma unroll 1
+                    for (int bb = 0; bb < (two ? 2 : 1); ++bb) {
+                        if (is_compute && ty == (bb ? tb1 : tb0)) {
+                            const int lr = bb ? rows : 1;
                             const uint2 out = update(lr);
                             if (G > 1) {
                                 if (lr == 1) st_packet2(send_up0 + c * cstride, out, seq);
                                 if (lr == rows) st_packet2(send_dn0 + c * cstride, out, seq);
                             }
                         }
-                    named_barrier_arrive(1, nbar);
-                } else {
-                    named_barrier_sync(1, nbar);    // interior-only warps start when the boundary rows have been sent
-                }
-                if (is_compute)
-                    for (int lr = lr_first; lr < rows; lr += tyc) update(lr);
-            } else if (is_comm && G > 1) {
-                // receive the neighbours' boundary rows of plane c: halo rows for the NEXT half-sweep
-                uint8_t *const halo = s_raw + c * plane_stride + col;
-#pragma unroll 1
-                for (int s = 0; s < 2; ++s) {
-                    const uint2 *src = recv0 + c * cstride + (uint32_t)s * wpr;
-                    uint4 v = ld_packet2(src);
-                    long long spins = 0;
-                    while (v.y != seq || v.w != seq) {
-                        if (++spins > RESIDENT_SPIN_LIMIT) { atomicExch(P.error, 1); break; }
-                        __nanosleep(40);
-                        v = ld_packet2(src);
                     }
-                    *reinterpret_cast<uint2 *>(halo + (s == 0 ? 0u : (uint32_t)((rows + 1) * pitch))) = make_uint2(v.x, v.z);
                 }
+            } else if (G > 1) {
+                // comm warps: receive the rows the neighbours sent at the end of the PREVIOUS half-sweep (plane 1-c,
+                // tag seq-1) into the halo rows of plane 1-c, which only the boundary phase of this half-sweep reads
+                if (is_comm && seq > 1) {
+                    uint8_t *const halo = s_raw + (1u - c) * plane_stride + col;
+#pragma unroll 1
+                    for (int s = 0; s < 2; ++s) {
+                        const uint2 *src = recv0 + (1u - c) * cstride + (uint32_t)s * wpr;
+                        uint4 v = ld_packet2(src);
+                        long long spins = 0;
+                        while (v.y != seq - 1 || v.w != seq - 1) {
+                            if (++spins > RESIDENT_SPIN_LIMIT) { atomicExch(P.error, 1); break; }
+                            __nanosleep(40);
+                            v = ld_packet2(src);
+                        }
+                        *reinterpret_cast<uint2 *>(halo + (s == 0 ? 0u : (uint32_t)((rows + 1) * pitch))) = make_uint2(v.x, v.z);
+                    }
+                }
+                named_barrier_arrive(1, halo_bar);
             }
             __syncthreads();                                        // plane c complete in shared memory
             if (G == 1) {
