@@ -126,10 +126,22 @@ potts::SweepParams sweep_params(const potts_t *h, uint32_t colour, const uint32_
     return P;
 }
 
-template <bool WIDE, bool MEASURE, bool HIST>
+template <int CM, bool MEASURE, bool HIST>
 void launch_hs(const potts::SweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
 {
-    potts::k_half_sweep_u8<WIDE, MEASURE, HIST><<<grid, dim3(32, potts::HS_WARPS), smem, st>>>(P);
+    potts::k_half_sweep_u8<CM, MEASURE, HIST><<<grid, dim3(32, potts::HS_WARPS), smem, st>>>(P);
+}
+
+template <int CM>
+void launch_hs_cm(const potts::SweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
+{
+    const int sel = (P.E_out ? 2 : 0) | (P.hist_out ? 1 : 0);
+    switch (sel) {
+    case 0: launch_hs<CM, false, false>(P, grid, smem, st); break;
+    case 1: launch_hs<CM, false, true>(P, grid, smem, st); break;
+    case 2: launch_hs<CM, true, false>(P, grid, smem, st); break;
+    default: launch_hs<CM, true, true>(P, grid, smem, st); break;
+    }
 }
 
 int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *E_out,
@@ -144,16 +156,11 @@ int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsign
     P.rpt = rpt;
     const dim3 grid(gx, (unsigned)(h->L / (potts::HS_WARPS * rpt)));
     const size_t smem = hist_out ? (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4 : 0;
-    const int sel = (h->q > 128 ? 4 : 0) | (E_out ? 2 : 0) | (hist_out ? 1 : 0);
-    switch (sel) {
-    case 0: launch_hs<false, false, false>(P, grid, smem, h->stream); break;
-    case 1: launch_hs<false, false, true>(P, grid, smem, h->stream); break;
-    case 2: launch_hs<false, true, false>(P, grid, smem, h->stream); break;
-    case 3: launch_hs<false, true, true>(P, grid, smem, h->stream); break;
-    case 4: launch_hs<true, false, false>(P, grid, smem, h->stream); break;
-    case 5: launch_hs<true, false, true>(P, grid, smem, h->stream); break;
-    case 6: launch_hs<true, true, false>(P, grid, smem, h->stream); break;
-    default: launch_hs<true, true, true>(P, grid, smem, h->stream); break;
+    switch (potts::compare_mode_of(h->q)) {
+    case potts::CM_7BIT: launch_hs_cm<potts::CM_7BIT>(P, grid, smem, h->stream); break;
+    case potts::CM_8BIT: launch_hs_cm<potts::CM_8BIT>(P, grid, smem, h->stream); break;
+    case potts::CM_NIB4: launch_hs_cm<potts::CM_NIB4>(P, grid, smem, h->stream); break;
+    default: launch_hs_cm<potts::CM_NIB3>(P, grid, smem, h->stream); break;
     }
     return check_launch(h, "k_half_sweep_u8");
 }
@@ -299,9 +306,14 @@ int launch_resident(potts_t *h, const ResidentPlan &R, const uint32_t thr[4], in
     P.error = h->error;
     P.rows_max = R.rows_max;
     P.tyc = R.tyc;
-    const bool small = R.nthreads <= 512;
-    const void *fn = h->q > 128 ? (small ? (const void *)potts::k_resident_u8<true, 512> : (const void *)potts::k_resident_u8<true, 1024>)
-                                : (small ? (const void *)potts::k_resident_u8<false, 512> : (const void *)potts::k_resident_u8<false, 1024>);
+    const bool small = R.nthreads <= 512;            // register budget: up to 128 per thread for 512 threads, else 64
+    const void *fn = nullptr;
+    switch (potts::compare_mode_of(h->q)) {
+    case potts::CM_7BIT: fn = small ? (const void *)potts::k_resident_u8<potts::CM_7BIT, 512> : (const void *)potts::k_resident_u8<potts::CM_7BIT, 1024>; break;
+    case potts::CM_8BIT: fn = small ? (const void *)potts::k_resident_u8<potts::CM_8BIT, 512> : (const void *)potts::k_resident_u8<potts::CM_8BIT, 1024>; break;
+    case potts::CM_NIB4: fn = small ? (const void *)potts::k_resident_u8<potts::CM_NIB4, 512> : (const void *)potts::k_resident_u8<potts::CM_NIB4, 1024>; break;
+    default: fn = small ? (const void *)potts::k_resident_u8<potts::CM_NIB3, 512> : (const void *)potts::k_resident_u8<potts::CM_NIB3, 1024>; break;
+    }
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
     int per_sm = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, R.nthreads, R.smem));

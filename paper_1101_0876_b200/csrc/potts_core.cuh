@@ -147,6 +147,40 @@ __device__ __forceinline__ uint32_t ne_count4(uint32_t s, uint32_t up, uint32_t 
            ((ne_flags<WIDE>(s, lf) >> 7) + (ne_flags<WIDE>(s, rt) >> 7));
 }
 
+// Compare modes of update_word: how the per-byte counts of unequal neighbours are formed.
+//   CM_7BIT  q <= 128: one flag word per (spin word, neighbour word) pair, 8 pairs per 4 sites
+//   CM_8BIT  q <= 256: the same with the carry-safe test
+//   CM_NIB4  q <= 16:  the current spin sits in the low nibble and the proposal in the high nibble of one byte,
+//                      the neighbour is doubled into both nibbles (x 0x11): ONE xor and one zero-nibble test give
+//                      the flags of both comparisons, and the shifted sum leaves n_old and n_new in the two nibbles
+//   CM_NIB3  q <= 8:   as CM_NIB4, but a 3-bit difference cannot carry out of its nibble: a shorter zero test
+constexpr int CM_7BIT = 0, CM_8BIT = 1, CM_NIB4 = 2, CM_NIB3 = 3;
+
+__host__ __device__ constexpr int compare_mode_of(int q) { return q > 128 ? CM_8BIT : (q > 16 ? CM_7BIT : (q > 8 ? CM_NIB4 : CM_NIB3)); }
+
+template <int CM>
+__device__ __forceinline__ void ne_counts(uint32_t own, uint32_t prop, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
+                                          uint32_t &c_old, uint32_t &c_new)
+{
+    if (CM == CM_7BIT || CM == CM_8BIT) {
+        c_old = ne_count4<CM == CM_8BIT>(own, up, dn, lf, rt);
+        c_new = ne_count4<CM == CM_8BIT>(prop, up, dn, lf, rt);
+    } else {
+        const uint32_t both = own | (prop << 4);
+        const uint32_t nb[4] = {up, dn, lf, rt};
+        uint32_t s = 0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const uint32_t x = both ^ (nb[k] * 0x11u);
+            const uint32_t f = CM == CM_NIB3 ? (x + 0x77777777u) & 0x88888888u
+                                             : (((x & 0x77777777u) + 0x77777777u) | x) & 0x88888888u;
+            s += f >> 3;
+        }
+        c_old = s & 0x0f0f0f0fu;
+        c_new = (s >> 4) & 0x0f0f0f0fu;
+    }
+}
+
 __device__ __forceinline__ uint32_t byte_sum(uint32_t v)   // sum of the 4 bytes (sum < 256)
 {
     return __dp4a(v, 0x01010101u, 0u);
@@ -183,7 +217,7 @@ __device__ __forceinline__ void horizontal(uint32_t p, uint32_t mid, uint32_t ad
 //   j0           column of byte 0 (columns advance by 2 per byte)
 //   lut          shared memory, 9 words: lut[d+4] = floor(2^32 exp(-d/T)) for d = 1..4 (entries 0..4 unused)
 // Returns the new word; ne_final = per-byte count of unequal neighbours of the final spins.
-template <bool WIDE>
+template <int CM>
 __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
                                                 uint32_t j0, uint32_t q, const HalfSweepKeys &K, const RowKeys &R,
                                                 const uint32_t *lut, uint32_t &ne_final)
@@ -197,8 +231,8 @@ __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint3
     const uint32_t prop = __byte_perm(s01, s23, 0x5410);
 
     // R5: d = n_old - n_new = ne_new - ne_old, biased by 4 so that every byte stays in 0..8
-    const uint32_t c_old = ne_count4<WIDE>(own, up, dn, lf, rt);
-    const uint32_t c_new = ne_count4<WIDE>(prop, up, dn, lf, rt);
+    uint32_t c_old, c_new;
+    ne_counts<CM>(own, prop, up, dn, lf, rt, c_old, c_new);
     const uint32_t dw = c_new + 0x04040404u - c_old;
     // R6: d <= 0 always accepts: byte <= 4  <=>  bit 7 of (0x84 - byte); replicate it over the byte
     uint32_t mask = msb_to_bytemask(0x84848484u - dw);

@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_half_sweep_packed(const __gri
                     const int n = 2 * m + hlf;                        // byte-per-site word n: sites 4n..4n+3
                     uint32_t lf, rt, nef;
                     horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
-                    out[hlf] = update_word<false>(own[hlf], up[hlf], dn[hlf], lf, rt, 2u * (uint32_t)(32 * x + 4 * n) + p, q, K,
+                    out[hlf] = update_word<FIVE ? CM_7BIT : CM_NIB4>(own[hlf], up[hlf], dn[hlf], lf, rt, 2u * (uint32_t)(32 * x + 4 * n) + p, q, K,
                                                   R, lut, nef);
                     if (MEASURE) nef_sum += nef;                      // bytes stay <= 32
                     if (HIST) hist_add_word(s_dyn, P.q, out[hlf], threadIdx.x);

@@ -89,7 +89,7 @@ __device__ __forceinline__ void named_barrier_arrive(int id, int nthreads)
     asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-template <bool WIDE, int MAXT>     // MAXT: block size the registers are budgeted for (512 -> up to 128 registers)
+template <int CM, int MAXT>     // MAXT: block size the registers are budgeted for (512 -> up to 128 registers)
 __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__ ResidentParams P)
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
@@ -199,8 +199,8 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
                     horizontal(p, mid.y, p ? adj : mid.x, lf1, rt1);
                     const RowKeys R = row_keys(K, i);
                     uint2 out;
-                    out.x = update_word<WIDE>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, lut, nef0);
-                    out.y = update_word<WIDE>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, lut, nef1);
+                    out.x = update_word<CM>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, lut, nef0);
+                    out.y = update_word<CM>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, lut, nef1);
                     *reinterpret_cast<uint2 *>(own_col + ro) = out;
                     if (count_E) { nef_sum += nef0 + nef1; words_done += 2; }
                     if (count_H) { hist_add_word(s_hist, P.q, out.x, tid & 31u); hist_add_word(s_hist, P.q, out.y, tid & 31u); }
