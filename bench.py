@@ -357,6 +357,26 @@ def per_config_table(pb, torch, flush, sm_max, hbm_gbs, which, skip=()):
     return out
 
 
+def paper_protocol_e6(pb, torch):
+    """The paper's end-to-end example: q=9, L=1024, 3 samples, T = 0.71 .. 0.73 in steps of 0.002,
+    t_tran = 2000, t_max = 8000, one measure every 50 sweeps; 193 s on a GTX 280, 8115 s on its CPU.  Here: the same
+    protocol through potts_ladder (heating from the ordered state), wall time including the series copy-back."""
+    Ts = [0.71 + 0.002 * k for k in range(11)]
+    t0 = time.perf_counter()
+    e_last = None
+    for sample in range(3):
+        g = pb.Potts(1024, 9, 100 + sample, pb.INIT_ORDERED)
+        E, H = g.potts_ladder(Ts, 2000, 8000, 50, hist=True)
+        e_last = float(E[-1].mean()) / (1024 * 1024)
+        g.close()
+    torch.cuda.synchronize()
+    sec = time.perf_counter() - t0
+    sweeps = 3 * 11 * 10000
+    return {"seconds": sec, "sweeps": sweeps, "spin_updates_per_s": sweeps * 1024 * 1024 / sec,
+            "mean_e_per_spin_at_T0.73_last_sample": e_last,
+            "paper_seconds_gtx280": 193.0, "paper_seconds_cpu": 8115.0, "note": "context only: other hardware and RNG"}
+
+
 # ---- main -----------------------------------------------------------------------------------------
 def main():
     ap = argparse.ArgumentParser()
@@ -427,9 +447,10 @@ def main():
     layout = "packed" if run.layout == pb.LAYOUT_PACKED else "u8"
     run.g.close()
 
-    per_cfg, cpu = None, None
+    per_cfg, cpu, e6 = None, None, None
     if rank == 0 and world == 1 and not args.no_per_config:
         per_cfg = per_config_table(pb, torch, flush, sm_max, hbm_gbs, which)
+        e6 = paper_protocol_e6(pb, torch)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(w)
     if dist is not None:
@@ -450,6 +471,7 @@ def main():
                    "l2": "each step starts from a fresh lattice after a 256 MiB L2 flush; within a step the "
                          "lattice is re-swept in place, so L2 residency for L <= 8192 is the workload's own"},
         "clocks": clk.summary(), "roofline": roof, "e2e": e2e, "cpu_baseline": cpu, "per_config": per_cfg,
+        "paper_protocol_e6": e6,
         "wall_s_timed_region": wall,
         "paper_context": {"ns_per_spin_flip_gtx480": 0.147, "note": "other hardware and RNG; context, not a target"},
     }

@@ -100,6 +100,16 @@ int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every,
 int potts_sweep_measured_dev(potts_t *h, double T, int64_t nsweeps, int64_t every,
                              int64_t *E_series_dev, int64_t *hist_series_dev);
 
+/* potts_ladder: the paper's simulation protocol (sec. 3: "fix T, run t_tran sweeps, then t_max sweeps
+ * with one measure each delta-t steps, keep the last configuration for the next T").  For each temperature T[k]
+ * (host, nT entries, in the order given: ascending = heating, descending = cooling): t_tran unmeasured sweeps,
+ * then t_max sweeps recording E and, if hist_series is non-null, N_0..N_{q-1} after every dt-th.  Configuration
+ * and sweep counter carry over.  E_series (host): nT rows of t_max/dt entries; hist_series (host): nT * t_max/dt
+ * rows of q.  Everything is enqueued at once; one synchronisation at the end.  Same chain as the equivalent
+ * sequence of potts_sweep / potts_sweep_measured calls. */
+int potts_ladder(potts_t *h, const double *T, int32_t nT, int64_t t_tran, int64_t t_max, int64_t dt,
+                 int64_t *E_series, int64_t *hist_series);
+
 /* ---- measurements (sec. 3.4) ---------------------------------------------------
  * potts_energy: E = -(number of satisfied nearest-neighbour bonds), range [-2 L^2, 0].  *E host. */
 int potts_energy(potts_t *h, int64_t *E);

@@ -50,6 +50,7 @@ def load_library() -> ctypes.CDLL:
         "potts_sweep": ([vp, dbl, i64], ctypes.c_int),
         "potts_sweep_measured": ([vp, dbl, i64, i64, vp, vp], ctypes.c_int),
         "potts_sweep_measured_dev": ([vp, dbl, i64, i64, vp, vp], ctypes.c_int),
+        "potts_ladder": ([vp, vp, i32, i64, i64, i64, vp, vp], ctypes.c_int),
         "potts_energy": ([vp, P(i64)], ctypes.c_int),
         "potts_histogram": ([vp, vp], ctypes.c_int),
         "potts_download": ([vp, vp], ctypes.c_int),
@@ -74,7 +75,7 @@ def load_library() -> ctypes.CDLL:
 
 EXPORTED_SYMBOLS = [
     "potts_create", "potts_create_ex", "potts_workspace_bytes", "potts_set_stream", "potts_destroy",
-    "potts_sweep", "potts_sweep_measured", "potts_sweep_measured_dev", "potts_energy", "potts_histogram",
+    "potts_sweep", "potts_sweep_measured", "potts_sweep_measured_dev", "potts_ladder", "potts_energy", "potts_histogram",
     "potts_download", "potts_upload", "potts_sweep_count", "potts_set_sweep_count", "potts_observables",
     "potts_magnetisation", "potts_launch_count", "potts_set_option", "potts_get_option", "potts_last_error",
     "potts_version",
@@ -178,6 +179,17 @@ class Potts:
             self._h, float(T), int(nsweeps), int(every),
             ctypes.c_void_p(E_dev.data_ptr()) if E_dev is not None else None,
             ctypes.c_void_p(hist_dev.data_ptr()) if hist_dev is not None else None))
+
+    def potts_ladder(self, temperatures, t_tran: int, t_max: int, dt: int, hist: bool = True):
+        """-> (E int64[nT, t_max/dt], hist int64[nT, t_max/dt, q] or None) on the host."""
+        self._sync_stream()
+        T = np.ascontiguousarray(temperatures, dtype=np.float64)
+        per = int(t_max) // int(dt) if dt >= 1 and t_max >= 0 else 0
+        E = np.zeros((T.size, per), dtype=np.int64)
+        H = np.zeros((T.size, per, self.q), dtype=np.int64) if hist else None
+        _check(self._lib.potts_ladder(self._h, T.ctypes.data, int(T.size), int(t_tran), int(t_max), int(dt),
+                                      E.ctypes.data, H.ctypes.data if hist else None))
+        return E, H
 
     def potts_energy(self) -> int:
         self._sync_stream()

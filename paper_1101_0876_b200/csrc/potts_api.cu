@@ -551,6 +551,43 @@ int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every, i
     return check_device_error(h);
 }
 
+int potts_ladder(potts_t *h, const double *T, int32_t nT, int64_t t_tran, int64_t t_max, int64_t dt, int64_t *E_series,
+                 int64_t *hist_series)
+{
+    if (!h || !T) return fail(POTTS_ERR_ARG, "null argument");
+    if (nT < 0 || t_tran < 0 || t_max < 0) return fail(POTTS_ERR_ARG, "negative count");
+    if (dt < 1 || t_max % dt != 0)
+        return fail(POTTS_ERR_ARG, "dt = %lld must be >= 1 and divide t_max = %lld", (long long)dt, (long long)t_max);
+    for (int32_t k = 0; k < nT; ++k)
+        if (!(T[k] > 0.0) || !std::isfinite(T[k])) return fail(POTTS_ERR_ARG, "T[%d] = %g must be finite and > 0", k, T[k]);
+    if (h->t + (uint64_t)nT * (uint64_t)(t_tran + t_max) > 0xFFFFFFFFull)
+        return fail(POTTS_ERR_ARG, "sweep counter would pass 2^32 - 1 (Philox counter word)");
+    const int64_t per_T = t_max / dt, ns = per_T * nT;
+    const size_t eb = E_series ? (size_t)ns * 8 : 0, hb = hist_series ? (size_t)ns * h->q * 8 : 0;
+    uint8_t *dev = nullptr;
+    if (eb + hb) {
+        CUDA_TRY(cudaMalloc(&dev, eb + hb));
+        cudaMemsetAsync(dev, 0, eb + hb, h->stream);
+    }
+    unsigned long long *dE = eb ? (unsigned long long *)dev : nullptr;
+    unsigned long long *dH = hb ? (unsigned long long *)(dev + eb) : nullptr;
+    int rc = POTTS_OK;
+    for (int32_t k = 0; k < nT && rc == POTTS_OK; ++k) {
+        rc = run_sweeps(h, T[k], t_tran, 0, nullptr, nullptr);
+        if (rc == POTTS_OK && per_T > 0)
+            rc = run_sweeps(h, T[k], t_max, dt, dE ? dE + k * per_T : nullptr, dH ? dH + k * per_T * h->q : nullptr);
+    }
+    cudaError_t e = cudaSuccess;
+    if (rc == POTTS_OK && eb) e = cudaMemcpyAsync(E_series, dE, eb, cudaMemcpyDeviceToHost, h->stream);
+    if (rc == POTTS_OK && e == cudaSuccess && hb) e = cudaMemcpyAsync(hist_series, dH, hb, cudaMemcpyDeviceToHost, h->stream);
+    const cudaError_t e2 = cudaStreamSynchronize(h->stream);
+    if (dev) cudaFree(dev);
+    if (rc) return rc;
+    if (e != cudaSuccess || e2 != cudaSuccess)
+        return fail(POTTS_ERR_CUDA, "ladder copy/sync failed: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
+    return check_device_error(h);
+}
+
 int potts_energy(potts_t *h, int64_t *E)
 {
     if (!h || !E) return fail(POTTS_ERR_ARG, "null argument");

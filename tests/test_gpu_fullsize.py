@@ -111,3 +111,18 @@ def test_cfg5_full_size_streaming(pb):
     _check_sampled_sites(w, T, t, S0, S1)
     assert int(H1[0].sum()) == w.L * w.L and -2 * w.L * w.L <= int(E1[0]) < 0
     assert int(E1[0]) == g.potts_energy() and (H1[0] == g.potts_histogram()).all()   # fused == standalone reduction
+
+
+@pytest.mark.parametrize("q,want_eo,want_ed", [(9, -1.633167, -1.033499), (15, -1.765905, -0.750492)])
+def test_p9_energies_of_the_coexisting_phases_at_tc(pb, q, want_eo, want_ed):
+    """SURVEY pin P9, the paper's own validation (Table 2 at :213-221): at T_c the ordered branch
+    (heated from the ordered start) sits at e_o and the disordered branch (cooled from a random start) at e_d.
+    Values are Table 2's exact columns (tests/golden/paper_constants.txt); L = 1024 keeps both branches metastable
+    for far longer than the run and finite-size shifts below the tolerance."""
+    L, N = 1024, 1024 * 1024
+    Tc = workloads.t_c(q)
+    for init, want in ((workloads.INIT_ORDERED, want_eo), (workloads.INIT_RANDOM, want_ed)):
+        g = pb.Potts(L, q, 17, init)
+        E, _ = g.potts_ladder([Tc], 6000, 2000, 20, hist=False)
+        e = float(E.mean()) / N
+        assert abs(e - want) < 6e-3, (q, init, e, want)

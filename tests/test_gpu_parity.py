@@ -222,3 +222,25 @@ def test_packed_limits(pb):
             pb.Potts(L, q, 1, layout=pb.LAYOUT_PACKED)
         assert e.value.code == pb.ERR_UNSUPPORTED
     assert pb.potts_workspace_bytes(8192, 24, pb.LAYOUT_PACKED) < 0.7 * pb.potts_workspace_bytes(8192, 24, pb.LAYOUT_U8)
+
+
+def test_ladder_protocol_matches_oracle_and_call_sequence(pb):
+    """T ladder with transient + measured sweeps, state carried over (here: a short cooling ladder)."""
+    L, q, seed = 128, 9, 3
+    Ts = [f * workloads.t_c(q) for f in (1.02, 1.0, 0.98)]
+    g, o = _pair(pb, L, q, seed, workloads.INIT_RANDOM, shape="resident")
+    E, H = g.potts_ladder(Ts, 7, 12, 4, hist=True)
+    assert E.shape == (3, 3) and H.shape == (3, 3, q)
+    g2 = pb.Potts(L, q, seed, workloads.INIT_RANDOM)
+    g2.potts_set_option("variant", 1)
+    for k, T in enumerate(Ts):
+        o.sweep(T, 7)
+        Eo, Ho = o.sweep_measured(T, 12, 4, hist=True)
+        g2.potts_sweep(T, 7)
+        E2, H2 = g2.potts_sweep_measured(T, 12, 4, hist=True)
+        assert (E[k] == Eo).all() and (H[k] == Ho).all() and (E2 == Eo).all() and (H2 == Ho).all()
+    assert (g.potts_download() == o.spins()).all() and g.potts_sweep_count() == o.t == 57
+    with pytest.raises(pb.PottsError):
+        g.potts_ladder(Ts, 1, 10, 3)
+    with pytest.raises(pb.PottsError):
+        g.potts_ladder([0.7, -1.0], 1, 10, 5)
