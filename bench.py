@@ -377,6 +377,25 @@ def paper_protocol_e6(pb, torch):
             "paper_seconds_gtx280": 193.0, "paper_seconds_cpu": 8115.0, "note": "context only: other hardware and RNG"}
 
 
+def batch_of_cfg1(pb, torch, n=1184):
+    """n independent samples of BASELINE configs[0] (q=9, L=64, 1000 sweeps, E + histogram every sweep)
+    advanced together by potts_batch_sweep_measured (one lattice per CTA, 8 per SM); wall time of the call, which
+    includes the copy of the series to the host.  Sample 0 is configs[0] itself (seed 1)."""
+    w = workloads.CONFIGS[1]
+    b = pb.PottsBatch(w.L, w.q, [w.seed + r for r in range(n)], w.init)
+    b.potts_batch_sweep_measured(w.temperatures[0], w.every, w.every)             # warm-up launch
+    b.close()
+    b = pb.PottsBatch(w.L, w.q, [w.seed + r for r in range(n)], w.init)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    E, H = b.potts_batch_sweep_measured(w.temperatures[0], w.sweeps_per_t, w.every)
+    sec = time.perf_counter() - t0
+    b.close()
+    ups = n * w.updates / sec
+    return {"lattices": n, "q": w.q, "L": w.L, "sweeps": w.sweeps_per_t, "seconds": sec, "spin_updates_per_s": ups,
+            "ns_per_spin_flip": 1e9 / ups, "kernel": "k_resident_batch_u8", "E_last_of_sample_0": int(E[0, -1])}
+
+
 # ---- main -----------------------------------------------------------------------------------------
 def main():
     ap = argparse.ArgumentParser()
@@ -451,6 +470,7 @@ def main():
     if rank == 0 and world == 1 and not args.no_per_config:
         per_cfg = per_config_table(pb, torch, flush, sm_max, hbm_gbs, which)
         e6 = paper_protocol_e6(pb, torch)
+        per_cfg["batch_cfg1_x1184"] = batch_of_cfg1(pb, torch)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(w)
     if dist is not None:

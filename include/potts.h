@@ -110,6 +110,26 @@ int potts_sweep_measured_dev(potts_t *h, double T, int64_t nsweeps, int64_t ever
 int potts_ladder(potts_t *h, const double *T, int32_t nT, int64_t t_tran, int64_t t_max, int64_t dt,
                  int64_t *E_series, int64_t *hist_series);
 
+/* ---- replica batch (the paper averages over samples and scans temperatures) --------
+ * n independent lattices of the same (L, q), lattice r with Philox key seeds[r], all advanced by one kernel launch
+ * per call: CTA r keeps lattice r in its shared memory (U8 layout, L % 32 == 0, 2 (L+2) L/2 bytes must fit one CTA:
+ * L <= 448).  Lattice r of a batch follows exactly the chain of a single handle created with (L, q, seeds[r], init).
+ * seeds, T: host arrays of n entries.  dev_workspace: device memory of potts_batch_workspace_bytes() bytes, 256-byte
+ * aligned, or null (the library allocates).  */
+typedef struct potts_batch_s potts_batch_t;
+int potts_batch_workspace_bytes(int32_t n, int32_t L, int32_t q, size_t *bytes);
+int potts_batch_create(potts_batch_t **out, int32_t n, int32_t L, int32_t q, const uint64_t *seeds, int32_t init,
+                       void *dev_workspace, size_t workspace_bytes, void *cuda_stream);
+void potts_batch_destroy(potts_batch_t *b);
+/* nsweeps sweeps of every lattice, lattice r at temperature T[r].  If E_series / hist_series (host; n rows of
+ * nsweeps/every entries / of nsweeps/every x q) are non-null, record after every `every`-th sweep; with both null
+ * `every` is ignored.  Synchronises. */
+int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t every,
+                               int64_t *E_series, int64_t *hist_series);
+int potts_batch_download(potts_batch_t *b, int32_t r, uint8_t *spins); /* lattice r, host, L*L row-major */
+int potts_batch_sweep_count(potts_batch_t *b, uint64_t *t);
+int potts_batch_launch_count(potts_batch_t *b, uint64_t *n);
+
 /* ---- measurements (sec. 3.4) ---------------------------------------------------
  * potts_energy: E = -(number of satisfied nearest-neighbour bonds), range [-2 L^2, 0].  *E host. */
 int potts_energy(potts_t *h, int64_t *E);

@@ -51,6 +51,13 @@ def load_library() -> ctypes.CDLL:
         "potts_sweep_measured": ([vp, dbl, i64, i64, vp, vp], ctypes.c_int),
         "potts_sweep_measured_dev": ([vp, dbl, i64, i64, vp, vp], ctypes.c_int),
         "potts_ladder": ([vp, vp, i32, i64, i64, i64, vp, vp], ctypes.c_int),
+        "potts_batch_workspace_bytes": ([i32, i32, i32, P(ctypes.c_size_t)], ctypes.c_int),
+        "potts_batch_create": ([P(vp), i32, i32, i32, vp, i32, vp, ctypes.c_size_t, vp], ctypes.c_int),
+        "potts_batch_destroy": ([vp], None),
+        "potts_batch_sweep_measured": ([vp, vp, i64, i64, vp, vp], ctypes.c_int),
+        "potts_batch_download": ([vp, i32, vp], ctypes.c_int),
+        "potts_batch_sweep_count": ([vp, P(u64)], ctypes.c_int),
+        "potts_batch_launch_count": ([vp, P(u64)], ctypes.c_int),
         "potts_energy": ([vp, P(i64)], ctypes.c_int),
         "potts_histogram": ([vp, vp], ctypes.c_int),
         "potts_download": ([vp, vp], ctypes.c_int),
@@ -78,7 +85,8 @@ EXPORTED_SYMBOLS = [
     "potts_sweep", "potts_sweep_measured", "potts_sweep_measured_dev", "potts_ladder", "potts_energy", "potts_histogram",
     "potts_download", "potts_upload", "potts_sweep_count", "potts_set_sweep_count", "potts_observables",
     "potts_magnetisation", "potts_launch_count", "potts_set_option", "potts_get_option", "potts_last_error",
-    "potts_version",
+    "potts_version", "potts_batch_workspace_bytes", "potts_batch_create", "potts_batch_destroy",
+    "potts_batch_sweep_measured", "potts_batch_download", "potts_batch_sweep_count", "potts_batch_launch_count",
 ]
 
 
@@ -238,3 +246,67 @@ class Potts:
         v = ctypes.c_int64()
         _check(self._lib.potts_get_option(self._h, key.encode(), ctypes.byref(v)))
         return int(v.value)
+
+
+class PottsBatch:
+    """n independent lattices of the same (L, q) advanced by one launch per call (replica batch)."""
+
+    def __init__(self, L: int, q: int, seeds, init: int = INIT_ORDERED, device: Optional[int] = None):
+        import torch
+
+        self._lib = load_library()
+        if not torch.cuda.is_available():
+            raise PottsError(ERR_CUDA, "no CUDA device: the Potts sweep has no CPU fallback")
+        self._torch = torch
+        self.device = torch.device("cuda", torch.cuda.current_device() if device is None else device)
+        self._seeds = np.ascontiguousarray(seeds, dtype=np.uint64)
+        self.n, self.L, self.q = int(self._seeds.size), int(L), int(q)
+        nb = ctypes.c_size_t(0)
+        _check(self._lib.potts_batch_workspace_bytes(self.n, self.L, self.q, ctypes.byref(nb)))
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nb.value + 256, dtype=torch.uint8, device=self.device)
+            base = self._ws.data_ptr()
+            off = (-base) % 256
+            h = ctypes.c_void_p()
+            stream = ctypes.c_void_p(torch.cuda.current_stream(self.device).cuda_stream)
+            _check(self._lib.potts_batch_create(ctypes.byref(h), self.n, self.L, self.q, self._seeds.ctypes.data, int(init),
+                                                ctypes.c_void_p(base + off), nb.value, stream))
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._torch.cuda.synchronize(self.device)
+            self._lib.potts_batch_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def potts_batch_sweep_measured(self, T, nsweeps: int, every: int = 1, energy: bool = True, hist: bool = True):
+        """T: one temperature per lattice.  -> (E int64[n, ns] or None, hist int64[n, ns, q] or None)."""
+        Ta = np.ascontiguousarray(np.broadcast_to(np.asarray(T, dtype=np.float64), (self.n,)))
+        ns = int(nsweeps) // int(every) if every >= 1 and nsweeps >= 0 else 0
+        E = np.zeros((self.n, ns), dtype=np.int64) if energy else None
+        H = np.zeros((self.n, ns, self.q), dtype=np.int64) if hist else None
+        _check(self._lib.potts_batch_sweep_measured(self._h, Ta.ctypes.data, int(nsweeps), int(every),
+                                                    E.ctypes.data if energy else None, H.ctypes.data if hist else None))
+        return E, H
+
+    def potts_batch_download(self, r: int) -> np.ndarray:
+        out = np.empty((self.L, self.L), dtype=np.uint8)
+        _check(self._lib.potts_batch_download(self._h, int(r), out.ctypes.data))
+        return out
+
+    def potts_batch_sweep_count(self) -> int:
+        t = ctypes.c_uint64()
+        _check(self._lib.potts_batch_sweep_count(self._h, ctypes.byref(t)))
+        return int(t.value)
+
+    def potts_batch_launch_count(self) -> int:
+        n = ctypes.c_uint64()
+        _check(self._lib.potts_batch_launch_count(self._h, ctypes.byref(n)))
+        return int(n.value)

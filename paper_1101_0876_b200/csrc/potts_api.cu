@@ -773,3 +773,241 @@ int potts_magnetisation(const int64_t *counts, int32_t q, double *m)
 }
 
 }  // extern "C"
+
+// ---- replica batch -------------------------------------------------------------------------------
+struct potts_batch_s {
+    int32_t n = 0, L = 0, q = 0;
+    uint64_t t = 0, launches = 0;
+    uint64_t *seeds = nullptr;            // host copy
+    uint8_t *ws = nullptr;
+    bool owns_ws = false;
+    size_t plane_bytes = 0;               // one colour plane of one lattice
+    int *error = nullptr;
+    cudaStream_t stream = nullptr;
+    size_t smem_optin = 0;
+};
+
+namespace {
+
+struct BatchPlan { bool ok = false; int tyc = 0, nthreads = 0; size_t smem = 0; const char *why = ""; };
+
+BatchPlan plan_batch(int32_t L, int32_t q, size_t smem_optin)
+{
+    BatchPlan R;
+    const int cpr = L / 16, comm = (cpr + 31) / 32 * 32;
+    int tyc = (1024 - comm) / cpr;
+    if (tyc > L) tyc = L;
+    R.tyc = tyc;
+    R.nthreads = (cpr * tyc + 31) / 32 * 32 + comm;
+    if ((L + tyc - 1) / tyc > 30) { R.why = "too many rows per thread"; return R; }
+    const size_t hist = (size_t)(q <= (int)potts::HIST_LANE_QMAX ? q * 32 : q) * 4;
+    R.smem = 2 * (size_t)(L + 2) * (L / 2) + hist;
+    if (R.smem + 1024 > smem_optin) { R.why = "one lattice does not fit the shared memory of a CTA"; return R; }
+    R.ok = true;
+    return R;
+}
+
+size_t batch_bytes_of(int32_t n, int32_t L) { return (size_t)n * 2 * align_up((size_t)L * (L / 2)) + ALIGN; }
+
+int check_batch_shape(int32_t n, int32_t L, int32_t q)
+{
+    if (n < 1) return fail(POTTS_ERR_ARG, "n = %d lattices", n);
+    int rc = check_shape(L, q, POTTS_LAYOUT_U8);
+    if (rc) return rc;
+    if (2 * (size_t)(L + 2) * (L / 2) > 200 * 1024) return fail(POTTS_ERR_UNSUPPORTED, "L = %d does not fit one CTA's shared memory", L);
+    return POTTS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int potts_batch_workspace_bytes(int32_t n, int32_t L, int32_t q, size_t *bytes)
+{
+    if (!bytes) return fail(POTTS_ERR_ARG, "null bytes pointer");
+    int rc = check_batch_shape(n, L, q);
+    if (rc) return rc;
+    *bytes = batch_bytes_of(n, L);
+    return POTTS_OK;
+}
+
+int potts_batch_create(potts_batch_t **out, int32_t n, int32_t L, int32_t q, const uint64_t *seeds, int32_t init,
+                       void *dev_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!out || !seeds) return fail(POTTS_ERR_ARG, "null argument");
+    if (init != POTTS_INIT_ORDERED && init != POTTS_INIT_RANDOM) return fail(POTTS_ERR_ARG, "bad init %d", init);
+    int rc = check_batch_shape(n, L, q);
+    if (rc) return rc;
+    const size_t need = batch_bytes_of(n, L);
+    if (dev_workspace && workspace_bytes < need) return fail(POTTS_ERR_NOMEM, "workspace of %zu bytes < %zu needed", workspace_bytes, need);
+    if (dev_workspace && (uintptr_t)dev_workspace % ALIGN) return fail(POTTS_ERR_ARG, "workspace not %zu-byte aligned", ALIGN);
+    int ndev = 0;
+    CUDA_TRY(cudaGetDeviceCount(&ndev));
+    if (ndev < 1) return fail(POTTS_ERR_CUDA, "no CUDA device");
+    potts_batch_t *b = new (std::nothrow) potts_batch_s;
+    if (!b) return fail(POTTS_ERR_NOMEM, "host allocation failed");
+    b->n = n; b->L = L; b->q = q;
+    b->stream = (cudaStream_t)cuda_stream;
+    b->seeds = new (std::nothrow) uint64_t[n];
+    if (!b->seeds) { delete b; return fail(POTTS_ERR_NOMEM, "host allocation failed"); }
+    std::memcpy(b->seeds, seeds, sizeof(uint64_t) * n);
+    if (dev_workspace) b->ws = (uint8_t *)dev_workspace;
+    else {
+        cudaError_t e = cudaMalloc(&b->ws, need);
+        if (e != cudaSuccess) {
+            delete[] b->seeds; delete b;
+            return fail(POTTS_ERR_NOMEM, "cudaMalloc(%zu) failed: %s", need, cudaGetErrorString(e));
+        }
+        b->owns_ws = true;
+    }
+    b->plane_bytes = align_up((size_t)L * (L / 2));
+    b->error = (int *)(b->ws + (size_t)n * 2 * b->plane_bytes);
+    {
+        int dev = 0, v = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        b->smem_optin = (size_t)v;
+    }
+    const BatchPlan R = plan_batch(L, q, b->smem_optin);
+    if (!R.ok) { potts_batch_destroy(b); return fail(POTTS_ERR_UNSUPPORTED, "batch: %s", R.why); }
+    cudaError_t e = cudaMemsetAsync(b->ws, 0, need, b->stream);
+    if (e == cudaSuccess && init == POTTS_INIT_RANDOM) {
+        const long long words = 2ll * L * (L / 8);
+        for (int r = 0; r < n; ++r) {
+            uint8_t *p0 = b->ws + (size_t)r * 2 * b->plane_bytes;
+            potts::k_init_random_u8<<<(unsigned)((words + 255) / 256), 256, 0, b->stream>>>(
+                p0, p0 + b->plane_bytes, L, L / 2, (uint32_t)q, (uint32_t)(seeds[r] & 0xFFFFFFFFull), (uint32_t)(seeds[r] >> 32));
+        }
+        b->launches += n;
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) { potts_batch_destroy(b); return fail(POTTS_ERR_CUDA, "batch initialisation failed: %s", cudaGetErrorString(e)); }
+    *out = b;
+    return POTTS_OK;
+}
+
+void potts_batch_destroy(potts_batch_t *b)
+{
+    if (!b) return;
+    if (b->owns_ws && b->ws) { cudaStreamSynchronize(b->stream); cudaFree(b->ws); }
+    delete[] b->seeds;
+    delete b;
+}
+
+int potts_batch_sweep_count(potts_batch_t *b, uint64_t *t)
+{
+    if (!b || !t) return fail(POTTS_ERR_ARG, "null argument");
+    *t = b->t;
+    return POTTS_OK;
+}
+
+int potts_batch_launch_count(potts_batch_t *b, uint64_t *n)
+{
+    if (!b || !n) return fail(POTTS_ERR_ARG, "null argument");
+    *n = b->launches;
+    return POTTS_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+template <int CM>
+cudaError_t launch_batch_cm(const potts::BatchParams &B, const potts::BatchTable &T, int n, int nthreads, size_t smem, cudaStream_t st)
+{
+    auto fn = potts::k_resident_batch_u8<CM, 1024>;          // 64 registers: several small lattices per SM
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    fn<<<(unsigned)n, (unsigned)nthreads, smem, st>>>(B, T);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+extern "C" {
+
+int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t every, int64_t *E_series,
+                               int64_t *hist_series)
+{
+    if (!b || !T) return fail(POTTS_ERR_ARG, "null argument");
+    if (nsweeps < 0 || nsweeps > (1ll << 30)) return fail(POTTS_ERR_ARG, "nsweeps = %lld outside [0, 2^30]", (long long)nsweeps);
+    for (int r = 0; r < b->n; ++r)
+        if (!(T[r] > 0.0) || !std::isfinite(T[r])) return fail(POTTS_ERR_ARG, "T[%d] = %g must be finite and > 0", r, T[r]);
+    if (b->t + (uint64_t)nsweeps > 0xFFFFFFFFull) return fail(POTTS_ERR_ARG, "sweep counter would pass 2^32 - 1");
+    const bool measure = E_series || hist_series;
+    if (measure && (every < 1 || nsweeps % every != 0))
+        return fail(POTTS_ERR_ARG, "every = %lld must be >= 1 and divide nsweeps = %lld", (long long)every, (long long)nsweeps);
+    if (nsweeps == 0) return POTTS_OK;
+    const int64_t ns = measure ? nsweeps / every : 0;
+    const size_t eb = E_series ? (size_t)b->n * ns * 8 : 0, hb = hist_series ? (size_t)b->n * ns * b->q * 8 : 0;
+    uint8_t *dev = nullptr;
+    if (eb + hb) {
+        CUDA_TRY(cudaMalloc(&dev, eb + hb));
+        cudaMemsetAsync(dev, 0, eb + hb, b->stream);
+    }
+    const BatchPlan R = plan_batch(b->L, b->q, b->smem_optin);
+    static thread_local potts::BatchTable tab;               // 24 KB: copied into the launch parameters
+    cudaError_t e = cudaSuccess;
+    for (int r0 = 0; r0 < b->n && e == cudaSuccess; r0 += potts::BATCH_MAX) {
+        const int m = b->n - r0 < potts::BATCH_MAX ? b->n - r0 : potts::BATCH_MAX;
+        for (int r = 0; r < m; ++r) {
+            tab.key[r][0] = (uint32_t)(b->seeds[r0 + r] & 0xFFFFFFFFull);
+            tab.key[r][1] = (uint32_t)(b->seeds[r0 + r] >> 32);
+            thresholds(T[r0 + r], tab.thr[r]);
+        }
+        potts::BatchParams B = {};
+        potts::ResidentParams &P = B.P;
+        P.plane[0] = b->ws + (size_t)r0 * 2 * b->plane_bytes;
+        P.plane[1] = P.plane[0] + b->plane_bytes;
+        P.L = b->L;
+        P.pitch = b->L / 2;
+        P.q = (uint32_t)b->q;
+        P.t0 = (uint32_t)b->t;
+        P.nsweeps = (uint32_t)nsweeps;
+        P.every = measure ? (uint32_t)every : 0u;
+        P.E_series = eb ? (unsigned long long *)dev + (size_t)r0 * ns : nullptr;
+        P.hist_series = hb ? (unsigned long long *)(dev + eb) + (size_t)r0 * ns * b->q : nullptr;
+        P.inbox = nullptr;
+        P.error = b->error;
+        P.rows_max = b->L;
+        P.tyc = R.tyc;
+        B.lattice_stride = 2ull * b->plane_bytes;
+        B.series_stride = (unsigned long long)ns;
+        switch (potts::compare_mode_of(b->q)) {
+        case potts::CM_7BIT: e = launch_batch_cm<potts::CM_7BIT>(B, tab, m, R.nthreads, R.smem, b->stream); break;
+        case potts::CM_8BIT: e = launch_batch_cm<potts::CM_8BIT>(B, tab, m, R.nthreads, R.smem, b->stream); break;
+        case potts::CM_NIB4: e = launch_batch_cm<potts::CM_NIB4>(B, tab, m, R.nthreads, R.smem, b->stream); break;
+        default: e = launch_batch_cm<potts::CM_NIB3>(B, tab, m, R.nthreads, R.smem, b->stream); break;
+        }
+        b->launches += 1;
+    }
+    if (e == cudaSuccess) b->t += (uint64_t)nsweeps;
+    if (e == cudaSuccess && eb) e = cudaMemcpyAsync(E_series, dev, eb, cudaMemcpyDeviceToHost, b->stream);
+    if (e == cudaSuccess && hb) e = cudaMemcpyAsync(hist_series, dev + eb, hb, cudaMemcpyDeviceToHost, b->stream);
+    const cudaError_t e2 = cudaStreamSynchronize(b->stream);
+    if (dev) cudaFree(dev);
+    if (e != cudaSuccess || e2 != cudaSuccess)
+        return fail(POTTS_ERR_CUDA, "batch sweep failed: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
+    return POTTS_OK;
+}
+
+int potts_batch_download(potts_batch_t *b, int32_t r, uint8_t *spins)
+{
+    if (!b || !spins) return fail(POTTS_ERR_ARG, "null argument");
+    if (r < 0 || r >= b->n) return fail(POTTS_ERR_ARG, "lattice index %d outside [0, %d)", r, b->n);
+    const int L = b->L;
+    uint8_t *stage = nullptr;
+    CUDA_TRY(cudaMalloc(&stage, (size_t)L * L));
+    uint8_t *p0 = b->ws + (size_t)r * 2 * b->plane_bytes;
+    const long long threads = (long long)L * (L / 8);
+    potts::k_planes_to_rowmajor<<<(unsigned)((threads + 255) / 256), 256, 0, b->stream>>>(p0, p0 + b->plane_bytes, stage, L, L / 2, 0, L);
+    b->launches += 1;
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(spins, stage, (size_t)L * L, cudaMemcpyDeviceToHost, b->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(b->stream);
+    cudaFree(stage);
+    if (e != cudaSuccess) return fail(POTTS_ERR_CUDA, "batch download failed: %s", cudaGetErrorString(e));
+    return POTTS_OK;
+}
+
+}  // extern "C"

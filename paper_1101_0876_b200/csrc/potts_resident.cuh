@@ -89,14 +89,23 @@ __device__ __forceinline__ void named_barrier_arrive(int id, int nthreads)
     asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-template <int CM, int MAXT>     // MAXT: block size the registers are budgeted for (512 -> up to 128 registers)
-__global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__ ResidentParams P)
+// What differs between one lattice split over the grid and a batch of independent lattices, one per CTA
+struct ResidentLattice {
+    uint32_t G, b;                    // CTAs sharing this lattice, my index among them
+    uint8_t *plane[2];
+    uint32_t key0, key1;
+    uint32_t thr[4];
+    unsigned long long *E_series, *hist_series;
+};
+
+template <int CM>
+__device__ __forceinline__ void resident_run(const ResidentParams &P, const ResidentLattice &X)
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
     __shared__ uint32_t lut[12];
     __shared__ uint32_t blockE;
 
-    const uint32_t G = gridDim.x, b = blockIdx.x;
+    const uint32_t G = X.G, b = X.b;
     const int L = P.L, pitch = P.pitch;
     const int r0 = (int)(((long long)b * L) / G), r1 = (int)(((long long)(b + 1) * L) / G);
     const int rows = r1 - r0;
@@ -131,10 +140,10 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
         const int lo = w1lo > w0lo ? w1lo : w0lo, hi = w1hi < w0hi ? w1hi : w0hi;
         nbw += (w1hi - w1lo + 1) - (hi >= lo ? hi - lo + 1 : 0);
     }
-    const bool do_hist = P.hist_series != nullptr && P.every != 0;
-    const bool do_E = P.E_series != nullptr && P.every != 0;
+    const bool do_hist = X.hist_series != nullptr && P.every != 0;
+    const bool do_E = X.E_series != nullptr && P.every != 0;
 
-    if (tid < 9) lut[tid] = tid >= 5 ? P.thr[tid - 5] : 0u;
+    if (tid >= 5 && tid < 9) lut[tid] = tid == 5 ? X.thr[0] : (tid == 6 ? X.thr[1] : (tid == 7 ? X.thr[2] : X.thr[3]));
     if (tid == 0) blockE = 0u;
     if (do_hist)
         for (uint32_t n = tid; n < hist_words(P.q); n += nthreads) s_hist[n] = 0u;
@@ -148,7 +157,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
                 if (c == 0 && (lr == 0 || lr == rows + 1)) continue;
                 const int gr = wrap(r0 + lr - 1, L);
                 *reinterpret_cast<uint4 *>(s_raw + c * plane_stride + (uint32_t)(lr * pitch + 16 * v)) =
-                    __ldcg(reinterpret_cast<const uint4 *>(P.plane[c] + (size_t)gr * pitch + 16 * v));
+                    __ldcg(reinterpret_cast<const uint4 *>(X.plane[c] + (size_t)gr * pitch + 16 * v));
             }
     }
     __syncthreads();
@@ -182,7 +191,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
             uint32_t nef_sum = 0, words_done = 0;
             const bool count_E = sample && c == 1 && do_E, count_H = sample && do_hist;
             if ((int)tid < nbar) {
-                const HalfSweepKeys K = half_sweep_keys(P.key0, P.key1, t, c);             // uniform registers
+                const HalfSweepKeys K = half_sweep_keys(X.key0, X.key1, t, c);             // uniform registers
                 // one chunk: local row lr, words 2cx and 2cx+1
                 auto update = [&](int lr) -> uint2 {
                     const uint32_t ro = (uint32_t)(lr * pitch);
@@ -265,11 +274,11 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
                     if ((tid & 31u) == 0 && satisfied) atomicAdd(&blockE, satisfied);
                     __syncthreads();
                     if (tid == 0) {
-                        atomicAdd(P.E_series + sample_idx, 0ull - (unsigned long long)blockE);
+                        atomicAdd(X.E_series + sample_idx, 0ull - (unsigned long long)blockE);
                         blockE = 0u;
                     }
                 }
-                if (do_hist) hist_flush(s_hist, P.q, P.hist_series + (size_t)sample_idx * P.q, tid, nthreads);
+                if (do_hist) hist_flush(s_hist, P.q, X.hist_series + (size_t)sample_idx * P.q, tid, nthreads);
                 ++sample_idx;
                 __syncthreads();
             }
@@ -281,10 +290,63 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
         for (int c = 0; c < 2; ++c)
             for (int n = (int)tid; n < rows * vpr; n += (int)nthreads) {
                 const int lr = n / vpr, v = n - lr * vpr;
-                *reinterpret_cast<uint4 *>(P.plane[c] + (size_t)(r0 + lr) * pitch + 16 * v) =
+                *reinterpret_cast<uint4 *>(X.plane[c] + (size_t)(r0 + lr) * pitch + 16 * v) =
                     *reinterpret_cast<const uint4 *>(s_raw + c * plane_stride + (uint32_t)((lr + 1) * pitch + 16 * v));
             }
     }
+}
+
+// One lattice over the whole grid (cooperative launch: the CTAs wait for each other's packets).
+template <int CM, int MAXT>     // MAXT: block size the registers are budgeted for (512 -> up to 128 registers)
+__global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__ ResidentParams P)
+{
+    ResidentLattice X;
+    X.G = gridDim.x;
+    X.b = blockIdx.x;
+    X.plane[0] = P.plane[0];
+    X.plane[1] = P.plane[1];
+    X.key0 = P.key0;
+    X.key1 = P.key1;
+#pragma unroll
+    for (int d = 0; d < 4; ++d) X.thr[d] = P.thr[d];
+    X.E_series = P.E_series;
+    X.hist_series = P.hist_series;
+    resident_run<CM>(P, X);
+}
+
+// Replica batch: CTA r runs lattice r of a batch of independent lattices of the same (L, q), each with
+// its own seed and temperature, entirely in its shared memory: no packets, no co-residency requirement, any grid
+// size.  Small lattices (the paper's L <= 256 studies with hundreds of samples) fill the GPU this
+// way.  Seeds and thresholds travel in the launch parameters, so they stay in uniform registers.
+constexpr int BATCH_MAX = 1024;       // lattices per launch (24 KB of launch parameters)
+
+struct BatchTable {
+    uint32_t key[BATCH_MAX][2];
+    uint32_t thr[BATCH_MAX][4];
+};
+
+struct BatchParams {
+    ResidentParams P;                 // plane[], E_series, hist_series: those of lattice 0; inbox unused
+    unsigned long long lattice_stride;   // bytes from one lattice's planes to the next one's
+    unsigned long long series_stride;    // samples per lattice in E_series (hist_series: x q)
+};
+
+template <int CM, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) k_resident_batch_u8(const __grid_constant__ BatchParams B, const __grid_constant__ BatchTable T)
+{
+    const uint32_t r = blockIdx.x;
+    ResidentLattice X;
+    X.G = 1u;
+    X.b = 0u;
+    X.plane[0] = B.P.plane[0] + r * B.lattice_stride;
+    X.plane[1] = B.P.plane[1] + r * B.lattice_stride;
+    X.key0 = T.key[r][0];
+    X.key1 = T.key[r][1];
+#pragma unroll
+    for (int d = 0; d < 4; ++d) X.thr[d] = T.thr[r][d];
+    X.E_series = B.P.E_series ? B.P.E_series + r * B.series_stride : nullptr;
+    X.hist_series = B.P.hist_series ? B.P.hist_series + r * B.series_stride * B.P.q : nullptr;
+    resident_run<CM>(B.P, X);
 }
 
 }  // namespace potts

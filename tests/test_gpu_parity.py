@@ -244,3 +244,35 @@ def test_ladder_protocol_matches_oracle_and_call_sequence(pb):
         g.potts_ladder(Ts, 1, 10, 3)
     with pytest.raises(pb.PottsError):
         g.potts_ladder([0.7, -1.0], 1, 10, 5)
+
+
+# ---- replica batch: lattice r of a batch == a single handle with (seed_r, T_r) ---------------------------
+@pytest.mark.parametrize("L,q,n", [(64, 9, 5), (32, 2, 3), (128, 24, 4), (96, 200, 2), (256, 6, 3)])
+def test_batch_replicas_match_oracle(pb, L, q, n):
+    seeds = [1000 + 7 * r + (r << 40) for r in range(n)]
+    Ts = [(0.9 + 0.1 * r) * workloads.t_c(q) for r in range(n)]
+    b = pb.PottsBatch(L, q, seeds, workloads.INIT_RANDOM)
+    E, H = b.potts_batch_sweep_measured(Ts, 12, 3)
+    E2, _ = b.potts_batch_sweep_measured(Ts, 5, 1, hist=False)          # the counter carries over
+    assert b.potts_batch_sweep_count() == 17
+    for r in range(n):
+        o = oracle.OraclePotts(L, q, seeds[r], workloads.INIT_RANDOM)
+        Eo, Ho = o.sweep_measured(Ts[r], 12, 3, hist=True)
+        assert (E[r] == Eo).all() and (H[r] == Ho).all(), r
+        Eo2, _ = o.sweep_measured(Ts[r], 5, 1, hist=False)
+        assert (E2[r] == Eo2).all() and (b.potts_batch_download(r) == o.spins()).all(), r
+
+
+def test_batch_larger_than_one_launch_and_ordered_start(pb):
+    L, q, n = 32, 6, 1030                                              # > 1024 lattices: two launches per call
+    seeds = list(range(5, 5 + n))
+    T = 1.005 * workloads.t_c(q)
+    b = pb.PottsBatch(L, q, seeds, workloads.INIT_ORDERED)
+    E, _ = b.potts_batch_sweep_measured(T, 6, 2, hist=False)
+    assert b.potts_batch_launch_count() == 2
+    for r in (0, 1, 511, 1023, 1024, 1029):
+        o = oracle.OraclePotts(L, q, seeds[r], workloads.INIT_ORDERED)
+        Eo, _ = o.sweep_measured(T, 6, 2, hist=False)
+        assert (E[r] == Eo).all() and (b.potts_batch_download(r) == o.spins()).all(), r
+    with pytest.raises(pb.PottsError):
+        pb.PottsBatch(512, 6, [1, 2])                                  # does not fit one CTA
