@@ -59,6 +59,7 @@ struct potts_s {
     uint64_t launches = 0;
     int num_sms = 0;
     size_t smem_optin = 0;
+    int coop = 0;                        // device supports cooperative launches (the resident kernel needs one)
     // options (how to launch, never what is computed)
     int64_t opt_variant = 0;             // 0 auto, 1 streaming (one launch per half-sweep), 2 resident
     int64_t opt_resident_ctas = 0;       // 0 auto, else the resident kernel's grid size
@@ -260,6 +261,7 @@ ResidentPlan plan_resident(const potts_t *h)
     const int L = h->L;
     R.wpr = L / 8;
     if (h->layout != POTTS_LAYOUT_U8) { R.why = "the resident kernel holds the U8 layout only"; return R; }
+    if (!h->coop) { R.why = "the device does not support cooperative launches"; return R; }
     if (L > RESIDENT_L_MAX || !h->inbox) { R.why = "L exceeds the resident kernel's 512 words per row"; return R; }
     const long long words = (long long)L * R.wpr;                   // 4-site words per half-sweep
     long long G = h->opt_resident_ctas > 0 ? h->opt_resident_ctas : words / 128;   // measured: more CTAs win down to ~4 rows each
@@ -448,6 +450,8 @@ int potts_create_ex(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t 
         h->num_sms = v;
         cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
         h->smem_optin = (size_t)v;
+        cudaDeviceGetAttribute(&v, cudaDevAttrCooperativeLaunch, dev);
+        h->coop = v;
         cudaMemsetAsync(h->acc, 0, ACC_WORDS * sizeof(unsigned long long), h->stream);
     }
 

@@ -54,18 +54,6 @@ struct ResidentParams {
 
 constexpr long long RESIDENT_SPIN_LIMIT = 1ll << 24;   // polls before a wait gives up (seconds)
 
-__device__ __forceinline__ uint2 ld_packet(const uint2 *p)
-{
-    uint2 v;
-    asm volatile("ld.relaxed.gpu.global.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p) : "memory");
-    return v;
-}
-
-__device__ __forceinline__ void st_packet(uint2 *p, uint32_t data, uint32_t seq)
-{
-    asm volatile("st.relaxed.gpu.global.v2.u32 [%0], {%1, %2};" ::"l"(p), "r"(data), "r"(seq) : "memory");
-}
-
 // two packets (an 8-site chunk) at once; each 8-byte half is still atomic on its own
 __device__ __forceinline__ uint4 ld_packet2(const uint2 *p)
 {
