@@ -169,6 +169,7 @@ int potts_launch_count(potts_t *h, uint64_t *n);
  *                      L2/HBM), 2 = resident (one persistent cooperative launch per call, lattice in shared
  *                      memory; U8 layout, L <= 4096; POTTS_ERR_UNSUPPORTED from the sweep call otherwise)
  *   "resident_ctas"    0 = automatic, else the number of CTAs the resident kernel splits the rows over
+ *   "resident_words"   0 = automatic, 1 / 2 = 4-site words a resident thread updates per row visit
  *   "resident_active"  read-only: CTAs the next sweep call would run resident on (0 = streaming) */
 int potts_set_option(potts_t *h, const char *key, int64_t value);
 int potts_get_option(potts_t *h, const char *key, int64_t *value);

@@ -63,6 +63,7 @@ struct potts_s {
     // options (how to launch, never what is computed)
     int64_t opt_variant = 0;             // 0 auto, 1 streaming (one launch per half-sweep), 2 resident
     int64_t opt_resident_ctas = 0;       // 0 auto, else the resident kernel's grid size
+    int64_t opt_resident_words = 0;      // 0 auto, 1 / 2: 4-site words per thread and row visit
 };
 
 namespace {
@@ -250,7 +251,7 @@ int check_sweep_args(potts_t *h, double T, int64_t nsweeps)
 // ---- resident (persistent, shared-memory) path ------------------------------------------------
 struct ResidentPlan {
     bool ok = false;
-    int G = 0, tyc = 0, wpr = 0, rows_max = 0, nthreads = 0;
+    int G = 0, tyc = 0, wpr = 0, rows_max = 0, nthreads = 0, W = 2;
     size_t smem = 0;
     const char *why = "";
 };
@@ -277,14 +278,48 @@ ResidentPlan plan_resident(const potts_t *h)
     int tyc = (1024 - comm) / cpr;
     if (tyc > R.rows_max) tyc = R.rows_max;
     if (tyc < 1) { R.why = "no room for a compute row in a 1024-thread block"; return R; }
+    int threads_per_row = cpr;
+    // One 4-site word per thread and row visit (W = 1) instead of an 8-site chunk (W = 2) wherever every thread still
+    // visits at most two rows inside a 576-thread block (112 registers): twice the warps for the latency-bound small
+    // lattices, and at L = 1024 on 148 SMs an even load on the four sub-partitions of an SM (7 rows as chunks are
+    // 14 warps -> 4,4,3,3; as words over 4 thread rows of 4 warps each: three thread rows with 2 rows, one with 1).
+    // Measured (profiles/r01c_kernels.md): 4 % faster at L = 1024, 20 - 40 % at L <= 512.  Larger lattices keep W = 2.
+    {
+        int t1 = (576 - comm) / (2 * cpr);
+        if (t1 > R.rows_max) t1 = R.rows_max;
+        const bool fits = t1 >= 1 && t1 >= (R.rows_max + 1) / 2;
+        if (h->opt_resident_words == 1 ? (t1 >= 1) : (h->opt_resident_words == 0 && fits)) {
+            R.W = 1;
+            threads_per_row = 2 * cpr;
+            tyc = t1;
+        }
+    }
     R.tyc = tyc;
-    R.nthreads = (cpr * tyc + 31) / 32 * 32 + comm;
+    R.nthreads = (threads_per_row * tyc + 31) / 32 * 32 + comm;
     if ((R.rows_max + tyc - 1) / tyc > 30) { R.why = "too many rows per thread"; return R; }
     const size_t hist = (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4;
     R.smem = 2 * (size_t)(R.rows_max + 2) * (L / 2) + hist;
     if (R.smem + 1024 > h->smem_optin) { R.why = "lattice does not fit the shared memory of the grid"; return R; }
     R.ok = true;
     return R;
+}
+
+// register budget: 112 per thread for blocks up to 576 threads, else 64
+template <int CM>
+const void *resident_kernel_cm(int W, bool small)
+{
+    if (W == 1) return small ? (const void *)potts::k_resident_u8<CM, 1, 576> : (const void *)potts::k_resident_u8<CM, 1, 1024>;
+    return small ? (const void *)potts::k_resident_u8<CM, 2, 576> : (const void *)potts::k_resident_u8<CM, 2, 1024>;
+}
+
+const void *resident_kernel(int cm, int W, bool small)
+{
+    switch (cm) {
+    case potts::CM_7BIT: return resident_kernel_cm<potts::CM_7BIT>(W, small);
+    case potts::CM_8BIT: return resident_kernel_cm<potts::CM_8BIT>(W, small);
+    case potts::CM_NIB4: return resident_kernel_cm<potts::CM_NIB4>(W, small);
+    default: return resident_kernel_cm<potts::CM_NIB3>(W, small);
+    }
 }
 
 int launch_resident(potts_t *h, const ResidentPlan &R, const uint32_t thr[4], int64_t nsweeps, int64_t every,
@@ -308,14 +343,7 @@ int launch_resident(potts_t *h, const ResidentPlan &R, const uint32_t thr[4], in
     P.error = h->error;
     P.rows_max = R.rows_max;
     P.tyc = R.tyc;
-    const bool small = R.nthreads <= 512;            // register budget: up to 128 per thread for 512 threads, else 64
-    const void *fn = nullptr;
-    switch (potts::compare_mode_of(h->q)) {
-    case potts::CM_7BIT: fn = small ? (const void *)potts::k_resident_u8<potts::CM_7BIT, 512> : (const void *)potts::k_resident_u8<potts::CM_7BIT, 1024>; break;
-    case potts::CM_8BIT: fn = small ? (const void *)potts::k_resident_u8<potts::CM_8BIT, 512> : (const void *)potts::k_resident_u8<potts::CM_8BIT, 1024>; break;
-    case potts::CM_NIB4: fn = small ? (const void *)potts::k_resident_u8<potts::CM_NIB4, 512> : (const void *)potts::k_resident_u8<potts::CM_NIB4, 1024>; break;
-    default: fn = small ? (const void *)potts::k_resident_u8<potts::CM_NIB3, 512> : (const void *)potts::k_resident_u8<potts::CM_NIB3, 1024>; break;
-    }
+    const void *fn = resident_kernel(potts::compare_mode_of(h->q), R.W, R.nthreads <= 576);
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
     int per_sm = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, R.nthreads, R.smem));
@@ -717,6 +745,10 @@ int potts_set_option(potts_t *h, const char *key, int64_t value)
         if (value < 0 || value > MAX_CTAS) return fail(POTTS_ERR_ARG, "resident_ctas must be in [0, %d]", MAX_CTAS);
         h->opt_resident_ctas = value; return POTTS_OK;
     }
+    if (!std::strcmp(key, "resident_words")) {
+        if (value < 0 || value > 2) return fail(POTTS_ERR_ARG, "resident_words must be 0 (auto), 1 or 2");
+        h->opt_resident_words = value; return POTTS_OK;
+    }
     return fail(POTTS_ERR_ARG, "unknown option '%s'", key);
 }
 
@@ -725,6 +757,7 @@ int potts_get_option(potts_t *h, const char *key, int64_t *value)
     if (!h || !key || !value) return fail(POTTS_ERR_ARG, "null argument");
     if (!std::strcmp(key, "variant")) { *value = h->opt_variant; return POTTS_OK; }
     if (!std::strcmp(key, "resident_ctas")) { *value = h->opt_resident_ctas; return POTTS_OK; }
+    if (!std::strcmp(key, "resident_words")) { *value = h->opt_resident_words; return POTTS_OK; }
     if (!std::strcmp(key, "resident_active")) {            // read-only: would the next sweep call run resident?
         *value = (h->opt_variant != 1 && plan_resident(h).ok) ? plan_resident(h).G : 0; return POTTS_OK;
     }

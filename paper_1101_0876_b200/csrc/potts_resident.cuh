@@ -67,6 +67,13 @@ __device__ __forceinline__ void st_packet2(uint2 *p, uint2 data, uint32_t seq)
     asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %2};" ::"l"(p), "r"(data.x), "r"(seq), "r"(data.y) : "memory");
 }
 
+template <int W>
+__device__ __forceinline__ void st_packets(uint2 *p, uint2 data, uint32_t seq)
+{
+    if (W == 2) st_packet2(p, data, seq);
+    else asm volatile("st.relaxed.gpu.global.v2.u32 [%0], {%1, %2};" ::"l"(p), "r"(data.x), "r"(seq) : "memory");
+}
+
 __device__ __forceinline__ void named_barrier_sync(int id, int nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
@@ -86,7 +93,9 @@ struct ResidentLattice {
     unsigned long long *E_series, *hist_series;
 };
 
-template <int CM>
+// W = words (4 sites each) a compute thread updates per row visit: 2 (an 8-site chunk: less bookkeeping per site) or
+// 1 (finer grain: the host picks it where chunks would leave the four sub-partitions of an SM unevenly loaded).
+template <int CM, int W>
 __device__ __forceinline__ void resident_run(const ResidentParams &P, const ResidentLattice &X)
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
@@ -103,16 +112,17 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
     uint32_t *s_hist = reinterpret_cast<uint32_t *>(s_raw + 2 * plane_stride);
 
     const uint32_t tid = threadIdx.x, nthreads = blockDim.x;
-    const int cpr = pitch >> 3;                                     // 8-site chunks (2 words) per plane row
+    const int cpr = pitch / (4 * W);                                // compute threads per plane row
+    const int ccomm = pitch >> 3;                                   // comm threads: always one 8-site chunk (2 packets) each
     const int tyc = P.tyc;
     const int ncompute = cpr * tyc;
     const int nbar = (ncompute + 31) & ~31;                         // compute warps, in threads
     const bool is_compute = (int)tid < ncompute;
     const int ctx = (int)tid - nbar;                                // comm thread index
-    const bool is_comm = ctx >= 0 && ctx < cpr;
+    const bool is_comm = ctx >= 0 && ctx < ccomm;
     const int ty = is_compute ? (int)tid / cpr : 0;
-    const int cx = is_compute ? (int)tid - ty * cpr : (is_comm ? ctx : 0);
-    const uint32_t col = 8u * (uint32_t)cx;                         // byte offset of my chunk in a plane row
+    const int cx = is_compute ? (int)tid - ty * cpr : 0;
+    const uint32_t col = is_comm ? 8u * (uint32_t)ctx : 4u * W * (uint32_t)cx;   // byte offset of my words in a plane row
     // Rows are dealt round-robin over the thread rows, interior rows (local 2..rows-1) first, the two
     // boundary rows (local 1 and `rows`) last: they are the only ones that read a halo row.
     const int ni = rows > 2 ? rows - 2 : 0;
@@ -151,13 +161,13 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
     __syncthreads();
 
     // the other-colour word left of my chunk (p = 0) / right of it (p = 1), periodic
-    const uint32_t col_prev = cx == 0 ? (uint32_t)pitch - 4u : col - 4u;
-    const uint32_t col_next = cx + 1 == cpr ? 0u : col + 8u;
+    const uint32_t col_prev = col == 0u ? (uint32_t)pitch - 4u : col - 4u;
+    const uint32_t col_next = col + 4u * W == (uint32_t)pitch ? 0u : col + 4u * W;
     const uint32_t q = in_register(P.q);
     // inbox of CTA x, colour c, side s (0: the row above x's first row, 1: the row below x's last row);
     // one packet {4 spins, seq} per word, so a chunk is two packets = 16 bytes
-    const uint32_t wpr = 2u * (uint32_t)cpr;
-    auto inbox = [&](uint32_t x, uint32_t c, uint32_t s) { return P.inbox + ((size_t)(x * 2 + c) * 2 + s) * wpr + 2u * (uint32_t)cx; };
+    const uint32_t wpr = (uint32_t)pitch >> 2;
+    auto inbox = [&](uint32_t x, uint32_t c, uint32_t s) { return P.inbox + ((size_t)(x * 2 + c) * 2 + s) * wpr + (col >> 2); };
     uint2 *const send_up0 = inbox(up_cta, 0, 1);     // my first row -> the row below the last row of the CTA above
     uint2 *const send_dn0 = inbox(dn_cta, 0, 0);     // my last row  -> the row above the first row of the CTA below
     const uint2 *const recv0 = inbox(b, 0, 0);       // colour c: + c * 2 * wpr, side s: + s * wpr
@@ -180,27 +190,41 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
             const bool count_E = sample && c == 1 && do_E, count_H = sample && do_hist;
             if ((int)tid < nbar) {
                 const HalfSweepKeys K = half_sweep_keys(X.key0, X.key1, t, c);             // uniform registers
-                // one chunk: local row lr, words 2cx and 2cx+1
+                // one visit: local row lr, my W words
                 auto update = [&](int lr) -> uint2 {
                     const uint32_t ro = (uint32_t)(lr * pitch);
                     const uint32_t i = (uint32_t)(r0 + lr - 1);
                     const uint32_t p = (i + c) & 1u;
                     const uint8_t *const orow = oth_row + ro;
-                    const uint2 own = *reinterpret_cast<const uint2 *>(own_col + ro);
-                    const uint2 mid = *reinterpret_cast<const uint2 *>(orow + col);
-                    const uint2 up = *reinterpret_cast<const uint2 *>(orow + col - pitch);
-                    const uint2 dn = *reinterpret_cast<const uint2 *>(orow + col + pitch);
                     const uint32_t adj = *reinterpret_cast<const uint32_t *>(orow + (p ? col_next : col_prev));
-                    uint32_t lf0, rt0, lf1, rt1, nef0, nef1;
-                    horizontal(p, mid.x, p ? mid.y : adj, lf0, rt0);
-                    horizontal(p, mid.y, p ? adj : mid.x, lf1, rt1);
                     const RowKeys R = row_keys(K, i);
                     uint2 out;
-                    out.x = update_word<CM>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, lut, nef0);
-                    out.y = update_word<CM>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, lut, nef1);
-                    *reinterpret_cast<uint2 *>(own_col + ro) = out;
-                    if (count_E) { nef_sum += nef0 + nef1; words_done += 2; }
-                    if (count_H) { hist_add_word(s_hist, P.q, out.x, tid & 31u); hist_add_word(s_hist, P.q, out.y, tid & 31u); }
+                    if (W == 2) {
+                        const uint2 own = *reinterpret_cast<const uint2 *>(own_col + ro);
+                        const uint2 mid = *reinterpret_cast<const uint2 *>(orow + col);
+                        const uint2 up = *reinterpret_cast<const uint2 *>(orow + col - pitch);
+                        const uint2 dn = *reinterpret_cast<const uint2 *>(orow + col + pitch);
+                        uint32_t lf0, rt0, lf1, rt1, nef0, nef1;
+                        horizontal(p, mid.x, p ? mid.y : adj, lf0, rt0);
+                        horizontal(p, mid.y, p ? adj : mid.x, lf1, rt1);
+                        out.x = update_word<CM>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, lut, nef0);
+                        out.y = update_word<CM>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, lut, nef1);
+                        *reinterpret_cast<uint2 *>(own_col + ro) = out;
+                        if (count_E) { nef_sum += nef0 + nef1; words_done += 2; }
+                        if (count_H) { hist_add_word(s_hist, P.q, out.x, tid & 31u); hist_add_word(s_hist, P.q, out.y, tid & 31u); }
+                    } else {
+                        const uint32_t own = *reinterpret_cast<const uint32_t *>(own_col + ro);
+                        const uint32_t mid = *reinterpret_cast<const uint32_t *>(orow + col);
+                        const uint32_t up = *reinterpret_cast<const uint32_t *>(orow + col - pitch);
+                        const uint32_t dn = *reinterpret_cast<const uint32_t *>(orow + col + pitch);
+                        uint32_t lf, rt, nef;
+                        horizontal(p, mid, adj, lf, rt);
+                        out.x = update_word<CM>(own, up, dn, lf, rt, 2u * col + p, q, K, R, lut, nef);
+                        out.y = 0u;
+                        *reinterpret_cast<uint32_t *>(own_col + ro) = out.x;
+                        if (count_E) { nef_sum += nef; words_done += 1; }
+                        if (count_H) hist_add_word(s_hist, P.q, out.x, tid & 31u);
+                    }
                     return out;
                 };
                 if (is_compute)
@@ -215,8 +239,8 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                             const int lr = bb ? rows : 1;
                             const uint2 out = update(lr);
                             if (G > 1) {
-                                if (lr == 1) st_packet2(send_up0 + c * cstride, out, seq);
-                                if (lr == rows) st_packet2(send_dn0 + c * cstride, out, seq);
+                                if (lr == 1) st_packets<W>(send_up0 + c * cstride, out, seq);
+                                if (lr == rows) st_packets<W>(send_dn0 + c * cstride, out, seq);
                             }
                         }
                     }
@@ -285,7 +309,7 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
 }
 
 // One lattice over the whole grid (cooperative launch: the CTAs wait for each other's packets).
-template <int CM, int MAXT>     // MAXT: block size the registers are budgeted for (512 -> up to 128 registers)
+template <int CM, int W, int MAXT>     // MAXT: block size the registers are budgeted for (576 -> 112 registers)
 __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__ ResidentParams P)
 {
     ResidentLattice X;
@@ -299,7 +323,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
     for (int d = 0; d < 4; ++d) X.thr[d] = P.thr[d];
     X.E_series = P.E_series;
     X.hist_series = P.hist_series;
-    resident_run<CM>(P, X);
+    resident_run<CM, W>(P, X);
 }
 
 // Replica batch: CTA r runs lattice r of a batch of independent lattices of the same (L, q), each with
@@ -334,7 +358,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_batch_u8(const __grid_cons
     for (int d = 0; d < 4; ++d) X.thr[d] = T.thr[r][d];
     X.E_series = B.P.E_series ? B.P.E_series + r * B.series_stride : nullptr;
     X.hist_series = B.P.hist_series ? B.P.hist_series + r * B.series_stride * B.P.q : nullptr;
-    resident_run<CM>(B.P, X);
+    resident_run<CM, 2>(B.P, X);
 }
 
 }  // namespace potts

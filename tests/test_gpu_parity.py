@@ -34,6 +34,9 @@ LAUNCH_SHAPES = {
     "resident3": {"variant": 2, "resident_ctas": 3},
     "resident7": {"variant": 2, "resident_ctas": 7},
     "resident148": {"variant": 2, "resident_ctas": 148},
+    "resident_w1": {"variant": 2, "resident_words": 1},          # one 4-site word per thread and row visit
+    "resident_w1_5": {"variant": 2, "resident_words": 1, "resident_ctas": 5},
+    "resident_w2": {"variant": 2, "resident_words": 2},          # an 8-site chunk per thread and row visit
 }
 
 
@@ -86,7 +89,8 @@ def test_cfg1_full_run_series_and_spins(pb, shape):
     (64, 5, workloads.INIT_RANDOM, 0.05, 10),       # cold: thresholds ~ 0
     (512, 9, workloads.INIT_RANDOM, 0.995, 5),      # many blocks
 ])
-@pytest.mark.parametrize("shape", ["streaming", "resident", "resident1", "resident3", "resident148"])
+@pytest.mark.parametrize("shape", ["streaming", "resident", "resident1", "resident3", "resident148", "resident_w1",
+                                   "resident_w1_5", "resident_w2"])
 def test_every_sweep_spins_energy_histogram(pb, L, q, init, f, seed, shape):
     g, o = _pair(pb, L, q, seed, init, shape=shape)
     T = f * workloads.t_c(q)
