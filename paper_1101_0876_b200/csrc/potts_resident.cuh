@@ -26,7 +26,8 @@
 // between, and the receiver sent those after its own comm warps had consumed the slot.
 // The global planes are written at the end of the launch only, so every other entry point
 // (and the next launch) sees the complete state.  Energy and histogram of a sampled sweep are fused:
-// per-thread sums, one block reduction, one atomicAdd per CTA into the series slot.
+// per-thread sums, a warp shuffle and one int64 atomicAdd per warp into the series slot for the energy, the
+// lane-privatised shared table and one atomicAdd per state and CTA for the histogram.
 //
 // The random stream is a pure function of (seed, t, colour, i, j), so the result does not depend on
 // the number of CTAs or the row split; tests check that bit for bit.
@@ -100,7 +101,6 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
     __shared__ uint32_t lut[12];
-    __shared__ uint32_t blockE;
 
     const uint32_t G = X.G, b = X.b;
     const int L = P.L, pitch = P.pitch;
@@ -142,7 +142,6 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
     const bool do_E = X.E_series != nullptr && P.every != 0;
 
     if (tid >= 5 && tid < 9) lut[tid] = tid == 5 ? X.thr[0] : (tid == 6 ? X.thr[1] : (tid == 7 ? X.thr[2] : X.thr[3]));
-    if (tid == 0) blockE = 0u;
     if (do_hist)
         for (uint32_t n = tid; n < hist_words(P.q); n += nthreads) s_hist[n] = 0u;
     // own rows of both planes, and the halo rows of plane 1 (read by the first half-sweep, colour 0):
@@ -279,20 +278,18 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
             if (sample && c == 1) {
                 if (do_E) {
                     // satisfied bonds seen from this thread's black sites = 4 per site - unequal neighbours
-                    // (nef_sum holds 4 byte counters, +<= 8 per chunk: the host keeps rows per thread <= 30)
+                    // (nef_sum holds 4 byte counters, +<= 8 per visit: the host keeps visits per thread <= 30);
+                    // one fire-and-forget int64 atomic per warp: no block-wide barrier for the energy
                     uint32_t satisfied = 16u * words_done - byte_sum(nef_sum);
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
-                    if ((tid & 31u) == 0 && satisfied) atomicAdd(&blockE, satisfied);
-                    __syncthreads();
-                    if (tid == 0) {
-                        atomicAdd(X.E_series + sample_idx, 0ull - (unsigned long long)blockE);
-                        blockE = 0u;
-                    }
+                    if ((tid & 31u) == 0 && satisfied) atomicAdd(X.E_series + sample_idx, 0ull - (unsigned long long)satisfied);
                 }
-                if (do_hist) hist_flush(s_hist, P.q, X.hist_series + (size_t)sample_idx * P.q, tid, nthreads);
+                if (do_hist) {
+                    hist_flush(s_hist, P.q, X.hist_series + (size_t)sample_idx * P.q, tid, nthreads);
+                    __syncthreads();                                // the table is zero again before the next sample counts
+                }
                 ++sample_idx;
-                __syncthreads();
             }
         }
     }
