@@ -79,6 +79,10 @@ def _load():
         lib.oracle_update_site.argtypes = [ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32,
                                            ctypes.c_uint64, ctypes.c_uint32, ctypes.c_double, ctypes.c_uint8, u8p]
         lib.oracle_update_site.restype = ctypes.c_uint8
+        lib.oracle_update_site_s.argtypes = lib.oracle_update_site.argtypes + [ctypes.c_int]
+        lib.oracle_update_site_s.restype = ctypes.c_uint8
+        lib.oracle_set_stream.argtypes = [vp, ctypes.c_int]
+        lib.oracle_set_stream.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -101,24 +105,27 @@ def thresholds(T: float):
     return [int(o[d]) for d in range(1, 5)]
 
 
-def update_site(i, j, t, colour, seed, q, T, s_old, nb):
+def update_site(i, j, t, colour, seed, q, T, s_old, nb, stream=1):
     """New spin of site (i,j) in half-sweep (t, colour) given its 4 neighbours (up, down, left, right)."""
     lib = _load()
     a = (ctypes.c_uint8 * 4)(*[int(x) for x in nb])
-    return int(lib.oracle_update_site(int(i), int(j), int(t) & 0xFFFFFFFF, int(colour), int(seed), int(q),
-                                      float(T), int(s_old), a))
+    return int(lib.oracle_update_site_s(int(i), int(j), int(t) & 0xFFFFFFFF, int(colour), int(seed), int(q),
+                                        float(T), int(s_old), a, int(stream)))
 
 
 class OraclePotts:
     """One lattice held by the C oracle.  Mirrors the call sequence of the product's C-ABI."""
 
-    def __init__(self, L: int, q: int, seed: int, init: int, threads: int = 1):
+    def __init__(self, L: int, q: int, seed: int, init: int, threads: int = 1, stream: int = 1):
         self._lib = _load()
         self._h = self._lib.oracle_create(int(L), int(q), int(seed), int(init))
         if not self._h:
             raise ValueError(f"oracle_create rejected L={L} q={q} init={init}")
         self.L, self.q, self.seed = int(L), int(q), int(seed)
         self._lib.oracle_set_threads(self._h, int(threads))
+        self.stream = int(stream)
+        if self._lib.oracle_set_stream(self._h, self.stream):
+            raise ValueError(f"oracle_set_stream rejected stream={stream} for L={L}")
 
     def close(self):
         if self._h:

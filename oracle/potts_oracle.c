@@ -30,6 +30,12 @@
  * proposal uniformity, and the SURVEY's independently computed golden trajectories.
  * No function in this file is "parity unpinned".
  *
+ * Stream-spec v2 (R3', reading S15; off unless oracle_set_stream(o, 2)): the same-colour
+ * sites of a row are numbered k = j >> 1; sites k = 2m and 2m+1 share ONE Philox block, the one R3 gives site 2m
+ * (counter (j of site 2m, i, t, colour)); site 2m takes (w0, w1) for (proposal, acceptance), site 2m+1 takes
+ * (w2, w3).  Everything else (R1, R2, R4..R9) is unchanged, so even-k sites draw exactly what they draw in v1.
+ * Needs L % 4 == 0.
+ *
  * Optional row parallelism (-fopenmp, oracle_set_threads): rows of one colour are independent
  * (a colour reads only the other colour; the random words are a pure function of the site), so
  * the threaded loop produces the same bits as the serial one; tests check that.
@@ -50,6 +56,7 @@ typedef struct {
     int64_t E_inc;   /* energy tracked incrementally: E(0) + sum of accepted d (R7) */
     uint8_t *s;      /* spins, row-major s[i*L + j] */
     int threads;     /* 1 = serial */
+    int stream;      /* random-stream definition: 1 = one Philox block per site (R3), 2 = per pair of sites (R3') */
 } oracle_potts;
 
 /* ---- R3: Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), written out from its definition:
@@ -115,7 +122,7 @@ oracle_potts *oracle_create(int32_t L, int32_t q, uint64_t seed, int32_t init)
     if (L < 2 || (L & 1) || q < 2 || q > 256 || (init != 0 && init != 1)) return NULL;
     oracle_potts *o = (oracle_potts *)calloc(1, sizeof *o);
     if (!o) return NULL;
-    o->L = L; o->q = q; o->seed = seed; o->t = 0; o->threads = 1;
+    o->L = L; o->q = q; o->seed = seed; o->t = 0; o->threads = 1; o->stream = 1;
     o->s = (uint8_t *)calloc((size_t)L * L, 1);
     if (!o->s) { free(o); return NULL; }
     if (init == 1) {                                   /* R9 */
@@ -142,6 +149,14 @@ void oracle_set_threads(oracle_potts *o, int threads)
     o->threads = threads < 1 ? 1 : threads;
 }
 
+/* choose the random-stream definition (1 or 2, see the header); returns 1 on a bad argument */
+int oracle_set_stream(oracle_potts *o, int stream)
+{
+    if (!o || (stream != 1 && stream != 2) || (stream == 2 && (o->L & 3))) return 1;
+    o->stream = stream;
+    return 0;
+}
+
 int oracle_get_threads(const oracle_potts *o)
 {
 #ifdef _OPENMP
@@ -166,11 +181,15 @@ static int64_t half_sweep(oracle_potts *o, uint32_t colour, const uint32_t thr[5
 #endif
     for (int32_t i = 0; i < L; ++i) {
         for (int32_t j = (int32_t)((i + colour) & 1u); j < L; j += 2) {
-            const uint32_t ctr[4] = { (uint32_t)j, (uint32_t)i, t32, colour };
+            /* R3: the site's own block, words 0 and 1.  R3': the block of the first site of its pair,
+             * words 0, 1 for the first site and 2, 3 for the second. */
+            const int second = o->stream == 2 && ((j >> 1) & 1);
+            const uint32_t ctr[4] = { (uint32_t)(second ? j - 2 : j), (uint32_t)i, t32, colour };
             uint32_t w[4];
-            oracle_philox4x32_10(ctr, key, w);                          /* R3 */
+            oracle_philox4x32_10(ctr, key, w);
+            const uint32_t w_prop = second ? w[2] : w[0], w_acc = second ? w[3] : w[1];
             const uint8_t s_old = S[(size_t)i * L + j];
-            const uint8_t s_new = (uint8_t)propose(w[0], q);            /* R4 */
+            const uint8_t s_new = (uint8_t)propose(w_prop, q);          /* R4 */
             const uint8_t nb[4] = {
                 S[(size_t)((i + L - 1) % L) * L + j],
                 S[(size_t)((i + 1) % L) * L + j],
@@ -180,7 +199,7 @@ static int64_t half_sweep(oracle_potts *o, uint32_t colour, const uint32_t thr[5
             int n_old = 0, n_new = 0;
             for (int k = 0; k < 4; ++k) { n_old += (nb[k] == s_old); n_new += (nb[k] == s_new); }
             const int d = n_old - n_new;                                /* R5 */
-            if (d <= 0 || w[1] < thr[d]) {                              /* R6 */
+            if (d <= 0 || w_acc < thr[d]) {                             /* R6 */
                 S[(size_t)i * L + j] = s_new;                           /* R7 */
                 dE += d;
             }
@@ -248,17 +267,24 @@ int oracle_set_state(oracle_potts *o, const uint8_t *spins, uint64_t t)
 
 /* One site of one half-sweep computed on its own from an explicit neighbourhood (used by the
  * full-size sampled parity checks): returns the new spin.  Same rules, same order. */
-uint8_t oracle_update_site(uint32_t i, uint32_t j, uint32_t t32, uint32_t colour, uint64_t seed,
-                           uint32_t q, double T, uint8_t s_old, const uint8_t nb[4])
+uint8_t oracle_update_site_s(uint32_t i, uint32_t j, uint32_t t32, uint32_t colour, uint64_t seed,
+                             uint32_t q, double T, uint8_t s_old, const uint8_t nb[4], int stream)
 {
     const uint32_t key[2] = { (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32) };
-    const uint32_t ctr[4] = { j, i, t32, colour };
+    const int second = stream == 2 && ((j >> 1) & 1u);
+    const uint32_t ctr[4] = { second ? j - 2u : j, i, t32, colour };
     uint32_t w[4], thr[5];
     oracle_philox4x32_10(ctr, key, w);
     oracle_thresholds(T, thr);
-    const uint8_t s_new = (uint8_t)propose(w[0], q);
+    const uint8_t s_new = (uint8_t)propose(second ? w[2] : w[0], q);
     int n_old = 0, n_new = 0;
     for (int k = 0; k < 4; ++k) { n_old += (nb[k] == s_old); n_new += (nb[k] == s_new); }
     const int d = n_old - n_new;
-    return (d <= 0 || w[1] < thr[d]) ? s_new : s_old;
+    return (d <= 0 || (second ? w[3] : w[1]) < thr[d]) ? s_new : s_old;
+}
+
+uint8_t oracle_update_site(uint32_t i, uint32_t j, uint32_t t32, uint32_t colour, uint64_t seed,
+                           uint32_t q, double T, uint8_t s_old, const uint8_t nb[4])
+{
+    return oracle_update_site_s(i, j, t32, colour, seed, q, T, s_old, nb, 1);
 }
