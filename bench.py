@@ -125,8 +125,9 @@ def slice_of(w: workloads.Workload, max_sweeps: int | None):
 class GpuRun:
     """Drives the product through the Python binding of the C-ABI (argument marshalling only)."""
 
-    def __init__(self, pb, torch, w: workloads.Workload, seed: int, max_sweeps: int | None, options=None):
+    def __init__(self, pb, torch, w: workloads.Workload, seed: int, max_sweeps: int | None, options=None, stream_spec=1):
         self.pb, self.torch, self.w, self.seed = pb, torch, w, seed
+        self.stream_spec = stream_spec
         self.temps, self.per_t = slice_of(w, max_sweeps)
         self.sweeps = self.per_t * len(self.temps)
         self.updates = self.sweeps * w.L * w.L
@@ -147,6 +148,8 @@ class GpuRun:
         self.g = self.pb.Potts(self.w.L, self.w.q, self.seed, self.w.init, layout=self.layout)
         for k, v in self.options.items():
             self.g.potts_set_option(k, v)
+        if self.stream_spec != 1:
+            self.g.potts_set_stream_spec(self.stream_spec)
         self.resident_ctas = self.g.potts_get_option("resident_active")     # 0: one launch per half-sweep
         return self.g
 
@@ -334,12 +337,12 @@ def roofline(w, kernel: str, updates_per_launch: float, ms_per_launch: float, sm
 PER_CONFIG_SLICE = {1: None, 2: 2000, 3: 1600, 4: 200, 5: 100}       # sweeps timed per step (None = all)
 
 
-def per_config_table(pb, torch, flush, sm_max, hbm_gbs, which, skip=()):
+def per_config_table(pb, torch, flush, sm_max, hbm_gbs, which, skip=(), stream_spec=1):
     out = {}
     for k, w in workloads.CONFIGS.items():
         if k in skip:
             continue
-        run = GpuRun(pb, torch, w, w.seed, PER_CONFIG_SLICE[k])
+        run = GpuRun(pb, torch, w, w.seed, PER_CONFIG_SLICE[k], stream_spec=stream_spec)
         ms, launches = time_steps(torch, run, steps=3, warmup=1, flush=flush)
         sec = statistics.median(ms) * 1e-3
         ups = run.updates / sec
@@ -471,6 +474,11 @@ def main():
         per_cfg = per_config_table(pb, torch, flush, sm_max, hbm_gbs, which)
         e6 = paper_protocol_e6(pb, torch)
         per_cfg["batch_cfg1_x1184"] = batch_of_cfg1(pb, torch)
+        # SURVEY 8(f)1, NOT the headline chain: the same workloads under stream-spec v2 (one Philox block per pair of
+        # sites, S15); its algorithmic instruction count is 19 per update, so alu_frac is not comparable
+        v2 = per_config_table(pb, torch, flush, sm_max, hbm_gbs, which, skip=(1,), stream_spec=2)
+        per_cfg["stream_spec_2"] = {k: {"ns_per_spin_flip": v["ns_per_spin_flip"], "spin_updates_per_s": v["spin_updates_per_s"],
+                                        "kernel": v["kernel"]} for k, v in v2.items()}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(w)
     if dist is not None:

@@ -159,6 +159,16 @@ int potts_observables(const int64_t *E_series, int64_t n, int64_t N, double T,
 /* *m = (q N_max/N - 1)/(q - 1) from a histogram (host, q entries). */
 int potts_magnetisation(const int64_t *counts, int32_t q, double *m);
 
+/* ---- random-stream definition ---------------------------------------------------------------------------------
+ * potts_set_stream_spec: 1 (default) = one Philox4x32-10 block per site and half-sweep, words (w0, w1), as in the
+ * header comment; 2 = "stream-spec v2" (reading S15): the same-colour sites of a row are numbered k = j>>1,
+ * sites 2m and 2m+1 share the block of counter (j of site 2m, i, t, colour), site 2m takes (w0, w1), site 2m+1
+ * (w2, w3).  This is NOT a launch option: it selects another Markov chain (same rules, same stationary distribution,
+ * other random numbers, half the random-number work).  Takes effect for all later sweeps of the handle. */
+int potts_set_stream_spec(potts_t *h, int32_t spec);
+int potts_get_stream_spec(potts_t *h, int32_t *spec);
+int potts_batch_set_stream_spec(potts_batch_t *b, int32_t spec);
+
 /* ---- introspection / tuning -------------------------------------------------------------------
  * potts_launch_count: kernels launched by this handle since creation (bench.py's gpu_launches). */
 int potts_launch_count(potts_t *h, uint64_t *n);

@@ -58,6 +58,9 @@ def load_library() -> ctypes.CDLL:
         "potts_batch_download": ([vp, i32, vp], ctypes.c_int),
         "potts_batch_sweep_count": ([vp, P(u64)], ctypes.c_int),
         "potts_batch_launch_count": ([vp, P(u64)], ctypes.c_int),
+        "potts_set_stream_spec": ([vp, i32], ctypes.c_int),
+        "potts_get_stream_spec": ([vp, P(i32)], ctypes.c_int),
+        "potts_batch_set_stream_spec": ([vp, i32], ctypes.c_int),
         "potts_energy": ([vp, P(i64)], ctypes.c_int),
         "potts_histogram": ([vp, vp], ctypes.c_int),
         "potts_download": ([vp, vp], ctypes.c_int),
@@ -87,6 +90,7 @@ EXPORTED_SYMBOLS = [
     "potts_magnetisation", "potts_launch_count", "potts_set_option", "potts_get_option", "potts_last_error",
     "potts_version", "potts_batch_workspace_bytes", "potts_batch_create", "potts_batch_destroy",
     "potts_batch_sweep_measured", "potts_batch_download", "potts_batch_sweep_count", "potts_batch_launch_count",
+    "potts_set_stream_spec", "potts_get_stream_spec", "potts_batch_set_stream_spec",
 ]
 
 
@@ -234,6 +238,14 @@ class Potts:
     def potts_set_sweep_count(self, t: int):
         _check(self._lib.potts_set_sweep_count(self._h, int(t)))
 
+    def potts_set_stream_spec(self, spec: int):
+        _check(self._lib.potts_set_stream_spec(self._h, int(spec)))
+
+    def potts_get_stream_spec(self) -> int:
+        v = ctypes.c_int32()
+        _check(self._lib.potts_get_stream_spec(self._h, ctypes.byref(v)))
+        return int(v.value)
+
     def potts_launch_count(self) -> int:
         n = ctypes.c_uint64()
         _check(self._lib.potts_launch_count(self._h, ctypes.byref(n)))
@@ -295,6 +307,9 @@ class PottsBatch:
         _check(self._lib.potts_batch_sweep_measured(self._h, Ta.ctypes.data, int(nsweeps), int(every),
                                                     E.ctypes.data if energy else None, H.ctypes.data if hist else None))
         return E, H
+
+    def potts_batch_set_stream_spec(self, spec: int):
+        _check(self._lib.potts_batch_set_stream_spec(self._h, int(spec)))
 
     def potts_batch_download(self, r: int) -> np.ndarray:
         out = np.empty((self.L, self.L), dtype=np.uint8)

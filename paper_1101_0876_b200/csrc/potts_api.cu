@@ -61,6 +61,7 @@ struct potts_s {
     size_t smem_optin = 0;
     int coop = 0;                        // device supports cooperative launches (the resident kernel needs one)
     // options (how to launch, never what is computed)
+    int32_t stream_spec = 1;             // random-stream definition (1 = R3, 2 = R3'): changes the chain, not an option
     int64_t opt_variant = 0;             // 0 auto, 1 streaming (one launch per half-sweep), 2 resident
     int64_t opt_resident_ctas = 0;       // 0 auto, else the resident kernel's grid size
     int64_t opt_resident_words = 0;      // 0 auto, 1 / 2: 4-site words per thread and row visit
@@ -128,22 +129,29 @@ potts::SweepParams sweep_params(const potts_t *h, uint32_t colour, const uint32_
     return P;
 }
 
-template <int CM, bool MEASURE, bool HIST>
+template <int CM, int ST, bool MEASURE, bool HIST>
 void launch_hs(const potts::SweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
 {
-    potts::k_half_sweep_u8<CM, MEASURE, HIST><<<grid, dim3(32, potts::HS_WARPS), smem, st>>>(P);
+    potts::k_half_sweep_u8<CM, ST, MEASURE, HIST><<<grid, dim3(32, potts::HS_WARPS), smem, st>>>(P);
 }
 
-template <int CM>
-void launch_hs_cm(const potts::SweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
+template <int CM, int ST>
+void launch_hs_st(const potts::SweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
 {
     const int sel = (P.E_out ? 2 : 0) | (P.hist_out ? 1 : 0);
     switch (sel) {
-    case 0: launch_hs<CM, false, false>(P, grid, smem, st); break;
-    case 1: launch_hs<CM, false, true>(P, grid, smem, st); break;
-    case 2: launch_hs<CM, true, false>(P, grid, smem, st); break;
-    default: launch_hs<CM, true, true>(P, grid, smem, st); break;
+    case 0: launch_hs<CM, ST, false, false>(P, grid, smem, st); break;
+    case 1: launch_hs<CM, ST, false, true>(P, grid, smem, st); break;
+    case 2: launch_hs<CM, ST, true, false>(P, grid, smem, st); break;
+    default: launch_hs<CM, ST, true, true>(P, grid, smem, st); break;
     }
+}
+
+template <int CM>
+void launch_hs_cm(int stream_spec, const potts::SweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
+{
+    if (stream_spec == 2) launch_hs_st<CM, 2>(P, grid, smem, st);
+    else launch_hs_st<CM, 1>(P, grid, smem, st);
 }
 
 int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *E_out,
@@ -159,18 +167,19 @@ int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsign
     const dim3 grid(gx, (unsigned)(h->L / (potts::HS_WARPS * rpt)));
     const size_t smem = hist_out ? (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4 : 0;
     switch (potts::compare_mode_of(h->q)) {
-    case potts::CM_7BIT: launch_hs_cm<potts::CM_7BIT>(P, grid, smem, h->stream); break;
-    case potts::CM_8BIT: launch_hs_cm<potts::CM_8BIT>(P, grid, smem, h->stream); break;
-    case potts::CM_NIB4: launch_hs_cm<potts::CM_NIB4>(P, grid, smem, h->stream); break;
-    default: launch_hs_cm<potts::CM_NIB3>(P, grid, smem, h->stream); break;
+    case potts::CM_7BIT: launch_hs_cm<potts::CM_7BIT>(h->stream_spec, P, grid, smem, h->stream); break;
+    case potts::CM_8BIT: launch_hs_cm<potts::CM_8BIT>(h->stream_spec, P, grid, smem, h->stream); break;
+    case potts::CM_NIB4: launch_hs_cm<potts::CM_NIB4>(h->stream_spec, P, grid, smem, h->stream); break;
+    default: launch_hs_cm<potts::CM_NIB3>(h->stream_spec, P, grid, smem, h->stream); break;
     }
     return check_launch(h, "k_half_sweep_u8");
 }
 
 template <bool FIVE, bool MEASURE, bool HIST>
-void launch_pk(const potts::PackedSweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
+void launch_pk(int stream_spec, const potts::PackedSweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
 {
-    potts::k_half_sweep_packed<FIVE, MEASURE, HIST><<<grid, dim3(32, potts::PK_WARPS), smem, st>>>(P);
+    if (stream_spec == 2) potts::k_half_sweep_packed<FIVE, 2, MEASURE, HIST><<<grid, dim3(32, potts::PK_WARPS), smem, st>>>(P);
+    else potts::k_half_sweep_packed<FIVE, 1, MEASURE, HIST><<<grid, dim3(32, potts::PK_WARPS), smem, st>>>(P);
 }
 
 int launch_half_sweep_packed(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *E_out,
@@ -193,14 +202,14 @@ int launch_half_sweep_packed(potts_t *h, uint32_t colour, const uint32_t thr[4],
     const size_t smem = hist_out ? (size_t)h->q * 32 * 4 : 0;
     const int sel = (h->q > 16 ? 4 : 0) | (E_out ? 2 : 0) | (hist_out ? 1 : 0);
     switch (sel) {
-    case 0: launch_pk<false, false, false>(P, grid, smem, h->stream); break;
-    case 1: launch_pk<false, false, true>(P, grid, smem, h->stream); break;
-    case 2: launch_pk<false, true, false>(P, grid, smem, h->stream); break;
-    case 3: launch_pk<false, true, true>(P, grid, smem, h->stream); break;
-    case 4: launch_pk<true, false, false>(P, grid, smem, h->stream); break;
-    case 5: launch_pk<true, false, true>(P, grid, smem, h->stream); break;
-    case 6: launch_pk<true, true, false>(P, grid, smem, h->stream); break;
-    default: launch_pk<true, true, true>(P, grid, smem, h->stream); break;
+    case 0: launch_pk<false, false, false>(h->stream_spec, P, grid, smem, h->stream); break;
+    case 1: launch_pk<false, false, true>(h->stream_spec, P, grid, smem, h->stream); break;
+    case 2: launch_pk<false, true, false>(h->stream_spec, P, grid, smem, h->stream); break;
+    case 3: launch_pk<false, true, true>(h->stream_spec, P, grid, smem, h->stream); break;
+    case 4: launch_pk<true, false, false>(h->stream_spec, P, grid, smem, h->stream); break;
+    case 5: launch_pk<true, false, true>(h->stream_spec, P, grid, smem, h->stream); break;
+    case 6: launch_pk<true, true, false>(h->stream_spec, P, grid, smem, h->stream); break;
+    default: launch_pk<true, true, true>(h->stream_spec, P, grid, smem, h->stream); break;
     }
     return check_launch(h, "k_half_sweep_packed");
 }
@@ -305,20 +314,26 @@ ResidentPlan plan_resident(const potts_t *h)
 }
 
 // register budget: 112 per thread for blocks up to 576 threads, else 64
-template <int CM>
-const void *resident_kernel_cm(int W, bool small)
+template <int CM, int ST>
+const void *resident_kernel_st(int W, bool small)
 {
-    if (W == 1) return small ? (const void *)potts::k_resident_u8<CM, 1, 576> : (const void *)potts::k_resident_u8<CM, 1, 1024>;
-    return small ? (const void *)potts::k_resident_u8<CM, 2, 576> : (const void *)potts::k_resident_u8<CM, 2, 1024>;
+    if (W == 1) return small ? (const void *)potts::k_resident_u8<CM, 1, ST, 576> : (const void *)potts::k_resident_u8<CM, 1, ST, 1024>;
+    return small ? (const void *)potts::k_resident_u8<CM, 2, ST, 576> : (const void *)potts::k_resident_u8<CM, 2, ST, 1024>;
 }
 
-const void *resident_kernel(int cm, int W, bool small)
+template <int CM>
+const void *resident_kernel_cm(int stream_spec, int W, bool small)
+{
+    return stream_spec == 2 ? resident_kernel_st<CM, 2>(W, small) : resident_kernel_st<CM, 1>(W, small);
+}
+
+const void *resident_kernel(int cm, int stream_spec, int W, bool small)
 {
     switch (cm) {
-    case potts::CM_7BIT: return resident_kernel_cm<potts::CM_7BIT>(W, small);
-    case potts::CM_8BIT: return resident_kernel_cm<potts::CM_8BIT>(W, small);
-    case potts::CM_NIB4: return resident_kernel_cm<potts::CM_NIB4>(W, small);
-    default: return resident_kernel_cm<potts::CM_NIB3>(W, small);
+    case potts::CM_7BIT: return resident_kernel_cm<potts::CM_7BIT>(stream_spec, W, small);
+    case potts::CM_8BIT: return resident_kernel_cm<potts::CM_8BIT>(stream_spec, W, small);
+    case potts::CM_NIB4: return resident_kernel_cm<potts::CM_NIB4>(stream_spec, W, small);
+    default: return resident_kernel_cm<potts::CM_NIB3>(stream_spec, W, small);
     }
 }
 
@@ -343,7 +358,7 @@ int launch_resident(potts_t *h, const ResidentPlan &R, const uint32_t thr[4], in
     P.error = h->error;
     P.rows_max = R.rows_max;
     P.tyc = R.tyc;
-    const void *fn = resident_kernel(potts::compare_mode_of(h->q), R.W, R.nthreads <= 576);
+    const void *fn = resident_kernel(potts::compare_mode_of(h->q), h->stream_spec, R.W, R.nthreads <= 576);
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
     int per_sm = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, R.nthreads, R.smem));
@@ -727,6 +742,21 @@ int potts_set_sweep_count(potts_t *h, uint64_t t)
     return POTTS_OK;
 }
 
+int potts_set_stream_spec(potts_t *h, int32_t spec)
+{
+    if (!h) return fail(POTTS_ERR_ARG, "null handle");
+    if (spec != 1 && spec != 2) return fail(POTTS_ERR_ARG, "stream spec must be 1 or 2");
+    h->stream_spec = spec;
+    return POTTS_OK;
+}
+
+int potts_get_stream_spec(potts_t *h, int32_t *spec)
+{
+    if (!h || !spec) return fail(POTTS_ERR_ARG, "null argument");
+    *spec = h->stream_spec;
+    return POTTS_OK;
+}
+
 int potts_launch_count(potts_t *h, uint64_t *n)
 {
     if (!h || !n) return fail(POTTS_ERR_ARG, "null argument");
@@ -815,6 +845,7 @@ int potts_magnetisation(const int64_t *counts, int32_t q, double *m)
 struct potts_batch_s {
     int32_t n = 0, L = 0, q = 0;
     uint64_t t = 0, launches = 0;
+    int32_t stream_spec = 1;
     uint64_t *seeds = nullptr;            // host copy
     uint8_t *ws = nullptr;
     bool owns_ws = false;
@@ -938,6 +969,14 @@ int potts_batch_sweep_count(potts_batch_t *b, uint64_t *t)
     return POTTS_OK;
 }
 
+int potts_batch_set_stream_spec(potts_batch_t *b, int32_t spec)
+{
+    if (!b) return fail(POTTS_ERR_ARG, "null handle");
+    if (spec != 1 && spec != 2) return fail(POTTS_ERR_ARG, "stream spec must be 1 or 2");
+    b->stream_spec = spec;
+    return POTTS_OK;
+}
+
 int potts_batch_launch_count(potts_batch_t *b, uint64_t *n)
 {
     if (!b || !n) return fail(POTTS_ERR_ARG, "null argument");
@@ -949,14 +988,21 @@ int potts_batch_launch_count(potts_batch_t *b, uint64_t *n)
 
 namespace {
 
-template <int CM>
-cudaError_t launch_batch_cm(const potts::BatchParams &B, const potts::BatchTable &T, int n, int nthreads, size_t smem, cudaStream_t st)
+template <int CM, int ST>
+cudaError_t launch_batch_st(const potts::BatchParams &B, const potts::BatchTable &T, int n, int nthreads, size_t smem, cudaStream_t st)
 {
-    auto fn = potts::k_resident_batch_u8<CM, 1024>;          // 64 registers: several small lattices per SM
+    auto fn = potts::k_resident_batch_u8<CM, ST, 1024>;      // 64 registers: several small lattices per SM
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     fn<<<(unsigned)n, (unsigned)nthreads, smem, st>>>(B, T);
     return cudaGetLastError();
+}
+
+template <int CM>
+cudaError_t launch_batch_cm(int stream_spec, const potts::BatchParams &B, const potts::BatchTable &T, int n, int nthreads, size_t smem,
+                            cudaStream_t st)
+{
+    return stream_spec == 2 ? launch_batch_st<CM, 2>(B, T, n, nthreads, smem, st) : launch_batch_st<CM, 1>(B, T, n, nthreads, smem, st);
 }
 
 }  // namespace
@@ -1011,10 +1057,10 @@ int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweep
         B.lattice_stride = 2ull * b->plane_bytes;
         B.series_stride = (unsigned long long)ns;
         switch (potts::compare_mode_of(b->q)) {
-        case potts::CM_7BIT: e = launch_batch_cm<potts::CM_7BIT>(B, tab, m, R.nthreads, R.smem, b->stream); break;
-        case potts::CM_8BIT: e = launch_batch_cm<potts::CM_8BIT>(B, tab, m, R.nthreads, R.smem, b->stream); break;
-        case potts::CM_NIB4: e = launch_batch_cm<potts::CM_NIB4>(B, tab, m, R.nthreads, R.smem, b->stream); break;
-        default: e = launch_batch_cm<potts::CM_NIB3>(B, tab, m, R.nthreads, R.smem, b->stream); break;
+        case potts::CM_7BIT: e = launch_batch_cm<potts::CM_7BIT>(b->stream_spec, B, tab, m, R.nthreads, R.smem, b->stream); break;
+        case potts::CM_8BIT: e = launch_batch_cm<potts::CM_8BIT>(b->stream_spec, B, tab, m, R.nthreads, R.smem, b->stream); break;
+        case potts::CM_NIB4: e = launch_batch_cm<potts::CM_NIB4>(b->stream_spec, B, tab, m, R.nthreads, R.smem, b->stream); break;
+        default: e = launch_batch_cm<potts::CM_NIB3>(b->stream_spec, B, tab, m, R.nthreads, R.smem, b->stream); break;
         }
         b->launches += 1;
     }

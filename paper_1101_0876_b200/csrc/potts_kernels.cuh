@@ -33,7 +33,7 @@ struct SweepParams {
 // prologue and the block turnover on large lattices; small ones keep rpt low to fill the GPU.
 constexpr int HS_WARPS = 4;
 
-template <int CM, bool MEASURE, bool HIST>
+template <int CM, int ST, bool MEASURE, bool HIST>
 __global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_u8(const __grid_constant__ SweepParams P)
 {
     extern __shared__ uint32_t s_dyn[];             // HIST: the block's histogram table
@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_u8(const __grid_co
             for (int n = 0; n < 4; ++n) {
                 uint32_t lf, rt, nef;
                 horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
-                out[n] = update_word<CM>(own[n], up[n], dn[n], lf, rt, 2u * (uint32_t)(k0 + 4 * n) + p, q, K, R, lut, nef);
+                out[n] = update_word<CM, ST>(own[n], up[n], dn[n], lf, rt, 2u * (uint32_t)(k0 + 4 * n) + p, q, K, R, lut, nef);
                 if (MEASURE) nef_sum += nef;                          // bytes stay <= 16
                 if (HIST) hist_add_word(s_dyn, P.q, out[n], threadIdx.x);
             }

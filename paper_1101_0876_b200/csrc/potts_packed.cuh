@@ -77,7 +77,7 @@ constexpr int PK_WARPS = 4;
 
 // Half-sweep, packed layout: a thread updates 32 consecutive same-colour sites of P.rpt consecutive rows.
 // grid = (ceil(L/64 / 32), L / (PK_WARPS * rpt)), block = (32, PK_WARPS).
-template <bool FIVE, bool MEASURE, bool HIST>
+template <bool FIVE, int ST, bool MEASURE, bool HIST>
 __global__ void __launch_bounds__(32 * PK_WARPS) k_half_sweep_packed(const __grid_constant__ PackedSweepParams P)
 {
     extern __shared__ uint32_t s_dyn[];
@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_half_sweep_packed(const __gri
                     const int n = 2 * m + hlf;                        // byte-per-site word n: sites 4n..4n+3
                     uint32_t lf, rt, nef;
                     horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
-                    out[hlf] = update_word<FIVE ? CM_7BIT : CM_NIB4>(own[hlf], up[hlf], dn[hlf], lf, rt, 2u * (uint32_t)(32 * x + 4 * n) + p, q, K,
+                    out[hlf] = update_word<FIVE ? CM_7BIT : CM_NIB4, ST>(own[hlf], up[hlf], dn[hlf], lf, rt, 2u * (uint32_t)(32 * x + 4 * n) + p, q, K,
                                                   R, lut, nef);
                     if (MEASURE) nef_sum += nef;                      // bytes stay <= 32
                     if (HIST) hist_add_word(s_dyn, P.q, out[hlf], threadIdx.x);

@@ -96,7 +96,7 @@ struct ResidentLattice {
 
 // W = words (4 sites each) a compute thread updates per row visit: 2 (an 8-site chunk: less bookkeeping per site) or
 // 1 (finer grain: the host picks it where chunks would leave the four sub-partitions of an SM unevenly loaded).
-template <int CM, int W>
+template <int CM, int W, int ST>
 __device__ __forceinline__ void resident_run(const ResidentParams &P, const ResidentLattice &X)
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
@@ -206,8 +206,8 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                         uint32_t lf0, rt0, lf1, rt1, nef0, nef1;
                         horizontal(p, mid.x, p ? mid.y : adj, lf0, rt0);
                         horizontal(p, mid.y, p ? adj : mid.x, lf1, rt1);
-                        out.x = update_word<CM>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, lut, nef0);
-                        out.y = update_word<CM>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, lut, nef1);
+                        out.x = update_word<CM, ST>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, lut, nef0);
+                        out.y = update_word<CM, ST>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, lut, nef1);
                         *reinterpret_cast<uint2 *>(own_col + ro) = out;
                         if (count_E) { nef_sum += nef0 + nef1; words_done += 2; }
                         if (count_H) { hist_add_word(s_hist, P.q, out.x, tid & 31u); hist_add_word(s_hist, P.q, out.y, tid & 31u); }
@@ -218,7 +218,7 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                         const uint32_t dn = *reinterpret_cast<const uint32_t *>(orow + col + pitch);
                         uint32_t lf, rt, nef;
                         horizontal(p, mid, adj, lf, rt);
-                        out.x = update_word<CM>(own, up, dn, lf, rt, 2u * col + p, q, K, R, lut, nef);
+                        out.x = update_word<CM, ST>(own, up, dn, lf, rt, 2u * col + p, q, K, R, lut, nef);
                         out.y = 0u;
                         *reinterpret_cast<uint32_t *>(own_col + ro) = out.x;
                         if (count_E) { nef_sum += nef; words_done += 1; }
@@ -306,7 +306,7 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
 }
 
 // One lattice over the whole grid (cooperative launch: the CTAs wait for each other's packets).
-template <int CM, int W, int MAXT>     // MAXT: block size the registers are budgeted for (576 -> 112 registers)
+template <int CM, int W, int ST, int MAXT>     // MAXT: block size the registers are budgeted for (576 -> 112 registers)
 __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__ ResidentParams P)
 {
     ResidentLattice X;
@@ -320,7 +320,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
     for (int d = 0; d < 4; ++d) X.thr[d] = P.thr[d];
     X.E_series = P.E_series;
     X.hist_series = P.hist_series;
-    resident_run<CM, W>(P, X);
+    resident_run<CM, W, ST>(P, X);
 }
 
 // Replica batch: CTA r runs lattice r of a batch of independent lattices of the same (L, q), each with
@@ -340,7 +340,7 @@ struct BatchParams {
     unsigned long long series_stride;    // samples per lattice in E_series (hist_series: x q)
 };
 
-template <int CM, int MAXT>
+template <int CM, int ST, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) k_resident_batch_u8(const __grid_constant__ BatchParams B, const __grid_constant__ BatchTable T)
 {
     const uint32_t r = blockIdx.x;
@@ -355,7 +355,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_batch_u8(const __grid_cons
     for (int d = 0; d < 4; ++d) X.thr[d] = T.thr[r][d];
     X.E_series = B.P.E_series ? B.P.E_series + r * B.series_stride : nullptr;
     X.hist_series = B.P.hist_series ? B.P.hist_series + r * B.series_stride * B.P.q : nullptr;
-    resident_run<CM, 2>(B.P, X);
+    resident_run<CM, 2, ST>(B.P, X);
 }
 
 }  // namespace potts

@@ -280,3 +280,46 @@ def test_batch_larger_than_one_launch_and_ordered_start(pb):
         assert (E[r] == Eo).all() and (b.potts_batch_download(r) == o.spins()).all(), r
     with pytest.raises(pb.PottsError):
         pb.PottsBatch(512, 6, [1, 2])                                  # does not fit one CTA
+
+
+# ---- stream-spec v2 (S15): one Philox block per pair of same-colour sites ------------------
+@pytest.mark.parametrize("L,q,init,f,seed,layout,shape", [
+    (64, 9, workloads.INIT_RANDOM, 0.99, 1, 0, "streaming"),
+    (64, 9, workloads.INIT_RANDOM, 0.99, 1, 0, "resident"),
+    (96, 6, workloads.INIT_ORDERED, 1.005, 7, 0, "resident3"),
+    (256, 24, workloads.INIT_RANDOM, 1.0, 4, 0, "resident_w2"),
+    (512, 200, workloads.INIT_RANDOM, 1.0, 9, 0, "resident_w1"),
+    (1024, 6, workloads.INIT_ORDERED, 1.005, 7, 0, "resident"),
+    (128, 129, workloads.INIT_RANDOM, 1.2, 5, 0, "streaming"),
+    (128, 24, workloads.INIT_ORDERED, 1.002, 4, 1, "streaming"),       # packed, 5 bits
+    (192, 9, workloads.INIT_RANDOM, 0.99, 2, 1, "streaming"),          # packed, 4 bits
+])
+def test_stream_spec_2_matches_oracle(pb, L, q, init, f, seed, layout, shape):
+    g = pb.Potts(L, q, seed, init, layout=layout)
+    for k, v in LAUNCH_SHAPES[shape].items():
+        g.potts_set_option(k, v)
+    g.potts_set_stream_spec(2)
+    assert g.potts_get_stream_spec() == 2
+    o = oracle.OraclePotts(L, q, seed, init, stream=2, threads=4)
+    T = f * workloads.t_c(q)
+    Eg, Hg = g.potts_sweep_measured(T, 12, 3, hist=True)
+    Eo, Ho = o.sweep_measured(T, 12, 3, hist=True)
+    assert (Eg == Eo).all() and (Hg == Ho).all()
+    g.potts_sweep(T, 3)
+    o.sweep(T, 3)
+    assert (g.potts_download() == o.spins()).all() and g.potts_energy() == o.energy()
+    with pytest.raises(pb.PottsError):
+        g.potts_set_stream_spec(3)
+
+
+def test_stream_spec_2_batch_and_default_unchanged(pb):
+    L, q, seeds, T = 64, 9, [11, 12, 13], 0.99 * workloads.t_c(9)
+    b = pb.PottsBatch(L, q, seeds, workloads.INIT_RANDOM)
+    b.potts_batch_set_stream_spec(2)
+    E, H = b.potts_batch_sweep_measured(T, 8, 2)
+    for r, s in enumerate(seeds):
+        o = oracle.OraclePotts(L, q, s, workloads.INIT_RANDOM, stream=2)
+        Eo, Ho = o.sweep_measured(T, 8, 2, hist=True)
+        assert (E[r] == Eo).all() and (H[r] == Ho).all() and (b.potts_batch_download(r) == o.spins()).all()
+    g = pb.Potts(L, q, 11, workloads.INIT_RANDOM)
+    assert g.potts_get_stream_spec() == 1                  # the default chain is north_star's per-site stream
