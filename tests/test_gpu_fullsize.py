@@ -126,3 +126,33 @@ def test_p9_energies_of_the_coexisting_phases_at_tc(pb, q, want_eo, want_ed):
         E, _ = g.potts_ladder([Tc], 6000, 2000, 20, hist=False)
         e = float(E.mean()) / N
         assert abs(e - want) < 6e-3, (q, init, e, want)
+
+
+def test_stream_spec_2_full_size(pb):
+    """Stream-spec v2 at full sizes: packed L = 8192 element by element, L = 32768 on sampled sites."""
+    w = workloads.CONFIGS[4]
+    T = w.temperatures[0]
+    g = _gpu(pb, w)
+    g.potts_set_stream_spec(2)
+    o = oracle.OraclePotts(w.L, w.q, w.seed, w.init, threads=THREADS, stream=2)
+    Eg, _ = g.potts_sweep_measured(T, 3, 1, hist=False)
+    Eo, _ = o.sweep_measured(T, 3, 1, hist=False)
+    assert (Eg == Eo).all() and (g.potts_download() == o.spins()).all()
+    del g, o
+    w = workloads.CONFIGS[5]
+    T = w.temperatures[0]
+    g = _gpu(pb, w)
+    g.potts_set_stream_spec(2)
+    g.potts_sweep(T, 5)
+    S0 = g.potts_download()
+    t = g.potts_sweep_count()
+    g.potts_sweep(T, 1)
+    S1 = g.potts_download()
+    rng = np.random.default_rng(3)
+    L = w.L
+    for i, j in zip(rng.integers(0, L, 1500), rng.integers(0, L, 1500)):
+        i, j = int(i), int(j)
+        c = (i + j) & 1
+        src = S0 if c == 0 else S1
+        nb = [src[(i - 1) % L, j], src[(i + 1) % L, j], src[i, (j - 1) % L], src[i, (j + 1) % L]]
+        assert int(S1[i, j]) == oracle.update_site(i, j, t, c, w.seed, w.q, T, int(S0[i, j]), nb, stream=2), (i, j)
