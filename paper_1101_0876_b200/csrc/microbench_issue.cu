@@ -97,7 +97,7 @@ __global__ void __launch_bounds__(256) kb(uint32_t *out, HalfSweepKeys K, uint32
             for (int b = 0; b < 4; ++b) { philox_site(K, R, j0 + 2u * b, w0, w1); acc ^= w0 + w1; }
         } else if (MODE == 1) {     // full update
             uint32_t nef;
-            own = update_word<false>(own, up, dn, lf, rt, j0, qq, K, R, lut, nef);
+            own = update_word<CM_7BIT, 1>(own, up, dn, lf, rt, j0, qq, K, R, lut, nef);
             acc += nef; up ^= own; 
         } else if (MODE == 2) {     // philox + proposal only
             uint32_t w0[4], w1[4];
