@@ -71,3 +71,20 @@ def test_host_observables_against_exact_arithmetic(pb):
     assert pb.potts_magnetisation(np.array([10, 70, 20], dtype=np.int64), 3) == pytest.approx((3 * 0.7 - 1) / 2, rel=1e-15)
     with pytest.raises(pb.PottsError):
         pb.potts_observables(np.zeros(0, dtype=np.int64), 16, 1.0)
+
+
+def test_product_fails_loudly_without_a_gpu(pb):
+    """No CPU fallback: on a box without a CUDA device every constructor refuses (on a GPU box this test is moot)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(pb.PottsError) as e:
+        pb.Potts(64, 4, 1)
+    assert e.value.code == pb.ERR_CUDA
+    with pytest.raises(pb.PottsError):
+        pb.PottsBatch(64, 4, [1, 2])
+    lib = pb.load_library()
+    h = ctypes.c_void_p()
+    rc = lib.potts_create(ctypes.byref(h), 64, 4, 1, 0)            # the C entry point itself, no Python in between
+    assert rc == pb.ERR_CUDA and not h.value
+    assert b"CUDA" in lib.potts_last_error() or b"device" in lib.potts_last_error()
