@@ -274,7 +274,7 @@ ResidentPlan plan_resident(const potts_t *h)
     if (!h->coop) { R.why = "the device does not support cooperative launches"; return R; }
     if (L > RESIDENT_L_MAX || !h->inbox) { R.why = "L exceeds the resident kernel's 512 words per row"; return R; }
     const long long words = (long long)L * R.wpr;                   // 4-site words per half-sweep
-    long long G = h->opt_resident_ctas > 0 ? h->opt_resident_ctas : words / 128;   // measured: more CTAs win down to ~4 rows each
+    long long G = h->opt_resident_ctas > 0 ? h->opt_resident_ctas : words / 256;   // measured (profiles/r01c_kernels.md): one CTA per 256 words of a half-sweep
     if (G < 1) G = 1;
     if (G > h->num_sms) G = h->num_sms;
     if (G > L) G = L;
