@@ -150,18 +150,21 @@ class GpuRun:
             self.g.potts_set_option(k, v)
         if self.stream_spec != 1:
             self.g.potts_set_stream_spec(self.stream_spec)
-        self.resident_ctas = self.g.potts_get_option("resident_active")     # 0: one launch per half-sweep
+        self.resident_ctas = self.g.potts_get_option("resident_active")     # 0: not the resident kernel
+        self.cluster_ctas = self.g.potts_get_option("cluster_active")       # 0: not the cluster kernel
         return self.g
 
     @property
     def kernel(self):
         if self.layout != self.pb.LAYOUT_U8:
             return "k_half_sweep_packed"
+        if self.cluster_ctas:
+            return "k_cluster_u8"
         return "k_resident_u8" if self.resident_ctas else "k_half_sweep_u8"
 
     @property
     def kernel_launches_per_step(self):
-        return len(self.temps) if self.resident_ctas else 2 * self.sweeps
+        return len(self.temps) if (self.resident_ctas or self.cluster_ctas) else 2 * self.sweeps
 
     def enqueue(self):
         """The step: all sweeps with the device-resident series; returns without a sync."""
@@ -350,7 +353,7 @@ def per_config_table(pb, torch, flush, sm_max, hbm_gbs, which, skip=(), stream_s
         r = roofline(w, run.kernel, run.updates / nl, sec * 1e3 / nl, sm_max, hbm_gbs, which, run.bytes_per_update)
         out[w.name] = {"q": w.q, "L": w.L, "sweeps_timed": run.sweeps, "of_sweeps": w.total_sweeps,
                        "ns_per_spin_flip": 1e9 / ups, "spin_updates_per_s": ups, "ms": sec * 1e3,
-                       "launches": launches // 3, "kernel": run.kernel, "resident_ctas": run.resident_ctas,
+                       "launches": launches // 3, "kernel": run.kernel, "resident_ctas": run.resident_ctas, "cluster_ctas": run.cluster_ctas,
                        "alu_frac": r["frac"], "alu_frac_of_measured_int_issue": r["frac_of_measured_int_issue"],
                        "hbm_frac": r["hbm"]["frac"],
                        "layout": "packed" if run.layout == pb.LAYOUT_PACKED else "u8"}

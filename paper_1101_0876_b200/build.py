@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libpotts_b200.so")
 SOURCES = ["potts_api.cu"]
-DEPS = ["potts_api.cu", "potts_core.cuh", "potts_kernels.cuh", "potts_resident.cuh", "potts_packed.cuh", os.path.join(INCLUDE, "potts.h")]
+DEPS = ["potts_api.cu", "potts_core.cuh", "potts_kernels.cuh", "potts_resident.cuh", "potts_packed.cuh", "potts_cluster.cuh", os.path.join(INCLUDE, "potts.h")]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -4,6 +4,7 @@
 #include "potts_kernels.cuh"
 #include "potts_resident.cuh"
 #include "potts_packed.cuh"
+#include "potts_cluster.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -38,7 +39,8 @@ int fail(int code, const char *fmt, ...)
 constexpr size_t ALIGN = 256;
 constexpr size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 constexpr int MAX_CTAS = 160;             // upper bound on the resident kernel's grid (>= SM count of B200)
-constexpr int RESIDENT_L_MAX = 4096;      // largest lattice the resident kernel can hold (512 words per row)
+constexpr int RESIDENT_L_MAX = 4096;
+constexpr int CLUSTER_AUTO_L_MAX = 128;    // lattices up to this size go to the cluster (DSMEM) kernel by default (measured: 2x the resident kernel)      // largest lattice the resident kernel can hold (512 words per row)
 constexpr int ACC_WORDS = 1 + 256 + 1;    // E, hist[256], flag/error word
 
 }  // namespace
@@ -65,6 +67,7 @@ struct potts_s {
     int64_t opt_variant = 0;             // 0 auto, 1 streaming (one launch per half-sweep), 2 resident
     int64_t opt_resident_ctas = 0;       // 0 auto, else the resident kernel's grid size
     int64_t opt_resident_words = 0;      // 0 auto, 1 / 2: 4-site words per thread and row visit
+    int64_t opt_cluster_ctas = 0;        // 0 auto, else the cluster kernel's cluster size (1..8)
 };
 
 namespace {
@@ -372,6 +375,85 @@ int launch_resident(potts_t *h, const ResidentPlan &R, const uint32_t thr[4], in
     return POTTS_OK;
 }
 
+// ---- cluster (DSMEM) path for tiny lattices -------------------------------------------------------
+struct ClusterPlan { bool ok = false; int G = 0, tyc = 0, rows_max = 0, nthreads = 0; size_t smem = 0; const char *why = ""; };
+
+ClusterPlan plan_cluster(const potts_t *h)
+{
+    ClusterPlan R;
+    const int L = h->L, wpr = L / 8;
+    if (h->layout != POTTS_LAYOUT_U8) { R.why = "the cluster kernel holds the U8 layout only"; return R; }
+    if (wpr > 1024) { R.why = "L/8 words per row exceed 1024 threads"; return R; }
+    long long G = h->opt_cluster_ctas > 0 ? h->opt_cluster_ctas : ((long long)L * wpr) / 128;   // measured: L = 64 -> 4, L = 128 -> 8
+    if (G < 1) G = 1;
+    if (G > potts::CLUSTER_MAX) G = potts::CLUSTER_MAX;
+    if (G > L) G = L;
+    R.G = (int)G;
+    R.rows_max = (L + R.G - 1) / R.G;
+    int tyc = 1024 / wpr;
+    if (tyc > R.rows_max) tyc = R.rows_max;
+    R.tyc = tyc;
+    R.nthreads = (wpr * tyc + 31) / 32 * 32;
+    if ((R.rows_max + tyc - 1) / tyc > 60) { R.why = "too many rows per thread"; return R; }
+    const size_t hist = (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4;
+    R.smem = 2 * (size_t)(R.rows_max + 2) * (L / 2) + hist;
+    if (R.smem + 1024 > h->smem_optin) { R.why = "lattice does not fit the shared memory of one cluster"; return R; }
+    R.ok = true;
+    return R;
+}
+
+template <int CM>
+const void *cluster_kernel_cm(int stream_spec)
+{
+    return stream_spec == 2 ? (const void *)potts::k_cluster_u8<CM, 2> : (const void *)potts::k_cluster_u8<CM, 1>;
+}
+
+int launch_cluster(potts_t *h, const ClusterPlan &R, const uint32_t thr[4], int64_t nsweeps, int64_t every,
+                   unsigned long long *E_series_dev, unsigned long long *hist_series_dev)
+{
+    potts::ResidentParams P = {};
+    P.plane[0] = h->plane[0];
+    P.plane[1] = h->plane[1];
+    P.L = h->L;
+    P.pitch = h->L / 2;
+    P.q = (uint32_t)h->q;
+    P.key0 = (uint32_t)(h->seed & 0xFFFFFFFFull);
+    P.key1 = (uint32_t)(h->seed >> 32);
+    for (int d = 0; d < 4; ++d) P.thr[d] = thr[d];
+    P.t0 = (uint32_t)h->t;
+    P.nsweeps = (uint32_t)nsweeps;
+    P.every = (uint32_t)every;
+    P.E_series = E_series_dev;
+    P.hist_series = hist_series_dev;
+    P.error = h->error;
+    P.rows_max = R.rows_max;
+    P.tyc = R.tyc;
+    const void *fn = nullptr;
+    switch (potts::compare_mode_of(h->q)) {
+    case potts::CM_7BIT: fn = cluster_kernel_cm<potts::CM_7BIT>(h->stream_spec); break;
+    case potts::CM_8BIT: fn = cluster_kernel_cm<potts::CM_8BIT>(h->stream_spec); break;
+    case potts::CM_NIB4: fn = cluster_kernel_cm<potts::CM_NIB4>(h->stream_spec); break;
+    default: fn = cluster_kernel_cm<potts::CM_NIB3>(h->stream_spec); break;
+    }
+    CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)R.G);
+    cfg.blockDim = dim3((unsigned)R.nthreads);
+    cfg.dynamicSmemBytes = R.smem;
+    cfg.stream = h->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)R.G;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    void *args[] = {(void *)&P};
+    CUDA_TRY(cudaLaunchKernelExC(&cfg, fn, args));
+    h->launches += 1;
+    return POTTS_OK;
+}
+
 // the sweep loop shared by potts_sweep and potts_sweep_measured_dev
 int run_sweeps(potts_t *h, double T, int64_t nsweeps, int64_t every, unsigned long long *E_series_dev,
                unsigned long long *hist_series_dev)
@@ -379,6 +461,23 @@ int run_sweeps(potts_t *h, double T, int64_t nsweeps, int64_t every, unsigned lo
     uint32_t thr[4];
     thresholds(T, thr);
     if (nsweeps == 0) return POTTS_OK;
+    if (h->opt_variant == 3 || (h->opt_variant == 0 && h->layout == POTTS_LAYOUT_U8 && h->L <= CLUSTER_AUTO_L_MAX)) {
+        const ClusterPlan C = plan_cluster(h);
+        if (C.ok) {
+            const int64_t piece = every > 0 ? (int64_t)((1ll << 30) / every) * every : (1ll << 30);
+            for (int64_t done = 0; done < nsweeps;) {
+                const int64_t n = nsweeps - done < piece ? nsweeps - done : piece;
+                const int64_t s0 = every > 0 ? done / every : 0;
+                int rc = launch_cluster(h, C, thr, n, every > 0 ? every : 0, E_series_dev ? E_series_dev + s0 : nullptr,
+                                        hist_series_dev ? hist_series_dev + s0 * h->q : nullptr);
+                if (rc) return rc;
+                h->t += (uint64_t)n;
+                done += n;
+            }
+            return POTTS_OK;
+        }
+        if (h->opt_variant == 3) return fail(POTTS_ERR_UNSUPPORTED, "cluster variant unavailable: %s", C.why);
+    }
     if (h->opt_variant != 1) {
         const ResidentPlan R = plan_resident(h);
         if (R.ok) {
@@ -768,12 +867,16 @@ int potts_set_option(potts_t *h, const char *key, int64_t value)
 {
     if (!h || !key) return fail(POTTS_ERR_ARG, "null argument");
     if (!std::strcmp(key, "variant")) {
-        if (value < 0 || value > 2) return fail(POTTS_ERR_ARG, "variant must be 0 (auto), 1 (streaming) or 2 (resident)");
+        if (value < 0 || value > 3) return fail(POTTS_ERR_ARG, "variant must be 0 (auto), 1 (streaming), 2 (resident) or 3 (cluster)");
         h->opt_variant = value; return POTTS_OK;
     }
     if (!std::strcmp(key, "resident_ctas")) {
         if (value < 0 || value > MAX_CTAS) return fail(POTTS_ERR_ARG, "resident_ctas must be in [0, %d]", MAX_CTAS);
         h->opt_resident_ctas = value; return POTTS_OK;
+    }
+    if (!std::strcmp(key, "cluster_ctas")) {
+        if (value < 0 || value > potts::CLUSTER_MAX) return fail(POTTS_ERR_ARG, "cluster_ctas must be in [0, %d]", potts::CLUSTER_MAX);
+        h->opt_cluster_ctas = value; return POTTS_OK;
     }
     if (!std::strcmp(key, "resident_words")) {
         if (value < 0 || value > 2) return fail(POTTS_ERR_ARG, "resident_words must be 0 (auto), 1 or 2");
@@ -788,8 +891,14 @@ int potts_get_option(potts_t *h, const char *key, int64_t *value)
     if (!std::strcmp(key, "variant")) { *value = h->opt_variant; return POTTS_OK; }
     if (!std::strcmp(key, "resident_ctas")) { *value = h->opt_resident_ctas; return POTTS_OK; }
     if (!std::strcmp(key, "resident_words")) { *value = h->opt_resident_words; return POTTS_OK; }
+    if (!std::strcmp(key, "cluster_ctas")) { *value = h->opt_cluster_ctas; return POTTS_OK; }
+    if (!std::strcmp(key, "cluster_active")) {             // read-only: cluster size the next sweep call would use (0 = not the cluster kernel)
+        const bool want = h->opt_variant == 3 || (h->opt_variant == 0 && h->layout == POTTS_LAYOUT_U8 && h->L <= CLUSTER_AUTO_L_MAX);
+        *value = (want && plan_cluster(h).ok) ? plan_cluster(h).G : 0; return POTTS_OK;
+    }
     if (!std::strcmp(key, "resident_active")) {            // read-only: would the next sweep call run resident?
-        *value = (h->opt_variant != 1 && plan_resident(h).ok) ? plan_resident(h).G : 0; return POTTS_OK;
+        const bool cluster = h->opt_variant == 3 || (h->opt_variant == 0 && h->layout == POTTS_LAYOUT_U8 && h->L <= CLUSTER_AUTO_L_MAX && plan_cluster(h).ok);
+        *value = (!cluster && h->opt_variant != 1 && plan_resident(h).ok) ? plan_resident(h).G : 0; return POTTS_OK;
     }
     return fail(POTTS_ERR_ARG, "unknown option '%s'", key);
 }

@@ -33,8 +33,10 @@ def _cases(n, seed):
         L = int(rng.choice([64, 128, 192, 256, 320]) if packed else rng.choice([32, 64, 96, 128, 160, 224, 256, 288, 384, 512]))
         shape = {}
         if not packed:
-            variant = int(rng.choice([1, 2, 2, 2]))
+            variant = int(rng.choice([1, 2, 2, 2, 3, 0]))
             shape["variant"] = variant
+            if variant == 3:
+                shape["cluster_ctas"] = int(rng.choice([0, 1, 2, 3, 5, 8]))
             if variant == 2:
                 shape["resident_ctas"] = int(rng.choice([0, 1, 2, 3, 5, 8, 13, 31, 64, 148]))
                 shape["resident_words"] = int(rng.choice([0, 1, 2]))
@@ -50,8 +52,9 @@ def test_random_case_matches_oracle(pb, case):
     g = pb.Potts(L, q, case["seed"], case["init"], layout=pb.LAYOUT_PACKED if case["packed"] else pb.LAYOUT_U8)
     for k, v in case["shape"].items():
         g.potts_set_option(k, v)
-    if case["shape"].get("variant") == 2 and g.potts_get_option("resident_active") == 0:
-        pytest.skip("forced resident shape cannot hold this lattice")
+    if (case["shape"].get("variant") == 2 and g.potts_get_option("resident_active") == 0) or \
+            (case["shape"].get("variant") == 3 and g.potts_get_option("cluster_active") == 0):
+        pytest.skip("forced launch shape cannot hold this lattice")
     o = oracle.OraclePotts(L, q, case["seed"], case["init"])
     T = case["f"] * workloads.t_c(q)
     n = case["nsweeps"] // case["every"] * case["every"]

@@ -37,6 +37,11 @@ LAUNCH_SHAPES = {
     "resident_w1": {"variant": 2, "resident_words": 1},          # one 4-site word per thread and row visit
     "resident_w1_5": {"variant": 2, "resident_words": 1, "resident_ctas": 5},
     "resident_w2": {"variant": 2, "resident_words": 2},          # an 8-site chunk per thread and row visit
+    "cluster": {"variant": 3},                                   # one thread-block cluster, boundary rows through DSMEM
+    "cluster1": {"variant": 3, "cluster_ctas": 1},
+    "cluster3": {"variant": 3, "cluster_ctas": 3},
+    "cluster8": {"variant": 3, "cluster_ctas": 8},
+    "auto": {"variant": 0},
 }
 
 
@@ -44,7 +49,9 @@ def _pair(pb, L, q, seed, init, layout=0, shape=None):
     g = pb.Potts(L, q, seed, init, layout=layout)
     for k, v in LAUNCH_SHAPES[shape or "streaming"].items():
         g.potts_set_option(k, v)
-    if (shape or "streaming").startswith("resident") and g.potts_get_option("resident_active") == 0:
+    sh = shape or "streaming"
+    if (sh.startswith("resident") and g.potts_get_option("resident_active") == 0) or \
+            (sh.startswith("cluster") and g.potts_get_option("cluster_active") == 0):
         with pytest.raises(pb.PottsError) as e:          # a forced shape that cannot hold the lattice is refused
             g.potts_sweep(1.0, 1)
         assert e.value.code == pb.ERR_UNSUPPORTED
@@ -53,7 +60,7 @@ def _pair(pb, L, q, seed, init, layout=0, shape=None):
     return g, o
 
 
-@pytest.mark.parametrize("shape", ["streaming", "resident", "resident2", "resident7"])
+@pytest.mark.parametrize("shape", ["streaming", "resident", "resident2", "resident7", "cluster", "auto"])
 def test_cfg1_full_run_series_and_spins(pb, shape):
     """BASELINE configs[0] in full: q=9, L=64, random start, 0.99 T_c, 1000 sweeps, E+hist every sweep."""
     w = workloads.CONFIGS[1]
@@ -90,7 +97,7 @@ def test_cfg1_full_run_series_and_spins(pb, shape):
     (512, 9, workloads.INIT_RANDOM, 0.995, 5),      # many blocks
 ])
 @pytest.mark.parametrize("shape", ["streaming", "resident", "resident1", "resident3", "resident148", "resident_w1",
-                                   "resident_w1_5", "resident_w2"])
+                                   "resident_w1_5", "resident_w2", "cluster", "cluster1", "cluster3", "cluster8", "auto"])
 def test_every_sweep_spins_energy_histogram(pb, L, q, init, f, seed, shape):
     g, o = _pair(pb, L, q, seed, init, shape=shape)
     T = f * workloads.t_c(q)
@@ -291,6 +298,7 @@ def test_batch_larger_than_one_launch_and_ordered_start(pb):
     (512, 200, workloads.INIT_RANDOM, 1.0, 9, 0, "resident_w1"),
     (1024, 6, workloads.INIT_ORDERED, 1.005, 7, 0, "resident"),
     (128, 129, workloads.INIT_RANDOM, 1.2, 5, 0, "streaming"),
+    (128, 9, workloads.INIT_RANDOM, 0.99, 3, 0, "cluster"),
     (128, 24, workloads.INIT_ORDERED, 1.002, 4, 1, "streaming"),       # packed, 5 bits
     (192, 9, workloads.INIT_RANDOM, 0.99, 2, 1, "streaming"),          # packed, 4 bits
 ])
