@@ -62,6 +62,8 @@ struct potts_s {
     int num_sms = 0;
     size_t smem_optin = 0;
     int coop = 0;                        // device supports cooperative launches (the resident kernel needs one)
+    uint8_t *scratch = nullptr;          // device scratch kept between calls (staging for up/download, host-series buffers)
+    size_t scratch_bytes = 0;
     // options (how to launch, never what is computed)
     int32_t stream_spec = 1;             // random-stream definition (1 = R3, 2 = R3'): changes the chain, not an option
     int64_t opt_variant = 0;             // 0 auto, 1 streaming (one launch per half-sweep), 2 resident
@@ -107,6 +109,18 @@ void thresholds(double T, uint32_t thr[4])
 {
     // reading R6: exactly floor(ldexp(exp(-d/T), 32)) in double
     for (int d = 1; d <= 4; ++d) thr[d - 1] = (uint32_t)std::floor(std::ldexp(std::exp(-(double)d / T), 32));
+}
+
+// device scratch of at least `bytes`, kept in the handle so that repeated calls do not pay cudaMalloc / cudaFree
+int get_scratch(potts_t *h, size_t bytes, uint8_t **out)
+{
+    if (h->scratch_bytes < bytes) {
+        if (h->scratch) { cudaStreamSynchronize(h->stream); cudaFree(h->scratch); h->scratch = nullptr; h->scratch_bytes = 0; }
+        CUDA_TRY(cudaMalloc(&h->scratch, bytes));
+        h->scratch_bytes = bytes;
+    }
+    *out = h->scratch;
+    return POTTS_OK;
 }
 
 int check_launch(potts_t *h, const char *what)
@@ -632,10 +646,9 @@ int potts_create(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t ini
 void potts_destroy(potts_t *h)
 {
     if (!h) return;
-    if (h->owns_ws && h->ws) {
-        cudaStreamSynchronize(h->stream);
-        cudaFree(h->ws);
-    }
+    if (h->scratch || (h->owns_ws && h->ws)) cudaStreamSynchronize(h->stream);
+    if (h->scratch) cudaFree(h->scratch);
+    if (h->owns_ws && h->ws) cudaFree(h->ws);
     delete h;
 }
 
@@ -681,7 +694,10 @@ int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every, i
     if (ns == 0) return POTTS_OK;
     const size_t eb = E_series ? (size_t)ns * 8 : 0, hb = hist_series ? (size_t)ns * h->q * 8 : 0;
     uint8_t *dev = nullptr;
-    if (eb + hb) CUDA_TRY(cudaMalloc(&dev, eb + hb));
+    if (eb + hb) {
+        rc = get_scratch(h, eb + hb, &dev);
+        if (rc) return rc;
+    }
     int64_t *dE = E_series ? (int64_t *)dev : nullptr;
     int64_t *dH = hist_series ? (int64_t *)(dev + eb) : nullptr;
     rc = potts_sweep_measured_dev(h, T, nsweeps, every, dE, dH);
@@ -690,7 +706,6 @@ int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every, i
     if (rc == POTTS_OK && e == cudaSuccess && hb)
         e = cudaMemcpyAsync(hist_series, dH, hb, cudaMemcpyDeviceToHost, h->stream);
     cudaError_t e2 = cudaStreamSynchronize(h->stream);
-    if (dev) cudaFree(dev);
     if (rc) return rc;
     if (e != cudaSuccess || e2 != cudaSuccess)
         return fail(POTTS_ERR_CUDA, "series copy/sync failed: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
@@ -712,7 +727,8 @@ int potts_ladder(potts_t *h, const double *T, int32_t nT, int64_t t_tran, int64_
     const size_t eb = E_series ? (size_t)ns * 8 : 0, hb = hist_series ? (size_t)ns * h->q * 8 : 0;
     uint8_t *dev = nullptr;
     if (eb + hb) {
-        CUDA_TRY(cudaMalloc(&dev, eb + hb));
+        int rc0 = get_scratch(h, eb + hb, &dev);
+        if (rc0) return rc0;
         cudaMemsetAsync(dev, 0, eb + hb, h->stream);
     }
     unsigned long long *dE = eb ? (unsigned long long *)dev : nullptr;
@@ -727,7 +743,6 @@ int potts_ladder(potts_t *h, const double *T, int32_t nT, int64_t t_tran, int64_
     if (rc == POTTS_OK && eb) e = cudaMemcpyAsync(E_series, dE, eb, cudaMemcpyDeviceToHost, h->stream);
     if (rc == POTTS_OK && e == cudaSuccess && hb) e = cudaMemcpyAsync(hist_series, dH, hb, cudaMemcpyDeviceToHost, h->stream);
     const cudaError_t e2 = cudaStreamSynchronize(h->stream);
-    if (dev) cudaFree(dev);
     if (rc) return rc;
     if (e != cudaSuccess || e2 != cudaSuccess)
         return fail(POTTS_ERR_CUDA, "ladder copy/sync failed: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
@@ -770,8 +785,8 @@ int potts_download(potts_t *h, uint8_t *spins)
     if (!h || !spins) return fail(POTTS_ERR_ARG, "null argument");
     const int L = h->L, rows = chunk_rows(L);
     uint8_t *stage = nullptr;
-    CUDA_TRY(cudaMalloc(&stage, (size_t)rows * L));
-    int rc = POTTS_OK;
+    int rc = get_scratch(h, (size_t)rows * L, &stage);
+    if (rc) return rc;
     for (int i0 = 0; i0 < L && rc == POTTS_OK; i0 += rows) {
         const int r = (L - i0 < rows) ? L - i0 : rows;
         const long long threads = (long long)r * (L / 8);
@@ -790,7 +805,6 @@ int potts_download(potts_t *h, uint8_t *spins)
             if (e != cudaSuccess) rc = fail(POTTS_ERR_CUDA, "download copy failed: %s", cudaGetErrorString(e));
         }
     }
-    cudaFree(stage);
     return rc ? rc : check_device_error(h);
 }
 
@@ -803,8 +817,8 @@ int potts_upload(potts_t *h, const uint8_t *spins)
         for (size_t n = 0; n < (size_t)L * L; ++n)
             if (spins[n] >= h->q) return fail(POTTS_ERR_ARG, "spin value %d >= q at offset %zu", (int)spins[n], n);
     uint8_t *stage = nullptr;
-    CUDA_TRY(cudaMalloc(&stage, (size_t)rows * L));
-    int rc = POTTS_OK;
+    int rc = get_scratch(h, (size_t)rows * L, &stage);
+    if (rc) return rc;
     cudaMemsetAsync(h->flag, 0, sizeof(int), h->stream);
     for (int i0 = 0; i0 < L && rc == POTTS_OK; i0 += rows) {
         const int r = (L - i0 < rows) ? L - i0 : rows;
@@ -822,7 +836,6 @@ int potts_upload(potts_t *h, const uint8_t *spins)
         if (rc == POTTS_OK && cudaStreamSynchronize(h->stream) != cudaSuccess)
             rc = fail(POTTS_ERR_CUDA, "upload sync failed");
     }
-    cudaFree(stage);
     return rc;
 }
 
