@@ -409,7 +409,7 @@ ClusterPlan plan_cluster(const potts_t *h)
     R.tyc = tyc;
     R.nthreads = (wpr * tyc + 31) / 32 * 32;
     if ((R.rows_max + tyc - 1) / tyc > 60) { R.why = "too many rows per thread"; return R; }
-    const size_t hist = (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4;
+    const size_t hist = 2 * (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4;   // two tables
     R.smem = 2 * (size_t)(R.rows_max + 2) * (L / 2) + hist;
     if (R.smem + 1024 > h->smem_optin) { R.why = "lattice does not fit the shared memory of one cluster"; return R; }
     R.ok = true;

@@ -36,7 +36,8 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
     const int rows_up = (int)(((long long)(up_cta + 1) * L) / G) - (int)(((long long)up_cta * L) / G);
     const int srows = P.rows_max + 2;
     const uint32_t plane_stride = (uint32_t)srows * (uint32_t)pitch;
-    uint32_t *s_hist = reinterpret_cast<uint32_t *>(s_raw + 2 * plane_stride);
+    // two histogram tables used by alternate samples: one is flushed (and zeroed) while the next sample already counts
+    uint32_t *const s_hist0 = reinterpret_cast<uint32_t *>(s_raw + 2 * plane_stride);
     // the same shared-memory layout in every CTA of the cluster: my pointers, seen in the neighbours' address space
     uint8_t *const up_raw = cluster.map_shared_rank(s_raw, up_cta);
     uint8_t *const dn_raw = cluster.map_shared_rank(s_raw, dn_cta);
@@ -54,7 +55,7 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
 
     if (tid < 9) lut[tid] = tid >= 5 ? P.thr[tid - 5] : 0u;
     if (do_hist)
-        for (uint32_t n = tid; n < hist_words(P.q); n += nthreads) s_hist[n] = 0u;
+        for (uint32_t n = tid; n < 2u * hist_words(P.q); n += nthreads) s_hist0[n] = 0u;
     {
         const int vpr = pitch >> 4;
         for (int c = 0; c < 2; ++c)
@@ -79,6 +80,7 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
             const HalfSweepKeys K = half_sweep_keys(P.key0, P.key1, t, c);
             const bool count_E = sample && c == 1 && do_E, count_H = sample && do_hist;
             uint32_t nef_sum = 0, words_done = 0;
+            uint32_t *const s_hist = s_hist0 + (sample_idx & 1u) * hist_words(P.q);
             if (is_compute)
                 for (int lr = 1 + ty; lr <= rows; lr += tyc) {
                     const uint32_t ro = (uint32_t)(lr * pitch);
@@ -110,10 +112,8 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
             }
             cluster.sync();                                         // plane c and its halos complete everywhere
             if (sample && c == 1) {
-                if (do_hist) {
-                    hist_flush(s_hist, P.q, P.hist_series + (size_t)sample_idx * P.q, tid, nthreads);
-                    __syncthreads();
-                }
+                // no barrier after the flush: the next sample counts into the other table
+                if (do_hist) hist_flush(s_hist, P.q, P.hist_series + (size_t)sample_idx * P.q, tid, nthreads);
                 ++sample_idx;
             }
         }
