@@ -984,11 +984,12 @@ struct BatchPlan { bool ok = false; int tyc = 0, nthreads = 0; size_t smem = 0; 
 BatchPlan plan_batch(int32_t L, int32_t q, size_t smem_optin)
 {
     BatchPlan R;
-    const int cpr = L / 16, comm = (cpr + 31) / 32 * 32;
-    int tyc = (1024 - comm) / cpr;
+    const int wpr = L / 8, comm = (L / 16 + 31) / 32 * 32;         // one 4-site word per compute thread and row visit
+    int tyc = (1024 - comm) / wpr;
     if (tyc > L) tyc = L;
+    if (tyc < 1) { R.why = "no room for a compute row in a 1024-thread block"; return R; }
     R.tyc = tyc;
-    R.nthreads = (cpr * tyc + 31) / 32 * 32 + comm;
+    R.nthreads = (wpr * tyc + 31) / 32 * 32 + comm;
     if ((L + tyc - 1) / tyc > 30) { R.why = "too many rows per thread"; return R; }
     const size_t hist = (size_t)(q <= (int)potts::HIST_LANE_QMAX ? q * 32 : q) * 4;
     R.smem = 2 * (size_t)(L + 2) * (L / 2) + hist;

@@ -355,7 +355,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_batch_u8(const __grid_cons
     for (int d = 0; d < 4; ++d) X.thr[d] = T.thr[r][d];
     X.E_series = B.P.E_series ? B.P.E_series + r * B.series_stride : nullptr;
     X.hist_series = B.P.hist_series ? B.P.hist_series + r * B.series_stride * B.P.q : nullptr;
-    resident_run<CM, 2, ST>(B.P, X);
+    resident_run<CM, 1, ST>(B.P, X);      // one word per thread and row visit: small lattices want warps, not amortisation
 }
 
 }  // namespace potts
