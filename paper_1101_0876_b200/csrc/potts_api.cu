@@ -450,6 +450,7 @@ int launch_cluster(potts_t *h, const ClusterPlan &R, const uint32_t thr[4], int6
     default: fn = cluster_kernel_cm<potts::CM_NIB3>(h->stream_spec); break;
     }
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
+    if (R.G > 8) CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)R.G);
     cfg.blockDim = dim3((unsigned)R.nthreads);

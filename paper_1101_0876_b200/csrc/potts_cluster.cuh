@@ -1,7 +1,7 @@
 // potts_cluster.cuh -- tiny lattices: one thread-block cluster, boundary rows through distributed shared memory.
 //
 // A lattice of L <= 256 is a few thousand words: the resident kernel's L2 packets (~1 us per half-sweep of flight and
-// polling) cost more than the update itself.  Here the whole lattice lives in the shared memory of ONE cluster of up to 8
+// polling) cost more than the update itself.  Here the whole lattice lives in the shared memory of ONE cluster of up to 16
 // CTAs (CTA b owns rows [bL/G, (b+1)L/G) of both planes, plus one halo row above and below per plane); the thread that
 // updates a word of a boundary row also stores it straight into the neighbour CTA's halo row (DSMEM,
 // cluster.map_shared_rank), and one hardware cluster barrier per half-sweep is the only synchronisation: no polling, no
@@ -16,7 +16,7 @@
 
 namespace potts {
 
-constexpr int CLUSTER_MAX = 8;      // portable cluster size
+constexpr int CLUSTER_MAX = 16;     // 8 is the portable cluster size; B200 takes 16 with the non-portable attribute
 
 // Block = wpr x tyc threads (wpr = L/8 words per plane row); thread (tx, ty) updates word tx of local rows
 // 1+ty, 1+ty+tyc, ...  P.inbox and P.error are unused.

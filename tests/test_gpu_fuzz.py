@@ -36,7 +36,7 @@ def _cases(n, seed):
             variant = int(rng.choice([1, 2, 2, 2, 3, 0]))
             shape["variant"] = variant
             if variant == 3:
-                shape["cluster_ctas"] = int(rng.choice([0, 1, 2, 3, 5, 8]))
+                shape["cluster_ctas"] = int(rng.choice([0, 1, 2, 3, 5, 8, 11, 16]))
             if variant == 2:
                 shape["resident_ctas"] = int(rng.choice([0, 1, 2, 3, 5, 8, 13, 31, 64, 148]))
                 shape["resident_words"] = int(rng.choice([0, 1, 2]))

@@ -41,6 +41,7 @@ LAUNCH_SHAPES = {
     "cluster1": {"variant": 3, "cluster_ctas": 1},
     "cluster3": {"variant": 3, "cluster_ctas": 3},
     "cluster8": {"variant": 3, "cluster_ctas": 8},
+    "cluster16": {"variant": 3, "cluster_ctas": 16},             # beyond the portable cluster size
     "auto": {"variant": 0},
 }
 
@@ -97,7 +98,7 @@ def test_cfg1_full_run_series_and_spins(pb, shape):
     (512, 9, workloads.INIT_RANDOM, 0.995, 5),      # many blocks
 ])
 @pytest.mark.parametrize("shape", ["streaming", "resident", "resident1", "resident3", "resident148", "resident_w1",
-                                   "resident_w1_5", "resident_w2", "cluster", "cluster1", "cluster3", "cluster8", "auto"])
+                                   "resident_w1_5", "resident_w2", "cluster", "cluster1", "cluster3", "cluster8", "cluster16", "auto"])
 def test_every_sweep_spins_energy_histogram(pb, L, q, init, f, seed, shape):
     g, o = _pair(pb, L, q, seed, init, shape=shape)
     T = f * workloads.t_c(q)
