@@ -183,6 +183,7 @@ int potts_launch_count(potts_t *h, uint64_t *n);
  *   "cluster_ctas"     0 = automatic, else the cluster size (1..16); "cluster_active" (read-only) = the cluster
  *                      size the next sweep call would use, 0 if it would not use the cluster kernel
  *   "resident_ctas"    0 = automatic, else the number of CTAs the resident kernel splits the rows over
+ *   "resident_rows"    0 = automatic, else at most this many thread rows in a resident block
  *   "resident_words"   0 = automatic, 1 / 2 = 4-site words a resident thread updates per row visit
  *   "resident_active"  read-only: CTAs the next sweep call would run resident on (0 = streaming) */
 int potts_set_option(potts_t *h, const char *key, int64_t value);

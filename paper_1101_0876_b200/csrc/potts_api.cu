@@ -69,6 +69,7 @@ struct potts_s {
     int64_t opt_variant = 0;             // 0 auto, 1 streaming (one launch per half-sweep), 2 resident
     int64_t opt_resident_ctas = 0;       // 0 auto, else the resident kernel's grid size
     int64_t opt_resident_words = 0;      // 0 auto, 1 / 2: 4-site words per thread and row visit
+    int64_t opt_resident_rows = 0;       // 0 auto, else at most this many thread rows in a resident block
     int64_t opt_cluster_ctas = 0;        // 0 auto, else the cluster kernel's cluster size (1..8)
 };
 
@@ -320,6 +321,24 @@ ResidentPlan plan_resident(const potts_t *h)
             tyc = t1;
         }
     }
+    if (R.W == 2 && h->opt_resident_rows == 0) {
+        // thread rows for the chunk-grained kernel: fewer rows than fit can be better, because the last visit of an
+        // uneven deal idles part of the block and blocks above 768 threads are held to 64 registers.  Cost model fitted
+        // to the measurements in profiles/r01c_kernels.md (L = 2048: 3 rows, L = 4096: 2 rows).
+        double best = 1e30;
+        int best_t = tyc;
+        for (int t = tyc; t >= 1; --t) {
+            const int visits = (R.rows_max + t - 1) / t;
+            const int threads = (cpr * t + 31) / 32 * 32 + comm, warps = cpr * t / 32;
+            double cost = (double)visits * t / R.rows_max;
+            if (threads > 768) cost *= 1.08;
+            if (warps < 12) cost *= 1.0 + 0.025 * (12 - warps);
+            if (visits > 30) continue;
+            if (cost < best - 1e-9) { best = cost; best_t = t; }
+        }
+        tyc = best_t;
+    }
+    if (h->opt_resident_rows > 0 && h->opt_resident_rows < tyc) tyc = (int)h->opt_resident_rows;
     R.tyc = tyc;
     R.nthreads = (threads_per_row * tyc + 31) / 32 * 32 + comm;
     if ((R.rows_max + tyc - 1) / tyc > 30) { R.why = "too many rows per thread"; return R; }
@@ -330,21 +349,22 @@ ResidentPlan plan_resident(const potts_t *h)
     return R;
 }
 
-// register budget: 112 per thread for blocks up to 576 threads, else 64
+// register budget: 112 per thread for blocks up to 576 threads, 80 up to 768, else 64
 template <int CM, int ST>
-const void *resident_kernel_st(int W, bool small)
+const void *resident_kernel_st(int W, int small)
 {
-    if (W == 1) return small ? (const void *)potts::k_resident_u8<CM, 1, ST, 576> : (const void *)potts::k_resident_u8<CM, 1, ST, 1024>;
-    return small ? (const void *)potts::k_resident_u8<CM, 2, ST, 576> : (const void *)potts::k_resident_u8<CM, 2, ST, 1024>;
+    if (W == 1) return small == 2 ? (const void *)potts::k_resident_u8<CM, 1, ST, 576> : (const void *)potts::k_resident_u8<CM, 1, ST, 1024>;
+    return small == 2 ? (const void *)potts::k_resident_u8<CM, 2, ST, 576>
+                      : (small == 1 ? (const void *)potts::k_resident_u8<CM, 2, ST, 768> : (const void *)potts::k_resident_u8<CM, 2, ST, 1024>);
 }
 
 template <int CM>
-const void *resident_kernel_cm(int stream_spec, int W, bool small)
+const void *resident_kernel_cm(int stream_spec, int W, int small)
 {
     return stream_spec == 2 ? resident_kernel_st<CM, 2>(W, small) : resident_kernel_st<CM, 1>(W, small);
 }
 
-const void *resident_kernel(int cm, int stream_spec, int W, bool small)
+const void *resident_kernel(int cm, int stream_spec, int W, int small)
 {
     switch (cm) {
     case potts::CM_7BIT: return resident_kernel_cm<potts::CM_7BIT>(stream_spec, W, small);
@@ -375,7 +395,7 @@ int launch_resident(potts_t *h, const ResidentPlan &R, const uint32_t thr[4], in
     P.error = h->error;
     P.rows_max = R.rows_max;
     P.tyc = R.tyc;
-    const void *fn = resident_kernel(potts::compare_mode_of(h->q), h->stream_spec, R.W, R.nthreads <= 576);
+    const void *fn = resident_kernel(potts::compare_mode_of(h->q), h->stream_spec, R.W, R.nthreads <= 576 ? 2 : (R.nthreads <= 768 ? 1 : 0));
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
     int per_sm = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, R.nthreads, R.smem));
@@ -892,6 +912,10 @@ int potts_set_option(potts_t *h, const char *key, int64_t value)
         if (value < 0 || value > potts::CLUSTER_MAX) return fail(POTTS_ERR_ARG, "cluster_ctas must be in [0, %d]", potts::CLUSTER_MAX);
         h->opt_cluster_ctas = value; return POTTS_OK;
     }
+    if (!std::strcmp(key, "resident_rows")) {
+        if (value < 0 || value > 1024) return fail(POTTS_ERR_ARG, "resident_rows must be in [0, 1024]");
+        h->opt_resident_rows = value; return POTTS_OK;
+    }
     if (!std::strcmp(key, "resident_words")) {
         if (value < 0 || value > 2) return fail(POTTS_ERR_ARG, "resident_words must be 0 (auto), 1 or 2");
         h->opt_resident_words = value; return POTTS_OK;
@@ -905,6 +929,7 @@ int potts_get_option(potts_t *h, const char *key, int64_t *value)
     if (!std::strcmp(key, "variant")) { *value = h->opt_variant; return POTTS_OK; }
     if (!std::strcmp(key, "resident_ctas")) { *value = h->opt_resident_ctas; return POTTS_OK; }
     if (!std::strcmp(key, "resident_words")) { *value = h->opt_resident_words; return POTTS_OK; }
+    if (!std::strcmp(key, "resident_rows")) { *value = h->opt_resident_rows; return POTTS_OK; }
     if (!std::strcmp(key, "cluster_ctas")) { *value = h->opt_cluster_ctas; return POTTS_OK; }
     if (!std::strcmp(key, "cluster_active")) {             // read-only: cluster size the next sweep call would use (0 = not the cluster kernel)
         const bool want = h->opt_variant == 3 || (h->opt_variant == 0 && h->layout == POTTS_LAYOUT_U8 && h->L <= CLUSTER_AUTO_L_MAX);
