@@ -47,8 +47,8 @@ MEASURED_INT_ISSUE_PER_CLK = 0.5
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for the workload)
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {          # profiles/r01c_kernels.md
-    "cfg2_q6_L1024": 1.117e6 + 4.9e3,      # resident kernel: the lattice is loaded once per launch, whatever the sweep count
-    "cfg3_q9_L4096": 17.26e6 + 8.4e3,
+    "cfg2_q6_L1024": 1.113e6 + 5.1e3,      # resident kernel: the lattice is loaded once per launch, whatever the sweep count
+    "cfg3_q9_L4096": 17.30e6 + 8.7e3,
     "cfg4_q24_L8192": 41.98e6 + 1.5e3,     # 40 MB of packed planes, L2-resident after the first touch
     "cfg5_q9_L32768": 1.0738e9 + 0.4973e9,
 }
