@@ -96,6 +96,16 @@ int potts_sweep(potts_t *h, double T, int64_t nsweeps);
 int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every,
                          int64_t *E_series, int64_t *hist_series);
 
+/* potts_sweep_delta: as potts_sweep, and for every sweep of this call record the energy CHANGE of that sweep
+ * accumulated on the fly from the accepted moves, dE = sum of d = n_old - n_new over accepted updates of both
+ * colours, without recounting the energy over the lattice -- the "parallel accumulation of local
+ * energy changes on-the-fly" that PAPER.md:361-363 proposes for reweighting / histogram techniques.  By Eq. 1
+ * E(after sweep n) = E(before) + dE_series[n]; the tests check exactly that against the oracle's
+ * recounted energies.  dE_series: caller-owned HOST buffer of nsweeps int64.  U8 layout only
+ * (POTTS_ERR_UNSUPPORTED otherwise); always one launch per half-sweep (k_half_sweep_delta_u8).  Synchronises;
+ * dE_series is untouched on error. */
+int potts_sweep_delta(potts_t *h, double T, int64_t nsweeps, int64_t *dE_series);
+
 /* Same, with E_series / hist_series in DEVICE memory; enqueues and returns without a sync. */
 int potts_sweep_measured_dev(potts_t *h, double T, int64_t nsweeps, int64_t every,
                              int64_t *E_series_dev, int64_t *hist_series_dev);

@@ -50,6 +50,7 @@ def load_library() -> ctypes.CDLL:
         "potts_sweep": ([vp, dbl, i64], ctypes.c_int),
         "potts_sweep_measured": ([vp, dbl, i64, i64, vp, vp], ctypes.c_int),
         "potts_sweep_measured_dev": ([vp, dbl, i64, i64, vp, vp], ctypes.c_int),
+        "potts_sweep_delta": ([vp, dbl, i64, vp], ctypes.c_int),
         "potts_ladder": ([vp, vp, i32, i64, i64, i64, vp, vp], ctypes.c_int),
         "potts_batch_workspace_bytes": ([i32, i32, i32, P(ctypes.c_size_t)], ctypes.c_int),
         "potts_batch_create": ([P(vp), i32, i32, i32, vp, i32, vp, ctypes.c_size_t, vp], ctypes.c_int),
@@ -85,7 +86,7 @@ def load_library() -> ctypes.CDLL:
 
 EXPORTED_SYMBOLS = [
     "potts_create", "potts_create_ex", "potts_workspace_bytes", "potts_set_stream", "potts_destroy",
-    "potts_sweep", "potts_sweep_measured", "potts_sweep_measured_dev", "potts_ladder", "potts_energy", "potts_histogram",
+    "potts_sweep", "potts_sweep_measured", "potts_sweep_measured_dev", "potts_sweep_delta", "potts_ladder", "potts_energy", "potts_histogram",
     "potts_download", "potts_upload", "potts_sweep_count", "potts_set_sweep_count", "potts_observables",
     "potts_magnetisation", "potts_launch_count", "potts_set_option", "potts_get_option", "potts_last_error",
     "potts_version", "potts_batch_workspace_bytes", "potts_batch_create", "potts_batch_destroy",
@@ -191,6 +192,13 @@ class Potts:
             self._h, float(T), int(nsweeps), int(every),
             ctypes.c_void_p(E_dev.data_ptr()) if E_dev is not None else None,
             ctypes.c_void_p(hist_dev.data_ptr()) if hist_dev is not None else None))
+
+    def potts_sweep_delta(self, T: float, nsweeps: int) -> np.ndarray:
+        """-> dE int64[nsweeps] on the host: the energy change of each sweep summed over its accepted moves."""
+        self._sync_stream()
+        dE = np.zeros(int(nsweeps), dtype=np.int64)
+        _check(self._lib.potts_sweep_delta(self._h, float(T), int(nsweeps), dE.ctypes.data))
+        return dE
 
     def potts_ladder(self, temperatures, t_tran: int, t_max: int, dt: int, hist: bool = True):
         """-> (E int64[nT, t_max/dt], hist int64[nT, t_max/dt, q] or None) on the host."""

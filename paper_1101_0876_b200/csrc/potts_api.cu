@@ -193,6 +193,30 @@ int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsign
     return check_launch(h, "k_half_sweep_u8");
 }
 
+template <int CM>
+void launch_hs_delta_cm(int stream_spec, const potts::SweepParams &P, dim3 grid, cudaStream_t st, unsigned long long *dE_out)
+{
+    if (stream_spec == 2) potts::k_half_sweep_delta_u8<CM, 2><<<grid, dim3(32, potts::HS_WARPS), 0, st>>>(P, dE_out);
+    else potts::k_half_sweep_delta_u8<CM, 1><<<grid, dim3(32, potts::HS_WARPS), 0, st>>>(P, dE_out);
+}
+
+// half-sweep that adds the sum of the accepted moves' d to *dE_out (U8 layout)
+int launch_half_sweep_delta(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *dE_out)
+{
+    potts::SweepParams P = sweep_params(h, colour, thr, nullptr);
+    P.hist_out = nullptr;
+    P.rpt = 1;
+    const int chunks = h->L / 32;
+    const dim3 grid((unsigned)((chunks + 31) / 32), (unsigned)(h->L / potts::HS_WARPS));
+    switch (potts::compare_mode_of(h->q)) {
+    case potts::CM_7BIT: launch_hs_delta_cm<potts::CM_7BIT>(h->stream_spec, P, grid, h->stream, dE_out); break;
+    case potts::CM_8BIT: launch_hs_delta_cm<potts::CM_8BIT>(h->stream_spec, P, grid, h->stream, dE_out); break;
+    case potts::CM_NIB4: launch_hs_delta_cm<potts::CM_NIB4>(h->stream_spec, P, grid, h->stream, dE_out); break;
+    default: launch_hs_delta_cm<potts::CM_NIB3>(h->stream_spec, P, grid, h->stream, dE_out); break;
+    }
+    return check_launch(h, "k_half_sweep_delta_u8");
+}
+
 template <bool FIVE, bool MEASURE, bool HIST>
 void launch_pk(int stream_spec, const potts::PackedSweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
 {
@@ -731,6 +755,35 @@ int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every, i
     if (e != cudaSuccess || e2 != cudaSuccess)
         return fail(POTTS_ERR_CUDA, "series copy/sync failed: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
     return check_device_error(h);
+}
+
+int potts_sweep_delta(potts_t *h, double T, int64_t nsweeps, int64_t *dE_series)
+{
+    int rc = check_sweep_args(h, T, nsweeps);
+    if (rc) return rc;
+    if (!dE_series) return fail(POTTS_ERR_ARG, "null dE_series");
+    if (h->layout != POTTS_LAYOUT_U8) return fail(POTTS_ERR_UNSUPPORTED, "potts_sweep_delta needs the U8 layout");
+    if (nsweeps == 0) return POTTS_OK;
+    uint32_t thr[4];
+    thresholds(T, thr);
+    uint8_t *dev = nullptr;
+    rc = get_scratch(h, (size_t)nsweeps * 8, &dev);
+    if (rc) return rc;
+    unsigned long long *d = (unsigned long long *)dev;
+    CUDA_TRY(cudaMemsetAsync(d, 0, (size_t)nsweeps * 8, h->stream));
+    for (int64_t n = 0; n < nsweeps; ++n) {
+        rc = launch_half_sweep_delta(h, 0u, thr, d + n);
+        if (rc == POTTS_OK) rc = launch_half_sweep_delta(h, 1u, thr, d + n);
+        if (rc) break;
+        h->t += 1;
+    }
+    cudaError_t e = cudaSuccess;
+    if (rc == POTTS_OK) e = cudaMemcpyAsync(dE_series, d, (size_t)nsweeps * 8, cudaMemcpyDeviceToHost, h->stream);
+    cudaError_t e2 = cudaStreamSynchronize(h->stream);
+    if (rc) return rc;
+    if (e != cudaSuccess || e2 != cudaSuccess)
+        return fail(POTTS_ERR_CUDA, "series copy/sync failed: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
+    return POTTS_OK;
 }
 
 int potts_ladder(potts_t *h, const double *T, int32_t nT, int64_t t_tran, int64_t t_max, int64_t dt, int64_t *E_series,

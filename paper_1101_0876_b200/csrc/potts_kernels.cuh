@@ -101,6 +101,65 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_u8(const __grid_co
 }
 
 // ---------------------------------------------------------------------------------------------
+// Half-sweep with the on-the-fly energy change ("keeping track of the energy changes at
+// each spin flip ... a parallel accumulation of local energy changes on-the-fly" for reweighting runs):
+// adds  sum over accepted moves of d = n_old - n_new  (R5, R7) of this half-sweep to *dE_out, as a
+// two's-complement int64.  No energy recount: per site d_accepted = ne(final spin) - ne(old spin), where ne is
+// the count of unequal neighbours, so the half-sweep's sum is byte_sum(ne_final) - byte_sum(ne_old).
+// Same thread map as k_half_sweep_u8 with one row per thread; a separate kernel so that the plain path's code
+// generation is untouched.
+template <int CM, int ST>
+__global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_delta_u8(const __grid_constant__ SweepParams P,
+                                                                       unsigned long long *dE_out)
+{
+    __shared__ uint32_t lut[12];
+    __shared__ int blockD;
+    const uint32_t tid = threadIdx.y * 32u + threadIdx.x;
+    if (tid < 9) lut[tid] = tid >= 5 ? P.thr[tid - 5] : 0u;
+    if (tid == 0) blockD = 0;
+    __syncthreads();
+
+    const int chunks = P.pitch >> 4;
+    const int x = (int)(blockIdx.x * 32u + threadIdx.x);
+    const int i = (int)(blockIdx.y * HS_WARPS + threadIdx.y);
+    int delta = 0;                                                     // |delta| <= 4 * 16 per thread
+    if (x < chunks) {
+        const int k0 = x << 4;
+        const HalfSweepKeys &K = P.K;
+        const uint32_t q = in_register(P.q);
+        const int kn = wrap(k0 + 16, P.pitch), kp = wrap(k0 - 4, P.pitch);
+        const uint32_t p = (uint32_t)(i + P.colour) & 1u;
+        const int iu = wrap(i - 1, P.L), id = wrap(i + 1, P.L);
+        const size_t row = (size_t)i * P.pitch;
+        const uint4 own4 = *reinterpret_cast<const uint4 *>(P.plane_own + row + k0);
+        const uint4 mid4 = *reinterpret_cast<const uint4 *>(P.plane_oth + row + k0);
+        const uint4 up4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)iu * P.pitch + k0);
+        const uint4 dn4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)id * P.pitch + k0);
+        const uint32_t adj = *reinterpret_cast<const uint32_t *>(P.plane_oth + row + (p ? kn : kp));
+        const RowKeys R = row_keys(K, (uint32_t)i);
+        const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
+        const uint32_t mid[6] = {adj, mid4.x, mid4.y, mid4.z, mid4.w, adj};
+        const uint32_t up[4] = {up4.x, up4.y, up4.z, up4.w};
+        const uint32_t dn[4] = {dn4.x, dn4.y, dn4.z, dn4.w};
+        uint32_t out[4];
+#pragma unroll
+        for (int n = 0; n < 4; ++n) {
+            uint32_t lf, rt, nef, ne_old, unused;
+            horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
+            ne_counts<CM>(own[n], own[n], up[n], dn[n], lf, rt, ne_old, unused);
+            out[n] = update_word<CM, ST>(own[n], up[n], dn[n], lf, rt, 2u * (uint32_t)(k0 + 4 * n) + p, q, K, R, lut, nef);
+            delta += (int)byte_sum(nef) - (int)byte_sum(ne_old);
+        }
+        *reinterpret_cast<uint4 *>(P.plane_own + row + k0) = make_uint4(out[0], out[1], out[2], out[3]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) delta += __shfl_xor_sync(0xffffffffu, delta, o);
+    if (threadIdx.x == 0) atomicAdd(&blockD, delta);
+    __syncthreads();
+    if (tid == 0) atomicAdd(dE_out, (unsigned long long)(long long)blockD);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Standalone measurement: energy from the black plane's sites (every bond joins a black and a
 // white site, so summing equal neighbours over black sites counts each bond once) and the
 // histogram of both planes.  One thread per 16-byte chunk of the black plane; the white chunk

@@ -1,0 +1,96 @@
+"""GPU parity of potts_sweep_delta (-m gpu): the per-sweep energy change accumulated on the fly from the accepted
+moves against the oracle.
+
+The oracle RECOUNTS Eq. 1 over the whole lattice after every sweep, so
+E0 + cumsum(dE_gpu) == E_oracle is a comparison of two different computations of the same integers: it fails
+if a single accepted move's d is dropped, double counted or has the wrong sign.  Spins must stay identical too
+(the delta kernel is one more launch shape of the same chain, P6).
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pb():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests selected but no CUDA device is visible")
+    import paper_1101_0876_b200 as pb
+    pb.load_library()
+    return pb
+
+
+# (L, q, seed, init, T / T_c, sweeps): every compare mode (q <= 8, <= 16, <= 128, <= 256), several tiles and a
+# ragged last warp (L = 96, 160), ordered and random starts, both sides of T_c
+CASES = [
+    (32, 2, 11, 1, 0.9, 40),
+    (64, 9, 1, 1, 0.99, 60),
+    (96, 6, 7, 0, 1.005, 40),
+    (160, 24, 4, 1, 1.002, 25),
+    (256, 15, 5, 1, 0.5, 20),
+    (128, 200, 9, 1, 1.3, 20),
+    (1088, 9, 3, 1, 0.995, 6),
+]
+
+
+@pytest.mark.parametrize("stream", [1, 2])
+@pytest.mark.parametrize("L,q,seed,init,f,n", CASES)
+def test_delta_series_matches_recounted_energy(pb, L, q, seed, init, f, n, stream):
+    T = f * workloads.t_c(q)
+    g = pb.Potts(L, q, seed, init)
+    g.potts_set_stream_spec(stream)
+    o = oracle.OraclePotts(L, q, seed, init, threads=4, stream=stream)
+    E0 = o.energy()
+    assert g.potts_energy() == E0
+    dE = g.potts_sweep_delta(T, n)
+    Eo, _ = o.sweep_measured(T, n, 1, hist=False)
+    assert dE.dtype == np.int64 and dE.shape == (n,)
+    assert (E0 + np.cumsum(dE) == Eo).all()
+    assert (g.potts_download() == o.spins()).all()
+    assert g.potts_energy() == int(Eo[-1]) == o.energy_incremental()
+    assert g.potts_sweep_count() == o.t == n
+
+
+def test_delta_is_the_same_chain_as_the_other_launch_shapes(pb):
+    """sweep(a); sweep_delta(b); sweep_measured(c) is the chain of sweep(a+b+c) (sweep counter lives in the handle)."""
+    L, q, seed = 128, 9, 21
+    T = 0.99 * workloads.t_c(q)
+    g = pb.Potts(L, q, seed, pb.INIT_RANDOM)
+    o = oracle.OraclePotts(L, q, seed, pb.INIT_RANDOM)
+    g.potts_sweep(T, 7)
+    Eo, _ = o.sweep_measured(T, 7, 1, hist=False)
+    dE = g.potts_sweep_delta(T, 9)
+    Eo2, _ = o.sweep_measured(T, 9, 1, hist=False)
+    assert (int(Eo[-1]) + np.cumsum(dE) == Eo2).all()
+    Eg3, _ = g.potts_sweep_measured(T, 5, 1, hist=False)
+    Eo3, _ = o.sweep_measured(T, 5, 1, hist=False)
+    assert (Eg3 == Eo3).all()
+    assert (g.potts_download() == o.spins()).all()
+
+
+def test_delta_degenerate_temperatures(pb):
+    """P7: at T -> 0+ only d <= 0 is accepted: every dE <= 0, and the ordered state never moves."""
+    g = pb.Potts(64, 6, 3, pb.INIT_RANDOM)
+    dE = g.potts_sweep_delta(0.01, 30)
+    assert (dE <= 0).all() and dE[0] < 0
+    g = pb.Potts(64, 6, 3, pb.INIT_ORDERED)
+    assert (g.potts_sweep_delta(0.01, 5) == 0).all()
+    assert g.potts_energy() == -2 * 64 * 64
+
+
+def test_delta_arguments(pb):
+    g = pb.Potts(64, 24, 1, pb.INIT_RANDOM, layout=pb.LAYOUT_PACKED)
+    with pytest.raises(pb.PottsError) as e:
+        g.potts_sweep_delta(1.0, 1)
+    assert e.value.code == pb.ERR_UNSUPPORTED
+    g = pb.Potts(64, 9, 1, pb.INIT_RANDOM)
+    with pytest.raises(pb.PottsError) as e:
+        g.potts_sweep_delta(-1.0, 1)
+    assert e.value.code == pb.ERR_ARG
+    assert g.potts_sweep_delta(1.0, 0).shape == (0,)
+    assert g.potts_sweep_count() == 0
