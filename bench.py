@@ -402,6 +402,31 @@ def batch_of_cfg1(pb, torch, n=1184):
             "ns_per_spin_flip": 1e9 / ups, "kernel": "k_resident_batch_u8", "E_last_of_sample_0": int(E[0, -1])}
 
 
+def delta_stream_cost(pb, torch, sweeps=20):
+    """SURVEY 8(f)4 / PAPER.md:361-363: cost of accumulating the energy change of every sweep on the fly
+    (potts_sweep_delta, k_half_sweep_delta_u8) against the plain streaming half-sweep (variant 1, no measurement)
+    on BASELINE configs[4]'s shape (q=9, L=32768).  CUDA events around the calls; the delta call includes the
+    copy of its series to the host."""
+    w = workloads.CONFIGS[5]
+    T = w.temperatures[0]
+    out = {"q": w.q, "L": w.L, "sweeps": sweeps}
+    for name in ("plain", "delta"):
+        g = pb.Potts(w.L, w.q, w.seed, w.init)
+        g.potts_set_option("variant", 1)
+        step = (lambda n: g.potts_sweep(T, n)) if name == "plain" else (lambda n: g.potts_sweep_delta(T, n))
+        step(3)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        step(sweeps)
+        e1.record()
+        torch.cuda.synchronize()
+        out[name + "_ns_per_spin_flip"] = e0.elapsed_time(e1) * 1e6 / (sweeps * w.L * w.L)
+        g.close()
+    out["delta_over_plain"] = out["delta_ns_per_spin_flip"] / out["plain_ns_per_spin_flip"]
+    return out
+
+
 # ---- main -----------------------------------------------------------------------------------------
 def main():
     ap = argparse.ArgumentParser()
@@ -477,6 +502,7 @@ def main():
         per_cfg = per_config_table(pb, torch, flush, sm_max, hbm_gbs, which)
         e6 = paper_protocol_e6(pb, torch)
         per_cfg["batch_cfg1_x1184"] = batch_of_cfg1(pb, torch)
+        per_cfg["delta_stream_cfg5"] = delta_stream_cost(pb, torch)
         # SURVEY 8(f)1, NOT the headline chain: the same workloads under stream-spec v2 (one Philox block per pair of
         # sites, S15); its algorithmic instruction count is 19 per update, so alu_frac is not comparable
         v2 = per_config_table(pb, torch, flush, sm_max, hbm_gbs, which, skip=(1,), stream_spec=2)

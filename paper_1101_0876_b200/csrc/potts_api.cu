@@ -205,9 +205,12 @@ int launch_half_sweep_delta(potts_t *h, uint32_t colour, const uint32_t thr[4], 
 {
     potts::SweepParams P = sweep_params(h, colour, thr, nullptr);
     P.hist_out = nullptr;
-    P.rpt = 1;
     const int chunks = h->L / 32;
-    const dim3 grid((unsigned)((chunks + 31) / 32), (unsigned)(h->L / potts::HS_WARPS));
+    const unsigned gx = (unsigned)((chunks + 31) / 32);
+    int rpt = 8;                                     // as launch_half_sweep
+    while (rpt > 1 && (long long)gx * (h->L / (potts::HS_WARPS * rpt)) < 8ll * h->num_sms) rpt >>= 1;
+    P.rpt = rpt;
+    const dim3 grid(gx, (unsigned)(h->L / (potts::HS_WARPS * rpt)));
     switch (potts::compare_mode_of(h->q)) {
     case potts::CM_7BIT: launch_hs_delta_cm<potts::CM_7BIT>(h->stream_spec, P, grid, h->stream, dE_out); break;
     case potts::CM_8BIT: launch_hs_delta_cm<potts::CM_8BIT>(h->stream_spec, P, grid, h->stream, dE_out); break;

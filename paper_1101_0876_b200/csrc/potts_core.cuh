@@ -239,11 +239,12 @@ __device__ __forceinline__ void horizontal(uint32_t p, uint32_t mid, uint32_t ad
 //   up,dn,lf,rt  the 4 neighbour words, byte b = that neighbour of site b
 //   j0           column of byte 0 (columns advance by 2 per byte)
 //   lut          shared memory, 9 words: lut[d+4] = floor(2^32 exp(-d/T)) for d = 1..4 (entries 0..4 unused)
-// Returns the new word; ne_final = per-byte count of unequal neighbours of the final spins.
+// Returns the new word; ne_final = per-byte count of unequal neighbours of the final spins, ne_old = the same of
+// the spins before the update (so that, per byte, ne_final - ne_old = d of an accepted move and 0 otherwise).
 template <int CM, int ST>     // ST: random-stream definition, 1 = one Philox block per site (R3), 2 = per pair (R3')
-__device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
-                                                uint32_t j0, uint32_t q, const HalfSweepKeys &K, const RowKeys &R,
-                                                const uint32_t *lut, uint32_t &ne_final)
+__device__ __forceinline__ uint32_t update_word_ex(uint32_t own, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
+                                                   uint32_t j0, uint32_t q, const HalfSweepKeys &K, const RowKeys &R,
+                                                   const uint32_t *lut, uint32_t &ne_final, uint32_t &ne_old)
 {
     uint32_t w0[4], w1[4];
     if (ST == 1) {
@@ -277,7 +278,17 @@ __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint3
         if (w1[b] < thr) mask |= 0xffu << (8 * b);
     }
     ne_final = (c_new & mask) | (c_old & ~mask);
+    ne_old = c_old;
     return (prop & mask) | (own & ~mask);                           // R7
+}
+
+template <int CM, int ST>
+__device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
+                                                uint32_t j0, uint32_t q, const HalfSweepKeys &K, const RowKeys &R,
+                                                const uint32_t *lut, uint32_t &ne_final)
+{
+    uint32_t ne_old;
+    return update_word_ex<CM, ST>(own, up, dn, lf, rt, j0, q, K, R, lut, ne_final, ne_old);
 }
 
 // ---------------------------------------------------------------------------------------------

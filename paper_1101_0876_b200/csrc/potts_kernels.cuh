@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_u8(const __grid_co
 // adds  sum over accepted moves of d = n_old - n_new  (R5, R7) of this half-sweep to *dE_out, as a
 // two's-complement int64.  No energy recount: per site d_accepted = ne(final spin) - ne(old spin), where ne is
 // the count of unequal neighbours, so the half-sweep's sum is byte_sum(ne_final) - byte_sum(ne_old).
-// Same thread map as k_half_sweep_u8 with one row per thread; a separate kernel so that the plain path's code
+// Same thread map as k_half_sweep_u8 (P.rpt rows per thread); a separate kernel so that the plain path's code
 // generation is untouched.
 template <int CM, int ST>
 __global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_delta_u8(const __grid_constant__ SweepParams P,
@@ -121,36 +121,40 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_delta_u8(const __g
 
     const int chunks = P.pitch >> 4;
     const int x = (int)(blockIdx.x * 32u + threadIdx.x);
-    const int i = (int)(blockIdx.y * HS_WARPS + threadIdx.y);
-    int delta = 0;                                                     // |delta| <= 4 * 16 per thread
+    const int i0 = (int)(blockIdx.y * HS_WARPS + threadIdx.y) * P.rpt;
+    int delta = 0;                                                     // |delta| <= 4 * 16 * rpt per thread
     if (x < chunks) {
         const int k0 = x << 4;
         const HalfSweepKeys &K = P.K;
         const uint32_t q = in_register(P.q);
         const int kn = wrap(k0 + 16, P.pitch), kp = wrap(k0 - 4, P.pitch);
-        const uint32_t p = (uint32_t)(i + P.colour) & 1u;
-        const int iu = wrap(i - 1, P.L), id = wrap(i + 1, P.L);
-        const size_t row = (size_t)i * P.pitch;
-        const uint4 own4 = *reinterpret_cast<const uint4 *>(P.plane_own + row + k0);
-        const uint4 mid4 = *reinterpret_cast<const uint4 *>(P.plane_oth + row + k0);
-        const uint4 up4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)iu * P.pitch + k0);
-        const uint4 dn4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)id * P.pitch + k0);
-        const uint32_t adj = *reinterpret_cast<const uint32_t *>(P.plane_oth + row + (p ? kn : kp));
-        const RowKeys R = row_keys(K, (uint32_t)i);
-        const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
-        const uint32_t mid[6] = {adj, mid4.x, mid4.y, mid4.z, mid4.w, adj};
-        const uint32_t up[4] = {up4.x, up4.y, up4.z, up4.w};
-        const uint32_t dn[4] = {dn4.x, dn4.y, dn4.z, dn4.w};
-        uint32_t out[4];
+#pragma unroll 1
+        for (int r = 0; r < P.rpt; ++r) {
+            const int i = i0 + r;
+            const uint32_t p = (uint32_t)(i + P.colour) & 1u;
+            const int iu = wrap(i - 1, P.L), id = wrap(i + 1, P.L);
+            const size_t row = (size_t)i * P.pitch;
+            const uint4 own4 = *reinterpret_cast<const uint4 *>(P.plane_own + row + k0);
+            const uint4 mid4 = *reinterpret_cast<const uint4 *>(P.plane_oth + row + k0);
+            const uint4 up4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)iu * P.pitch + k0);
+            const uint4 dn4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)id * P.pitch + k0);
+            const uint32_t adj = *reinterpret_cast<const uint32_t *>(P.plane_oth + row + (p ? kn : kp));
+            const RowKeys R = row_keys(K, (uint32_t)i);
+            const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
+            const uint32_t mid[6] = {adj, mid4.x, mid4.y, mid4.z, mid4.w, adj};
+            const uint32_t up[4] = {up4.x, up4.y, up4.z, up4.w};
+            const uint32_t dn[4] = {dn4.x, dn4.y, dn4.z, dn4.w};
+            uint32_t out[4], d_sum = 0;
 #pragma unroll
-        for (int n = 0; n < 4; ++n) {
-            uint32_t lf, rt, nef, ne_old, unused;
-            horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
-            ne_counts<CM>(own[n], own[n], up[n], dn[n], lf, rt, ne_old, unused);
-            out[n] = update_word<CM, ST>(own[n], up[n], dn[n], lf, rt, 2u * (uint32_t)(k0 + 4 * n) + p, q, K, R, lut, nef);
-            delta += (int)byte_sum(nef) - (int)byte_sum(ne_old);
+            for (int n = 0; n < 4; ++n) {
+                uint32_t lf, rt, nef, neo;
+                horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
+                out[n] = update_word_ex<CM, ST>(own[n], up[n], dn[n], lf, rt, 2u * (uint32_t)(k0 + 4 * n) + p, q, K, R, lut, nef, neo);
+                d_sum += nef + 0x04040404u - neo;                       // d + 4 per byte; bytes stay <= 32
+            }
+            *reinterpret_cast<uint4 *>(P.plane_own + row + k0) = make_uint4(out[0], out[1], out[2], out[3]);
+            delta += (int)byte_sum(d_sum) - 64;
         }
-        *reinterpret_cast<uint4 *>(P.plane_own + row + k0) = make_uint4(out[0], out[1], out[2], out[3]);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) delta += __shfl_xor_sync(0xffffffffu, delta, o);

@@ -94,3 +94,22 @@ def test_delta_arguments(pb):
     assert e.value.code == pb.ERR_ARG
     assert g.potts_sweep_delta(1.0, 0).shape == (0,)
     assert g.potts_sweep_count() == 0
+
+
+def test_delta_full_size_invariant(pb):
+    """R7 / R8 at BASELINE configs[4]'s size (L = 32768, 2^30 spins), where the oracle cannot follow every sweep:
+    E(0) + sum of the accepted moves' d == the recounted Eq. 1 energy (potts_energy, itself compared with the
+    oracle at this size in test_gpu_fullsize.py), and the chain is the one the plain streaming kernel makes."""
+    w = workloads.CONFIGS[5]
+    T = w.temperatures[0]
+    g = pb.Potts(w.L, w.q, w.seed, w.init)
+    E0 = g.potts_energy()
+    dE = g.potts_sweep_delta(T, 4)
+    assert E0 + int(dE.sum()) == g.potts_energy()
+    assert (dE < 0).all()                                   # cooling a random start below T_c: the energy falls
+    r = pb.Potts(w.L, w.q, w.seed, w.init)
+    r.potts_set_option("variant", 1)
+    Er, _ = r.potts_sweep_measured(T, 4, 1, hist=False)
+    assert (E0 + np.cumsum(dE) == Er).all()
+    h = r.potts_histogram()
+    assert (g.potts_histogram() == h).all() and int(h.sum()) == w.L * w.L
