@@ -101,9 +101,9 @@ int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every,
  * colours, without recounting the energy over the lattice -- the "parallel accumulation of local
  * energy changes on-the-fly" that PAPER.md:361-363 proposes for reweighting / histogram techniques.  By Eq. 1
  * E(after sweep n) = E(before) + dE_series[n]; the tests check exactly that against the oracle's
- * recounted energies.  dE_series: caller-owned HOST buffer of nsweeps int64.  U8 layout only
- * (POTTS_ERR_UNSUPPORTED otherwise); always one launch per half-sweep (k_half_sweep_delta_u8).  Synchronises;
- * dE_series is untouched on error. */
+ * recounted energies.  dE_series: caller-owned HOST buffer of nsweeps int64.  Both layouts; always one launch
+ * per half-sweep (k_half_sweep_delta_u8, or k_half_sweep_packed in its delta form).  Synchronises; dE_series is
+ * untouched on error. */
 int potts_sweep_delta(potts_t *h, double T, int64_t nsweeps, int64_t *dE_series);
 
 /* Same, with E_series / hist_series in DEVICE memory; enqueues and returns without a sync. */

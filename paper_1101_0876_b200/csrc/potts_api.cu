@@ -227,8 +227,16 @@ void launch_pk(int stream_spec, const potts::PackedSweepParams &P, dim3 grid, si
     else potts::k_half_sweep_packed<FIVE, 1, MEASURE, HIST><<<grid, dim3(32, potts::PK_WARPS), smem, st>>>(P);
 }
 
+template <bool FIVE>
+void launch_pk_delta(int stream_spec, const potts::PackedSweepParams &P, dim3 grid, cudaStream_t st)
+{
+    if (stream_spec == 2) potts::k_half_sweep_packed<FIVE, 2, false, false, true><<<grid, dim3(32, potts::PK_WARPS), 0, st>>>(P);
+    else potts::k_half_sweep_packed<FIVE, 1, false, false, true><<<grid, dim3(32, potts::PK_WARPS), 0, st>>>(P);
+}
+
+// delta = true: E_out receives the sum of the accepted moves' d instead of the energy (hist_out must be null)
 int launch_half_sweep_packed(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *E_out,
-                             unsigned long long *hist_out)
+                             unsigned long long *hist_out, bool delta = false)
 {
     potts::PackedSweepParams P;
     P.S = h->pk;
@@ -245,6 +253,11 @@ int launch_half_sweep_packed(potts_t *h, uint32_t colour, const uint32_t thr[4],
     P.rpt = rpt;
     const dim3 grid(gx, (unsigned)(h->L / (potts::PK_WARPS * rpt)));
     const size_t smem = hist_out ? (size_t)h->q * 32 * 4 : 0;
+    if (delta) {
+        if (h->q > 16) launch_pk_delta<true>(h->stream_spec, P, grid, h->stream);
+        else launch_pk_delta<false>(h->stream_spec, P, grid, h->stream);
+        return check_launch(h, "k_half_sweep_packed (delta)");
+    }
     const int sel = (h->q > 16 ? 4 : 0) | (E_out ? 2 : 0) | (hist_out ? 1 : 0);
     switch (sel) {
     case 0: launch_pk<false, false, false>(h->stream_spec, P, grid, smem, h->stream); break;
@@ -765,7 +778,6 @@ int potts_sweep_delta(potts_t *h, double T, int64_t nsweeps, int64_t *dE_series)
     int rc = check_sweep_args(h, T, nsweeps);
     if (rc) return rc;
     if (!dE_series) return fail(POTTS_ERR_ARG, "null dE_series");
-    if (h->layout != POTTS_LAYOUT_U8) return fail(POTTS_ERR_UNSUPPORTED, "potts_sweep_delta needs the U8 layout");
     if (nsweeps == 0) return POTTS_OK;
     uint32_t thr[4];
     thresholds(T, thr);
@@ -775,8 +787,10 @@ int potts_sweep_delta(potts_t *h, double T, int64_t nsweeps, int64_t *dE_series)
     unsigned long long *d = (unsigned long long *)dev;
     CUDA_TRY(cudaMemsetAsync(d, 0, (size_t)nsweeps * 8, h->stream));
     for (int64_t n = 0; n < nsweeps; ++n) {
-        rc = launch_half_sweep_delta(h, 0u, thr, d + n);
-        if (rc == POTTS_OK) rc = launch_half_sweep_delta(h, 1u, thr, d + n);
+        const bool pk = h->layout == POTTS_LAYOUT_PACKED;
+        rc = pk ? launch_half_sweep_packed(h, 0u, thr, d + n, nullptr, true) : launch_half_sweep_delta(h, 0u, thr, d + n);
+        if (rc == POTTS_OK)
+            rc = pk ? launch_half_sweep_packed(h, 1u, thr, d + n, nullptr, true) : launch_half_sweep_delta(h, 1u, thr, d + n);
         if (rc) break;
         h->t += 1;
     }

@@ -83,11 +83,33 @@ def test_delta_degenerate_temperatures(pb):
     assert g.potts_energy() == -2 * 64 * 64
 
 
+# packed layout: 4-bit (q <= 16) and 5-bit (q <= 32) codes, several chunks per row and a ragged last warp
+PACKED_CASES = [
+    (64, 9, 1, 1, 0.99, 40),
+    (128, 24, 4, 0, 1.002, 30),
+    (192, 16, 6, 1, 0.7, 25),
+    (320, 32, 8, 1, 1.2, 15),
+    (2112, 24, 2, 1, 0.995, 4),
+]
+
+
+@pytest.mark.parametrize("stream", [1, 2])
+@pytest.mark.parametrize("L,q,seed,init,f,n", PACKED_CASES)
+def test_delta_series_packed_layout(pb, L, q, seed, init, f, n, stream):
+    T = f * workloads.t_c(q)
+    g = pb.Potts(L, q, seed, init, layout=pb.LAYOUT_PACKED)
+    g.potts_set_stream_spec(stream)
+    o = oracle.OraclePotts(L, q, seed, init, threads=4, stream=stream)
+    E0 = o.energy()
+    dE = g.potts_sweep_delta(T, n)
+    Eo, _ = o.sweep_measured(T, n, 1, hist=False)
+    assert (E0 + np.cumsum(dE) == Eo).all()
+    assert (g.potts_download() == o.spins()).all()
+    assert g.potts_energy() == int(Eo[-1])
+    assert g.potts_sweep_count() == o.t == n
+
+
 def test_delta_arguments(pb):
-    g = pb.Potts(64, 24, 1, pb.INIT_RANDOM, layout=pb.LAYOUT_PACKED)
-    with pytest.raises(pb.PottsError) as e:
-        g.potts_sweep_delta(1.0, 1)
-    assert e.value.code == pb.ERR_UNSUPPORTED
     g = pb.Potts(64, 9, 1, pb.INIT_RANDOM)
     with pytest.raises(pb.PottsError) as e:
         g.potts_sweep_delta(-1.0, 1)
