@@ -2,7 +2,8 @@
 
     python -m paper_1101_0876_b200.build [--force]
 
-nvcc cross-compiles without a GPU.  The library links the CUDA runtime statically, so it needs
+nvcc cross-compiles without a GPU.  One translation unit per kernel family, compiled in parallel into
+`paper_1101_0876_b200/build/*.o`, then linked.  The library links the CUDA runtime statically, so it needs
 only the driver at run time and shares the primary context (memory, streams) with PyTorch.
 """
 from __future__ import annotations
@@ -10,18 +11,21 @@ from __future__ import annotations
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libpotts_b200.so")
-SOURCES = ["potts_api.cu"]
-DEPS = ["potts_api.cu", "potts_core.cuh", "potts_kernels.cuh", "potts_resident.cuh", "potts_packed.cuh", "potts_cluster.cuh", os.path.join(INCLUDE, "potts.h")]
+SOURCES = ["potts_api.cu", "k_stream.cu", "k_resident.cu", "k_cluster.cu", "k_packed.cu"]
+HEADERS = ["potts_core.cuh", "potts_kernels.cuh", "potts_resident.cuh", "potts_packed.cuh", "potts_cluster.cuh",
+           "potts_launch.cuh", os.path.join(INCLUDE, "potts.h")]
 
-NVCC_FLAGS = [
-    "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-Xptxas", "-v",
-]
+ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
+NVCC_FLAGS = ["-O3", "-std=c++17", *ARCH, "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+
+last_action = "none"          # "compiled" or "reused": what the last build() call did
 
 
 def _nvcc() -> str:
@@ -31,40 +35,54 @@ def _nvcc() -> str:
     return "nvcc"
 
 
+def _mtime(p: str) -> float:
+    return os.path.getmtime(p) if os.path.exists(p) else 0.0
+
+
+def _stale(target: str, deps) -> bool:
+    t = _mtime(target)
+    return t == 0.0 or any(_mtime(d) > t for d in deps)
+
+
 def needs_build() -> bool:
-    if not os.path.exists(LIB):
-        return True
-    t = os.path.getmtime(LIB)
-    for d in DEPS:
-        p = d if os.path.isabs(d) else os.path.join(CSRC, d)
-        if os.path.getmtime(p) > t:
-            return True
-    return False
+    deps = [os.path.join(CSRC, s) for s in SOURCES] + [h if os.path.isabs(h) else os.path.join(CSRC, h) for h in HEADERS]
+    return _stale(LIB, deps)
+
+
+def _compile(src: str, verbose: bool) -> str:
+    obj = os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
+    cmd = [_nvcc(), *NVCC_FLAGS, "-I", INCLUDE, "-c", "-o", obj, os.path.join(CSRC, src)]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if verbose or res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed: " + " ".join(cmd))
+    return obj
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if force or needs_build():
-        tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [_nvcc(), *NVCC_FLAGS, "-I", INCLUDE, "-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
-        res = subprocess.run(cmd, capture_output=True, text=True)
-        if verbose or res.returncode != 0:
-            sys.stderr.write(res.stdout + res.stderr)
-        if res.returncode != 0:
-            raise RuntimeError("nvcc failed: " + " ".join(cmd))
-        os.replace(tmp, LIB)
+    """Compile what is out of date and link.  Sets `last_action` to "compiled" or "reused"."""
+    global last_action
+    hdrs = [h if os.path.isabs(h) else os.path.join(CSRC, h) for h in HEADERS]
+    os.makedirs(OBJ, exist_ok=True)
+    todo = [s for s in SOURCES
+            if force or _stale(os.path.join(OBJ, os.path.splitext(s)[0] + ".o"), [os.path.join(CSRC, s)] + hdrs)]
+    if not todo and not _stale(LIB, [os.path.join(OBJ, os.path.splitext(s)[0] + ".o") for s in SOURCES]):
+        last_action = "reused"
+        return LIB
+    with ThreadPoolExecutor(max_workers=len(SOURCES)) as pool:
+        list(pool.map(lambda s: _compile(s, verbose), todo))
+    tmp = LIB + f".tmp{os.getpid()}"
+    objs = [os.path.join(OBJ, os.path.splitext(s)[0] + ".o") for s in SOURCES]
+    cmd = [_nvcc(), *ARCH, "-shared", "-cudart", "static", "-o", tmp, *objs]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("link failed: " + " ".join(cmd))
+    os.replace(tmp, LIB)
+    last_action = "compiled"
     return LIB
 
 
-def build_microbench() -> str:
-    """The issue-model microbenchmark (a measurement tool, see csrc/microbench_issue.cu)."""
-    out = os.path.join(HERE, "microbench_issue")
-    cmd = [_nvcc(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-o", out,
-           os.path.join(CSRC, "microbench_issue.cu")]
-    subprocess.check_call(cmd)
-    return out
-
-
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose=True))
-    if "--microbench" in sys.argv:
-        print(build_microbench())
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv), last_action)

@@ -1,0 +1,25 @@
+// k_cluster.cu -- instantiations of the single-cluster (DSMEM) kernel, see potts_cluster.cuh.
+#include "potts_launch.cuh"
+
+namespace potts {
+namespace {
+
+template <int CM>
+const void *cluster_kernel_cm(int stream_spec)
+{
+    return stream_spec == 2 ? (const void *)k_cluster_u8<CM, 2> : (const void *)k_cluster_u8<CM, 1>;
+}
+
+}  // namespace
+
+const void *cluster_kernel(int cm, int stream_spec)
+{
+    switch (cm) {
+    case CM_7BIT: return cluster_kernel_cm<CM_7BIT>(stream_spec);
+    case CM_8BIT: return cluster_kernel_cm<CM_8BIT>(stream_spec);
+    case CM_NIB4: return cluster_kernel_cm<CM_NIB4>(stream_spec);
+    default: return cluster_kernel_cm<CM_NIB3>(stream_spec);
+    }
+}
+
+}  // namespace potts

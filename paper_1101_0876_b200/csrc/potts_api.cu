@@ -1,10 +1,7 @@
 // potts_api.cu -- the C-ABI of include/potts.h: argument checking, device memory, launches.
 // Every step of the hot path runs in the kernels of potts_kernels.cuh; this file only marshals.
 #include "../../include/potts.h"
-#include "potts_kernels.cuh"
-#include "potts_resident.cuh"
-#include "potts_packed.cuh"
-#include "potts_cluster.cuh"
+#include "potts_launch.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -70,7 +67,8 @@ struct potts_s {
     int64_t opt_resident_ctas = 0;       // 0 auto, else the resident kernel's grid size
     int64_t opt_resident_words = 0;      // 0 auto, 1 / 2: 4-site words per thread and row visit
     int64_t opt_resident_rows = 0;       // 0 auto, else at most this many thread rows in a resident block
-    int64_t opt_cluster_ctas = 0;        // 0 auto, else the cluster kernel's cluster size (1..8)
+    int64_t opt_cluster_ctas = 0;        // 0 auto, else the cluster kernel's cluster size (1..16)
+    int64_t opt_stream_rows = 0;         // 0 auto, else rows per warp of the streaming kernel (even, divides L/4)
 };
 
 namespace {
@@ -147,91 +145,38 @@ potts::SweepParams sweep_params(const potts_t *h, uint32_t colour, const uint32_
     return P;
 }
 
-template <int CM, int ST, bool MEASURE, bool HIST>
-void launch_hs(const potts::SweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
+// Rows per warp of k_sweep_rows_u8: a power of two that divides L / HS_WARPS (L % 32 == 0, so 8 always does).  More rows
+// per warp spread the block's start-up (accept table, ColKeys of 1024 columns, first two neighbour rows) over more
+// sites; too many leave too few blocks to fill 148 SMs evenly.
+int rows_per_warp(const potts_t *h, unsigned gx)
 {
-    potts::k_half_sweep_u8<CM, ST, MEASURE, HIST><<<grid, dim3(32, potts::HS_WARPS), smem, st>>>(P);
-}
-
-template <int CM, int ST>
-void launch_hs_st(const potts::SweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
-{
-    const int sel = (P.E_out ? 2 : 0) | (P.hist_out ? 1 : 0);
-    switch (sel) {
-    case 0: launch_hs<CM, ST, false, false>(P, grid, smem, st); break;
-    case 1: launch_hs<CM, ST, false, true>(P, grid, smem, st); break;
-    case 2: launch_hs<CM, ST, true, false>(P, grid, smem, st); break;
-    default: launch_hs<CM, ST, true, true>(P, grid, smem, st); break;
+    const double startup = 2.0;                             // start-up of a block, in row visits per warp
+    int best = 2;
+    double best_cost = 1e300;
+    for (int rpw = 2; rpw <= 64; rpw <<= 1) {
+        if ((h->L / potts::HS_WARPS) % rpw) break;
+        const long long blocks = (long long)gx * (h->L / (potts::HS_WARPS * rpw));
+        const long long per_sm = (blocks + h->num_sms - 1) / h->num_sms;      // blocks the busiest SM runs
+        double cost = (double)per_sm * (rpw + startup);
+        if (per_sm < 4) cost *= 1.0 + 0.15 * (double)(4 - per_sm);            // too few warps to fill the issue slots
+        if (cost < best_cost * 0.999) { best_cost = cost; best = rpw; }
     }
+    return best;
 }
 
-template <int CM>
-void launch_hs_cm(int stream_spec, const potts::SweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
-{
-    if (stream_spec == 2) launch_hs_st<CM, 2>(P, grid, smem, st);
-    else launch_hs_st<CM, 1>(P, grid, smem, st);
-}
-
+// delta = true: E_out receives the sum of the accepted moves' d instead of the energy (hist_out must be null)
 int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *E_out,
-                      unsigned long long *hist_out)
+                      unsigned long long *hist_out, bool delta = false)
 {
     potts::SweepParams P = sweep_params(h, colour, thr, E_out);
     P.hist_out = hist_out;
     const int chunks = h->L / 32;
     const unsigned gx = (unsigned)((chunks + 31) / 32);
-    int rpt = 8;                                     // L % 32 == 0, so 8 divides L / HS_WARPS
-    while (rpt > 1 && (long long)gx * (h->L / (potts::HS_WARPS * rpt)) < 8ll * h->num_sms) rpt >>= 1;
-    P.rpt = rpt;
-    const dim3 grid(gx, (unsigned)(h->L / (potts::HS_WARPS * rpt)));
-    const size_t smem = hist_out ? (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4 : 0;
-    switch (potts::compare_mode_of(h->q)) {
-    case potts::CM_7BIT: launch_hs_cm<potts::CM_7BIT>(h->stream_spec, P, grid, smem, h->stream); break;
-    case potts::CM_8BIT: launch_hs_cm<potts::CM_8BIT>(h->stream_spec, P, grid, smem, h->stream); break;
-    case potts::CM_NIB4: launch_hs_cm<potts::CM_NIB4>(h->stream_spec, P, grid, smem, h->stream); break;
-    default: launch_hs_cm<potts::CM_NIB3>(h->stream_spec, P, grid, smem, h->stream); break;
-    }
-    return check_launch(h, "k_half_sweep_u8");
-}
-
-template <int CM>
-void launch_hs_delta_cm(int stream_spec, const potts::SweepParams &P, dim3 grid, cudaStream_t st, unsigned long long *dE_out)
-{
-    if (stream_spec == 2) potts::k_half_sweep_delta_u8<CM, 2><<<grid, dim3(32, potts::HS_WARPS), 0, st>>>(P, dE_out);
-    else potts::k_half_sweep_delta_u8<CM, 1><<<grid, dim3(32, potts::HS_WARPS), 0, st>>>(P, dE_out);
-}
-
-// half-sweep that adds the sum of the accepted moves' d to *dE_out (U8 layout)
-int launch_half_sweep_delta(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *dE_out)
-{
-    potts::SweepParams P = sweep_params(h, colour, thr, nullptr);
-    P.hist_out = nullptr;
-    const int chunks = h->L / 32;
-    const unsigned gx = (unsigned)((chunks + 31) / 32);
-    int rpt = 8;                                     // as launch_half_sweep
-    while (rpt > 1 && (long long)gx * (h->L / (potts::HS_WARPS * rpt)) < 8ll * h->num_sms) rpt >>= 1;
-    P.rpt = rpt;
-    const dim3 grid(gx, (unsigned)(h->L / (potts::HS_WARPS * rpt)));
-    switch (potts::compare_mode_of(h->q)) {
-    case potts::CM_7BIT: launch_hs_delta_cm<potts::CM_7BIT>(h->stream_spec, P, grid, h->stream, dE_out); break;
-    case potts::CM_8BIT: launch_hs_delta_cm<potts::CM_8BIT>(h->stream_spec, P, grid, h->stream, dE_out); break;
-    case potts::CM_NIB4: launch_hs_delta_cm<potts::CM_NIB4>(h->stream_spec, P, grid, h->stream, dE_out); break;
-    default: launch_hs_delta_cm<potts::CM_NIB3>(h->stream_spec, P, grid, h->stream, dE_out); break;
-    }
-    return check_launch(h, "k_half_sweep_delta_u8");
-}
-
-template <bool FIVE, bool MEASURE, bool HIST>
-void launch_pk(int stream_spec, const potts::PackedSweepParams &P, dim3 grid, size_t smem, cudaStream_t st)
-{
-    if (stream_spec == 2) potts::k_half_sweep_packed<FIVE, 2, MEASURE, HIST><<<grid, dim3(32, potts::PK_WARPS), smem, st>>>(P);
-    else potts::k_half_sweep_packed<FIVE, 1, MEASURE, HIST><<<grid, dim3(32, potts::PK_WARPS), smem, st>>>(P);
-}
-
-template <bool FIVE>
-void launch_pk_delta(int stream_spec, const potts::PackedSweepParams &P, dim3 grid, cudaStream_t st)
-{
-    if (stream_spec == 2) potts::k_half_sweep_packed<FIVE, 2, false, false, true><<<grid, dim3(32, potts::PK_WARPS), 0, st>>>(P);
-    else potts::k_half_sweep_packed<FIVE, 1, false, false, true><<<grid, dim3(32, potts::PK_WARPS), 0, st>>>(P);
+    P.rpw = h->opt_stream_rows > 0 ? (int)h->opt_stream_rows : rows_per_warp(h, gx);
+    const dim3 grid(gx, (unsigned)(h->L / (potts::HS_WARPS * P.rpw)));
+    const size_t smem = hist_out ? (size_t)potts::hist_words((uint32_t)h->q) * 4 : 0;
+    potts::launch_sweep_rows_u8(potts::compare_mode_of(h->q), h->stream_spec, delta, P, grid, smem, h->stream);
+    return check_launch(h, "k_sweep_rows_u8");
 }
 
 // delta = true: E_out receives the sum of the accepted moves' d instead of the energy (hist_out must be null)
@@ -253,22 +198,7 @@ int launch_half_sweep_packed(potts_t *h, uint32_t colour, const uint32_t thr[4],
     P.rpt = rpt;
     const dim3 grid(gx, (unsigned)(h->L / (potts::PK_WARPS * rpt)));
     const size_t smem = hist_out ? (size_t)h->q * 32 * 4 : 0;
-    if (delta) {
-        if (h->q > 16) launch_pk_delta<true>(h->stream_spec, P, grid, h->stream);
-        else launch_pk_delta<false>(h->stream_spec, P, grid, h->stream);
-        return check_launch(h, "k_half_sweep_packed (delta)");
-    }
-    const int sel = (h->q > 16 ? 4 : 0) | (E_out ? 2 : 0) | (hist_out ? 1 : 0);
-    switch (sel) {
-    case 0: launch_pk<false, false, false>(h->stream_spec, P, grid, smem, h->stream); break;
-    case 1: launch_pk<false, false, true>(h->stream_spec, P, grid, smem, h->stream); break;
-    case 2: launch_pk<false, true, false>(h->stream_spec, P, grid, smem, h->stream); break;
-    case 3: launch_pk<false, true, true>(h->stream_spec, P, grid, smem, h->stream); break;
-    case 4: launch_pk<true, false, false>(h->stream_spec, P, grid, smem, h->stream); break;
-    case 5: launch_pk<true, false, true>(h->stream_spec, P, grid, smem, h->stream); break;
-    case 6: launch_pk<true, true, false>(h->stream_spec, P, grid, smem, h->stream); break;
-    default: launch_pk<true, true, true>(h->stream_spec, P, grid, smem, h->stream); break;
-    }
+    potts::launch_sweep_rows_packed(h->q > 16, h->stream_spec, delta, P, grid, delta ? 0 : smem, h->stream);
     return check_launch(h, "k_half_sweep_packed");
 }
 
@@ -389,33 +319,8 @@ ResidentPlan plan_resident(const potts_t *h)
     return R;
 }
 
-// register budget: 112 per thread for blocks up to 576 threads, 80 up to 768, else 64
-template <int CM, int ST>
-const void *resident_kernel_st(int W, int small)
-{
-    if (W == 1) return small == 2 ? (const void *)potts::k_resident_u8<CM, 1, ST, 576> : (const void *)potts::k_resident_u8<CM, 1, ST, 1024>;
-    return small == 2 ? (const void *)potts::k_resident_u8<CM, 2, ST, 576>
-                      : (small == 1 ? (const void *)potts::k_resident_u8<CM, 2, ST, 768> : (const void *)potts::k_resident_u8<CM, 2, ST, 1024>);
-}
-
-template <int CM>
-const void *resident_kernel_cm(int stream_spec, int W, int small)
-{
-    return stream_spec == 2 ? resident_kernel_st<CM, 2>(W, small) : resident_kernel_st<CM, 1>(W, small);
-}
-
-const void *resident_kernel(int cm, int stream_spec, int W, int small)
-{
-    switch (cm) {
-    case potts::CM_7BIT: return resident_kernel_cm<potts::CM_7BIT>(stream_spec, W, small);
-    case potts::CM_8BIT: return resident_kernel_cm<potts::CM_8BIT>(stream_spec, W, small);
-    case potts::CM_NIB4: return resident_kernel_cm<potts::CM_NIB4>(stream_spec, W, small);
-    default: return resident_kernel_cm<potts::CM_NIB3>(stream_spec, W, small);
-    }
-}
-
 int launch_resident(potts_t *h, const ResidentPlan &R, const uint32_t thr[4], int64_t nsweeps, int64_t every,
-                    unsigned long long *E_series_dev, unsigned long long *hist_series_dev)
+                    unsigned long long *E_series_dev, unsigned long long *hist_series_dev, unsigned long long *dE_series_dev)
 {
     potts::ResidentParams P;
     P.plane[0] = h->plane[0];
@@ -431,11 +336,12 @@ int launch_resident(potts_t *h, const ResidentPlan &R, const uint32_t thr[4], in
     P.every = (uint32_t)every;
     P.E_series = E_series_dev;
     P.hist_series = hist_series_dev;
+    P.dE_series = dE_series_dev;
     P.inbox = (uint2 *)h->inbox;
     P.error = h->error;
     P.rows_max = R.rows_max;
     P.tyc = R.tyc;
-    const void *fn = resident_kernel(potts::compare_mode_of(h->q), h->stream_spec, R.W, R.nthreads <= 576 ? 2 : (R.nthreads <= 768 ? 1 : 0));
+    const void *fn = potts::resident_kernel(potts::compare_mode_of(h->q), h->stream_spec, R.W, R.nthreads <= 576 ? 2 : (R.nthreads <= 768 ? 1 : 0));
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
     int per_sm = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, R.nthreads, R.smem));
@@ -476,14 +382,8 @@ ClusterPlan plan_cluster(const potts_t *h)
     return R;
 }
 
-template <int CM>
-const void *cluster_kernel_cm(int stream_spec)
-{
-    return stream_spec == 2 ? (const void *)potts::k_cluster_u8<CM, 2> : (const void *)potts::k_cluster_u8<CM, 1>;
-}
-
 int launch_cluster(potts_t *h, const ClusterPlan &R, const uint32_t thr[4], int64_t nsweeps, int64_t every,
-                   unsigned long long *E_series_dev, unsigned long long *hist_series_dev)
+                   unsigned long long *E_series_dev, unsigned long long *hist_series_dev, unsigned long long *dE_series_dev)
 {
     potts::ResidentParams P = {};
     P.plane[0] = h->plane[0];
@@ -499,16 +399,11 @@ int launch_cluster(potts_t *h, const ClusterPlan &R, const uint32_t thr[4], int6
     P.every = (uint32_t)every;
     P.E_series = E_series_dev;
     P.hist_series = hist_series_dev;
+    P.dE_series = dE_series_dev;
     P.error = h->error;
     P.rows_max = R.rows_max;
     P.tyc = R.tyc;
-    const void *fn = nullptr;
-    switch (potts::compare_mode_of(h->q)) {
-    case potts::CM_7BIT: fn = cluster_kernel_cm<potts::CM_7BIT>(h->stream_spec); break;
-    case potts::CM_8BIT: fn = cluster_kernel_cm<potts::CM_8BIT>(h->stream_spec); break;
-    case potts::CM_NIB4: fn = cluster_kernel_cm<potts::CM_NIB4>(h->stream_spec); break;
-    default: fn = cluster_kernel_cm<potts::CM_NIB3>(h->stream_spec); break;
-    }
+    const void *fn = potts::cluster_kernel(potts::compare_mode_of(h->q), h->stream_spec);
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
     if (R.G > 8) CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     cudaLaunchConfig_t cfg = {};
@@ -529,22 +424,25 @@ int launch_cluster(potts_t *h, const ClusterPlan &R, const uint32_t thr[4], int6
     return POTTS_OK;
 }
 
-// the sweep loop shared by potts_sweep and potts_sweep_measured_dev
+// The sweep loop shared by every entry point that sweeps.  every = 0: no samples.  dE_series_dev (nsweeps zeroed
+// int64 slots, or null): slot n += the energy change of sweep n, summed over its accepted moves.
 int run_sweeps(potts_t *h, double T, int64_t nsweeps, int64_t every, unsigned long long *E_series_dev,
-               unsigned long long *hist_series_dev)
+               unsigned long long *hist_series_dev, unsigned long long *dE_series_dev = nullptr)
 {
     uint32_t thr[4];
     thresholds(T, thr);
     if (nsweeps == 0) return POTTS_OK;
+    // the persistent kernels' sweep and sample counters are 32-bit: long calls are split into pieces of whole samples
+    const int64_t piece = every > 0 ? ((1ll << 30) / every) * every : (1ll << 30);
     if (h->opt_variant == 3 || (h->opt_variant == 0 && h->layout == POTTS_LAYOUT_U8 && h->L <= CLUSTER_AUTO_L_MAX)) {
         const ClusterPlan C = plan_cluster(h);
         if (C.ok) {
-            const int64_t piece = every > 0 ? (int64_t)((1ll << 30) / every) * every : (1ll << 30);
             for (int64_t done = 0; done < nsweeps;) {
                 const int64_t n = nsweeps - done < piece ? nsweeps - done : piece;
                 const int64_t s0 = every > 0 ? done / every : 0;
                 int rc = launch_cluster(h, C, thr, n, every > 0 ? every : 0, E_series_dev ? E_series_dev + s0 : nullptr,
-                                        hist_series_dev ? hist_series_dev + s0 * h->q : nullptr);
+                                        hist_series_dev ? hist_series_dev + s0 * h->q : nullptr,
+                                        dE_series_dev ? dE_series_dev + done : nullptr);
                 if (rc) return rc;
                 h->t += (uint64_t)n;
                 done += n;
@@ -556,14 +454,13 @@ int run_sweeps(potts_t *h, double T, int64_t nsweeps, int64_t every, unsigned lo
     if (h->opt_variant != 1) {
         const ResidentPlan R = plan_resident(h);
         if (R.ok) {
-            // the kernel's sweep and sample counters are 32-bit: split very long calls
-            const int64_t piece = every > 0 ? (int64_t)((1ll << 30) / every) * every : (1ll << 30);
             for (int64_t done = 0; done < nsweeps;) {
                 const int64_t n = nsweeps - done < piece ? nsweeps - done : piece;
                 const int64_t s0 = every > 0 ? done / every : 0;
                 int rc = launch_resident(h, R, thr, n, every > 0 ? every : 0,
                                          E_series_dev ? E_series_dev + s0 : nullptr,
-                                         hist_series_dev ? hist_series_dev + s0 * h->q : nullptr);
+                                         hist_series_dev ? hist_series_dev + s0 * h->q : nullptr,
+                                         dE_series_dev ? dE_series_dev + done : nullptr);
                 if (rc) return rc;
                 h->t += (uint64_t)n;
                 done += n;
@@ -572,13 +469,24 @@ int run_sweeps(potts_t *h, double T, int64_t nsweeps, int64_t every, unsigned lo
         }
         if (h->opt_variant == 2) return fail(POTTS_ERR_UNSUPPORTED, "resident variant unavailable: %s", R.why);
     }
+    const bool pk = h->layout == POTTS_LAYOUT_PACKED;
     for (int64_t n = 0; n < nsweeps; ++n) {
+        int rc;
+        if (dE_series_dev) {
+            // streaming kernels: the energy-change form of the half-sweep (no samples in the same call)
+            for (uint32_t c = 0; c < 2; ++c) {
+                rc = pk ? launch_half_sweep_packed(h, c, thr, dE_series_dev + n, nullptr, true)
+                        : launch_half_sweep(h, c, thr, dE_series_dev + n, nullptr, true);
+                if (rc) return rc;
+            }
+            h->t += 1;
+            continue;
+        }
         const bool sample = every > 0 && ((n + 1) % every == 0);
         const int64_t idx = sample ? (n + 1) / every - 1 : 0;
         unsigned long long *Hs = (sample && hist_series_dev) ? hist_series_dev + idx * h->q : nullptr;
-        const bool pk = h->layout == POTTS_LAYOUT_PACKED;
         unsigned long long *Es = (sample && E_series_dev) ? E_series_dev + idx : nullptr;
-        int rc = pk ? launch_half_sweep_packed(h, 0u, thr, nullptr, Hs) : launch_half_sweep(h, 0u, thr, nullptr, Hs);
+        rc = pk ? launch_half_sweep_packed(h, 0u, thr, nullptr, Hs) : launch_half_sweep(h, 0u, thr, nullptr, Hs);
         if (rc) return rc;
         rc = pk ? launch_half_sweep_packed(h, 1u, thr, Es, Hs) : launch_half_sweep(h, 1u, thr, Es, Hs);
         if (rc) return rc;
@@ -732,8 +640,8 @@ int potts_sweep_measured_dev(potts_t *h, double T, int64_t nsweeps, int64_t ever
 {
     int rc = check_sweep_args(h, T, nsweeps);
     if (rc) return rc;
-    if (every < 1 || nsweeps % every != 0)
-        return fail(POTTS_ERR_ARG, "every = %lld must be >= 1 and divide nsweeps = %lld", (long long)every,
+    if (every < 1 || every > (1ll << 30) || nsweeps % every != 0)
+        return fail(POTTS_ERR_ARG, "every = %lld must be in [1, 2^30] and divide nsweeps = %lld", (long long)every,
                     (long long)nsweeps);
     const int64_t ns = nsweeps / every;
     if (ns == 0) return POTTS_OK;
@@ -748,8 +656,8 @@ int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every, i
 {
     int rc = check_sweep_args(h, T, nsweeps);
     if (rc) return rc;
-    if (every < 1 || nsweeps % every != 0)
-        return fail(POTTS_ERR_ARG, "every = %lld must be >= 1 and divide nsweeps = %lld", (long long)every,
+    if (every < 1 || every > (1ll << 30) || nsweeps % every != 0)
+        return fail(POTTS_ERR_ARG, "every = %lld must be in [1, 2^30] and divide nsweeps = %lld", (long long)every,
                     (long long)nsweeps);
     const int64_t ns = nsweeps / every;
     if (ns == 0) return POTTS_OK;
@@ -786,21 +694,14 @@ int potts_sweep_delta(potts_t *h, double T, int64_t nsweeps, int64_t *dE_series)
     if (rc) return rc;
     unsigned long long *d = (unsigned long long *)dev;
     CUDA_TRY(cudaMemsetAsync(d, 0, (size_t)nsweeps * 8, h->stream));
-    for (int64_t n = 0; n < nsweeps; ++n) {
-        const bool pk = h->layout == POTTS_LAYOUT_PACKED;
-        rc = pk ? launch_half_sweep_packed(h, 0u, thr, d + n, nullptr, true) : launch_half_sweep_delta(h, 0u, thr, d + n);
-        if (rc == POTTS_OK)
-            rc = pk ? launch_half_sweep_packed(h, 1u, thr, d + n, nullptr, true) : launch_half_sweep_delta(h, 1u, thr, d + n);
-        if (rc) break;
-        h->t += 1;
-    }
+    rc = run_sweeps(h, T, nsweeps, 0, nullptr, nullptr, d);
     cudaError_t e = cudaSuccess;
     if (rc == POTTS_OK) e = cudaMemcpyAsync(dE_series, d, (size_t)nsweeps * 8, cudaMemcpyDeviceToHost, h->stream);
     cudaError_t e2 = cudaStreamSynchronize(h->stream);
     if (rc) return rc;
     if (e != cudaSuccess || e2 != cudaSuccess)
         return fail(POTTS_ERR_CUDA, "series copy/sync failed: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
-    return POTTS_OK;
+    return check_device_error(h);
 }
 
 int potts_ladder(potts_t *h, const double *T, int32_t nT, int64_t t_tran, int64_t t_max, int64_t dt, int64_t *E_series,
@@ -990,6 +891,11 @@ int potts_set_option(potts_t *h, const char *key, int64_t value)
         if (value < 0 || value > 2) return fail(POTTS_ERR_ARG, "resident_words must be 0 (auto), 1 or 2");
         h->opt_resident_words = value; return POTTS_OK;
     }
+    if (!std::strcmp(key, "stream_rows")) {
+        if (value < 0 || (value > 0 && ((value & 1) || (h->L / potts::HS_WARPS) % value)))
+            return fail(POTTS_ERR_ARG, "stream_rows must be 0 (auto) or an even divisor of L / %d", potts::HS_WARPS);
+        h->opt_stream_rows = value; return POTTS_OK;
+    }
     return fail(POTTS_ERR_ARG, "unknown option '%s'", key);
 }
 
@@ -1001,6 +907,7 @@ int potts_get_option(potts_t *h, const char *key, int64_t *value)
     if (!std::strcmp(key, "resident_words")) { *value = h->opt_resident_words; return POTTS_OK; }
     if (!std::strcmp(key, "resident_rows")) { *value = h->opt_resident_rows; return POTTS_OK; }
     if (!std::strcmp(key, "cluster_ctas")) { *value = h->opt_cluster_ctas; return POTTS_OK; }
+    if (!std::strcmp(key, "stream_rows")) { *value = h->opt_stream_rows; return POTTS_OK; }
     if (!std::strcmp(key, "cluster_active")) {             // read-only: cluster size the next sweep call would use (0 = not the cluster kernel)
         const bool want = h->opt_variant == 3 || (h->opt_variant == 0 && h->layout == POTTS_LAYOUT_U8 && h->L <= CLUSTER_AUTO_L_MAX);
         *value = (want && plan_cluster(h).ok) ? plan_cluster(h).G : 0; return POTTS_OK;
@@ -1205,27 +1112,6 @@ int potts_batch_launch_count(potts_batch_t *b, uint64_t *n)
 
 }  // extern "C"
 
-namespace {
-
-template <int CM, int ST>
-cudaError_t launch_batch_st(const potts::BatchParams &B, const potts::BatchTable &T, int n, int nthreads, size_t smem, cudaStream_t st)
-{
-    auto fn = potts::k_resident_batch_u8<CM, ST, 1024>;      // 64 registers: several small lattices per SM
-    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    fn<<<(unsigned)n, (unsigned)nthreads, smem, st>>>(B, T);
-    return cudaGetLastError();
-}
-
-template <int CM>
-cudaError_t launch_batch_cm(int stream_spec, const potts::BatchParams &B, const potts::BatchTable &T, int n, int nthreads, size_t smem,
-                            cudaStream_t st)
-{
-    return stream_spec == 2 ? launch_batch_st<CM, 2>(B, T, n, nthreads, smem, st) : launch_batch_st<CM, 1>(B, T, n, nthreads, smem, st);
-}
-
-}  // namespace
-
 extern "C" {
 
 int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t every, int64_t *E_series,
@@ -1275,12 +1161,7 @@ int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweep
         P.tyc = R.tyc;
         B.lattice_stride = 2ull * b->plane_bytes;
         B.series_stride = (unsigned long long)ns;
-        switch (potts::compare_mode_of(b->q)) {
-        case potts::CM_7BIT: e = launch_batch_cm<potts::CM_7BIT>(b->stream_spec, B, tab, m, R.nthreads, R.smem, b->stream); break;
-        case potts::CM_8BIT: e = launch_batch_cm<potts::CM_8BIT>(b->stream_spec, B, tab, m, R.nthreads, R.smem, b->stream); break;
-        case potts::CM_NIB4: e = launch_batch_cm<potts::CM_NIB4>(b->stream_spec, B, tab, m, R.nthreads, R.smem, b->stream); break;
-        default: e = launch_batch_cm<potts::CM_NIB3>(b->stream_spec, B, tab, m, R.nthreads, R.smem, b->stream); break;
-        }
+        e = potts::launch_batch(potts::compare_mode_of(b->q), b->stream_spec, B, tab, m, R.nthreads, R.smem, b->stream);
         b->launches += 1;
     }
     if (e == cudaSuccess) b->t += (uint64_t)nsweeps;

@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) uint8_t s_raw[];
-    __shared__ uint32_t lut[12];
+    __shared__ AcceptEntry<true> lut[ACCEPT_ENTRIES];
 
     const uint32_t G = cluster.num_blocks(), b = cluster.block_rank();
     const int L = P.L, pitch = P.pitch;
@@ -51,9 +51,10 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
     const uint32_t col_next = col + 4u == (uint32_t)pitch ? 0u : col + 4u;
     const bool do_hist = P.hist_series != nullptr && P.every != 0;
     const bool do_E = P.E_series != nullptr && P.every != 0;
+    const bool do_D = P.dE_series != nullptr;
     const uint32_t q = in_register(P.q);
 
-    if (tid < 9) lut[tid] = tid >= 5 ? P.thr[tid - 5] : 0u;
+    accept_lut_fill<true>(lut, P.thr, tid, nthreads);
     if (do_hist)
         for (uint32_t n = tid; n < 2u * hist_words(P.q); n += nthreads) s_hist0[n] = 0u;
     {
@@ -79,7 +80,9 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
             const uint8_t *const oth_row = s_raw + (1u - c) * plane_stride;
             const HalfSweepKeys K = half_sweep_keys(P.key0, P.key1, t, c);
             const bool count_E = sample && c == 1 && do_E, count_H = sample && do_hist;
-            uint32_t nef_sum = 0, words_done = 0;
+            int d_sum = 0, c_sum = 0;
+            uint32_t words_done = 0;
+            const bool ex = count_E || do_D;
             uint32_t *const s_hist = s_hist0 + (sample_idx & 1u) * hist_words(P.q);
             if (is_compute)
                 for (int lr = 1 + ty; lr <= rows; lr += tyc) {
@@ -92,20 +95,26 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
                     const uint32_t up = *reinterpret_cast<const uint32_t *>(orow + col - pitch);
                     const uint32_t dn = *reinterpret_cast<const uint32_t *>(orow + col + pitch);
                     const uint32_t adj = *reinterpret_cast<const uint32_t *>(orow + (p ? col_next : col_prev));
-                    uint32_t lf, rt, nef;
+                    uint32_t lf, rt;
                     horizontal(p, mid, adj, lf, rt);
                     const RowKeys R = row_keys(K, i);
-                    const uint32_t out = update_word<CM, ST>(own, up, dn, lf, rt, 2u * col + p, q, K, R, lut, nef);
+                    const uint32_t out = update_word<CM, ST>(own, up, dn, lf, rt, 2u * col + p, q, K, R, lut, ex, d_sum, c_sum);
                     *reinterpret_cast<uint32_t *>(own_col + ro) = out;
                     // my first row is the row below the last row of the CTA above, my last row the row above the first of the CTA below
                     if (lr == 1)
                         *reinterpret_cast<uint32_t *>(up_raw + c * plane_stride + (uint32_t)((rows_up + 1) * pitch) + col) = out;
                     if (lr == rows) *reinterpret_cast<uint32_t *>(dn_raw + c * plane_stride + col) = out;
-                    if (count_E) { nef_sum += nef; ++words_done; }
+                    ++words_done;
                     if (count_H) hist_add_word(s_hist, P.q, out, tid & 31u);
                 }
+            if (do_D) {
+                int dd = d_sum;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) dd += __shfl_xor_sync(0xffffffffu, dd, o);
+                if ((tid & 31u) == 0 && dd) atomicAdd(P.dE_series + n, (unsigned long long)(long long)dd);
+            }
             if (count_E) {
-                uint32_t satisfied = 16u * words_done - byte_sum(nef_sum);
+                uint32_t satisfied = 16u * words_done - (uint32_t)(c_sum + d_sum);
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
                 if ((tid & 31u) == 0 && satisfied) atomicAdd(P.E_series + sample_idx, 0ull - (unsigned long long)satisfied);

@@ -7,9 +7,15 @@
 // Cost model this file is written against (profiles/r01b_pipe_model.md, measured on B200): for this
 // integer mix an SM sub-partition retires one warp instruction every 2 clocks whichever pipe it goes to
 // (IMAD.WIDE, IMAD, LOP3, IADD3, SHF, PRMT alike; IMAD.HI and POPC take 4), so the time of an update is
-// its instruction count.  One update needs 17 IMAD.WIDE + 18 LOP3 of Philox (fixed by the stream
-// definition) + 1 multiply for the proposal; everything else (neighbour compare, acceptance, packing,
-// loads and stores: ~22 instructions per update at 16 sites per thread) is overhead to keep small.
+// its instruction count.  Round 2 (profiles/r02a_update_word.md) therefore cut instructions:
+//   * Philox: the three multiplies and two XORs of rounds 1-3 that depend on the column j only (not on the
+//     row) are computed once per column and half-sweep (ColKeys) and reused by every row of the tile:
+//     14 IMAD.WIDE + 16 LOP3 per site instead of 17 + 18;
+//   * neighbour compare: the four "differs" flags of the current spin and the four of the proposal are
+//     gathered into ONE code byte per site (no counting, no subtraction);
+//   * acceptance: the code byte indexes a 256-entry shared table of 64-bit values 2^64 - threshold(d),
+//     and the 64-bit sum  w1 + entry  (add, add-with-carry) leaves the accept mask (0 / 0xffffffff) in its
+//     high word: d <= 0 ("always") and threshold 0 ("never") need no special case and no mask start-up.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -40,6 +46,18 @@ __device__ __forceinline__ uint32_t in_register(uint32_t v)
     return r;
 }
 
+// three-input logic in one LOP3; LUT = f(0xF0, 0xCC, 0xAA)
+template <int LUT>
+__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t r;
+    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(r) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+    return r;
+}
+constexpr int LOP_XOR_AND = (0xF0 ^ 0xCC) & 0xAA;              // (a ^ b) & c
+constexpr int LOP_OR_XOR = 0xF0 | (0xCC ^ 0xAA);               // a | (b ^ c)
+constexpr int LOP_SEL = (0xF0 & 0xAA) | (0xCC & ~0xAA & 0xFF); // (a & c) | (b & ~c): bits of a where c is set, else b
+
 // full 4-word Philox4x32-10 (random start, R9)
 __device__ __forceinline__ void philox4x32_10(uint32_t c[4], uint32_t k0, uint32_t k1)
 {
@@ -62,9 +80,11 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c[4], uint32_t k0, uint32
 // depends on so that nothing is computed twice:
 //   HalfSweepKeys  depends on (seed, t, colour)   -- uniform over a half-sweep
 //   RowKeys        adds the row i                 -- one wide multiply per thread and row
-//   philox_site    adds the column j              -- 17 wide multiplies + 18 three-input XORs
-// Round 1 multiplies the counter words c0 = j and c2 = t; round 2 multiplies c0' = hi(M1 t)^i^k0,
-// which does not depend on j.
+//   ColKeys        adds the column j, NOT the row -- three wide multiplies per column and half-sweep
+//   philox_site    adds the column j to a row     -- 17 wide multiplies + 18 three-input XORs (no ColKeys)
+//   philox_site_h  the same from ColKeys          -- 14 wide multiplies + 16 XORs
+// Round 1 multiplies the counter words c0 = j and c2 = t; round 2 multiplies c0' = hi(M1 t)^i^k0 (no j) and
+// c2' = hi(M0 j)^colour^k1 (no i); round 3 multiplies c0'' = hi(M1 c2')^lo(M1 t)^k0' (no i).
 struct HalfSweepKeys {
     uint32_t xa;      // hi(M1*t) ^ k0[0]          c0 after round 1 is xa ^ i
     uint32_t xb;      // colour ^ k1[0]            c2 after round 1 is hi(M0*j) ^ xb
@@ -150,10 +170,280 @@ __device__ __forceinline__ void philox_pair(const HalfSweepKeys &K, const RowKey
     w[0] = c0; w[1] = c1; w[2] = c2; w[3] = c3;
 }
 
+// The column part: everything of rounds 1-3 that depends on j but not on the row i.  One uint4 per column.
+struct ColKeys {
+    uint32_t l0;      // lo(M0*j)                      c2 after round 2 is l0 ^ R.xd
+    uint32_t l1;      // lo(M1*(hi(M0*j)^xb))          c1 after round 2
+    uint32_t ph, pl;  // M0 * (hi(M1*(hi(M0*j)^xb)) ^ xc): round 3's M0*c0 product
+};
+
+__device__ __forceinline__ ColKeys col_keys(const HalfSweepKeys &K, uint32_t j)
+{
+    ColKeys C;
+    uint32_t h0, h1;
+    mul_wide(PHILOX_M0, j, h0, C.l0);
+    mul_wide(PHILOX_M1, h0 ^ K.xb, h1, C.l1);
+    mul_wide(PHILOX_M0, h1 ^ K.xc, C.ph, C.pl);
+    return C;
+}
+
+// row part for the hoisted form: RowKeys plus c3 ^ (k1 of round 3)
+struct RowKeysH {
+    uint32_t xd;      // as RowKeys
+    uint32_t rc;      // R.c3 ^ (k1 + 2 W1): c2 after round 3 is C.ph ^ rc
+};
+
+__device__ __forceinline__ RowKeysH row_keys_h(const HalfSweepKeys &K, uint32_t i)
+{
+    const RowKeys R = row_keys(K, i);
+    RowKeysH H;
+    H.xd = R.xd;
+    H.rc = R.c3 ^ (K.k1 + 2u * PHILOX_W1);
+    return H;
+}
+
+// rounds 3-9 from (ColKeys, RowKeysH); leaves the state before round 10 and the keys of round 10
+__device__ __forceinline__ void philox_rounds_h(const HalfSweepKeys &K, const RowKeysH &R, const ColKeys &C,
+                                                uint32_t &c0, uint32_t &c1, uint32_t &c2, uint32_t &c3, uint32_t &k0, uint32_t &k1)
+{
+    uint32_t h0, l0, h1, l1;
+    mul_wide(PHILOX_M1, C.l0 ^ R.xd, h1, l1);        // round 3: the M1*c2 product (M0*c0 is in C)
+    c0 = h1 ^ C.l1 ^ (K.k0 + 2u * PHILOX_W0);
+    c1 = l1;
+    c2 = C.ph ^ R.rc;
+    c3 = C.pl;
+    k0 = K.k0 + 3u * PHILOX_W0;
+    k1 = K.k1 + 3u * PHILOX_W1;
+#pragma unroll
+    for (int r = 3; r < 9; ++r) {
+        mul_wide(PHILOX_M0, c0, h0, l0);
+        mul_wide(PHILOX_M1, c2, h1, l1);
+        c0 = h1 ^ c1 ^ k0;
+        c1 = l1;
+        c2 = h0 ^ c3 ^ k1;
+        c3 = l0;
+        k0 += PHILOX_W0;
+        k1 += PHILOX_W1;
+    }
+}
+
+__device__ __forceinline__ void philox_site_h(const HalfSweepKeys &K, const RowKeysH &R, const ColKeys &C,
+                                              uint32_t &w0, uint32_t &w1)
+{
+    uint32_t c0, c1, c2, c3, k0, k1, h1, l1;
+    philox_rounds_h(K, R, C, c0, c1, c2, c3, k0, k1);
+    mul_wide(PHILOX_M1, c2, h1, l1);                 // round 10: only words 0 and 1 are used
+    w0 = h1 ^ c1 ^ k0;
+    w1 = l1;
+}
+
+__device__ __forceinline__ void philox_pair_h(const HalfSweepKeys &K, const RowKeysH &R, const ColKeys &C, uint32_t w[4])
+{
+    uint32_t c0, c1, c2, c3, k0, k1, h0, l0, h1, l1;
+    philox_rounds_h(K, R, C, c0, c1, c2, c3, k0, k1);
+    mul_wide(PHILOX_M0, c0, h0, l0);
+    mul_wide(PHILOX_M1, c2, h1, l1);
+    w[0] = h1 ^ c1 ^ k0; w[1] = l1; w[2] = h0 ^ c3 ^ k1; w[3] = l0;
+}
+
 // ---------------------------------------------------------------------------------------------
-// Byte-parallel "not equal" flags: bit 7 of every byte of the result is set iff the bytes of a
-// and b differ.  WIDE = false assumes all spin values < 128 (q <= 128), so a^b has bit 7 clear
-// in every byte and adding 0x7f cannot carry across bytes.
+// Compare modes: how the "differs" flags of a word's four sites against one neighbour word are formed.
+//   CM_7BIT  q <= 128: own and proposal are compared separately, flag in bit 7 of ((a^b) + 0x7f)
+//   CM_8BIT  q <= 256: the same with the carry-safe test
+//   CM_NIB4  q <= 16:  the current spin sits in the low nibble and the proposal in the high nibble of one byte,
+//                      the neighbour is doubled into both nibbles (x 0x11, once per loaded word): ONE three-input
+//                      logic op, one add and one more logic op give the flags of both comparisons (bits 3 and 7)
+//   CM_NIB3  q <= 8:   as CM_NIB4, but a 3-bit difference cannot carry out of its nibble: one XOR and one add
+constexpr int CM_7BIT = 0, CM_8BIT = 1, CM_NIB4 = 2, CM_NIB3 = 3;
+
+__host__ __device__ constexpr int compare_mode_of(int q) { return q > 128 ? CM_8BIT : (q > 16 ? CM_7BIT : (q > 8 ? CM_NIB4 : CM_NIB3)); }
+__host__ __device__ constexpr bool is_nibble_mode(int cm) { return cm == CM_NIB4 || cm == CM_NIB3; }
+
+// a neighbour word as the compare wants it: doubled into both nibbles for the nibble modes
+template <int CM>
+__device__ __forceinline__ uint32_t prep_nbr(uint32_t w) { return is_nibble_mode(CM) ? w * 0x11u : w; }
+
+// One code byte per site: bit k (k = 0..3) = neighbour k differs from the CURRENT spin, bit 4+k = neighbour k
+// differs from the PROPOSAL.  nb[] = the four neighbour words, prepared by prep_nbr.  The flags of neighbour k
+// are moved to their bit by one shift and merged by one bit-select; bits the select leaves behind are garbage
+// of an earlier stage that a later select overwrites.
+template <int CM>
+__device__ __forceinline__ uint32_t ne_code(uint32_t own, uint32_t prop, const uint32_t nb[4])
+{
+    if (is_nibble_mode(CM)) {
+        const uint32_t both = prop * 16u + own;                       // one IMAD: the nibbles do not overlap
+        uint32_t u[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (CM == CM_NIB3) {
+                u[k] = (both ^ nb[k]) + 0x77777777u;                  // bit 3 of a nibble = its 3-bit difference is non-zero
+            } else {
+                const uint32_t m = lop3<LOP_XOR_AND>(both, nb[k], 0x77777777u);
+                u[k] = lop3<LOP_OR_XOR>(m + 0x77777777u, both, nb[k]);
+            }
+        }
+        uint32_t c = lop3<LOP_SEL>(u[0] >> 3, u[1] >> 2, 0x11111111u);
+        c = lop3<LOP_SEL>(c, u[2] >> 1, 0x33333333u);
+        return lop3<LOP_SEL>(c, u[3], 0x77777777u);
+    } else {
+        uint32_t o[4], n[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (CM == CM_7BIT) {
+                o[k] = (own ^ nb[k]) + 0x7f7f7f7fu;                   // bit 7 of a byte = its 7-bit difference is non-zero
+                n[k] = (prop ^ nb[k]) + 0x7f7f7f7fu;
+            } else {
+                o[k] = lop3<LOP_OR_XOR>(lop3<LOP_XOR_AND>(own, nb[k], 0x7f7f7f7fu) + 0x7f7f7f7fu, own, nb[k]);
+                n[k] = lop3<LOP_OR_XOR>(lop3<LOP_XOR_AND>(prop, nb[k], 0x7f7f7f7fu) + 0x7f7f7f7fu, prop, nb[k]);
+            }
+        }
+        uint32_t a = lop3<LOP_SEL>(o[0] >> 7, o[1] >> 6, 0x01010101u);
+        a = lop3<LOP_SEL>(a, o[2] >> 5, 0x03030303u);
+        a = lop3<LOP_SEL>(a, o[3] >> 4, 0x07070707u);                 // bits 0..3 of every byte
+        uint32_t b = lop3<LOP_SEL>(n[0] >> 3, n[1] >> 2, 0x10101010u);
+        b = lop3<LOP_SEL>(b, n[2] >> 1, 0x30303030u);
+        b = lop3<LOP_SEL>(b, n[3], 0x70707070u);                      // bits 4..7 of every byte
+        return lop3<LOP_SEL>(a, b, 0x0f0f0f0fu);
+    }
+}
+
+__device__ __forceinline__ int wrap(int x, int n) { return x < 0 ? x + n : (x >= n ? x - n : x); }
+
+// The two horizontal neighbour words of a 4-site word.  mid = other-colour word at the same
+// (row, k); adj = the other-colour word at k+1 (p = 1) or k-1 (p = 0), periodic.  Works on prepared
+// (doubled) words as well: the shift is a whole byte.
+__device__ __forceinline__ void horizontal(uint32_t p, uint32_t mid, uint32_t adj, uint32_t &lf, uint32_t &rt)
+{
+    if (p) {   // neighbours at k and k+1
+        lf = mid;
+        rt = __funnelshift_r(mid, adj, 8);
+    } else {   // neighbours at k-1 and k
+        lf = __funnelshift_l(adj, mid, 8);
+        rt = mid;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Acceptance table (shared memory), indexed by the code byte.  With c_old = popc(code & 15) neighbours that
+// differ from the current spin and c_new = popc(code >> 4) that differ from the proposal,
+//   d = n_old - n_new = c_new - c_old                                   (R5)
+//   threshold(d) = 2^32 for d <= 0 (always accept), thr[d-1] = floor(2^32 exp(-d/T)) for d = 1..4   (R6)
+//   entry = 2^64 - threshold(d)  (mod 2^64)
+// so that the high word of  w1 + entry  is 0xffffffff iff w1 < threshold(d) and 0 otherwise: exact for every
+// threshold in [0, 2^32].  EX entries (16 bytes) also hold -d and c_old for the fused energy / energy-change sums.
+constexpr int ACCEPT_ENTRIES = 256;
+template <bool T16> struct AcceptEntry;                      // T16: 16-byte entries (the EX sums need them)
+template <> struct AcceptEntry<false> { uint2 v; };
+template <> struct AcceptEntry<true> { uint4 v; };
+template <bool T16> __host__ __device__ constexpr int accept_shift() { return T16 ? 4 : 3; }
+
+template <bool T16>
+__device__ __forceinline__ void accept_lut_fill(AcceptEntry<T16> *lut, const uint32_t thr[4], uint32_t tid, uint32_t nthreads)
+{
+    for (uint32_t code = tid; code < (uint32_t)ACCEPT_ENTRIES; code += nthreads) {
+        const int c_old = __popc(code & 15u), c_new = __popc(code >> 4);
+        const int d = c_new - c_old;
+        const unsigned long long th = d <= 0 ? (1ull << 32) : (unsigned long long)(d == 1 ? thr[0] : (d == 2 ? thr[1] : (d == 3 ? thr[2] : thr[3])));
+        const unsigned long long e = 0ull - th;
+        if constexpr (T16) lut[code].v = make_uint4((uint32_t)e, (uint32_t)(e >> 32), (uint32_t)(-d), (uint32_t)c_old);
+        else lut[code].v = make_uint2((uint32_t)e, (uint32_t)(e >> 32));
+    }
+}
+
+// accept masks of the four sites of a word: byte b = 0xff iff site b accepts its proposal.
+// EX: d_sum += sum of d over the accepted sites, c_sum += sum of c_old over the four sites.
+template <bool EX, bool T16>
+__device__ __forceinline__ uint32_t accept_mask(uint32_t code, const uint32_t w1[4], const AcceptEntry<T16> *lut,
+                                                int &d_sum, int &c_sum)
+{
+    static_assert(T16 || !EX, "the EX sums need 16-byte table entries");
+    constexpr int S = accept_shift<T16>();
+    constexpr uint32_t M = 0xffu << S;
+    uint32_t a[4];
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        const uint32_t off = b == 0 ? (code << S) & M : (code >> (8 * b - S)) & M;
+        const char *p = reinterpret_cast<const char *>(lut) + off;
+        unsigned long long e, r;
+        uint32_t lo;
+        if constexpr (EX) {
+            const uint4 v = *reinterpret_cast<const uint4 *>(p);
+            asm("mov.b64 %0, {%1, %2};" : "=l"(e) : "r"(v.x), "r"(v.y));
+            r = e + (unsigned long long)w1[b];
+            asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(a[b]) : "l"(r));
+            d_sum += (int)(a[b] * v.z);                               // (-1) * (-d) for an accepted site
+            c_sum += (int)v.w;
+        } else {
+            const uint2 v = *reinterpret_cast<const uint2 *>(p);
+            asm("mov.b64 %0, {%1, %2};" : "=l"(e) : "r"(v.x), "r"(v.y));
+            r = e + (unsigned long long)w1[b];
+            asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(a[b]) : "l"(r));
+        }
+    }
+    const uint32_t m01 = lop3<LOP_SEL>(a[0], a[1], 0x000000ffu);
+    const uint32_t m23 = lop3<LOP_SEL>(a[2], a[3], 0x00ffffffu);
+    return lop3<LOP_SEL>(m01, m23, 0x0000ffffu);
+}
+
+// ---------------------------------------------------------------------------------------------
+// One word (4 same-colour sites, consecutive k) of the Metropolis update (R4-R7), random words given.
+//   own      current spins of the 4 sites
+//   nb[4]    the 4 neighbour words (up, down, left, right: any order), prepared by prep_nbr<CM>
+//   w0, w1   Philox words of the 4 sites: proposal and acceptance
+// Returns the new word.  EX: d_sum += sum of d = n_old - n_new over the accepted sites (the energy change of
+// the word), c_sum += unequal neighbours of the OLD spins (so that the unequal neighbours
+// of the final spins sum to c_sum + d_sum).
+template <int CM, bool EX, bool T16 = EX>
+__device__ __forceinline__ uint32_t metropolis_word(uint32_t own, const uint32_t nb[4], uint32_t q, const uint32_t w0[4],
+                                                    const uint32_t w1[4], const AcceptEntry<T16> *lut,
+                                                    int &d_sum, int &c_sum)
+{
+    // R4: proposal floor(w0 q / 2^32), packed one byte per site
+    const uint32_t s01 = __byte_perm(__umulhi(w0[0], q), __umulhi(w0[1], q), 0x0040);
+    const uint32_t s23 = __byte_perm(__umulhi(w0[2], q), __umulhi(w0[3], q), 0x0040);
+    const uint32_t prop = __byte_perm(s01, s23, 0x5410);
+    const uint32_t code = ne_code<CM>(own, prop, nb);                 // R5
+    const uint32_t mask = accept_mask<EX, T16>(code, w1, lut, d_sum, c_sum);   // R6
+    return lop3<LOP_SEL>(prop, own, mask);                            // R7
+}
+
+// The random words of a word's four sites drawn without ColKeys (kernels that keep the lattice in shared memory):
+//   j0  column of byte 0 (columns advance by 2 per byte)
+template <int ST>     // ST: random-stream definition, 1 = one Philox block per site (R3), 2 = per pair (R3')
+__device__ __forceinline__ void draw_words(const HalfSweepKeys &K, const RowKeys &R, uint32_t j0, uint32_t w0[4], uint32_t w1[4])
+{
+    if (ST == 1) {
+#pragma unroll
+        for (int b = 0; b < 4; ++b) philox_site(K, R, j0 + 2u * b, w0[b], w1[b]);
+    } else {
+        // byte 0 of a word is an even same-colour site, so the word holds two whole pairs
+#pragma unroll
+        for (int m = 0; m < 2; ++m) {
+            uint32_t w[4];
+            philox_pair(K, R, j0 + 4u * m, w);
+            w0[2 * m] = w[0]; w1[2 * m] = w[1]; w0[2 * m + 1] = w[2]; w1[2 * m + 1] = w[3];
+        }
+    }
+}
+
+// One word of the update from the neighbour words as loaded (byte b = that neighbour of site b).  `ex` is uniform
+// over the warp: with it the EX sums are formed (sampled sweeps, energy-change series), without it the table is
+// read 8 bytes at a time and the two extra instructions per site are skipped.
+template <int CM, int ST>
+__device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
+                                                uint32_t j0, uint32_t q, const HalfSweepKeys &K, const RowKeys &R,
+                                                const AcceptEntry<true> *lut, bool ex, int &d_sum, int &c_sum)
+{
+    uint32_t w0[4], w1[4];
+    draw_words<ST>(K, R, j0, w0, w1);
+    const uint32_t nb[4] = {prep_nbr<CM>(up), prep_nbr<CM>(dn), prep_nbr<CM>(lf), prep_nbr<CM>(rt)};
+    if (ex) return metropolis_word<CM, true, true>(own, nb, q, w0, w1, lut, d_sum, c_sum);
+    return metropolis_word<CM, false, true>(own, nb, q, w0, w1, lut, d_sum, c_sum);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Standalone measurement helpers: byte-parallel "not equal" flags (bit 7 of every byte of the result is
+// set iff the bytes of a and b differ).  WIDE = false assumes all spin values < 128.
 template <bool WIDE>
 __device__ __forceinline__ uint32_t ne_flags(uint32_t a, uint32_t b)
 {
@@ -170,125 +460,9 @@ __device__ __forceinline__ uint32_t ne_count4(uint32_t s, uint32_t up, uint32_t 
            ((ne_flags<WIDE>(s, lf) >> 7) + (ne_flags<WIDE>(s, rt) >> 7));
 }
 
-// Compare modes of update_word: how the per-byte counts of unequal neighbours are formed.
-//   CM_7BIT  q <= 128: one flag word per (spin word, neighbour word) pair, 8 pairs per 4 sites
-//   CM_8BIT  q <= 256: the same with the carry-safe test
-//   CM_NIB4  q <= 16:  the current spin sits in the low nibble and the proposal in the high nibble of one byte,
-//                      the neighbour is doubled into both nibbles (x 0x11): ONE xor and one zero-nibble test give
-//                      the flags of both comparisons, and the shifted sum leaves n_old and n_new in the two nibbles
-//   CM_NIB3  q <= 8:   as CM_NIB4, but a 3-bit difference cannot carry out of its nibble: a shorter zero test
-constexpr int CM_7BIT = 0, CM_8BIT = 1, CM_NIB4 = 2, CM_NIB3 = 3;
-
-__host__ __device__ constexpr int compare_mode_of(int q) { return q > 128 ? CM_8BIT : (q > 16 ? CM_7BIT : (q > 8 ? CM_NIB4 : CM_NIB3)); }
-
-template <int CM>
-__device__ __forceinline__ void ne_counts(uint32_t own, uint32_t prop, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
-                                          uint32_t &c_old, uint32_t &c_new)
-{
-    if (CM == CM_7BIT || CM == CM_8BIT) {
-        c_old = ne_count4<CM == CM_8BIT>(own, up, dn, lf, rt);
-        c_new = ne_count4<CM == CM_8BIT>(prop, up, dn, lf, rt);
-    } else {
-        const uint32_t both = own | (prop << 4);
-        const uint32_t nb[4] = {up, dn, lf, rt};
-        uint32_t s = 0;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const uint32_t x = both ^ (nb[k] * 0x11u);
-            const uint32_t f = CM == CM_NIB3 ? (x + 0x77777777u) & 0x88888888u
-                                             : (((x & 0x77777777u) + 0x77777777u) | x) & 0x88888888u;
-            s += f >> 3;
-        }
-        c_old = s & 0x0f0f0f0fu;
-        c_new = (s >> 4) & 0x0f0f0f0fu;
-    }
-}
-
 __device__ __forceinline__ uint32_t byte_sum(uint32_t v)   // sum of the 4 bytes (sum < 256)
 {
     return __dp4a(v, 0x01010101u, 0u);
-}
-
-// every byte of the result = 0xff if bit 7 of that byte of v is set, else 0x00 (PRMT with the
-// "replicate sign" bit of each selector nibble; __byte_perm masks that bit off)
-__device__ __forceinline__ uint32_t msb_to_bytemask(uint32_t v)
-{
-    uint32_t r;
-    asm("prmt.b32 %0, %1, %1, 0xba98;" : "=r"(r) : "r"(v));
-    return r;
-}
-
-__device__ __forceinline__ int wrap(int x, int n) { return x < 0 ? x + n : (x >= n ? x - n : x); }
-
-// The two horizontal neighbour words of a 4-site word.  mid = other-colour word at the same
-// (row, k); adj = the other-colour word at k+1 (p = 1) or k-1 (p = 0), periodic.
-__device__ __forceinline__ void horizontal(uint32_t p, uint32_t mid, uint32_t adj, uint32_t &lf, uint32_t &rt)
-{
-    if (p) {   // neighbours at k and k+1
-        lf = mid;
-        rt = __funnelshift_r(mid, adj, 8);
-    } else {   // neighbours at k-1 and k
-        lf = __funnelshift_l(adj, mid, 8);
-        rt = mid;
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// One word (4 same-colour sites, consecutive k) of the Metropolis update (R4-R7).
-//   own          current spins of the 4 sites
-//   up,dn,lf,rt  the 4 neighbour words, byte b = that neighbour of site b
-//   j0           column of byte 0 (columns advance by 2 per byte)
-//   lut          shared memory, 9 words: lut[d+4] = floor(2^32 exp(-d/T)) for d = 1..4 (entries 0..4 unused)
-// Returns the new word; ne_final = per-byte count of unequal neighbours of the final spins, ne_old = the same of
-// the spins before the update (so that, per byte, ne_final - ne_old = d of an accepted move and 0 otherwise).
-template <int CM, int ST>     // ST: random-stream definition, 1 = one Philox block per site (R3), 2 = per pair (R3')
-__device__ __forceinline__ uint32_t update_word_ex(uint32_t own, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
-                                                   uint32_t j0, uint32_t q, const HalfSweepKeys &K, const RowKeys &R,
-                                                   const uint32_t *lut, uint32_t &ne_final, uint32_t &ne_old)
-{
-    uint32_t w0[4], w1[4];
-    if (ST == 1) {
-#pragma unroll
-        for (int b = 0; b < 4; ++b) philox_site(K, R, j0 + 2u * b, w0[b], w1[b]);
-    } else {
-        // byte 0 of a word is an even same-colour site, so the word holds two whole pairs
-#pragma unroll
-        for (int m = 0; m < 2; ++m) {
-            uint32_t w[4];
-            philox_pair(K, R, j0 + 4u * m, w);
-            w0[2 * m] = w[0]; w1[2 * m] = w[1]; w0[2 * m + 1] = w[2]; w1[2 * m + 1] = w[3];
-        }
-    }
-    // R4: proposal floor(w0 q / 2^32), packed one byte per site
-    const uint32_t s01 = __byte_perm(__umulhi(w0[0], q), __umulhi(w0[1], q), 0x0040);
-    const uint32_t s23 = __byte_perm(__umulhi(w0[2], q), __umulhi(w0[3], q), 0x0040);
-    const uint32_t prop = __byte_perm(s01, s23, 0x5410);
-
-    // R5: d = n_old - n_new = ne_new - ne_old, biased by 4 so that every byte stays in 0..8
-    uint32_t c_old, c_new;
-    ne_counts<CM>(own, prop, up, dn, lf, rt, c_old, c_new);
-    const uint32_t dw = c_new + 0x04040404u - c_old;
-    // R6: d <= 0 always accepts: byte <= 4  <=>  bit 7 of (0x84 - byte); replicate it over the byte
-    uint32_t mask = msb_to_bytemask(0x84848484u - dw);
-    const uint32_t dw4 = dw << 2;                                   // byte offsets into lut
-#pragma unroll
-    for (int b = 0; b < 4; ++b) {
-        const uint32_t off = (dw4 >> (8 * b)) & 0xffu;
-        const uint32_t thr = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(lut) + off);
-        if (w1[b] < thr) mask |= 0xffu << (8 * b);
-    }
-    ne_final = (c_new & mask) | (c_old & ~mask);
-    ne_old = c_old;
-    return (prop & mask) | (own & ~mask);                           // R7
-}
-
-template <int CM, int ST>
-__device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
-                                                uint32_t j0, uint32_t q, const HalfSweepKeys &K, const RowKeys &R,
-                                                const uint32_t *lut, uint32_t &ne_final)
-{
-    uint32_t ne_old;
-    return update_word_ex<CM, ST>(own, up, dn, lf, rt, j0, q, K, R, lut, ne_final, ne_old);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -298,7 +472,7 @@ __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint3
 // the table would be too large: one counter per state and a warp-aggregated add instead.
 constexpr uint32_t HIST_LANE_QMAX = 64;
 
-__device__ __forceinline__ uint32_t hist_words(uint32_t q) { return q <= HIST_LANE_QMAX ? q * 32u : q; }
+__host__ __device__ inline uint32_t hist_words(uint32_t q) { return q <= HIST_LANE_QMAX ? q * 32u : q; }
 
 __device__ __forceinline__ void hist_add_word(uint32_t *s_hist, uint32_t q, uint32_t word, uint32_t lane)
 {

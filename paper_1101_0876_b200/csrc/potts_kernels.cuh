@@ -8,6 +8,8 @@
 // plane 1-c:  up [i-1][k], down [i+1][k], and horizontally [i][k],[i][k+1] if p = 1 or
 // [i][k-1],[i][k] if p = 0 (indices periodic).
 #pragma once
+#include <type_traits>
+
 #include "potts_core.cuh"
 
 namespace potts {
@@ -21,146 +23,154 @@ struct SweepParams {
     uint32_t colour;            // 0 = white ((i+j) even), 1 = black
     HalfSweepKeys K;            // Philox key material of (seed, t, colour), built on the host
     uint32_t thr[4];            // floor(2^32 exp(-d/T)), d = 1..4
-    unsigned long long *E_out;  // MEASURE: -= satisfied bonds seen from this colour's sites
+    unsigned long long *E_out;  // MEASURE: -= satisfied bonds seen from this colour's sites; DELTA: += energy change
     unsigned long long *hist_out;  // HIST: += occupancies of this colour's sites after the update
-    int32_t rpt;                // rows per thread (divides L / HS_WARPS)
+    int32_t rpw;                // rows per warp (even, divides L / HS_WARPS)
 };
 
 // ---------------------------------------------------------------------------------------------
-// Half-sweep, U8 layout.  A thread updates 16 consecutive same-colour sites (one 16-byte chunk) of
-// P.rpt consecutive rows; a warp covers 32 chunks, a block HS_WARPS groups of rows.
-// grid = (ceil(L/32 / 32), L / (HS_WARPS * rpt)).  Requires L % 32 == 0.  rpt up to 8 amortises the
-// prologue and the block turnover on large lattices; small ones keep rpt low to fill the GPU.
+// Half-sweep, U8 layout, one launch per colour.  A block is HS_WARPS warps; it owns a tile of 32 x 16 = 512
+// same-colour sites (1024 lattice columns) x HS_WARPS * rpw rows.  Warp w walks DOWN its rpw consecutive rows; a
+// lane updates one 16-byte chunk (16 consecutive same-colour sites) per row.  Walking down means
+//   * the other-colour rows i-1, i, i+1 roll through registers: one 16-byte load of row i+1 per row visit
+//     instead of three (the word left / right of the chunk is a fourth, 4-byte load from L1);
+//   * the nibble-doubling of a neighbour word (prep_nbr) is done once per loaded word, not once per use;
+//   * the column part of Philox (ColKeys: 3 of the 17 multiplies, 2 of the 18 XORs per site) is computed once
+//     per block for the tile's 2 x 512 columns (both row parities), kept in 16 KB of shared memory and read
+//     back with one conflict-free 16-byte load per site.
+// grid = (ceil(L/32 / 32), L / (HS_WARPS * rpw)).  Requires L % 32 == 0.
+// MEASURE: E -= satisfied bonds seen from this colour's sites (colour 1 of a sampled sweep).  HIST: occupancy of
+// the words just written.  DELTA (potts_sweep_delta: "a parallel accumulation of local energy
+// changes on-the-fly"): E_out += sum over accepted moves of d = n_old - n_new (R5, R7), no energy recount.
 constexpr int HS_WARPS = 4;
+constexpr int HS_SITES = 16;          // same-colour sites per lane and row
 
-template <int CM, int ST, bool MEASURE, bool HIST>
-__global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_u8(const __grid_constant__ SweepParams P)
+template <int CM, int ST, bool MEASURE, bool HIST, bool DELTA>
+__global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_constant__ SweepParams P)
 {
-    extern __shared__ uint32_t s_dyn[];             // HIST: the block's histogram table
-    __shared__ uint32_t lut[12];
-    __shared__ uint32_t blockE;
-    const uint32_t tid = threadIdx.y * 32u + threadIdx.x;
-    if (tid < 9) lut[tid] = tid >= 5 ? P.thr[tid - 5] : 0u;
-    if (MEASURE && tid == 0) blockE = 0u;
+    constexpr bool EX = MEASURE || DELTA;
+    extern __shared__ uint32_t s_dyn[];                       // HIST: the block's histogram table
+    __shared__ uint4 s_col[2][HS_SITES][32];                  // ColKeys of [row parity p][site of the chunk][lane]
+    __shared__ AcceptEntry<EX> lut[ACCEPT_ENTRIES];
+    __shared__ int blockAcc;
+    const uint32_t lane = threadIdx.x, wy = threadIdx.y, tid = wy * 32u + lane;
+    accept_lut_fill<EX>(lut, P.thr, tid, 32 * HS_WARPS);
+    if (EX && tid == 0) blockAcc = 0;
     if (HIST)
         for (uint32_t n = tid; n < hist_words(P.q); n += 32 * HS_WARPS) s_dyn[n] = 0u;
-    __syncthreads();
 
     const int chunks = P.pitch >> 4;                                  // 16-byte chunks per row
-    const int x = (int)(blockIdx.x * 32u + threadIdx.x);
-    const int i0 = (int)(blockIdx.y * HS_WARPS + threadIdx.y) * P.rpt;
-    uint32_t satisfied = 0;
-    if (x < chunks) {
-        const int k0 = x << 4;
-        const HalfSweepKeys &K = P.K;
-        const uint32_t q = in_register(P.q);
-        const int kn = wrap(k0 + 16, P.pitch), kp = wrap(k0 - 4, P.pitch);
-#pragma unroll 1
-        for (int r = 0; r < P.rpt; ++r) {
-            const int i = i0 + r;
-            const uint32_t p = (uint32_t)(i + P.colour) & 1u;
-            const int iu = wrap(i - 1, P.L), id = wrap(i + 1, P.L);
-            const size_t row = (size_t)i * P.pitch;
-            const uint4 own4 = *reinterpret_cast<const uint4 *>(P.plane_own + row + k0);
-            const uint4 mid4 = *reinterpret_cast<const uint4 *>(P.plane_oth + row + k0);
-            const uint4 up4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)iu * P.pitch + k0);
-            const uint4 dn4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)id * P.pitch + k0);
-            // the one word outside the chunk: [i][k0+16..] if p = 1, [i][..k0-1] if p = 0 (periodic)
-            const uint32_t adj = *reinterpret_cast<const uint32_t *>(P.plane_oth + row + (p ? kn : kp));
-
-            const RowKeys R = row_keys(K, (uint32_t)i);
-            const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
-            const uint32_t mid[6] = {adj, mid4.x, mid4.y, mid4.z, mid4.w, adj};
-            const uint32_t up[4] = {up4.x, up4.y, up4.z, up4.w};
-            const uint32_t dn[4] = {dn4.x, dn4.y, dn4.z, dn4.w};
-            uint32_t out[4], nef_sum = 0;
+    const int x = (int)(blockIdx.x * 32u + lane);
+    const bool active = x < chunks;
+    const int k0 = x << 4;
+    const HalfSweepKeys &K = P.K;
+    if (active) {
+        // site n of my chunk in a row of parity p sits at column j = 2 (k0 + n) + p
 #pragma unroll
-            for (int n = 0; n < 4; ++n) {
-                uint32_t lf, rt, nef;
-                horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
-                out[n] = update_word<CM, ST>(own[n], up[n], dn[n], lf, rt, 2u * (uint32_t)(k0 + 4 * n) + p, q, K, R, lut, nef);
-                if (MEASURE) nef_sum += nef;                          // bytes stay <= 16
-                if (HIST) hist_add_word(s_dyn, P.q, out[n], threadIdx.x);
+        for (int nn = 0; nn < HS_SITES / HS_WARPS; ++nn) {
+            const int n = (int)wy * (HS_SITES / HS_WARPS) + nn;
+#pragma unroll
+            for (int p = 0; p < 2; ++p) {
+                const ColKeys C = col_keys(K, 2u * (uint32_t)(k0 + n) + (uint32_t)p);
+                s_col[p][n][lane] = make_uint4(C.l0, C.l1, C.ph, C.pl);
             }
-            *reinterpret_cast<uint4 *>(P.plane_own + row + k0) = make_uint4(out[0], out[1], out[2], out[3]);
-            if (MEASURE) satisfied += 64u - byte_sum(nef_sum);
         }
     }
-    if (MEASURE) {
+    __syncthreads();
+
+    int d_sum = 0, c_sum = 0;
+    if (active) {
+        const uint32_t q = in_register(P.q);
+        const int L = P.L, pitch = P.pitch;
+        const int i0 = (int)(blockIdx.y * HS_WARPS + wy) * P.rpw;
+        const int kn = wrap(k0 + 16, pitch), kp = wrap(k0 - 4, pitch);
+        const uint8_t *const oth = P.plane_oth + k0;
+        uint8_t *const ownp = P.plane_own + k0;
+
+        // one row visit; PAR = (i + colour) & 1 is uniform over the block row
+        auto visit = [&](auto par, int i, const uint4 &own4, const uint32_t (&up)[4], const uint32_t (&mid)[4], uint32_t adjp,
+                         const uint32_t (&dn)[4]) {
+            constexpr int PAR = decltype(par)::value;
+            const RowKeysH R = row_keys_h(K, (uint32_t)i);
+            const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
+            uint32_t out[4];
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
-        if (threadIdx.x == 0) atomicAdd(&blockE, satisfied);
+            for (int n = 0; n < 4; ++n) {
+                uint32_t nb[4];
+                nb[0] = up[n];
+                nb[1] = dn[n];
+                if (PAR) {      // horizontal neighbours at k and k+1
+                    nb[2] = mid[n];
+                    nb[3] = __funnelshift_r(mid[n], n < 3 ? mid[n < 3 ? n + 1 : 3] : adjp, 8);
+                } else {        // at k-1 and k
+                    nb[2] = __funnelshift_l(n > 0 ? mid[n > 0 ? n - 1 : 0] : adjp, mid[n], 8);
+                    nb[3] = mid[n];
+                }
+                uint32_t w0[4], w1[4];
+                if (ST == 1) {
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) {
+                        const uint4 c = s_col[PAR][4 * n + b][lane];
+                        philox_site_h(K, R, ColKeys{c.x, c.y, c.z, c.w}, w0[b], w1[b]);
+                    }
+                } else {
+#pragma unroll
+                    for (int m = 0; m < 2; ++m) {
+                        const uint4 c = s_col[PAR][4 * n + 2 * m][lane];
+                        uint32_t w[4];
+                        philox_pair_h(K, R, ColKeys{c.x, c.y, c.z, c.w}, w);
+                        w0[2 * m] = w[0]; w1[2 * m] = w[1]; w0[2 * m + 1] = w[2]; w1[2 * m + 1] = w[3];
+                    }
+                }
+                out[n] = metropolis_word<CM, EX>(own[n], nb, q, w0, w1, lut, d_sum, c_sum);
+                if (HIST) hist_add_word(s_dyn, P.q, out[n], lane);
+            }
+            *reinterpret_cast<uint4 *>(ownp + (size_t)i * pitch) = make_uint4(out[0], out[1], out[2], out[3]);
+        };
+        auto ld16 = [](const uint8_t *p) { return *reinterpret_cast<const uint4 *>(p); };
+        auto prep4 = [](const uint4 &v, uint32_t (&w)[4]) {
+            w[0] = prep_nbr<CM>(v.x); w[1] = prep_nbr<CM>(v.y); w[2] = prep_nbr<CM>(v.z); w[3] = prep_nbr<CM>(v.w);
+        };
+
+        uint32_t up[4], mid[4], dn[4];
+        prep4(ld16(oth + (size_t)wrap(i0 - 1, L) * pitch), up);
+        prep4(ld16(oth + (size_t)i0 * pitch), mid);
+        uint32_t p = (uint32_t)(i0 + P.colour) & 1u;
+        uint4 own4 = ld16(ownp + (size_t)i0 * pitch);
+        uint4 dn4 = ld16(oth + (size_t)wrap(i0 + 1, L) * pitch);
+        uint32_t adj = *reinterpret_cast<const uint32_t *>(P.plane_oth + (size_t)i0 * pitch + (p ? kn : kp));
+#pragma unroll 1
+        for (int r = 0; r < P.rpw; ++r) {
+            const int i = i0 + r;
+            // next row's loads first: they have the whole visit to arrive (the last visit reloads its own row)
+            const int inx = r + 1 < P.rpw ? i + 1 : i;
+            const uint4 own_nx = ld16(ownp + (size_t)inx * pitch);
+            const uint4 dn_nx = ld16(oth + (size_t)wrap(inx + 1, L) * pitch);
+            const uint32_t adj_nx = *reinterpret_cast<const uint32_t *>(P.plane_oth + (size_t)inx * pitch + (p ? kp : kn));
+            prep4(dn4, dn);
+            const uint32_t adjp = prep_nbr<CM>(adj);
+            if (p) visit(std::integral_constant<int, 1>{}, i, own4, up, mid, adjp, dn);
+            else visit(std::integral_constant<int, 0>{}, i, own4, up, mid, adjp, dn);
+#pragma unroll
+            for (int n = 0; n < 4; ++n) { up[n] = mid[n]; mid[n] = dn[n]; }
+            own4 = own_nx; dn4 = dn_nx; adj = adj_nx;
+            p ^= 1u;
+        }
+    }
+    if (EX) {
+        // MEASURE: satisfied bonds = 4 per site - unequal neighbours of the final spins = 64 rpw - (c_sum + d_sum)
+        int v = DELTA ? d_sum : (active ? 64 * P.rpw - (c_sum + d_sum) : 0);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) atomicAdd(&blockAcc, v);
         __syncthreads();
-        // E = -(satisfied bonds): accumulate the two's-complement negative into the int64 slot
-        if (tid == 0) atomicAdd(P.E_out, 0ull - (unsigned long long)blockE);
+        // E = -(satisfied bonds): accumulate the two's-complement negative into the int64 slot; DELTA: += the change
+        if (tid == 0) atomicAdd(P.E_out, DELTA ? (unsigned long long)(long long)blockAcc : 0ull - (unsigned long long)(long long)blockAcc);
     }
     if (HIST) {
         __syncthreads();
         hist_flush(s_dyn, P.q, P.hist_out, tid, 32 * HS_WARPS);
     }
-}
-
-// ---------------------------------------------------------------------------------------------
-// Half-sweep with the on-the-fly energy change ("keeping track of the energy changes at
-// each spin flip ... a parallel accumulation of local energy changes on-the-fly" for reweighting runs):
-// adds  sum over accepted moves of d = n_old - n_new  (R5, R7) of this half-sweep to *dE_out, as a
-// two's-complement int64.  No energy recount: per site d_accepted = ne(final spin) - ne(old spin), where ne is
-// the count of unequal neighbours, so the half-sweep's sum is byte_sum(ne_final) - byte_sum(ne_old).
-// Same thread map as k_half_sweep_u8 (P.rpt rows per thread); a separate kernel so that the plain path's code
-// generation is untouched.
-template <int CM, int ST>
-__global__ void __launch_bounds__(32 * HS_WARPS) k_half_sweep_delta_u8(const __grid_constant__ SweepParams P,
-                                                                       unsigned long long *dE_out)
-{
-    __shared__ uint32_t lut[12];
-    __shared__ int blockD;
-    const uint32_t tid = threadIdx.y * 32u + threadIdx.x;
-    if (tid < 9) lut[tid] = tid >= 5 ? P.thr[tid - 5] : 0u;
-    if (tid == 0) blockD = 0;
-    __syncthreads();
-
-    const int chunks = P.pitch >> 4;
-    const int x = (int)(blockIdx.x * 32u + threadIdx.x);
-    const int i0 = (int)(blockIdx.y * HS_WARPS + threadIdx.y) * P.rpt;
-    int delta = 0;                                                     // |delta| <= 4 * 16 * rpt per thread
-    if (x < chunks) {
-        const int k0 = x << 4;
-        const HalfSweepKeys &K = P.K;
-        const uint32_t q = in_register(P.q);
-        const int kn = wrap(k0 + 16, P.pitch), kp = wrap(k0 - 4, P.pitch);
-#pragma unroll 1
-        for (int r = 0; r < P.rpt; ++r) {
-            const int i = i0 + r;
-            const uint32_t p = (uint32_t)(i + P.colour) & 1u;
-            const int iu = wrap(i - 1, P.L), id = wrap(i + 1, P.L);
-            const size_t row = (size_t)i * P.pitch;
-            const uint4 own4 = *reinterpret_cast<const uint4 *>(P.plane_own + row + k0);
-            const uint4 mid4 = *reinterpret_cast<const uint4 *>(P.plane_oth + row + k0);
-            const uint4 up4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)iu * P.pitch + k0);
-            const uint4 dn4 = *reinterpret_cast<const uint4 *>(P.plane_oth + (size_t)id * P.pitch + k0);
-            const uint32_t adj = *reinterpret_cast<const uint32_t *>(P.plane_oth + row + (p ? kn : kp));
-            const RowKeys R = row_keys(K, (uint32_t)i);
-            const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
-            const uint32_t mid[6] = {adj, mid4.x, mid4.y, mid4.z, mid4.w, adj};
-            const uint32_t up[4] = {up4.x, up4.y, up4.z, up4.w};
-            const uint32_t dn[4] = {dn4.x, dn4.y, dn4.z, dn4.w};
-            uint32_t out[4], d_sum = 0;
-#pragma unroll
-            for (int n = 0; n < 4; ++n) {
-                uint32_t lf, rt, nef, neo;
-                horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
-                out[n] = update_word_ex<CM, ST>(own[n], up[n], dn[n], lf, rt, 2u * (uint32_t)(k0 + 4 * n) + p, q, K, R, lut, nef, neo);
-                d_sum += nef + 0x04040404u - neo;                       // d + 4 per byte; bytes stay <= 32
-            }
-            *reinterpret_cast<uint4 *>(P.plane_own + row + k0) = make_uint4(out[0], out[1], out[2], out[3]);
-            delta += (int)byte_sum(d_sum) - 64;
-        }
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) delta += __shfl_xor_sync(0xffffffffu, delta, o);
-    if (threadIdx.x == 0) atomicAdd(&blockD, delta);
-    __syncthreads();
-    if (tid == 0) atomicAdd(dE_out, (unsigned long long)(long long)blockD);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -240,7 +250,7 @@ __global__ void __launch_bounds__(256) k_measure_u8(const MeasureParams P)
 // ---------------------------------------------------------------------------------------------
 // Random start (R9): s(i,j) = floor(w0 q / 2^32), (w0,..) = Philox((j, i, 0, 2), seed).
 // One thread per 4 consecutive k of one plane row.
-__global__ void k_init_random_u8(uint8_t *plane0, uint8_t *plane1, int L, int pitch, uint32_t q,
+static __global__ void k_init_random_u8(uint8_t *plane0, uint8_t *plane1, int L, int pitch, uint32_t q,
                                  uint32_t key0, uint32_t key1)
 {
     const long long words_per_plane = (long long)L * (pitch >> 2);
@@ -265,7 +275,7 @@ __global__ void k_init_random_u8(uint8_t *plane0, uint8_t *plane1, int L, int pi
 // ---------------------------------------------------------------------------------------------
 // Layout conversion: split planes <-> canonical row-major s[i*L + j], for `rows` rows starting
 // at row i0.  One thread per 4 sites of a plane row (= 8 columns of the lattice row).
-__global__ void k_planes_to_rowmajor(const uint8_t *plane0, const uint8_t *plane1, uint8_t *out,
+static __global__ void k_planes_to_rowmajor(const uint8_t *plane0, const uint8_t *plane1, uint8_t *out,
                                      int L, int pitch, int i0, int rows)
 {
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -283,7 +293,7 @@ __global__ void k_planes_to_rowmajor(const uint8_t *plane0, const uint8_t *plane
     *reinterpret_cast<uint2 *>(out + (size_t)r * L + 8 * kw) = o;
 }
 
-__global__ void k_rowmajor_to_planes(const uint8_t *in, uint8_t *plane0, uint8_t *plane1, int L,
+static __global__ void k_rowmajor_to_planes(const uint8_t *in, uint8_t *plane0, uint8_t *plane1, int L,
                                      int pitch, int i0, int rows, uint32_t q, int *bad)
 {
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;

@@ -82,14 +82,14 @@ constexpr int PK_WARPS = 4;
 template <bool FIVE, int ST, bool MEASURE, bool HIST, bool DELTA = false>
 __global__ void __launch_bounds__(32 * PK_WARPS) k_half_sweep_packed(const __grid_constant__ PackedSweepParams P)
 {
+    constexpr bool EX = MEASURE || DELTA;
+    constexpr int CM = FIVE ? CM_7BIT : CM_NIB4;
     extern __shared__ uint32_t s_dyn[];
-    __shared__ uint32_t lut[12];
-    __shared__ uint32_t blockE;
-    __shared__ int blockD;
+    __shared__ AcceptEntry<EX> lut[ACCEPT_ENTRIES];
+    __shared__ int blockAcc;
     const uint32_t tid = threadIdx.y * 32u + threadIdx.x;
-    if (tid < 9) lut[tid] = tid >= 5 ? P.thr[tid - 5] : 0u;
-    if (MEASURE && tid == 0) blockE = 0u;
-    if (DELTA && tid == 0) blockD = 0;
+    accept_lut_fill<EX>(lut, P.thr, tid, 32 * PK_WARPS);
+    if (EX && tid == 0) blockAcc = 0;
     if (HIST)
         for (uint32_t n = tid; n < hist_words(P.q); n += 32 * PK_WARPS) s_dyn[n] = 0u;
     __syncthreads();
@@ -99,8 +99,7 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_half_sweep_packed(const __gri
     const int x = (int)(blockIdx.x * 32u + threadIdx.x);
     const int i0 = (int)(blockIdx.y * PK_WARPS + threadIdx.y) * P.rpt;
     const int c = (int)P.colour, o = 1 - c;
-    uint32_t satisfied = 0;
-    int delta = 0;
+    int d_sum = 0, c_sum = 0, rows_done = 0;
     if (x < chunks) {
         const HalfSweepKeys &K = P.K;
         const uint32_t q = in_register(P.q);
@@ -136,7 +135,7 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_half_sweep_packed(const __gri
             const uint32_t own_w[4] = {own_n.x, own_n.y, own_n.z, own_n.w};
             const uint32_t up_w[4] = {up_n.x, up_n.y, up_n.z, up_n.w};
             const uint32_t dn_w[4] = {dn_n.x, dn_n.y, dn_n.z, dn_n.w};
-            uint32_t out_w[4], out_h = 0, nef_sum = 0, d_sum = 0;
+            uint32_t out_w[4], out_h = 0;
 #pragma unroll
             for (int m = 0; m < 4; ++m) {
                 uint32_t own[2], up[2], dn[2], out[2];
@@ -146,35 +145,28 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_half_sweep_packed(const __gri
 #pragma unroll
                 for (int hlf = 0; hlf < 2; ++hlf) {
                     const int n = 2 * m + hlf;                        // byte-per-site word n: sites 4n..4n+3
-                    uint32_t lf, rt, nef, neo;
+                    uint32_t lf, rt, w0[4], w1[4];
                     horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
-                    out[hlf] = update_word_ex<FIVE ? CM_7BIT : CM_NIB4, ST>(own[hlf], up[hlf], dn[hlf], lf, rt, 2u * (uint32_t)(32 * x + 4 * n) + p, q, K,
-                                                     R, lut, nef, neo);
-                    if (MEASURE) nef_sum += nef;                      // bytes stay <= 32
-                    if (DELTA) d_sum += nef + 0x04040404u - neo;      // d + 4 per byte; bytes stay <= 64
+                    draw_words<ST>(K, R, 2u * (uint32_t)(32 * x + 4 * n) + p, w0, w1);
+                    const uint32_t nb[4] = {prep_nbr<CM>(up[hlf]), prep_nbr<CM>(dn[hlf]), prep_nbr<CM>(lf), prep_nbr<CM>(rt)};
+                    out[hlf] = metropolis_word<CM, EX>(own[hlf], nb, q, w0, w1, lut, d_sum, c_sum);
                     if (HIST) hist_add_word(s_dyn, P.q, out[hlf], threadIdx.x);
                 }
                 out_w[m] = pack_pair<FIVE>(out[0], out[1], m, out_h);
             }
             *reinterpret_cast<uint4 *>(S.nib[c] + (size_t)i * S.pn + 16 * x) = make_uint4(out_w[0], out_w[1], out_w[2], out_w[3]);
             if (FIVE) *reinterpret_cast<uint32_t *>(S.hb[c] + (size_t)i * S.ph + 4 * x) = out_h;
-            if (MEASURE) satisfied += 128u - byte_sum(nef_sum);
-            if (DELTA) delta += (int)byte_sum(d_sum) - 128;
+            ++rows_done;
         }
     }
-    if (DELTA) {
+    if (EX) {
+        // MEASURE: satisfied bonds = 4 per site - unequal neighbours of the final spins (c_sum + d_sum); DELTA: the change
+        int v = DELTA ? d_sum : 128 * rows_done - (c_sum + d_sum);
 #pragma unroll
-        for (int s = 16; s > 0; s >>= 1) delta += __shfl_xor_sync(0xffffffffu, delta, s);
-        if (threadIdx.x == 0) atomicAdd(&blockD, delta);
+        for (int s = 16; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
+        if (threadIdx.x == 0) atomicAdd(&blockAcc, v);
         __syncthreads();
-        if (tid == 0) atomicAdd(P.E_out, (unsigned long long)(long long)blockD);
-    }
-    if (MEASURE) {
-#pragma unroll
-        for (int s = 16; s > 0; s >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, s);
-        if (threadIdx.x == 0) atomicAdd(&blockE, satisfied);
-        __syncthreads();
-        if (tid == 0) atomicAdd(P.E_out, 0ull - (unsigned long long)blockE);
+        if (tid == 0) atomicAdd(P.E_out, DELTA ? (unsigned long long)(long long)blockAcc : 0ull - (unsigned long long)(long long)blockAcc);
     }
     if (HIST) {
         __syncthreads();

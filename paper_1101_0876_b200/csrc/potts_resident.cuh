@@ -5,9 +5,9 @@
 // [r0, r1) of both colour planes in its shared memory.  A half-sweep of colour c reads only the other
 // plane (sec. 3), so the only data that crosses CTAs are the two boundary rows of the
 // plane just written.  They travel as 8-byte packets {4 spins, sequence number} written straight into
-// the neighbour's inbox in global memory (L2) by the thread that computed them; an aligned 8-byte
-// store is single-copy atomic, so the receiver just polls the packet until the sequence number is
-// the one it expects: no fence, no separate flag, one L2 round trip.
+// the neighbour's inbox in global memory (L2) by the thread that computed them; a packet is one aligned
+// 64-bit scalar, single-copy atomic in the PTX memory model, so the receiver just polls the packet until
+// the sequence number is the one it expects: no fence, no separate flag, one L2 round trip.
 //
 //   Threads [0, ncw*32) compute: thread (cx, ty) owns the 8-site chunk cx (two words) of the rows dealt to
 //   thread row ty (round-robin, interior rows first, the CTA's first and last row at the very end).
@@ -47,6 +47,7 @@ struct ResidentParams {
     uint32_t every;                   // sample after every `every`-th sweep of this launch; 0 = never
     unsigned long long *E_series;     // device, nsweeps/every entries, may be null
     unsigned long long *hist_series;  // device, nsweeps/every rows of q, may be null
+    unsigned long long *dE_series;    // device, nsweeps entries (zeroed), may be null: += energy change of every sweep
     uint2 *inbox;                     // [gridDim.x][2 colours][2 sides][wpr] packets, zeroed before the launch
     int *error;                       // set to 1 if a wait gave up
     int32_t rows_max;                 // rows of shared memory per plane = rows_max + 2
@@ -55,24 +56,29 @@ struct ResidentParams {
 
 constexpr long long RESIDENT_SPIN_LIMIT = 1ll << 24;   // polls before a wait gives up (seconds)
 
-// two packets (an 8-site chunk) at once; each 8-byte half is still atomic on its own
+// A packet is ONE 64-bit scalar {4 spins | sequence number << 32}: the PTX memory model treats a vector access as
+// independent accesses of its elements, so with 64-bit elements "spins and tag arrive together" is guaranteed by the
+// model (single-copy atomicity of an aligned scalar), not by the hardware's habit.  Two packets (an 8-site chunk)
+// travel as one .v2.b64 access: two such elements.
 __device__ __forceinline__ uint4 ld_packet2(const uint2 *p)
 {
-    uint4 v;
-    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
-    return v;
+    unsigned long long a, b;
+    asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+    return make_uint4((uint32_t)a, (uint32_t)(a >> 32), (uint32_t)b, (uint32_t)(b >> 32));
 }
 
-__device__ __forceinline__ void st_packet2(uint2 *p, uint2 data, uint32_t seq)
+__device__ __forceinline__ unsigned long long make_packet(uint32_t spins, uint32_t seq)
 {
-    asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %2};" ::"l"(p), "r"(data.x), "r"(seq), "r"(data.y) : "memory");
+    unsigned long long v;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "r"(spins), "r"(seq));
+    return v;
 }
 
 template <int W>
 __device__ __forceinline__ void st_packets(uint2 *p, uint2 data, uint32_t seq)
 {
-    if (W == 2) st_packet2(p, data, seq);
-    else asm volatile("st.relaxed.gpu.global.v2.u32 [%0], {%1, %2};" ::"l"(p), "r"(data.x), "r"(seq) : "memory");
+    if (W == 2) asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"(make_packet(data.x, seq)), "l"(make_packet(data.y, seq)) : "memory");
+    else asm volatile("st.relaxed.gpu.global.b64 [%0], %1;" ::"l"(p), "l"(make_packet(data.x, seq)) : "memory");
 }
 
 __device__ __forceinline__ void named_barrier_sync(int id, int nthreads)
@@ -91,7 +97,7 @@ struct ResidentLattice {
     uint8_t *plane[2];
     uint32_t key0, key1;
     uint32_t thr[4];
-    unsigned long long *E_series, *hist_series;
+    unsigned long long *E_series, *hist_series, *dE_series;
 };
 
 // W = words (4 sites each) a compute thread updates per row visit: 2 (an 8-site chunk: less bookkeeping per site) or
@@ -100,7 +106,7 @@ template <int CM, int W, int ST>
 __device__ __forceinline__ void resident_run(const ResidentParams &P, const ResidentLattice &X)
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
-    __shared__ uint32_t lut[12];
+    __shared__ AcceptEntry<true> lut[ACCEPT_ENTRIES];
 
     const uint32_t G = X.G, b = X.b;
     const int L = P.L, pitch = P.pitch;
@@ -140,8 +146,9 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
     }
     const bool do_hist = X.hist_series != nullptr && P.every != 0;
     const bool do_E = X.E_series != nullptr && P.every != 0;
+    const bool do_D = X.dE_series != nullptr;
 
-    if (tid >= 5 && tid < 9) lut[tid] = tid == 5 ? X.thr[0] : (tid == 6 ? X.thr[1] : (tid == 7 ? X.thr[2] : X.thr[3]));
+    accept_lut_fill<true>(lut, X.thr, tid, nthreads);
     if (do_hist)
         for (uint32_t n = tid; n < hist_words(P.q); n += nthreads) s_hist[n] = 0u;
     // own rows of both planes, and the halo rows of plane 1 (read by the first half-sweep, colour 0):
@@ -185,8 +192,10 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
             ++seq;
             uint8_t *const own_col = s_raw + c * plane_stride + col;                      // + lr*pitch: my chunk
             const uint8_t *const oth_row = s_raw + (1u - c) * plane_stride;               // + lr*pitch: row start
-            uint32_t nef_sum = 0, words_done = 0;
+            int d_sum = 0, c_sum = 0;
+            uint32_t words_done = 0;
             const bool count_E = sample && c == 1 && do_E, count_H = sample && do_hist;
+            const bool ex = count_E || do_D;                        // form the EX sums (uniform over the block)
             if ((int)tid < nbar) {
                 const HalfSweepKeys K = half_sweep_keys(X.key0, X.key1, t, c);             // uniform registers
                 // one visit: local row lr, my W words
@@ -203,25 +212,25 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                         const uint2 mid = *reinterpret_cast<const uint2 *>(orow + col);
                         const uint2 up = *reinterpret_cast<const uint2 *>(orow + col - pitch);
                         const uint2 dn = *reinterpret_cast<const uint2 *>(orow + col + pitch);
-                        uint32_t lf0, rt0, lf1, rt1, nef0, nef1;
+                        uint32_t lf0, rt0, lf1, rt1;
                         horizontal(p, mid.x, p ? mid.y : adj, lf0, rt0);
                         horizontal(p, mid.y, p ? adj : mid.x, lf1, rt1);
-                        out.x = update_word<CM, ST>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, lut, nef0);
-                        out.y = update_word<CM, ST>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, lut, nef1);
+                        out.x = update_word<CM, ST>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, lut, ex, d_sum, c_sum);
+                        out.y = update_word<CM, ST>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, lut, ex, d_sum, c_sum);
                         *reinterpret_cast<uint2 *>(own_col + ro) = out;
-                        if (count_E) { nef_sum += nef0 + nef1; words_done += 2; }
+                        words_done += 2;
                         if (count_H) { hist_add_word(s_hist, P.q, out.x, tid & 31u); hist_add_word(s_hist, P.q, out.y, tid & 31u); }
                     } else {
                         const uint32_t own = *reinterpret_cast<const uint32_t *>(own_col + ro);
                         const uint32_t mid = *reinterpret_cast<const uint32_t *>(orow + col);
                         const uint32_t up = *reinterpret_cast<const uint32_t *>(orow + col - pitch);
                         const uint32_t dn = *reinterpret_cast<const uint32_t *>(orow + col + pitch);
-                        uint32_t lf, rt, nef;
+                        uint32_t lf, rt;
                         horizontal(p, mid, adj, lf, rt);
-                        out.x = update_word<CM, ST>(own, up, dn, lf, rt, 2u * col + p, q, K, R, lut, nef);
+                        out.x = update_word<CM, ST>(own, up, dn, lf, rt, 2u * col + p, q, K, R, lut, ex, d_sum, c_sum);
                         out.y = 0u;
                         *reinterpret_cast<uint32_t *>(own_col + ro) = out.x;
-                        if (count_E) { nef_sum += nef; words_done += 1; }
+                        words_done += 1;
                         if (count_H) hist_add_word(s_hist, P.q, out.x, tid & 31u);
                     }
                     return out;
@@ -275,12 +284,18 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                 __syncthreads();
             }
 
+            if (do_D) {
+                // energy change of this half-sweep = sum of d over its accepted moves (R5, R7): one int64 atomic per warp
+                int dd = d_sum;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) dd += __shfl_xor_sync(0xffffffffu, dd, o);
+                if ((tid & 31u) == 0 && dd) atomicAdd(X.dE_series + n, (unsigned long long)(long long)dd);
+            }
             if (sample && c == 1) {
                 if (do_E) {
-                    // satisfied bonds seen from this thread's black sites = 4 per site - unequal neighbours
-                    // (nef_sum holds 4 byte counters, +<= 8 per visit: the host keeps visits per thread <= 30);
-                    // one fire-and-forget int64 atomic per warp: no block-wide barrier for the energy
-                    uint32_t satisfied = 16u * words_done - byte_sum(nef_sum);
+                    // satisfied bonds seen from this thread's black sites = 4 per site - unequal neighbours of the final
+                    // spins (c_sum + d_sum); one fire-and-forget int64 atomic per warp: no block-wide barrier for the energy
+                    uint32_t satisfied = 16u * words_done - (uint32_t)(c_sum + d_sum);
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
                     if ((tid & 31u) == 0 && satisfied) atomicAdd(X.E_series + sample_idx, 0ull - (unsigned long long)satisfied);
@@ -320,6 +335,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
     for (int d = 0; d < 4; ++d) X.thr[d] = P.thr[d];
     X.E_series = P.E_series;
     X.hist_series = P.hist_series;
+    X.dE_series = P.dE_series;
     resident_run<CM, W, ST>(P, X);
 }
 
@@ -355,6 +371,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_batch_u8(const __grid_cons
     for (int d = 0; d < 4; ++d) X.thr[d] = T.thr[r][d];
     X.E_series = B.P.E_series ? B.P.E_series + r * B.series_stride : nullptr;
     X.hist_series = B.P.hist_series ? B.P.hist_series + r * B.series_stride * B.P.q : nullptr;
+    X.dE_series = B.P.dE_series ? B.P.dE_series + r * (unsigned long long)B.P.nsweeps : nullptr;
     resident_run<CM, 1, ST>(B.P, X);      // one word per thread and row visit: small lattices want warps, not amortisation
 }
 
