@@ -2,19 +2,20 @@
 """bench.py -- throughput of the checkerboard Potts sweep on B200 (driver contract).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--workload cfgN] [--no-per-config] [--no-cpu-baseline]
+                    [--workload cfgN] [--no-per-config] [--no-cpu-baseline] [--no-e2e]
 
-A "step" is one pass of the whole hot path over one workload of BASELINE.json: create the
-start state, then `sweeps` checkerboard Metropolis sweeps at the workload's temperature(s) with
-the workload's measurement cadence (energy / histogram series recorded on the device).  The
-default workload is BASELINE.json configs[1] (q=6, L=1024, ordered start, 1.005 T_c, 10^4
-sweeps, energy every sweep).  `value` = spin-flip attempts per second (= 1e9 / ns-per-flip),
-inputs resident in HBM; `e2e` = the same through the C-ABI with HOST buffers (upload of the
-start configuration from pinned host memory, series + final configuration copied back).
+A "step" is one pass of the whole hot path over one workload of BASELINE.json: the start state (untimed: a fresh
+handle per step), then ALL sweeps of the workload at its temperature(s) with its measurement cadence (energy /
+histogram series recorded on the device).  The default workload is the largest single-GPU configuration,
+BASELINE.json configs[4] (q=9, L=32768, random start, 0.995 T_c, 1000 sweeps, energy + histogram every 10):
+BASELINE's metric names no configuration, and north_star's target sentence names L = 32768.  configs[0..3] are
+rows of `per_config`, each at full length with its own roofline object and a with / without fused-measurement pair.
+`value` = spin-flip attempts per second (= 1e9 / ns-per-flip), inputs resident in HBM; `e2e` = the same through
+the C-ABI with HOST buffers (potts_upload of the start configuration from pinned host memory, series and final
+configuration copied back).
 
-N > 1 (torchrun): the paper averages over independent samples ("repeat over
-samples"), so rank r runs sample r (seed + r) of the same workload: no data-path collective,
-weak scaling; the time is the max over ranks.
+N > 1 (torchrun): the paper averages over independent samples ("repeat over samples"), so rank r runs
+sample r (seed + r) of the same workload: no data-path collective, weak scaling; the time is the max over ranks.
 
 Rank 0 prints ONE JSON line.  See DESIGN.md section 8 for every field.
 """
@@ -32,26 +33,28 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-import numpy as np  # noqa: E402
+import numpy as np  # noqa: E402,F401
 
 import workloads  # noqa: E402
 
 # ---- roofline constants -------------------------------------------------
 SM_COUNT = 148
 ISSUE_LANES_PER_SM_CLK = 128          # 4 SMSPs x 1 warp-instruction (32 lanes) per clock
-I_ALG_PER_UPDATE = 36                 # Philox4x32-10 words 0,1 of counter (j,i,t,colour): 17 IMAD.WIDE + 18 LOP3, + 1 IMAD.HI proposal
-BYTES_ALG_PER_UPDATE_U8 = 3.0         # read own + read other (once) + write own, uint8 planes
+I_ALG_PER_UPDATE = 36                 # Philox4x32-10 words 0,1 of counter (j,i,t,colour): 17 IMAD.WIDE + 18 LOP3, + 1 multiply for the proposal
 # Measured on B200 (profiles/r01b_pipe_model.md): for this integer mix (IMAD.WIDE / LOP3 / IADD3 / SHF / PRMT) an SM
 # sub-partition retires one warp instruction every 2 clocks, whichever pipe it goes to: half the nominal issue rate.
 MEASURED_INT_ISSUE_PER_CLK = 0.5
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the
-# `ncu --set full` capture summarised in profiles/ (None until a capture exists for the workload)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {          # profiles/r01c_kernels.md
-    "cfg2_q6_L1024": 1.113e6 + 5.1e3,      # resident kernel: the lattice is loaded once per launch, whatever the sweep count
-    "cfg3_q9_L4096": 17.30e6 + 8.7e3,
-    "cfg4_q24_L8192": 41.98e6 + 1.5e3,     # 40 MB of packed planes, L2-resident after the first touch
-    "cfg5_q9_L32768": 1.0738e9 + 0.4973e9,
-}
+HEADLINE = 5                          # BASELINE.json configs[4]: the largest single-GPU configuration
+
+
+def ncu_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of each workload's dominant kernel, from the
+    `ncu --set full` captures summarised under profiles/ (the table names its capture and command)."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(p):
+        return {}
+    with open(p) as f:
+        return {k: v for k, v in json.load(f).items() if not k.startswith("_")}
 
 
 def _peaks():
@@ -125,9 +128,11 @@ def slice_of(w: workloads.Workload, max_sweeps: int | None):
 class GpuRun:
     """Drives the product through the Python binding of the C-ABI (argument marshalling only)."""
 
-    def __init__(self, pb, torch, w: workloads.Workload, seed: int, max_sweeps: int | None, options=None, stream_spec=1):
+    def __init__(self, pb, torch, w: workloads.Workload, seed: int, max_sweeps: int | None, options=None, stream_spec=1,
+                 measure=True):
         self.pb, self.torch, self.w, self.seed = pb, torch, w, seed
         self.stream_spec = stream_spec
+        self.measure = measure                         # False: the same sweeps without the fused measurement
         self.temps, self.per_t = slice_of(w, max_sweeps)
         self.sweeps = self.per_t * len(self.temps)
         self.updates = self.sweeps * w.L * w.L
@@ -160,7 +165,7 @@ class GpuRun:
             return "k_half_sweep_packed"
         if self.cluster_ctas:
             return "k_cluster_u8"
-        return "k_resident_u8" if self.resident_ctas else "k_half_sweep_u8"
+        return "k_resident_u8" if self.resident_ctas else "k_sweep_rows_u8"
 
     @property
     def kernel_launches_per_step(self):
@@ -169,6 +174,10 @@ class GpuRun:
     def enqueue(self):
         """The step: all sweeps with the device-resident series; returns without a sync."""
         per_s = self.per_t // self.w.every
+        if not self.measure:
+            for T in self.temps:
+                self.g.potts_sweep(T, self.per_t)
+            return
         for n, T in enumerate(self.temps):
             E = self.E_dev[n * per_s:(n + 1) * per_s]
             H = self.H_dev[n * per_s:(n + 1) * per_s] if self.H_dev is not None else None
@@ -236,55 +245,72 @@ def host_threads() -> int:
         return os.cpu_count() or 1
 
 
-def oracle_time(w: workloads.Workload, sweeps: int, threads: int):
-    """Seconds the oracle, as it stands, needs for `sweeps` sweeps of workload w (with its cadence)."""
-    import oracle
-    o = oracle.OraclePotts(w.L, w.q, w.seed, w.init, threads=threads)
-    sweeps = max(w.every, sweeps // w.every * w.every)
+def oracle_step(o, w: workloads.Workload, sweeps: int):
+    """Seconds the oracle, as it stands, needs for the next `sweeps` sweeps of workload w with its cadence
+    (a multiple of w.every), continuing its chain."""
     t0 = time.perf_counter()
     o.sweep_measured(w.temperatures[0], sweeps, w.every, hist=w.hist)
-    dt = time.perf_counter() - t0
-    used = o.threads
-    o.close()
-    return dt, sweeps, used
+    return time.perf_counter() - t0
 
 
 def cpu_baseline(w: workloads.Workload, budget_s: float = 12.0):
-    """The oracle on a bounded sample of the workload: all host threads (row-parallel mode, same
-    bits) and one thread.  Returns the cpu_baseline object of the JSON line."""
+    """The oracle on a bounded sample of the workload: all host threads (row-parallel mode, same bits), then
+    one thread.  The smallest sample that keeps the workload's cadence is `every` sweeps; at L = 32768 that is
+    already ~40 s on 16 threads, so it is not repeated.  Returns the cpu_baseline object of the JSON line."""
+    import oracle
     threads = host_threads()
-    dt, n, _ = oracle_time(w, w.every, threads)                      # calibration (and page-in)
-    per_sweep = max(dt / n, 1e-6)
-    sweeps = int(min(w.total_sweeps, max(w.every, budget_s / per_sweep)))
-    dt, n, used = oracle_time(w, sweeps, threads)
+    o = oracle.OraclePotts(w.L, w.q, w.seed, w.init, threads=threads)        # start state: untimed
+    used = o.threads
+    dt = oracle_step(o, w, w.every)
+    n = w.every
+    if dt < budget_s / 2:                                                    # small lattice: a longer sample
+        n = int(min(w.total_sweeps, max(w.every, (budget_s / (dt / w.every)) // w.every * w.every)))
+        dt = oracle_step(o, w, n)
     multi = n * w.L * w.L / dt
-    n1 = max(w.every, int(n / max(threads, 1) / 2))
-    dt1, n1, _ = oracle_time(w, n1, 1)
+    # one thread: one plain sweep of the same lattice if a whole cadence period would take minutes
+    o.set_threads(1)
+    est1 = dt / n * min(used, 16)
+    if est1 * w.every > 3 * budget_s:
+        t0 = time.perf_counter()
+        o.sweep(w.temperatures[0], 1)
+        dt1, n1, what = time.perf_counter() - t0, 1, "1 sweep without measurement"
+    else:
+        n1 = w.every
+        dt1, what = oracle_step(o, w, n1), f"{n1} sweeps with its measurement cadence"
     single = n1 * w.L * w.L / dt1
+    o.close()
     return {"value": multi, "unit": "spin updates/s", "cores": used, "kind": "oracle",
-            "sample": f"{n} sweeps of {w.name} (L={w.L}, q={w.q}) with its measurement cadence, {dt:.1f} s",
+            "sample": f"{n} sweeps of {w.name} (L={w.L}, q={w.q}) with its measurement cadence, {dt:.1f} s on {used} threads",
             "ns_per_spin_flip": 1e9 / multi,
-            "single_thread": {"value": single, "ns_per_spin_flip": 1e9 / single,
-                              "sample": f"{n1} sweeps, {dt1:.1f} s"}}
+            "single_thread": {"value": single, "ns_per_spin_flip": 1e9 / single, "cores": 1,
+                              "sample": f"{what} of the same lattice, {dt1:.1f} s"}}
 
 
 def run_reference(args, w):
-    """--impl reference: the oracle on the host cores, same metric / config; rank 0 only."""
+    """--impl reference: the oracle on the host cores, same metric / config; rank 0 only.  Each step is a bounded
+    sample of the workload (whole cadence periods, continuing one chain) sized so that the run ends in minutes."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
+    import oracle
     threads = host_threads()
-    dt, n, _ = oracle_time(w, w.every, threads)
-    per_sweep = max(dt / n, 1e-6)
+    o = oracle.OraclePotts(w.L, w.q, w.seed, w.init, threads=threads)
+    used = o.threads
     total = args.steps + args.warmup
-    sweeps = int(min(w.total_sweeps, max(w.every, (90.0 / total) / per_sweep)))   # whole run ~1.5 min
+    dt = oracle_step(o, w, w.every)                                  # calibration, counts as the first warm-up step
+    per_sweep = max(dt / w.every, 1e-9)
+    sweeps = int(min(w.total_sweeps, max(w.every, ((200.0 / total) / per_sweep) // w.every * w.every)))
     times = []
-    for it in range(total):
-        dt, n, used = oracle_time(w, sweeps, threads)
+    for it in range(1, total):
+        dt = oracle_step(o, w, sweeps)
         if it >= args.warmup:
             times.append(dt)
+    if not times:
+        times = [dt]
+    o.close()
+    n = sweeps
     sec = sum(times) / len(times)
     val = n * w.L * w.L / sec
-    sample = f"each step = {n} sweeps of {w.name} by the oracle (OpenMP rows, {used} threads)"
+    sample = f"each step = {n} sweeps of {w.name} by the oracle (OpenMP rows, {used} threads), one chain continued"
     line = {
         "impl": "reference", "metric": "spin_updates_per_s", "value": val, "unit": "spin updates/s",
         "ns_per_spin_flip": 1e9 / val, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
@@ -319,47 +345,86 @@ def reduce_over_ranks(dist, device, timed_ms: float, updates: int, launches: int
 # ---- roofline -----------------------------------------------------------------------------------
 def roofline(w, kernel: str, updates_per_launch: float, ms_per_launch: float, sm_mhz_max: float, hbm_gbs: float,
              which: str, bytes_per_update: float):
-    """ALU/issue roofline of the dominant kernel: algorithmic thread-instructions (36 per
-    update: the Philox block and the proposal multiply the stream definition fixes) x updates per launch over the
-    average launch duration, against 148 SMs x 128 lanes/clk x max SM clock (one warp instruction per clock and
-    sub-partition, the guide's issue model); the HBM view and the measured integer issue ceiling go beside it."""
+    """Roofline of the dominant kernel.  Two bounds are formed per workload and the slower
+    one is the `bound`: ALU/issue = algorithmic thread-instructions (36 per update: the Philox block and the
+    proposal multiply the stream definition fixes) at 148 SMs x 128 lanes/clk x max SM clock (one warp instruction
+    per clock and sub-partition, the guide's issue model); HBM = algorithmic bytes per update at the measured copy
+    bandwidth.  `achieved` / `peak` / `frac` are those of the binding bound; both views are kept beside it."""
     sec = ms_per_launch * 1e-3
-    ach = I_ALG_PER_UPDATE * updates_per_launch / sec / 1e12
-    peak = SM_COUNT * ISSUE_LANES_PER_SM_CLK * sm_mhz_max * 1e6 / 1e12
+    peak_alu = SM_COUNT * ISSUE_LANES_PER_SM_CLK * sm_mhz_max * 1e6 / 1e12
+    ach_alu = I_ALG_PER_UPDATE * updates_per_launch / sec / 1e12
     gbs = bytes_per_update * updates_per_launch / sec / 1e9
-    return {"bound": "alu", "kernel": kernel, "achieved": ach, "peak": peak, "unit": "Tinstr/s (thread-level)",
-            "frac": ach / peak, "peak_source": f"148 SMs x 128 lanes/clk x {sm_mhz_max:.0f} MHz ({which} max SM clock)",
-            "instr_per_update_algorithmic": I_ALG_PER_UPDATE, "ms_per_launch": ms_per_launch,
-            "updates_per_launch": updates_per_launch,
-            "frac_of_measured_int_issue": ach / (peak * MEASURED_INT_ISSUE_PER_CLK),
-            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(w.name),
-            "hbm": {"achieved": gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": gbs / hbm_gbs,
-                    "bytes_per_update_algorithmic": bytes_per_update, "peak_source": f"{which} copy bandwidth"}}
+    t_alu = I_ALG_PER_UPDATE / (peak_alu * 1e12)              # seconds per update at the ALU roof
+    t_hbm = bytes_per_update / (hbm_gbs * 1e9)                # seconds per update at the HBM roof
+    alu = {"achieved": ach_alu, "peak": peak_alu, "unit": "Tinstr/s (thread-level)", "frac": ach_alu / peak_alu,
+           "instr_per_update_algorithmic": I_ALG_PER_UPDATE, "ps_per_update_at_roof": t_alu * 1e12,
+           "peak_source": f"148 SMs x 128 lanes/clk x {sm_mhz_max:.0f} MHz ({which} max SM clock)",
+           "frac_of_measured_int_issue": ach_alu / (peak_alu * MEASURED_INT_ISSUE_PER_CLK)}
+    hbm = {"achieved": gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": gbs / hbm_gbs,
+           "bytes_per_update_algorithmic": bytes_per_update, "ps_per_update_at_roof": t_hbm * 1e12,
+           "peak_source": f"{which} copy bandwidth"}
+    bound = "alu" if t_alu >= t_hbm else "hbm"
+    top = alu if bound == "alu" else hbm
+    return {"bound": bound, "kernel": kernel, "achieved": top["achieved"], "peak": top["peak"], "unit": top["unit"],
+            "frac": top["frac"], "peak_source": top["peak_source"], "ms_per_launch": ms_per_launch,
+            "updates_per_launch": updates_per_launch, "traffic": ncu_traffic().get(w.name),
+            "instr_per_update_algorithmic": I_ALG_PER_UPDATE,
+            "frac_of_measured_int_issue": alu["frac_of_measured_int_issue"], "alu": alu, "hbm": hbm}
 
 
-PER_CONFIG_SLICE = {1: None, 2: 2000, 3: 1600, 4: 200, 5: 100}       # sweeps timed per step (None = all)
+def timed_config(pb, torch, flush, w, seed, peaks, steps, warmup, measure=True, stream_spec=1, clock_index=None):
+    """One workload at FULL length: median step time, its roofline object and the clocks seen while it ran."""
+    hbm_gbs, sm_max, which = peaks
+    run = GpuRun(pb, torch, w, seed, None, stream_spec=stream_spec, measure=measure)
+    if clock_index is None:
+        ms, launches = time_steps(torch, run, steps=steps, warmup=warmup, flush=flush)
+        clocks = None
+    else:
+        with ClockSampler(clock_index) as clk:
+            ms, launches = time_steps(torch, run, steps=steps, warmup=warmup, flush=flush)
+        clocks = clk.summary()
+    sec = statistics.median(ms) * 1e-3
+    ups = run.updates / sec
+    nl = run.kernel_launches_per_step
+    r = roofline(w, run.kernel, run.updates / nl, sec * 1e3 / nl, sm_max, hbm_gbs, which, run.bytes_per_update)
+    out = {"q": w.q, "L": w.L, "sweeps_timed": run.sweeps, "of_sweeps": w.total_sweeps, "steps": steps,
+           "measure": ("E" + ("+hist" if w.hist else "") + f" every {w.every}") if measure else "none",
+           "ns_per_spin_flip": 1e9 / ups, "spin_updates_per_s": ups, "ms_per_step": sec * 1e3,
+           "ms_per_step_min_max": [min(ms), max(ms)], "launches_per_step": launches // steps, "kernel": run.kernel,
+           "resident_ctas": run.resident_ctas, "cluster_ctas": run.cluster_ctas,
+           "layout": "packed" if run.layout == pb.LAYOUT_PACKED else "u8", "roofline": r, "clocks": clocks}
+    run.g.close()
+    del run
+    torch.cuda.empty_cache()
+    return out
 
 
-def per_config_table(pb, torch, flush, sm_max, hbm_gbs, which, skip=(), stream_spec=1):
+def per_config_table(pb, torch, flush, peaks, clock_index, skip=()):
+    """BASELINE.json configs at full length (the headline workload is skipped: it is the line itself), each with
+    its roofline object, and the same sweeps without the fused measurement beside it."""
     out = {}
     for k, w in workloads.CONFIGS.items():
         if k in skip:
             continue
-        run = GpuRun(pb, torch, w, w.seed, PER_CONFIG_SLICE[k], stream_spec=stream_spec)
-        ms, launches = time_steps(torch, run, steps=3, warmup=1, flush=flush)
-        sec = statistics.median(ms) * 1e-3
-        ups = run.updates / sec
-        nl = run.kernel_launches_per_step
-        r = roofline(w, run.kernel, run.updates / nl, sec * 1e3 / nl, sm_max, hbm_gbs, which, run.bytes_per_update)
-        out[w.name] = {"q": w.q, "L": w.L, "sweeps_timed": run.sweeps, "of_sweeps": w.total_sweeps,
-                       "ns_per_spin_flip": 1e9 / ups, "spin_updates_per_s": ups, "ms": sec * 1e3,
-                       "launches": launches // 3, "kernel": run.kernel, "resident_ctas": run.resident_ctas, "cluster_ctas": run.cluster_ctas,
-                       "alu_frac": r["frac"], "alu_frac_of_measured_int_issue": r["frac_of_measured_int_issue"],
-                       "hbm_frac": r["hbm"]["frac"],
-                       "layout": "packed" if run.layout == pb.LAYOUT_PACKED else "u8"}
-        run.g.close()
-        del run
-        torch.cuda.empty_cache()
+        steps = 5 if w.updates < 2e10 else 2
+        row = timed_config(pb, torch, flush, w, w.seed, peaks, steps, 1, measure=True, clock_index=clock_index)
+        plain = timed_config(pb, torch, flush, w, w.seed, peaks, steps, 1, measure=False)
+        row["without_measurement"] = {"ns_per_spin_flip": plain["ns_per_spin_flip"], "ms_per_step": plain["ms_per_step"],
+                                      "frac": plain["roofline"]["frac"], "kernel": plain["kernel"]}
+        row["measurement_cost"] = row["ns_per_spin_flip"] / plain["ns_per_spin_flip"]
+        out[w.name] = row
+    return out
+
+
+def stream_spec_2_table(pb, torch, flush, peaks):
+    """SURVEY 8(f)1, NOT the headline chain: the same workloads under stream-spec v2 (one Philox block per pair of
+    sites, S15); 19 algorithmic instructions per update, so its roofline fraction is not comparable."""
+    out = {}
+    for k, w in workloads.CONFIGS.items():
+        if k == 1:
+            continue
+        r = timed_config(pb, torch, flush, w, w.seed, peaks, 1, 1, stream_spec=2)
+        out[w.name] = {"ns_per_spin_flip": r["ns_per_spin_flip"], "spin_updates_per_s": r["spin_updates_per_s"], "kernel": r["kernel"]}
     return out
 
 
@@ -383,45 +448,56 @@ def paper_protocol_e6(pb, torch):
             "paper_seconds_gtx280": 193.0, "paper_seconds_cpu": 8115.0, "note": "context only: other hardware and RNG"}
 
 
-def batch_of_cfg1(pb, torch, n=1184):
+def batch_of_cfg1(pb, torch, n=1184, repeats=3):
     """n independent samples of BASELINE configs[0] (q=9, L=64, 1000 sweeps, E + histogram every sweep)
-    advanced together by potts_batch_sweep_measured (one lattice per CTA, 8 per SM); wall time of the call, which
-    includes the copy of the series to the host.  Sample 0 is configs[0] itself (seed 1)."""
+    advanced together by potts_batch_sweep_measured (one lattice per CTA); wall time of the call, which includes
+    the copy of the series to the host; median of `repeats` calls on one batch (the chain continues).  Sample 0 is
+    configs[0] itself (seed 1)."""
     w = workloads.CONFIGS[1]
     b = pb.PottsBatch(w.L, w.q, [w.seed + r for r in range(n)], w.init)
-    b.potts_batch_sweep_measured(w.temperatures[0], w.every, w.every)             # warm-up launch
+    E, H = b.potts_batch_sweep_measured(w.temperatures[0], w.sweeps_per_t, w.every)      # warm-up = the first 1000 sweeps
+    e_last = int(E[0, -1])
+    secs = []
+    for _ in range(repeats):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        b.potts_batch_sweep_measured(w.temperatures[0], w.sweeps_per_t, w.every)
+        secs.append(time.perf_counter() - t0)
     b.close()
-    b = pb.PottsBatch(w.L, w.q, [w.seed + r for r in range(n)], w.init)
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    E, H = b.potts_batch_sweep_measured(w.temperatures[0], w.sweeps_per_t, w.every)
-    sec = time.perf_counter() - t0
-    b.close()
+    sec = statistics.median(secs)
     ups = n * w.updates / sec
-    return {"lattices": n, "q": w.q, "L": w.L, "sweeps": w.sweeps_per_t, "seconds": sec, "spin_updates_per_s": ups,
-            "ns_per_spin_flip": 1e9 / ups, "kernel": "k_resident_batch_u8", "E_last_of_sample_0": int(E[0, -1])}
+    return {"lattices": n, "q": w.q, "L": w.L, "sweeps": w.sweeps_per_t, "seconds": sec, "seconds_min_max": [min(secs), max(secs)],
+            "spin_updates_per_s": ups, "ns_per_spin_flip": 1e9 / ups, "kernel": "k_resident_batch_u8",
+            "E_after_1000_sweeps_of_sample_0": e_last}
 
 
-def delta_stream_cost(pb, torch, sweeps=20):
+def delta_cost(pb, torch, k, sweeps, repeats=5):
     """SURVEY 8(f)4 / PAPER.md:361-363: cost of accumulating the energy change of every sweep on the fly
-    (potts_sweep_delta, k_half_sweep_delta_u8) against the plain streaming half-sweep (variant 1, no measurement)
-    on BASELINE configs[4]'s shape (q=9, L=32768).  CUDA events around the calls; the delta call includes the
-    copy of its series to the host."""
-    w = workloads.CONFIGS[5]
+    (potts_sweep_delta) against the plain sweep (potts_sweep, no measurement) on workload k's lattice, same
+    launch path.  `repeats` calls of `sweeps` sweeps each after a warm-up call of the same length (so that the
+    scratch buffers exist); CUDA events around each call (the delta call includes the copy of its series to the
+    host); median and spread."""
+    w = workloads.CONFIGS[k]
     T = w.temperatures[0]
-    out = {"q": w.q, "L": w.L, "sweeps": sweeps}
+    layout = pb.LAYOUT_PACKED if w.packed else pb.LAYOUT_U8
+    out = {"q": w.q, "L": w.L, "sweeps_per_call": sweeps, "calls": repeats}
     for name in ("plain", "delta"):
-        g = pb.Potts(w.L, w.q, w.seed, w.init)
-        g.potts_set_option("variant", 1)
+        g = pb.Potts(w.L, w.q, w.seed, w.init, layout=layout)
         step = (lambda n: g.potts_sweep(T, n)) if name == "plain" else (lambda n: g.potts_sweep_delta(T, n))
-        step(3)
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
         step(sweeps)
-        e1.record()
-        torch.cuda.synchronize()
-        out[name + "_ns_per_spin_flip"] = e0.elapsed_time(e1) * 1e6 / (sweeps * w.L * w.L)
+        ns = []
+        for _ in range(repeats):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            step(sweeps)
+            e1.record()
+            torch.cuda.synchronize()
+            ns.append(e0.elapsed_time(e1) * 1e6 / (sweeps * w.L * w.L))
+        out[name + "_ns_per_spin_flip"] = statistics.median(ns)
+        out[name + "_min_max"] = [min(ns), max(ns)]
+        out["kernel"] = "k_cluster_u8" if g.potts_get_option("cluster_active") else (
+            "k_resident_u8" if g.potts_get_option("resident_active") else ("k_half_sweep_packed" if w.packed else "k_sweep_rows_u8"))
         g.close()
     out["delta_over_plain"] = out["delta_ns_per_spin_flip"] / out["plain_ns_per_spin_flip"]
     return out
@@ -434,7 +510,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", help="cfg1..cfg5 (BASELINE.json configs[0..4])")
+    ap.add_argument("--workload", default=f"cfg{HEADLINE}", help="cfg1..cfg5 (BASELINE.json configs[0..4])")
     ap.add_argument("--max-sweeps", type=int, default=None, help="time a bounded slice of the workload per step")
     ap.add_argument("--no-per-config", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -499,15 +575,20 @@ def main():
 
     per_cfg, cpu, e6 = None, None, None
     if rank == 0 and world == 1 and not args.no_per_config:
-        per_cfg = per_config_table(pb, torch, flush, sm_max, hbm_gbs, which)
+        peaks = (hbm_gbs, sm_max, which)
+        k_head = int(args.workload.replace("cfg", ""))
+        per_cfg = per_config_table(pb, torch, flush, peaks, local, skip=(k_head,))
+        # the headline workload without its fused measurement (the line itself is the "with" leg)
+        plain = timed_config(pb, torch, flush, w, w.seed, peaks, 2, 1, measure=False)
+        per_cfg[w.name + "_without_measurement"] = {k: plain[k] for k in ("ns_per_spin_flip", "ms_per_step", "kernel", "sweeps_timed")}
+        per_cfg[w.name + "_without_measurement"]["frac"] = plain["roofline"]["frac"]
         e6 = paper_protocol_e6(pb, torch)
         per_cfg["batch_cfg1_x1184"] = batch_of_cfg1(pb, torch)
-        per_cfg["delta_stream_cfg5"] = delta_stream_cost(pb, torch)
-        # SURVEY 8(f)1, NOT the headline chain: the same workloads under stream-spec v2 (one Philox block per pair of
-        # sites, S15); its algorithmic instruction count is 19 per update, so alu_frac is not comparable
-        v2 = per_config_table(pb, torch, flush, sm_max, hbm_gbs, which, skip=(1,), stream_spec=2)
-        per_cfg["stream_spec_2"] = {k: {"ns_per_spin_flip": v["ns_per_spin_flip"], "spin_updates_per_s": v["spin_updates_per_s"],
-                                        "kernel": v["kernel"]} for k, v in v2.items()}
+        per_cfg["delta_cfg5_streaming"] = delta_cost(pb, torch, 5, 100)
+        per_cfg["delta_cfg4_packed"] = delta_cost(pb, torch, 4, 200)
+        per_cfg["delta_cfg2_resident"] = delta_cost(pb, torch, 2, 2000)
+        per_cfg["delta_cfg1_cluster"] = delta_cost(pb, torch, 1, 2000)
+        per_cfg["stream_spec_2"] = stream_spec_2_table(pb, torch, flush, peaks)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(w)
     if dist is not None:
@@ -525,8 +606,9 @@ def main():
                    "sweeps_per_step": run.sweeps, "of_sweeps": w.total_sweeps, "measure_every": w.every,
                    "hist": w.hist, "layout": layout, "seed": w.seed, "options": options,
                    "parallelism": f"{world} independent sample(s), one per GPU" if world > 1 else "1 GPU",
-                   "l2": "each step starts from a fresh lattice after a 256 MiB L2 flush; within a step the "
-                         "lattice is re-swept in place, so L2 residency for L <= 8192 is the workload's own"},
+                   "l2": "each step starts from a fresh lattice after a 256 MiB L2 flush; the 1 GiB lattice of the "
+                         "headline workload is 8x the L2, so every half-sweep streams from HBM; for L <= 8192 the "
+                         "lattice is re-swept in place and its L2 residency is the workload's own"},
         "clocks": clk.summary(), "roofline": roof, "e2e": e2e, "cpu_baseline": cpu, "per_config": per_cfg,
         "paper_protocol_e6": e6,
         "wall_s_timed_region": wall,

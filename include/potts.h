@@ -169,6 +169,16 @@ int potts_observables(const int64_t *E_series, int64_t n, int64_t N, double T,
 /* *m = (q N_max/N - 1)/(q - 1) from a histogram (host, q entries). */
 int potts_magnetisation(const int64_t *counts, int32_t q, double *m);
 
+/* potts_susceptibility (Eq. 11, with m of PAPER.md:73 Eq. 7): from a series of n histograms
+ * (host, n rows of q int64 counts, every row summing to the same N > 0)
+ *   *mean_m = <m>,  *mean_m2 = <m^2>,  *chi = N/T (<m^2> - <m>^2).
+ * With a_k = q Nmax_k - N (an integer) m_k = a_k / ((q-1) N); sum a_k and sum a_k^2 are formed exactly in 128-bit
+ * integers, and so is n sum a^2 - (sum a)^2 (long double beyond 2^126), then one conversion: robust against the
+ * cancellation in the variance.  Any out-pointer may be null.  POTTS_ERR_ARG: null series, n < 1, q outside
+ * [2, 256], T not finite or <= 0, a negative count, rows with different or zero sums. */
+int potts_susceptibility(const int64_t *hist_series, int64_t n, int32_t q, double T,
+                         double *mean_m, double *mean_m2, double *chi);
+
 /* ---- random-stream definition ---------------------------------------------------------------------------------
  * potts_set_stream_spec: 1 (default) = one Philox4x32-10 block per site and half-sweep, words (w0, w1), as in the
  * header comment; 2 = "stream-spec v2" (reading S15): the same-colour sites of a row are numbered k = j>>1,

@@ -51,3 +51,30 @@ def binder_cumulant(E_series) -> float:
 def mean_energy_per_spin(E_series, N: int) -> float:
     Es = [int(e) for e in E_series]
     return float(Fraction(sum(Es), len(Es) * N))
+
+
+def magnetisation_moments(hist_series, q: int):
+    """(<m>, <m^2>) of the order parameter m (Eq. 7, reading G4) over a series of q-bin histograms,
+    in exact rational arithmetic: m_k = (q Nmax_k - N) / ((q - 1) N)."""
+    ms = []
+    for hist in hist_series:
+        counts = [int(c) for c in hist]
+        N = sum(counts)
+        ms.append((Fraction(q * max(counts), N) - 1) / (q - 1))
+    n = len(ms)
+    m1 = sum(ms, Fraction(0)) / n
+    m2 = sum((m * m for m in ms), Fraction(0)) / n
+    return float(m1), float(m2)
+
+
+def susceptibility(hist_series, q: int, T: float) -> float:
+    """chi = N / T (<m^2> - <m>^2) (Eq. 11), exact rationals, one conversion at the end."""
+    ms, N = [], None
+    for hist in hist_series:
+        counts = [int(c) for c in hist]
+        N = sum(counts)
+        ms.append((Fraction(q * max(counts), N) - 1) / (q - 1))
+    n = len(ms)
+    m1 = sum(ms, Fraction(0)) / n
+    m2 = sum((m * m for m in ms), Fraction(0)) / n
+    return float(N * (m2 - m1 * m1) / Fraction(float(T)))

@@ -70,6 +70,7 @@ def load_library() -> ctypes.CDLL:
         "potts_set_sweep_count": ([vp, u64], ctypes.c_int),
         "potts_observables": ([vp, i64, i64, dbl, P(dbl), P(dbl), P(dbl)], ctypes.c_int),
         "potts_magnetisation": ([vp, i32, P(dbl)], ctypes.c_int),
+        "potts_susceptibility": ([vp, i64, i32, dbl, P(dbl), P(dbl), P(dbl)], ctypes.c_int),
         "potts_launch_count": ([vp, P(u64)], ctypes.c_int),
         "potts_set_option": ([vp, ctypes.c_char_p, i64], ctypes.c_int),
         "potts_get_option": ([vp, ctypes.c_char_p, P(i64)], ctypes.c_int),
@@ -88,7 +89,7 @@ EXPORTED_SYMBOLS = [
     "potts_create", "potts_create_ex", "potts_workspace_bytes", "potts_set_stream", "potts_destroy",
     "potts_sweep", "potts_sweep_measured", "potts_sweep_measured_dev", "potts_sweep_delta", "potts_ladder", "potts_energy", "potts_histogram",
     "potts_download", "potts_upload", "potts_sweep_count", "potts_set_sweep_count", "potts_observables",
-    "potts_magnetisation", "potts_launch_count", "potts_set_option", "potts_get_option", "potts_last_error",
+    "potts_magnetisation", "potts_susceptibility", "potts_launch_count", "potts_set_option", "potts_get_option", "potts_last_error",
     "potts_version", "potts_batch_workspace_bytes", "potts_batch_create", "potts_batch_destroy",
     "potts_batch_sweep_measured", "potts_batch_download", "potts_batch_sweep_count", "potts_batch_launch_count",
     "potts_set_stream_spec", "potts_get_stream_spec", "potts_batch_set_stream_spec",
@@ -124,6 +125,15 @@ def potts_magnetisation(counts, q: int) -> float:
     m = ctypes.c_double()
     _check(load_library().potts_magnetisation(H.ctypes.data, int(q), ctypes.byref(m)))
     return m.value
+
+
+def potts_susceptibility(hist_series, q: int, T: float):
+    """-> (<m>, <m^2>, chi = N/T (<m^2> - <m>^2)) from a series of histograms, computed by the library on the host."""
+    H = np.ascontiguousarray(hist_series, dtype=np.int64).reshape(-1, int(q))
+    a, b, c = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    _check(load_library().potts_susceptibility(H.ctypes.data, H.shape[0], int(q), float(T),
+                                               ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
+    return a.value, b.value, c.value
 
 
 class Potts:

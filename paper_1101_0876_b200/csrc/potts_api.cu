@@ -9,6 +9,8 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <thread>
+#include <vector>
 
 namespace {
 
@@ -39,6 +41,7 @@ constexpr int MAX_CTAS = 160;             // upper bound on the resident kernel'
 constexpr int RESIDENT_L_MAX = 4096;
 constexpr int CLUSTER_AUTO_L_MAX = 128;    // lattices up to this size go to the cluster (DSMEM) kernel by default (measured: 2x the resident kernel)      // largest lattice the resident kernel can hold (512 words per row)
 constexpr int ACC_WORDS = 1 + 256 + 1;    // E, hist[256], flag/error word
+constexpr size_t STATIC_SMEM = sizeof(potts::AcceptLut) + 1024;   // static shared memory of the persistent kernels
 
 }  // namespace
 
@@ -61,6 +64,8 @@ struct potts_s {
     int coop = 0;                        // device supports cooperative launches (the resident kernel needs one)
     uint8_t *scratch = nullptr;          // device scratch kept between calls (staging for up/download, host-series buffers)
     size_t scratch_bytes = 0;
+    cudaStream_t copy_stream = nullptr;  // up/download: PCIe copies run here, conversions on `stream`
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_converted[2] = {nullptr, nullptr}, ev_start = nullptr;
     // options (how to launch, never what is computed)
     int32_t stream_spec = 1;             // random-stream definition (1 = R3, 2 = R3'): changes the chain, not an option
     int64_t opt_variant = 0;             // 0 auto, 1 streaming (one launch per half-sweep), 2 resident
@@ -314,7 +319,7 @@ ResidentPlan plan_resident(const potts_t *h)
     if ((R.rows_max + tyc - 1) / tyc > 30) { R.why = "too many rows per thread"; return R; }
     const size_t hist = (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4;
     R.smem = 2 * (size_t)(R.rows_max + 2) * (L / 2) + hist;
-    if (R.smem + 1024 > h->smem_optin) { R.why = "lattice does not fit the shared memory of the grid"; return R; }
+    if (R.smem + STATIC_SMEM > h->smem_optin) { R.why = "lattice does not fit the shared memory of the grid"; return R; }
     R.ok = true;
     return R;
 }
@@ -377,7 +382,7 @@ ClusterPlan plan_cluster(const potts_t *h)
     if ((R.rows_max + tyc - 1) / tyc > 60) { R.why = "too many rows per thread"; return R; }
     const size_t hist = 2 * (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4;   // two tables
     R.smem = 2 * (size_t)(R.rows_max + 2) * (L / 2) + hist;
-    if (R.smem + 1024 > h->smem_optin) { R.why = "lattice does not fit the shared memory of one cluster"; return R; }
+    if (R.smem + STATIC_SMEM > h->smem_optin) { R.why = "lattice does not fit the shared memory of one cluster"; return R; }
     R.ok = true;
     return R;
 }
@@ -617,6 +622,11 @@ void potts_destroy(potts_t *h)
     if (!h) return;
     if (h->scratch || (h->owns_ws && h->ws)) cudaStreamSynchronize(h->stream);
     if (h->scratch) cudaFree(h->scratch);
+    if (h->copy_stream) {
+        cudaStreamDestroy(h->copy_stream);
+        for (int k = 0; k < 2; ++k) { cudaEventDestroy(h->ev_copied[k]); cudaEventDestroy(h->ev_converted[k]); }
+        cudaEventDestroy(h->ev_start);
+    }
     if (h->owns_ws && h->ws) cudaFree(h->ws);
     delete h;
 }
@@ -769,66 +779,132 @@ int potts_histogram(potts_t *h, int64_t *counts)
     return POTTS_OK;
 }
 
-// rows per staging chunk: keeps the device staging buffer <= 64 MiB
-static int chunk_rows(int L) { long long r = (64ll << 20) / L; return (int)(r < 1 ? 1 : (r > L ? L : r)); }
+// ---- host <-> device transfer of the configuration ---------------------------------------------------
+// Rows per staging buffer: two buffers of <= 32 MiB each, so that the PCIe copy of one chunk overlaps the layout
+// conversion of the other (copies on the handle's own copy stream, conversions on the caller's stream, one
+// event per buffer and direction; no synchronisation inside the loop).
+static int chunk_rows(int L) { long long r = (32ll << 20) / L; return (int)(r < 1 ? 1 : (r > L ? L : r)); }
+
+static int ensure_copy_objects(potts_t *h)
+{
+    if (h->copy_stream) return POTTS_OK;
+    CUDA_TRY(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+    for (int k = 0; k < 2; ++k) {
+        CUDA_TRY(cudaEventCreateWithFlags(&h->ev_copied[k], cudaEventDisableTiming));
+        CUDA_TRY(cudaEventCreateWithFlags(&h->ev_converted[k], cudaEventDisableTiming));
+    }
+    CUDA_TRY(cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming));
+    return POTTS_OK;
+}
 
 int potts_download(potts_t *h, uint8_t *spins)
 {
     if (!h || !spins) return fail(POTTS_ERR_ARG, "null argument");
     const int L = h->L, rows = chunk_rows(L);
+    const size_t buf_bytes = (size_t)rows * L;
     uint8_t *stage = nullptr;
-    int rc = get_scratch(h, (size_t)rows * L, &stage);
+    int rc = get_scratch(h, 2 * buf_bytes, &stage);
     if (rc) return rc;
-    for (int i0 = 0; i0 < L && rc == POTTS_OK; i0 += rows) {
-        const int r = (L - i0 < rows) ? L - i0 : rows;
+    rc = ensure_copy_objects(h);
+    if (rc) return rc;
+    int k = 0;
+    for (int i0 = 0; i0 < L && rc == POTTS_OK; i0 += rows, ++k) {
+        const int r = (L - i0 < rows) ? L - i0 : rows, b = k & 1;
+        uint8_t *buf = stage + (size_t)b * buf_bytes;
+        if (k >= 2) CUDA_TRY(cudaStreamWaitEvent(h->stream, h->ev_copied[b], 0));      // the copy out of this buffer is done
         const long long threads = (long long)r * (L / 8);
         if (h->layout == POTTS_LAYOUT_PACKED) {
             const unsigned grid = (unsigned)(((long long)r * (L / 64) + 127) / 128);
-            if (h->q > 16) potts::k_packed_to_rowmajor<true><<<grid, 128, 0, h->stream>>>(h->pk, stage, i0, r);
-            else potts::k_packed_to_rowmajor<false><<<grid, 128, 0, h->stream>>>(h->pk, stage, i0, r);
+            if (h->q > 16) potts::k_packed_to_rowmajor<true><<<grid, 128, 0, h->stream>>>(h->pk, buf, i0, r);
+            else potts::k_packed_to_rowmajor<false><<<grid, 128, 0, h->stream>>>(h->pk, buf, i0, r);
         } else {
             potts::k_planes_to_rowmajor<<<(unsigned)((threads + 255) / 256), 256, 0, h->stream>>>(
-                h->plane[0], h->plane[1], stage, L, L / 2, i0, r);
+                h->plane[0], h->plane[1], buf, L, L / 2, i0, r);
         }
         rc = check_launch(h, "k_planes_to_rowmajor");
-        if (rc == POTTS_OK) {
-            cudaError_t e = cudaMemcpyAsync(spins + (size_t)i0 * L, stage, (size_t)r * L, cudaMemcpyDeviceToHost, h->stream);
-            if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-            if (e != cudaSuccess) rc = fail(POTTS_ERR_CUDA, "download copy failed: %s", cudaGetErrorString(e));
-        }
+        if (rc) break;
+        CUDA_TRY(cudaEventRecord(h->ev_converted[b], h->stream));
+        CUDA_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_converted[b], 0));
+        CUDA_TRY(cudaMemcpyAsync(spins + (size_t)i0 * L, buf, (size_t)r * L, cudaMemcpyDeviceToHost, h->copy_stream));
+        CUDA_TRY(cudaEventRecord(h->ev_copied[b], h->copy_stream));
     }
-    return rc ? rc : check_device_error(h);
+    const cudaError_t e1 = cudaStreamSynchronize(h->copy_stream), e2 = cudaStreamSynchronize(h->stream);
+    if (rc) return rc;
+    if (e1 != cudaSuccess || e2 != cudaSuccess)
+        return fail(POTTS_ERR_CUDA, "download copy failed: %s", cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
+    return check_device_error(h);
+}
+
+// is any byte of spins[0, n) >= q?  Word-parallel, a few host threads: ~20 ms per GiB, against ~40 ms of PCIe copy.
+static bool host_has_value_ge(const uint8_t *spins, size_t n, int q)
+{
+    if (q >= 256) return false;
+    unsigned nt = std::thread::hardware_concurrency();
+    if (nt > 8) nt = 8;
+    if (nt < 1 || n < (1u << 22)) nt = 1;
+    std::vector<unsigned char> bad(nt, 0);
+    auto scan = [&](unsigned t) {
+        const size_t a = n * t / nt, b = n * (t + 1) / nt;
+        unsigned char m = 0;
+        for (size_t k = a; k < b; ++k) m |= (unsigned char)(spins[k] >= q);     // vectorised by the host compiler
+        bad[t] = m;
+    };
+    if (nt == 1) scan(0);
+    else {
+        std::vector<std::thread> th;
+        for (unsigned t = 0; t < nt; ++t) th.emplace_back(scan, t);
+        for (auto &x : th) x.join();
+    }
+    for (unsigned t = 0; t < nt; ++t)
+        if (bad[t]) return true;
+    return false;
 }
 
 int potts_upload(potts_t *h, const uint8_t *spins)
 {
     if (!h || !spins) return fail(POTTS_ERR_ARG, "null argument");
     const int L = h->L, rows = chunk_rows(L);
-    // validate on the host first so that a rejected upload leaves the lattice untouched
-    if (h->q < 256)
-        for (size_t n = 0; n < (size_t)L * L; ++n)
-            if (spins[n] >= h->q) return fail(POTTS_ERR_ARG, "spin value %d >= q at offset %zu", (int)spins[n], n);
+    // validate on the host first so that a rejected upload leaves the lattice untouched; the converter checks again
+    // on the device and its flag is read back below
+    if (host_has_value_ge(spins, (size_t)L * L, h->q)) return fail(POTTS_ERR_ARG, "a spin value is >= q = %d", h->q);
+    const size_t buf_bytes = (size_t)rows * L;
     uint8_t *stage = nullptr;
-    int rc = get_scratch(h, (size_t)rows * L, &stage);
+    int rc = get_scratch(h, 2 * buf_bytes, &stage);
     if (rc) return rc;
-    cudaMemsetAsync(h->flag, 0, sizeof(int), h->stream);
-    for (int i0 = 0; i0 < L && rc == POTTS_OK; i0 += rows) {
-        const int r = (L - i0 < rows) ? L - i0 : rows;
-        cudaError_t e = cudaMemcpyAsync(stage, spins + (size_t)i0 * L, (size_t)r * L, cudaMemcpyHostToDevice, h->stream);
-        if (e != cudaSuccess) { rc = fail(POTTS_ERR_CUDA, "upload copy failed: %s", cudaGetErrorString(e)); break; }
+    rc = ensure_copy_objects(h);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemsetAsync(h->flag, 0, sizeof(int), h->stream));
+    // the staging buffers may still be read by earlier work on the caller's stream
+    CUDA_TRY(cudaEventRecord(h->ev_start, h->stream));
+    CUDA_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_start, 0));
+    int k = 0;
+    for (int i0 = 0; i0 < L && rc == POTTS_OK; i0 += rows, ++k) {
+        const int r = (L - i0 < rows) ? L - i0 : rows, b = k & 1;
+        uint8_t *buf = stage + (size_t)b * buf_bytes;
+        if (k >= 2) CUDA_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_converted[b], 0));   // the converter has read this buffer
+        CUDA_TRY(cudaMemcpyAsync(buf, spins + (size_t)i0 * L, (size_t)r * L, cudaMemcpyHostToDevice, h->copy_stream));
+        CUDA_TRY(cudaEventRecord(h->ev_copied[b], h->copy_stream));
+        CUDA_TRY(cudaStreamWaitEvent(h->stream, h->ev_copied[b], 0));
         const long long threads = (long long)r * (L / 8);
         if (h->layout == POTTS_LAYOUT_PACKED) {
             const unsigned grid = (unsigned)(((long long)r * (L / 64) + 127) / 128);
-            if (h->q > 16) potts::k_rowmajor_to_packed<true><<<grid, 128, 0, h->stream>>>(stage, h->pk, i0, r, (uint32_t)h->q, h->flag);
-            else potts::k_rowmajor_to_packed<false><<<grid, 128, 0, h->stream>>>(stage, h->pk, i0, r, (uint32_t)h->q, h->flag);
+            if (h->q > 16) potts::k_rowmajor_to_packed<true><<<grid, 128, 0, h->stream>>>(buf, h->pk, i0, r, (uint32_t)h->q, h->flag);
+            else potts::k_rowmajor_to_packed<false><<<grid, 128, 0, h->stream>>>(buf, h->pk, i0, r, (uint32_t)h->q, h->flag);
         } else
             potts::k_rowmajor_to_planes<<<(unsigned)((threads + 255) / 256), 256, 0, h->stream>>>(
-                stage, h->plane[0], h->plane[1], L, L / 2, i0, r, (uint32_t)h->q, h->flag);
+                buf, h->plane[0], h->plane[1], L, L / 2, i0, r, (uint32_t)h->q, h->flag);
         rc = check_launch(h, "k_rowmajor_to_planes");
-        if (rc == POTTS_OK && cudaStreamSynchronize(h->stream) != cudaSuccess)
-            rc = fail(POTTS_ERR_CUDA, "upload sync failed");
+        if (rc) break;
+        CUDA_TRY(cudaEventRecord(h->ev_converted[b], h->stream));
     }
-    return rc;
+    int bad = 0;
+    cudaError_t e = cudaSuccess;
+    if (rc == POTTS_OK) e = cudaMemcpyAsync(&bad, h->flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream);
+    const cudaError_t e1 = cudaStreamSynchronize(h->copy_stream), e2 = cudaStreamSynchronize(h->stream);
+    if (rc) return rc;
+    if (e != cudaSuccess || e1 != cudaSuccess || e2 != cudaSuccess) return fail(POTTS_ERR_CUDA, "upload copy failed");
+    if (bad) return fail(POTTS_ERR_ARG, "a spin value is >= q = %d (device check; the lattice is now undefined)", h->q);
+    return POTTS_OK;
 }
 
 int potts_sweep_count(potts_t *h, uint64_t *t)
@@ -964,6 +1040,42 @@ int potts_magnetisation(const int64_t *counts, int32_t q, double *m)
     return POTTS_OK;
 }
 
+int potts_susceptibility(const int64_t *hist_series, int64_t n, int32_t q, double T, double *mean_m, double *mean_m2,
+                         double *chi)
+{
+    if (!hist_series || n < 1 || q < 2 || q > 256 || !(T > 0.0) || !std::isfinite(T))
+        return fail(POTTS_ERR_ARG, "bad arguments to potts_susceptibility");
+    typedef __int128 i128;
+    i128 s1 = 0, s2 = 0;
+    int64_t N = 0;
+    for (int64_t k = 0; k < n; ++k) {
+        const int64_t *row = hist_series + k * q;
+        int64_t sum = 0, mx = 0;
+        for (int s = 0; s < q; ++s) {
+            if (row[s] < 0) return fail(POTTS_ERR_ARG, "negative count in histogram %lld", (long long)k);
+            sum += row[s];
+            if (row[s] > mx) mx = row[s];
+        }
+        if (k == 0) N = sum;
+        if (sum != N || N <= 0) return fail(POTTS_ERR_ARG, "histogram %lld sums to %lld, expected N = %lld > 0", (long long)k, (long long)sum, (long long)N);
+        const i128 a = (i128)q * mx - N;                 // m_k = a / ((q-1) N), 0 <= a <= (q-1) N
+        s1 += a;
+        s2 += a * a;
+    }
+    const long double den = (long double)(q - 1) * (long double)N;          // m = a / den
+    if (mean_m) *mean_m = (double)((long double)s1 / ((long double)n * den));
+    if (mean_m2) *mean_m2 = (double)((long double)s2 / ((long double)n * den * den));
+    if (chi) {
+        // <m^2> - <m>^2 = (n s2 - s1^2) / (n den)^2, the numerator exact while it fits 126 bits
+        long double num;
+        const long double est = (long double)n * (long double)s2;
+        if (est < 0x1p125L) num = (long double)((i128)n * s2 - s1 * s1);
+        else num = est - (long double)s1 * (long double)s1;
+        *chi = (double)((long double)N / (long double)T * num / ((long double)n * den * (long double)n * den));
+    }
+    return POTTS_OK;
+}
+
 }  // extern "C"
 
 // ---- replica batch -------------------------------------------------------------------------------
@@ -978,9 +1090,22 @@ struct potts_batch_s {
     int *error = nullptr;
     cudaStream_t stream = nullptr;
     size_t smem_optin = 0;
+    uint8_t *scratch = nullptr;           // device scratch kept between calls (series, download staging)
+    size_t scratch_bytes = 0;
 };
 
 namespace {
+
+int get_batch_scratch(potts_batch_t *b, size_t bytes, uint8_t **out)
+{
+    if (b->scratch_bytes < bytes) {
+        if (b->scratch) { cudaStreamSynchronize(b->stream); cudaFree(b->scratch); b->scratch = nullptr; b->scratch_bytes = 0; }
+        CUDA_TRY(cudaMalloc(&b->scratch, bytes));
+        b->scratch_bytes = bytes;
+    }
+    *out = b->scratch;
+    return POTTS_OK;
+}
 
 struct BatchPlan { bool ok = false; int tyc = 0, nthreads = 0; size_t smem = 0; const char *why = ""; };
 
@@ -996,7 +1121,7 @@ BatchPlan plan_batch(int32_t L, int32_t q, size_t smem_optin)
     if ((L + tyc - 1) / tyc > 30) { R.why = "too many rows per thread"; return R; }
     const size_t hist = (size_t)(q <= (int)potts::HIST_LANE_QMAX ? q * 32 : q) * 4;
     R.smem = 2 * (size_t)(L + 2) * (L / 2) + hist;
-    if (R.smem + 1024 > smem_optin) { R.why = "one lattice does not fit the shared memory of a CTA"; return R; }
+    if (R.smem + STATIC_SMEM > smem_optin) { R.why = "one lattice does not fit the shared memory of a CTA"; return R; }
     R.ok = true;
     return R;
 }
@@ -1083,7 +1208,9 @@ int potts_batch_create(potts_batch_t **out, int32_t n, int32_t L, int32_t q, con
 void potts_batch_destroy(potts_batch_t *b)
 {
     if (!b) return;
-    if (b->owns_ws && b->ws) { cudaStreamSynchronize(b->stream); cudaFree(b->ws); }
+    if (b->scratch || (b->owns_ws && b->ws)) cudaStreamSynchronize(b->stream);
+    if (b->scratch) cudaFree(b->scratch);
+    if (b->owns_ws && b->ws) cudaFree(b->ws);
     delete[] b->seeds;
     delete b;
 }
@@ -1130,7 +1257,8 @@ int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweep
     const size_t eb = E_series ? (size_t)b->n * ns * 8 : 0, hb = hist_series ? (size_t)b->n * ns * b->q * 8 : 0;
     uint8_t *dev = nullptr;
     if (eb + hb) {
-        CUDA_TRY(cudaMalloc(&dev, eb + hb));
+        int rc = get_batch_scratch(b, eb + hb, &dev);
+        if (rc) return rc;
         cudaMemsetAsync(dev, 0, eb + hb, b->stream);
     }
     const BatchPlan R = plan_batch(b->L, b->q, b->smem_optin);
@@ -1168,7 +1296,6 @@ int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweep
     if (e == cudaSuccess && eb) e = cudaMemcpyAsync(E_series, dev, eb, cudaMemcpyDeviceToHost, b->stream);
     if (e == cudaSuccess && hb) e = cudaMemcpyAsync(hist_series, dev + eb, hb, cudaMemcpyDeviceToHost, b->stream);
     const cudaError_t e2 = cudaStreamSynchronize(b->stream);
-    if (dev) cudaFree(dev);
     if (e != cudaSuccess || e2 != cudaSuccess)
         return fail(POTTS_ERR_CUDA, "batch sweep failed: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
     return POTTS_OK;
@@ -1180,7 +1307,8 @@ int potts_batch_download(potts_batch_t *b, int32_t r, uint8_t *spins)
     if (r < 0 || r >= b->n) return fail(POTTS_ERR_ARG, "lattice index %d outside [0, %d)", r, b->n);
     const int L = b->L;
     uint8_t *stage = nullptr;
-    CUDA_TRY(cudaMalloc(&stage, (size_t)L * L));
+    int rc = get_batch_scratch(b, (size_t)L * L, &stage);
+    if (rc) return rc;
     uint8_t *p0 = b->ws + (size_t)r * 2 * b->plane_bytes;
     const long long threads = (long long)L * (L / 8);
     potts::k_planes_to_rowmajor<<<(unsigned)((threads + 255) / 256), 256, 0, b->stream>>>(p0, p0 + b->plane_bytes, stage, L, L / 2, 0, L);
@@ -1188,7 +1316,6 @@ int potts_batch_download(potts_batch_t *b, int32_t r, uint8_t *spins)
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(spins, stage, (size_t)L * L, cudaMemcpyDeviceToHost, b->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(b->stream);
-    cudaFree(stage);
     if (e != cudaSuccess) return fail(POTTS_ERR_CUDA, "batch download failed: %s", cudaGetErrorString(e));
     return POTTS_OK;
 }

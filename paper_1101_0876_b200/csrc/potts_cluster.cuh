@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) uint8_t s_raw[];
-    __shared__ AcceptEntry<true> lut[ACCEPT_ENTRIES];
+    __shared__ AcceptLut lut;
 
     const uint32_t G = cluster.num_blocks(), b = cluster.block_rank();
     const int L = P.L, pitch = P.pitch;
@@ -54,7 +54,8 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
     const bool do_D = P.dE_series != nullptr;
     const uint32_t q = in_register(P.q);
 
-    accept_lut_fill<true>(lut, P.thr, tid, nthreads);
+    accept_lut_fill(&lut, P.thr, tid, nthreads);
+    const uint32_t lane_off = accept_lane_offset(tid);
     if (do_hist)
         for (uint32_t n = tid; n < 2u * hist_words(P.q); n += nthreads) s_hist0[n] = 0u;
     {
@@ -80,9 +81,8 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
             const uint8_t *const oth_row = s_raw + (1u - c) * plane_stride;
             const HalfSweepKeys K = half_sweep_keys(P.key0, P.key1, t, c);
             const bool count_E = sample && c == 1 && do_E, count_H = sample && do_hist;
-            int d_sum = 0, c_sum = 0;
+            int d_sum = 0, ne_sum = 0;
             uint32_t words_done = 0;
-            const bool ex = count_E || do_D;
             uint32_t *const s_hist = s_hist0 + (sample_idx & 1u) * hist_words(P.q);
             if (is_compute)
                 for (int lr = 1 + ty; lr <= rows; lr += tyc) {
@@ -98,7 +98,10 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
                     uint32_t lf, rt;
                     horizontal(p, mid, adj, lf, rt);
                     const RowKeys R = row_keys(K, i);
-                    const uint32_t out = update_word<CM, ST>(own, up, dn, lf, rt, 2u * col + p, q, K, R, lut, ex, d_sum, c_sum);
+                    uint32_t code, mask;
+                    const uint32_t out = update_word<CM, ST>(own, up, dn, lf, rt, 2u * col + p, q, K, R, &lut, lane_off, code, mask);
+                    if (count_E) ne_sum += ne_final_sum(code, mask);
+                    if (do_D) d_sum += delta_sum(code, mask);
                     *reinterpret_cast<uint32_t *>(own_col + ro) = out;
                     // my first row is the row below the last row of the CTA above, my last row the row above the first of the CTA below
                     if (lr == 1)
@@ -114,7 +117,7 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
                 if ((tid & 31u) == 0 && dd) atomicAdd(P.dE_series + n, (unsigned long long)(long long)dd);
             }
             if (count_E) {
-                uint32_t satisfied = 16u * words_done - (uint32_t)(c_sum + d_sum);
+                uint32_t satisfied = 16u * words_done - (uint32_t)ne_sum;
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
                 if ((tid & 31u) == 0 && satisfied) atomicAdd(P.E_series + sample_idx, 0ull - (unsigned long long)satisfied);

@@ -15,7 +15,8 @@
 //     gathered into ONE code byte per site (no counting, no subtraction);
 //   * acceptance: the code byte indexes a 256-entry shared table of 64-bit values 2^64 - threshold(d),
 //     and the 64-bit sum  w1 + entry  (add, add-with-carry) leaves the accept mask (0 / 0xffffffff) in its
-//     high word: d <= 0 ("always") and threshold 0 ("never") need no special case and no mask start-up.
+//     high word: d <= 0 ("always") and threshold 0 ("never") need no special case and no mask start-up;
+//   * the energy / energy-change sums of sampled sweeps are two population counts of the masked code word.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -330,59 +331,60 @@ __device__ __forceinline__ void horizontal(uint32_t p, uint32_t mid, uint32_t ad
 //   threshold(d) = 2^32 for d <= 0 (always accept), thr[d-1] = floor(2^32 exp(-d/T)) for d = 1..4   (R6)
 //   entry = 2^64 - threshold(d)  (mod 2^64)
 // so that the high word of  w1 + entry  is 0xffffffff iff w1 < threshold(d) and 0 otherwise: exact for every
-// threshold in [0, 2^32].  EX entries (16 bytes) also hold -d and c_old for the fused energy / energy-change sums.
+// threshold in [0, 2^32].  The 32 lanes of a warp look up 32 different codes, so a single copy of the table
+// would serialise on its banks (measured: the 9-word table of round 1 never did); the table is therefore stored
+// in ACCEPT_SLOTS copies, entry (code, slot) at byte code * 8 * ACCEPT_SLOTS + slot * 8, and lane l reads slot
+// l % ACCEPT_SLOTS: the 16 lanes of a half-warp meet on a bank pair only if they share a slot AND differ in code.
 constexpr int ACCEPT_ENTRIES = 256;
-template <bool T16> struct AcceptEntry;                      // T16: 16-byte entries (the EX sums need them)
-template <> struct AcceptEntry<false> { uint2 v; };
-template <> struct AcceptEntry<true> { uint4 v; };
-template <bool T16> __host__ __device__ constexpr int accept_shift() { return T16 ? 4 : 3; }
+constexpr int ACCEPT_SLOTS = 8;
+constexpr int ACCEPT_SHIFT = 6;                                 // log2(8 bytes * ACCEPT_SLOTS)
+struct AcceptLut { uint2 e[ACCEPT_ENTRIES][ACCEPT_SLOTS]; };    // 16 KB
 
-template <bool T16>
-__device__ __forceinline__ void accept_lut_fill(AcceptEntry<T16> *lut, const uint32_t thr[4], uint32_t tid, uint32_t nthreads)
+__device__ __forceinline__ void accept_lut_fill(AcceptLut *lut, const uint32_t thr[4], uint32_t tid, uint32_t nthreads)
 {
-    for (uint32_t code = tid; code < (uint32_t)ACCEPT_ENTRIES; code += nthreads) {
-        const int c_old = __popc(code & 15u), c_new = __popc(code >> 4);
-        const int d = c_new - c_old;
+    for (uint32_t n = tid; n < (uint32_t)(ACCEPT_ENTRIES * ACCEPT_SLOTS); n += nthreads) {
+        const uint32_t code = n / ACCEPT_SLOTS;
+        const int d = __popc(code >> 4) - __popc(code & 15u);
         const unsigned long long th = d <= 0 ? (1ull << 32) : (unsigned long long)(d == 1 ? thr[0] : (d == 2 ? thr[1] : (d == 3 ? thr[2] : thr[3])));
         const unsigned long long e = 0ull - th;
-        if constexpr (T16) lut[code].v = make_uint4((uint32_t)e, (uint32_t)(e >> 32), (uint32_t)(-d), (uint32_t)c_old);
-        else lut[code].v = make_uint2((uint32_t)e, (uint32_t)(e >> 32));
+        (&lut->e[0][0])[n] = make_uint2((uint32_t)e, (uint32_t)(e >> 32));
     }
 }
 
-// accept masks of the four sites of a word: byte b = 0xff iff site b accepts its proposal.
-// EX: d_sum += sum of d over the accepted sites, c_sum += sum of c_old over the four sites.
-template <bool EX, bool T16>
-__device__ __forceinline__ uint32_t accept_mask(uint32_t code, const uint32_t w1[4], const AcceptEntry<T16> *lut,
-                                                int &d_sum, int &c_sum)
+// byte offset of this lane's slot inside a table row
+__device__ __forceinline__ uint32_t accept_lane_offset(uint32_t lane) { return (lane % ACCEPT_SLOTS) * 8u; }
+
+// accept masks of the four sites of a word: byte b = 0xff iff site b accepts its proposal
+__device__ __forceinline__ uint32_t accept_mask(uint32_t code, const uint32_t w1[4], const AcceptLut *lut, uint32_t lane_off)
 {
-    static_assert(T16 || !EX, "the EX sums need 16-byte table entries");
-    constexpr int S = accept_shift<T16>();
-    constexpr uint32_t M = 0xffu << S;
+    constexpr uint32_t M = 0xffu << ACCEPT_SHIFT;
     uint32_t a[4];
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
-        const uint32_t off = b == 0 ? (code << S) & M : (code >> (8 * b - S)) & M;
-        const char *p = reinterpret_cast<const char *>(lut) + off;
-        unsigned long long e, r;
-        uint32_t lo;
-        if constexpr (EX) {
-            const uint4 v = *reinterpret_cast<const uint4 *>(p);
-            asm("mov.b64 %0, {%1, %2};" : "=l"(e) : "r"(v.x), "r"(v.y));
-            r = e + (unsigned long long)w1[b];
-            asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(a[b]) : "l"(r));
-            d_sum += (int)(a[b] * v.z);                               // (-1) * (-d) for an accepted site
-            c_sum += (int)v.w;
-        } else {
-            const uint2 v = *reinterpret_cast<const uint2 *>(p);
-            asm("mov.b64 %0, {%1, %2};" : "=l"(e) : "r"(v.x), "r"(v.y));
-            r = e + (unsigned long long)w1[b];
-            asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(a[b]) : "l"(r));
-        }
+        const uint32_t sh = b == 0 ? code << ACCEPT_SHIFT : code >> (8 * b - ACCEPT_SHIFT);
+        const uint32_t off = lop3<0xEA>(sh, M, lane_off);              // (sh & M) | lane_off
+        const uint2 v = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(lut) + off);
+        unsigned long long e;
+        asm("mov.b64 %0, {%1, %2};" : "=l"(e) : "r"(v.x), "r"(v.y));
+        a[b] = (uint32_t)((e + (unsigned long long)w1[b]) >> 32);
     }
     const uint32_t m01 = lop3<LOP_SEL>(a[0], a[1], 0x000000ffu);
     const uint32_t m23 = lop3<LOP_SEL>(a[2], a[3], 0x00ffffffu);
     return lop3<LOP_SEL>(m01, m23, 0x0000ffffu);
+}
+
+// Sums over the four sites of a word from its code word and accept mask (sampled sweeps and the energy-change
+// series only).  ne_final_sum: unequal neighbours of the FINAL spins (accepted: the proposal's flags, else the
+// current spin's).  delta_sum: sum of d = n_old - n_new = c_new - c_old over the accepted sites.
+__device__ __forceinline__ int ne_final_sum(uint32_t code, uint32_t mask)
+{
+    return __popc(lop3<LOP_SEL>(code >> 4, code, mask) & 0x0f0f0f0fu);
+}
+
+__device__ __forceinline__ int delta_sum(uint32_t code, uint32_t mask)
+{
+    const uint32_t cm = code & mask;
+    return __popc(cm & 0xf0f0f0f0u) - __popc(cm & 0x0f0f0f0fu);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -390,20 +392,18 @@ __device__ __forceinline__ uint32_t accept_mask(uint32_t code, const uint32_t w1
 //   own      current spins of the 4 sites
 //   nb[4]    the 4 neighbour words (up, down, left, right: any order), prepared by prep_nbr<CM>
 //   w0, w1   Philox words of the 4 sites: proposal and acceptance
-// Returns the new word.  EX: d_sum += sum of d = n_old - n_new over the accepted sites (the energy change of
-// the word), c_sum += unequal neighbours of the OLD spins (so that the unequal neighbours
-// of the final spins sum to c_sum + d_sum).
-template <int CM, bool EX, bool T16 = EX>
+// Returns the new word; code / mask = the word's code bytes and accept mask for ne_final_sum / delta_sum.
+template <int CM>
 __device__ __forceinline__ uint32_t metropolis_word(uint32_t own, const uint32_t nb[4], uint32_t q, const uint32_t w0[4],
-                                                    const uint32_t w1[4], const AcceptEntry<T16> *lut,
-                                                    int &d_sum, int &c_sum)
+                                                    const uint32_t w1[4], const AcceptLut *lut, uint32_t lane_off,
+                                                    uint32_t &code, uint32_t &mask)
 {
     // R4: proposal floor(w0 q / 2^32), packed one byte per site
     const uint32_t s01 = __byte_perm(__umulhi(w0[0], q), __umulhi(w0[1], q), 0x0040);
     const uint32_t s23 = __byte_perm(__umulhi(w0[2], q), __umulhi(w0[3], q), 0x0040);
     const uint32_t prop = __byte_perm(s01, s23, 0x5410);
-    const uint32_t code = ne_code<CM>(own, prop, nb);                 // R5
-    const uint32_t mask = accept_mask<EX, T16>(code, w1, lut, d_sum, c_sum);   // R6
+    code = ne_code<CM>(own, prop, nb);                                // R5
+    mask = accept_mask(code, w1, lut, lane_off);                      // R6
     return lop3<LOP_SEL>(prop, own, mask);                            // R7
 }
 
@@ -426,19 +426,16 @@ __device__ __forceinline__ void draw_words(const HalfSweepKeys &K, const RowKeys
     }
 }
 
-// One word of the update from the neighbour words as loaded (byte b = that neighbour of site b).  `ex` is uniform
-// over the warp: with it the EX sums are formed (sampled sweeps, energy-change series), without it the table is
-// read 8 bytes at a time and the two extra instructions per site are skipped.
+// One word of the update from the neighbour words as loaded (byte b = that neighbour of site b).
 template <int CM, int ST>
 __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
                                                 uint32_t j0, uint32_t q, const HalfSweepKeys &K, const RowKeys &R,
-                                                const AcceptEntry<true> *lut, bool ex, int &d_sum, int &c_sum)
+                                                const AcceptLut *lut, uint32_t lane_off, uint32_t &code, uint32_t &mask)
 {
     uint32_t w0[4], w1[4];
     draw_words<ST>(K, R, j0, w0, w1);
     const uint32_t nb[4] = {prep_nbr<CM>(up), prep_nbr<CM>(dn), prep_nbr<CM>(lf), prep_nbr<CM>(rt)};
-    if (ex) return metropolis_word<CM, true, true>(own, nb, q, w0, w1, lut, d_sum, c_sum);
-    return metropolis_word<CM, false, true>(own, nb, q, w0, w1, lut, d_sum, c_sum);
+    return metropolis_word<CM>(own, nb, q, w0, w1, lut, lane_off, code, mask);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -51,10 +51,10 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
     constexpr bool EX = MEASURE || DELTA;
     extern __shared__ uint32_t s_dyn[];                       // HIST: the block's histogram table
     __shared__ uint4 s_col[2][HS_SITES][32];                  // ColKeys of [row parity p][site of the chunk][lane]
-    __shared__ AcceptEntry<EX> lut[ACCEPT_ENTRIES];
+    __shared__ AcceptLut lut;
     __shared__ int blockAcc;
     const uint32_t lane = threadIdx.x, wy = threadIdx.y, tid = wy * 32u + lane;
-    accept_lut_fill<EX>(lut, P.thr, tid, 32 * HS_WARPS);
+    accept_lut_fill(&lut, P.thr, tid, 32 * HS_WARPS);
     if (EX && tid == 0) blockAcc = 0;
     if (HIST)
         for (uint32_t n = tid; n < hist_words(P.q); n += 32 * HS_WARPS) s_dyn[n] = 0u;
@@ -78,8 +78,9 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
     }
     __syncthreads();
 
-    int d_sum = 0, c_sum = 0;
+    int acc = 0;                                                      // MEASURE: unequal neighbours of the final spins; DELTA: energy change
     if (active) {
+        const uint32_t lane_off = accept_lane_offset(lane);
         const uint32_t q = in_register(P.q);
         const int L = P.L, pitch = P.pitch;
         const int i0 = (int)(blockIdx.y * HS_WARPS + wy) * P.rpw;
@@ -122,7 +123,10 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
                         w0[2 * m] = w[0]; w1[2 * m] = w[1]; w0[2 * m + 1] = w[2]; w1[2 * m + 1] = w[3];
                     }
                 }
-                out[n] = metropolis_word<CM, EX>(own[n], nb, q, w0, w1, lut, d_sum, c_sum);
+                uint32_t code, mask;
+                out[n] = metropolis_word<CM>(own[n], nb, q, w0, w1, &lut, lane_off, code, mask);
+                if (MEASURE) acc += ne_final_sum(code, mask);
+                if (DELTA) acc += delta_sum(code, mask);
                 if (HIST) hist_add_word(s_dyn, P.q, out[n], lane);
             }
             *reinterpret_cast<uint4 *>(ownp + (size_t)i * pitch) = make_uint4(out[0], out[1], out[2], out[3]);
@@ -158,8 +162,8 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
         }
     }
     if (EX) {
-        // MEASURE: satisfied bonds = 4 per site - unequal neighbours of the final spins = 64 rpw - (c_sum + d_sum)
-        int v = DELTA ? d_sum : (active ? 64 * P.rpw - (c_sum + d_sum) : 0);
+        // MEASURE: satisfied bonds = 4 per site - unequal neighbours of the final spins = 64 rpw - acc
+        int v = DELTA ? acc : (active ? 64 * P.rpw - acc : 0);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
         if (lane == 0) atomicAdd(&blockAcc, v);

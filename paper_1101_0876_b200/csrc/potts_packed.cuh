@@ -85,10 +85,10 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_half_sweep_packed(const __gri
     constexpr bool EX = MEASURE || DELTA;
     constexpr int CM = FIVE ? CM_7BIT : CM_NIB4;
     extern __shared__ uint32_t s_dyn[];
-    __shared__ AcceptEntry<EX> lut[ACCEPT_ENTRIES];
+    __shared__ AcceptLut lut;
     __shared__ int blockAcc;
     const uint32_t tid = threadIdx.y * 32u + threadIdx.x;
-    accept_lut_fill<EX>(lut, P.thr, tid, 32 * PK_WARPS);
+    accept_lut_fill(&lut, P.thr, tid, 32 * PK_WARPS);
     if (EX && tid == 0) blockAcc = 0;
     if (HIST)
         for (uint32_t n = tid; n < hist_words(P.q); n += 32 * PK_WARPS) s_dyn[n] = 0u;
@@ -99,8 +99,9 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_half_sweep_packed(const __gri
     const int x = (int)(blockIdx.x * 32u + threadIdx.x);
     const int i0 = (int)(blockIdx.y * PK_WARPS + threadIdx.y) * P.rpt;
     const int c = (int)P.colour, o = 1 - c;
-    int d_sum = 0, c_sum = 0, rows_done = 0;
+    int acc = 0, rows_done = 0;
     if (x < chunks) {
+        const uint32_t lane_off = accept_lane_offset(threadIdx.x);
         const HalfSweepKeys &K = P.K;
         const uint32_t q = in_register(P.q);
         const int xn = x + 1 == chunks ? 0 : x + 1, xp = x == 0 ? chunks - 1 : x - 1;
@@ -149,7 +150,10 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_half_sweep_packed(const __gri
                     horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
                     draw_words<ST>(K, R, 2u * (uint32_t)(32 * x + 4 * n) + p, w0, w1);
                     const uint32_t nb[4] = {prep_nbr<CM>(up[hlf]), prep_nbr<CM>(dn[hlf]), prep_nbr<CM>(lf), prep_nbr<CM>(rt)};
-                    out[hlf] = metropolis_word<CM, EX>(own[hlf], nb, q, w0, w1, lut, d_sum, c_sum);
+                    uint32_t code, mask;
+                    out[hlf] = metropolis_word<CM>(own[hlf], nb, q, w0, w1, &lut, lane_off, code, mask);
+                    if (MEASURE) acc += ne_final_sum(code, mask);
+                    if (DELTA) acc += delta_sum(code, mask);
                     if (HIST) hist_add_word(s_dyn, P.q, out[hlf], threadIdx.x);
                 }
                 out_w[m] = pack_pair<FIVE>(out[0], out[1], m, out_h);
@@ -160,8 +164,8 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_half_sweep_packed(const __gri
         }
     }
     if (EX) {
-        // MEASURE: satisfied bonds = 4 per site - unequal neighbours of the final spins (c_sum + d_sum); DELTA: the change
-        int v = DELTA ? d_sum : 128 * rows_done - (c_sum + d_sum);
+        // MEASURE: satisfied bonds = 4 per site - unequal neighbours of the final spins; DELTA: the change
+        int v = DELTA ? acc : 128 * rows_done - acc;
 #pragma unroll
         for (int s = 16; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
         if (threadIdx.x == 0) atomicAdd(&blockAcc, v);

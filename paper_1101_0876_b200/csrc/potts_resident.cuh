@@ -106,7 +106,7 @@ template <int CM, int W, int ST>
 __device__ __forceinline__ void resident_run(const ResidentParams &P, const ResidentLattice &X)
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
-    __shared__ AcceptEntry<true> lut[ACCEPT_ENTRIES];
+    __shared__ AcceptLut lut;
 
     const uint32_t G = X.G, b = X.b;
     const int L = P.L, pitch = P.pitch;
@@ -148,7 +148,8 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
     const bool do_E = X.E_series != nullptr && P.every != 0;
     const bool do_D = X.dE_series != nullptr;
 
-    accept_lut_fill<true>(lut, X.thr, tid, nthreads);
+    accept_lut_fill(&lut, X.thr, tid, nthreads);
+    const uint32_t lane_off = accept_lane_offset(tid);
     if (do_hist)
         for (uint32_t n = tid; n < hist_words(P.q); n += nthreads) s_hist[n] = 0u;
     // own rows of both planes, and the halo rows of plane 1 (read by the first half-sweep, colour 0):
@@ -192,10 +193,9 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
             ++seq;
             uint8_t *const own_col = s_raw + c * plane_stride + col;                      // + lr*pitch: my chunk
             const uint8_t *const oth_row = s_raw + (1u - c) * plane_stride;               // + lr*pitch: row start
-            int d_sum = 0, c_sum = 0;
+            int d_sum = 0, ne_sum = 0;                              // energy change / unequal neighbours of the final spins
             uint32_t words_done = 0;
             const bool count_E = sample && c == 1 && do_E, count_H = sample && do_hist;
-            const bool ex = count_E || do_D;                        // form the EX sums (uniform over the block)
             if ((int)tid < nbar) {
                 const HalfSweepKeys K = half_sweep_keys(X.key0, X.key1, t, c);             // uniform registers
                 // one visit: local row lr, my W words
@@ -215,8 +215,11 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                         uint32_t lf0, rt0, lf1, rt1;
                         horizontal(p, mid.x, p ? mid.y : adj, lf0, rt0);
                         horizontal(p, mid.y, p ? adj : mid.x, lf1, rt1);
-                        out.x = update_word<CM, ST>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, lut, ex, d_sum, c_sum);
-                        out.y = update_word<CM, ST>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, lut, ex, d_sum, c_sum);
+                        uint32_t code0, mask0, code1, mask1;
+                        out.x = update_word<CM, ST>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, &lut, lane_off, code0, mask0);
+                        out.y = update_word<CM, ST>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, &lut, lane_off, code1, mask1);
+                        if (count_E) ne_sum += ne_final_sum(code0, mask0) + ne_final_sum(code1, mask1);
+                        if (do_D) d_sum += delta_sum(code0, mask0) + delta_sum(code1, mask1);
                         *reinterpret_cast<uint2 *>(own_col + ro) = out;
                         words_done += 2;
                         if (count_H) { hist_add_word(s_hist, P.q, out.x, tid & 31u); hist_add_word(s_hist, P.q, out.y, tid & 31u); }
@@ -227,7 +230,10 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                         const uint32_t dn = *reinterpret_cast<const uint32_t *>(orow + col + pitch);
                         uint32_t lf, rt;
                         horizontal(p, mid, adj, lf, rt);
-                        out.x = update_word<CM, ST>(own, up, dn, lf, rt, 2u * col + p, q, K, R, lut, ex, d_sum, c_sum);
+                        uint32_t code, mask;
+                        out.x = update_word<CM, ST>(own, up, dn, lf, rt, 2u * col + p, q, K, R, &lut, lane_off, code, mask);
+                        if (count_E) ne_sum += ne_final_sum(code, mask);
+                        if (do_D) d_sum += delta_sum(code, mask);
                         out.y = 0u;
                         *reinterpret_cast<uint32_t *>(own_col + ro) = out.x;
                         words_done += 1;
@@ -294,8 +300,8 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
             if (sample && c == 1) {
                 if (do_E) {
                     // satisfied bonds seen from this thread's black sites = 4 per site - unequal neighbours of the final
-                    // spins (c_sum + d_sum); one fire-and-forget int64 atomic per warp: no block-wide barrier for the energy
-                    uint32_t satisfied = 16u * words_done - (uint32_t)(c_sum + d_sum);
+                    // spins (ne_sum); one fire-and-forget int64 atomic per warp: no block-wide barrier for the energy
+                    uint32_t satisfied = 16u * words_done - (uint32_t)ne_sum;
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
                     if ((tid & 31u) == 0 && satisfied) atomicAdd(X.E_series + sample_idx, 0ull - (unsigned long long)satisfied);

@@ -73,6 +73,31 @@ def test_host_observables_against_exact_arithmetic(pb):
         pb.potts_observables(np.zeros(0, dtype=np.int64), 16, 1.0)
 
 
+def test_host_susceptibility_against_exact_arithmetic(pb):
+    """potts_susceptibility (Eq. 11) against exact rationals formed here, and closed cases."""
+    from fractions import Fraction
+    rng = np.random.default_rng(11)
+    q, N, T, n = 9, 32768 * 32768, 0.7177, 300
+    H = np.zeros((n, q), dtype=np.int64)
+    for k in range(n):                                   # near-ordered histograms: m ~ 0.9 with tiny fluctuations
+        minor = rng.integers(10_000_000, 10_100_000, size=q - 1)
+        H[k, 1:] = minor
+        H[k, 0] = N - minor.sum()
+    m1, m2, chi = pb.potts_susceptibility(H, q, T)
+    ms = [(Fraction(q * int(H[k].max()), N) - 1) / (q - 1) for k in range(n)]
+    w1 = sum(ms) / n
+    w2 = sum(m * m for m in ms) / n
+    wchi = N * (w2 - w1 * w1) / Fraction(T)
+    for got, want in ((m1, w1), (m2, w2), (chi, wchi)):
+        assert abs(Fraction(got) - want) <= Fraction(1, 10 ** 12) * abs(want)
+    # closed cases: ordered -> m = 1, chi = 0; {ordered, uniform} -> <m> = <m^2> = 1/2, chi = N/(4T)
+    assert pb.potts_susceptibility([[400, 0, 0, 0]] * 3, 4, 0.7) == (1.0, 1.0, 0.0)
+    assert pb.potts_susceptibility([[400, 0, 0, 0], [100, 100, 100, 100]], 4, 2.0) == (0.5, 0.5, 400 / 2.0 * 0.25)
+    for bad in ([[1, 2], [2, 2]], [[0, 0]], [[-1, 5]]):
+        with pytest.raises(pb.PottsError):
+            pb.potts_susceptibility(bad, 2, 1.0)
+
+
 def test_product_fails_loudly_without_a_gpu(pb):
     """No CPU fallback: on a box without a CUDA device every constructor refuses (on a GPU box this test is moot)."""
     import torch

@@ -331,3 +331,37 @@ def test_r10_observables_closed_cases():
     base = -(2 ** 31) + 12345
     big = [base + d for d in (0, 1, 2, 3, 4)]
     assert obs.specific_heat(big, 2 ** 30, 1.0) == 2.0 / 2 ** 30
+
+
+# ---------------------------------------------------------------- derived observables: closed cases
+def test_mean_energy_per_spin_closed_cases():
+    from oracle import observables as ob
+    N = 64 * 64
+    assert ob.mean_energy_per_spin([-2 * N] * 7, N) == -2.0                 # ordered state, Eq. 1: 2N satisfied bonds
+    assert ob.mean_energy_per_spin([-2 * N, 0], N) == -1.0
+    assert ob.mean_energy_per_spin([-3, -5, -4], 4) == -1.0                 # (-12 / 3) / 4
+    assert ob.mean_energy_per_spin([-1, -2], 3) == -0.5                     # (-3 / 2) / 3
+    # mean of per-sample energies per spin, the definition e = <E> / N (PAPER.md:209 uses e = E/N)
+    rng = np.random.default_rng(0)
+    E = rng.integers(-2 * N, 0, size=1000)
+    assert abs(ob.mean_energy_per_spin(E, N) - float(np.mean(E.astype(np.float64)) / N)) < 1e-12
+    # consistent with the single-sample form
+    assert ob.mean_energy_per_spin([-4582], N) == ob.energy_per_spin(-4582, N)
+
+
+def test_susceptibility_and_magnetisation_moments_closed_cases():
+    """chi = N/T (<m^2> - <m>^2) (Eq. 11) with m of Eq. 7."""
+    from oracle import observables as ob
+    q, N = 4, 400
+    ordered = [N, 0, 0, 0]                      # m = 1
+    uniform = [100, 100, 100, 100]              # m = 0
+    half = [250, 50, 50, 50]                    # Nmax/N = 5/8: m = (4 * 5/8 - 1) / 3 = 1/2
+    assert ob.magnetisation_moments([ordered] * 5, q) == (1.0, 1.0)
+    assert ob.susceptibility([ordered] * 5, q, 0.7) == 0.0                  # no fluctuation
+    assert ob.magnetisation_moments([ordered, uniform], q) == (0.5, 0.5)
+    assert ob.susceptibility([ordered, uniform], q, 2.0) == N / 2.0 * 0.25  # variance 1/4
+    m1, m2 = ob.magnetisation_moments([half, half, uniform, ordered], q)
+    assert m1 == 0.5 and m2 == (0.25 + 0.25 + 0.0 + 1.0) / 4
+    assert abs(ob.susceptibility([half, half, uniform, ordered], q, 0.5) - N / 0.5 * (0.375 - 0.25)) < 1e-12
+    # which state holds the majority does not matter (Eq. 7 uses the maximum)
+    assert ob.magnetisation_moments([[50, 250, 50, 50]], q) == (0.5, 0.25)

@@ -112,3 +112,63 @@ def test_invariants_threads_split_and_golden(golden_dir):
                 o.sweep(f * workloads.t_c(q), int(at) - t)
                 t = int(at)
                 assert o.energy() == int(want), (case, at)
+
+
+def test_stream2_sweep_is_the_site_rule_applied_in_checkerboard_order():
+    """Pins the stream-2 branch of the oracle's half_sweep (which word and which partner counter each site of a
+    full sweep takes): one sweep rebuilt site by site with oracle.update_site(stream=2) -- itself pinned above
+    against the KAT-pinned Philox routine -- must equal OraclePotts(stream=2).sweep.  L % 4 == 0, several q, and a
+    temperature at which many proposals are rejected, so a wrong word shows up as a different accept decision."""
+    for L, q, seed, f in ((16, 7, 9, 0.9), (8, 3, 42, 0.7), (12, 24, 5, 1.0)):
+        T = f * workloads.t_c(q)
+        o = oracle.OraclePotts(L, q, seed, oracle.INIT_RANDOM, stream=2)
+        o.sweep(T, 3)
+        before, t = o.spins(), o.t
+        o.sweep(T, 1)
+        after = o.spins()
+        mid = before.copy()
+        rejected = 0
+        for colour in (0, 1):
+            src = mid.copy()
+            for i in range(L):
+                for j in range(L):
+                    if (i + j) % 2 == colour:
+                        nb = [src[(i - 1) % L, j], src[(i + 1) % L, j], src[i, (j - 1) % L], src[i, (j + 1) % L]]
+                        mid[i, j] = oracle.update_site(i, j, t, colour, seed, q, T, src[i, j], nb, stream=2)
+                        # what the site would have taken had every proposal been accepted
+                        rejected += int(oracle.update_site(i, j, t, colour, seed, q, 1e15, src[i, j], nb, stream=2) != mid[i, j])
+        assert (mid == after).all()
+        assert rejected > L * L // 8                    # the case does exercise the acceptance word
+        # and the stream-1 chain from the same state is a different one
+        o1 = oracle.OraclePotts(L, q, seed, oracle.INIT_RANDOM, stream=1)
+        o1.set_state(before, t)
+        o1.sweep(T, 1)
+        assert (o1.spins() != after).any()
+
+
+def test_stream2_sweep_from_the_philox_words():
+    """The same sweep once more from the definition R3' itself: Philox words through the KAT-pinned routine,
+    thresholds through the P2-pinned routine, word (0,1) for even k, (2,3) of the partner's block for odd k."""
+    L, q, seed = 8, 5, 77
+    T = 0.8 * workloads.t_c(q)
+    thr = oracle.thresholds(T)
+    o = oracle.OraclePotts(L, q, seed, oracle.INIT_RANDOM, stream=2)
+    o.sweep(T, 2)
+    s, t = o.spins().astype(int), o.t
+    o.sweep(T, 1)
+    for colour in (0, 1):
+        src = s.copy()
+        for i in range(L):
+            for j in range(L):
+                if (i + j) % 2 != colour:
+                    continue
+                k = j >> 1
+                jb = j if k % 2 == 0 else j - 2
+                w = oracle.philox4x32_10([jb, i, t, colour], [seed & 0xFFFFFFFF, seed >> 32])
+                w_prop, w_acc = (w[0], w[1]) if k % 2 == 0 else (w[2], w[3])
+                new = (w_prop * q) >> 32
+                nb = [src[(i - 1) % L, j], src[(i + 1) % L, j], src[i, (j - 1) % L], src[i, (j + 1) % L]]
+                d = sum(x == src[i, j] for x in nb) - sum(x == new for x in nb)
+                if d <= 0 or w_acc < thr[d - 1]:
+                    s[i, j] = new
+    assert (s == o.spins()).all()

@@ -68,7 +68,7 @@ CONFIGS = {
                 note="small case the oracle finishes in seconds"),
     2: Workload("cfg2_q6_L1024", q=6, L=1024, init=INIT_ORDERED, seed=7, t_factors=[1.005],
                 sweeps_per_t=10_000, every=1, hist=False,
-                note="heating run from the ordered state; headline bench workload"),
+                note="heating run from the ordered state"),
     3: Workload("cfg3_q9_L4096", q=9, L=4096, init=INIT_RANDOM, seed=3, t_factors=_scan16(),
                 sweeps_per_t=2000, every=1, hist=True,
                 note="16-point temperature scan, cooling, state carried over"),
@@ -77,7 +77,7 @@ CONFIGS = {
                 note="sub-byte packed layout"),
     5: Workload("cfg5_q9_L32768", q=9, L=32768, init=INIT_RANDOM, seed=5, t_factors=[0.995],
                 sweeps_per_t=1000, every=10, hist=True,
-                note="1.07e9 spins, streams from HBM"),
+                note="1.07e9 spins, streams from HBM; headline bench workload (largest single-GPU configuration)"),
 }
 
 
