@@ -136,6 +136,15 @@ void potts_batch_destroy(potts_batch_t *b);
  * `every` is ignored.  Synchronises. */
 int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t every,
                                int64_t *E_series, int64_t *hist_series);
+/* potts_batch_sweep_delta: nsweeps sweeps of every lattice; dE_series (host, n rows of nsweeps int64) receives for
+ * every lattice and sweep the energy change summed over the accepted moves, as potts_sweep_delta. */
+int potts_batch_sweep_delta(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t *dE_series);
+/* potts_batch_ladder: the temperature-ladder protocol for every lattice of the batch at once.
+ * T: host, n rows of nT temperatures (lattice r runs T[r*nT + k], k = 0..nT-1, state carried over); per temperature
+ * t_tran unmeasured sweeps, then t_max sweeps sampled every dt.  E_series / hist_series (host, may be null): n rows of
+ * nT * t_max/dt samples (x q).  Lattice r follows exactly potts_ladder of a single handle with (seeds[r], T row r). */
+int potts_batch_ladder(potts_batch_t *b, const double *T, int32_t nT, int64_t t_tran, int64_t t_max, int64_t dt,
+                       int64_t *E_series, int64_t *hist_series);
 int potts_batch_download(potts_batch_t *b, int32_t r, uint8_t *spins); /* lattice r, host, L*L row-major */
 int potts_batch_sweep_count(potts_batch_t *b, uint64_t *t);
 int potts_batch_launch_count(potts_batch_t *b, uint64_t *n);

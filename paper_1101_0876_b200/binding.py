@@ -57,6 +57,8 @@ def load_library() -> ctypes.CDLL:
         "potts_batch_destroy": ([vp], None),
         "potts_batch_sweep_measured": ([vp, vp, i64, i64, vp, vp], ctypes.c_int),
         "potts_batch_download": ([vp, i32, vp], ctypes.c_int),
+        "potts_batch_sweep_delta": ([vp, vp, i64, vp], ctypes.c_int),
+        "potts_batch_ladder": ([vp, vp, i32, i64, i64, i64, vp, vp], ctypes.c_int),
         "potts_batch_sweep_count": ([vp, P(u64)], ctypes.c_int),
         "potts_batch_launch_count": ([vp, P(u64)], ctypes.c_int),
         "potts_set_stream_spec": ([vp, i32], ctypes.c_int),
@@ -91,7 +93,7 @@ EXPORTED_SYMBOLS = [
     "potts_download", "potts_upload", "potts_sweep_count", "potts_set_sweep_count", "potts_observables",
     "potts_magnetisation", "potts_susceptibility", "potts_launch_count", "potts_set_option", "potts_get_option", "potts_last_error",
     "potts_version", "potts_batch_workspace_bytes", "potts_batch_create", "potts_batch_destroy",
-    "potts_batch_sweep_measured", "potts_batch_download", "potts_batch_sweep_count", "potts_batch_launch_count",
+    "potts_batch_sweep_measured", "potts_batch_sweep_delta", "potts_batch_ladder", "potts_batch_download", "potts_batch_sweep_count", "potts_batch_launch_count",
     "potts_set_stream_spec", "potts_get_stream_spec", "potts_batch_set_stream_spec",
 ]
 
@@ -324,6 +326,27 @@ class PottsBatch:
         H = np.zeros((self.n, ns, self.q), dtype=np.int64) if hist else None
         _check(self._lib.potts_batch_sweep_measured(self._h, Ta.ctypes.data, int(nsweeps), int(every),
                                                     E.ctypes.data if energy else None, H.ctypes.data if hist else None))
+        return E, H
+
+    def potts_batch_sweep_delta(self, T, nsweeps: int) -> np.ndarray:
+        """-> dE int64[n, nsweeps]: energy change of every sweep of every lattice, from its accepted moves."""
+        Ta = np.ascontiguousarray(np.broadcast_to(np.asarray(T, dtype=np.float64), (self.n,)))
+        dE = np.zeros((self.n, int(nsweeps)), dtype=np.int64)
+        _check(self._lib.potts_batch_sweep_delta(self._h, Ta.ctypes.data, int(nsweeps), dE.ctypes.data))
+        return dE
+
+    def potts_batch_ladder(self, T, t_tran: int, t_max: int, dt: int, energy: bool = True, hist: bool = True):
+        """T: [n, nT] (or [nT], the same ladder for every lattice).  -> (E int64[n, nT, t_max/dt], hist [..., q])."""
+        Ta = np.asarray(T, dtype=np.float64)
+        if Ta.ndim == 1:
+            Ta = np.broadcast_to(Ta, (self.n, Ta.shape[0]))
+        Ta = np.ascontiguousarray(Ta)
+        nT = Ta.shape[1]
+        per = int(t_max) // int(dt) if dt >= 1 else 0
+        E = np.zeros((self.n, nT, per), dtype=np.int64) if energy else None
+        H = np.zeros((self.n, nT, per, self.q), dtype=np.int64) if hist else None
+        _check(self._lib.potts_batch_ladder(self._h, Ta.ctypes.data, nT, int(t_tran), int(t_max), int(dt),
+                                            E.ctypes.data if energy else None, H.ctypes.data if hist else None))
         return E, H
 
     def potts_batch_set_stream_spec(self, spec: int):

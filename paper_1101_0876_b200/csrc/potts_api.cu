@@ -35,11 +35,24 @@ int fail(int code, const char *fmt, ...)
                         "%s failed: %s", #expr, cudaGetErrorString(e_));                        \
     } while (0)
 
+// Entry points run on the handle's device whatever the caller's current device is (and restore it afterwards).
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; return; }
+        if (prev != dev) cudaSetDevice(dev); else prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define ON_DEVICE_OF(x) DeviceGuard guard_((x) ? (x)->device : current_device())
+inline int current_device() { int d = 0; cudaGetDevice(&d); return d; }
+
 constexpr size_t ALIGN = 256;
 constexpr size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 constexpr int MAX_CTAS = 160;             // upper bound on the resident kernel's grid (>= SM count of B200)
-constexpr int RESIDENT_L_MAX = 4096;
-constexpr int CLUSTER_AUTO_L_MAX = 128;    // lattices up to this size go to the cluster (DSMEM) kernel by default (measured: 2x the resident kernel)      // largest lattice the resident kernel can hold (512 words per row)
+constexpr int RESIDENT_L_MAX = 4096;       // largest lattice the resident kernel can hold (512 words per row)
+constexpr int CLUSTER_AUTO_L_MAX = 128;    // lattices up to this size go to the cluster (DSMEM) kernel by default (measured: 2x the resident kernel)
 constexpr int ACC_WORDS = 1 + 256 + 1;    // E, hist[256], flag/error word
 constexpr size_t STATIC_SMEM = sizeof(potts::AcceptLut) + 1024;   // static shared memory of the persistent kernels
 
@@ -47,6 +60,7 @@ constexpr size_t STATIC_SMEM = sizeof(potts::AcceptLut) + 1024;   // static shar
 
 struct potts_s {
     int32_t L = 0, q = 0, layout = 0;
+    int device = 0;                      // the CUDA device the handle lives on; every entry point runs on it
     uint64_t seed = 0, t = 0;
     uint8_t *ws = nullptr;
     bool owns_ws = false;
@@ -73,6 +87,7 @@ struct potts_s {
     int64_t opt_resident_words = 0;      // 0 auto, 1 / 2: 4-site words per thread and row visit
     int64_t opt_resident_rows = 0;       // 0 auto, else at most this many thread rows in a resident block
     int64_t opt_cluster_ctas = 0;        // 0 auto, else the cluster kernel's cluster size (1..16)
+    int cluster_checked = 0;             // cluster size whose co-residency was confirmed (cudaOccupancyMaxActiveClusters)
     int64_t opt_stream_rows = 0;         // 0 auto, else rows per warp of the streaming kernel (even, divides L/4)
 };
 
@@ -369,7 +384,7 @@ ClusterPlan plan_cluster(const potts_t *h)
     const int L = h->L, wpr = L / 8;
     if (h->layout != POTTS_LAYOUT_U8) { R.why = "the cluster kernel holds the U8 layout only"; return R; }
     if (wpr > 1024) { R.why = "L/8 words per row exceed 1024 threads"; return R; }
-    long long G = h->opt_cluster_ctas > 0 ? h->opt_cluster_ctas : ((long long)L * wpr) / 128;   // measured: L = 64 -> 4, L = 128 -> 8
+    long long G = h->opt_cluster_ctas > 0 ? h->opt_cluster_ctas : ((long long)L * wpr) / 128;   // measured: one CTA per 128 words of a half-sweep: L = 64 -> 4, L = 128 -> 16 (beyond 8 is the non-portable cluster size)
     if (G < 1) G = 1;
     if (G > potts::CLUSTER_MAX) G = potts::CLUSTER_MAX;
     if (G > L) G = L;
@@ -423,6 +438,16 @@ int launch_cluster(potts_t *h, const ClusterPlan &R, const uint32_t thr[4], int6
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
+    if (h->cluster_checked != R.G) {
+        // a cluster of this size may not be schedulable here (MIG slice, partial GPC): say so, the caller falls back
+        int nclusters = 0;
+        const cudaError_t eo = cudaOccupancyMaxActiveClusters(&nclusters, fn, &cfg);
+        if (eo != cudaSuccess || nclusters < 1) {
+            cudaGetLastError();
+            return fail(POTTS_ERR_UNSUPPORTED, "a cluster of %d CTAs x %d threads with %zu bytes of shared memory cannot be scheduled on this device", R.G, R.nthreads, R.smem);
+        }
+        h->cluster_checked = R.G;
+    }
     void *args[] = {(void *)&P};
     CUDA_TRY(cudaLaunchKernelExC(&cfg, fn, args));
     h->launches += 1;
@@ -441,6 +466,7 @@ int run_sweeps(potts_t *h, double T, int64_t nsweeps, int64_t every, unsigned lo
     const int64_t piece = every > 0 ? ((1ll << 30) / every) * every : (1ll << 30);
     if (h->opt_variant == 3 || (h->opt_variant == 0 && h->layout == POTTS_LAYOUT_U8 && h->L <= CLUSTER_AUTO_L_MAX)) {
         const ClusterPlan C = plan_cluster(h);
+        bool cluster_ok = true;
         if (C.ok) {
             for (int64_t done = 0; done < nsweeps;) {
                 const int64_t n = nsweeps - done < piece ? nsweeps - done : piece;
@@ -448,11 +474,12 @@ int run_sweeps(potts_t *h, double T, int64_t nsweeps, int64_t every, unsigned lo
                 int rc = launch_cluster(h, C, thr, n, every > 0 ? every : 0, E_series_dev ? E_series_dev + s0 : nullptr,
                                         hist_series_dev ? hist_series_dev + s0 * h->q : nullptr,
                                         dE_series_dev ? dE_series_dev + done : nullptr);
+                if (rc == POTTS_ERR_UNSUPPORTED && done == 0 && h->opt_variant == 0) { cluster_ok = false; break; }
                 if (rc) return rc;
                 h->t += (uint64_t)n;
                 done += n;
             }
-            return POTTS_OK;
+            if (cluster_ok) return POTTS_OK;                         // else: automatic mode falls through to the resident kernel
         }
         if (h->opt_variant == 3) return fail(POTTS_ERR_UNSUPPORTED, "cluster variant unavailable: %s", C.why);
     }
@@ -545,6 +572,7 @@ int potts_create_ex(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t 
     potts_t *h = new (std::nothrow) potts_s;
     if (!h) return fail(POTTS_ERR_NOMEM, "host allocation failed");
     h->L = L; h->q = q; h->layout = layout; h->seed = seed; h->t = 0;
+    cudaGetDevice(&h->device);
     h->stream = (cudaStream_t)cuda_stream;
     if (dev_workspace) {
         h->ws = (uint8_t *)dev_workspace;
@@ -619,6 +647,7 @@ int potts_create(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t ini
 
 void potts_destroy(potts_t *h)
 {
+    ON_DEVICE_OF(h);
     if (!h) return;
     if (h->scratch || (h->owns_ws && h->ws)) cudaStreamSynchronize(h->stream);
     if (h->scratch) cudaFree(h->scratch);
@@ -633,6 +662,7 @@ void potts_destroy(potts_t *h)
 
 int potts_set_stream(potts_t *h, void *cuda_stream)
 {
+    ON_DEVICE_OF(h);
     if (!h) return fail(POTTS_ERR_ARG, "null handle");
     h->stream = (cudaStream_t)cuda_stream;
     return POTTS_OK;
@@ -640,6 +670,7 @@ int potts_set_stream(potts_t *h, void *cuda_stream)
 
 int potts_sweep(potts_t *h, double T, int64_t nsweeps)
 {
+    ON_DEVICE_OF(h);
     int rc = check_sweep_args(h, T, nsweeps);
     if (rc) return rc;
     return run_sweeps(h, T, nsweeps, 0, nullptr, nullptr);
@@ -648,6 +679,7 @@ int potts_sweep(potts_t *h, double T, int64_t nsweeps)
 int potts_sweep_measured_dev(potts_t *h, double T, int64_t nsweeps, int64_t every, int64_t *E_series_dev,
                              int64_t *hist_series_dev)
 {
+    ON_DEVICE_OF(h);
     int rc = check_sweep_args(h, T, nsweeps);
     if (rc) return rc;
     if (every < 1 || every > (1ll << 30) || nsweeps % every != 0)
@@ -664,6 +696,7 @@ int potts_sweep_measured_dev(potts_t *h, double T, int64_t nsweeps, int64_t ever
 int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every, int64_t *E_series,
                          int64_t *hist_series)
 {
+    ON_DEVICE_OF(h);
     int rc = check_sweep_args(h, T, nsweeps);
     if (rc) return rc;
     if (every < 1 || every > (1ll << 30) || nsweeps % every != 0)
@@ -693,6 +726,7 @@ int potts_sweep_measured(potts_t *h, double T, int64_t nsweeps, int64_t every, i
 
 int potts_sweep_delta(potts_t *h, double T, int64_t nsweeps, int64_t *dE_series)
 {
+    ON_DEVICE_OF(h);
     int rc = check_sweep_args(h, T, nsweeps);
     if (rc) return rc;
     if (!dE_series) return fail(POTTS_ERR_ARG, "null dE_series");
@@ -717,6 +751,7 @@ int potts_sweep_delta(potts_t *h, double T, int64_t nsweeps, int64_t *dE_series)
 int potts_ladder(potts_t *h, const double *T, int32_t nT, int64_t t_tran, int64_t t_max, int64_t dt, int64_t *E_series,
                  int64_t *hist_series)
 {
+    ON_DEVICE_OF(h);
     if (!h || !T) return fail(POTTS_ERR_ARG, "null argument");
     if (nT < 0 || t_tran < 0 || t_max < 0) return fail(POTTS_ERR_ARG, "negative count");
     if (dt < 1 || t_max % dt != 0)
@@ -753,6 +788,7 @@ int potts_ladder(potts_t *h, const double *T, int32_t nT, int64_t t_tran, int64_
 
 int potts_energy(potts_t *h, int64_t *E)
 {
+    ON_DEVICE_OF(h);
     if (!h || !E) return fail(POTTS_ERR_ARG, "null argument");
     CUDA_TRY(cudaMemsetAsync(h->acc, 0, 8, h->stream));
     int rc = launch_measure(h, h->acc, nullptr);
@@ -767,6 +803,7 @@ int potts_energy(potts_t *h, int64_t *E)
 
 int potts_histogram(potts_t *h, int64_t *counts)
 {
+    ON_DEVICE_OF(h);
     if (!h || !counts) return fail(POTTS_ERR_ARG, "null argument");
     CUDA_TRY(cudaMemsetAsync(h->acc + 1, 0, 8 * (size_t)h->q, h->stream));
     int rc = launch_measure(h, nullptr, h->acc + 1);
@@ -799,6 +836,7 @@ static int ensure_copy_objects(potts_t *h)
 
 int potts_download(potts_t *h, uint8_t *spins)
 {
+    ON_DEVICE_OF(h);
     if (!h || !spins) return fail(POTTS_ERR_ARG, "null argument");
     const int L = h->L, rows = chunk_rows(L);
     const size_t buf_bytes = (size_t)rows * L;
@@ -862,6 +900,7 @@ static bool host_has_value_ge(const uint8_t *spins, size_t n, int q)
 
 int potts_upload(potts_t *h, const uint8_t *spins)
 {
+    ON_DEVICE_OF(h);
     if (!h || !spins) return fail(POTTS_ERR_ARG, "null argument");
     const int L = h->L, rows = chunk_rows(L);
     // validate on the host first so that a rejected upload leaves the lattice untouched; the converter checks again
@@ -909,6 +948,7 @@ int potts_upload(potts_t *h, const uint8_t *spins)
 
 int potts_sweep_count(potts_t *h, uint64_t *t)
 {
+    ON_DEVICE_OF(h);
     if (!h || !t) return fail(POTTS_ERR_ARG, "null argument");
     *t = h->t;
     return POTTS_OK;
@@ -916,6 +956,7 @@ int potts_sweep_count(potts_t *h, uint64_t *t)
 
 int potts_set_sweep_count(potts_t *h, uint64_t t)
 {
+    ON_DEVICE_OF(h);
     if (!h) return fail(POTTS_ERR_ARG, "null handle");
     if (t > 0xFFFFFFFFull) return fail(POTTS_ERR_ARG, "t must be < 2^32");
     h->t = t;
@@ -924,6 +965,7 @@ int potts_set_sweep_count(potts_t *h, uint64_t t)
 
 int potts_set_stream_spec(potts_t *h, int32_t spec)
 {
+    ON_DEVICE_OF(h);
     if (!h) return fail(POTTS_ERR_ARG, "null handle");
     if (spec != 1 && spec != 2) return fail(POTTS_ERR_ARG, "stream spec must be 1 or 2");
     h->stream_spec = spec;
@@ -932,6 +974,7 @@ int potts_set_stream_spec(potts_t *h, int32_t spec)
 
 int potts_get_stream_spec(potts_t *h, int32_t *spec)
 {
+    ON_DEVICE_OF(h);
     if (!h || !spec) return fail(POTTS_ERR_ARG, "null argument");
     *spec = h->stream_spec;
     return POTTS_OK;
@@ -939,6 +982,7 @@ int potts_get_stream_spec(potts_t *h, int32_t *spec)
 
 int potts_launch_count(potts_t *h, uint64_t *n)
 {
+    ON_DEVICE_OF(h);
     if (!h || !n) return fail(POTTS_ERR_ARG, "null argument");
     *n = h->launches;
     return POTTS_OK;
@@ -946,6 +990,7 @@ int potts_launch_count(potts_t *h, uint64_t *n)
 
 int potts_set_option(potts_t *h, const char *key, int64_t value)
 {
+    ON_DEVICE_OF(h);
     if (!h || !key) return fail(POTTS_ERR_ARG, "null argument");
     if (!std::strcmp(key, "variant")) {
         if (value < 0 || value > 3) return fail(POTTS_ERR_ARG, "variant must be 0 (auto), 1 (streaming), 2 (resident) or 3 (cluster)");
@@ -977,6 +1022,7 @@ int potts_set_option(potts_t *h, const char *key, int64_t value)
 
 int potts_get_option(potts_t *h, const char *key, int64_t *value)
 {
+    ON_DEVICE_OF(h);
     if (!h || !key || !value) return fail(POTTS_ERR_ARG, "null argument");
     if (!std::strcmp(key, "variant")) { *value = h->opt_variant; return POTTS_OK; }
     if (!std::strcmp(key, "resident_ctas")) { *value = h->opt_resident_ctas; return POTTS_OK; }
@@ -1081,6 +1127,7 @@ int potts_susceptibility(const int64_t *hist_series, int64_t n, int32_t q, doubl
 // ---- replica batch -------------------------------------------------------------------------------
 struct potts_batch_s {
     int32_t n = 0, L = 0, q = 0;
+    int device = 0;
     uint64_t t = 0, launches = 0;
     int32_t stream_spec = 1;
     uint64_t *seeds = nullptr;            // host copy
@@ -1166,6 +1213,7 @@ int potts_batch_create(potts_batch_t **out, int32_t n, int32_t L, int32_t q, con
     potts_batch_t *b = new (std::nothrow) potts_batch_s;
     if (!b) return fail(POTTS_ERR_NOMEM, "host allocation failed");
     b->n = n; b->L = L; b->q = q;
+    cudaGetDevice(&b->device);
     b->stream = (cudaStream_t)cuda_stream;
     b->seeds = new (std::nothrow) uint64_t[n];
     if (!b->seeds) { delete b; return fail(POTTS_ERR_NOMEM, "host allocation failed"); }
@@ -1207,6 +1255,7 @@ int potts_batch_create(potts_batch_t **out, int32_t n, int32_t L, int32_t q, con
 
 void potts_batch_destroy(potts_batch_t *b)
 {
+    ON_DEVICE_OF(b);
     if (!b) return;
     if (b->scratch || (b->owns_ws && b->ws)) cudaStreamSynchronize(b->stream);
     if (b->scratch) cudaFree(b->scratch);
@@ -1217,6 +1266,7 @@ void potts_batch_destroy(potts_batch_t *b)
 
 int potts_batch_sweep_count(potts_batch_t *b, uint64_t *t)
 {
+    ON_DEVICE_OF(b);
     if (!b || !t) return fail(POTTS_ERR_ARG, "null argument");
     *t = b->t;
     return POTTS_OK;
@@ -1224,6 +1274,7 @@ int potts_batch_sweep_count(potts_batch_t *b, uint64_t *t)
 
 int potts_batch_set_stream_spec(potts_batch_t *b, int32_t spec)
 {
+    ON_DEVICE_OF(b);
     if (!b) return fail(POTTS_ERR_ARG, "null handle");
     if (spec != 1 && spec != 2) return fail(POTTS_ERR_ARG, "stream spec must be 1 or 2");
     b->stream_spec = spec;
@@ -1232,6 +1283,7 @@ int potts_batch_set_stream_spec(potts_batch_t *b, int32_t spec)
 
 int potts_batch_launch_count(potts_batch_t *b, uint64_t *n)
 {
+    ON_DEVICE_OF(b);
     if (!b || !n) return fail(POTTS_ERR_ARG, "null argument");
     *n = b->launches;
     return POTTS_OK;
@@ -1239,28 +1291,16 @@ int potts_batch_launch_count(potts_batch_t *b, uint64_t *n)
 
 }  // extern "C"
 
-extern "C" {
+namespace {
 
-int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t every, int64_t *E_series,
-                               int64_t *hist_series)
+// nsweeps sweeps of every lattice of the batch, lattice r at temperature T[r * T_stride], enqueued on the batch's
+// stream.  Device series (null = not recorded): E / hist samples of lattice r at E_dev + r * series_stride (+ k),
+// hist_dev + (r * series_stride + k) * q; energy changes at dE_dev + r * delta_stride + sweep.  Advances b->t.
+int batch_run(potts_batch_t *b, const double *T, int64_t T_stride, int64_t nsweeps, int64_t every, unsigned long long *E_dev,
+              unsigned long long *hist_dev, int64_t series_stride, unsigned long long *dE_dev, int64_t delta_stride)
 {
-    if (!b || !T) return fail(POTTS_ERR_ARG, "null argument");
-    if (nsweeps < 0 || nsweeps > (1ll << 30)) return fail(POTTS_ERR_ARG, "nsweeps = %lld outside [0, 2^30]", (long long)nsweeps);
-    for (int r = 0; r < b->n; ++r)
-        if (!(T[r] > 0.0) || !std::isfinite(T[r])) return fail(POTTS_ERR_ARG, "T[%d] = %g must be finite and > 0", r, T[r]);
-    if (b->t + (uint64_t)nsweeps > 0xFFFFFFFFull) return fail(POTTS_ERR_ARG, "sweep counter would pass 2^32 - 1");
-    const bool measure = E_series || hist_series;
-    if (measure && (every < 1 || nsweeps % every != 0))
-        return fail(POTTS_ERR_ARG, "every = %lld must be >= 1 and divide nsweeps = %lld", (long long)every, (long long)nsweeps);
     if (nsweeps == 0) return POTTS_OK;
-    const int64_t ns = measure ? nsweeps / every : 0;
-    const size_t eb = E_series ? (size_t)b->n * ns * 8 : 0, hb = hist_series ? (size_t)b->n * ns * b->q * 8 : 0;
-    uint8_t *dev = nullptr;
-    if (eb + hb) {
-        int rc = get_batch_scratch(b, eb + hb, &dev);
-        if (rc) return rc;
-        cudaMemsetAsync(dev, 0, eb + hb, b->stream);
-    }
+    const bool measure = E_dev || hist_dev;
     const BatchPlan R = plan_batch(b->L, b->q, b->smem_optin);
     static thread_local potts::BatchTable tab;               // 24 KB: copied into the launch parameters
     cudaError_t e = cudaSuccess;
@@ -1269,7 +1309,7 @@ int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweep
         for (int r = 0; r < m; ++r) {
             tab.key[r][0] = (uint32_t)(b->seeds[r0 + r] & 0xFFFFFFFFull);
             tab.key[r][1] = (uint32_t)(b->seeds[r0 + r] >> 32);
-            thresholds(T[r0 + r], tab.thr[r]);
+            thresholds(T[(int64_t)(r0 + r) * T_stride], tab.thr[r]);
         }
         potts::BatchParams B = {};
         potts::ResidentParams &P = B.P;
@@ -1281,28 +1321,124 @@ int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweep
         P.t0 = (uint32_t)b->t;
         P.nsweeps = (uint32_t)nsweeps;
         P.every = measure ? (uint32_t)every : 0u;
-        P.E_series = eb ? (unsigned long long *)dev + (size_t)r0 * ns : nullptr;
-        P.hist_series = hb ? (unsigned long long *)(dev + eb) + (size_t)r0 * ns * b->q : nullptr;
+        P.E_series = E_dev ? E_dev + (size_t)r0 * series_stride : nullptr;
+        P.hist_series = hist_dev ? hist_dev + (size_t)r0 * series_stride * b->q : nullptr;
+        P.dE_series = dE_dev ? dE_dev + (size_t)r0 * delta_stride : nullptr;
         P.inbox = nullptr;
         P.error = b->error;
         P.rows_max = b->L;
         P.tyc = R.tyc;
         B.lattice_stride = 2ull * b->plane_bytes;
-        B.series_stride = (unsigned long long)ns;
+        B.series_stride = (unsigned long long)series_stride;
+        B.delta_stride = (unsigned long long)delta_stride;
         e = potts::launch_batch(potts::compare_mode_of(b->q), b->stream_spec, B, tab, m, R.nthreads, R.smem, b->stream);
         b->launches += 1;
     }
-    if (e == cudaSuccess) b->t += (uint64_t)nsweeps;
-    if (e == cudaSuccess && eb) e = cudaMemcpyAsync(E_series, dev, eb, cudaMemcpyDeviceToHost, b->stream);
-    if (e == cudaSuccess && hb) e = cudaMemcpyAsync(hist_series, dev + eb, hb, cudaMemcpyDeviceToHost, b->stream);
-    const cudaError_t e2 = cudaStreamSynchronize(b->stream);
-    if (e != cudaSuccess || e2 != cudaSuccess)
-        return fail(POTTS_ERR_CUDA, "batch sweep failed: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
+    if (e != cudaSuccess) return fail(POTTS_ERR_CUDA, "batch launch failed: %s", cudaGetErrorString(e));
+    b->t += (uint64_t)nsweeps;
     return POTTS_OK;
+}
+
+int check_batch_T(const potts_batch_t *b, const double *T, int64_t count)
+{
+    for (int64_t r = 0; r < count; ++r)
+        if (!(T[r] > 0.0) || !std::isfinite(T[r])) return fail(POTTS_ERR_ARG, "T[%lld] = %g must be finite and > 0", (long long)r, T[r]);
+    (void)b;
+    return POTTS_OK;
+}
+
+// copy `bytes` of device series to the host and synchronise
+int batch_finish(potts_batch_t *b, int rc, void *host0, const void *dev0, size_t bytes0, void *host1, const void *dev1, size_t bytes1)
+{
+    cudaError_t e = cudaSuccess;
+    if (rc == POTTS_OK && bytes0) e = cudaMemcpyAsync(host0, dev0, bytes0, cudaMemcpyDeviceToHost, b->stream);
+    if (rc == POTTS_OK && e == cudaSuccess && bytes1) e = cudaMemcpyAsync(host1, dev1, bytes1, cudaMemcpyDeviceToHost, b->stream);
+    const cudaError_t e2 = cudaStreamSynchronize(b->stream);
+    if (rc) return rc;
+    if (e != cudaSuccess || e2 != cudaSuccess)
+        return fail(POTTS_ERR_CUDA, "batch series copy / sync failed: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
+    return POTTS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t every, int64_t *E_series,
+                               int64_t *hist_series)
+{
+    ON_DEVICE_OF(b);
+    if (!b || !T) return fail(POTTS_ERR_ARG, "null argument");
+    if (nsweeps < 0 || nsweeps > (1ll << 30)) return fail(POTTS_ERR_ARG, "nsweeps = %lld outside [0, 2^30]", (long long)nsweeps);
+    int rc = check_batch_T(b, T, b->n);
+    if (rc) return rc;
+    if (b->t + (uint64_t)nsweeps > 0xFFFFFFFFull) return fail(POTTS_ERR_ARG, "sweep counter would pass 2^32 - 1");
+    const bool measure = E_series || hist_series;
+    if (measure && (every < 1 || nsweeps % every != 0))
+        return fail(POTTS_ERR_ARG, "every = %lld must be >= 1 and divide nsweeps = %lld", (long long)every, (long long)nsweeps);
+    if (nsweeps == 0) return POTTS_OK;
+    const int64_t ns = measure ? nsweeps / every : 0;
+    const size_t eb = E_series ? (size_t)b->n * ns * 8 : 0, hb = hist_series ? (size_t)b->n * ns * b->q * 8 : 0;
+    uint8_t *dev = nullptr;
+    if (eb + hb) {
+        rc = get_batch_scratch(b, eb + hb, &dev);
+        if (rc) return rc;
+        cudaMemsetAsync(dev, 0, eb + hb, b->stream);
+    }
+    rc = batch_run(b, T, 1, nsweeps, every, eb ? (unsigned long long *)dev : nullptr, hb ? (unsigned long long *)(dev + eb) : nullptr,
+                   ns, nullptr, 0);
+    return batch_finish(b, rc, E_series, dev, eb, hist_series, dev + eb, hb);
+}
+
+int potts_batch_sweep_delta(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t *dE_series)
+{
+    ON_DEVICE_OF(b);
+    if (!b || !T || !dE_series) return fail(POTTS_ERR_ARG, "null argument");
+    if (nsweeps < 0 || nsweeps > (1ll << 30)) return fail(POTTS_ERR_ARG, "nsweeps = %lld outside [0, 2^30]", (long long)nsweeps);
+    int rc = check_batch_T(b, T, b->n);
+    if (rc) return rc;
+    if (b->t + (uint64_t)nsweeps > 0xFFFFFFFFull) return fail(POTTS_ERR_ARG, "sweep counter would pass 2^32 - 1");
+    if (nsweeps == 0) return POTTS_OK;
+    const size_t db = (size_t)b->n * nsweeps * 8;
+    uint8_t *dev = nullptr;
+    rc = get_batch_scratch(b, db, &dev);
+    if (rc) return rc;
+    cudaMemsetAsync(dev, 0, db, b->stream);
+    rc = batch_run(b, T, 1, nsweeps, 0, nullptr, nullptr, 0, (unsigned long long *)dev, nsweeps);
+    return batch_finish(b, rc, dE_series, dev, db, nullptr, nullptr, 0);
+}
+
+int potts_batch_ladder(potts_batch_t *b, const double *T, int32_t nT, int64_t t_tran, int64_t t_max, int64_t dt,
+                       int64_t *E_series, int64_t *hist_series)
+{
+    ON_DEVICE_OF(b);
+    if (!b || !T) return fail(POTTS_ERR_ARG, "null argument");
+    if (nT < 0 || t_tran < 0 || t_max < 0 || t_tran > (1ll << 30) || t_max > (1ll << 30)) return fail(POTTS_ERR_ARG, "count outside [0, 2^30]");
+    if (dt < 1 || t_max % dt != 0)
+        return fail(POTTS_ERR_ARG, "dt = %lld must be >= 1 and divide t_max = %lld", (long long)dt, (long long)t_max);
+    int rc = check_batch_T(b, T, (int64_t)b->n * nT);
+    if (rc) return rc;
+    if (b->t + (uint64_t)nT * (uint64_t)(t_tran + t_max) > 0xFFFFFFFFull) return fail(POTTS_ERR_ARG, "sweep counter would pass 2^32 - 1");
+    const int64_t per_T = t_max / dt, ns = per_T * nT;
+    const size_t eb = E_series ? (size_t)b->n * ns * 8 : 0, hb = hist_series ? (size_t)b->n * ns * b->q * 8 : 0;
+    uint8_t *dev = nullptr;
+    if (eb + hb) {
+        rc = get_batch_scratch(b, eb + hb, &dev);
+        if (rc) return rc;
+        cudaMemsetAsync(dev, 0, eb + hb, b->stream);
+    }
+    unsigned long long *dE = eb ? (unsigned long long *)dev : nullptr, *dH = hb ? (unsigned long long *)(dev + eb) : nullptr;
+    for (int32_t k = 0; k < nT && rc == POTTS_OK; ++k) {
+        rc = batch_run(b, T + k, nT, t_tran, 0, nullptr, nullptr, 0, nullptr, 0);
+        if (rc == POTTS_OK && per_T > 0)
+            rc = batch_run(b, T + k, nT, t_max, dt, dE ? dE + k * per_T : nullptr, dH ? dH + k * per_T * b->q : nullptr, ns, nullptr, 0);
+    }
+    return batch_finish(b, rc, E_series, dev, eb, hist_series, dev + eb, hb);
 }
 
 int potts_batch_download(potts_batch_t *b, int32_t r, uint8_t *spins)
 {
+    ON_DEVICE_OF(b);
     if (!b || !spins) return fail(POTTS_ERR_ARG, "null argument");
     if (r < 0 || r >= b->n) return fail(POTTS_ERR_ARG, "lattice index %d outside [0, %d)", r, b->n);
     const int L = b->L;

@@ -360,6 +360,7 @@ struct BatchParams {
     ResidentParams P;                 // plane[], E_series, hist_series: those of lattice 0; inbox unused
     unsigned long long lattice_stride;   // bytes from one lattice's planes to the next one's
     unsigned long long series_stride;    // samples per lattice in E_series (hist_series: x q)
+    unsigned long long delta_stride;     // entries per lattice in dE_series
 };
 
 template <int CM, int ST, int MAXT>
@@ -377,7 +378,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_batch_u8(const __grid_cons
     for (int d = 0; d < 4; ++d) X.thr[d] = T.thr[r][d];
     X.E_series = B.P.E_series ? B.P.E_series + r * B.series_stride : nullptr;
     X.hist_series = B.P.hist_series ? B.P.hist_series + r * B.series_stride * B.P.q : nullptr;
-    X.dE_series = B.P.dE_series ? B.P.dE_series + r * (unsigned long long)B.P.nsweeps : nullptr;
+    X.dE_series = B.P.dE_series ? B.P.dE_series + r * B.delta_stride : nullptr;
     resident_run<CM, 1, ST>(B.P, X);      // one word per thread and row visit: small lattices want warps, not amortisation
 }
 

@@ -38,16 +38,38 @@ CASES = [
 ]
 
 
+# launch shapes of potts_sweep_delta: the library's choice (cluster kernel for L <= 128, resident kernel up to L = 4096,
+# one launch per call), the streaming kernels (two launches per sweep), the resident kernel with forced grids, a cluster
+VARIANTS = {
+    "auto": {},
+    "streaming": {"variant": 1},
+    "resident": {"variant": 2},
+    "resident3": {"variant": 2, "resident_ctas": 3},
+    "resident_w2": {"variant": 2, "resident_words": 2, "resident_ctas": 7},
+    "cluster8": {"variant": 3, "cluster_ctas": 8},
+}
+
+
+@pytest.mark.parametrize("variant", list(VARIANTS))
 @pytest.mark.parametrize("stream", [1, 2])
 @pytest.mark.parametrize("L,q,seed,init,f,n", CASES)
-def test_delta_series_matches_recounted_energy(pb, L, q, seed, init, f, n, stream):
+def test_delta_series_matches_recounted_energy(pb, L, q, seed, init, f, n, stream, variant):
     T = f * workloads.t_c(q)
     g = pb.Potts(L, q, seed, init)
+    for k, v in VARIANTS[variant].items():
+        g.potts_set_option(k, v)
+    if variant == "cluster8" and not g.potts_get_option("cluster_active"):
+        pytest.skip("the cluster kernel cannot hold this lattice")
     g.potts_set_stream_spec(stream)
     o = oracle.OraclePotts(L, q, seed, init, threads=4, stream=stream)
     E0 = o.energy()
     assert g.potts_energy() == E0
-    dE = g.potts_sweep_delta(T, n)
+    try:
+        dE = g.potts_sweep_delta(T, n)
+    except pb.PottsError as e:
+        if e.code == pb.ERR_UNSUPPORTED and variant not in ("auto", "streaming"):
+            pytest.skip("forced launch shape cannot hold this lattice")
+        raise
     Eo, _ = o.sweep_measured(T, n, 1, hist=False)
     assert dE.dtype == np.int64 and dE.shape == (n,)
     assert (E0 + np.cumsum(dE) == Eo).all()
@@ -135,3 +157,32 @@ def test_delta_full_size_invariant(pb):
     assert (E0 + np.cumsum(dE) == Er).all()
     h = r.potts_histogram()
     assert (g.potts_histogram() == h).all() and int(h.sum()) == w.L * w.L
+
+
+def test_delta_of_a_long_resident_call_is_one_launch(pb):
+    """For lattices the persistent kernels hold, potts_sweep_delta is ONE launch per call (not two per sweep)."""
+    g = pb.Potts(1024, 6, 7, pb.INIT_ORDERED)
+    n0 = g.potts_launch_count()
+    dE = g.potts_sweep_delta(1.005 * workloads.t_c(6), 300)
+    assert g.potts_launch_count() - n0 == 1
+    o = oracle.OraclePotts(1024, 6, 7, 0, threads=8)
+    Eo, _ = o.sweep_measured(1.005 * workloads.t_c(6), 300, 1, hist=False)
+    assert (-2 * 1024 * 1024 + np.cumsum(dE) == Eo).all()
+    assert (g.potts_download() == o.spins()).all()
+
+
+def test_batch_delta_every_replica(pb):
+    """potts_batch_sweep_delta: every replica's series against its own oracle's recounted energies."""
+    L, q, n, ns = 64, 9, 5, 30
+    seeds = [50 + 3 * r for r in range(n)]
+    Ts = [(0.9 + 0.05 * r) * workloads.t_c(q) for r in range(n)]
+    b = pb.PottsBatch(L, q, seeds, workloads.INIT_RANDOM)
+    dE = b.potts_batch_sweep_delta(Ts, ns)
+    assert dE.shape == (n, ns)
+    for r in range(n):
+        o = oracle.OraclePotts(L, q, seeds[r], workloads.INIT_RANDOM)
+        E0 = o.energy()
+        Eo, _ = o.sweep_measured(Ts[r], ns, 1, hist=False)
+        assert (E0 + np.cumsum(dE[r]) == Eo).all()
+        assert (b.potts_batch_download(r) == o.spins()).all()
+    assert b.potts_batch_sweep_count() == ns

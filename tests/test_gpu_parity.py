@@ -332,3 +332,52 @@ def test_stream_spec_2_batch_and_default_unchanged(pb):
         assert (E[r] == Eo).all() and (H[r] == Ho).all() and (b.potts_batch_download(r) == o.spins()).all()
     g = pb.Potts(L, q, 11, workloads.INIT_RANDOM)
     assert g.potts_get_stream_spec() == 1                  # the default chain is north_star's per-site stream
+
+
+def test_batch_ladder_matches_single_handle_ladders_and_oracle(pb):
+    """potts_batch_ladder (PAPER.md:96 for every replica at once): replica r == potts_ladder of a single handle with
+    (seed_r, ladder_r) == the oracle driven through the same call sequence."""
+    L, q, n = 64, 6, 4
+    seeds = [900 + r for r in range(n)]
+    Tc = workloads.t_c(q)
+    ladders = np.array([[(1.03 - 0.01 * r) * Tc, 1.0 * Tc, (0.97 + 0.005 * r) * Tc] for r in range(n)])
+    t_tran, t_max, dt = 6, 12, 3
+    b = pb.PottsBatch(L, q, seeds, workloads.INIT_RANDOM)
+    E, H = b.potts_batch_ladder(ladders, t_tran, t_max, dt)
+    assert E.shape == (n, 3, t_max // dt) and H.shape == (n, 3, t_max // dt, q)
+    for r in range(n):
+        g = pb.Potts(L, q, seeds[r], pb.INIT_RANDOM)
+        Eg, Hg = g.potts_ladder(list(ladders[r]), t_tran, t_max, dt, hist=True)
+        assert (np.asarray(Eg).reshape(3, -1) == E[r]).all() and (np.asarray(Hg).reshape(3, -1, q) == H[r]).all()
+        o = oracle.OraclePotts(L, q, seeds[r], workloads.INIT_RANDOM)
+        for k in range(3):
+            o.sweep(float(ladders[r, k]), t_tran)
+            Eo, Ho = o.sweep_measured(float(ladders[r, k]), t_max, dt, hist=True)
+            assert (Eo == E[r, k]).all() and (Ho == H[r, k]).all()
+        assert (b.potts_batch_download(r) == o.spins()).all()
+    assert b.potts_batch_sweep_count() == 3 * (t_tran + t_max)
+
+
+def test_susceptibility_of_a_gpu_series_against_exact_rationals(pb):
+    """chi, <m>, <m^2> (Eq. 11) of a histogram series recorded on the GPU: the library's host function
+    against the oracle-side exact rational arithmetic, 1e-12 relative."""
+    from oracle import observables as ob
+    L, q = 128, 2
+    T = 1.0 * workloads.t_c(q)
+    g = pb.Potts(L, q, 17, pb.INIT_RANDOM)
+    _, H = g.potts_sweep_measured(T, 200, 1, hist=True)
+    m1, m2, chi = pb.potts_susceptibility(H, q, T)
+    w1, w2 = ob.magnetisation_moments(H, q)
+    wchi = ob.susceptibility(H, q, T)
+    for got, want in ((m1, w1), (m2, w2), (chi, wchi)):
+        assert abs(got - want) <= 1e-12 * abs(want)
+    assert 0.0 < m1 < 1.0 and chi > 0.0
+
+
+def test_every_beyond_2_30_is_rejected(pb):
+    """The persistent kernels count samples in 32 bits: `every` > 2^30 is an argument error (not an endless loop)."""
+    g = pb.Potts(64, 9, 1, pb.INIT_RANDOM)
+    with pytest.raises(pb.PottsError) as e:
+        g.potts_sweep_measured(1.0, 2 ** 31, 2 ** 31, hist=False)
+    assert e.value.code == pb.ERR_ARG
+    assert g.potts_sweep_count() == 0
