@@ -162,7 +162,7 @@ class GpuRun:
     @property
     def kernel(self):
         if self.layout != self.pb.LAYOUT_U8:
-            return "k_half_sweep_packed"
+            return "k_sweep_rows_packed"
         if self.cluster_ctas:
             return "k_cluster_u8"
         return "k_resident_u8" if self.resident_ctas else "k_sweep_rows_u8"
@@ -497,7 +497,7 @@ def delta_cost(pb, torch, k, sweeps, repeats=5):
         out[name + "_ns_per_spin_flip"] = statistics.median(ns)
         out[name + "_min_max"] = [min(ns), max(ns)]
         out["kernel"] = "k_cluster_u8" if g.potts_get_option("cluster_active") else (
-            "k_resident_u8" if g.potts_get_option("resident_active") else ("k_half_sweep_packed" if w.packed else "k_sweep_rows_u8"))
+            "k_resident_u8" if g.potts_get_option("resident_active") else ("k_sweep_rows_packed" if w.packed else "k_sweep_rows_u8"))
         g.close()
     out["delta_over_plain"] = out["delta_ns_per_spin_flip"] / out["plain_ns_per_spin_flip"]
     return out

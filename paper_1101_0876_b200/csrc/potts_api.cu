@@ -53,7 +53,7 @@ constexpr size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 constexpr int MAX_CTAS = 160;             // upper bound on the resident kernel's grid (>= SM count of B200)
 constexpr int RESIDENT_L_MAX = 4096;       // largest lattice the resident kernel can hold (512 words per row)
 constexpr int CLUSTER_AUTO_L_MAX = 128;    // lattices up to this size go to the cluster (DSMEM) kernel by default (measured: 2x the resident kernel)
-constexpr int ACC_WORDS = 1 + 256 + 1;    // E, hist[256], flag/error word
+constexpr int ACC_WORDS = 1 + 256 + 2;    // E, hist[256], flag/error word, tile counter of the streaming kernels
 constexpr size_t STATIC_SMEM = sizeof(potts::AcceptLut) + 1024;   // static shared memory of the persistent kernels
 
 }  // namespace
@@ -70,6 +70,7 @@ struct potts_s {
     unsigned long long *acc = nullptr;   // device scratch: [0] = E, [1..q] = histogram
     int *flag = nullptr;                 // device scratch flag (upload validation)
     int *error = nullptr;                // device: set by the resident kernel if a neighbour wait gave up
+    uint32_t *tile_counter = nullptr;    // device: tile counter of the streaming kernels (0 between launches)
     uint8_t *inbox = nullptr;            // device: resident kernel's boundary-row packets (null if L too large)
     cudaStream_t stream = nullptr;
     uint64_t launches = 0;
@@ -165,24 +166,10 @@ potts::SweepParams sweep_params(const potts_t *h, uint32_t colour, const uint32_
     return P;
 }
 
-// Rows per warp of k_sweep_rows_u8: a power of two that divides L / HS_WARPS (L % 32 == 0, so 8 always does).  More rows
-// per warp spread the block's start-up (accept table, ColKeys of 1024 columns, first two neighbour rows) over more
-// sites; too many leave too few blocks to fill 148 SMs evenly.
-int rows_per_warp(const potts_t *h, unsigned gx)
-{
-    const double startup = 2.0;                             // start-up of a block, in row visits per warp
-    int best = 2;
-    double best_cost = 1e300;
-    for (int rpw = 2; rpw <= 64; rpw <<= 1) {
-        if ((h->L / potts::HS_WARPS) % rpw) break;
-        const long long blocks = (long long)gx * (h->L / (potts::HS_WARPS * rpw));
-        const long long per_sm = (blocks + h->num_sms - 1) / h->num_sms;      // blocks the busiest SM runs
-        double cost = (double)per_sm * (rpw + startup);
-        if (per_sm < 4) cost *= 1.0 + 0.15 * (double)(4 - per_sm);            // too few warps to fill the issue slots
-        if (cost < best_cost * 0.999) { best_cost = cost; best = rpw; }
-    }
-    return best;
-}
+// Rows per warp of a tile of the streaming kernels (L % 32 == 0, so 8 divides L / HS_WARPS).  Tiles are drawn from a
+// counter by as many blocks as are resident at once, so small tiles cost nothing but the two neighbour rows a warp
+// loads before its first visit; measured on B200 (profiles/r02b_kernels.md).
+constexpr int STREAM_ROWS_PER_WARP = 8;
 
 // delta = true: E_out receives the sum of the accepted moves' d instead of the energy (hist_out must be null)
 int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsigned long long *E_out,
@@ -192,10 +179,12 @@ int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsign
     P.hist_out = hist_out;
     const int chunks = h->L / 32;
     const unsigned gx = (unsigned)((chunks + 31) / 32);
-    P.rpw = h->opt_stream_rows > 0 ? (int)h->opt_stream_rows : rows_per_warp(h, gx);
-    const dim3 grid(gx, (unsigned)(h->L / (potts::HS_WARPS * P.rpw)));
+    P.rpw = h->opt_stream_rows > 0 ? (int)h->opt_stream_rows : STREAM_ROWS_PER_WARP;
+    P.row_groups = h->L / (potts::HS_WARPS * P.rpw);
+    P.total_tiles = gx * (uint32_t)P.row_groups;
+    P.tile_counter = h->tile_counter;
     const size_t smem = hist_out ? (size_t)potts::hist_words((uint32_t)h->q) * 4 : 0;
-    potts::launch_sweep_rows_u8(potts::compare_mode_of(h->q), h->stream_spec, delta, P, grid, smem, h->stream);
+    potts::launch_sweep_rows_u8(potts::compare_mode_of(h->q), h->stream_spec, delta, P, h->num_sms, smem, h->stream);
     return check_launch(h, "k_sweep_rows_u8");
 }
 
@@ -213,13 +202,13 @@ int launch_half_sweep_packed(potts_t *h, uint32_t colour, const uint32_t thr[4],
     P.hist_out = hist_out;
     const int chunks = h->L / 64;
     const unsigned gx = (unsigned)((chunks + 31) / 32);
-    int rpt = 4;                                     // L % 64 == 0, so 4 divides L / PK_WARPS
-    while (rpt > 1 && (long long)gx * (h->L / (potts::PK_WARPS * rpt)) < 8ll * h->num_sms) rpt >>= 1;
-    P.rpt = rpt;
-    const dim3 grid(gx, (unsigned)(h->L / (potts::PK_WARPS * rpt)));
-    const size_t smem = hist_out ? (size_t)h->q * 32 * 4 : 0;
-    potts::launch_sweep_rows_packed(h->q > 16, h->stream_spec, delta, P, grid, delta ? 0 : smem, h->stream);
-    return check_launch(h, "k_half_sweep_packed");
+    P.rpw = h->opt_stream_rows > 0 ? (int)h->opt_stream_rows : STREAM_ROWS_PER_WARP;
+    P.row_groups = h->L / (potts::PK_WARPS * P.rpw);
+    P.total_tiles = gx * (uint32_t)P.row_groups;
+    P.tile_counter = h->tile_counter;
+    const size_t smem = hist_out ? (size_t)potts::hist_words((uint32_t)h->q) * 4 : 0;
+    potts::launch_sweep_rows_packed(h->q > 16, h->stream_spec, delta, P, h->num_sms, smem, h->stream);
+    return check_launch(h, "k_sweep_rows_packed");
 }
 
 int launch_measure(potts_t *h, unsigned long long *E_out, unsigned long long *hist_out)
@@ -600,6 +589,7 @@ int potts_create_ex(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t 
     h->acc = (unsigned long long *)(h->ws + 2 * h->plane_bytes);
     h->flag = (int *)(h->acc + 257);
     h->error = h->flag + 1;
+    h->tile_counter = (uint32_t *)(h->acc + 258);
     h->inbox = inbox_bytes_of(L) ? h->ws + 2 * h->plane_bytes + align_up(ACC_WORDS * sizeof(unsigned long long)) : nullptr;
     {
         int dev = 0, v = 0;

@@ -90,7 +90,7 @@ struct HalfSweepKeys {
     uint32_t xa;      // hi(M1*t) ^ k0[0]          c0 after round 1 is xa ^ i
     uint32_t xb;      // colour ^ k1[0]            c2 after round 1 is hi(M0*j) ^ xb
     uint32_t xc;      // lo(M1*t) ^ k0[1]          c0 after round 2 is hi(M1*c2') ^ xc
-    uint32_t k0, k1;  // the key itself (round r uses k + r*W)
+    uint32_t r0[10], r1[10];  // the round keys: round r (0-based) uses r0[r] = key0 + r W0, r1[r] = key1 + r W1
 };
 
 // Host and device: the streaming kernels get the keys as launch parameters (if every thread derived
@@ -105,8 +105,11 @@ __host__ __device__ inline HalfSweepKeys half_sweep_keys(uint32_t key0, uint32_t
     K.xa = hi ^ key0;
     K.xb = colour ^ key1;
     K.xc = lo ^ (key0 + PHILOX_W0);
-    K.k0 = key0;
-    K.k1 = key1;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        K.r0[r] = key0 + (uint32_t)r * PHILOX_W0;
+        K.r1[r] = key1 + (uint32_t)r * PHILOX_W1;
+    }
     return K;
 }
 
@@ -120,7 +123,7 @@ __device__ __forceinline__ RowKeys row_keys(const HalfSweepKeys &K, uint32_t i)
     RowKeys R;
     uint32_t hi;
     mul_wide(PHILOX_M0, K.xa ^ i, hi, R.c3);
-    R.xd = hi ^ (K.k1 + PHILOX_W1);
+    R.xd = hi ^ K.r1[1];
     return R;
 }
 
@@ -131,20 +134,17 @@ __device__ __forceinline__ void philox_site(const HalfSweepKeys &K, const RowKey
     mul_wide(PHILOX_M0, j, h0, l0);                  // round 1, the M0*c0 product
     mul_wide(PHILOX_M1, h0 ^ K.xb, h1, l1);          // round 2, the M1*c2 product
     uint32_t c0 = h1 ^ K.xc, c1 = l1, c2 = l0 ^ R.xd, c3 = R.c3;
-    uint32_t k0 = K.k0 + 2u * PHILOX_W0, k1 = K.k1 + 2u * PHILOX_W1;
 #pragma unroll
     for (int r = 2; r < 9; ++r) {
         mul_wide(PHILOX_M0, c0, h0, l0);
         mul_wide(PHILOX_M1, c2, h1, l1);
-        c0 = h1 ^ c1 ^ k0;
+        c0 = h1 ^ c1 ^ K.r0[r];
         c1 = l1;
-        c2 = h0 ^ c3 ^ k1;
+        c2 = h0 ^ c3 ^ K.r1[r];
         c3 = l0;
-        k0 += PHILOX_W0;
-        k1 += PHILOX_W1;
     }
     mul_wide(PHILOX_M1, c2, h1, l1);                 // round 10: only words 0 and 1 are used
-    w0 = h1 ^ c1 ^ k0;
+    w0 = h1 ^ c1 ^ K.r0[9];
     w1 = l1;
 }
 
@@ -156,17 +156,14 @@ __device__ __forceinline__ void philox_pair(const HalfSweepKeys &K, const RowKey
     mul_wide(PHILOX_M0, j, h0, l0);
     mul_wide(PHILOX_M1, h0 ^ K.xb, h1, l1);
     uint32_t c0 = h1 ^ K.xc, c1 = l1, c2 = l0 ^ R.xd, c3 = R.c3;
-    uint32_t k0 = K.k0 + 2u * PHILOX_W0, k1 = K.k1 + 2u * PHILOX_W1;
 #pragma unroll
     for (int r = 2; r < 10; ++r) {
         mul_wide(PHILOX_M0, c0, h0, l0);
         mul_wide(PHILOX_M1, c2, h1, l1);
-        c0 = h1 ^ c1 ^ k0;
+        c0 = h1 ^ c1 ^ K.r0[r];
         c1 = l1;
-        c2 = h0 ^ c3 ^ k1;
+        c2 = h0 ^ c3 ^ K.r1[r];
         c3 = l0;
-        k0 += PHILOX_W0;
-        k1 += PHILOX_W1;
     }
     w[0] = c0; w[1] = c1; w[2] = c2; w[3] = c3;
 }
@@ -199,52 +196,48 @@ __device__ __forceinline__ RowKeysH row_keys_h(const HalfSweepKeys &K, uint32_t 
     const RowKeys R = row_keys(K, i);
     RowKeysH H;
     H.xd = R.xd;
-    H.rc = R.c3 ^ (K.k1 + 2u * PHILOX_W1);
+    H.rc = R.c3 ^ K.r1[2];
     return H;
 }
 
 // rounds 3-9 from (ColKeys, RowKeysH); leaves the state before round 10 and the keys of round 10
 __device__ __forceinline__ void philox_rounds_h(const HalfSweepKeys &K, const RowKeysH &R, const ColKeys &C,
-                                                uint32_t &c0, uint32_t &c1, uint32_t &c2, uint32_t &c3, uint32_t &k0, uint32_t &k1)
+                                                uint32_t &c0, uint32_t &c1, uint32_t &c2, uint32_t &c3)
 {
     uint32_t h0, l0, h1, l1;
     mul_wide(PHILOX_M1, C.l0 ^ R.xd, h1, l1);        // round 3: the M1*c2 product (M0*c0 is in C)
-    c0 = h1 ^ C.l1 ^ (K.k0 + 2u * PHILOX_W0);
+    c0 = h1 ^ C.l1 ^ K.r0[2];
     c1 = l1;
     c2 = C.ph ^ R.rc;
     c3 = C.pl;
-    k0 = K.k0 + 3u * PHILOX_W0;
-    k1 = K.k1 + 3u * PHILOX_W1;
 #pragma unroll
     for (int r = 3; r < 9; ++r) {
         mul_wide(PHILOX_M0, c0, h0, l0);
         mul_wide(PHILOX_M1, c2, h1, l1);
-        c0 = h1 ^ c1 ^ k0;
+        c0 = h1 ^ c1 ^ K.r0[r];
         c1 = l1;
-        c2 = h0 ^ c3 ^ k1;
+        c2 = h0 ^ c3 ^ K.r1[r];
         c3 = l0;
-        k0 += PHILOX_W0;
-        k1 += PHILOX_W1;
     }
 }
 
 __device__ __forceinline__ void philox_site_h(const HalfSweepKeys &K, const RowKeysH &R, const ColKeys &C,
                                               uint32_t &w0, uint32_t &w1)
 {
-    uint32_t c0, c1, c2, c3, k0, k1, h1, l1;
-    philox_rounds_h(K, R, C, c0, c1, c2, c3, k0, k1);
+    uint32_t c0, c1, c2, c3, h1, l1;
+    philox_rounds_h(K, R, C, c0, c1, c2, c3);
     mul_wide(PHILOX_M1, c2, h1, l1);                 // round 10: only words 0 and 1 are used
-    w0 = h1 ^ c1 ^ k0;
+    w0 = h1 ^ c1 ^ K.r0[9];
     w1 = l1;
 }
 
 __device__ __forceinline__ void philox_pair_h(const HalfSweepKeys &K, const RowKeysH &R, const ColKeys &C, uint32_t w[4])
 {
-    uint32_t c0, c1, c2, c3, k0, k1, h0, l0, h1, l1;
-    philox_rounds_h(K, R, C, c0, c1, c2, c3, k0, k1);
+    uint32_t c0, c1, c2, c3, h0, l0, h1, l1;
+    philox_rounds_h(K, R, C, c0, c1, c2, c3);
     mul_wide(PHILOX_M0, c0, h0, l0);
     mul_wide(PHILOX_M1, c2, h1, l1);
-    w[0] = h1 ^ c1 ^ k0; w[1] = l1; w[2] = h0 ^ c3 ^ k1; w[3] = l0;
+    w[0] = h1 ^ c1 ^ K.r0[9]; w[1] = l1; w[2] = h0 ^ c3 ^ K.r1[9]; w[3] = l0;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -340,16 +333,20 @@ constexpr int ACCEPT_SLOTS = 8;
 constexpr int ACCEPT_SHIFT = 6;                                 // log2(8 bytes * ACCEPT_SLOTS)
 struct AcceptLut { uint2 e[ACCEPT_ENTRIES][ACCEPT_SLOTS]; };    // 16 KB
 
-__device__ __forceinline__ void accept_lut_fill(AcceptLut *lut, const uint32_t thr[4], uint32_t tid, uint32_t nthreads)
+// fast = true (allowed only if every thr[d] >= 1, i.e. no "never accept" entry): the entry's first word is
+// threshold(d) - 1 instead, and a site accepts iff w1 <= that word (0xffffffff for d <= 0): one 32-bit compare.
+__device__ __forceinline__ void accept_lut_fill(AcceptLut *lut, const uint32_t thr[4], uint32_t tid, uint32_t nthreads, bool fast = false)
 {
     for (uint32_t n = tid; n < (uint32_t)(ACCEPT_ENTRIES * ACCEPT_SLOTS); n += nthreads) {
         const uint32_t code = n / ACCEPT_SLOTS;
         const int d = __popc(code >> 4) - __popc(code & 15u);
         const unsigned long long th = d <= 0 ? (1ull << 32) : (unsigned long long)(d == 1 ? thr[0] : (d == 2 ? thr[1] : (d == 3 ? thr[2] : thr[3])));
-        const unsigned long long e = 0ull - th;
+        const unsigned long long e = fast ? th - 1ull : 0ull - th;
         (&lut->e[0][0])[n] = make_uint2((uint32_t)e, (uint32_t)(e >> 32));
     }
 }
+
+__host__ __device__ inline bool accept_fast_ok(const uint32_t thr[4]) { return thr[0] && thr[1] && thr[2] && thr[3]; }
 
 // byte offset of this lane's slot inside a table row
 __device__ __forceinline__ uint32_t accept_lane_offset(uint32_t lane) { return (lane % ACCEPT_SLOTS) * 8u; }
@@ -373,6 +370,23 @@ __device__ __forceinline__ uint32_t accept_mask(uint32_t code, const uint32_t w1
     return lop3<LOP_SEL>(m01, m23, 0x0000ffffu);
 }
 
+// Fast form (table filled with fast = true): the new word directly, one compare and one predicated byte insert per site.
+__device__ __forceinline__ uint32_t accept_insert(uint32_t own, uint32_t prop, uint32_t code, const uint32_t w1[4], const AcceptLut *lut,
+                                                  uint32_t lane_off)
+{
+    constexpr uint32_t M = 0xffu << ACCEPT_SHIFT;
+    uint32_t out = own;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        const uint32_t sh = b == 0 ? code << ACCEPT_SHIFT : code >> (8 * b - ACCEPT_SHIFT);
+        const uint32_t off = lop3<0xEA>(sh, M, lane_off);
+        const uint32_t t = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(lut) + off);
+        const uint32_t ins = __byte_perm(out, prop, b == 0 ? 0x3214 : (b == 1 ? 0x3250 : (b == 2 ? 0x3610 : 0x7210)));
+        out = w1[b] <= t ? ins : out;
+    }
+    return out;
+}
+
 // Sums over the four sites of a word from its code word and accept mask (sampled sweeps and the energy-change
 // series only).  ne_final_sum: unequal neighbours of the FINAL spins (accepted: the proposal's flags, else the
 // current spin's).  delta_sum: sum of d = n_old - n_new = c_new - c_old over the accepted sites.
@@ -393,7 +407,7 @@ __device__ __forceinline__ int delta_sum(uint32_t code, uint32_t mask)
 //   nb[4]    the 4 neighbour words (up, down, left, right: any order), prepared by prep_nbr<CM>
 //   w0, w1   Philox words of the 4 sites: proposal and acceptance
 // Returns the new word; code / mask = the word's code bytes and accept mask for ne_final_sum / delta_sum.
-template <int CM>
+template <int CM, bool FAST = false>
 __device__ __forceinline__ uint32_t metropolis_word(uint32_t own, const uint32_t nb[4], uint32_t q, const uint32_t w0[4],
                                                     const uint32_t w1[4], const AcceptLut *lut, uint32_t lane_off,
                                                     uint32_t &code, uint32_t &mask)
@@ -403,6 +417,10 @@ __device__ __forceinline__ uint32_t metropolis_word(uint32_t own, const uint32_t
     const uint32_t s23 = __byte_perm(__umulhi(w0[2], q), __umulhi(w0[3], q), 0x0040);
     const uint32_t prop = __byte_perm(s01, s23, 0x5410);
     code = ne_code<CM>(own, prop, nb);                                // R5
+    if (FAST) {
+        mask = 0u;                                                    // not formed: the sums need the exact form
+        return accept_insert(own, prop, code, w1, lut, lane_off);     // R6, R7
+    }
     mask = accept_mask(code, w1, lut, lane_off);                      // R6
     return lop3<LOP_SEL>(prop, own, mask);                            // R7
 }

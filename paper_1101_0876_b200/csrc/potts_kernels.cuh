@@ -26,6 +26,9 @@ struct SweepParams {
     unsigned long long *E_out;  // MEASURE: -= satisfied bonds seen from this colour's sites; DELTA: += energy change
     unsigned long long *hist_out;  // HIST: += occupancies of this colour's sites after the update
     int32_t rpw;                // rows per warp (even, divides L / HS_WARPS)
+    int32_t row_groups;         // tiles per column block = L / (HS_WARPS * rpw)
+    uint32_t total_tiles;       // column blocks x row_groups
+    uint32_t *tile_counter;     // device word, 0 at launch and again after it: the blocks draw their tiles from it
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -38,7 +41,7 @@ struct SweepParams {
 //   * the column part of Philox (ColKeys: 3 of the 17 multiplies, 2 of the 18 XORs per site) is computed once
 //     per block for the tile's 2 x 512 columns (both row parities), kept in 16 KB of shared memory and read
 //     back with one conflict-free 16-byte load per site.
-// grid = (ceil(L/32 / 32), L / (HS_WARPS * rpw)).  Requires L % 32 == 0.
+// grid = as many blocks as are resident at once (or fewer tiles); tiles drawn dynamically.  Requires L % 32 == 0.
 // MEASURE: E -= satisfied bonds seen from this colour's sites (colour 1 of a sampled sweep).  HIST: occupancy of
 // the words just written.  DELTA (potts_sweep_delta: "a parallel accumulation of local energy
 // changes on-the-fly"): E_out += sum over accepted moves of d = n_old - n_new (R5, R7), no energy recount.
@@ -54,16 +57,35 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
     __shared__ AcceptLut lut;
     __shared__ int blockAcc;
     const uint32_t lane = threadIdx.x, wy = threadIdx.y, tid = wy * 32u + lane;
-    accept_lut_fill(&lut, P.thr, tid, 32 * HS_WARPS);
+    // plain half-sweeps at ordinary temperatures take the one-compare form of the acceptance (see accept_lut_fill)
+    const bool fast = !EX && accept_fast_ok(P.thr);
+    accept_lut_fill(&lut, P.thr, tid, 32 * HS_WARPS, fast);
     if (EX && tid == 0) blockAcc = 0;
     if (HIST)
         for (uint32_t n = tid; n < hist_words(P.q); n += 32 * HS_WARPS) s_dyn[n] = 0u;
 
     const int chunks = P.pitch >> 4;                                  // 16-byte chunks per row
-    const int x = (int)(blockIdx.x * 32u + lane);
+    const HalfSweepKeys &K = P.K;
+    const uint32_t lane_off = accept_lane_offset(lane);
+    const uint32_t q = in_register(P.q);
+    const int L = P.L, pitch = P.pitch;
+    int acc = 0, rows_done = 0;                                       // acc: MEASURE unequal neighbours of the final spins; DELTA energy change
+    // Tiles (column block cb, row group rg) are drawn from a global counter: tile = cb * row_groups + rg, so a block
+    // mostly stays in its column block and keeps its ColKeys.  atomicInc wraps to 0 after the last of the
+    // total_tiles + gridDim.x draws of a launch (every block draws exactly one tile number >= total_tiles and stops).
+    __shared__ uint32_t s_tile[2];
+    int cb_cur = -1;
+    for (uint32_t it = 0;; ++it) {
+    if (tid == 0) s_tile[it & 1u] = atomicInc(P.tile_counter, P.total_tiles + gridDim.x - 1u);
+    __syncthreads();                                                  // also: every thread is done with the previous tile
+    const uint32_t tile = s_tile[it & 1u];
+    if (tile >= P.total_tiles) break;
+    const int cb = (int)(tile / (uint32_t)P.row_groups), rg = (int)(tile - (uint32_t)cb * (uint32_t)P.row_groups);
+    const int x = cb * 32 + (int)lane;
     const bool active = x < chunks;
     const int k0 = x << 4;
-    const HalfSweepKeys &K = P.K;
+    if (cb != cb_cur) {
+    cb_cur = cb;
     if (active) {
         // site n of my chunk in a row of parity p sits at column j = 2 (k0 + n) + p
 #pragma unroll
@@ -77,13 +99,11 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
         }
     }
     __syncthreads();
+    }
 
-    int acc = 0;                                                      // MEASURE: unequal neighbours of the final spins; DELTA: energy change
     if (active) {
-        const uint32_t lane_off = accept_lane_offset(lane);
-        const uint32_t q = in_register(P.q);
-        const int L = P.L, pitch = P.pitch;
-        const int i0 = (int)(blockIdx.y * HS_WARPS + wy) * P.rpw;
+        rows_done += P.rpw;
+        const int i0 = (rg * HS_WARPS + (int)wy) * P.rpw;
         const int kn = wrap(k0 + 16, pitch), kp = wrap(k0 - 4, pitch);
         const uint8_t *const oth = P.plane_oth + k0;
         uint8_t *const ownp = P.plane_own + k0;
@@ -124,7 +144,8 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
                     }
                 }
                 uint32_t code, mask;
-                out[n] = metropolis_word<CM>(own[n], nb, q, w0, w1, &lut, lane_off, code, mask);
+                if (!EX && fast) out[n] = metropolis_word<CM, true>(own[n], nb, q, w0, w1, &lut, lane_off, code, mask);
+                else out[n] = metropolis_word<CM>(own[n], nb, q, w0, w1, &lut, lane_off, code, mask);
                 if (MEASURE) acc += ne_final_sum(code, mask);
                 if (DELTA) acc += delta_sum(code, mask);
                 if (HIST) hist_add_word(s_dyn, P.q, out[n], lane);
@@ -161,9 +182,10 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
             p ^= 1u;
         }
     }
+    }   // tiles
     if (EX) {
-        // MEASURE: satisfied bonds = 4 per site - unequal neighbours of the final spins = 64 rpw - acc
-        int v = DELTA ? acc : (active ? 64 * P.rpw - acc : 0);
+        // MEASURE: satisfied bonds = 4 per site - unequal neighbours of the final spins = 64 per row visit - acc
+        int v = DELTA ? acc : 64 * rows_done - acc;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
         if (lane == 0) atomicAdd(&blockAcc, v);

@@ -16,6 +16,8 @@
 // A thread handles 32 consecutive same-colour sites (16 bytes of nibbles + 4 bytes of high bits), so
 // the packed layout needs L % 64 == 0.
 #pragma once
+#include <type_traits>
+
 #include "potts_core.cuh"
 
 namespace potts {
@@ -70,111 +72,187 @@ struct PackedSweepParams {
     uint32_t thr[4];
     unsigned long long *E_out;
     unsigned long long *hist_out;
-    int32_t rpt;                 // rows per thread
+    int32_t rpw;                 // rows per warp (even, divides L / PK_WARPS)
+    int32_t row_groups;          // tiles per column block = L / (PK_WARPS * rpw)
+    uint32_t total_tiles;        // column blocks x row_groups
+    uint32_t *tile_counter;      // device word, 0 at launch and again after it (see k_sweep_rows_u8)
 };
 
 constexpr int PK_WARPS = 4;
+constexpr int PK_SITES = 32;     // same-colour sites per lane and row: 16 bytes of nibbles (+ 4 bytes of high bits)
 
-// Half-sweep, packed layout: a thread updates 32 consecutive same-colour sites of P.rpt consecutive rows.
-// grid = (ceil(L/64 / 32), L / (PK_WARPS * rpt)), block = (32, PK_WARPS).
-// DELTA (potts_sweep_delta; see k_half_sweep_delta_u8): instead of the energy, add the sum of the
-// accepted moves' d = n_old - n_new of this half-sweep to *P.E_out (two's-complement int64).
+// Half-sweep, packed layout, one launch per colour: k_sweep_rows_u8 (potts_kernels.cuh) on packed planes.  A block owns
+// 32 x 32 = 1024 same-colour sites (2048 lattice columns) x PK_WARPS * rpw rows; warp w walks DOWN its rpw rows, a lane
+// updates one 32-site chunk per row.  The other-colour rows i-1, i, i+1 roll through registers UNPACKED (and doubled
+// for the nibble compare), so a loaded word is unpacked once instead of once per use (three rows use it); the column
+// part of Philox (ColKeys) of the tile's 2 x 1024 columns is computed once per block into 32 KB of shared memory.
+// grid = as many blocks as are resident at once (or fewer tiles), block = (32, PK_WARPS); tiles drawn dynamically.
+// DELTA (potts_sweep_delta): instead of the energy, add the sum of the accepted moves'
+// d = n_old - n_new of this half-sweep to *P.E_out (two's-complement int64).
 template <bool FIVE, int ST, bool MEASURE, bool HIST, bool DELTA = false>
-__global__ void __launch_bounds__(32 * PK_WARPS) k_half_sweep_packed(const __grid_constant__ PackedSweepParams P)
+__global__ void __launch_bounds__(32 * PK_WARPS) k_sweep_rows_packed(const __grid_constant__ PackedSweepParams P)
 {
     constexpr bool EX = MEASURE || DELTA;
     constexpr int CM = FIVE ? CM_7BIT : CM_NIB4;
-    extern __shared__ uint32_t s_dyn[];
+    extern __shared__ __align__(16) uint8_t s_dyn_raw[];
+    uint4 (*s_col)[PK_SITES][32] = reinterpret_cast<uint4 (*)[PK_SITES][32]>(s_dyn_raw);          // [2][32][32]: 32 KB
+    uint32_t *s_hist = reinterpret_cast<uint32_t *>(s_dyn_raw + 2 * PK_SITES * 32 * sizeof(uint4));  // HIST table
     __shared__ AcceptLut lut;
     __shared__ int blockAcc;
-    const uint32_t tid = threadIdx.y * 32u + threadIdx.x;
-    accept_lut_fill(&lut, P.thr, tid, 32 * PK_WARPS);
+    const uint32_t lane = threadIdx.x, wy = threadIdx.y, tid = wy * 32u + lane;
+    const bool fast = !EX && accept_fast_ok(P.thr);                   // see k_sweep_rows_u8
+    accept_lut_fill(&lut, P.thr, tid, 32 * PK_WARPS, fast);
     if (EX && tid == 0) blockAcc = 0;
     if (HIST)
-        for (uint32_t n = tid; n < hist_words(P.q); n += 32 * PK_WARPS) s_dyn[n] = 0u;
-    __syncthreads();
+        for (uint32_t n = tid; n < hist_words(P.q); n += 32 * PK_WARPS) s_hist[n] = 0u;
 
     const PackedPlanes &S = P.S;
     const int chunks = S.L >> 6;                                       // 32-site chunks per plane row
-    const int x = (int)(blockIdx.x * 32u + threadIdx.x);
-    const int i0 = (int)(blockIdx.y * PK_WARPS + threadIdx.y) * P.rpt;
+    const HalfSweepKeys &K = P.K;
     const int c = (int)P.colour, o = 1 - c;
-    int acc = 0, rows_done = 0;
-    if (x < chunks) {
-        const uint32_t lane_off = accept_lane_offset(threadIdx.x);
-        const HalfSweepKeys &K = P.K;
-        const uint32_t q = in_register(P.q);
-        const int xn = x + 1 == chunks ? 0 : x + 1, xp = x == 0 ? chunks - 1 : x - 1;
-#pragma unroll 1
-        for (int r = 0; r < P.rpt; ++r) {
-            const int i = i0 + r;
-            const uint32_t p = (uint32_t)(i + c) & 1u;
-            const int iu = wrap(i - 1, S.L), id = wrap(i + 1, S.L);
-            const uint4 own_n = *reinterpret_cast<const uint4 *>(S.nib[c] + (size_t)i * S.pn + 16 * x);
-            const uint4 up_n = *reinterpret_cast<const uint4 *>(S.nib[o] + (size_t)iu * S.pn + 16 * x);
-            const uint4 dn_n = *reinterpret_cast<const uint4 *>(S.nib[o] + (size_t)id * S.pn + 16 * x);
-            uint32_t own_h = 0, up_h = 0, dn_h = 0;
-            if (FIVE) {
-                own_h = *reinterpret_cast<const uint32_t *>(S.hb[c] + (size_t)i * S.ph + 4 * x);
-                up_h = *reinterpret_cast<const uint32_t *>(S.hb[o] + (size_t)iu * S.ph + 4 * x);
-                dn_h = *reinterpret_cast<const uint32_t *>(S.hb[o] + (size_t)id * S.ph + 4 * x);
-            }
-            // other-colour sites of my row: mid[1..8] = my 32 columns, mid[0] / mid[9] = the word before / after
-            uint32_t mid[10];
-            load32<FIVE>(S, o, i, x, mid + 1);
-            {
-                // p = 1 needs site 32 (first site of the next chunk), p = 0 site -1 (last site of the previous one)
-                const int xa = p ? xn : xp;
-                const uint32_t an = *reinterpret_cast<const uint32_t *>(S.nib[o] + (size_t)i * S.pn + 16 * xa + (p ? 0 : 12));
-                const uint32_t ah = FIVE ? *reinterpret_cast<const uint32_t *>(S.hb[o] + (size_t)i * S.ph + 4 * xa) : 0u;
-                uint32_t lo, hi;
-                unpack_pair<FIVE>(an, ah, p ? 0 : 3, lo, hi);
-                mid[0] = hi;     // used when p = 0: sites -4..-1
-                mid[9] = lo;     // used when p = 1: sites 32..35
-            }
-            const RowKeys R = row_keys(K, (uint32_t)i);
-            const uint32_t own_w[4] = {own_n.x, own_n.y, own_n.z, own_n.w};
-            const uint32_t up_w[4] = {up_n.x, up_n.y, up_n.z, up_n.w};
-            const uint32_t dn_w[4] = {dn_n.x, dn_n.y, dn_n.z, dn_n.w};
-            uint32_t out_w[4], out_h = 0;
+    const uint32_t lane_off = accept_lane_offset(lane);
+    const uint32_t q = in_register(P.q);
+    const int L = S.L;
+    int acc = 0, rows_done = 0;                                       // acc: MEASURE unequal neighbours of the final spins; DELTA energy change
+    __shared__ uint32_t s_tile[2];                                    // dynamic tiles, as k_sweep_rows_u8
+    int cb_cur = -1;
+    for (uint32_t it = 0;; ++it) {
+    if (tid == 0) s_tile[it & 1u] = atomicInc(P.tile_counter, P.total_tiles + gridDim.x - 1u);
+    __syncthreads();
+    const uint32_t tile = s_tile[it & 1u];
+    if (tile >= P.total_tiles) break;
+    const int cb = (int)(tile / (uint32_t)P.row_groups), rg = (int)(tile - (uint32_t)cb * (uint32_t)P.row_groups);
+    const int x = cb * 32 + (int)lane;
+    const bool active = x < chunks;
+    if (cb != cb_cur) {
+    cb_cur = cb;
+    if (active) {
+        // site n of my chunk in a row of parity p sits at column j = 2 (32 x + n) + p
 #pragma unroll
-            for (int m = 0; m < 4; ++m) {
-                uint32_t own[2], up[2], dn[2], out[2];
-                unpack_pair<FIVE>(own_w[m], own_h, m, own[0], own[1]);
-                unpack_pair<FIVE>(up_w[m], up_h, m, up[0], up[1]);
-                unpack_pair<FIVE>(dn_w[m], dn_h, m, dn[0], dn[1]);
+        for (int nn = 0; nn < PK_SITES / PK_WARPS; ++nn) {
+            const int n = (int)wy * (PK_SITES / PK_WARPS) + nn;
 #pragma unroll
-                for (int hlf = 0; hlf < 2; ++hlf) {
-                    const int n = 2 * m + hlf;                        // byte-per-site word n: sites 4n..4n+3
-                    uint32_t lf, rt, w0[4], w1[4];
-                    horizontal(p, mid[n + 1], p ? mid[n + 2] : mid[n], lf, rt);
-                    draw_words<ST>(K, R, 2u * (uint32_t)(32 * x + 4 * n) + p, w0, w1);
-                    const uint32_t nb[4] = {prep_nbr<CM>(up[hlf]), prep_nbr<CM>(dn[hlf]), prep_nbr<CM>(lf), prep_nbr<CM>(rt)};
-                    uint32_t code, mask;
-                    out[hlf] = metropolis_word<CM>(own[hlf], nb, q, w0, w1, &lut, lane_off, code, mask);
-                    if (MEASURE) acc += ne_final_sum(code, mask);
-                    if (DELTA) acc += delta_sum(code, mask);
-                    if (HIST) hist_add_word(s_dyn, P.q, out[hlf], threadIdx.x);
-                }
-                out_w[m] = pack_pair<FIVE>(out[0], out[1], m, out_h);
+            for (int p = 0; p < 2; ++p) {
+                const ColKeys C = col_keys(K, 2u * (uint32_t)(32 * x + n) + (uint32_t)p);
+                s_col[p][n][lane] = make_uint4(C.l0, C.l1, C.ph, C.pl);
             }
-            *reinterpret_cast<uint4 *>(S.nib[c] + (size_t)i * S.pn + 16 * x) = make_uint4(out_w[0], out_w[1], out_w[2], out_w[3]);
-            if (FIVE) *reinterpret_cast<uint32_t *>(S.hb[c] + (size_t)i * S.ph + 4 * x) = out_h;
-            ++rows_done;
         }
     }
+    __syncthreads();
+    }
+
+    if (active) {
+        rows_done += P.rpw;
+        const int i0 = (rg * PK_WARPS + (int)wy) * P.rpw;
+        const int xn = x + 1 == chunks ? 0 : x + 1, xp = x == 0 ? chunks - 1 : x - 1;
+        struct Raw { uint4 nib; uint32_t hb; };
+        auto ld_row = [&](int pl, int i) {
+            Raw r;
+            r.nib = *reinterpret_cast<const uint4 *>(S.nib[pl] + (size_t)i * S.pn + 16 * x);
+            r.hb = FIVE ? *reinterpret_cast<const uint32_t *>(S.hb[pl] + (size_t)i * S.ph + 4 * x) : 0u;
+            return r;
+        };
+        // the word outside my chunk a row of parity p needs: sites 32..35 (p = 1) or -4..-1 (p = 0) of plane o
+        auto ld_adj = [&](int i, uint32_t p) {
+            Raw r;
+            const int xa = p ? xn : xp;
+            r.nib.x = *reinterpret_cast<const uint32_t *>(S.nib[o] + (size_t)i * S.pn + 16 * xa + (p ? 0 : 12));
+            r.hb = FIVE ? *reinterpret_cast<const uint32_t *>(S.hb[o] + (size_t)i * S.ph + 4 * xa) : 0u;
+            return r;
+        };
+        auto prep8 = [](const Raw &r, uint32_t (&w)[8]) {
+            unpack32<FIVE>(r.nib, r.hb, w);
+#pragma unroll
+            for (int n = 0; n < 8; ++n) w[n] = prep_nbr<CM>(w[n]);
+        };
+        auto prep_adj = [](const Raw &r, uint32_t p) {
+            uint32_t lo, hi;
+            unpack_pair<FIVE>(r.nib.x, r.hb, p ? 0 : 3, lo, hi);
+            return prep_nbr<CM>(p ? lo : hi);
+        };
+
+        auto visit = [&](auto par, int i, const Raw &own_raw, const uint32_t (&up)[8], const uint32_t (&mid)[8], uint32_t adjp,
+                         const uint32_t (&dn)[8]) {
+            constexpr int PAR = decltype(par)::value;
+            const RowKeysH R = row_keys_h(K, (uint32_t)i);
+            uint32_t own[8], out[8];
+            unpack32<FIVE>(own_raw.nib, own_raw.hb, own);
+#pragma unroll
+            for (int n = 0; n < 8; ++n) {
+                uint32_t nb[4];
+                nb[0] = up[n];
+                nb[1] = dn[n];
+                if (PAR) {      // horizontal neighbours at k and k+1
+                    nb[2] = mid[n];
+                    nb[3] = __funnelshift_r(mid[n], n < 7 ? mid[n < 7 ? n + 1 : 7] : adjp, 8);
+                } else {        // at k-1 and k
+                    nb[2] = __funnelshift_l(n > 0 ? mid[n > 0 ? n - 1 : 0] : adjp, mid[n], 8);
+                    nb[3] = mid[n];
+                }
+                uint32_t w0[4], w1[4];
+                if (ST == 1) {
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) {
+                        const uint4 ck = s_col[PAR][4 * n + b][lane];
+                        philox_site_h(K, R, ColKeys{ck.x, ck.y, ck.z, ck.w}, w0[b], w1[b]);
+                    }
+                } else {
+#pragma unroll
+                    for (int m = 0; m < 2; ++m) {
+                        const uint4 ck = s_col[PAR][4 * n + 2 * m][lane];
+                        uint32_t w[4];
+                        philox_pair_h(K, R, ColKeys{ck.x, ck.y, ck.z, ck.w}, w);
+                        w0[2 * m] = w[0]; w1[2 * m] = w[1]; w0[2 * m + 1] = w[2]; w1[2 * m + 1] = w[3];
+                    }
+                }
+                uint32_t code, mask;
+                if (!EX && fast) out[n] = metropolis_word<CM, true>(own[n], nb, q, w0, w1, &lut, lane_off, code, mask);
+                else out[n] = metropolis_word<CM>(own[n], nb, q, w0, w1, &lut, lane_off, code, mask);
+                if (MEASURE) acc += ne_final_sum(code, mask);
+                if (DELTA) acc += delta_sum(code, mask);
+                if (HIST) hist_add_word(s_hist, P.q, out[n], lane);
+            }
+            uint32_t out_h = 0, out_w[4];
+#pragma unroll
+            for (int m = 0; m < 4; ++m) out_w[m] = pack_pair<FIVE>(out[2 * m], out[2 * m + 1], m, out_h);
+            *reinterpret_cast<uint4 *>(S.nib[c] + (size_t)i * S.pn + 16 * x) = make_uint4(out_w[0], out_w[1], out_w[2], out_w[3]);
+            if (FIVE) *reinterpret_cast<uint32_t *>(S.hb[c] + (size_t)i * S.ph + 4 * x) = out_h;
+        };
+
+        uint32_t up[8], mid[8], dn[8];
+        prep8(ld_row(o, wrap(i0 - 1, L)), up);
+        prep8(ld_row(o, i0), mid);
+        uint32_t p = (uint32_t)(i0 + c) & 1u;
+        Raw own_raw = ld_row(c, i0), dn_raw = ld_row(o, wrap(i0 + 1, L)), adj_raw = ld_adj(i0, p);
+#pragma unroll 1
+        for (int r = 0; r < P.rpw; ++r) {
+            const int i = i0 + r;
+            // next row's loads first: they have the whole visit to arrive (the last visit reloads its own row)
+            const int inx = r + 1 < P.rpw ? i + 1 : i;
+            const Raw own_nx = ld_row(c, inx), dn_nx = ld_row(o, wrap(inx + 1, L)), adj_nx = ld_adj(inx, p ^ 1u);
+            prep8(dn_raw, dn);
+            const uint32_t adjp = prep_adj(adj_raw, p);
+            if (p) visit(std::integral_constant<int, 1>{}, i, own_raw, up, mid, adjp, dn);
+            else visit(std::integral_constant<int, 0>{}, i, own_raw, up, mid, adjp, dn);
+#pragma unroll
+            for (int n = 0; n < 8; ++n) { up[n] = mid[n]; mid[n] = dn[n]; }
+            own_raw = own_nx; dn_raw = dn_nx; adj_raw = adj_nx;
+            p ^= 1u;
+        }
+    }
+    }   // tiles
     if (EX) {
-        // MEASURE: satisfied bonds = 4 per site - unequal neighbours of the final spins; DELTA: the change
+        // MEASURE: satisfied bonds = 4 per site - unequal neighbours of the final spins = 128 per row visit - acc; DELTA: the change
         int v = DELTA ? acc : 128 * rows_done - acc;
 #pragma unroll
         for (int s = 16; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
-        if (threadIdx.x == 0) atomicAdd(&blockAcc, v);
+        if (lane == 0) atomicAdd(&blockAcc, v);
         __syncthreads();
         if (tid == 0) atomicAdd(P.E_out, DELTA ? (unsigned long long)(long long)blockAcc : 0ull - (unsigned long long)(long long)blockAcc);
     }
     if (HIST) {
         __syncthreads();
-        hist_flush(s_dyn, P.q, P.hist_out, tid, 32 * PK_WARPS);
+        hist_flush(s_hist, P.q, P.hist_out, tid, 32 * PK_WARPS);
     }
 }
 
