@@ -1,0 +1,4 @@
+// k_stream_s1c1.cu -- streaming half-sweep kernel (U8), stream definition 1, colour 1; see k_stream.inl
+#define POTTS_ST 1
+#define POTTS_COLOUR 1
+#include "k_stream.inl"

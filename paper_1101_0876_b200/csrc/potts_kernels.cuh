@@ -48,18 +48,21 @@ struct SweepParams {
 constexpr int HS_WARPS = 4;
 constexpr int HS_SITES = 16;          // same-colour sites per lane and row
 
-template <int CM, int ST, bool MEASURE, bool HIST, bool DELTA>
+// COLOUR = P.colour as a template argument: with it the row parity of every visit is a literal, the row loop
+// handles two rows per trip and the next row's loads alternate between two register sets instead of being copied.
+// FAST: the one-compare form of the acceptance (accept_lut_fill); the host selects it for launches without the
+// energy / energy-change sums when no threshold is zero.
+template <int CM, int ST, int COLOUR, bool MEASURE, bool HIST, bool DELTA, bool FAST>
 __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_constant__ SweepParams P)
 {
     constexpr bool EX = MEASURE || DELTA;
+    static_assert(!(FAST && EX), "the sums need the exact form of the acceptance");
     extern __shared__ uint32_t s_dyn[];                       // HIST: the block's histogram table
     __shared__ uint4 s_col[2][HS_SITES][32];                  // ColKeys of [row parity p][site of the chunk][lane]
     __shared__ AcceptLut lut;
     __shared__ int blockAcc;
     const uint32_t lane = threadIdx.x, wy = threadIdx.y, tid = wy * 32u + lane;
-    // plain half-sweeps at ordinary temperatures take the one-compare form of the acceptance (see accept_lut_fill)
-    const bool fast = !EX && accept_fast_ok(P.thr);
-    accept_lut_fill(&lut, P.thr, tid, 32 * HS_WARPS, fast);
+    accept_lut_fill(&lut, P.thr, tid, 32 * HS_WARPS, FAST);
     if (EX && tid == 0) blockAcc = 0;
     if (HIST)
         for (uint32_t n = tid; n < hist_words(P.q); n += 32 * HS_WARPS) s_dyn[n] = 0u;
@@ -144,8 +147,7 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
                     }
                 }
                 uint32_t code, mask;
-                if (!EX && fast) out[n] = metropolis_word<CM, true>(own[n], nb, q, w0, w1, &lut, lane_off, code, mask);
-                else out[n] = metropolis_word<CM>(own[n], nb, q, w0, w1, &lut, lane_off, code, mask);
+                out[n] = metropolis_word<CM, FAST>(own[n], nb, q, w0, w1, &lut, lane_off, code, mask);
                 if (MEASURE) acc += ne_final_sum(code, mask);
                 if (DELTA) acc += delta_sum(code, mask);
                 if (HIST) hist_add_word(s_dyn, P.q, out[n], lane);
@@ -157,29 +159,33 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
             w[0] = prep_nbr<CM>(v.x); w[1] = prep_nbr<CM>(v.y); w[2] = prep_nbr<CM>(v.z); w[3] = prep_nbr<CM>(v.w);
         };
 
-        uint32_t up[4], mid[4], dn[4];
+        // rows i0 (parity COLOUR: i0 is even), i0 + 1 (the other parity), ...: two visits per trip.  Register sets a / b
+        // hold the loads of the even / odd visit; each visit first issues the loads of the NEXT row into the other
+        // set, so they have a whole visit to arrive (the tile's last visit reloads its own row, unused).
+        uint32_t up[4], mid[4], dn[4], dn2[4];
         prep4(ld16(oth + (size_t)wrap(i0 - 1, L) * pitch), up);
         prep4(ld16(oth + (size_t)i0 * pitch), mid);
-        uint32_t p = (uint32_t)(i0 + P.colour) & 1u;
-        uint4 own4 = ld16(ownp + (size_t)i0 * pitch);
-        uint4 dn4 = ld16(oth + (size_t)wrap(i0 + 1, L) * pitch);
-        uint32_t adj = *reinterpret_cast<const uint32_t *>(P.plane_oth + (size_t)i0 * pitch + (p ? kn : kp));
+        constexpr int PA = COLOUR, PB = 1 - COLOUR;
+        const int k_a = PA ? kn : kp, k_b = PB ? kn : kp;             // column of the word outside the chunk
+        uint4 own_a = ld16(ownp + (size_t)i0 * pitch);
+        uint4 dn_a = ld16(oth + (size_t)wrap(i0 + 1, L) * pitch);
+        uint32_t adj_a = *reinterpret_cast<const uint32_t *>(P.plane_oth + (size_t)i0 * pitch + k_a);
 #pragma unroll 1
-        for (int r = 0; r < P.rpw; ++r) {
+        for (int r = 0; r < P.rpw; r += 2) {
             const int i = i0 + r;
-            // next row's loads first: they have the whole visit to arrive (the last visit reloads its own row)
-            const int inx = r + 1 < P.rpw ? i + 1 : i;
-            const uint4 own_nx = ld16(ownp + (size_t)inx * pitch);
-            const uint4 dn_nx = ld16(oth + (size_t)wrap(inx + 1, L) * pitch);
-            const uint32_t adj_nx = *reinterpret_cast<const uint32_t *>(P.plane_oth + (size_t)inx * pitch + (p ? kp : kn));
-            prep4(dn4, dn);
-            const uint32_t adjp = prep_nbr<CM>(adj);
-            if (p) visit(std::integral_constant<int, 1>{}, i, own4, up, mid, adjp, dn);
-            else visit(std::integral_constant<int, 0>{}, i, own4, up, mid, adjp, dn);
+            const uint4 own_b = ld16(ownp + (size_t)(i + 1) * pitch);
+            const uint4 dn_b = ld16(oth + (size_t)wrap(i + 2, L) * pitch);
+            const uint32_t adj_b = *reinterpret_cast<const uint32_t *>(P.plane_oth + (size_t)(i + 1) * pitch + k_b);
+            prep4(dn_a, dn);
+            visit(std::integral_constant<int, PA>{}, i, own_a, up, mid, prep_nbr<CM>(adj_a), dn);
+            const int inx = r + 2 < P.rpw ? i + 2 : i + 1;
+            own_a = ld16(ownp + (size_t)inx * pitch);
+            dn_a = ld16(oth + (size_t)wrap(inx + 1, L) * pitch);
+            adj_a = *reinterpret_cast<const uint32_t *>(P.plane_oth + (size_t)inx * pitch + k_a);
+            prep4(dn_b, dn2);
+            visit(std::integral_constant<int, PB>{}, i + 1, own_b, mid, dn, prep_nbr<CM>(adj_b), dn2);
 #pragma unroll
-            for (int n = 0; n < 4; ++n) { up[n] = mid[n]; mid[n] = dn[n]; }
-            own4 = own_nx; dn4 = dn_nx; adj = adj_nx;
-            p ^= 1u;
+            for (int n = 0; n < 4; ++n) { up[n] = dn[n]; mid[n] = dn2[n]; }
         }
     }
     }   // tiles

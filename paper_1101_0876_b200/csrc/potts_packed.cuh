@@ -89,10 +89,11 @@ constexpr int PK_SITES = 32;     // same-colour sites per lane and row: 16 bytes
 // grid = as many blocks as are resident at once (or fewer tiles), block = (32, PK_WARPS); tiles drawn dynamically.
 // DELTA (potts_sweep_delta): instead of the energy, add the sum of the accepted moves'
 // d = n_old - n_new of this half-sweep to *P.E_out (two's-complement int64).
-template <bool FIVE, int ST, bool MEASURE, bool HIST, bool DELTA = false>
+template <bool FIVE, int ST, int COLOUR, bool MEASURE, bool HIST, bool DELTA, bool FAST>
 __global__ void __launch_bounds__(32 * PK_WARPS) k_sweep_rows_packed(const __grid_constant__ PackedSweepParams P)
 {
     constexpr bool EX = MEASURE || DELTA;
+    static_assert(!(FAST && EX), "the sums need the exact form of the acceptance");
     constexpr int CM = FIVE ? CM_7BIT : CM_NIB4;
     extern __shared__ __align__(16) uint8_t s_dyn_raw[];
     uint4 (*s_col)[PK_SITES][32] = reinterpret_cast<uint4 (*)[PK_SITES][32]>(s_dyn_raw);          // [2][32][32]: 32 KB
@@ -100,8 +101,7 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_sweep_rows_packed(const __gri
     __shared__ AcceptLut lut;
     __shared__ int blockAcc;
     const uint32_t lane = threadIdx.x, wy = threadIdx.y, tid = wy * 32u + lane;
-    const bool fast = !EX && accept_fast_ok(P.thr);                   // see k_sweep_rows_u8
-    accept_lut_fill(&lut, P.thr, tid, 32 * PK_WARPS, fast);
+    accept_lut_fill(&lut, P.thr, tid, 32 * PK_WARPS, FAST);
     if (EX && tid == 0) blockAcc = 0;
     if (HIST)
         for (uint32_t n = tid; n < hist_words(P.q); n += 32 * PK_WARPS) s_hist[n] = 0u;
@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_sweep_rows_packed(const __gri
     const PackedPlanes &S = P.S;
     const int chunks = S.L >> 6;                                       // 32-site chunks per plane row
     const HalfSweepKeys &K = P.K;
-    const int c = (int)P.colour, o = 1 - c;
+    constexpr int c = COLOUR, o = 1 - COLOUR;
     const uint32_t lane_off = accept_lane_offset(lane);
     const uint32_t q = in_register(P.q);
     const int L = S.L;
@@ -206,8 +206,7 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_sweep_rows_packed(const __gri
                     }
                 }
                 uint32_t code, mask;
-                if (!EX && fast) out[n] = metropolis_word<CM, true>(own[n], nb, q, w0, w1, &lut, lane_off, code, mask);
-                else out[n] = metropolis_word<CM>(own[n], nb, q, w0, w1, &lut, lane_off, code, mask);
+                out[n] = metropolis_word<CM, FAST>(own[n], nb, q, w0, w1, &lut, lane_off, code, mask);
                 if (MEASURE) acc += ne_final_sum(code, mask);
                 if (DELTA) acc += delta_sum(code, mask);
                 if (HIST) hist_add_word(s_hist, P.q, out[n], lane);
@@ -219,25 +218,24 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_sweep_rows_packed(const __gri
             if (FIVE) *reinterpret_cast<uint32_t *>(S.hb[c] + (size_t)i * S.ph + 4 * x) = out_h;
         };
 
-        uint32_t up[8], mid[8], dn[8];
+        // two visits per trip, loads alternating between register sets a / b (see k_sweep_rows_u8)
+        uint32_t up[8], mid[8], dn[8], dn2[8];
         prep8(ld_row(o, wrap(i0 - 1, L)), up);
         prep8(ld_row(o, i0), mid);
-        uint32_t p = (uint32_t)(i0 + c) & 1u;
-        Raw own_raw = ld_row(c, i0), dn_raw = ld_row(o, wrap(i0 + 1, L)), adj_raw = ld_adj(i0, p);
+        constexpr uint32_t PA = COLOUR, PB = 1 - COLOUR;             // i0 is even
+        Raw own_a = ld_row(c, i0), dn_a = ld_row(o, wrap(i0 + 1, L)), adj_a = ld_adj(i0, PA);
 #pragma unroll 1
-        for (int r = 0; r < P.rpw; ++r) {
+        for (int r = 0; r < P.rpw; r += 2) {
             const int i = i0 + r;
-            // next row's loads first: they have the whole visit to arrive (the last visit reloads its own row)
-            const int inx = r + 1 < P.rpw ? i + 1 : i;
-            const Raw own_nx = ld_row(c, inx), dn_nx = ld_row(o, wrap(inx + 1, L)), adj_nx = ld_adj(inx, p ^ 1u);
-            prep8(dn_raw, dn);
-            const uint32_t adjp = prep_adj(adj_raw, p);
-            if (p) visit(std::integral_constant<int, 1>{}, i, own_raw, up, mid, adjp, dn);
-            else visit(std::integral_constant<int, 0>{}, i, own_raw, up, mid, adjp, dn);
+            const Raw own_b = ld_row(c, i + 1), dn_b = ld_row(o, wrap(i + 2, L)), adj_b = ld_adj(i + 1, PB);
+            prep8(dn_a, dn);
+            visit(std::integral_constant<int, (int)PA>{}, i, own_a, up, mid, prep_adj(adj_a, PA), dn);
+            const int inx = r + 2 < P.rpw ? i + 2 : i + 1;
+            own_a = ld_row(c, inx); dn_a = ld_row(o, wrap(inx + 1, L)); adj_a = ld_adj(inx, PA);
+            prep8(dn_b, dn2);
+            visit(std::integral_constant<int, (int)PB>{}, i + 1, own_b, mid, dn, prep_adj(adj_b, PB), dn2);
 #pragma unroll
-            for (int n = 0; n < 8; ++n) { up[n] = mid[n]; mid[n] = dn[n]; }
-            own_raw = own_nx; dn_raw = dn_nx; adj_raw = adj_nx;
-            p ^= 1u;
+            for (int n = 0; n < 8; ++n) { up[n] = dn[n]; mid[n] = dn2[n]; }
         }
     }
     }   // tiles
