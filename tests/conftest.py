@@ -15,6 +15,16 @@ GOLDEN = os.path.join(HERE, "golden")
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run with -m gpu on the B200 box)")
+    config.addinivalue_line("markers", "slow: hours of oracle time; runs only with POTTS_RUN_SLOW=1")
+
+
+def pytest_collection_modifyitems(config, items):
+    if os.environ.get("POTTS_RUN_SLOW") == "1":
+        return
+    skip = pytest.mark.skip(reason="full-length run: set POTTS_RUN_SLOW=1")
+    for item in items:
+        if "slow" in item.keywords:
+            item.add_marker(skip)
 
 
 @pytest.fixture(scope="session")

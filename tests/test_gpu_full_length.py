@@ -1,13 +1,15 @@
-"""Full-length parity of a BASELINE.json configuration: every sweep of the run, GPU against the oracle.
+"""Full-length parity of the BASELINE.json configurations: every sweep of the run, GPU against the oracle (-m gpu).
 
-Not collected by pytest (hours of CPU for the large lattices): run by hand on a GPU box,
+Marked `slow` (hours of oracle time for the large lattices): collected, but skipped unless POTTS_RUN_SLOW=1, e.g.
 
-    python tests/full_length_parity.py cfgN [max_sweeps]
+    POTTS_RUN_SLOW=1 python -m pytest tests/test_gpu_full_length.py -m gpu -q -k cfg2
+    POTTS_FULL_LENGTH_LIMIT=100 POTTS_RUN_SLOW=1 python -m pytest tests/test_gpu_full_length.py -m gpu -q -k cfg5
 
 Both sides run the configuration's temperature ladder from its start state in chunks of `chunk` sweeps; after every
 chunk the energy (and histogram) series of the chunk are compared entry by entry, and every `spin_every` chunks the whole
 spin configuration.  The oracle runs in its row-parallel mode (same bits as serial, tests/test_oracle_pins.py).
-Prints one summary line; the record of round 1 is profiles/r01d_full_length_parity.md.
+POTTS_FULL_LENGTH_LIMIT bounds the number of sweeps.  Records: profiles/r01d_full_length_parity.md (round 1),
+profiles/r02d_full_length_parity.md (round 2).
 """
 import os
 import sys
@@ -16,16 +18,19 @@ import time
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 sys.path.insert(0, ROOT)
 
-import numpy as np  # noqa: E402
+import numpy as np  # noqa: E402,F401
+import pytest  # noqa: E402
 
 import oracle  # noqa: E402
 import workloads  # noqa: E402
 
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
 
-def main():
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5], ids=lambda k: f"cfg{k}")
+def test_full_length_parity(k):
     import paper_1101_0876_b200 as pb
-    k = int(sys.argv[1].replace("cfg", ""))
-    limit = int(sys.argv[2]) if len(sys.argv) > 2 else None
+    limit = int(os.environ["POTTS_FULL_LENGTH_LIMIT"]) if os.environ.get("POTTS_FULL_LENGTH_LIMIT") else None
     w = workloads.CONFIGS[k]
     threads = len(os.sched_getaffinity(0))
     g = pb.Potts(w.L, w.q, w.seed, w.init, layout=pb.LAYOUT_PACKED if w.packed else pb.LAYOUT_U8)
@@ -57,6 +62,3 @@ def main():
           f"and {spin_checks} full configurations identical, kernel variant resident_ctas={g.potts_get_option('resident_active')}, "
           f"oracle threads={threads}, {time.time() - t0:.0f} s", flush=True)
 
-
-if __name__ == "__main__":
-    main()

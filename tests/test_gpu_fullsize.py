@@ -111,6 +111,16 @@ def test_cfg5_full_size_streaming(pb):
     _check_sampled_sites(w, T, t, S0, S1)
     assert int(H1[0].sum()) == w.L * w.L and -2 * w.L * w.L <= int(E1[0]) < 0
     assert int(E1[0]) == g.potts_energy() and (H1[0] == g.potts_histogram()).all()   # fused == standalone reduction
+    # mid-run restart: the oracle takes over the GPU's state at t = 13 (state = spins + t, the RNG is stateless) and
+    # both run the next two sweeps of the workload's cadence in full; every spin, the energy and the histogram agree
+    t1 = g.potts_sweep_count()
+    o.set_state(S1, t1)
+    del S0
+    E2, H2 = g.potts_sweep_measured(T, 2, 2, hist=True)
+    o.sweep(T, 2)
+    assert int(E2[0]) == o.energy() == o.energy_incremental()
+    assert (H2[0] == o.histogram()).all()
+    assert (g.potts_download(S1) == o.spins()).all()
 
 
 @pytest.mark.parametrize("q,want_eo,want_ed", [(9, -1.633167, -1.033499), (15, -1.765905, -0.750492)])

@@ -381,3 +381,25 @@ def test_every_beyond_2_30_is_rejected(pb):
         g.potts_sweep_measured(1.0, 2 ** 31, 2 ** 31, hist=False)
     assert e.value.code == pb.ERR_ARG
     assert g.potts_sweep_count() == 0
+
+
+def test_persistent_kernels_are_deterministic_under_repetition(pb):
+    """compute-sanitizer is closed on this pool (profiles/r02c_sanitizer.md), so the hand-rolled inter-CTA packet
+    protocol and the DSMEM exchange are exercised instead: the same run repeated on many grid shapes must give the
+    same bits every time (a race shows up as run-to-run differences), and those bits are the oracle's."""
+    L, q, seed, n = 256, 9, 4, 60
+    T = 0.99 * workloads.t_c(q)
+    o = oracle.OraclePotts(L, q, seed, workloads.INIT_RANDOM, threads=4)
+    Eo, Ho = o.sweep_measured(T, n, 1, hist=True)
+    want = o.spins()
+    shapes = [{"variant": 2, "resident_ctas": c} for c in (2, 5, 16, 37, 64, 148)] + \
+             [{"variant": 2, "resident_ctas": 148, "resident_words": 2}, {"variant": 3, "cluster_ctas": 16}, {"variant": 3, "cluster_ctas": 8}]
+    for shape in shapes:
+        for rep in range(4):
+            g = pb.Potts(L, q, seed, workloads.INIT_RANDOM)
+            for k, v in shape.items():
+                g.potts_set_option(k, v)
+            Eg, Hg = g.potts_sweep_measured(T, n, 1, hist=True)
+            assert (Eg == Eo).all() and (Hg == Ho).all(), (shape, rep)
+            assert (g.potts_download() == want).all(), (shape, rep)
+            g.close()
