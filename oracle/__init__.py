@@ -20,6 +20,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "potts_oracle.c")
+_SRC3 = os.path.join(_HERE, "potts3d_oracle.c")       # the 3D generalisation, same library
 _LIB = os.path.join(_HERE, "libpotts_oracle.so")
 _lock = threading.Lock()
 _lib = None
@@ -31,11 +32,11 @@ INIT_RANDOM = 1
 def build(force: bool = False) -> str:
     """Compile potts_oracle.c -> libpotts_oracle.so (plain -O2, OpenMP for the optional row-parallel mode)."""
     with _lock:
-        if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC3)):
             tmp = _LIB + f".tmp{os.getpid()}"
             subprocess.check_call(
                 ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
-                 "-o", tmp, _SRC, "-lm"])
+                 "-o", tmp, _SRC, _SRC3, "-lm"])
             os.replace(tmp, _LIB)
     return _LIB
 
@@ -83,6 +84,30 @@ def _load():
         lib.oracle_update_site_s.restype = ctypes.c_uint8
         lib.oracle_set_stream.argtypes = [vp, ctypes.c_int]
         lib.oracle_set_stream.restype = ctypes.c_int
+        lib.oracle3_thresholds.argtypes = [ctypes.c_double, u32p]
+        lib.oracle3_thresholds.restype = None
+        lib.oracle3_create.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_uint64, ctypes.c_int32]
+        lib.oracle3_create.restype = vp
+        lib.oracle3_destroy.argtypes = [vp]
+        lib.oracle3_destroy.restype = None
+        lib.oracle3_set_threads.argtypes = [vp, ctypes.c_int]
+        lib.oracle3_set_threads.restype = None
+        lib.oracle3_sweep.argtypes = [vp, ctypes.c_double, ctypes.c_int64]
+        lib.oracle3_sweep.restype = ctypes.c_int
+        lib.oracle3_sweep_measured.argtypes = [vp, ctypes.c_double, ctypes.c_int64, ctypes.c_int64, i64p, i64p]
+        lib.oracle3_sweep_measured.restype = ctypes.c_int
+        lib.oracle3_energy.argtypes = [vp]
+        lib.oracle3_energy.restype = ctypes.c_int64
+        lib.oracle3_energy_incremental.argtypes = [vp]
+        lib.oracle3_energy_incremental.restype = ctypes.c_int64
+        lib.oracle3_histogram.argtypes = [vp, i64p]
+        lib.oracle3_histogram.restype = None
+        lib.oracle3_spins.argtypes = [vp]
+        lib.oracle3_spins.restype = u8p
+        lib.oracle3_sweep_count.argtypes = [vp]
+        lib.oracle3_sweep_count.restype = ctypes.c_uint64
+        lib.oracle3_set_state.argtypes = [vp, u8p, ctypes.c_uint64]
+        lib.oracle3_set_state.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -190,3 +215,74 @@ class OraclePotts:
         rc = self._lib.oracle_set_state(self._h, a.ctypes.data_as(ctypes.POINTER(ctypes.c_uint8)), int(t))
         if rc:
             raise ValueError("oracle_set_state rejected the configuration")
+
+
+def thresholds3(T: float):
+    """[thr(1) .. thr(6)] = floor(2^32 exp(-d/T)) for the 3D lattice (R6')."""
+    lib = _load()
+    o = (ctypes.c_uint32 * 7)()
+    lib.oracle3_thresholds(float(T), o)
+    return [int(o[d]) for d in range(1, 7)]
+
+
+class OraclePotts3D:
+    """The 3D (simple-cubic, 6 neighbours) checkerboard chain of potts3d_oracle.c; spins()[z, y, x]."""
+
+    def __init__(self, L: int, q: int, seed: int, init: int, threads: int = 1):
+        self._lib = _load()
+        self.L, self.q, self.seed = int(L), int(q), int(seed)
+        self._h = self._lib.oracle3_create(self.L, self.q, self.seed, int(init))
+        if not self._h:
+            raise ValueError(f"bad arguments L={L} q={q} init={init}")
+        self._lib.oracle3_set_threads(self._h, int(threads))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.oracle3_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def t(self) -> int:
+        return int(self._lib.oracle3_sweep_count(self._h))
+
+    def sweep(self, T: float, nsweeps: int):
+        if self._lib.oracle3_sweep(self._h, float(T), int(nsweeps)):
+            raise ValueError("bad arguments to sweep")
+
+    def sweep_measured(self, T: float, nsweeps: int, every: int = 1, hist: bool = True):
+        ns = int(nsweeps) // int(every)
+        E = np.zeros(ns, dtype=np.int64)
+        H = np.zeros((ns, self.q), dtype=np.int64) if hist else None
+        i64p = ctypes.POINTER(ctypes.c_int64)
+        rc = self._lib.oracle3_sweep_measured(self._h, float(T), int(nsweeps), int(every), E.ctypes.data_as(i64p),
+                                              H.ctypes.data_as(i64p) if hist else None)
+        if rc:
+            raise ValueError("bad arguments to sweep_measured")
+        return E, H
+
+    def energy(self) -> int:
+        return int(self._lib.oracle3_energy(self._h))
+
+    def energy_incremental(self) -> int:
+        return int(self._lib.oracle3_energy_incremental(self._h))
+
+    def histogram(self) -> np.ndarray:
+        out = np.zeros(self.q, dtype=np.int64)
+        self._lib.oracle3_histogram(self._h, out.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)))
+        return out
+
+    def spins(self) -> np.ndarray:
+        p = self._lib.oracle3_spins(self._h)
+        return np.ctypeslib.as_array(p, shape=(self.L, self.L, self.L)).copy()
+
+    def set_state(self, spins: np.ndarray, t: int):
+        a = np.ascontiguousarray(spins, dtype=np.uint8)
+        assert a.shape == (self.L, self.L, self.L)
+        if self._lib.oracle3_set_state(self._h, a.ctypes.data_as(ctypes.POINTER(ctypes.c_uint8)), int(t)):
+            raise ValueError("spin value >= q")
