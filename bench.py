@@ -44,6 +44,7 @@ I_ALG_PER_UPDATE = 36                 # Philox4x32-10 words 0,1 of counter (j,i,
 # Measured on B200 (profiles/r01b_pipe_model.md): for this integer mix (IMAD.WIDE / LOP3 / IADD3 / SHF / PRMT) an SM
 # sub-partition retires one warp instruction every 2 clocks, whichever pipe it goes to: half the nominal issue rate.
 MEASURED_INT_ISSUE_PER_CLK = 0.5
+BYTES_PER_UPDATE_U8 = 3.0             # read own + read other (once) + write own, uint8 planes
 HEADLINE = 5                          # BASELINE.json configs[4]: the largest single-GPU configuration
 
 
@@ -428,6 +429,33 @@ def stream_spec_2_table(pb, torch, flush, peaks):
     return out
 
 
+def cubic_lattice(pb, torch, peaks, L=512, q=9, sweeps=40, repeats=3):
+    """SURVEY 8(f)4 / PAPER.md:359: the 3D generalisation (potts3_sweep, k_sweep3_u8: one launch per half-sweep, first
+    CUDA path of this row) on an L^3 lattice, random start, T = 1.3 (ordering phase); CUDA events around calls of
+    `sweeps` sweeps after a warm-up call, median.  Same algorithmic counts as the 2D path: 36 instructions and 3 bytes
+    per update."""
+    hbm_gbs, sm_max, which = peaks
+    T = 1.3
+    g = pb.Potts3D(L, q, 5, pb.INIT_RANDOM)
+    g.potts3_sweep(T, 5)
+    ms = []
+    for _ in range(repeats):
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        g.potts3_sweep(T, sweeps)
+        e1.record()
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    g.close()
+    sec = statistics.median(ms) * 1e-3
+    w = type("W", (), {"name": f"potts3d_q{q}_L{L}"})
+    r = roofline(w, "k_sweep3_u8", L ** 3 / 2, sec * 1e3 / (2 * sweeps), sm_max, hbm_gbs, which, BYTES_PER_UPDATE_U8)
+    ups = sweeps * L ** 3 / sec
+    return {"q": q, "L": L, "sites": L ** 3, "sweeps_per_call": sweeps, "calls": repeats, "T": T, "ns_per_spin_flip": 1e9 / ups,
+            "spin_updates_per_s": ups, "ms_per_call_min_max": [min(ms), max(ms)], "kernel": "k_sweep3_u8", "roofline": r}
+
+
 def paper_protocol_e6(pb, torch):
     """The paper's end-to-end example: q=9, L=1024, 3 samples, T = 0.71 .. 0.73 in steps of 0.002,
     t_tran = 2000, t_max = 8000, one measure every 50 sweeps; 193 s on a GTX 280, 8115 s on its CPU.  Here: the same
@@ -589,6 +617,7 @@ def main():
         per_cfg["delta_cfg2_resident"] = delta_cost(pb, torch, 2, 2000)
         per_cfg["delta_cfg1_cluster"] = delta_cost(pb, torch, 1, 2000)
         per_cfg["stream_spec_2"] = stream_spec_2_table(pb, torch, flush, peaks)
+        per_cfg["potts3d_q9_L512"] = cubic_lattice(pb, torch, peaks)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(w)
     if dist is not None:

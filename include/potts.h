@@ -224,6 +224,30 @@ const char *potts_last_error(void);
 /* Library version string, e.g. "potts-b200 0.1 (sm_100a)". */
 const char *potts_version(void);
 
+/* ---- 3D generalisation (sec. 7: "For the generalization to the 3D case, the checkerboard scheme defining
+ * two independent sub-networks persists, however the cell-packing scheme should be updated") -----------------------
+ * The same Metropolis chain on an L x L x L periodic simple-cubic lattice with 6 nearest neighbours (DESIGN.md reading
+ * S16): E = -sum over sites of [delta(s, s_{x+1}) + delta(s, s_{y+1}) + delta(s, s_{z+1})] in [-3 L^3, 0]; sweep = all
+ * sites with (x+y+z) even, then all with (x+y+z) odd; random words Philox4x32-10(counter = (x, y, t, colour + 4 z),
+ * key = seed); proposal floor(w0 q / 2^32); accept iff d <= 0 or w1 < floor(2^32 exp(-d/T)), d = n_old - n_new in
+ * -6..6; random start from counter (x, y, 0, 2 + 4 z).  Spins cross the boundary as s[(z L + y) L + x] (host, L^3
+ * bytes).  L even, L % 32 == 0 (POTTS_ERR_UNSUPPORTED otherwise), L <= 2048; U8 layout only.  cuda_stream: the stream
+ * every call of the handle uses (null = default stream).  Conventions as for potts_t: return codes, potts_last_error(),
+ * out-parameters untouched on error, potts3_sweep may return before the GPU finishes, the others synchronise.
+ * E_series / hist_series of potts3_sweep_measured: host, nsweeps/every entries (x q), either may be null. */
+typedef struct potts3_s potts3_t;
+int  potts3_create(potts3_t **out, int32_t L, int32_t q, uint64_t seed, int32_t init, void *cuda_stream);
+void potts3_destroy(potts3_t *h);
+int  potts3_sweep(potts3_t *h, double T, int64_t nsweeps);
+int  potts3_sweep_measured(potts3_t *h, double T, int64_t nsweeps, int64_t every, int64_t *E_series, int64_t *hist_series);
+int  potts3_energy(potts3_t *h, int64_t *E);
+int  potts3_histogram(potts3_t *h, int64_t *counts);
+int  potts3_download(potts3_t *h, uint8_t *spins);
+int  potts3_upload(potts3_t *h, const uint8_t *spins);
+int  potts3_sweep_count(potts3_t *h, uint64_t *t);
+int  potts3_set_sweep_count(potts3_t *h, uint64_t t);
+int  potts3_launch_count(potts3_t *h, uint64_t *n);
+
 #ifdef __cplusplus
 }
 #endif

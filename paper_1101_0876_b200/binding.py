@@ -76,6 +76,17 @@ def load_library() -> ctypes.CDLL:
         "potts_launch_count": ([vp, P(u64)], ctypes.c_int),
         "potts_set_option": ([vp, ctypes.c_char_p, i64], ctypes.c_int),
         "potts_get_option": ([vp, ctypes.c_char_p, P(i64)], ctypes.c_int),
+        "potts3_create": ([P(vp), i32, i32, u64, i32, vp], ctypes.c_int),
+        "potts3_destroy": ([vp], None),
+        "potts3_sweep": ([vp, dbl, i64], ctypes.c_int),
+        "potts3_sweep_measured": ([vp, dbl, i64, i64, vp, vp], ctypes.c_int),
+        "potts3_energy": ([vp, P(i64)], ctypes.c_int),
+        "potts3_histogram": ([vp, vp], ctypes.c_int),
+        "potts3_download": ([vp, vp], ctypes.c_int),
+        "potts3_upload": ([vp, vp], ctypes.c_int),
+        "potts3_sweep_count": ([vp, P(u64)], ctypes.c_int),
+        "potts3_set_sweep_count": ([vp, u64], ctypes.c_int),
+        "potts3_launch_count": ([vp, P(u64)], ctypes.c_int),
         "potts_last_error": ([], ctypes.c_char_p),
         "potts_version": ([], ctypes.c_char_p),
     }
@@ -95,6 +106,8 @@ EXPORTED_SYMBOLS = [
     "potts_version", "potts_batch_workspace_bytes", "potts_batch_create", "potts_batch_destroy",
     "potts_batch_sweep_measured", "potts_batch_sweep_delta", "potts_batch_ladder", "potts_batch_download", "potts_batch_sweep_count", "potts_batch_launch_count",
     "potts_set_stream_spec", "potts_get_stream_spec", "potts_batch_set_stream_spec",
+    "potts3_create", "potts3_destroy", "potts3_sweep", "potts3_sweep_measured", "potts3_energy", "potts3_histogram",
+    "potts3_download", "potts3_upload", "potts3_sweep_count", "potts3_set_sweep_count", "potts3_launch_count",
 ]
 
 
@@ -365,4 +378,75 @@ class PottsBatch:
     def potts_batch_launch_count(self) -> int:
         n = ctypes.c_uint64()
         _check(self._lib.potts_batch_launch_count(self._h, ctypes.byref(n)))
+        return int(n.value)
+
+
+class Potts3D:
+    """One L x L x L lattice on the current CUDA device.  Methods mirror the potts3_* entry points."""
+
+    def __init__(self, L: int, q: int, seed: int, init: int = INIT_ORDERED):
+        import torch
+        if not torch.cuda.is_available():
+            raise PottsError(ERR_CUDA, "no CUDA device: the product has no CPU fallback")
+        self._lib = load_library()
+        self.L, self.q, self.seed = int(L), int(q), int(seed)
+        self._stream = torch.cuda.current_stream().cuda_stream
+        h = ctypes.c_void_p()
+        _check(self._lib.potts3_create(ctypes.byref(h), self.L, self.q, self.seed, int(init), ctypes.c_void_p(self._stream)))
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.potts3_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def potts3_sweep(self, T: float, nsweeps: int):
+        _check(self._lib.potts3_sweep(self._h, float(T), int(nsweeps)))
+
+    def potts3_sweep_measured(self, T: float, nsweeps: int, every: int = 1, hist: bool = True):
+        ns = int(nsweeps) // int(every) if every >= 1 and nsweeps >= 0 else 0
+        E = np.zeros(ns, dtype=np.int64)
+        H = np.zeros((ns, self.q), dtype=np.int64) if hist else None
+        _check(self._lib.potts3_sweep_measured(self._h, float(T), int(nsweeps), int(every), E.ctypes.data,
+                                               H.ctypes.data if hist else None))
+        return E, H
+
+    def potts3_energy(self) -> int:
+        E = ctypes.c_int64()
+        _check(self._lib.potts3_energy(self._h, ctypes.byref(E)))
+        return int(E.value)
+
+    def potts3_histogram(self) -> np.ndarray:
+        out = np.zeros(self.q, dtype=np.int64)
+        _check(self._lib.potts3_histogram(self._h, out.ctypes.data))
+        return out
+
+    def potts3_download(self) -> np.ndarray:
+        out = np.empty((self.L, self.L, self.L), dtype=np.uint8)
+        _check(self._lib.potts3_download(self._h, out.ctypes.data))
+        return out
+
+    def potts3_upload(self, spins):
+        a = np.ascontiguousarray(spins, dtype=np.uint8)
+        if a.shape != (self.L, self.L, self.L):
+            raise ValueError("spins must be L x L x L")
+        _check(self._lib.potts3_upload(self._h, a.ctypes.data))
+
+    def potts3_sweep_count(self) -> int:
+        t = ctypes.c_uint64()
+        _check(self._lib.potts3_sweep_count(self._h, ctypes.byref(t)))
+        return int(t.value)
+
+    def potts3_set_sweep_count(self, t: int):
+        _check(self._lib.potts3_set_sweep_count(self._h, int(t)))
+
+    def potts3_launch_count(self) -> int:
+        n = ctypes.c_uint64()
+        _check(self._lib.potts3_launch_count(self._h, ctypes.byref(n)))
         return int(n.value)

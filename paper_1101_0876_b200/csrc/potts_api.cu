@@ -58,6 +58,11 @@ constexpr size_t STATIC_SMEM = sizeof(potts::AcceptLut) + 1024;   // static shar
 
 }  // namespace
 
+namespace potts {
+// the thread-local error message of potts_last_error(), for the other host translation units (potts3d_api.cu)
+int set_error(int code, const char *msg) { g_err = msg; return code; }
+}  // namespace potts
+
 struct potts_s {
     int32_t L = 0, q = 0, layout = 0;
     int device = 0;                      // the CUDA device the handle lives on; every entry point runs on it
