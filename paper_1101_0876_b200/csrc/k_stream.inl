@@ -22,9 +22,33 @@ void launch_hs(const SweepParams &P, int num_sms, size_t smem, cudaStream_t st)
     fn<<<grid, dim3(32, HS_WARPS), smem, st>>>(P);
 }
 
+// the staged form of the plain half-sweep (experiment, option stream_stage): dynamic shared memory = the warps' stages
+template <int CM, bool FAST>
+void launch_hs_bulk(const SweepParams &P, int num_sms, cudaStream_t st)
+{
+    auto fn = k_sweep_rows_u8<CM, POTTS_ST, POTTS_COLOUR, false, false, false, FAST, true>;
+    const size_t smem = (size_t)HS_WARPS * (size_t)(P.rpw + 2) * BULK_ROW;
+    static size_t cached_smem = ~(size_t)0;
+    static int per_sm = 1;
+    if (cached_smem != smem) {
+        cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 << 10);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 32 * HS_WARPS, smem);
+        if (per_sm < 1) per_sm = 1;
+        cached_smem = smem;
+    }
+    const unsigned long long want = (unsigned long long)per_sm * (unsigned)num_sms;
+    const unsigned grid = (unsigned)(want < P.total_tiles ? want : P.total_tiles);
+    fn<<<grid, dim3(32, HS_WARPS), smem, st>>>(P);
+}
+
 template <int CM>
 void launch_hs_cm(const SweepParams &P, bool delta, int num_sms, size_t smem, cudaStream_t st)
 {
+    if (P.bulk && !delta && !P.E_out && !P.hist_out) {
+        if (accept_fast_ok(P.thr)) launch_hs_bulk<CM, true>(P, num_sms, st);
+        else launch_hs_bulk<CM, false>(P, num_sms, st);
+        return;
+    }
     if (delta) { launch_hs<CM, false, false, true, false>(P, num_sms, smem, st); return; }
     const bool fast = accept_fast_ok(P.thr);          // no "never accept" entry: the one-compare form is exact
     if (P.E_out) {

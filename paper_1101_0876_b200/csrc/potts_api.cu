@@ -94,6 +94,7 @@ struct potts_s {
     int64_t opt_resident_rows = 0;       // 0 auto, else at most this many thread rows in a resident block
     int64_t opt_cluster_ctas = 0;        // 0 auto, else the cluster kernel's cluster size (1..16)
     int cluster_checked = 0;             // cluster size whose co-residency was confirmed (cudaOccupancyMaxActiveClusters)
+    int64_t opt_stream_stage = 0;        // 0: other-colour rows through registers; 1: staged in shared memory by cp.async.bulk (experiment)
     int64_t opt_stream_rows = 0;         // 0 auto, else rows per warp of the streaming kernel (even, divides L/4)
 };
 
@@ -188,6 +189,7 @@ int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsign
     P.row_groups = h->L / (potts::HS_WARPS * P.rpw);
     P.total_tiles = gx * (uint32_t)P.row_groups;
     P.tile_counter = h->tile_counter;
+    P.bulk = (h->opt_stream_stage == 1 && (h->L / 2) % 512 == 0 && P.rpw + 2 <= 32) ? 1 : 0;
     const size_t smem = hist_out ? (size_t)potts::hist_words((uint32_t)h->q) * 4 : 0;
     potts::launch_sweep_rows_u8(potts::compare_mode_of(h->q), h->stream_spec, delta, P, h->num_sms, smem, h->stream);
     return check_launch(h, "k_sweep_rows_u8");
@@ -1007,6 +1009,10 @@ int potts_set_option(potts_t *h, const char *key, int64_t value)
         if (value < 0 || value > 2) return fail(POTTS_ERR_ARG, "resident_words must be 0 (auto), 1 or 2");
         h->opt_resident_words = value; return POTTS_OK;
     }
+    if (!std::strcmp(key, "stream_stage")) {
+        if (value < 0 || value > 1) return fail(POTTS_ERR_ARG, "stream_stage must be 0 (registers) or 1 (cp.async.bulk staging)");
+        h->opt_stream_stage = value; return POTTS_OK;
+    }
     if (!std::strcmp(key, "stream_rows")) {
         if (value < 0 || (value > 0 && ((value & 1) || (h->L / potts::HS_WARPS) % value)))
             return fail(POTTS_ERR_ARG, "stream_rows must be 0 (auto) or an even divisor of L / %d", potts::HS_WARPS);
@@ -1025,6 +1031,7 @@ int potts_get_option(potts_t *h, const char *key, int64_t *value)
     if (!std::strcmp(key, "resident_rows")) { *value = h->opt_resident_rows; return POTTS_OK; }
     if (!std::strcmp(key, "cluster_ctas")) { *value = h->opt_cluster_ctas; return POTTS_OK; }
     if (!std::strcmp(key, "stream_rows")) { *value = h->opt_stream_rows; return POTTS_OK; }
+    if (!std::strcmp(key, "stream_stage")) { *value = h->opt_stream_stage; return POTTS_OK; }
     if (!std::strcmp(key, "cluster_active")) {             // read-only: cluster size the next sweep call would use (0 = not the cluster kernel)
         const bool want = h->opt_variant == 3 || (h->opt_variant == 0 && h->layout == POTTS_LAYOUT_U8 && h->L <= CLUSTER_AUTO_L_MAX);
         *value = (want && plan_cluster(h).ok) ? plan_cluster(h).G : 0; return POTTS_OK;

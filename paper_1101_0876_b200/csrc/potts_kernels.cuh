@@ -29,6 +29,7 @@ struct SweepParams {
     int32_t row_groups;         // tiles per column block = L / (HS_WARPS * rpw)
     uint32_t total_tiles;       // column blocks x row_groups
     uint32_t *tile_counter;     // device word, 0 at launch and again after it: the blocks draw their tiles from it
+    int32_t bulk;               // 1: plain half-sweeps take the BULK (cp.async.bulk staging) form of the kernel
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -52,12 +53,22 @@ constexpr int HS_SITES = 16;          // same-colour sites per lane and row
 // handles two rows per trip and the next row's loads alternate between two register sets instead of being copied.
 // FAST: the one-compare form of the acceptance (accept_lut_fill); the host selects it for launches without the
 // energy / energy-change sums when no threshold is zero.
-template <int CM, int ST, int COLOUR, bool MEASURE, bool HIST, bool DELTA, bool FAST>
+// BULK (experiment of round 2, option stream_stage = 1, profiles/r02e_bulk_staging.md): the other-colour rows of a
+// warp's strip (rpw + 2 rows of 512 bytes + a 16-byte halo on either side) are staged in shared memory with
+// cp.async.bulk copies that complete on the warp's mbarrier, and the visits read them from there instead of from
+// global memory.  Needs pitch % 512 == 0 (every lane active) and no histogram (the dynamic shared memory is the stage).
+constexpr int BULK_ROW = 544;                                 // 16 + 512 + 16 bytes
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+template <int CM, int ST, int COLOUR, bool MEASURE, bool HIST, bool DELTA, bool FAST, bool BULK = false>
 __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_constant__ SweepParams P)
 {
     constexpr bool EX = MEASURE || DELTA;
     static_assert(!(FAST && EX), "the sums need the exact form of the acceptance");
-    extern __shared__ uint32_t s_dyn[];                       // HIST: the block's histogram table
+    static_assert(!(BULK && HIST), "the staging buffer takes the dynamic shared memory");
+    extern __shared__ __align__(16) uint32_t s_dyn[];         // HIST: the block's histogram table; BULK: the staged rows
+    __shared__ __align__(8) unsigned long long s_mbar[HS_WARPS];
     __shared__ uint4 s_col[2][HS_SITES][32];                  // ColKeys of [row parity p][site of the chunk][lane]
     __shared__ AcceptLut lut;
     __shared__ int blockAcc;
@@ -66,6 +77,13 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
     if (EX && tid == 0) blockAcc = 0;
     if (HIST)
         for (uint32_t n = tid; n < hist_words(P.q); n += 32 * HS_WARPS) s_dyn[n] = 0u;
+    uint32_t bulk_phase = 0;
+    const uint32_t mbar = smem_u32(&s_mbar[threadIdx.y]);
+    const uint32_t stage = smem_u32(s_dyn) + threadIdx.y * (uint32_t)((P.rpw + 2) * BULK_ROW);   // this warp's rows
+    if (BULK && threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
 
     const int chunks = P.pitch >> 4;                                  // 16-byte chunks per row
     const HalfSweepKeys &K = P.K;
@@ -110,6 +128,43 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
         const int kn = wrap(k0 + 16, pitch), kp = wrap(k0 - 4, pitch);
         const uint8_t *const oth = P.plane_oth + k0;
         uint8_t *const ownp = P.plane_own + k0;
+        if (BULK) {
+            // the previous tile's reads of the stage are done (generic proxy) before the copies overwrite it (async proxy)
+            __syncwarp();
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            const uint32_t bytes = (uint32_t)((P.rpw + 2) * BULK_ROW);
+            if (lane == 0) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+            __syncwarp();
+            if ((int)lane < P.rpw + 2) {
+                const int kb = cb * 512;                                   // first byte of the block's columns in a plane row
+                const uint8_t *src = P.plane_oth + (size_t)wrap(i0 - 1 + (int)lane, L) * pitch;
+                const uint32_t dst = stage + lane * BULK_ROW;
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 512, [%2];" ::"r"(dst + 16), "l"(src + kb), "r"(mbar) : "memory");
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 16, [%2];" ::"r"(dst), "l"(src + wrap(kb - 16, pitch)), "r"(mbar) : "memory");
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 16, [%2];" ::"r"(dst + 528), "l"(src + wrap(kb + 512, pitch)), "r"(mbar) : "memory");
+            }
+            uint32_t done = 0;
+            while (!done)
+                asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mbar), "r"(bulk_phase) : "memory");
+            bulk_phase ^= 1u;
+        }
+        // other-colour row i (rr = i - (i0 - 1) in the stage): my chunk, and the word beside it a visit of parity par needs
+        auto oth16 = [&](int i) {
+            if (BULK) {
+                uint4 v;
+                asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(stage + (uint32_t)((i - i0 + 1) * BULK_ROW) + 16u + lane * 16u));
+                return v;
+            }
+            return *reinterpret_cast<const uint4 *>(oth + (size_t)wrap(i, L) * pitch);
+        };
+        auto oth_adj = [&](int i, int par, int kcol) {
+            if (BULK) {
+                uint32_t v;
+                asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(stage + (uint32_t)((i - i0 + 1) * BULK_ROW) + 16u + lane * 16u + (par ? 16u : 0xfffffffcu)));
+                return v;
+            }
+            return *reinterpret_cast<const uint32_t *>(P.plane_oth + (size_t)i * pitch + kcol);
+        };
 
         // one row visit; PAR = (i + colour) & 1 is uniform over the block row
         auto visit = [&](auto par, int i, const uint4 &own4, const uint32_t (&up)[4], const uint32_t (&mid)[4], uint32_t adjp,
@@ -163,25 +218,25 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
         // hold the loads of the even / odd visit; each visit first issues the loads of the NEXT row into the other
         // set, so they have a whole visit to arrive (the tile's last visit reloads its own row, unused).
         uint32_t up[4], mid[4], dn[4], dn2[4];
-        prep4(ld16(oth + (size_t)wrap(i0 - 1, L) * pitch), up);
-        prep4(ld16(oth + (size_t)i0 * pitch), mid);
+        prep4(oth16(i0 - 1), up);
+        prep4(oth16(i0), mid);
         constexpr int PA = COLOUR, PB = 1 - COLOUR;
         const int k_a = PA ? kn : kp, k_b = PB ? kn : kp;             // column of the word outside the chunk
         uint4 own_a = ld16(ownp + (size_t)i0 * pitch);
-        uint4 dn_a = ld16(oth + (size_t)wrap(i0 + 1, L) * pitch);
-        uint32_t adj_a = *reinterpret_cast<const uint32_t *>(P.plane_oth + (size_t)i0 * pitch + k_a);
+        uint4 dn_a = oth16(i0 + 1);
+        uint32_t adj_a = oth_adj(i0, PA, k_a);
 #pragma unroll 1
         for (int r = 0; r < P.rpw; r += 2) {
             const int i = i0 + r;
             const uint4 own_b = ld16(ownp + (size_t)(i + 1) * pitch);
-            const uint4 dn_b = ld16(oth + (size_t)wrap(i + 2, L) * pitch);
-            const uint32_t adj_b = *reinterpret_cast<const uint32_t *>(P.plane_oth + (size_t)(i + 1) * pitch + k_b);
+            const uint4 dn_b = oth16(i + 2);
+            const uint32_t adj_b = oth_adj(i + 1, PB, k_b);
             prep4(dn_a, dn);
             visit(std::integral_constant<int, PA>{}, i, own_a, up, mid, prep_nbr<CM>(adj_a), dn);
             const int inx = r + 2 < P.rpw ? i + 2 : i + 1;
             own_a = ld16(ownp + (size_t)inx * pitch);
-            dn_a = ld16(oth + (size_t)wrap(inx + 1, L) * pitch);
-            adj_a = *reinterpret_cast<const uint32_t *>(P.plane_oth + (size_t)inx * pitch + k_a);
+            dn_a = oth16(inx + 1);
+            adj_a = oth_adj(inx, PA, k_a);
             prep4(dn_b, dn2);
             visit(std::integral_constant<int, PB>{}, i + 1, own_b, mid, dn, prep_nbr<CM>(adj_b), dn2);
 #pragma unroll

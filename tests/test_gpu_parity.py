@@ -403,3 +403,24 @@ def test_persistent_kernels_are_deterministic_under_repetition(pb):
             assert (Eg == Eo).all() and (Hg == Ho).all(), (shape, rep)
             assert (g.potts_download() == want).all(), (shape, rep)
             g.close()
+
+
+@pytest.mark.parametrize("L,q,seed,rows", [(1024, 9, 3, 0), (2048, 6, 8, 4), (1024, 24, 5, 16), (1024, 200, 2, 2)])
+def test_streaming_kernel_with_bulk_staged_rows(pb, L, q, seed, rows):
+    """Option stream_stage = 1 (cp.async.bulk staging of the other-colour rows, an experiment kept for its A/B record)
+    is one more launch shape of the same chain."""
+    T = 0.99 * workloads.t_c(q)
+    g = pb.Potts(L, q, seed, workloads.INIT_RANDOM)
+    g.potts_set_option("variant", 1)
+    g.potts_set_option("stream_stage", 1)
+    if rows:
+        g.potts_set_option("stream_rows", rows)
+    o = oracle.OraclePotts(L, q, seed, workloads.INIT_RANDOM, threads=8)
+    g.potts_sweep(T, 3)
+    Eg, Hg = g.potts_sweep_measured(T, 2, 1, hist=True)      # sampled sweeps take the unstaged kernel
+    g.potts_sweep(T, 2)
+    o.sweep(T, 3)
+    Eo, Ho = o.sweep_measured(T, 2, 1, hist=True)
+    o.sweep(T, 2)
+    assert (Eg == Eo).all() and (Hg == Ho).all()
+    assert (g.potts_download() == o.spins()).all()
