@@ -21,6 +21,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "potts_oracle.c")
 _SRC3 = os.path.join(_HERE, "potts3d_oracle.c")       # the 3D generalisation, same library
+_SRC8 = os.path.join(_HERE, "potts8_oracle.c")        # first + second neighbours, nine sub-networks
 _LIB = os.path.join(_HERE, "libpotts_oracle.so")
 _lock = threading.Lock()
 _lib = None
@@ -32,11 +33,11 @@ INIT_RANDOM = 1
 def build(force: bool = False) -> str:
     """Compile potts_oracle.c -> libpotts_oracle.so (plain -O2, OpenMP for the optional row-parallel mode)."""
     with _lock:
-        if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC3)):
+        if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC3), os.path.getmtime(_SRC8)):
             tmp = _LIB + f".tmp{os.getpid()}"
             subprocess.check_call(
                 ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
-                 "-o", tmp, _SRC, _SRC3, "-lm"])
+                 "-o", tmp, _SRC, _SRC3, _SRC8, "-lm"])
             os.replace(tmp, _LIB)
     return _LIB
 
@@ -108,6 +109,30 @@ def _load():
         lib.oracle3_sweep_count.restype = ctypes.c_uint64
         lib.oracle3_set_state.argtypes = [vp, u8p, ctypes.c_uint64]
         lib.oracle3_set_state.restype = ctypes.c_int
+        lib.oracle8_thresholds.argtypes = [ctypes.c_double, u32p]
+        lib.oracle8_thresholds.restype = None
+        lib.oracle8_create.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_uint64, ctypes.c_int32]
+        lib.oracle8_create.restype = vp
+        lib.oracle8_destroy.argtypes = [vp]
+        lib.oracle8_destroy.restype = None
+        lib.oracle8_set_threads.argtypes = [vp, ctypes.c_int]
+        lib.oracle8_set_threads.restype = None
+        lib.oracle8_sweep.argtypes = [vp, ctypes.c_double, ctypes.c_int64]
+        lib.oracle8_sweep.restype = ctypes.c_int
+        lib.oracle8_sweep_measured.argtypes = [vp, ctypes.c_double, ctypes.c_int64, ctypes.c_int64, i64p, i64p]
+        lib.oracle8_sweep_measured.restype = ctypes.c_int
+        lib.oracle8_energy.argtypes = [vp]
+        lib.oracle8_energy.restype = ctypes.c_int64
+        lib.oracle8_energy_incremental.argtypes = [vp]
+        lib.oracle8_energy_incremental.restype = ctypes.c_int64
+        lib.oracle8_histogram.argtypes = [vp, i64p]
+        lib.oracle8_histogram.restype = None
+        lib.oracle8_spins.argtypes = [vp]
+        lib.oracle8_spins.restype = u8p
+        lib.oracle8_sweep_count.argtypes = [vp]
+        lib.oracle8_sweep_count.restype = ctypes.c_uint64
+        lib.oracle8_set_state.argtypes = [vp, u8p, ctypes.c_uint64]
+        lib.oracle8_set_state.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -286,3 +311,43 @@ class OraclePotts3D:
         assert a.shape == (self.L, self.L, self.L)
         if self._lib.oracle3_set_state(self._h, a.ctypes.data_as(ctypes.POINTER(ctypes.c_uint8)), int(t)):
             raise ValueError("spin value >= q")
+
+
+def thresholds8(T: float):
+    """[thr(1) .. thr(8)] = floor(2^32 exp(-d/T)) for the 8-neighbour model (R6")."""
+    lib = _load()
+    o = (ctypes.c_uint32 * 9)()
+    lib.oracle8_thresholds(float(T), o)
+    return [int(o[d]) for d in range(1, 9)]
+
+
+class OraclePotts8(OraclePotts3D):
+    """The 2D chain with first and second neighbours, nine sub-networks (potts8_oracle.c); spins()[i, j]."""
+
+    def __init__(self, L: int, q: int, seed: int, init: int, threads: int = 1):
+        self._lib = _Prefixed(_load(), "oracle8_")
+        self.L, self.q, self.seed = int(L), int(q), int(seed)
+        self._h = self._lib.oracle3_create(self.L, self.q, self.seed, int(init))
+        if not self._h:
+            raise ValueError(f"bad arguments L={L} q={q} init={init}")
+        self._lib.oracle3_set_threads(self._h, int(threads))
+
+    def spins(self) -> np.ndarray:
+        p = self._lib.oracle3_spins(self._h)
+        return np.ctypeslib.as_array(p, shape=(self.L, self.L)).copy()
+
+    def set_state(self, spins: np.ndarray, t: int):
+        a = np.ascontiguousarray(spins, dtype=np.uint8)
+        assert a.shape == (self.L, self.L)
+        if self._lib.oracle3_set_state(self._h, a.ctypes.data_as(ctypes.POINTER(ctypes.c_uint8)), int(t)):
+            raise ValueError("spin value >= q")
+
+
+class _Prefixed:
+    """Lets OraclePotts8 reuse OraclePotts3D's marshalling: oracle3_xyz -> oracle8_xyz of the same library."""
+
+    def __init__(self, lib, prefix):
+        self._lib, self._prefix = lib, prefix
+
+    def __getattr__(self, name):
+        return getattr(self._lib, name.replace("oracle3_", self._prefix))
