@@ -456,6 +456,33 @@ def cubic_lattice(pb, torch, peaks, L=512, q=9, sweeps=40, repeats=3):
             "spin_updates_per_s": ups, "ms_per_call_min_max": [min(ms), max(ms)], "kernel": "k_sweep3_u8", "roofline": r}
 
 
+def second_neighbour_lattice(pb, torch, peaks, L=12288, q=9, sweeps=20, repeats=3):
+    """SURVEY 8(f)4 / PAPER.md:359: first + second neighbour interactions, nine sub-networks (potts8_sweep, k_sweep8_u8:
+    one launch per sub-network, one 4-site word per thread, first CUDA path of this row); random start, T = 2.0.
+    Algorithmic counts per update: 36 instructions; bytes: own read + write, each other site read once per sub-network
+    that neighbours it (8 of 9): 10 B without on-chip reuse across launches."""
+    hbm_gbs, sm_max, which = peaks
+    T = 2.0
+    g = pb.Potts8(L, q, 5, pb.INIT_RANDOM)
+    g.potts8_sweep(T, 3)
+    ms = []
+    for _ in range(repeats):
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        g.potts8_sweep(T, sweeps)
+        e1.record()
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    g.close()
+    sec = statistics.median(ms) * 1e-3
+    w = type("W", (), {"name": f"potts8_q{q}_L{L}"})
+    r = roofline(w, "k_sweep8_u8", L * L / 9, sec * 1e3 / (9 * sweeps), sm_max, hbm_gbs, which, 10.0)
+    ups = sweeps * L * L / sec
+    return {"q": q, "L": L, "sweeps_per_call": sweeps, "calls": repeats, "T": T, "ns_per_spin_flip": 1e9 / ups,
+            "spin_updates_per_s": ups, "ms_per_call_min_max": [min(ms), max(ms)], "kernel": "k_sweep8_u8", "roofline": r}
+
+
 def paper_protocol_e6(pb, torch):
     """The paper's end-to-end example: q=9, L=1024, 3 samples, T = 0.71 .. 0.73 in steps of 0.002,
     t_tran = 2000, t_max = 8000, one measure every 50 sweeps; 193 s on a GTX 280, 8115 s on its CPU.  Here: the same
@@ -618,6 +645,7 @@ def main():
         per_cfg["delta_cfg1_cluster"] = delta_cost(pb, torch, 1, 2000)
         per_cfg["stream_spec_2"] = stream_spec_2_table(pb, torch, flush, peaks)
         per_cfg["potts3d_q9_L512"] = cubic_lattice(pb, torch, peaks)
+        per_cfg["potts8_q9_L12288"] = second_neighbour_lattice(pb, torch, peaks)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(w)
     if dist is not None:

@@ -248,6 +248,29 @@ int  potts3_sweep_count(potts3_t *h, uint64_t *t);
 int  potts3_set_sweep_count(potts3_t *h, uint64_t t);
 int  potts3_launch_count(potts3_t *h, uint64_t *n);
 
+/* ---- first AND second neighbour interactions (sec. 7: "For the 2D case with first and second neighbors
+ * interactions, there are nine independent sub-networks to update instead of two") --------------------------------
+ * The same Metropolis chain on the L x L periodic square lattice where every site interacts with its 4 first and its 4
+ * second (diagonal) neighbours, equal coupling J = 1 (reading S17):
+ * E = -sum over sites of [d(s, s_{i,j+1}) + d(s, s_{i+1,j}) + d(s, s_{i+1,j+1}) + d(s, s_{i+1,j-1})] in [-4 L^2, 0];
+ * sweep = the nine sub-networks c = 3 (i mod 3) + (j mod 3), c = 0..8 in this order; random words
+ * Philox4x32-10(counter = (j, i, t, 16 + c), key = seed); d = n_old - n_new in -8..8, thresholds floor(2^32 exp(-d/T)),
+ * d = 1..8; start states as potts_create (the random start is the same configuration).  Spins cross the boundary
+ * row-major s[i L + j] (host).  L a multiple of 3 (POTTS_ERR_ARG otherwise) and of 12 (POTTS_ERR_UNSUPPORTED otherwise).
+ * Conventions as for potts3_*. */
+typedef struct potts8_s potts8_t;
+int  potts8_create(potts8_t **out, int32_t L, int32_t q, uint64_t seed, int32_t init, void *cuda_stream);
+void potts8_destroy(potts8_t *h);
+int  potts8_sweep(potts8_t *h, double T, int64_t nsweeps);
+int  potts8_sweep_measured(potts8_t *h, double T, int64_t nsweeps, int64_t every, int64_t *E_series, int64_t *hist_series);
+int  potts8_energy(potts8_t *h, int64_t *E);
+int  potts8_histogram(potts8_t *h, int64_t *counts);
+int  potts8_download(potts8_t *h, uint8_t *spins);
+int  potts8_upload(potts8_t *h, const uint8_t *spins);
+int  potts8_sweep_count(potts8_t *h, uint64_t *t);
+int  potts8_set_sweep_count(potts8_t *h, uint64_t t);
+int  potts8_launch_count(potts8_t *h, uint64_t *n);
+
 #ifdef __cplusplus
 }
 #endif

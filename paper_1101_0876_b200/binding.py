@@ -87,6 +87,17 @@ def load_library() -> ctypes.CDLL:
         "potts3_sweep_count": ([vp, P(u64)], ctypes.c_int),
         "potts3_set_sweep_count": ([vp, u64], ctypes.c_int),
         "potts3_launch_count": ([vp, P(u64)], ctypes.c_int),
+        "potts8_create": ([P(vp), i32, i32, u64, i32, vp], ctypes.c_int),
+        "potts8_destroy": ([vp], None),
+        "potts8_sweep": ([vp, dbl, i64], ctypes.c_int),
+        "potts8_sweep_measured": ([vp, dbl, i64, i64, vp, vp], ctypes.c_int),
+        "potts8_energy": ([vp, P(i64)], ctypes.c_int),
+        "potts8_histogram": ([vp, vp], ctypes.c_int),
+        "potts8_download": ([vp, vp], ctypes.c_int),
+        "potts8_upload": ([vp, vp], ctypes.c_int),
+        "potts8_sweep_count": ([vp, P(u64)], ctypes.c_int),
+        "potts8_set_sweep_count": ([vp, u64], ctypes.c_int),
+        "potts8_launch_count": ([vp, P(u64)], ctypes.c_int),
         "potts_last_error": ([], ctypes.c_char_p),
         "potts_version": ([], ctypes.c_char_p),
     }
@@ -108,6 +119,8 @@ EXPORTED_SYMBOLS = [
     "potts_set_stream_spec", "potts_get_stream_spec", "potts_batch_set_stream_spec",
     "potts3_create", "potts3_destroy", "potts3_sweep", "potts3_sweep_measured", "potts3_energy", "potts3_histogram",
     "potts3_download", "potts3_upload", "potts3_sweep_count", "potts3_set_sweep_count", "potts3_launch_count",
+    "potts8_create", "potts8_destroy", "potts8_sweep", "potts8_sweep_measured", "potts8_energy", "potts8_histogram",
+    "potts8_download", "potts8_upload", "potts8_sweep_count", "potts8_set_sweep_count", "potts8_launch_count",
 ]
 
 
@@ -449,4 +462,75 @@ class Potts3D:
     def potts3_launch_count(self) -> int:
         n = ctypes.c_uint64()
         _check(self._lib.potts3_launch_count(self._h, ctypes.byref(n)))
+        return int(n.value)
+
+
+class Potts8:
+    """One L x L x L lattice on the current CUDA device.  Methods mirror the potts8_* entry points."""
+
+    def __init__(self, L: int, q: int, seed: int, init: int = INIT_ORDERED):
+        import torch
+        if not torch.cuda.is_available():
+            raise PottsError(ERR_CUDA, "no CUDA device: the product has no CPU fallback")
+        self._lib = load_library()
+        self.L, self.q, self.seed = int(L), int(q), int(seed)
+        self._stream = torch.cuda.current_stream().cuda_stream
+        h = ctypes.c_void_p()
+        _check(self._lib.potts8_create(ctypes.byref(h), self.L, self.q, self.seed, int(init), ctypes.c_void_p(self._stream)))
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.potts8_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def potts8_sweep(self, T: float, nsweeps: int):
+        _check(self._lib.potts8_sweep(self._h, float(T), int(nsweeps)))
+
+    def potts8_sweep_measured(self, T: float, nsweeps: int, every: int = 1, hist: bool = True):
+        ns = int(nsweeps) // int(every) if every >= 1 and nsweeps >= 0 else 0
+        E = np.zeros(ns, dtype=np.int64)
+        H = np.zeros((ns, self.q), dtype=np.int64) if hist else None
+        _check(self._lib.potts8_sweep_measured(self._h, float(T), int(nsweeps), int(every), E.ctypes.data,
+                                               H.ctypes.data if hist else None))
+        return E, H
+
+    def potts8_energy(self) -> int:
+        E = ctypes.c_int64()
+        _check(self._lib.potts8_energy(self._h, ctypes.byref(E)))
+        return int(E.value)
+
+    def potts8_histogram(self) -> np.ndarray:
+        out = np.zeros(self.q, dtype=np.int64)
+        _check(self._lib.potts8_histogram(self._h, out.ctypes.data))
+        return out
+
+    def potts8_download(self) -> np.ndarray:
+        out = np.empty((self.L, self.L), dtype=np.uint8)
+        _check(self._lib.potts8_download(self._h, out.ctypes.data))
+        return out
+
+    def potts8_upload(self, spins):
+        a = np.ascontiguousarray(spins, dtype=np.uint8)
+        if a.shape != (self.L, self.L):
+            raise ValueError("spins must be L x L")
+        _check(self._lib.potts8_upload(self._h, a.ctypes.data))
+
+    def potts8_sweep_count(self) -> int:
+        t = ctypes.c_uint64()
+        _check(self._lib.potts8_sweep_count(self._h, ctypes.byref(t)))
+        return int(t.value)
+
+    def potts8_set_sweep_count(self, t: int):
+        _check(self._lib.potts8_set_sweep_count(self._h, int(t)))
+
+    def potts8_launch_count(self) -> int:
+        n = ctypes.c_uint64()
+        _check(self._lib.potts8_launch_count(self._h, ctypes.byref(n)))
         return int(n.value)

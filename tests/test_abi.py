@@ -22,7 +22,7 @@ def pb():
 def _declared():
     text = open(os.path.join(ROOT, "include", "potts.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(potts3?_[a-z_0-9]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(potts[38]?_[a-z_0-9]+)\s*\(", text)))
 
 
 def test_every_declared_symbol_is_exported(pb):
