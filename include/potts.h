@@ -224,6 +224,25 @@ const char *potts_last_error(void);
 /* Library version string, e.g. "potts-b200 0.1 (sm_100a)". */
 const char *potts_version(void);
 
+/* ---- one lattice split into row strips over several GPUs -------------------------------------------------
+ * A strip handle holds rows [row0, row0 + rows) of the L x L lattice (U8 layout, both ends multiples of 32) plus one
+ * halo row above and one below per colour plane.  Because the random words are a pure function of the GLOBAL site
+ * (R3) the strips together follow exactly the chain of one potts_create handle, whatever their number.  The caller
+ * drives the sweep: for colour 0 then 1: potts_strip_half_sweep on every strip, then copy each strip's first / last
+ * row of the plane just written (potts_strip_rows: device pointers, row_bytes = L/2) into the halo_below / halo_above
+ * of the strip above / below it (periodic; device-to-device or NCCL send/recv); then potts_strip_advance.  Before the
+ * first half-sweep the halos of BOTH planes must be filled the same way.  E_dev (colour 1 only) / hist_dev: device
+ * int64 accumulators (1 / q entries, zeroed by the caller) that receive this strip's part of the energy / histogram
+ * of the sites just written, or null.  potts_energy, potts_histogram (partial sums over the strip; the halos of plane 0
+ * must be current), potts_download / potts_upload (rows x L bytes) work on strip handles; potts_sweep* do not
+ * (POTTS_ERR_UNSUPPORTED).  paper_1101_0876_b200/strips.py drives strips over torch.distributed. */
+int potts_create_strip(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t init, int32_t row0, int32_t rows,
+                       void *cuda_stream);
+int potts_strip_half_sweep(potts_t *h, double T, int32_t colour, int64_t *E_dev, int64_t *hist_dev);
+int potts_strip_advance(potts_t *h);
+int potts_strip_rows(potts_t *h, int32_t colour, void **first_row, void **last_row, void **halo_above, void **halo_below,
+                     size_t *row_bytes);
+
 /* ---- 3D generalisation (sec. 7: "For the generalization to the 3D case, the checkerboard scheme defining
  * two independent sub-networks persists, however the cell-packing scheme should be updated") -----------------------
  * The same Metropolis chain on an L x L x L periodic simple-cubic lattice with 6 nearest neighbours (DESIGN.md reading

@@ -76,6 +76,10 @@ def load_library() -> ctypes.CDLL:
         "potts_launch_count": ([vp, P(u64)], ctypes.c_int),
         "potts_set_option": ([vp, ctypes.c_char_p, i64], ctypes.c_int),
         "potts_get_option": ([vp, ctypes.c_char_p, P(i64)], ctypes.c_int),
+        "potts_create_strip": ([P(vp), i32, i32, u64, i32, i32, i32, vp], ctypes.c_int),
+        "potts_strip_half_sweep": ([vp, dbl, i32, vp, vp], ctypes.c_int),
+        "potts_strip_advance": ([vp], ctypes.c_int),
+        "potts_strip_rows": ([vp, i32, P(vp), P(vp), P(vp), P(vp), P(ctypes.c_size_t)], ctypes.c_int),
         "potts3_create": ([P(vp), i32, i32, u64, i32, vp], ctypes.c_int),
         "potts3_destroy": ([vp], None),
         "potts3_sweep": ([vp, dbl, i64], ctypes.c_int),
@@ -117,6 +121,7 @@ EXPORTED_SYMBOLS = [
     "potts_version", "potts_batch_workspace_bytes", "potts_batch_create", "potts_batch_destroy",
     "potts_batch_sweep_measured", "potts_batch_sweep_delta", "potts_batch_ladder", "potts_batch_download", "potts_batch_sweep_count", "potts_batch_launch_count",
     "potts_set_stream_spec", "potts_get_stream_spec", "potts_batch_set_stream_spec",
+    "potts_create_strip", "potts_strip_half_sweep", "potts_strip_advance", "potts_strip_rows",
     "potts3_create", "potts3_destroy", "potts3_sweep", "potts3_sweep_measured", "potts3_energy", "potts3_histogram",
     "potts3_download", "potts3_upload", "potts3_sweep_count", "potts3_set_sweep_count", "potts3_launch_count",
     "potts8_create", "potts8_destroy", "potts8_sweep", "potts8_sweep_measured", "potts8_energy", "potts8_histogram",

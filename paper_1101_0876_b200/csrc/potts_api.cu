@@ -65,6 +65,8 @@ int set_error(int code, const char *msg) { g_err = msg; return code; }
 
 struct potts_s {
     int32_t L = 0, q = 0, layout = 0;
+    int32_t rows = 0, row0 = 0;          // rows held by this handle: the whole lattice (rows = L, row0 = 0) or a row strip of it
+    bool strip = false;                  // row strip of a lattice split over several GPUs: halo rows instead of the periodic wrap
     int device = 0;                      // the CUDA device the handle lives on; every entry point runs on it
     uint64_t seed = 0, t = 0;
     uint8_t *ws = nullptr;
@@ -169,6 +171,9 @@ potts::SweepParams sweep_params(const potts_t *h, uint32_t colour, const uint32_
     P.K = potts::half_sweep_keys((uint32_t)(h->seed & 0xFFFFFFFFull), (uint32_t)(h->seed >> 32), (uint32_t)h->t, colour);
     for (int d = 0; d < 4; ++d) P.thr[d] = thr[d];
     P.E_out = E_out;
+    P.rows = h->rows;
+    P.row0 = h->row0;
+    P.strip = h->strip ? 1 : 0;
     return P;
 }
 
@@ -186,7 +191,7 @@ int launch_half_sweep(potts_t *h, uint32_t colour, const uint32_t thr[4], unsign
     const int chunks = h->L / 32;
     const unsigned gx = (unsigned)((chunks + 31) / 32);
     P.rpw = h->opt_stream_rows > 0 ? (int)h->opt_stream_rows : STREAM_ROWS_PER_WARP;
-    P.row_groups = h->L / (potts::HS_WARPS * P.rpw);
+    P.row_groups = h->rows / (potts::HS_WARPS * P.rpw);
     P.total_tiles = gx * (uint32_t)P.row_groups;
     P.tile_counter = h->tile_counter;
     P.bulk = (h->opt_stream_stage == 1 && (h->L / 2) % 512 == 0 && P.rpw + 2 <= 32) ? 1 : 0;
@@ -236,12 +241,14 @@ int launch_measure(potts_t *h, unsigned long long *E_out, unsigned long long *hi
     potts::MeasureParams M;
     M.plane0 = h->plane[0];
     M.plane1 = h->plane[1];
-    M.L = h->L;
+    M.L = h->rows;
     M.pitch = h->L / 2;
+    M.row0 = h->row0;
+    M.strip = h->strip ? 1 : 0;
     M.q = (uint32_t)h->q;
     M.E_out = E_out;
     M.hist_out = hist_out;
-    const long long threads = (long long)h->L * (h->L / 32);
+    const long long threads = (long long)h->rows * (h->L / 32);
     const int block = 256;
     long long blocks = (threads + block - 1) / block;
     if (blocks > 148 * 8) blocks = 148 * 8;
@@ -254,6 +261,7 @@ int launch_measure(potts_t *h, unsigned long long *E_out, unsigned long long *hi
 int check_sweep_args(potts_t *h, double T, int64_t nsweeps)
 {
     if (!h) return fail(POTTS_ERR_ARG, "null handle");
+    if (h->strip) return fail(POTTS_ERR_UNSUPPORTED, "a row strip is advanced half-sweep by half-sweep (potts_strip_half_sweep): its halo rows must be exchanged in between");
     if (!(T > 0.0) || !std::isfinite(T)) return fail(POTTS_ERR_ARG, "T = %g must be finite and > 0", T);
     if (nsweeps < 0) return fail(POTTS_ERR_ARG, "nsweeps = %lld < 0", (long long)nsweeps);
     if (h->t + (uint64_t)nsweeps > 0xFFFFFFFFull)
@@ -568,6 +576,7 @@ int potts_create_ex(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t 
     potts_t *h = new (std::nothrow) potts_s;
     if (!h) return fail(POTTS_ERR_NOMEM, "host allocation failed");
     h->L = L; h->q = q; h->layout = layout; h->seed = seed; h->t = 0;
+    h->rows = L;
     cudaGetDevice(&h->device);
     h->stream = (cudaStream_t)cuda_stream;
     if (dev_workspace) {
@@ -843,8 +852,8 @@ int potts_download(potts_t *h, uint8_t *spins)
     rc = ensure_copy_objects(h);
     if (rc) return rc;
     int k = 0;
-    for (int i0 = 0; i0 < L && rc == POTTS_OK; i0 += rows, ++k) {
-        const int r = (L - i0 < rows) ? L - i0 : rows, b = k & 1;
+    for (int i0 = 0; i0 < h->rows && rc == POTTS_OK; i0 += rows, ++k) {          // h->rows = L, or the rows of a strip
+        const int r = (h->rows - i0 < rows) ? h->rows - i0 : rows, b = k & 1;
         uint8_t *buf = stage + (size_t)b * buf_bytes;
         if (k >= 2) CUDA_TRY(cudaStreamWaitEvent(h->stream, h->ev_copied[b], 0));      // the copy out of this buffer is done
         const long long threads = (long long)r * (L / 8);
@@ -902,7 +911,7 @@ int potts_upload(potts_t *h, const uint8_t *spins)
     const int L = h->L, rows = chunk_rows(L);
     // validate on the host first so that a rejected upload leaves the lattice untouched; the converter checks again
     // on the device and its flag is read back below
-    if (host_has_value_ge(spins, (size_t)L * L, h->q)) return fail(POTTS_ERR_ARG, "a spin value is >= q = %d", h->q);
+    if (host_has_value_ge(spins, (size_t)h->rows * L, h->q)) return fail(POTTS_ERR_ARG, "a spin value is >= q = %d", h->q);
     const size_t buf_bytes = (size_t)rows * L;
     uint8_t *stage = nullptr;
     int rc = get_scratch(h, 2 * buf_bytes, &stage);
@@ -914,8 +923,8 @@ int potts_upload(potts_t *h, const uint8_t *spins)
     CUDA_TRY(cudaEventRecord(h->ev_start, h->stream));
     CUDA_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_start, 0));
     int k = 0;
-    for (int i0 = 0; i0 < L && rc == POTTS_OK; i0 += rows, ++k) {
-        const int r = (L - i0 < rows) ? L - i0 : rows, b = k & 1;
+    for (int i0 = 0; i0 < h->rows && rc == POTTS_OK; i0 += rows, ++k) {          // h->rows = L, or the rows of a strip
+        const int r = (h->rows - i0 < rows) ? h->rows - i0 : rows, b = k & 1;
         uint8_t *buf = stage + (size_t)b * buf_bytes;
         if (k >= 2) CUDA_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_converted[b], 0));   // the converter has read this buffer
         CUDA_TRY(cudaMemcpyAsync(buf, spins + (size_t)i0 * L, (size_t)r * L, cudaMemcpyHostToDevice, h->copy_stream));
@@ -940,6 +949,99 @@ int potts_upload(potts_t *h, const uint8_t *spins)
     if (rc) return rc;
     if (e != cudaSuccess || e1 != cudaSuccess || e2 != cudaSuccess) return fail(POTTS_ERR_CUDA, "upload copy failed");
     if (bad) return fail(POTTS_ERR_ARG, "a spin value is >= q = %d (device check; the lattice is now undefined)", h->q);
+    return POTTS_OK;
+}
+
+// ---- one lattice split into row strips over several GPUs ------------------------------------------
+int potts_create_strip(potts_t **out, int32_t L, int32_t q, uint64_t seed, int32_t init, int32_t row0, int32_t rows,
+                       void *cuda_stream)
+{
+    if (!out) return fail(POTTS_ERR_ARG, "null out pointer");
+    if (init != POTTS_INIT_ORDERED && init != POTTS_INIT_RANDOM) return fail(POTTS_ERR_ARG, "bad init %d", init);
+    int rc = check_shape(L, q, POTTS_LAYOUT_U8);
+    if (rc) return rc;
+    if (row0 < 0 || rows < 32 || row0 + rows > L || row0 % 32 || rows % 32)
+        return fail(POTTS_ERR_ARG, "strip rows [%d, %d) must lie in [0, %d) with both ends multiples of 32", row0, row0 + rows, L);
+    int ndev = 0;
+    CUDA_TRY(cudaGetDeviceCount(&ndev));
+    if (ndev < 1) return fail(POTTS_ERR_CUDA, "no CUDA device");
+    potts_t *h = new (std::nothrow) potts_s;
+    if (!h) return fail(POTTS_ERR_NOMEM, "host allocation failed");
+    h->L = L; h->q = q; h->layout = POTTS_LAYOUT_U8; h->seed = seed; h->t = 0;
+    h->rows = rows; h->row0 = row0; h->strip = true;
+    h->opt_variant = 1;                                                  // streaming kernels only
+    h->stream = (cudaStream_t)cuda_stream;
+    cudaGetDevice(&h->device);
+    const size_t pitch = (size_t)L / 2;
+    h->plane_bytes = align_up((size_t)(rows + 2) * pitch);              // one halo row above and one below
+    const size_t need = 2 * h->plane_bytes + align_up(ACC_WORDS * sizeof(unsigned long long)) + ALIGN;
+    cudaError_t e = cudaMalloc(&h->ws, need);
+    if (e != cudaSuccess) {
+        delete h;
+        return fail(e == cudaErrorMemoryAllocation ? POTTS_ERR_NOMEM : POTTS_ERR_CUDA, "cudaMalloc(%zu) failed: %s", need, cudaGetErrorString(e));
+    }
+    h->owns_ws = true;
+    h->plane[0] = h->ws + pitch;                                         // local row 0; the halo row above it is at -pitch
+    h->plane[1] = h->ws + h->plane_bytes + pitch;
+    h->acc = (unsigned long long *)(h->ws + 2 * h->plane_bytes);
+    h->flag = (int *)(h->acc + 257);
+    h->error = h->flag + 1;
+    h->tile_counter = (uint32_t *)(h->acc + 258);
+    {
+        int v = 0;
+        cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, h->device);
+        h->num_sms = v;
+        cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
+        h->smem_optin = (size_t)v;
+    }
+    e = cudaMemsetAsync(h->ws, 0, need, h->stream);
+    if (e == cudaSuccess && init == POTTS_INIT_RANDOM) {
+        const long long words = 2ll * rows * (L / 8);
+        potts::k_init_random_u8<<<(unsigned)((words + 255) / 256), 256, 0, h->stream>>>(
+            h->plane[0], h->plane[1], rows, L / 2, (uint32_t)q, (uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32), row0);
+        h->launches += 1;
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) {
+        potts_destroy(h);
+        return fail(POTTS_ERR_CUDA, "strip initialisation failed: %s", cudaGetErrorString(e));
+    }
+    *out = h;
+    return POTTS_OK;
+}
+
+int potts_strip_half_sweep(potts_t *h, double T, int32_t colour, int64_t *E_dev, int64_t *hist_dev)
+{
+    ON_DEVICE_OF(h);
+    if (!h || !h->strip) return fail(POTTS_ERR_ARG, "not a strip handle");
+    if (!(T > 0.0) || !std::isfinite(T)) return fail(POTTS_ERR_ARG, "T = %g must be finite and > 0", T);
+    if (colour != 0 && colour != 1) return fail(POTTS_ERR_ARG, "colour must be 0 or 1");
+    if (E_dev && colour != 1) return fail(POTTS_ERR_ARG, "the energy is counted from the colour-1 sites");
+    if (h->t >= 0xFFFFFFFFull) return fail(POTTS_ERR_ARG, "sweep counter would pass 2^32 - 1");
+    uint32_t thr[4];
+    thresholds(T, thr);
+    return launch_half_sweep(h, (uint32_t)colour, thr, (unsigned long long *)E_dev, (unsigned long long *)hist_dev);
+}
+
+int potts_strip_advance(potts_t *h)
+{
+    if (!h || !h->strip) return fail(POTTS_ERR_ARG, "not a strip handle");
+    h->t += 1;
+    return POTTS_OK;
+}
+
+int potts_strip_rows(potts_t *h, int32_t colour, void **first_row, void **last_row, void **halo_above, void **halo_below,
+                     size_t *row_bytes)
+{
+    if (!h || !h->strip || !first_row || !last_row || !halo_above || !halo_below || !row_bytes) return fail(POTTS_ERR_ARG, "bad argument");
+    if (colour != 0 && colour != 1) return fail(POTTS_ERR_ARG, "colour must be 0 or 1");
+    const size_t pitch = (size_t)h->L / 2;
+    uint8_t *p = h->plane[colour];
+    *first_row = p;
+    *last_row = p + (size_t)(h->rows - 1) * pitch;
+    *halo_above = p - pitch;
+    *halo_below = p + (size_t)h->rows * pitch;
+    *row_bytes = pitch;
     return POTTS_OK;
 }
 

@@ -30,6 +30,11 @@ struct SweepParams {
     uint32_t total_tiles;       // column blocks x row_groups
     uint32_t *tile_counter;     // device word, 0 at launch and again after it: the blocks draw their tiles from it
     int32_t bulk;               // 1: plain half-sweeps take the BULK (cp.async.bulk staging) form of the kernel
+    // Row strip of a lattice split over several GPUs: the planes hold `rows` rows, local row r = global row
+    // row0 + r (row0 even), with one halo row above local row 0 and one below local row rows-1 that the host fills
+    // from the neighbouring strips; plane_own / plane_oth point at local row 0.  rows = L, row0 = 0, strip = 0: the whole
+    // (periodic) lattice.
+    int32_t rows, row0, strip;
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -89,7 +94,7 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
     const HalfSweepKeys &K = P.K;
     const uint32_t lane_off = accept_lane_offset(lane);
     const uint32_t q = in_register(P.q);
-    const int L = P.L, pitch = P.pitch;
+    const int L = P.rows, pitch = P.pitch;                            // L: rows of this plane (the lattice's, or the strip's)
     int acc = 0, rows_done = 0;                                       // acc: MEASURE unequal neighbours of the final spins; DELTA energy change
     // Tiles (column block cb, row group rg) are drawn from a global counter: tile = cb * row_groups + rg, so a block
     // mostly stays in its column block and keeps its ColKeys.  atomicInc wraps to 0 after the last of the
@@ -137,7 +142,7 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
             __syncwarp();
             if ((int)lane < P.rpw + 2) {
                 const int kb = cb * 512;                                   // first byte of the block's columns in a plane row
-                const uint8_t *src = P.plane_oth + (size_t)wrap(i0 - 1 + (int)lane, L) * pitch;
+                const uint8_t *src = P.plane_oth + (long long)(P.strip ? i0 - 1 + (int)lane : wrap(i0 - 1 + (int)lane, L)) * pitch;
                 const uint32_t dst = stage + lane * BULK_ROW;
                 asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 512, [%2];" ::"r"(dst + 16), "l"(src + kb), "r"(mbar) : "memory");
                 asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 16, [%2];" ::"r"(dst), "l"(src + wrap(kb - 16, pitch)), "r"(mbar) : "memory");
@@ -155,7 +160,7 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
                 asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(stage + (uint32_t)((i - i0 + 1) * BULK_ROW) + 16u + lane * 16u));
                 return v;
             }
-            return *reinterpret_cast<const uint4 *>(oth + (size_t)wrap(i, L) * pitch);
+            return *reinterpret_cast<const uint4 *>(oth + (long long)(P.strip ? i : wrap(i, L)) * pitch);   // a strip has halo rows at -1 and L
         };
         auto oth_adj = [&](int i, int par, int kcol) {
             if (BULK) {
@@ -170,7 +175,7 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
         auto visit = [&](auto par, int i, const uint4 &own4, const uint32_t (&up)[4], const uint32_t (&mid)[4], uint32_t adjp,
                          const uint32_t (&dn)[4]) {
             constexpr int PAR = decltype(par)::value;
-            const RowKeysH R = row_keys_h(K, (uint32_t)i);
+            const RowKeysH R = row_keys_h(K, (uint32_t)(i + P.row0));
             const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
             uint32_t out[4];
 #pragma unroll
@@ -267,7 +272,8 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
 // at the same (row, k-range) is the thread's "mid" word, so every white site is counted once.
 struct MeasureParams {
     const uint8_t *plane0, *plane1;
-    int32_t L, pitch;
+    int32_t L, pitch;               // L: rows of the planes (the lattice's, or the strip's); pitch = lattice L / 2
+    int32_t row0, strip;            // row strip (see SweepParams): halo rows instead of the periodic wrap
     uint32_t q;
     unsigned long long *E_out;      // may be null
     unsigned long long *hist_out;   // q entries, may be null
@@ -292,15 +298,15 @@ __global__ void __launch_bounds__(256) k_measure_u8(const MeasureParams P)
         const int i = (int)(gid / chunks);
         const int x = (int)(gid - (long long)i * chunks);
         const int k0 = x << 4;
-        const uint32_t p = (uint32_t)(i + 1) & 1u;                   // colour 1 sites
-        const int iu = wrap(i - 1, P.L), id = wrap(i + 1, P.L);
+        const uint32_t p = (uint32_t)(i + P.row0 + 1) & 1u;          // colour 1 sites
+        const long long iu = P.strip ? i - 1 : wrap(i - 1, P.L), id = P.strip ? i + 1 : wrap(i + 1, P.L);
         const size_t row = (size_t)i * P.pitch;
         const uint4 own4 = *reinterpret_cast<const uint4 *>(P.plane1 + row + k0);
         const uint4 mid4 = *reinterpret_cast<const uint4 *>(P.plane0 + row + k0);
         const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
         if (P.E_out) {
-            const uint4 up4 = *reinterpret_cast<const uint4 *>(P.plane0 + (size_t)iu * P.pitch + k0);
-            const uint4 dn4 = *reinterpret_cast<const uint4 *>(P.plane0 + (size_t)id * P.pitch + k0);
+            const uint4 up4 = *reinterpret_cast<const uint4 *>(P.plane0 + iu * P.pitch + k0);
+            const uint4 dn4 = *reinterpret_cast<const uint4 *>(P.plane0 + id * P.pitch + k0);
             const int ka = p ? wrap(k0 + 16, P.pitch) : wrap(k0 - 4, P.pitch);
             const uint32_t adj = *reinterpret_cast<const uint32_t *>(P.plane0 + row + ka);
             const uint32_t mid[6] = {adj, mid4.x, mid4.y, mid4.z, mid4.w, adj};
@@ -337,8 +343,9 @@ __global__ void __launch_bounds__(256) k_measure_u8(const MeasureParams P)
 // ---------------------------------------------------------------------------------------------
 // Random start (R9): s(i,j) = floor(w0 q / 2^32), (w0,..) = Philox((j, i, 0, 2), seed).
 // One thread per 4 consecutive k of one plane row.
+// L = rows of the planes; row0 = global index of their first row (0 unless the planes are a row strip; even).
 static __global__ void k_init_random_u8(uint8_t *plane0, uint8_t *plane1, int L, int pitch, uint32_t q,
-                                 uint32_t key0, uint32_t key1)
+                                 uint32_t key0, uint32_t key1, int row0 = 0)
 {
     const long long words_per_plane = (long long)L * (pitch >> 2);
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -351,7 +358,7 @@ static __global__ void k_init_random_u8(uint8_t *plane0, uint8_t *plane1, int L,
     uint32_t word = 0;
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
-        uint32_t ctr[4] = {2u * (uint32_t)(4 * kw + b) + p, (uint32_t)i, 0u, 2u};
+        uint32_t ctr[4] = {2u * (uint32_t)(4 * kw + b) + p, (uint32_t)(i + row0), 0u, 2u};
         philox4x32_10(ctr, key0, key1);
         word |= __umulhi(ctr[0], q) << (8 * b);
     }
