@@ -54,7 +54,7 @@ constexpr int MAX_CTAS = 160;             // upper bound on the resident kernel'
 constexpr int RESIDENT_L_MAX = 4096;       // largest lattice the resident kernel can hold (512 words per row)
 constexpr int CLUSTER_AUTO_L_MAX = 128;    // lattices up to this size go to the cluster (DSMEM) kernel by default (measured: 2x the resident kernel)
 constexpr int ACC_WORDS = 1 + 256 + 2;    // E, hist[256], flag/error word, tile counter of the streaming kernels
-constexpr size_t STATIC_SMEM = sizeof(potts::AcceptLut) + 1024;   // static shared memory of the persistent kernels
+constexpr size_t STATIC_SMEM = sizeof(potts::AcceptLutWide) + 1024;   // static shared memory of the persistent kernels
 
 }  // namespace
 

@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) uint8_t s_raw[];
-    __shared__ AcceptLut lut;
+    __shared__ AcceptLutWide lut;
 
     const uint32_t G = cluster.num_blocks(), b = cluster.block_rank();
     const int L = P.L, pitch = P.pitch;
@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
     const uint32_t q = in_register(P.q);
 
     accept_lut_fill(&lut, P.thr, tid, nthreads);
-    const uint32_t lane_off = accept_lane_offset(tid);
+    const uint32_t lane_off = accept_lane_offset<AcceptLutWide::slots>(tid);
     if (do_hist)
         for (uint32_t n = tid; n < 2u * hist_words(P.q); n += nthreads) s_hist0[n] = 0u;
     {
@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
                     horizontal(p, mid, adj, lf, rt);
                     const RowKeys R = row_keys(K, i);
                     uint32_t code, mask;
-                    const uint32_t out = update_word<CM, ST>(own, up, dn, lf, rt, 2u * col + p, q, K, R, &lut, lane_off, code, mask);
+                    const uint32_t out = update_word<CM, ST, AcceptLutWide::slots>(own, up, dn, lf, rt, 2u * col + p, q, K, R, &lut, lane_off, code, mask);
                     if (count_E) ne_sum += ne_final_sum(code, mask);
                     if (do_D) d_sum += delta_sum(code, mask);
                     *reinterpret_cast<uint32_t *>(own_col + ro) = out;

@@ -326,19 +326,26 @@ __device__ __forceinline__ void horizontal(uint32_t p, uint32_t mid, uint32_t ad
 // so that the high word of  w1 + entry  is 0xffffffff iff w1 < threshold(d) and 0 otherwise: exact for every
 // threshold in [0, 2^32].  The 32 lanes of a warp look up 32 different codes, so a single copy of the table
 // would serialise on its banks (measured: the 9-word table of round 1 never did); the table is therefore stored
-// in ACCEPT_SLOTS copies, entry (code, slot) at byte code * 8 * ACCEPT_SLOTS + slot * 8, and lane l reads slot
-// l % ACCEPT_SLOTS: the 16 lanes of a half-warp meet on a bank pair only if they share a slot AND differ in code.
+// in SLOTS copies, entry (code, slot) at byte code * 8 * SLOTS + slot * 8, and lane l reads slot
+// l % SLOTS: the 16 lanes of a half-warp meet on a bank pair only if they share a slot AND differ in code.
 constexpr int ACCEPT_ENTRIES = 256;
-constexpr int ACCEPT_SLOTS = 8;
-constexpr int ACCEPT_SHIFT = 6;                                 // log2(8 bytes * ACCEPT_SLOTS)
-struct AcceptLut { uint2 e[ACCEPT_ENTRIES][ACCEPT_SLOTS]; };    // 16 KB
+template <int SLOTS>
+struct AcceptLutT {
+    static_assert(SLOTS == 4 || SLOTS == 8 || SLOTS == 16, "slot copies: 4, 8 or 16");
+    static constexpr int slots = SLOTS;
+    static constexpr int shift = SLOTS == 4 ? 5 : (SLOTS == 8 ? 6 : 7);     // log2(8 bytes * SLOTS)
+    uint2 e[ACCEPT_ENTRIES][SLOTS];
+};
+using AcceptLut = AcceptLutT<8>;           // streaming kernels: 16 KB beside the 16 KB of ColKeys
+using AcceptLutWide = AcceptLutT<16>;      // persistent kernels: 32 KB, no two lanes of a half-warp share a slot
 
 // fast = true (allowed only if every thr[d] >= 1, i.e. no "never accept" entry): the entry's first word is
 // threshold(d) - 1 instead, and a site accepts iff w1 <= that word (0xffffffff for d <= 0): one 32-bit compare.
-__device__ __forceinline__ void accept_lut_fill(AcceptLut *lut, const uint32_t thr[4], uint32_t tid, uint32_t nthreads, bool fast = false)
+template <int SLOTS>
+__device__ __forceinline__ void accept_lut_fill(AcceptLutT<SLOTS> *lut, const uint32_t thr[4], uint32_t tid, uint32_t nthreads, bool fast = false)
 {
-    for (uint32_t n = tid; n < (uint32_t)(ACCEPT_ENTRIES * ACCEPT_SLOTS); n += nthreads) {
-        const uint32_t code = n / ACCEPT_SLOTS;
+    for (uint32_t n = tid; n < (uint32_t)(ACCEPT_ENTRIES * SLOTS); n += nthreads) {
+        const uint32_t code = n / SLOTS;
         const int d = __popc(code >> 4) - __popc(code & 15u);
         const unsigned long long th = d <= 0 ? (1ull << 32) : (unsigned long long)(d == 1 ? thr[0] : (d == 2 ? thr[1] : (d == 3 ? thr[2] : thr[3])));
         const unsigned long long e = fast ? th - 1ull : 0ull - th;
@@ -349,11 +356,14 @@ __device__ __forceinline__ void accept_lut_fill(AcceptLut *lut, const uint32_t t
 __host__ __device__ inline bool accept_fast_ok(const uint32_t thr[4]) { return thr[0] && thr[1] && thr[2] && thr[3]; }
 
 // byte offset of this lane's slot inside a table row
-__device__ __forceinline__ uint32_t accept_lane_offset(uint32_t lane) { return (lane % ACCEPT_SLOTS) * 8u; }
+template <int SLOTS = 8>
+__device__ __forceinline__ uint32_t accept_lane_offset(uint32_t lane) { return (lane % SLOTS) * 8u; }
 
 // accept masks of the four sites of a word: byte b = 0xff iff site b accepts its proposal
-__device__ __forceinline__ uint32_t accept_mask(uint32_t code, const uint32_t w1[4], const AcceptLut *lut, uint32_t lane_off)
+template <int SLOTS>
+__device__ __forceinline__ uint32_t accept_mask(uint32_t code, const uint32_t w1[4], const AcceptLutT<SLOTS> *lut, uint32_t lane_off)
 {
+    constexpr int ACCEPT_SHIFT = AcceptLutT<SLOTS>::shift;
     constexpr uint32_t M = 0xffu << ACCEPT_SHIFT;
     uint32_t a[4];
 #pragma unroll
@@ -371,9 +381,11 @@ __device__ __forceinline__ uint32_t accept_mask(uint32_t code, const uint32_t w1
 }
 
 // Fast form (table filled with fast = true): the new word directly, one compare and one predicated byte insert per site.
-__device__ __forceinline__ uint32_t accept_insert(uint32_t own, uint32_t prop, uint32_t code, const uint32_t w1[4], const AcceptLut *lut,
+template <int SLOTS>
+__device__ __forceinline__ uint32_t accept_insert(uint32_t own, uint32_t prop, uint32_t code, const uint32_t w1[4], const AcceptLutT<SLOTS> *lut,
                                                   uint32_t lane_off)
 {
+    constexpr int ACCEPT_SHIFT = AcceptLutT<SLOTS>::shift;
     constexpr uint32_t M = 0xffu << ACCEPT_SHIFT;
     uint32_t out = own;
 #pragma unroll
@@ -407,9 +419,9 @@ __device__ __forceinline__ int delta_sum(uint32_t code, uint32_t mask)
 //   nb[4]    the 4 neighbour words (up, down, left, right: any order), prepared by prep_nbr<CM>
 //   w0, w1   Philox words of the 4 sites: proposal and acceptance
 // Returns the new word; code / mask = the word's code bytes and accept mask for ne_final_sum / delta_sum.
-template <int CM, bool FAST = false>
+template <int CM, bool FAST = false, int SLOTS = 8>
 __device__ __forceinline__ uint32_t metropolis_word(uint32_t own, const uint32_t nb[4], uint32_t q, const uint32_t w0[4],
-                                                    const uint32_t w1[4], const AcceptLut *lut, uint32_t lane_off,
+                                                    const uint32_t w1[4], const AcceptLutT<SLOTS> *lut, uint32_t lane_off,
                                                     uint32_t &code, uint32_t &mask)
 {
     // R4: proposal floor(w0 q / 2^32), packed one byte per site
@@ -445,15 +457,15 @@ __device__ __forceinline__ void draw_words(const HalfSweepKeys &K, const RowKeys
 }
 
 // One word of the update from the neighbour words as loaded (byte b = that neighbour of site b).
-template <int CM, int ST>
+template <int CM, int ST, int SLOTS>
 __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
                                                 uint32_t j0, uint32_t q, const HalfSweepKeys &K, const RowKeys &R,
-                                                const AcceptLut *lut, uint32_t lane_off, uint32_t &code, uint32_t &mask)
+                                                const AcceptLutT<SLOTS> *lut, uint32_t lane_off, uint32_t &code, uint32_t &mask)
 {
     uint32_t w0[4], w1[4];
     draw_words<ST>(K, R, j0, w0, w1);
     const uint32_t nb[4] = {prep_nbr<CM>(up), prep_nbr<CM>(dn), prep_nbr<CM>(lf), prep_nbr<CM>(rt)};
-    return metropolis_word<CM>(own, nb, q, w0, w1, lut, lane_off, code, mask);
+    return metropolis_word<CM, false, SLOTS>(own, nb, q, w0, w1, lut, lane_off, code, mask);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -106,7 +106,7 @@ template <int CM, int W, int ST>
 __device__ __forceinline__ void resident_run(const ResidentParams &P, const ResidentLattice &X)
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
-    __shared__ AcceptLut lut;
+    __shared__ AcceptLutWide lut;
 
     const uint32_t G = X.G, b = X.b;
     const int L = P.L, pitch = P.pitch;
@@ -149,7 +149,7 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
     const bool do_D = X.dE_series != nullptr;
 
     accept_lut_fill(&lut, X.thr, tid, nthreads);
-    const uint32_t lane_off = accept_lane_offset(tid);
+    const uint32_t lane_off = accept_lane_offset<AcceptLutWide::slots>(tid);
     if (do_hist)
         for (uint32_t n = tid; n < hist_words(P.q); n += nthreads) s_hist[n] = 0u;
     // own rows of both planes, and the halo rows of plane 1 (read by the first half-sweep, colour 0):
@@ -216,8 +216,8 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                         horizontal(p, mid.x, p ? mid.y : adj, lf0, rt0);
                         horizontal(p, mid.y, p ? adj : mid.x, lf1, rt1);
                         uint32_t code0, mask0, code1, mask1;
-                        out.x = update_word<CM, ST>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, &lut, lane_off, code0, mask0);
-                        out.y = update_word<CM, ST>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, &lut, lane_off, code1, mask1);
+                        out.x = update_word<CM, ST, AcceptLutWide::slots>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, &lut, lane_off, code0, mask0);
+                        out.y = update_word<CM, ST, AcceptLutWide::slots>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, &lut, lane_off, code1, mask1);
                         if (count_E) ne_sum += ne_final_sum(code0, mask0) + ne_final_sum(code1, mask1);
                         if (do_D) d_sum += delta_sum(code0, mask0) + delta_sum(code1, mask1);
                         *reinterpret_cast<uint2 *>(own_col + ro) = out;
@@ -231,7 +231,7 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                         uint32_t lf, rt;
                         horizontal(p, mid, adj, lf, rt);
                         uint32_t code, mask;
-                        out.x = update_word<CM, ST>(own, up, dn, lf, rt, 2u * col + p, q, K, R, &lut, lane_off, code, mask);
+                        out.x = update_word<CM, ST, AcceptLutWide::slots>(own, up, dn, lf, rt, 2u * col + p, q, K, R, &lut, lane_off, code, mask);
                         if (count_E) ne_sum += ne_final_sum(code, mask);
                         if (do_D) d_sum += delta_sum(code, mask);
                         out.y = 0u;
