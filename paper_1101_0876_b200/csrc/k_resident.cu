@@ -9,6 +9,9 @@ namespace {
 template <int CM, int ST>
 const void *resident_kernel_st(int W, int small)
 {
+    if (W == 3)          // W = 2 with the ColKeys table (potts_resident.cuh, COL)
+        return small == 2 ? (const void *)k_resident_u8<CM, 2, ST, 576, true>
+                          : (small == 1 ? (const void *)k_resident_u8<CM, 2, ST, 768, true> : (const void *)k_resident_u8<CM, 2, ST, 1024, true>);
     if (W == 1) return small == 2 ? (const void *)k_resident_u8<CM, 1, ST, 576> : (const void *)k_resident_u8<CM, 1, ST, 1024>;
     return small == 2 ? (const void *)k_resident_u8<CM, 2, ST, 576>
                       : (small == 1 ? (const void *)k_resident_u8<CM, 2, ST, 768> : (const void *)k_resident_u8<CM, 2, ST, 1024>);

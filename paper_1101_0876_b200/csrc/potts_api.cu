@@ -96,6 +96,7 @@ struct potts_s {
     int64_t opt_resident_rows = 0;       // 0 auto, else at most this many thread rows in a resident block
     int64_t opt_cluster_ctas = 0;        // 0 auto, else the cluster kernel's cluster size (1..16)
     int cluster_checked = 0;             // cluster size whose co-residency was confirmed (cudaOccupancyMaxActiveClusters)
+    int64_t opt_resident_col = 1;        // 1: ColKeys table in the resident kernel where it pays; 0: never
     int64_t opt_stream_stage = 0;        // 0: other-colour rows through registers; 1: staged in shared memory by cp.async.bulk (experiment)
     int64_t opt_stream_rows = 0;         // 0 auto, else rows per warp of the streaming kernel (even, divides L/4)
 };
@@ -274,6 +275,8 @@ struct ResidentPlan {
     bool ok = false;
     int G = 0, tyc = 0, wpr = 0, rows_max = 0, nthreads = 0, W = 2;
     size_t smem = 0;
+    bool col = false;                    // ColKeys table in shared memory (W = 2, >= 3 visits per thread)
+    uint32_t col_offset = 0;
     const char *why = "";
 };
 
@@ -339,6 +342,14 @@ ResidentPlan plan_resident(const potts_t *h)
     const size_t hist = (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4;
     R.smem = 2 * (size_t)(R.rows_max + 2) * (L / 2) + hist;
     if (R.smem + STATIC_SMEM > h->smem_optin) { R.why = "lattice does not fit the shared memory of the grid"; return R; }
+    // the column part of Philox shared by a thread's visits of a half-sweep: 16 L bytes more, if they fit
+    const int visits = (R.rows_max + tyc - 1) / tyc;
+    const size_t col_at = (R.smem + 15) / 16 * 16;
+    if (R.W == 2 && visits >= 3 && h->opt_resident_col != 0 && col_at + 16 * (size_t)L + STATIC_SMEM <= h->smem_optin) {
+        R.col = true;
+        R.col_offset = (uint32_t)col_at;
+        R.smem = col_at + 16 * (size_t)L;
+    }
     R.ok = true;
     return R;
 }
@@ -365,7 +376,8 @@ int launch_resident(potts_t *h, const ResidentPlan &R, const uint32_t thr[4], in
     P.error = h->error;
     P.rows_max = R.rows_max;
     P.tyc = R.tyc;
-    const void *fn = potts::resident_kernel(potts::compare_mode_of(h->q), h->stream_spec, R.W, R.nthreads <= 576 ? 2 : (R.nthreads <= 768 ? 1 : 0));
+    P.col_offset = R.col_offset;
+    const void *fn = potts::resident_kernel(potts::compare_mode_of(h->q), h->stream_spec, R.col ? 3 : R.W, R.nthreads <= 576 ? 2 : (R.nthreads <= 768 ? 1 : 0));
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
     int per_sm = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, R.nthreads, R.smem));
@@ -1111,6 +1123,10 @@ int potts_set_option(potts_t *h, const char *key, int64_t value)
         if (value < 0 || value > 2) return fail(POTTS_ERR_ARG, "resident_words must be 0 (auto), 1 or 2");
         h->opt_resident_words = value; return POTTS_OK;
     }
+    if (!std::strcmp(key, "resident_col")) {
+        if (value < 0 || value > 1) return fail(POTTS_ERR_ARG, "resident_col must be 0 or 1");
+        h->opt_resident_col = value; return POTTS_OK;
+    }
     if (!std::strcmp(key, "stream_stage")) {
         if (value < 0 || value > 1) return fail(POTTS_ERR_ARG, "stream_stage must be 0 (registers) or 1 (cp.async.bulk staging)");
         h->opt_stream_stage = value; return POTTS_OK;
@@ -1134,6 +1150,7 @@ int potts_get_option(potts_t *h, const char *key, int64_t *value)
     if (!std::strcmp(key, "cluster_ctas")) { *value = h->opt_cluster_ctas; return POTTS_OK; }
     if (!std::strcmp(key, "stream_rows")) { *value = h->opt_stream_rows; return POTTS_OK; }
     if (!std::strcmp(key, "stream_stage")) { *value = h->opt_stream_stage; return POTTS_OK; }
+    if (!std::strcmp(key, "resident_col")) { *value = h->opt_resident_col; return POTTS_OK; }
     if (!std::strcmp(key, "cluster_active")) {             // read-only: cluster size the next sweep call would use (0 = not the cluster kernel)
         const bool want = h->opt_variant == 3 || (h->opt_variant == 0 && h->layout == POTTS_LAYOUT_U8 && h->L <= CLUSTER_AUTO_L_MAX);
         *value = (want && plan_cluster(h).ok) ? plan_cluster(h).G : 0; return POTTS_OK;

@@ -468,6 +468,33 @@ __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint3
     return metropolis_word<CM, false, SLOTS>(own, nb, q, w0, w1, lut, lane_off, code, mask);
 }
 
+// The same with the column part of Philox read from a table: ck[b * ck_stride] = ColKeys of the word's column b, in the
+// row parity of this visit (persistent kernels that visit a column often enough to share it: L >= 2048).
+template <int CM, int ST, int SLOTS>
+__device__ __forceinline__ uint32_t update_word_h(uint32_t own, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
+                                                  const uint4 *ck, uint32_t ck_stride, uint32_t q, const HalfSweepKeys &K, const RowKeysH &R,
+                                                  const AcceptLutT<SLOTS> *lut, uint32_t lane_off, uint32_t &code, uint32_t &mask)
+{
+    uint32_t w0[4], w1[4];
+    if (ST == 1) {
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const uint4 c = ck[b * ck_stride];
+            philox_site_h(K, R, ColKeys{c.x, c.y, c.z, c.w}, w0[b], w1[b]);
+        }
+    } else {
+#pragma unroll
+        for (int m = 0; m < 2; ++m) {
+            const uint4 c = ck[2 * m * ck_stride];
+            uint32_t w[4];
+            philox_pair_h(K, R, ColKeys{c.x, c.y, c.z, c.w}, w);
+            w0[2 * m] = w[0]; w1[2 * m] = w[1]; w0[2 * m + 1] = w[2]; w1[2 * m + 1] = w[3];
+        }
+    }
+    const uint32_t nb[4] = {prep_nbr<CM>(up), prep_nbr<CM>(dn), prep_nbr<CM>(lf), prep_nbr<CM>(rt)};
+    return metropolis_word<CM, false, SLOTS>(own, nb, q, w0, w1, lut, lane_off, code, mask);
+}
+
 // ---------------------------------------------------------------------------------------------
 // Standalone measurement helpers: byte-parallel "not equal" flags (bit 7 of every byte of the result is
 // set iff the bytes of a and b differ).  WIDE = false assumes all spin values < 128.

@@ -52,6 +52,7 @@ struct ResidentParams {
     int *error;                       // set to 1 if a wait gave up
     int32_t rows_max;                 // rows of shared memory per plane = rows_max + 2
     int32_t tyc;                      // thread rows that compute
+    uint32_t col_offset;              // COL kernels: byte offset of the ColKeys table (2 x pitch entries of 16 bytes) in the dynamic shared memory
 };
 
 constexpr long long RESIDENT_SPIN_LIMIT = 1ll << 24;   // polls before a wait gives up (seconds)
@@ -102,9 +103,12 @@ struct ResidentLattice {
 
 // W = words (4 sites each) a compute thread updates per row visit: 2 (an 8-site chunk: less bookkeeping per site) or
 // 1 (finer grain: the host picks it where chunks would leave the four sub-partitions of an SM unevenly loaded).
-template <int CM, int W, int ST>
+// COL (W = 2 only): the column part of Philox (ColKeys) of all L columns is rebuilt at the start of every half-sweep
+// into shared memory and shared by the rows a thread visits: pays from ~3 visits per thread and half-sweep (L >= 2048).
+template <int CM, int W, int ST, bool COL = false>
 __device__ __forceinline__ void resident_run(const ResidentParams &P, const ResidentLattice &X)
 {
+    static_assert(!COL || W == 2, "ColKeys table: chunk-grained kernel only");
     extern __shared__ __align__(16) uint8_t s_raw[];
     __shared__ AcceptLutWide lut;
 
@@ -196,8 +200,23 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
             int d_sum = 0, ne_sum = 0;                              // energy change / unequal neighbours of the final spins
             uint32_t words_done = 0;
             const bool count_E = sample && c == 1 && do_E, count_H = sample && do_hist;
+            if (COL) {
+                // every thread of the block (comm warps too) rebuilds the table for (t, c); nobody reads the old one any more
+                // (the barrier that ended the previous half-sweep), nobody reads the new one before the barrier below
+                const HalfSweepKeys Kc = half_sweep_keys(X.key0, X.key1, t, c);
+                uint4 *const tab = reinterpret_cast<uint4 *>(s_raw + P.col_offset);
+                for (uint32_t n = tid; n < 2u * (uint32_t)pitch; n += nthreads) {
+                    // entry (par, s, cx) = column 2 (8 cx + s) + par: the lanes of a warp (consecutive cx) read consecutive entries
+                    const uint32_t par = n >= (uint32_t)pitch ? 1u : 0u, m = n - par * (uint32_t)pitch;
+                    const uint32_t sx = m / (uint32_t)cpr, cxx = m - sx * (uint32_t)cpr;
+                    const ColKeys C = col_keys(Kc, 2u * (8u * cxx + sx) + par);
+                    tab[n] = make_uint4(C.l0, C.l1, C.ph, C.pl);
+                }
+                __syncthreads();
+            }
             if ((int)tid < nbar) {
                 const HalfSweepKeys K = half_sweep_keys(X.key0, X.key1, t, c);             // uniform registers
+                const uint4 *const s_col = reinterpret_cast<const uint4 *>(s_raw + P.col_offset);
                 // one visit: local row lr, my W words
                 auto update = [&](int lr) -> uint2 {
                     const uint32_t ro = (uint32_t)(lr * pitch);
@@ -216,8 +235,15 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                         horizontal(p, mid.x, p ? mid.y : adj, lf0, rt0);
                         horizontal(p, mid.y, p ? adj : mid.x, lf1, rt1);
                         uint32_t code0, mask0, code1, mask1;
-                        out.x = update_word<CM, ST, AcceptLutWide::slots>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, &lut, lane_off, code0, mask0);
-                        out.y = update_word<CM, ST, AcceptLutWide::slots>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, &lut, lane_off, code1, mask1);
+                        if (COL) {
+                            const RowKeysH RH = {R.xd, R.c3 ^ K.r1[2]};
+                            const uint4 *const ck = s_col + p * (uint32_t)pitch + (uint32_t)cx;   // + s * cpr: site s of my chunk
+                            out.x = update_word_h<CM, ST, AcceptLutWide::slots>(own.x, up.x, dn.x, lf0, rt0, ck, (uint32_t)cpr, q, K, RH, &lut, lane_off, code0, mask0);
+                            out.y = update_word_h<CM, ST, AcceptLutWide::slots>(own.y, up.y, dn.y, lf1, rt1, ck + 4 * cpr, (uint32_t)cpr, q, K, RH, &lut, lane_off, code1, mask1);
+                        } else {
+                            out.x = update_word<CM, ST, AcceptLutWide::slots>(own.x, up.x, dn.x, lf0, rt0, 2u * col + p, q, K, R, &lut, lane_off, code0, mask0);
+                            out.y = update_word<CM, ST, AcceptLutWide::slots>(own.y, up.y, dn.y, lf1, rt1, 2u * col + 8u + p, q, K, R, &lut, lane_off, code1, mask1);
+                        }
                         if (count_E) ne_sum += ne_final_sum(code0, mask0) + ne_final_sum(code1, mask1);
                         if (do_D) d_sum += delta_sum(code0, mask0) + delta_sum(code1, mask1);
                         *reinterpret_cast<uint2 *>(own_col + ro) = out;
@@ -327,7 +353,7 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
 }
 
 // One lattice over the whole grid (cooperative launch: the CTAs wait for each other's packets).
-template <int CM, int W, int ST, int MAXT>     // MAXT: block size the registers are budgeted for (576 -> 112 registers)
+template <int CM, int W, int ST, int MAXT, bool COL = false>     // MAXT: block size the registers are budgeted for (576 -> 112 registers)
 __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__ ResidentParams P)
 {
     ResidentLattice X;
@@ -342,7 +368,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident_u8(const __grid_constant__
     X.E_series = P.E_series;
     X.hist_series = P.hist_series;
     X.dE_series = P.dE_series;
-    resident_run<CM, W, ST>(P, X);
+    resident_run<CM, W, ST, COL>(P, X);
 }
 
 // Replica batch: CTA r runs lattice r of a batch of independent lattices of the same (L, q), each with
