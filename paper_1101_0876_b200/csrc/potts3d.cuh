@@ -169,8 +169,7 @@ __global__ void __launch_bounds__(256) k_measure3_u8(const Measure3Params P)
         }
     }
     if (P.E_out) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
+        satisfied = __reduce_add_sync(0xffffffffu, satisfied);                     // one REDUX instead of a five-step shuffle tree
         if ((threadIdx.x & 31) == 0) atomicAdd(&blockE, (unsigned long long)satisfied);
     }
     __syncthreads();

@@ -112,14 +112,12 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
                 }
             if (do_D) {
                 int dd = d_sum;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) dd += __shfl_xor_sync(0xffffffffu, dd, o);
+                dd = __reduce_add_sync(0xffffffffu, dd);                     // one REDUX instead of a five-step shuffle tree
                 if ((tid & 31u) == 0 && dd) atomicAdd(P.dE_series + n, (unsigned long long)(long long)dd);
             }
             if (count_E) {
                 uint32_t satisfied = 16u * words_done - (uint32_t)ne_sum;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
+                satisfied = __reduce_add_sync(0xffffffffu, satisfied);                     // one REDUX instead of a five-step shuffle tree
                 if ((tid & 31u) == 0 && satisfied) atomicAdd(P.E_series + sample_idx, 0ull - (unsigned long long)satisfied);
             }
             cluster.sync();                                         // plane c and its halos complete everywhere

@@ -556,8 +556,7 @@ __device__ __forceinline__ void hist_flush(uint32_t *s_hist, uint32_t q, unsigne
         for (uint32_t k = warp; k < q; k += nwarps) {
             uint32_t v = s_hist[k * 32u + lane];
             s_hist[k * 32u + lane] = 0u;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            v = __reduce_add_sync(0xffffffffu, v);                     // one REDUX instead of a five-step shuffle tree
             if (lane == 0 && v) atomicAdd(hist_out + k, (unsigned long long)v);
         }
     } else {

@@ -252,8 +252,7 @@ __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_co
     if (EX) {
         // MEASURE: satisfied bonds = 4 per site - unequal neighbours of the final spins = 64 per row visit - acc
         int v = DELTA ? acc : 64 * rows_done - acc;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        v = __reduce_add_sync(0xffffffffu, v);                     // one REDUX instead of a five-step shuffle tree
         if (lane == 0) atomicAdd(&blockAcc, v);
         __syncthreads();
         // E = -(satisfied bonds): accumulate the two's-complement negative into the int64 slot; DELTA: += the change
@@ -331,8 +330,7 @@ __global__ void __launch_bounds__(256) k_measure_u8(const MeasureParams P)
         }
     }
     if (P.E_out) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
+        satisfied = __reduce_add_sync(0xffffffffu, satisfied);                     // one REDUX instead of a five-step shuffle tree
         if ((threadIdx.x & 31) == 0) atomicAdd(&blockE, (unsigned long long)satisfied);
     }
     __syncthreads();

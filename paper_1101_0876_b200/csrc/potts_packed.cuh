@@ -242,8 +242,7 @@ __global__ void __launch_bounds__(32 * PK_WARPS) k_sweep_rows_packed(const __gri
     if (EX) {
         // MEASURE: satisfied bonds = 4 per site - unequal neighbours of the final spins = 128 per row visit - acc; DELTA: the change
         int v = DELTA ? acc : 128 * rows_done - acc;
-#pragma unroll
-        for (int s = 16; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
+        v = __reduce_add_sync(0xffffffffu, v);                     // one REDUX instead of a five-step shuffle tree
         if (lane == 0) atomicAdd(&blockAcc, v);
         __syncthreads();
         if (tid == 0) atomicAdd(P.E_out, DELTA ? (unsigned long long)(long long)blockAcc : 0ull - (unsigned long long)(long long)blockAcc);
@@ -312,8 +311,7 @@ __global__ void __launch_bounds__(256) k_measure_packed(const PackedMeasureParam
         }
     }
     if (P.E_out) {
-#pragma unroll
-        for (int s = 16; s > 0; s >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, s);
+        satisfied = __reduce_add_sync(0xffffffffu, satisfied);                     // one REDUX instead of a five-step shuffle tree
         if ((threadIdx.x & 31) == 0) atomicAdd(&blockE, (unsigned long long)satisfied);
     }
     __syncthreads();

@@ -319,8 +319,7 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
             if (do_D) {
                 // energy change of this half-sweep = sum of d over its accepted moves (R5, R7): one int64 atomic per warp
                 int dd = d_sum;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) dd += __shfl_xor_sync(0xffffffffu, dd, o);
+                dd = __reduce_add_sync(0xffffffffu, dd);                     // one REDUX instead of a five-step shuffle tree
                 if ((tid & 31u) == 0 && dd) atomicAdd(X.dE_series + n, (unsigned long long)(long long)dd);
             }
             if (sample && c == 1) {
@@ -328,8 +327,7 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                     // satisfied bonds seen from this thread's black sites = 4 per site - unequal neighbours of the final
                     // spins (ne_sum); one fire-and-forget int64 atomic per warp: no block-wide barrier for the energy
                     uint32_t satisfied = 16u * words_done - (uint32_t)ne_sum;
-#pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) satisfied += __shfl_xor_sync(0xffffffffu, satisfied, o);
+                    satisfied = __reduce_add_sync(0xffffffffu, satisfied);                     // one REDUX instead of a five-step shuffle tree
                     if ((tid & 31u) == 0 && satisfied) atomicAdd(X.E_series + sample_idx, 0ull - (unsigned long long)satisfied);
                 }
                 if (do_hist) {
