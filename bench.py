@@ -518,10 +518,23 @@ def batch_of_cfg1(pb, torch, n=1184, repeats=3):
         t0 = time.perf_counter()
         b.potts_batch_sweep_measured(w.temperatures[0], w.sweeps_per_t, w.every)
         secs.append(time.perf_counter() - t0)
+    # the same with the series left on the device (potts_batch_sweep_measured_dev), CUDA events
+    E_dev = torch.zeros((n, w.sweeps_per_t // w.every), dtype=torch.int64, device="cuda")
+    H_dev = torch.zeros((n, w.sweeps_per_t // w.every, w.q), dtype=torch.int64, device="cuda")
+    ms_dev = []
+    for _ in range(repeats):
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        b.potts_batch_sweep_measured_dev(w.temperatures[0], w.sweeps_per_t, w.every, E_dev, H_dev)
+        e1.record()
+        torch.cuda.synchronize()
+        ms_dev.append(e0.elapsed_time(e1))
     b.close()
     sec = statistics.median(secs)
     ups = n * w.updates / sec
-    return {"lattices": n, "q": w.q, "L": w.L, "sweeps": w.sweeps_per_t, "seconds": sec, "seconds_min_max": [min(secs), max(secs)],
+    dev_ns = statistics.median(ms_dev) * 1e6 / (n * w.updates)
+    return {"series_on_device_ns_per_spin_flip": dev_ns, "lattices": n, "q": w.q, "L": w.L, "sweeps": w.sweeps_per_t, "seconds": sec, "seconds_min_max": [min(secs), max(secs)],
             "spin_updates_per_s": ups, "ns_per_spin_flip": 1e9 / ups, "kernel": "k_resident_batch_u8",
             "E_after_1000_sweeps_of_sample_0": e_last}
 

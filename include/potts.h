@@ -136,6 +136,9 @@ void potts_batch_destroy(potts_batch_t *b);
  * `every` is ignored.  Synchronises. */
 int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t every,
                                int64_t *E_series, int64_t *hist_series);
+/* The same with DEVICE series (int64, n rows of nsweeps/every entries / x q; zeroed by the call), no synchronisation. */
+int potts_batch_sweep_measured_dev(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t every,
+                                   int64_t *E_series_dev, int64_t *hist_series_dev);
 /* potts_batch_sweep_delta: nsweeps sweeps of every lattice; dE_series (host, n rows of nsweeps int64) receives for
  * every lattice and sweep the energy change summed over the accepted moves, as potts_sweep_delta. */
 int potts_batch_sweep_delta(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t *dE_series);

@@ -58,6 +58,7 @@ def load_library() -> ctypes.CDLL:
         "potts_batch_sweep_measured": ([vp, vp, i64, i64, vp, vp], ctypes.c_int),
         "potts_batch_download": ([vp, i32, vp], ctypes.c_int),
         "potts_batch_sweep_delta": ([vp, vp, i64, vp], ctypes.c_int),
+        "potts_batch_sweep_measured_dev": ([vp, vp, i64, i64, vp, vp], ctypes.c_int),
         "potts_batch_ladder": ([vp, vp, i32, i64, i64, i64, vp, vp], ctypes.c_int),
         "potts_batch_sweep_count": ([vp, P(u64)], ctypes.c_int),
         "potts_batch_launch_count": ([vp, P(u64)], ctypes.c_int),
@@ -119,7 +120,7 @@ EXPORTED_SYMBOLS = [
     "potts_download", "potts_upload", "potts_sweep_count", "potts_set_sweep_count", "potts_observables",
     "potts_magnetisation", "potts_susceptibility", "potts_launch_count", "potts_set_option", "potts_get_option", "potts_last_error",
     "potts_version", "potts_batch_workspace_bytes", "potts_batch_create", "potts_batch_destroy",
-    "potts_batch_sweep_measured", "potts_batch_sweep_delta", "potts_batch_ladder", "potts_batch_download", "potts_batch_sweep_count", "potts_batch_launch_count",
+    "potts_batch_sweep_measured", "potts_batch_sweep_measured_dev", "potts_batch_sweep_delta", "potts_batch_ladder", "potts_batch_download", "potts_batch_sweep_count", "potts_batch_launch_count",
     "potts_set_stream_spec", "potts_get_stream_spec", "potts_batch_set_stream_spec",
     "potts_create_strip", "potts_strip_half_sweep", "potts_strip_advance", "potts_strip_rows",
     "potts3_create", "potts3_destroy", "potts3_sweep", "potts3_sweep_measured", "potts3_energy", "potts3_histogram",
@@ -358,6 +359,13 @@ class PottsBatch:
         _check(self._lib.potts_batch_sweep_measured(self._h, Ta.ctypes.data, int(nsweeps), int(every),
                                                     E.ctypes.data if energy else None, H.ctypes.data if hist else None))
         return E, H
+
+    def potts_batch_sweep_measured_dev(self, T, nsweeps: int, every: int, E_dev, hist_dev=None):
+        """E_dev / hist_dev: torch.int64 CUDA tensors [n, nsweeps/every] / [n, nsweeps/every, q]; no sync."""
+        Ta = np.ascontiguousarray(np.broadcast_to(np.asarray(T, dtype=np.float64), (self.n,)))
+        _check(self._lib.potts_batch_sweep_measured_dev(self._h, Ta.ctypes.data, int(nsweeps), int(every),
+                                                        ctypes.c_void_p(E_dev.data_ptr()) if E_dev is not None else None,
+                                                        ctypes.c_void_p(hist_dev.data_ptr()) if hist_dev is not None else None))
 
     def potts_batch_sweep_delta(self, T, nsweeps: int) -> np.ndarray:
         """-> dE int64[n, nsweeps]: energy change of every sweep of every lattice, from its accepted moves."""

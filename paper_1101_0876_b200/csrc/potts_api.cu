@@ -1512,6 +1512,25 @@ int potts_batch_sweep_measured(potts_batch_t *b, const double *T, int64_t nsweep
     return batch_finish(b, rc, E_series, dev, eb, hist_series, dev + eb, hb);
 }
 
+int potts_batch_sweep_measured_dev(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t every, int64_t *E_series_dev,
+                                   int64_t *hist_series_dev)
+{
+    ON_DEVICE_OF(b);
+    if (!b || !T) return fail(POTTS_ERR_ARG, "null argument");
+    if (nsweeps < 0 || nsweeps > (1ll << 30)) return fail(POTTS_ERR_ARG, "nsweeps = %lld outside [0, 2^30]", (long long)nsweeps);
+    int rc = check_batch_T(b, T, b->n);
+    if (rc) return rc;
+    if (b->t + (uint64_t)nsweeps > 0xFFFFFFFFull) return fail(POTTS_ERR_ARG, "sweep counter would pass 2^32 - 1");
+    const bool measure = E_series_dev || hist_series_dev;
+    if (measure && (every < 1 || nsweeps % every != 0))
+        return fail(POTTS_ERR_ARG, "every = %lld must be >= 1 and divide nsweeps = %lld", (long long)every, (long long)nsweeps);
+    if (nsweeps == 0) return POTTS_OK;
+    const int64_t ns = measure ? nsweeps / every : 0;
+    if (E_series_dev) CUDA_TRY(cudaMemsetAsync(E_series_dev, 0, (size_t)b->n * ns * 8, b->stream));
+    if (hist_series_dev) CUDA_TRY(cudaMemsetAsync(hist_series_dev, 0, (size_t)b->n * ns * b->q * 8, b->stream));
+    return batch_run(b, T, 1, nsweeps, every, (unsigned long long *)E_series_dev, (unsigned long long *)hist_series_dev, ns, nullptr, 0);
+}
+
 int potts_batch_sweep_delta(potts_batch_t *b, const double *T, int64_t nsweeps, int64_t *dE_series)
 {
     ON_DEVICE_OF(b);

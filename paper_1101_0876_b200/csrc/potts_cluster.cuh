@@ -70,6 +70,7 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
     }
     cluster.sync();      // nobody writes a neighbour's halo before every CTA has loaded its start state
 
+    const HalfSweepKeys K0 = half_sweep_keys(P.key0, P.key1, 0u, 0u);
     uint32_t until = P.every, sample_idx = 0;
     for (uint32_t n = 0; n < P.nsweeps; ++n) {
         const uint32_t t = P.t0 + n;
@@ -79,7 +80,8 @@ __global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ 
         for (uint32_t c = 0; c < 2; ++c) {
             uint8_t *const own_col = s_raw + c * plane_stride + col;
             const uint8_t *const oth_row = s_raw + (1u - c) * plane_stride;
-            const HalfSweepKeys K = half_sweep_keys(P.key0, P.key1, t, c);
+            HalfSweepKeys K = K0;
+            half_sweep_rekey(K, P.key0, P.key1, t, c);
             const bool count_E = sample && c == 1 && do_E, count_H = sample && do_hist;
             int d_sum = 0, ne_sum = 0;
             uint32_t words_done = 0;

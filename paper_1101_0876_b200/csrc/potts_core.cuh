@@ -113,6 +113,15 @@ __host__ __device__ inline HalfSweepKeys half_sweep_keys(uint32_t key0, uint32_t
     return K;
 }
 
+// the (t, colour) part only: the round keys depend on the seed alone (persistent kernels build them once per launch)
+__host__ __device__ inline void half_sweep_rekey(HalfSweepKeys &K, uint32_t key0, uint32_t key1, uint32_t t, uint32_t colour)
+{
+    const unsigned long long p = (unsigned long long)PHILOX_M1 * (unsigned long long)t;
+    K.xa = (uint32_t)(p >> 32) ^ key0;
+    K.xb = colour ^ key1;
+    K.xc = (uint32_t)p ^ (key0 + PHILOX_W0);
+}
+
 struct RowKeys {
     uint32_t xd;      // hi(M0*(xa^i)) ^ k1[1]     c2 after round 2 is lo(M0*j) ^ xd
     uint32_t c3;      // lo(M0*(xa^i))             c3 after round 2

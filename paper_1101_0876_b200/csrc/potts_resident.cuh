@@ -185,6 +185,7 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
     const uint32_t cstride = 2u * wpr;
     const int halo_bar = 32 * nbw + ((int)nthreads - nbar);         // boundary warps + comm warps, in threads
 
+    const HalfSweepKeys K0 = half_sweep_keys(X.key0, X.key1, 0u, 0u);
     uint32_t until = P.every;                                       // sweeps until the next sample
     uint32_t sample_idx = 0;
     uint32_t seq = 0;                                               // launch-local half-sweep number, from 1
@@ -203,7 +204,8 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
             if (COL) {
                 // every thread of the block (comm warps too) rebuilds the table for (t, c); nobody reads the old one any more
                 // (the barrier that ended the previous half-sweep), nobody reads the new one before the barrier below
-                const HalfSweepKeys Kc = half_sweep_keys(X.key0, X.key1, t, c);
+                HalfSweepKeys Kc = K0;
+                half_sweep_rekey(Kc, X.key0, X.key1, t, c);
                 uint4 *const tab = reinterpret_cast<uint4 *>(s_raw + P.col_offset);
                 for (uint32_t n = tid; n < 2u * (uint32_t)pitch; n += nthreads) {
                     // entry (par, s, cx) = column 2 (8 cx + s) + par: the lanes of a warp (consecutive cx) read consecutive entries
@@ -215,7 +217,8 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                 __syncthreads();
             }
             if ((int)tid < nbar) {
-                const HalfSweepKeys K = half_sweep_keys(X.key0, X.key1, t, c);             // uniform registers
+                HalfSweepKeys K = K0;                                                       // uniform registers; round keys built once
+                half_sweep_rekey(K, X.key0, X.key1, t, c);
                 const uint4 *const s_col = reinterpret_cast<const uint4 *>(s_raw + P.col_offset);
                 // one visit: local row lr, my W words
                 auto update = [&](int lr) -> uint2 {

@@ -424,3 +424,20 @@ def test_streaming_kernel_with_bulk_staged_rows(pb, L, q, seed, rows):
     o.sweep(T, 2)
     assert (Eg == Eo).all() and (Hg == Ho).all()
     assert (g.potts_download() == o.spins()).all()
+
+
+def test_batch_series_on_the_device_equal_the_host_series(pb):
+    """potts_batch_sweep_measured_dev leaves the series on the device: same numbers as the host variant / the oracle."""
+    import torch
+    L, q, n, ns = 64, 9, 4, 12
+    seeds = [70 + r for r in range(n)]
+    Ts = [(0.95 + 0.03 * r) * workloads.t_c(q) for r in range(n)]
+    b = pb.PottsBatch(L, q, seeds, workloads.INIT_RANDOM)
+    E_dev = torch.full((n, ns // 2), 123, dtype=torch.int64, device="cuda")     # stale contents must be cleared by the call
+    H_dev = torch.full((n, ns // 2, q), 7, dtype=torch.int64, device="cuda")
+    b.potts_batch_sweep_measured_dev(Ts, ns, 2, E_dev, H_dev)
+    torch.cuda.synchronize()
+    for r in range(n):
+        o = oracle.OraclePotts(L, q, seeds[r], workloads.INIT_RANDOM)
+        Eo, Ho = o.sweep_measured(Ts[r], ns, 2, hist=True)
+        assert (E_dev[r].cpu().numpy() == Eo).all() and (H_dev[r].cpu().numpy() == Ho).all()
