@@ -216,6 +216,7 @@ int launch_half_sweep_packed(potts_t *h, uint32_t colour, const uint32_t thr[4],
     const int chunks = h->L / 64;
     const unsigned gx = (unsigned)((chunks + 31) / 32);
     P.rpw = h->opt_stream_rows > 0 ? (int)h->opt_stream_rows : STREAM_ROWS_PER_WARP;
+    while ((h->L / potts::PK_WARPS) % P.rpw) P.rpw >>= 1;               // L % 64 == 0: 2, 4 and 8 always divide
     P.row_groups = h->L / (potts::PK_WARPS * P.rpw);
     P.total_tiles = gx * (uint32_t)P.row_groups;
     P.tile_counter = h->tile_counter;
