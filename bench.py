@@ -430,10 +430,10 @@ def stream_spec_2_table(pb, torch, flush, peaks):
 
 
 def cubic_lattice(pb, torch, peaks, L=512, q=9, sweeps=40, repeats=3):
-    """SURVEY 8(f)4 / PAPER.md:359: the 3D generalisation (potts3_sweep, k_sweep3_u8: one launch per half-sweep, first
-    CUDA path of this row) on an L^3 lattice, random start, T = 1.3 (ordering phase); CUDA events around calls of
-    `sweeps` sweeps after a warm-up call, median.  Same algorithmic counts as the 2D path: 36 instructions and 3 bytes
-    per update."""
+    """SURVEY 8(f)4 / PAPER.md:359: the 3D generalisation (potts3_sweep, k_sweep3_rows_u8: one launch per half-sweep,
+    row-walking tiles at fixed z) on an L^3 lattice, random start, T = 1.3 (ordering phase); CUDA events around calls
+    of `sweeps` sweeps after a warm-up call, median.  Same algorithmic counts as the 2D path: 36 instructions and 3
+    bytes per update."""
     hbm_gbs, sm_max, which = peaks
     T = 1.3
     g = pb.Potts3D(L, q, 5, pb.INIT_RANDOM)
@@ -450,10 +450,10 @@ def cubic_lattice(pb, torch, peaks, L=512, q=9, sweeps=40, repeats=3):
     g.close()
     sec = statistics.median(ms) * 1e-3
     w = type("W", (), {"name": f"potts3d_q{q}_L{L}"})
-    r = roofline(w, "k_sweep3_u8", L ** 3 / 2, sec * 1e3 / (2 * sweeps), sm_max, hbm_gbs, which, BYTES_PER_UPDATE_U8)
+    r = roofline(w, "k_sweep3_rows_u8", L ** 3 / 2, sec * 1e3 / (2 * sweeps), sm_max, hbm_gbs, which, BYTES_PER_UPDATE_U8)
     ups = sweeps * L ** 3 / sec
     return {"q": q, "L": L, "sites": L ** 3, "sweeps_per_call": sweeps, "calls": repeats, "T": T, "ns_per_spin_flip": 1e9 / ups,
-            "spin_updates_per_s": ups, "ms_per_call_min_max": [min(ms), max(ms)], "kernel": "k_sweep3_u8", "roofline": r}
+            "spin_updates_per_s": ups, "ms_per_call_min_max": [min(ms), max(ms)], "kernel": "k_sweep3_rows_u8", "roofline": r}
 
 
 def second_neighbour_lattice(pb, torch, peaks, L=12288, q=9, sweeps=20, repeats=3):
@@ -578,13 +578,29 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default=f"cfg{HEADLINE}", help="cfg1..cfg5 (BASELINE.json configs[0..4])")
+    ap.add_argument("--workload", default=f"cfg{HEADLINE}",
+                    help="cfg1..cfg5 (BASELINE.json configs[0..4]); cubic / second_neighbour: that generalisation's row alone")
+    ap.add_argument("--lattice-L", type=int, default=0, help="L of --workload cubic / second_neighbour")
     ap.add_argument("--max-sweeps", type=int, default=None, help="time a bounded slice of the workload per step")
     ap.add_argument("--no-per-config", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--option", action="append", default=[], help="key=value passed to potts_set_option")
     args = ap.parse_args()
+    if args.workload in ("cubic", "second_neighbour"):
+        # one of the two generalisations alone (the ncu captures of profiles/ use this): prints that row only
+        import torch
+        import paper_1101_0876_b200 as pb
+        pb.load_library()
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+        fn = cubic_lattice if args.workload == "cubic" else second_neighbour_lattice
+        kw = {"L": args.lattice_L} if args.lattice_L else {}
+        if args.max_sweeps:
+            kw["sweeps"] = args.max_sweeps
+        print(json.dumps({"workload": args.workload, **fn(pb, torch, _peaks(), repeats=max(1, args.steps), **kw)}), flush=True)
+        return
     w = workloads.CONFIGS[int(args.workload.replace("cfg", ""))]
 
     if args.impl == "reference":
@@ -658,6 +674,7 @@ def main():
         per_cfg["delta_cfg1_cluster"] = delta_cost(pb, torch, 1, 2000)
         per_cfg["stream_spec_2"] = stream_spec_2_table(pb, torch, flush, peaks)
         per_cfg["potts3d_q9_L512"] = cubic_lattice(pb, torch, peaks)
+        per_cfg["potts3d_q9_L1024"] = cubic_lattice(pb, torch, peaks, L=1024, sweeps=10)      # 2^30 sites, as the headline
         per_cfg["potts8_q9_L12288"] = second_neighbour_lattice(pb, torch, peaks)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(w)

@@ -269,6 +269,14 @@ int  potts3_upload(potts3_t *h, const uint8_t *spins);
 int  potts3_sweep_count(potts3_t *h, uint64_t *t);
 int  potts3_set_sweep_count(potts3_t *h, uint64_t t);
 int  potts3_launch_count(potts3_t *h, uint64_t *n);
+/* potts3_set_option: launch knobs of the 3D half-sweep that never change WHAT it computes (tests assert bit-identity
+ * across them).  Unknown key or bad value -> POTTS_ERR_ARG.  Keys:
+ *   "stream_words"  0 = automatic (4; the one-chunk-per-thread kernel where a quarter of the lanes would idle, L = 3 2^k),
+ *                   1 / 2 / 4 = 4-site words a lane of the row-walking kernel k_sweep3_rows_u8 updates per row visit,
+ *                   -1 = the one-chunk-per-thread kernel k_sweep3_u8
+ *   "stream_rows"   0 = automatic (16, halved while a launch would have fewer than 1024 tiles), else rows a lane walks
+ *                   per tile (2, 4, 8, 16 or 32) */
+int  potts3_set_option(potts3_t *h, const char *key, int64_t value);
 
 /* ---- first AND second neighbour interactions (sec. 7: "For the 2D case with first and second neighbors
  * interactions, there are nine independent sub-networks to update instead of two") --------------------------------

@@ -12,6 +12,8 @@
 #pragma once
 #include "potts_core.cuh"
 
+#include <type_traits>
+
 namespace potts {
 
 struct Sweep3Params {
@@ -109,6 +111,247 @@ __global__ void __launch_bounds__(128) k_sweep3_u8(const __grid_constant__ Sweep
         }
         *reinterpret_cast<uint4 *>(P.plane_own + r_mid + k0) = make_uint4(out[0], out[1], out[2], out[3]);
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Row-walking form (the 2D streaming kernel k_sweep_rows_u8 carried to three dimensions).  A block of H3_WARPS
+// warps owns a tile of one z.  A lane updates 4 W same-colour sites per row visit and walks down a window of rpw rows
+// at fixed z: the other-colour rows y-1, y, y+1 of plane z roll through registers (one load per visit), the rows
+// (z-1, y) and (z+1, y) are two more loads.  A row narrower than a warp of such lanes (L < 256 W) takes 2^lpr_log2
+// lanes, and the 32 >> lpr_log2 lane groups of the warp walk different windows of the same columns, so that no lane
+// idles down to L = 32 W.  Every window starts at a row of parity (z & 1): the first visit of every tile has row
+// parity COLOUR and the parities are literals as in 2D.  ColKeys depend on z through
+// xb = (colour + 4 z) ^ key1: the table of the tile's columns is rebuilt whenever (column block, z) changes; tiles
+// are numbered (cb, z, row group) so that a block draws the row groups of one z in a row.
+//
+// Compare: the six "differs" flag words of a 4-site word are added bit-sliced by a carry-save tree of three-input
+// logic ops (8 for six neighbours) into the bit planes ones / twos / fours; code byte = c_old in bits 0-2 and c_new
+// in bits 4-6 (bits 3, 7 are garbage and masked out of the table offset).  Accept table: AcceptLut indexed by that
+// code, entry = 2^64 - threshold(c_new - c_old) (FAST: threshold - 1), as in 2D.
+constexpr int H3_WARPS = 4;
+constexpr uint32_t CODE3_BITS = 0x77u;
+
+struct Sweep3RowsParams {
+    uint8_t *plane_own;
+    const uint8_t *plane_oth;
+    int32_t L, pitch;
+    uint32_t q, key1;             // xb(z) = (colour + 4 z) ^ key1
+    HalfSweepKeys K;              // of (seed, t): xb is redone per z
+    uint32_t thr[6];              // threshold(d) for d = 1..6 (R6')
+    int32_t rpw, row_groups;      // rows per window; tiles per (column block, z)
+    int32_t lpr_log2;             // log2 of the lanes that cover a row (5 if the row is a warp wide or wider)
+    uint32_t total_tiles;
+    uint32_t *tile_counter;
+};
+
+__host__ __device__ inline bool accept_fast_ok3(const uint32_t thr[6]) { return thr[0] && thr[1] && thr[2] && thr[3] && thr[4] && thr[5]; }
+
+template <int SLOTS>
+__device__ __forceinline__ void accept_lut_fill3(AcceptLutT<SLOTS> *lut, const uint32_t thr[6], uint32_t tid, uint32_t nthreads, bool fast)
+{
+    for (uint32_t n = tid; n < (uint32_t)(128 * SLOTS); n += nthreads) {
+        const uint32_t code = n / SLOTS;
+        const int c_old = (int)(code & 7u), c_new = (int)((code >> 4) & 7u);
+        const int d = c_new - c_old > 6 ? 6 : c_new - c_old;          // counts of 7 never occur
+        const unsigned long long th = d <= 0 ? (1ull << 32) : (unsigned long long)thr[d - 1];
+        const unsigned long long e = fast ? th - 1ull : 0ull - th;
+        (&lut->e[0][0])[n] = make_uint2((uint32_t)e, (uint32_t)(e >> 32));
+    }
+}
+
+// carry-save count of six flag words: bit planes of the per-position sum (0..6)
+__device__ __forceinline__ void csa6(const uint32_t u[6], uint32_t &ones, uint32_t &twos, uint32_t &fours)
+{
+    constexpr int XOR3 = 0x96, MAJ = 0xE8;
+    const uint32_t s1 = lop3<XOR3>(u[0], u[1], u[2]), c1 = lop3<MAJ>(u[0], u[1], u[2]);
+    const uint32_t s2 = lop3<XOR3>(u[3], u[4], u[5]), c2 = lop3<MAJ>(u[3], u[4], u[5]);
+    ones = s1 ^ s2;
+    const uint32_t c3 = s1 & s2;
+    twos = lop3<XOR3>(c1, c2, c3);
+    fours = lop3<MAJ>(c1, c2, c3);
+}
+
+// code byte per site: bits 0-2 = neighbours that differ from the current spin, bits 4-6 = from the proposal
+template <int CM>
+__device__ __forceinline__ uint32_t ne_code6(uint32_t own, uint32_t prop, const uint32_t nb[6])
+{
+    if (is_nibble_mode(CM)) {
+        const uint32_t both = prop * 16u + own;
+        uint32_t u[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            if (CM == CM_NIB3) u[k] = (both ^ nb[k]) + 0x77777777u;
+            else u[k] = lop3<LOP_OR_XOR>(lop3<LOP_XOR_AND>(both, nb[k], 0x77777777u) + 0x77777777u, both, nb[k]);
+        }
+        uint32_t ones, twos, fours;                                    // flags in bits 3 and 7 of every byte
+        csa6(u, ones, twos, fours);
+        const uint32_t c = lop3<LOP_SEL>(ones >> 3, twos >> 2, 0x11111111u);
+        return lop3<LOP_SEL>(c, fours >> 1, 0x33333333u);
+    } else {
+        uint32_t o[6], n[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            if (CM == CM_7BIT) {
+                o[k] = (own ^ nb[k]) + 0x7f7f7f7fu;
+                n[k] = (prop ^ nb[k]) + 0x7f7f7f7fu;
+            } else {
+                o[k] = lop3<LOP_OR_XOR>(lop3<LOP_XOR_AND>(own, nb[k], 0x7f7f7f7fu) + 0x7f7f7f7fu, own, nb[k]);
+                n[k] = lop3<LOP_OR_XOR>(lop3<LOP_XOR_AND>(prop, nb[k], 0x7f7f7f7fu) + 0x7f7f7f7fu, prop, nb[k]);
+            }
+        }
+        uint32_t o1, o2, o4, n1, n2, n4;                               // flags in bit 7 of every byte
+        csa6(o, o1, o2, o4);
+        csa6(n, n1, n2, n4);
+        uint32_t a = lop3<LOP_SEL>(o1 >> 7, o2 >> 6, 0x01010101u);
+        a = lop3<LOP_SEL>(a, o4 >> 5, 0x03030303u);
+        uint32_t b = lop3<LOP_SEL>(n1 >> 3, n2 >> 2, 0x10101010u);
+        b = lop3<LOP_SEL>(b, n4 >> 1, 0x30303030u);
+        return lop3<LOP_SEL>(a, b, 0x0f0f0f0fu);
+    }
+}
+
+template <int W> struct Words3 { uint32_t w[W]; };
+
+template <int W>
+__device__ __forceinline__ Words3<W> ld_words3(const uint8_t *p)
+{
+    Words3<W> r;
+    if constexpr (W == 4) { const uint4 v = *reinterpret_cast<const uint4 *>(p); r.w[0] = v.x; r.w[1] = v.y; r.w[2] = v.z; r.w[3] = v.w; }
+    else if constexpr (W == 2) { const uint2 v = *reinterpret_cast<const uint2 *>(p); r.w[0] = v.x; r.w[1] = v.y; }
+    else r.w[0] = *reinterpret_cast<const uint32_t *>(p);
+    return r;
+}
+
+template <int W>
+__device__ __forceinline__ void st_words3(uint8_t *p, const uint32_t (&o)[W])
+{
+    if constexpr (W == 4) *reinterpret_cast<uint4 *>(p) = make_uint4(o[0], o[1], o[2], o[3]);
+    else if constexpr (W == 2) *reinterpret_cast<uint2 *>(p) = make_uint2(o[0], o[1]);
+    else *reinterpret_cast<uint32_t *>(p) = o[0];
+}
+
+template <int CM, int COLOUR, int W, bool FAST>
+__global__ void __launch_bounds__(32 * H3_WARPS) k_sweep3_rows_u8(const __grid_constant__ Sweep3RowsParams P)
+{
+    constexpr int SITES = 4 * W;                                      // same-colour sites per lane and row
+    __shared__ uint4 s_col[2][SITES][32];                             // ColKeys of [row parity][site of the chunk][lane]
+    __shared__ AcceptLut lut;
+    __shared__ uint32_t s_tile[2];
+    const uint32_t lane = threadIdx.x, wy = threadIdx.y, tid = wy * 32u + lane;
+    accept_lut_fill3(&lut, P.thr, tid, 32 * H3_WARPS, FAST);
+    const HalfSweepKeys &K = P.K;
+    const uint32_t lane_off = accept_lane_offset(lane);
+    const uint32_t q = in_register(P.q);
+    const int L = P.L, pitch = P.pitch, chunks = pitch / SITES;
+    const size_t plane_z = (size_t)L * pitch;                         // bytes of one z of a colour plane
+    int key_cur = -1;
+    for (uint32_t it = 0;; ++it) {
+    if (tid == 0) s_tile[it & 1u] = atomicInc(P.tile_counter, P.total_tiles + gridDim.x - 1u);
+    __syncthreads();                                                  // also: every thread is done with the previous tile
+    const uint32_t tile = s_tile[it & 1u];
+    if (tile >= P.total_tiles) break;
+    const int cz = (int)(tile / (uint32_t)P.row_groups), rg = (int)(tile - (uint32_t)cz * (uint32_t)P.row_groups);
+    const int cb = cz / L, z = cz - cb * L;
+    const int xl = (int)lane & ((1 << P.lpr_log2) - 1), sub = (int)lane >> P.lpr_log2;   // lane of the row, window of the warp
+    const int x = cb * 32 + xl;
+    const int win = ((rg * H3_WARPS + (int)wy) << (5 - P.lpr_log2)) + sub;                 // window of the plane
+    const bool active = x < chunks && win * P.rpw < L;
+    const int k0 = x * SITES;
+    if (cz != key_cur) {
+        key_cur = cz;
+        if (x < chunks && sub == 0) {
+            const uint32_t xb = ((uint32_t)COLOUR + 4u * (uint32_t)z) ^ P.key1;
+            for (int n = (int)wy; n < SITES; n += H3_WARPS) {
+#pragma unroll
+                for (int p = 0; p < 2; ++p) {
+                    const ColKeys C = col_keys(xb, K.xc, 2u * (uint32_t)(k0 + n) + (uint32_t)p);
+                    s_col[p][n][xl] = make_uint4(C.l0, C.l1, C.ph, C.pl);
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    if (active) {
+        const int ys = win * P.rpw + (z & 1);                         // first row of the window: parity of visit r is (r + COLOUR) & 1
+        const uint8_t *const oth_z = P.plane_oth + (size_t)z * plane_z + k0;
+        const uint8_t *const oth_lo = P.plane_oth + (size_t)wrap(z - 1, L) * plane_z + k0;
+        const uint8_t *const oth_hi = P.plane_oth + (size_t)wrap(z + 1, L) * plane_z + k0;
+        uint8_t *const own_z = P.plane_own + (size_t)z * plane_z + k0;
+        const int kn = wrap(k0 + SITES, pitch) - k0, kp = wrap(k0 - 4, pitch) - k0;
+        struct Loads { Words3<W> own, dn, lo, hi; uint32_t adj; };
+        auto load_row = [&](int y, int kadj) {
+            const size_t r = (size_t)wrap(y, L) * pitch;
+            Loads l;
+            l.own = ld_words3<W>(own_z + r);
+            l.dn = ld_words3<W>(oth_z + (size_t)wrap(wrap(y, L) + 1, L) * pitch);
+            l.lo = ld_words3<W>(oth_lo + r);
+            l.hi = ld_words3<W>(oth_hi + r);
+            l.adj = *reinterpret_cast<const uint32_t *>(oth_z + (ptrdiff_t)r + kadj);
+            return l;
+        };
+        auto prep = [](const Words3<W> &v, uint32_t (&w)[W]) {
+#pragma unroll
+            for (int n = 0; n < W; ++n) w[n] = prep_nbr<CM>(v.w[n]);
+        };
+        auto visit = [&](auto par, int y, const Loads &ld, const uint32_t (&up)[W], const uint32_t (&mid)[W], const uint32_t (&dn)[W]) {
+            constexpr int PAR = decltype(par)::value;
+            const int yw = wrap(y, L);
+            const RowKeysH R = row_keys_h(K, (uint32_t)yw);
+            const uint32_t adjp = prep_nbr<CM>(ld.adj);
+            uint32_t lo[W], hi[W], out[W];
+            prep(ld.lo, lo);
+            prep(ld.hi, hi);
+#pragma unroll
+            for (int n = 0; n < W; ++n) {
+                uint32_t nb[6];
+                nb[0] = up[n];
+                nb[1] = dn[n];
+                if (PAR) {
+                    nb[2] = mid[n];
+                    nb[3] = __funnelshift_r(mid[n], n < W - 1 ? mid[n < W - 1 ? n + 1 : W - 1] : adjp, 8);
+                } else {
+                    nb[2] = __funnelshift_l(n > 0 ? mid[n > 0 ? n - 1 : 0] : adjp, mid[n], 8);
+                    nb[3] = mid[n];
+                }
+                nb[4] = lo[n];
+                nb[5] = hi[n];
+                uint32_t w0[4], w1[4];
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const uint4 c = s_col[PAR][4 * n + b][xl];
+                    philox_site_h(K, R, ColKeys{c.x, c.y, c.z, c.w}, w0[b], w1[b]);
+                }
+                const uint32_t s01 = __byte_perm(__umulhi(w0[0], q), __umulhi(w0[1], q), 0x0040);
+                const uint32_t s23 = __byte_perm(__umulhi(w0[2], q), __umulhi(w0[3], q), 0x0040);
+                const uint32_t prop = __byte_perm(s01, s23, 0x5410);                       // R4
+                const uint32_t code = ne_code6<CM>(ld.own.w[n], prop, nb);                 // R5'
+                if (FAST) out[n] = accept_insert<8, CODE3_BITS>(ld.own.w[n], prop, code, w1, &lut, lane_off);   // R6', R7
+                else out[n] = lop3<LOP_SEL>(prop, ld.own.w[n], accept_mask<8, CODE3_BITS>(code, w1, &lut, lane_off));
+            }
+            st_words3<W>(own_z + (size_t)yw * pitch, out);
+        };
+
+        uint32_t up[W], mid[W], dn[W], dn2[W];
+        prep(ld_words3<W>(oth_z + (size_t)wrap(ys - 1, L) * pitch), up);
+        prep(ld_words3<W>(oth_z + (size_t)wrap(ys, L) * pitch), mid);
+        constexpr int PA = COLOUR, PB = 1 - COLOUR;
+        const int k_a = PA ? kn : kp, k_b = PB ? kn : kp;
+        Loads a = load_row(ys, k_a);
+#pragma unroll 1
+        for (int r = 0; r < P.rpw; r += 2) {
+            const int y = ys + r;
+            const Loads b = load_row(y + 1, k_b);
+            prep(a.dn, dn);
+            visit(std::integral_constant<int, PA>{}, y, a, up, mid, dn);
+            a = load_row(r + 2 < P.rpw ? y + 2 : y + 1, k_a);
+            prep(b.dn, dn2);
+            visit(std::integral_constant<int, PB>{}, y + 1, b, mid, dn, dn2);
+#pragma unroll
+            for (int n = 0; n < W; ++n) { up[n] = dn[n]; mid[n] = dn2[n]; }
+        }
+    }
+    }   // tiles
 }
 
 // Energy (from the colour-1 sites: every bond joins the two colours) and histogram of both planes.

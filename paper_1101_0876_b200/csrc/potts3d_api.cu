@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstring>
 #include <new>
 
 namespace potts {
@@ -54,11 +55,13 @@ struct potts3_s {
     uint8_t *ws = nullptr;
     size_t plane_bytes = 0;
     uint8_t *plane[2] = {nullptr, nullptr};
-    unsigned long long *acc = nullptr;     // device: [0] = E, [1..256] = histogram, [257] = upload flag
+    unsigned long long *acc = nullptr;     // device: [0] = E, [1..256] = histogram, [257] = upload flag, [258] = tile counter
     uint8_t *scratch = nullptr;            // device: series of a measured call / staging of up- and download
     size_t scratch_bytes = 0;
     cudaStream_t stream = nullptr;
     int num_sms = 0;
+    uint32_t *tile_counter = nullptr;      // device: tile scheduler of k_sweep3_rows_u8 (returns to 0 at the end of every launch)
+    int32_t opt_rows = 0, opt_words = 0;   // potts3_set_option
 };
 
 namespace {
@@ -82,8 +85,86 @@ int launched3(potts3_t *h, const char *what)
     return POTTS_OK;
 }
 
-int half_sweep3(potts3_t *h, uint32_t colour, const unsigned long long neg_thr[13])
+// the row-walking kernel: W words per lane and row, grid = the blocks resident at once
+template <int CM, int COLOUR, int W, bool FAST>
+void launch_rows3(const potts::Sweep3RowsParams &P, int num_sms, cudaStream_t st)
 {
+    auto fn = potts::k_sweep3_rows_u8<CM, COLOUR, W, FAST>;
+    static int per_sm = 0;
+    if (per_sm == 0) {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 32 * potts::H3_WARPS, 0);
+        if (per_sm < 1) per_sm = 1;
+    }
+    const unsigned long long want = (unsigned long long)per_sm * (unsigned)num_sms;
+    const unsigned grid = (unsigned)(want < P.total_tiles ? want : P.total_tiles);
+    fn<<<grid, dim3(32, potts::H3_WARPS), 0, st>>>(P);
+}
+
+template <int CM, int W>
+void launch_rows3_cw(const potts::Sweep3RowsParams &P, uint32_t colour, int num_sms, cudaStream_t st)
+{
+    const bool fast = potts::accept_fast_ok3(P.thr);
+    if (colour == 0) { if (fast) launch_rows3<CM, 0, W, true>(P, num_sms, st); else launch_rows3<CM, 0, W, false>(P, num_sms, st); }
+    else { if (fast) launch_rows3<CM, 1, W, true>(P, num_sms, st); else launch_rows3<CM, 1, W, false>(P, num_sms, st); }
+}
+
+template <int CM>
+void launch_rows3_c(const potts::Sweep3RowsParams &P, uint32_t colour, int W, int num_sms, cudaStream_t st)
+{
+    if (W == 4) launch_rows3_cw<CM, 4>(P, colour, num_sms, st);
+    else if (W == 2) launch_rows3_cw<CM, 2>(P, colour, num_sms, st);
+    else launch_rows3_cw<CM, 1>(P, colour, num_sms, st);
+}
+
+struct Thresholds3 {
+    uint32_t thr[6];                       // floor(2^32 exp(-d/T)), d = 1..6 (reading R6')
+    unsigned long long neg_thr[13];        // 2^64 - threshold(d), d = -6..6
+};
+
+int half_sweep3(potts3_t *h, uint32_t colour, const Thresholds3 &TH)
+{
+    int W = h->opt_words < 0 ? 0 : (h->opt_words > 0 ? h->opt_words : 4);
+    if (h->opt_words == 0) {
+        // lanes are dealt to a row in powers of two (or whole warps): with L = 3 * 2^k a quarter of them would idle,
+        // and the one-chunk-per-thread kernel is the faster one (measured at L = 384: 3.40 against 3.62 ps)
+        const int chunks = h->L / 32;
+        int lanes = 1;
+        while (lanes < 32 && lanes < chunks) lanes <<= 1;
+        if (chunks > 32) lanes = (chunks + 31) / 32 * 32;
+        if (10 * chunks < 9 * lanes) W = 0;
+    }
+    if (W > 0) {
+        potts::Sweep3RowsParams P;
+        P.plane_own = h->plane[colour];
+        P.plane_oth = h->plane[1 - colour];
+        P.L = h->L;
+        P.pitch = h->L / 2;
+        P.q = (uint32_t)h->q;
+        P.key1 = (uint32_t)(h->seed >> 32);
+        P.K = potts::half_sweep_keys((uint32_t)(h->seed & 0xFFFFFFFFull), P.key1, (uint32_t)h->t, colour);
+        for (int d = 0; d < 6; ++d) P.thr[d] = TH.thr[d];
+        const int chunks = P.pitch / (4 * W);                           // lanes a row takes
+        P.lpr_log2 = 0;
+        while (P.lpr_log2 < 5 && (1 << P.lpr_log2) < chunks) P.lpr_log2 += 1;
+        const int windows_per_tile = potts::H3_WARPS << (5 - P.lpr_log2);
+        P.rpw = h->opt_rows > 0 ? h->opt_rows : 16;                     // L % 32 == 0: 2 .. 32 all divide L
+        const int cbs = (chunks + 31) / 32;
+        for (;;) {
+            P.row_groups = (h->L / P.rpw + windows_per_tile - 1) / windows_per_tile;
+            P.total_tiles = (uint32_t)cbs * (uint32_t)h->L * (uint32_t)P.row_groups;
+            // automatic: shorter windows until there are ~7 tiles per SM to draw (L = 256: 16 -> 4 rows, 3.92 -> 3.21 ps)
+            if (h->opt_rows > 0 || P.rpw <= 2 || P.total_tiles >= 1024u) break;
+            P.rpw >>= 1;
+        }
+        P.tile_counter = h->tile_counter;
+        switch (potts::compare_mode_of(h->q)) {
+        case potts::CM_7BIT: launch_rows3_c<potts::CM_7BIT>(P, colour, W, h->num_sms, h->stream); break;
+        case potts::CM_8BIT: launch_rows3_c<potts::CM_8BIT>(P, colour, W, h->num_sms, h->stream); break;
+        case potts::CM_NIB4: launch_rows3_c<potts::CM_NIB4>(P, colour, W, h->num_sms, h->stream); break;
+        default: launch_rows3_c<potts::CM_NIB3>(P, colour, W, h->num_sms, h->stream); break;
+        }
+        return launched3(h, "k_sweep3_rows_u8");
+    }
     potts::Sweep3Params P;
     P.plane_own = h->plane[colour];
     P.plane_oth = h->plane[1 - colour];
@@ -94,7 +175,7 @@ int half_sweep3(potts3_t *h, uint32_t colour, const unsigned long long neg_thr[1
     P.key0 = (uint32_t)(h->seed & 0xFFFFFFFFull);
     P.key1 = (uint32_t)(h->seed >> 32);
     P.t = (uint32_t)h->t;
-    for (int k = 0; k < 13; ++k) P.neg_thr[k] = neg_thr[k];
+    for (int k = 0; k < 13; ++k) P.neg_thr[k] = TH.neg_thr[k];
     const long long chunks = (long long)h->L * h->L * (h->L / 32);
     long long blocks = (chunks + 127) / 128;
     const long long cap = (long long)h->num_sms * 8;
@@ -130,15 +211,16 @@ int measure3(potts3_t *h, unsigned long long *E_out, unsigned long long *hist_ou
 // nsweeps sweeps; every > 0: after every `every`-th sweep the energy / histogram go to the device series
 int run3(potts3_t *h, double T, int64_t nsweeps, int64_t every, unsigned long long *E_dev, unsigned long long *hist_dev)
 {
-    unsigned long long neg_thr[13];
+    Thresholds3 TH;
     for (int d = -6; d <= 6; ++d) {
         // reading R6': threshold(d) = 2^32 for d <= 0, floor(ldexp(exp(-d/T), 32)) for d = 1..6
         const unsigned long long th = d <= 0 ? (1ull << 32) : (unsigned long long)(uint32_t)std::floor(std::ldexp(std::exp(-(double)d / T), 32));
-        neg_thr[d + 6] = 0ull - th;
+        TH.neg_thr[d + 6] = 0ull - th;
+        if (d > 0) TH.thr[d - 1] = (uint32_t)th;
     }
     for (int64_t n = 0; n < nsweeps; ++n) {
-        int rc = half_sweep3(h, 0u, neg_thr);
-        if (rc == POTTS_OK) rc = half_sweep3(h, 1u, neg_thr);
+        int rc = half_sweep3(h, 0u, TH);
+        if (rc == POTTS_OK) rc = half_sweep3(h, 1u, TH);
         if (rc) return rc;
         h->t += 1;
         if (every > 0 && (n + 1) % every == 0 && (E_dev || hist_dev)) {
@@ -182,7 +264,7 @@ int potts3_create(potts3_t **out, int32_t L, int32_t q, uint64_t seed, int32_t i
     cudaGetDevice(&h->device);
     cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device);
     h->plane_bytes = align_up3((size_t)L * L * (L / 2));
-    const size_t need = 2 * h->plane_bytes + align_up3(258 * sizeof(unsigned long long));
+    const size_t need = 2 * h->plane_bytes + align_up3(260 * sizeof(unsigned long long));
     const cudaError_t e = cudaMalloc(&h->ws, need);
     if (e != cudaSuccess) {
         delete h;
@@ -191,6 +273,7 @@ int potts3_create(potts3_t **out, int32_t L, int32_t q, uint64_t seed, int32_t i
     h->plane[0] = h->ws;
     h->plane[1] = h->ws + h->plane_bytes;
     h->acc = (unsigned long long *)(h->ws + 2 * h->plane_bytes);
+    h->tile_counter = (uint32_t *)(h->acc + 258);
     cudaError_t e2 = cudaMemsetAsync(h->ws, 0, need, h->stream);
     if (e2 == cudaSuccess && init == POTTS_INIT_RANDOM) {
         const long long words = 2ll * L * L * (L / 8);
@@ -345,6 +428,22 @@ int potts3_launch_count(potts3_t *h, uint64_t *n)
     if (!h || !n) return fail(POTTS_ERR_ARG, "null argument");
     *n = h->launches;
     return POTTS_OK;
+}
+
+int potts3_set_option(potts3_t *h, const char *key, int64_t value)
+{
+    if (!h || !key) return fail(POTTS_ERR_ARG, "null argument");
+    if (!std::strcmp(key, "stream_words")) {
+        if (value != 0 && value != 1 && value != 2 && value != 4 && value != -1) return fail(POTTS_ERR_ARG, "stream_words = %lld not in {-1, 0, 1, 2, 4}", (long long)value);
+        h->opt_words = (int32_t)value;
+        return POTTS_OK;
+    }
+    if (!std::strcmp(key, "stream_rows")) {
+        if (value != 0 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32) return fail(POTTS_ERR_ARG, "stream_rows = %lld not in {0, 2, 4, 8, 16, 32}", (long long)value);
+        h->opt_rows = (int32_t)value;
+        return POTTS_OK;
+    }
+    return fail(POTTS_ERR_ARG, "unknown option '%s'", key);
 }
 
 }  // extern "C"

@@ -184,15 +184,17 @@ struct ColKeys {
     uint32_t ph, pl;  // M0 * (hi(M1*(hi(M0*j)^xb)) ^ xc): round 3's M0*c0 product
 };
 
-__device__ __forceinline__ ColKeys col_keys(const HalfSweepKeys &K, uint32_t j)
+__device__ __forceinline__ ColKeys col_keys(uint32_t xb, uint32_t xc, uint32_t j)
 {
     ColKeys C;
     uint32_t h0, h1;
     mul_wide(PHILOX_M0, j, h0, C.l0);
-    mul_wide(PHILOX_M1, h0 ^ K.xb, h1, C.l1);
-    mul_wide(PHILOX_M0, h1 ^ K.xc, C.ph, C.pl);
+    mul_wide(PHILOX_M1, h0 ^ xb, h1, C.l1);
+    mul_wide(PHILOX_M0, h1 ^ xc, C.ph, C.pl);
     return C;
 }
+
+__device__ __forceinline__ ColKeys col_keys(const HalfSweepKeys &K, uint32_t j) { return col_keys(K.xb, K.xc, j); }
 
 // row part for the hoisted form: RowKeys plus c3 ^ (k1 of round 3)
 struct RowKeysH {
@@ -369,11 +371,12 @@ template <int SLOTS = 8>
 __device__ __forceinline__ uint32_t accept_lane_offset(uint32_t lane) { return (lane % SLOTS) * 8u; }
 
 // accept masks of the four sites of a word: byte b = 0xff iff site b accepts its proposal
-template <int SLOTS>
+// CODE_BITS: the bits of a code byte that index the table (the 3D code leaves garbage in bits 3 and 7: 0x77)
+template <int SLOTS, uint32_t CODE_BITS = 0xffu>
 __device__ __forceinline__ uint32_t accept_mask(uint32_t code, const uint32_t w1[4], const AcceptLutT<SLOTS> *lut, uint32_t lane_off)
 {
     constexpr int ACCEPT_SHIFT = AcceptLutT<SLOTS>::shift;
-    constexpr uint32_t M = 0xffu << ACCEPT_SHIFT;
+    constexpr uint32_t M = CODE_BITS << ACCEPT_SHIFT;
     uint32_t a[4];
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
@@ -390,12 +393,12 @@ __device__ __forceinline__ uint32_t accept_mask(uint32_t code, const uint32_t w1
 }
 
 // Fast form (table filled with fast = true): the new word directly, one compare and one predicated byte insert per site.
-template <int SLOTS>
+template <int SLOTS, uint32_t CODE_BITS = 0xffu>
 __device__ __forceinline__ uint32_t accept_insert(uint32_t own, uint32_t prop, uint32_t code, const uint32_t w1[4], const AcceptLutT<SLOTS> *lut,
                                                   uint32_t lane_off)
 {
     constexpr int ACCEPT_SHIFT = AcceptLutT<SLOTS>::shift;
-    constexpr uint32_t M = 0xffu << ACCEPT_SHIFT;
+    constexpr uint32_t M = CODE_BITS << ACCEPT_SHIFT;
     uint32_t out = own;
 #pragma unroll
     for (int b = 0; b < 4; ++b) {

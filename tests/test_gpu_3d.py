@@ -107,3 +107,44 @@ def test_3d_large_lattice_prefix(pb):
     Eo, Ho = o.sweep_measured(T, 2, 1, hist=True)
     assert (Eg == Eo).all() and (Hg == Ho).all()
     assert (g.potts3_download() == o.spins()).all()
+
+
+# the row-walking kernel k_sweep3_rows_u8 in every shape (several windows per warp at these sizes: the point is every template
+# argument -- compare mode, colour, words per lane, exact / one-compare acceptance (T = 0.05 has zero thresholds) --
+# and every rows-per-warp value against the oracle), and the one-chunk-per-thread kernel forced where the other is automatic
+@pytest.mark.parametrize("words,rows", [(1, 2), (2, 4), (4, 8), (1, 32), (4, 0), (2, 16), (-1, 0)])
+@pytest.mark.parametrize("L,q,init,T,seed,n", CASES[:8])
+def test_3d_row_walking_kernel(pb, L, q, init, T, seed, n, words, rows):
+    n = min(n, 6)
+    g = pb.Potts3D(L, q, seed, init)
+    g.potts3_set_option("stream_words", words)
+    g.potts3_set_option("stream_rows", rows)
+    o = oracle.OraclePotts3D(L, q, seed, init, threads=8)
+    Eg, Hg = g.potts3_sweep_measured(T, n, 1, hist=True)
+    Eo, Ho = o.sweep_measured(T, n, 1, hist=True)
+    assert (Eg == Eo).all() and (Hg == Ho).all()
+    assert (g.potts3_download() == o.spins()).all()
+
+
+def test_3d_options(pb):
+    g = pb.Potts3D(32, 9, 1)
+    for key, value in (("stream_words", 3), ("stream_rows", 5), ("nonsense", 1)):
+        with pytest.raises(pb.PottsError) as e:
+            g.potts3_set_option(key, value)
+        assert e.value.code == pb.ERR_ARG
+
+
+@pytest.mark.parametrize("L,q,words", [(256, 9, 0), (256, 24, 2), (512, 6, 0), (512, 9, 1)])
+def test_3d_kernels_agree_where_lanes_are_full(pb, L, q, words):
+    """L = 256 / 512: the automatic choice (4 words per lane: two / four windows per warp) and narrower lanes (words = 1
+    at L = 512: two column blocks) against the one-chunk-per-thread kernel, which the cases above pin to the oracle."""
+    T, seed = 1.3, 77
+    a = pb.Potts3D(L, q, seed, pb.INIT_RANDOM)
+    b = pb.Potts3D(L, q, seed, pb.INIT_RANDOM)
+    a.potts3_set_option("stream_words", words)
+    b.potts3_set_option("stream_words", -1)
+    Ea, Ha = a.potts3_sweep_measured(T, 3, 1, hist=True)
+    Eb, Hb = b.potts3_sweep_measured(T, 3, 1, hist=True)
+    assert (Ea == Eb).all() and (Ha == Hb).all()
+    assert a.potts3_launch_count() == b.potts3_launch_count()
+    assert (a.potts3_download() == b.potts3_download()).all()
