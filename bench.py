@@ -477,10 +477,10 @@ def second_neighbour_lattice(pb, torch, peaks, L=12288, q=9, sweeps=20, repeats=
     g.close()
     sec = statistics.median(ms) * 1e-3
     w = type("W", (), {"name": f"potts8_q{q}_L{L}"})
-    r = roofline(w, "k_sweep8_u8", L * L / 9, sec * 1e3 / (9 * sweeps), sm_max, hbm_gbs, which, 10.0)
+    r = roofline(w, "k_sweep8_rows_u8", L * L / 9, sec * 1e3 / (9 * sweeps), sm_max, hbm_gbs, which, 10.0)
     ups = sweeps * L * L / sec
     return {"q": q, "L": L, "sweeps_per_call": sweeps, "calls": repeats, "T": T, "ns_per_spin_flip": 1e9 / ups,
-            "spin_updates_per_s": ups, "ms_per_call_min_max": [min(ms), max(ms)], "kernel": "k_sweep8_u8", "roofline": r}
+            "spin_updates_per_s": ups, "ms_per_call_min_max": [min(ms), max(ms)], "kernel": "k_sweep8_rows_u8", "roofline": r}
 
 
 def paper_protocol_e6(pb, torch):

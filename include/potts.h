@@ -300,6 +300,13 @@ int  potts8_upload(potts8_t *h, const uint8_t *spins);
 int  potts8_sweep_count(potts8_t *h, uint64_t *t);
 int  potts8_set_sweep_count(potts8_t *h, uint64_t t);
 int  potts8_launch_count(potts8_t *h, uint64_t *n);
+/* potts8_set_option: launch knobs that never change WHAT is computed.  Unknown key or bad value -> POTTS_ERR_ARG.  Keys:
+ *   "stream_words"  0 = automatic (the row-walking kernel k_sweep8_rows_u8, 16 sites per lane and row visit, for
+ *                   L >= 3072 with L % 48 == 0; else the one-word-per-thread kernel k_sweep8_u8), 4 = k_sweep8_rows_u8
+ *                   wherever L % 48 == 0 and L < 65536, -1 = k_sweep8_u8
+ *   "stream_rows"   0 = automatic (16, halved while a launch would have fewer than 1024 tiles), else rows a lane walks
+ *                   per tile (1, 2, 4, 8 or 16) */
+int  potts8_set_option(potts8_t *h, const char *key, int64_t value);
 
 #ifdef __cplusplus
 }

@@ -93,6 +93,7 @@ def load_library() -> ctypes.CDLL:
         "potts3_set_sweep_count": ([vp, u64], ctypes.c_int),
         "potts3_launch_count": ([vp, P(u64)], ctypes.c_int),
         "potts3_set_option": ([vp, ctypes.c_char_p, i64], ctypes.c_int),
+        "potts8_set_option": ([vp, ctypes.c_char_p, i64], ctypes.c_int),
         "potts8_create": ([P(vp), i32, i32, u64, i32, vp], ctypes.c_int),
         "potts8_destroy": ([vp], None),
         "potts8_sweep": ([vp, dbl, i64], ctypes.c_int),
@@ -127,7 +128,7 @@ EXPORTED_SYMBOLS = [
     "potts3_create", "potts3_destroy", "potts3_sweep", "potts3_sweep_measured", "potts3_energy", "potts3_histogram",
     "potts3_download", "potts3_upload", "potts3_sweep_count", "potts3_set_sweep_count", "potts3_launch_count", "potts3_set_option",
     "potts8_create", "potts8_destroy", "potts8_sweep", "potts8_sweep_measured", "potts8_energy", "potts8_histogram",
-    "potts8_download", "potts8_upload", "potts8_sweep_count", "potts8_set_sweep_count", "potts8_launch_count",
+    "potts8_download", "potts8_upload", "potts8_sweep_count", "potts8_set_sweep_count", "potts8_launch_count", "potts8_set_option",
 ]
 
 
@@ -551,3 +552,6 @@ class Potts8:
         n = ctypes.c_uint64()
         _check(self._lib.potts8_launch_count(self._h, ctypes.byref(n)))
         return int(n.value)
+
+    def potts8_set_option(self, key: str, value: int):
+        _check(self._lib.potts8_set_option(self._h, key.encode(), int(value)))

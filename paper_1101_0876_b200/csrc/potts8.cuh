@@ -108,6 +108,210 @@ __global__ void __launch_bounds__(128) k_sweep8_u8(const __grid_constant__ Sweep
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Row-walking form.  A lane updates 16 sites (one 16-byte chunk of a plane row, columns J = k0..k0+15) per row visit
+// and walks a window of rpw rows; a block of H8_WARPS warps owns a tile of 32 chunks x its windows (rows narrower than
+// a warp: 2^lpr_log2 lanes per row and several windows per warp, as in k_sweep3_rows_u8); tiles are drawn from a
+// counter.  What walking buys here is not load reuse (the eight neighbours of consecutive rows lie in eight different
+// (plane, row) pairs) but everything per column and per visit: the ColKeys of the tile's columns j = 3 J + b (the
+// column part of Philox, shared by all rows) sit in shared memory, the row keys, addresses and neighbour preparation
+// are paid once per 16 sites.  B = c mod 3 is a template argument: the column shift of every direction is a literal.
+// Compare: the eight flag words are added bit-sliced by a carry-save tree (14 three-input logic ops) into the planes
+// ones / twos / fours / eights; code byte = c_old in bits 0-3, c_new in bits 4-7, index of the 2D accept table filled
+// with threshold(c_new - c_old).  Needs pitch % 16 == 0 (L % 48 == 0).
+constexpr int H8_WARPS = 4;
+
+struct Sweep8RowsParams {
+    uint8_t *planes;
+    unsigned long long plane_bytes;
+    int32_t pitch, rows;          // both L/3
+    uint32_t q, c;
+    HalfSweepKeys K;              // of (seed, t, 16 + c)
+    Nbr8 nbr[8];                  // directions in the order (di, dj) = (0,1) (1,0) (1,1) (1,-1) (0,-1) (-1,0) (-1,-1) (-1,1)
+    uint32_t thr[8];              // threshold(d), d = 1..8 (R6")
+    int32_t rpw, row_groups, lpr_log2;
+    uint32_t total_tiles;
+    uint32_t *tile_counter;
+};
+
+__host__ __device__ constexpr int dir8_dj(int k) { return (k == 0 || k == 2 || k == 7) ? 1 : ((k == 1 || k == 5) ? 0 : -1); }
+// column shift of direction k for the sites of column residue b (Nbr8::shift, as a literal)
+__host__ __device__ constexpr int dir8_shift(int b, int k) { return (b == 0 && dir8_dj(k) < 0) ? -1 : ((b == 2 && dir8_dj(k) > 0) ? 1 : 0); }
+
+__host__ __device__ inline bool accept_fast_ok8(const uint32_t thr[8])
+{
+    bool ok = true;
+    for (int d = 0; d < 8; ++d) ok = ok && thr[d] != 0u;
+    return ok;
+}
+
+template <int SLOTS>
+__device__ __forceinline__ void accept_lut_fill8(AcceptLutT<SLOTS> *lut, const uint32_t thr[8], uint32_t tid, uint32_t nthreads, bool fast)
+{
+    for (uint32_t n = tid; n < (uint32_t)(ACCEPT_ENTRIES * SLOTS); n += nthreads) {
+        const uint32_t code = n / SLOTS;
+        int d = (int)(code >> 4) - (int)(code & 15u);
+        d = d > 8 ? 8 : d;                                             // counts above 8 never occur
+        const unsigned long long th = d <= 0 ? (1ull << 32) : (unsigned long long)thr[d - 1];
+        const unsigned long long e = fast ? th - 1ull : 0ull - th;
+        (&lut->e[0][0])[n] = make_uint2((uint32_t)e, (uint32_t)(e >> 32));
+    }
+}
+
+// carry-save count of eight flag words: bit planes of the per-position sum (0..8)
+__device__ __forceinline__ void csa8(const uint32_t u[8], uint32_t &ones, uint32_t &twos, uint32_t &fours, uint32_t &eights)
+{
+    constexpr int XOR3 = 0x96, MAJ = 0xE8;
+    const uint32_t s1 = lop3<XOR3>(u[0], u[1], u[2]), c1 = lop3<MAJ>(u[0], u[1], u[2]);
+    const uint32_t s2 = lop3<XOR3>(u[3], u[4], u[5]), c2 = lop3<MAJ>(u[3], u[4], u[5]);
+    const uint32_t s3 = lop3<XOR3>(s1, s2, u[6]), c3 = lop3<MAJ>(s1, s2, u[6]);
+    ones = s3 ^ u[7];
+    const uint32_t c4 = s3 & u[7];
+    const uint32_t t1 = lop3<XOR3>(c1, c2, c3), d1 = lop3<MAJ>(c1, c2, c3);
+    twos = t1 ^ c4;
+    const uint32_t d2 = t1 & c4;
+    fours = d1 ^ d2;
+    eights = d1 & d2;
+}
+
+template <int CM>
+__device__ __forceinline__ uint32_t ne_code8(uint32_t own, uint32_t prop, const uint32_t nb[8])
+{
+    if (is_nibble_mode(CM)) {
+        const uint32_t both = prop * 16u + own;
+        uint32_t u[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            if (CM == CM_NIB3) u[k] = (both ^ nb[k]) + 0x77777777u;
+            else u[k] = lop3<LOP_OR_XOR>(lop3<LOP_XOR_AND>(both, nb[k], 0x77777777u) + 0x77777777u, both, nb[k]);
+        }
+        uint32_t c1, c2, c4, c8;                                       // flags in bits 3 and 7 of every byte
+        csa8(u, c1, c2, c4, c8);
+        uint32_t c = lop3<LOP_SEL>(c1 >> 3, c2 >> 2, 0x11111111u);
+        c = lop3<LOP_SEL>(c, c4 >> 1, 0x33333333u);
+        return lop3<LOP_SEL>(c, c8, 0x77777777u);
+    } else {
+        uint32_t o[8], n[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            if (CM == CM_7BIT) {
+                o[k] = (own ^ nb[k]) + 0x7f7f7f7fu;
+                n[k] = (prop ^ nb[k]) + 0x7f7f7f7fu;
+            } else {
+                o[k] = lop3<LOP_OR_XOR>(lop3<LOP_XOR_AND>(own, nb[k], 0x7f7f7f7fu) + 0x7f7f7f7fu, own, nb[k]);
+                n[k] = lop3<LOP_OR_XOR>(lop3<LOP_XOR_AND>(prop, nb[k], 0x7f7f7f7fu) + 0x7f7f7f7fu, prop, nb[k]);
+            }
+        }
+        uint32_t o1, o2, o4, o8, n1, n2, n4, n8;                       // flags in bit 7 of every byte
+        csa8(o, o1, o2, o4, o8);
+        csa8(n, n1, n2, n4, n8);
+        uint32_t a = lop3<LOP_SEL>(o1 >> 7, o2 >> 6, 0x01010101u);
+        a = lop3<LOP_SEL>(a, o4 >> 5, 0x03030303u);
+        a = lop3<LOP_SEL>(a, o8 >> 4, 0x07070707u);
+        uint32_t b = lop3<LOP_SEL>(n1 >> 3, n2 >> 2, 0x10101010u);
+        b = lop3<LOP_SEL>(b, n4 >> 1, 0x30303030u);
+        b = lop3<LOP_SEL>(b, n8, 0x70707070u);
+        return lop3<LOP_SEL>(a, b, 0x0f0f0f0fu);
+    }
+}
+
+template <int CM, int B, bool FAST>
+__global__ void __launch_bounds__(32 * H8_WARPS, 5) k_sweep8_rows_u8(const __grid_constant__ Sweep8RowsParams P)
+{
+    __shared__ uint4 s_col[16][32];                                   // ColKeys of [site of the chunk][lane of the row]
+    __shared__ AcceptLut lut;
+    __shared__ uint32_t s_tile[2];
+    const uint32_t lane = threadIdx.x, wy = threadIdx.y, tid = wy * 32u + lane;
+    accept_lut_fill8(&lut, P.thr, tid, 32 * H8_WARPS, FAST);
+    const HalfSweepKeys &K = P.K;
+    const uint32_t lane_off = accept_lane_offset(lane);
+    const uint32_t q = in_register(P.q);
+    const int pitch = P.pitch, rows = P.rows, chunks = pitch >> 4;
+    const uint32_t a = P.c / 3u;
+    uint8_t *const own_plane = P.planes + P.c * P.plane_bytes;
+    int cb_cur = -1;
+    for (uint32_t it = 0;; ++it) {
+    if (tid == 0) s_tile[it & 1u] = atomicInc(P.tile_counter, P.total_tiles + gridDim.x - 1u);
+    __syncthreads();                                                  // also: every thread is done with the previous tile
+    const uint32_t tile = s_tile[it & 1u];
+    if (tile >= P.total_tiles) break;
+    const int cb = (int)(tile / (uint32_t)P.row_groups), rg = (int)(tile - (uint32_t)cb * (uint32_t)P.row_groups);
+    const int xl = (int)lane & ((1 << P.lpr_log2) - 1), sub = (int)lane >> P.lpr_log2;
+    const int x = cb * 32 + xl;
+    const int win = ((rg * H8_WARPS + (int)wy) << (5 - P.lpr_log2)) + sub;
+    const bool active = x < chunks && win * P.rpw < rows;
+    const int k0 = x << 4;
+    if (cb != cb_cur) {
+        cb_cur = cb;
+        if (x < chunks && sub == 0)
+            for (int n = (int)wy; n < 16; n += H8_WARPS) {
+                const ColKeys C = col_keys(K, 3u * (uint32_t)(k0 + n) + (uint32_t)B);
+                s_col[n][xl] = make_uint4(C.l0, C.l1, C.ph, C.pl);
+            }
+        __syncthreads();
+    }
+    if (active) {
+        const int kn = wrap(k0 + 16, pitch) - k0, kp = wrap(k0 - 4, pitch) - k0;
+        const int I0 = win * P.rpw;
+#pragma unroll 1
+        for (int r = 0; r < P.rpw; ++r) {
+            const int I = I0 + r;
+            // the ColKeys of the lane's columns do not depend on the row: without this the compiler hoists the 16
+            // loads out of the row loop and spills the 64 registers they need
+            int xc = xl;
+            asm volatile("" : "+r"(xc));
+            // byte offsets of rows I-1, I, I+1 inside a plane (32 bit: nine planes stay below 4 GB)
+            const uint32_t r_0 = (uint32_t)(I * pitch + k0), r_m = (uint32_t)(wrap(I - 1, rows) * pitch + k0), r_p = (uint32_t)(wrap(I + 1, rows) * pitch + k0);
+            const uint4 own4 = *reinterpret_cast<const uint4 *>(own_plane + r_0);
+            uint32_t nbw[8][4];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const int dI = P.nbr[k].dI;
+                const uint32_t ro = dI == 0 ? r_0 : (dI < 0 ? r_m : r_p);
+                const uint8_t *rowp = P.planes + ((uint32_t)P.nbr[k].plane * (uint32_t)P.plane_bytes + ro);
+                const uint4 v = *reinterpret_cast<const uint4 *>(rowp);
+                const int sh = dir8_shift(B, k);
+                if (sh > 0) {
+                    const uint32_t adj = *reinterpret_cast<const uint32_t *>(rowp + kn);
+                    nbw[k][0] = __funnelshift_r(v.x, v.y, 8); nbw[k][1] = __funnelshift_r(v.y, v.z, 8);
+                    nbw[k][2] = __funnelshift_r(v.z, v.w, 8); nbw[k][3] = __funnelshift_r(v.w, adj, 8);
+                } else if (sh < 0) {
+                    const uint32_t adj = *reinterpret_cast<const uint32_t *>(rowp + kp);
+                    nbw[k][0] = __funnelshift_l(adj, v.x, 8); nbw[k][1] = __funnelshift_l(v.x, v.y, 8);
+                    nbw[k][2] = __funnelshift_l(v.y, v.z, 8); nbw[k][3] = __funnelshift_l(v.z, v.w, 8);
+                } else {
+                    nbw[k][0] = v.x; nbw[k][1] = v.y; nbw[k][2] = v.z; nbw[k][3] = v.w;
+                }
+#pragma unroll
+                for (int n = 0; n < 4; ++n) nbw[k][n] = prep_nbr<CM>(nbw[k][n]);
+            }
+            const RowKeysH R = row_keys_h(K, 3u * (uint32_t)I + a);
+            const uint32_t own[4] = {own4.x, own4.y, own4.z, own4.w};
+            uint32_t out[4];
+#pragma unroll
+            for (int n = 0; n < 4; ++n) {
+                uint32_t nb[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) nb[k] = nbw[k][n];
+                uint32_t w0[4], w1[4];
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const uint4 c = s_col[4 * n + b][xc];
+                    philox_site_h(K, R, ColKeys{c.x, c.y, c.z, c.w}, w0[b], w1[b]);
+                }
+                const uint32_t s01 = __byte_perm(__umulhi(w0[0], q), __umulhi(w0[1], q), 0x0040);
+                const uint32_t s23 = __byte_perm(__umulhi(w0[2], q), __umulhi(w0[3], q), 0x0040);
+                const uint32_t prop = __byte_perm(s01, s23, 0x5410);                       // R4
+                const uint32_t code = ne_code8<CM>(own[n], prop, nb);                      // R5"
+                if (FAST) out[n] = accept_insert(own[n], prop, code, w1, &lut, lane_off);  // R6", R7
+                else out[n] = lop3<LOP_SEL>(prop, own[n], accept_mask(code, w1, &lut, lane_off));
+            }
+            *reinterpret_cast<uint4 *>(own_plane + r_0) = make_uint4(out[0], out[1], out[2], out[3]);
+        }
+    }
+    }   // tiles
+}
+
 // Energy: for every word of sub-network P.c the equal neighbours in the four FORWARD directions (0,1), (1,0), (1,1),
 // (1,-1) (descriptors nbr[0..3]), so that every bond is counted once over the nine launches; histogram of the plane.
 template <bool WIDE>

@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstring>
 #include <new>
 
 namespace potts {
@@ -58,6 +59,8 @@ struct potts8_s {
     size_t scratch_bytes = 0;
     cudaStream_t stream = nullptr;
     int num_sms = 0;
+    uint32_t *tile_counter = nullptr;      // device: tile scheduler of k_sweep8_rows_u8 (returns to 0 at the end of every launch)
+    int32_t opt_rows = 0, opt_words = 0;   // potts8_set_option
 };
 
 namespace {
@@ -118,10 +121,78 @@ unsigned grid8(const potts8_t *h, int block)
     return (unsigned)(blocks > cap ? cap : (blocks < 1 ? 1 : blocks));
 }
 
-int class_sweep8(potts8_t *h, uint32_t c, const unsigned long long neg_thr[17])
+struct Thresholds8 {
+    uint32_t thr[8];                       // floor(2^32 exp(-d/T)), d = 1..8 (reading R6")
+    unsigned long long neg_thr[17];        // 2^64 - threshold(d), d = -8..8
+};
+
+template <int CM, int B, bool FAST>
+void launch_rows8(const potts::Sweep8RowsParams &P, int num_sms, cudaStream_t st)
 {
-    potts::Sweep8Params P = params8(h, c);
-    for (int k = 0; k < 17; ++k) P.neg_thr[k] = neg_thr[k];
+    auto fn = potts::k_sweep8_rows_u8<CM, B, FAST>;
+    static int per_sm = 0;
+    if (per_sm == 0) {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 32 * potts::H8_WARPS, 0);
+        if (per_sm < 1) per_sm = 1;
+    }
+    const unsigned long long want = (unsigned long long)per_sm * (unsigned)num_sms;
+    const unsigned grid = (unsigned)(want < P.total_tiles ? want : P.total_tiles);
+    fn<<<grid, dim3(32, potts::H8_WARPS), 0, st>>>(P);
+}
+
+template <int CM>
+void launch_rows8_c(const potts::Sweep8RowsParams &P, int num_sms, cudaStream_t st)
+{
+    const bool fast = potts::accept_fast_ok8(P.thr);
+    switch (P.c % 3u) {
+    case 0: if (fast) launch_rows8<CM, 0, true>(P, num_sms, st); else launch_rows8<CM, 0, false>(P, num_sms, st); break;
+    case 1: if (fast) launch_rows8<CM, 1, true>(P, num_sms, st); else launch_rows8<CM, 1, false>(P, num_sms, st); break;
+    default: if (fast) launch_rows8<CM, 2, true>(P, num_sms, st); else launch_rows8<CM, 2, false>(P, num_sms, st); break;
+    }
+}
+
+int class_sweep8(potts8_t *h, uint32_t c, const Thresholds8 &TH)
+{
+    const potts::Sweep8Params P = [&] {
+        potts::Sweep8Params p = params8(h, c);
+        for (int k = 0; k < 17; ++k) p.neg_thr[k] = TH.neg_thr[k];
+        return p;
+    }();
+    const int pitch = h->L / 3;
+    // automatic: from 2^20 sites per launch on; below, a launch is a few blocks per SM and the per-block tables
+    // (accept table, ColKeys) cost more than they save (measured at L = 768: 129 against 63 ps, launch latency both)
+    const bool rows_kernel = h->opt_words > 0 || (h->opt_words == 0 && h->L >= 3072);
+    if (rows_kernel && pitch % 16 == 0 && 9ull * h->plane_bytes < (1ull << 32)) {   // the kernel's plane offsets are 32 bit
+        potts::Sweep8RowsParams R;
+        R.planes = P.planes;
+        R.plane_bytes = P.plane_bytes;
+        R.pitch = R.rows = pitch;
+        R.q = P.q;
+        R.c = c;
+        R.K = potts::half_sweep_keys(P.key0, P.key1, P.t, 16u + c);
+        for (int k = 0; k < 8; ++k) R.nbr[k] = P.nbr[k];
+        for (int d = 0; d < 8; ++d) R.thr[d] = TH.thr[d];
+        const int chunks = pitch / 16;
+        R.lpr_log2 = 0;
+        while (R.lpr_log2 < 5 && (1 << R.lpr_log2) < chunks) R.lpr_log2 += 1;
+        const int windows_per_tile = potts::H8_WARPS << (5 - R.lpr_log2);
+        R.rpw = h->opt_rows > 0 ? h->opt_rows : 16;                     // pitch % 16 == 0: 2 .. 16 divide the rows
+        const int cbs = (chunks + 31) / 32;
+        for (;;) {
+            R.row_groups = (pitch / R.rpw + windows_per_tile - 1) / windows_per_tile;
+            R.total_tiles = (uint32_t)cbs * (uint32_t)R.row_groups;
+            if (h->opt_rows > 0 || R.rpw <= 2 || R.total_tiles >= 1024u) break;   // automatic: ~7 tiles per SM to draw
+            R.rpw >>= 1;
+        }
+        R.tile_counter = h->tile_counter;
+        switch (potts::compare_mode_of(h->q)) {
+        case potts::CM_7BIT: launch_rows8_c<potts::CM_7BIT>(R, h->num_sms, h->stream); break;
+        case potts::CM_8BIT: launch_rows8_c<potts::CM_8BIT>(R, h->num_sms, h->stream); break;
+        case potts::CM_NIB4: launch_rows8_c<potts::CM_NIB4>(R, h->num_sms, h->stream); break;
+        default: launch_rows8_c<potts::CM_NIB3>(R, h->num_sms, h->stream); break;
+        }
+        return launched8(h, "k_sweep8_rows_u8");
+    }
     const unsigned blocks = grid8(h, 128);
     switch (potts::compare_mode_of(h->q)) {
     case potts::CM_7BIT: potts::k_sweep8_u8<potts::CM_7BIT><<<blocks, 128, 0, h->stream>>>(P); break;
@@ -148,15 +219,16 @@ int measure8(potts8_t *h, unsigned long long *E_out, unsigned long long *hist_ou
 // nsweeps sweeps; every > 0: after every `every`-th sweep the energy / histogram go to the device series
 int run8(potts8_t *h, double T, int64_t nsweeps, int64_t every, unsigned long long *E_dev, unsigned long long *hist_dev)
 {
-    unsigned long long neg_thr[17];
+    Thresholds8 TH;
     for (int d = -8; d <= 8; ++d) {
         // reading R6": threshold(d) = 2^32 for d <= 0, floor(ldexp(exp(-d/T), 32)) for d = 1..8
         const unsigned long long th = d <= 0 ? (1ull << 32) : (unsigned long long)(uint32_t)std::floor(std::ldexp(std::exp(-(double)d / T), 32));
-        neg_thr[d + 8] = 0ull - th;
+        TH.neg_thr[d + 8] = 0ull - th;
+        if (d > 0) TH.thr[d - 1] = (uint32_t)th;
     }
     for (int64_t n = 0; n < nsweeps; ++n) {
         for (uint32_t c = 0; c < 9; ++c) {                                   // R2": the nine sub-networks in order
-            const int rc = class_sweep8(h, c, neg_thr);
+            const int rc = class_sweep8(h, c, TH);
             if (rc) return rc;
         }
         h->t += 1;
@@ -199,13 +271,14 @@ int potts8_create(potts8_t **out, int32_t L, int32_t q, uint64_t seed, int32_t i
     cudaGetDevice(&h->device);
     cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device);
     h->plane_bytes = align_up8((size_t)(L / 3) * (L / 3));
-    const size_t need = 9 * h->plane_bytes + align_up8(258 * sizeof(unsigned long long));
+    const size_t need = 9 * h->plane_bytes + align_up8(260 * sizeof(unsigned long long));
     const cudaError_t e = cudaMalloc(&h->ws, need);
     if (e != cudaSuccess) {
         delete h;
         return fail(e == cudaErrorMemoryAllocation ? POTTS_ERR_NOMEM : POTTS_ERR_CUDA, "cudaMalloc(%zu) failed: %s", need, cudaGetErrorString(e));
     }
     h->acc = (unsigned long long *)(h->ws + 9 * h->plane_bytes);
+    h->tile_counter = (uint32_t *)(h->acc + 258);
     cudaError_t e2 = cudaMemsetAsync(h->ws, 0, need, h->stream);
     if (e2 == cudaSuccess && init == POTTS_INIT_RANDOM) {
         const long long sites = (long long)L * L;
@@ -349,6 +422,22 @@ int potts8_launch_count(potts8_t *h, uint64_t *n)
     if (!h || !n) return fail(POTTS_ERR_ARG, "null argument");
     *n = h->launches;
     return POTTS_OK;
+}
+
+int potts8_set_option(potts8_t *h, const char *key, int64_t value)
+{
+    if (!h || !key) return fail(POTTS_ERR_ARG, "null argument");
+    if (!std::strcmp(key, "stream_words")) {
+        if (value != 0 && value != 4 && value != -1) return fail(POTTS_ERR_ARG, "stream_words = %lld not in {-1, 0, 4}", (long long)value);
+        h->opt_words = (int32_t)value;
+        return POTTS_OK;
+    }
+    if (!std::strcmp(key, "stream_rows")) {
+        if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8 && value != 16) return fail(POTTS_ERR_ARG, "stream_rows = %lld not in {0, 1, 2, 4, 8, 16}", (long long)value);
+        h->opt_rows = (int32_t)value;
+        return POTTS_OK;
+    }
+    return fail(POTTS_ERR_ARG, "unknown option '%s'", key);
 }
 
 }  // extern "C"

@@ -75,3 +75,49 @@ def test_nnn_split_calls_upload_restart_and_arguments(pb):
     assert (E == -4 * 24 * 24).all() and (H[:, 0] == 24 * 24).all()
     with pytest.raises(pb.PottsError):
         c.potts8_sweep_measured(1.0, 5, 2)
+
+
+# the row-walking kernel k_sweep8_rows_u8 (automatic for L % 48 == 0): every compare mode, the three column residues
+# of every launch set, exact / one-compare acceptance (T = 0.05 has zero thresholds), rows narrower than a warp with
+# idle lanes (L = 144: 3 chunks on 4 lanes), rows per window 1 .. 16, several column blocks (L = 3072: 64 chunks);
+# words = -1: the one-word-per-thread kernel at the same sizes
+ROWS_CASES = [
+    (48, 2, 1, 4.0, 11, 8),
+    (96, 9, 1, 2.0, 1, 6),
+    (144, 6, 0, 2.6, 7, 6),
+    (96, 24, 1, 1.6, 4, 6),
+    (192, 200, 1, 1.5, 9, 4),
+    (48, 129, 1, 80.0, 6, 6),
+    (96, 5, 1, 0.05, 10, 6),
+]
+
+
+@pytest.mark.parametrize("words,rows", [(0, 0), (4, 1), (4, 2), (4, 8), (4, 16), (-1, 0)])
+@pytest.mark.parametrize("L,q,init,T,seed,n", ROWS_CASES)
+def test_nnn_row_walking_kernel(pb, L, q, init, T, seed, n, words, rows):
+    g = pb.Potts8(L, q, seed, init)
+    g.potts8_set_option("stream_words", words)
+    g.potts8_set_option("stream_rows", rows)
+    o = oracle.OraclePotts8(L, q, seed, init, threads=8)
+    Eg, Hg = g.potts8_sweep_measured(T, n, 1, hist=True)
+    Eo, Ho = o.sweep_measured(T, n, 1, hist=True)
+    assert (Eg == Eo).all() and (Hg == Ho).all()
+    assert (g.potts8_download() == o.spins()).all()
+
+
+def test_nnn_options_and_kernels_agree_at_several_column_blocks(pb):
+    g = pb.Potts8(48, 9, 1)
+    for key, value in (("stream_words", 2), ("stream_rows", 3), ("nonsense", 1)):
+        with pytest.raises(pb.PottsError) as e:
+            g.potts8_set_option(key, value)
+        assert e.value.code == pb.ERR_ARG
+    L, q, T, seed = 3072, 9, 2.0, 21
+    a = pb.Potts8(L, q, seed, pb.INIT_RANDOM)
+    b = pb.Potts8(L, q, seed, pb.INIT_RANDOM)
+    b.potts8_set_option("stream_words", -1)
+    o = oracle.OraclePotts8(L, q, seed, pb.INIT_RANDOM, threads=16)
+    Ea, Ha = a.potts8_sweep_measured(T, 2, 1, hist=True)
+    Eb, Hb = b.potts8_sweep_measured(T, 2, 1, hist=True)
+    Eo, Ho = o.sweep_measured(T, 2, 1, hist=True)
+    assert (Ea == Eo).all() and (Ha == Ho).all() and (Eb == Eo).all() and (Hb == Ho).all()
+    assert (a.potts8_download() == o.spins()).all() and (b.potts8_download() == o.spins()).all()
