@@ -457,8 +457,8 @@ def cubic_lattice(pb, torch, peaks, L=512, q=9, sweeps=40, repeats=3):
 
 
 def second_neighbour_lattice(pb, torch, peaks, L=12288, q=9, sweeps=20, repeats=3):
-    """SURVEY 8(f)4 / PAPER.md:359: first + second neighbour interactions, nine sub-networks (potts8_sweep, k_sweep8_u8:
-    one launch per sub-network, one 4-site word per thread, first CUDA path of this row); random start, T = 2.0.
+    """SURVEY 8(f)4 / PAPER.md:359: first + second neighbour interactions, nine sub-networks (potts8_sweep,
+    k_sweep8_rows_u8: one launch per sub-network, 16 sites per lane and row visit); random start, T = 2.0.
     Algorithmic counts per update: 36 instructions; bytes: own read + write, each other site read once per sub-network
     that neighbours it (8 of 9): 10 B without on-chip reuse across launches."""
     hbm_gbs, sm_max, which = peaks
@@ -676,6 +676,7 @@ def main():
         per_cfg["potts3d_q9_L512"] = cubic_lattice(pb, torch, peaks)
         per_cfg["potts3d_q9_L1024"] = cubic_lattice(pb, torch, peaks, L=1024, sweeps=10)      # 2^30 sites, as the headline
         per_cfg["potts8_q9_L12288"] = second_neighbour_lattice(pb, torch, peaks)
+        per_cfg["potts8_q9_L24576"] = second_neighbour_lattice(pb, torch, peaks, L=24576, sweeps=10)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(w)
     if dist is not None:
