@@ -308,6 +308,28 @@ int  potts8_launch_count(potts8_t *h, uint64_t *n);
  *                   per tile (1, 2, 4, 8 or 16) */
 int  potts8_set_option(potts8_t *h, const char *key, int64_t value);
 
+/* ---- no-allocation entry point ------------------------------------------------------------------------------------
+ * potts_measure_noalloc: energy (R1: E = -(number of satisfied bonds), Eq. 1) and q-bin histogram (R8,
+ * PAPER.md:175) of a lattice the CALLER holds on the device, for callers that cannot call cudaMalloc (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it).  The same kernel as potts_energy / potts_histogram
+ * (k_measure_u8), with its colour planes and accumulators in a file-scope device array of fixed size instead of a
+ * handle's cudaMalloc'ed workspace: the call allocates and frees nothing, needs no handle, and every GPU that loads the
+ * library holds that array (POTTS_NOALLOC_MAX_L^2 + 4096 bytes = 4 MiB + 4 KiB) until the process exits.
+ *   spins_dev  DEVICE pointer, L*L bytes, row-major s[i*L + j] in 0..q-1, 8-byte aligned; read only
+ *   L, q       L even, L % 32 == 0 (POTTS_ERR_UNSUPPORTED otherwise), L <= POTTS_NOALLOC_MAX_L (POTTS_ERR_UNSUPPORTED
+ *              beyond: use a potts_t handle); 2 <= q <= 256
+ *   E_dev      DEVICE pointer to one int64, or null;  hist_dev  DEVICE pointer to q int64, or null (not both null);
+ *              caller-owned, written by the call.  A spin value >= q cannot be reported through the return code
+ *              without a synchronisation: it sets *E_dev = INT64_MIN and every hist_dev[k] = -1 instead.
+ *   cuda_stream  the stream the work is enqueued on (null = default stream); the device of the pointers must be current.
+ * The call returns once the work is enqueued (no synchronisation); results are valid when the stream reaches that point.
+ * The first call on a device resolves the array's address (cudaGetSymbolAddress; this may load the module): a caller
+ * that captures graphs makes one call outside capture first.  ALL calls share the one array: it is cleared where needed
+ * at the start of each call, and calls that overlap on the GPU (different streams without ordering, several host
+ * threads) race on it -- the caller serialises them.  Argument errors are returned before any CUDA call. */
+#define POTTS_NOALLOC_MAX_L 2048
+int  potts_measure_noalloc(const uint8_t *spins_dev, int32_t L, int32_t q, int64_t *E_dev, int64_t *hist_dev, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -94,6 +94,7 @@ def load_library() -> ctypes.CDLL:
         "potts3_launch_count": ([vp, P(u64)], ctypes.c_int),
         "potts3_set_option": ([vp, ctypes.c_char_p, i64], ctypes.c_int),
         "potts8_set_option": ([vp, ctypes.c_char_p, i64], ctypes.c_int),
+        "potts_measure_noalloc": ([vp, i32, i32, vp, vp, vp], ctypes.c_int),
         "potts8_create": ([P(vp), i32, i32, u64, i32, vp], ctypes.c_int),
         "potts8_destroy": ([vp], None),
         "potts8_sweep": ([vp, dbl, i64], ctypes.c_int),
@@ -129,6 +130,7 @@ EXPORTED_SYMBOLS = [
     "potts3_download", "potts3_upload", "potts3_sweep_count", "potts3_set_sweep_count", "potts3_launch_count", "potts3_set_option",
     "potts8_create", "potts8_destroy", "potts8_sweep", "potts8_sweep_measured", "potts8_energy", "potts8_histogram",
     "potts8_download", "potts8_upload", "potts8_sweep_count", "potts8_set_sweep_count", "potts8_launch_count", "potts8_set_option",
+    "potts_measure_noalloc",
 ]
 
 
@@ -154,6 +156,27 @@ def potts_observables(E_series, N: int, T: float):
     _check(load_library().potts_observables(E.ctypes.data, E.size, int(N), float(T),
                                             ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
     return a.value, b.value, c.value
+
+
+NOALLOC_MAX_L = 2048     # POTTS_NOALLOC_MAX_L of include/potts.h
+
+
+def potts_measure_noalloc(spins, q: int, E_out=None, hist_out=None, stream: int = 0):
+    """Energy and histogram of a device lattice without any allocation (include/potts.h, potts_measure_noalloc).
+
+    spins: uint8 CUDA tensor [L, L] (contiguous); E_out: int64 CUDA tensor of 1 element or None; hist_out: int64 CUDA
+    tensor of q elements or None -- all caller-owned, on the current device.  Enqueues on `stream` (a raw CUDA stream
+    handle, 0 = default) and returns without synchronising."""
+    L = int(spins.shape[0])
+    if tuple(spins.shape) != (L, L) or not spins.is_contiguous() or not spins.is_cuda or spins.element_size() != 1:
+        raise PottsError(ERR_ARG, "spins must be a contiguous uint8 CUDA tensor of shape [L, L]")
+    for t, n in ((E_out, 1), (hist_out, int(q))):
+        if t is not None and (not t.is_cuda or t.element_size() != 8 or t.numel() != n or not t.is_contiguous()):
+            raise PottsError(ERR_ARG, "E_out / hist_out must be contiguous int64 CUDA tensors of 1 / q elements")
+    _check(load_library().potts_measure_noalloc(
+        ctypes.c_void_p(spins.data_ptr()), L, int(q),
+        ctypes.c_void_p(E_out.data_ptr()) if E_out is not None else None,
+        ctypes.c_void_p(hist_out.data_ptr()) if hist_out is not None else None, ctypes.c_void_p(int(stream))))
 
 
 def potts_magnetisation(counts, q: int) -> float:

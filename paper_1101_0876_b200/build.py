@@ -19,7 +19,8 @@ OBJ = os.path.join(HERE, "build")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libpotts_b200.so")
 SOURCES = ["potts_api.cu", "k_stream.cu", "k_stream_s1c0.cu", "k_stream_s1c1.cu", "k_stream_s2c0.cu", "k_stream_s2c1.cu",
-           "k_packed.cu", "k_packed_s1.cu", "k_packed_s2.cu", "k_resident.cu", "k_cluster.cu", "potts3d_api.cu", "potts8_api.cu"]
+           "k_packed.cu", "k_packed_s1.cu", "k_packed_s2.cu", "k_resident.cu", "k_cluster.cu", "potts3d_api.cu", "potts8_api.cu",
+           "potts_noalloc.cu"]
 HEADERS = ["potts_core.cuh", "potts_kernels.cuh", "potts_resident.cuh", "potts_packed.cuh", "potts_cluster.cuh",
            "potts_launch.cuh", "potts3d.cuh", "potts8.cuh", "k_stream.inl", "k_packed.inl", os.path.join(INCLUDE, "potts.h")]
 
