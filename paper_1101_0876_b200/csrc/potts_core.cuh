@@ -47,6 +47,9 @@ __device__ __forceinline__ uint32_t in_register(uint32_t v)
     return r;
 }
 
+// 32-bit shared-window address of a shared-memory pointer (operand of mbarrier / bulk-copy / st.async instructions)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
 // three-input logic in one LOP3; LUT = f(0xF0, 0xCC, 0xAA)
 template <int LUT>
 __device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c)
@@ -563,13 +566,26 @@ __device__ __forceinline__ void hist_flush(uint32_t *s_hist, uint32_t q, unsigne
                                            uint32_t nthreads)
 {
     if (q <= HIST_LANE_QMAX) {
-        // one warp per state: lanes read the 32 private counters, shuffle-reduce
+        // one warp per state: lanes read the 32 private counters, one REDUX per state.  Four states per trip, so that the
+        // loads, the reductions and the atomics of a warp's states overlap instead of forming one dependent chain per state
+        // (the flush sits between two half-sweeps of the persistent kernels: its latency is on their critical path)
         const uint32_t warp = tid >> 5, lane = tid & 31u, nwarps = nthreads >> 5;
-        for (uint32_t k = warp; k < q; k += nwarps) {
-            uint32_t v = s_hist[k * 32u + lane];
-            s_hist[k * 32u + lane] = 0u;
-            v = __reduce_add_sync(0xffffffffu, v);                     // one REDUX instead of a five-step shuffle tree
-            if (lane == 0 && v) atomicAdd(hist_out + k, (unsigned long long)v);
+        for (uint32_t k0 = warp; k0 < q; k0 += 4u * nwarps) {
+            uint32_t v[4];
+#pragma unroll
+            for (uint32_t u = 0; u < 4; ++u) {
+                const uint32_t k = k0 + u * nwarps;
+                v[u] = 0u;
+                if (k < q) {
+                    v[u] = s_hist[k * 32u + lane];
+                    s_hist[k * 32u + lane] = 0u;
+                }
+            }
+#pragma unroll
+            for (uint32_t u = 0; u < 4; ++u) v[u] = __reduce_add_sync(0xffffffffu, v[u]);
+#pragma unroll
+            for (uint32_t u = 0; u < 4; ++u)
+                if (lane == 0 && v[u]) atomicAdd(hist_out + k0 + u * nwarps, (unsigned long long)v[u]);
         }
     } else {
         for (uint32_t k = tid; k < q; k += nthreads) {

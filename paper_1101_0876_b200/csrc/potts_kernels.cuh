@@ -64,8 +64,6 @@ constexpr int HS_SITES = 16;          // same-colour sites per lane and row
 // global memory.  Needs pitch % 512 == 0 (every lane active) and no histogram (the dynamic shared memory is the stage).
 constexpr int BULK_ROW = 544;                                 // 16 + 512 + 16 bytes
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
 template <int CM, int ST, int COLOUR, bool MEASURE, bool HIST, bool DELTA, bool FAST, bool BULK = false>
 __global__ void __launch_bounds__(32 * HS_WARPS) k_sweep_rows_u8(const __grid_constant__ SweepParams P)
 {

@@ -405,6 +405,48 @@ def test_persistent_kernels_are_deterministic_under_repetition(pb):
             g.close()
 
 
+@pytest.mark.parametrize("L,q,ctas", [(64, 9, 4), (64, 9, 1), (32, 6, 2), (128, 24, 16), (96, 3, 3), (64, 200, 8)])
+def test_cluster_kernel_mbarrier_phases_over_many_launches(pb, L, q, ctas):
+    """The cluster kernel's neighbour exchange (st.async into the neighbour's halo, completion counted by an mbarrier in
+    the receiver's shared memory, potts_cluster.cuh) keeps one phase per sweep and halo: launches of 1, 2, 3, ... sweeps
+    (odd and even phase counts, the wait-free first half-sweep, the drained last one), with every measurement form in
+    turn, must follow the oracle's chain bit for bit, and repeat it."""
+    seed = 21
+    T = 0.99 * workloads.t_c(q)
+    for rep in range(2):
+        g = pb.Potts(L, q, seed, workloads.INIT_RANDOM)
+        g.potts_set_option("variant", 3)
+        g.potts_set_option("cluster_ctas", ctas)
+        assert g.potts_get_option("cluster_active") == ctas
+        o = oracle.OraclePotts(L, q, seed, workloads.INIT_RANDOM)
+        for k, n in enumerate([1, 1, 2, 3, 1, 4, 7, 2, 5, 16, 1]):
+            kind = k % 4
+            if kind == 0:
+                g.potts_sweep(T, n)
+                o.sweep(T, n)
+            elif kind == 1:
+                Eg, Hg = g.potts_sweep_measured(T, n, 1, hist=True)
+                Eo, Ho = o.sweep_measured(T, n, 1, hist=True)
+                assert (Eg == Eo).all() and (Hg == Ho).all(), (rep, k, n)
+            elif kind == 2:
+                e0 = o.energy()
+                d = g.potts_sweep_delta(T, n)
+                es = []
+                for _ in range(n):
+                    o.sweep(T, 1)
+                    es.append(o.energy())
+                assert (d == np.diff(np.array([e0] + es, dtype=np.int64))).all(), (rep, k, n)
+            else:
+                every = 2 if n % 2 == 0 else 1
+                Eg, Hg = g.potts_sweep_measured(T, n, every, hist=False)
+                Eo, Ho = o.sweep_measured(T, n, every, hist=False)
+                assert (Eg == Eo).all(), (rep, k, n)
+            assert g.potts_energy() == o.energy(), (rep, k, n)
+        assert (g.potts_download() == o.spins()).all()
+        assert (g.potts_histogram() == o.histogram()).all()
+        g.close()
+
+
 @pytest.mark.parametrize("L,q,seed,rows", [(1024, 9, 3, 0), (2048, 6, 8, 4), (1024, 24, 5, 16), (1024, 200, 2, 2)])
 def test_streaming_kernel_with_bulk_staged_rows(pb, L, q, seed, rows):
     """Option stream_stage = 1 (cp.async.bulk staging of the other-colour rows, an experiment kept for its A/B record)
