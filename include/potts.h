@@ -211,7 +211,7 @@ int potts_launch_count(potts_t *h, uint64_t *n);
  *                      L2/HBM), 2 = resident (one persistent cooperative launch per call, lattice in shared
  *                      memory; U8 layout, L <= 4096; POTTS_ERR_UNSUPPORTED from the sweep call otherwise)
  *                      3 = cluster (one thread-block cluster of up to 16 CTAs, boundary rows through distributed
- *                      shared memory; the automatic choice for L <= 128)
+ *                      shared memory; the automatic choice for L <= 288)
  *   "cluster_ctas"     0 = automatic, else the cluster size (1..16); "cluster_active" (read-only) = the cluster
  *                      size the next sweep call would use, 0 if it would not use the cluster kernel
  *   "resident_ctas"    0 = automatic, else the number of CTAs the resident kernel splits the rows over

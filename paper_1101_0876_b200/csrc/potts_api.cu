@@ -52,7 +52,7 @@ constexpr size_t ALIGN = 256;
 constexpr size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 constexpr int MAX_CTAS = 160;             // upper bound on the resident kernel's grid (>= SM count of B200)
 constexpr int RESIDENT_L_MAX = 4096;       // largest lattice the resident kernel can hold (512 words per row)
-constexpr int CLUSTER_AUTO_L_MAX = 128;    // lattices up to this size go to the cluster (DSMEM) kernel by default (measured: 2x the resident kernel)
+constexpr int CLUSTER_AUTO_L_MAX = 288;    // lattices up to this size go to the cluster (DSMEM) kernel by default (measured, profiles/r02h_cluster_exchange.md: 2.3x the resident kernel at L = 128, 1.2x at L = 288, 0.96x at L = 320)
 constexpr int ACC_WORDS = 1 + 256 + 2;    // E, hist[256], flag/error word, tile counter of the streaming kernels
 constexpr size_t STATIC_SMEM = sizeof(potts::AcceptLutWide) + 1024;   // static shared memory of the persistent kernels
 

@@ -38,7 +38,7 @@ CASES = [
 ]
 
 
-# launch shapes of potts_sweep_delta: the library's choice (cluster kernel for L <= 128, resident kernel up to L = 4096,
+# launch shapes of potts_sweep_delta: the library's choice (cluster kernel for L <= 288, resident kernel up to L = 4096,
 # one launch per call), the streaming kernels (two launches per sweep), the resident kernel with forced grids, a cluster
 VARIANTS = {
     "auto": {},
