@@ -668,7 +668,7 @@ def main():
         per_cfg[w.name + "_without_measurement"]["frac"] = plain["roofline"]["frac"]
         e6 = paper_protocol_e6(pb, torch)
         per_cfg["batch_cfg1_x1184"] = batch_of_cfg1(pb, torch)
-        # 6 such CTAs are resident per SM: 888 lattices are exactly one wave (1184 are two, the second 1/3 full)
+        # 3 such CTAs (256 threads, 78 registers) are resident per SM: 888 lattices are exactly two waves, 1184 are 2 2/3
         per_cfg["batch_cfg1_x888"] = batch_of_cfg1(pb, torch, n=888)
         per_cfg["delta_cfg5_streaming"] = delta_cost(pb, torch, 5, 100)
         per_cfg["delta_cfg4_packed"] = delta_cost(pb, torch, 4, 200)

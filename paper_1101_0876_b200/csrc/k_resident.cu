@@ -23,14 +23,22 @@ const void *resident_kernel_cm(int stream_spec, int W, int small)
     return stream_spec == 2 ? resident_kernel_st<CM, 2>(W, small) : resident_kernel_st<CM, 1>(W, small);
 }
 
-template <int CM, int ST>
-cudaError_t launch_batch_st(const BatchParams &B, const BatchTable &T, int n, int nthreads, size_t smem, cudaStream_t st)
+template <int CM, int ST, int MAXT>
+cudaError_t launch_batch_fn(const BatchParams &B, const BatchTable &T, int n, int nthreads, size_t smem, cudaStream_t st)
 {
-    auto fn = k_resident_batch_u8<CM, ST, 1024>;      // 64 registers: several small lattices per SM
+    auto fn = k_resident_batch_u8<CM, ST, MAXT>;
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     fn<<<(unsigned)n, (unsigned)nthreads, smem, st>>>(B, T);
     return cudaGetLastError();
+}
+
+template <int CM, int ST>
+cudaError_t launch_batch_st(const BatchParams &B, const BatchTable &T, int n, int nthreads, size_t smem, cudaStream_t st)
+{
+    // register budget by block size: up to 256 threads several blocks per SM, up to 512 threads 128 registers, else 64
+    if (nthreads <= 256) return launch_batch_fn<CM, ST, 256>(B, T, n, nthreads, smem, st);
+    return nthreads <= 512 ? launch_batch_fn<CM, ST, 512>(B, T, n, nthreads, smem, st) : launch_batch_fn<CM, ST, 1024>(B, T, n, nthreads, smem, st);
 }
 
 template <int CM>

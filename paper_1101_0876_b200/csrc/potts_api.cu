@@ -1281,14 +1281,22 @@ struct BatchPlan { bool ok = false; int tyc = 0, nthreads = 0; size_t smem = 0; 
 BatchPlan plan_batch(int32_t L, int32_t q, size_t smem_optin)
 {
     BatchPlan R;
-    const int wpr = L / 8, comm = (L / 16 + 31) / 32 * 32;         // one 4-site word per compute thread and row visit
-    int tyc = (1024 - comm) / wpr;
-    if (tyc > L) tyc = L;
-    if (tyc > (L + 1) / 2) tyc = (L + 1) / 2;                      // two visits per thread: measured 4.6 against 6.9 ps per update at L = 64 (half the per-half-sweep bookkeeping per site, twice the CTAs per SM)
-    if (tyc < 1) { R.why = "no room for a compute row in a 1024-thread block"; return R; }
+    const int wpr = L / 8;                                         // one 4-site word per thread and row visit; no comm warps (one CTA = one lattice)
+    // Two visits per thread where the block allows (measured 4.6 against 6.9 ps per update at L = 64 for two visits against
+    // one: half the per-half-sweep bookkeeping per site, twice the CTAs per SM), in a block of at most 512 threads (up to 128
+    // registers); lattices too large for that within 8 visits take a block of up to 1024 threads (64 registers).
+    // An EVEN number of thread rows: a thread's rows then share one parity and its ColKeys (potts_resident.cuh).
+    int tyc = 512 / wpr;
+    if (tyc > L / 2) tyc = L / 2;
+    tyc &= ~1;
+    if (tyc < 2 || (L + tyc - 1) / tyc > 8) {
+        tyc = 1024 / wpr;
+        if (tyc > L / 2) tyc = L / 2;
+        tyc &= ~1;
+    }
+    if (tyc < 2) { R.why = "no room for two thread rows in a 1024-thread block"; return R; }
     R.tyc = tyc;
-    R.nthreads = (wpr * tyc + 31) / 32 * 32 + comm;
-    if ((L + tyc - 1) / tyc > 30) { R.why = "too many rows per thread"; return R; }
+    R.nthreads = (wpr * tyc + 31) / 32 * 32;
     const size_t hist = (size_t)(q <= (int)potts::HIST_LANE_QMAX ? q * 32 : q) * 4;
     R.smem = 2 * (size_t)(L + 2) * (L / 2) + hist;
     if (R.smem + STATIC_SMEM > smem_optin) { R.why = "one lattice does not fit the shared memory of a CTA"; return R; }

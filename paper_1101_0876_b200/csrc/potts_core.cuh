@@ -510,6 +510,29 @@ __device__ __forceinline__ uint32_t update_word_h(uint32_t own, uint32_t up, uin
     return metropolis_word<CM, false, SLOTS>(own, nb, q, w0, w1, lut, lane_off, code, mask);
 }
 
+// The same with the ColKeys of the word's four columns in the caller's registers (the replica-batch kernel, whose
+// threads visit rows of one parity only).
+template <int CM, int ST, int SLOTS>
+__device__ __forceinline__ uint32_t update_word_r(uint32_t own, uint32_t up, uint32_t dn, uint32_t lf, uint32_t rt,
+                                                  const ColKeys *ck, uint32_t q, const HalfSweepKeys &K, const RowKeysH &R,
+                                                  const AcceptLutT<SLOTS> *lut, uint32_t lane_off, uint32_t &code, uint32_t &mask)
+{
+    uint32_t w0[4], w1[4];
+    if (ST == 1) {
+#pragma unroll
+        for (int b = 0; b < 4; ++b) philox_site_h(K, R, ck[b], w0[b], w1[b]);
+    } else {
+#pragma unroll
+        for (int m = 0; m < 2; ++m) {
+            uint32_t w[4];
+            philox_pair_h(K, R, ck[2 * m], w);
+            w0[2 * m] = w[0]; w1[2 * m] = w[1]; w0[2 * m + 1] = w[2]; w1[2 * m + 1] = w[3];
+        }
+    }
+    const uint32_t nb[4] = {prep_nbr<CM>(up), prep_nbr<CM>(dn), prep_nbr<CM>(lf), prep_nbr<CM>(rt)};
+    return metropolis_word<CM, false, SLOTS>(own, nb, q, w0, w1, lut, lane_off, code, mask);
+}
+
 // ---------------------------------------------------------------------------------------------
 // Standalone measurement helpers: byte-parallel "not equal" flags (bit 7 of every byte of the result is
 // set iff the bytes of a and b differ).  WIDE = false assumes all spin values < 128.

@@ -390,23 +390,127 @@ struct BatchParams {
     unsigned long long delta_stride;     // entries per lattice in dE_series
 };
 
+// One CTA = one whole lattice, so the body is much simpler than resident_run: no packets, no comm warps, no halo rows
+// to fill (the row above local row 1 IS local row L, read in place), one block barrier per half-sweep.  Block =
+// L/8 x tyc threads with tyc EVEN: thread row ty visits the rows 1+ty, 1+ty+tyc, ..., all of one parity, so the column
+// part of Philox (ColKeys) of its four columns is computed once per half-sweep into registers and serves every visit.
+#ifndef POTTS_BATCH_MINB
+#define POTTS_BATCH_MINB 3
+#endif
 template <int CM, int ST, int MAXT>
-__global__ void __launch_bounds__(MAXT, 1) k_resident_batch_u8(const __grid_constant__ BatchParams B, const __grid_constant__ BatchTable T)
+__global__ void __launch_bounds__(MAXT, MAXT <= 256 ? POTTS_BATCH_MINB : 1) k_resident_batch_u8(const __grid_constant__ BatchParams B, const __grid_constant__ BatchTable T)
 {
+    extern __shared__ __align__(16) uint8_t s_raw[];
+    __shared__ AcceptLutWide lut;
+    const ResidentParams &P = B.P;
     const uint32_t r = blockIdx.x;
-    ResidentLattice X;
-    X.G = 1u;
-    X.b = 0u;
-    X.plane[0] = B.P.plane[0] + r * B.lattice_stride;
-    X.plane[1] = B.P.plane[1] + r * B.lattice_stride;
-    X.key0 = T.key[r][0];
-    X.key1 = T.key[r][1];
+    uint8_t *const plane0 = P.plane[0] + r * B.lattice_stride, *const plane1 = P.plane[1] + r * B.lattice_stride;
+    const uint32_t key0 = T.key[r][0], key1 = T.key[r][1];
+    unsigned long long *const E_series = P.E_series ? P.E_series + r * B.series_stride : nullptr;
+    unsigned long long *const hist_series = P.hist_series ? P.hist_series + r * B.series_stride * P.q : nullptr;
+    unsigned long long *const dE_series = P.dE_series ? P.dE_series + r * B.delta_stride : nullptr;
+
+    const int L = P.L, pitch = P.pitch, rows = L;
+    const uint32_t plane_stride = (uint32_t)(rows + 2) * (uint32_t)pitch;   // local row lr at lr * pitch; rows 0 and L+1 unused
+    uint32_t *s_hist = reinterpret_cast<uint32_t *>(s_raw + 2 * plane_stride);
+    const uint32_t tid = threadIdx.x, nthreads = blockDim.x;
+    const int wpr = pitch >> 2, tyc = P.tyc;
+    const bool is_compute = (int)tid < wpr * tyc;
+    const int ty = is_compute ? (int)tid / wpr : 0;
+    const uint32_t col = is_compute ? 4u * (uint32_t)((int)tid - ty * wpr) : 0u;
+    const uint32_t col_prev = col == 0u ? (uint32_t)pitch - 4u : col - 4u;
+    const uint32_t col_next = col + 4u == (uint32_t)pitch ? 0u : col + 4u;
+    const bool do_hist = hist_series != nullptr && P.every != 0;
+    const bool do_E = E_series != nullptr && P.every != 0;
+    const bool do_D = dE_series != nullptr;
+    const uint32_t q = in_register(P.q);
+
+    accept_lut_fill(&lut, T.thr[r], tid, nthreads);
+    const uint32_t lane_off = accept_lane_offset<AcceptLutWide::slots>(tid);
+    if (do_hist)
+        for (uint32_t n = tid; n < hist_words(P.q); n += nthreads) s_hist[n] = 0u;
+    {
+        const int vpr = pitch >> 4;
+        for (int c = 0; c < 2; ++c)
+            for (int n = (int)tid; n < rows * vpr; n += (int)nthreads) {
+                const int gr = n / vpr, v = n - gr * vpr;
+                *reinterpret_cast<uint4 *>(s_raw + c * plane_stride + (uint32_t)((gr + 1) * pitch + 16 * v)) =
+                    __ldcg(reinterpret_cast<const uint4 *>((c ? plane1 : plane0) + (size_t)gr * pitch + 16 * v));
+            }
+    }
+    __syncthreads();
+
+    const HalfSweepKeys K0 = half_sweep_keys(key0, key1, 0u, 0u);
+    uint32_t until = P.every, sample_idx = 0;
+    for (uint32_t n = 0; n < P.nsweeps; ++n) {
+        const uint32_t t = P.t0 + n;
+        const bool sample = P.every != 0 && --until == 0;
+        if (sample) until = P.every;
 #pragma unroll
-    for (int d = 0; d < 4; ++d) X.thr[d] = T.thr[r][d];
-    X.E_series = B.P.E_series ? B.P.E_series + r * B.series_stride : nullptr;
-    X.hist_series = B.P.hist_series ? B.P.hist_series + r * B.series_stride * B.P.q : nullptr;
-    X.dE_series = B.P.dE_series ? B.P.dE_series + r * B.delta_stride : nullptr;
-    resident_run<CM, 1, ST>(B.P, X);      // one word per thread and row visit: small lattices want warps, not amortisation
+        for (uint32_t c = 0; c < 2; ++c) {
+            uint8_t *const own_col = s_raw + c * plane_stride + col;
+            const uint8_t *const oth = s_raw + (1u - c) * plane_stride;
+            HalfSweepKeys K = K0;
+            half_sweep_rekey(K, key0, key1, t, c);
+            const bool count_E = sample && c == 1 && do_E, count_H = sample && do_hist;
+            int d_sum = 0, ne_sum = 0;
+            uint32_t words_done = 0;
+            if (is_compute) {
+                // global row i = lr - 1; every row of this thread has the parity of ty, so p and the columns are fixed
+                const uint32_t p = ((uint32_t)ty + c) & 1u;
+                ColKeys ck[4];
+#pragma unroll
+                for (int s = 0; s < 4; ++s) ck[s] = col_keys(K, 2u * col + p + 2u * (uint32_t)s);
+                for (int lr = 1 + ty; lr <= rows; lr += tyc) {
+                    const uint32_t ro = (uint32_t)(lr * pitch);
+                    const uint32_t ro_up = lr == 1 ? (uint32_t)(rows * pitch) : ro - (uint32_t)pitch;      // periodic, in place
+                    const uint32_t ro_dn = lr == rows ? (uint32_t)pitch : ro + (uint32_t)pitch;
+                    const uint32_t own = *reinterpret_cast<const uint32_t *>(own_col + ro);
+                    const uint32_t mid = *reinterpret_cast<const uint32_t *>(oth + ro + col);
+                    const uint32_t up = *reinterpret_cast<const uint32_t *>(oth + ro_up + col);
+                    const uint32_t dn = *reinterpret_cast<const uint32_t *>(oth + ro_dn + col);
+                    const uint32_t adj = *reinterpret_cast<const uint32_t *>(oth + ro + (p ? col_next : col_prev));
+                    uint32_t lf, rt;
+                    horizontal(p, mid, adj, lf, rt);
+                    const RowKeysH R = row_keys_h(K, (uint32_t)(lr - 1));
+                    uint32_t code, mask;
+                    const uint32_t out = update_word_r<CM, ST, AcceptLutWide::slots>(own, up, dn, lf, rt, ck, q, K, R, &lut, lane_off, code, mask);
+                    *reinterpret_cast<uint32_t *>(own_col + ro) = out;
+                    if (count_E) ne_sum += ne_final_sum(code, mask);
+                    if (do_D) d_sum += delta_sum(code, mask);
+                    ++words_done;
+                    if (count_H) hist_add_word(s_hist, P.q, out, tid & 31u);
+                }
+            }
+            __syncthreads();                                        // plane c complete
+            if (do_D) {
+                int dd = d_sum;
+                dd = __reduce_add_sync(0xffffffffu, dd);                     // one REDUX instead of a five-step shuffle tree
+                if ((tid & 31u) == 0 && dd) atomicAdd(dE_series + n, (unsigned long long)(long long)dd);
+            }
+            if (sample && c == 1) {
+                if (do_E) {
+                    uint32_t satisfied = 16u * words_done - (uint32_t)ne_sum;
+                    satisfied = __reduce_add_sync(0xffffffffu, satisfied);                     // one REDUX instead of a five-step shuffle tree
+                    if ((tid & 31u) == 0 && satisfied) atomicAdd(E_series + sample_idx, 0ull - (unsigned long long)satisfied);
+                }
+                if (do_hist) {
+                    hist_flush(s_hist, P.q, hist_series + (size_t)sample_idx * P.q, tid, nthreads);
+                    __syncthreads();                                // the table is zero again before the next sample counts
+                }
+                ++sample_idx;
+            }
+        }
+    }
+    {
+        const int vpr = pitch >> 4;
+        for (int c = 0; c < 2; ++c)
+            for (int n = (int)tid; n < rows * vpr; n += (int)nthreads) {
+                const int gr = n / vpr, v = n - gr * vpr;
+                *reinterpret_cast<uint4 *>((c ? plane1 : plane0) + (size_t)gr * pitch + 16 * v) =
+                    *reinterpret_cast<const uint4 *>(s_raw + c * plane_stride + (uint32_t)((gr + 1) * pitch + 16 * v));
+            }
+    }
 }
 
 }  // namespace potts
