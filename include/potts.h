@@ -123,7 +123,7 @@ int potts_ladder(potts_t *h, const double *T, int32_t nT, int64_t t_tran, int64_
 /* ---- replica batch (the paper averages over samples and scans temperatures) --------
  * n independent lattices of the same (L, q), lattice r with Philox key seeds[r], all advanced by one kernel launch
  * per call: CTA r keeps lattice r in its shared memory (U8 layout, L % 32 == 0, 2 (L+2) L/2 bytes must fit one CTA:
- * L <= 448).  Lattice r of a batch follows exactly the chain of a single handle created with (L, q, seeds[r], init).
+ * L <= 416).  Lattice r of a batch follows exactly the chain of a single handle created with (L, q, seeds[r], init).
  * seeds, T: host arrays of n entries.  dev_workspace: device memory of potts_batch_workspace_bytes() bytes, 256-byte
  * aligned, or null (the library allocates).  */
 typedef struct potts_batch_s potts_batch_t;

@@ -134,6 +134,17 @@ EXPORTED_SYMBOLS = [
 ]
 
 
+def _host_series(shape) -> np.ndarray:
+    """int64 host array for a series the library copies from the device: page-locked (torch's caching host allocator, so
+    repeated calls reuse the pages) once it is large enough for the copy to matter -- a pageable destination takes the
+    driver's bounce-buffer path at a fraction of the PCIe rate.  Marshalling only; the contents come from the kernels."""
+    n = int(np.prod(shape))
+    if n * 8 >= (1 << 20):
+        import torch
+        return torch.empty(tuple(int(x) for x in shape), dtype=torch.int64, pin_memory=True).numpy()
+    return np.zeros(shape, dtype=np.int64)
+
+
 def _check(rc: int):
     if rc != OK:
         raise PottsError(rc, load_library().potts_last_error().decode())
@@ -379,8 +390,8 @@ class PottsBatch:
         """T: one temperature per lattice.  -> (E int64[n, ns] or None, hist int64[n, ns, q] or None)."""
         Ta = np.ascontiguousarray(np.broadcast_to(np.asarray(T, dtype=np.float64), (self.n,)))
         ns = int(nsweeps) // int(every) if every >= 1 and nsweeps >= 0 else 0
-        E = np.zeros((self.n, ns), dtype=np.int64) if energy else None
-        H = np.zeros((self.n, ns, self.q), dtype=np.int64) if hist else None
+        E = _host_series((self.n, ns)) if energy else None
+        H = _host_series((self.n, ns, self.q)) if hist else None
         _check(self._lib.potts_batch_sweep_measured(self._h, Ta.ctypes.data, int(nsweeps), int(every),
                                                     E.ctypes.data if energy else None, H.ctypes.data if hist else None))
         return E, H
@@ -395,7 +406,7 @@ class PottsBatch:
     def potts_batch_sweep_delta(self, T, nsweeps: int) -> np.ndarray:
         """-> dE int64[n, nsweeps]: energy change of every sweep of every lattice, from its accepted moves."""
         Ta = np.ascontiguousarray(np.broadcast_to(np.asarray(T, dtype=np.float64), (self.n,)))
-        dE = np.zeros((self.n, int(nsweeps)), dtype=np.int64)
+        dE = _host_series((self.n, int(nsweeps)))
         _check(self._lib.potts_batch_sweep_delta(self._h, Ta.ctypes.data, int(nsweeps), dE.ctypes.data))
         return dE
 
@@ -407,8 +418,8 @@ class PottsBatch:
         Ta = np.ascontiguousarray(Ta)
         nT = Ta.shape[1]
         per = int(t_max) // int(dt) if dt >= 1 else 0
-        E = np.zeros((self.n, nT, per), dtype=np.int64) if energy else None
-        H = np.zeros((self.n, nT, per, self.q), dtype=np.int64) if hist else None
+        E = _host_series((self.n, nT, per)) if energy else None
+        H = _host_series((self.n, nT, per, self.q)) if hist else None
         _check(self._lib.potts_batch_ladder(self._h, Ta.ctypes.data, nT, int(t_tran), int(t_max), int(dt),
                                             E.ctypes.data if energy else None, H.ctypes.data if hist else None))
         return E, H

@@ -440,7 +440,7 @@ int launch_cluster(potts_t *h, const ClusterPlan &R, const uint32_t thr[4], int6
     P.error = h->error;
     P.rows_max = R.rows_max;
     P.tyc = R.tyc;
-    const void *fn = potts::cluster_kernel(potts::compare_mode_of(h->q), h->stream_spec);
+    const void *fn = potts::cluster_kernel(potts::compare_mode_of(h->q), h->stream_spec, R.nthreads);
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R.smem));
     if (R.G > 8) CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     cudaLaunchConfig_t cfg = {};

@@ -69,8 +69,9 @@ constexpr int CLUSTER_MAX = 16;     // 8 is the portable cluster size; B200 take
 
 // Block = wpr x tyc threads (wpr = L/8 words per plane row); thread (tx, ty) updates word tx of local rows
 // 1+ty, 1+ty+tyc, ...  P.inbox is unused; P.error is set if a wait for a neighbour gives up.
-template <int CM, int ST>
-__global__ void __launch_bounds__(1024, 1) k_cluster_u8(const __grid_constant__ ResidentParams P)
+// MAXT: the block size the registers are budgeted for (256: small blocks get what the compiler asks for, 1024: 64)
+template <int CM, int ST, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) k_cluster_u8(const __grid_constant__ ResidentParams P)
 {
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();

@@ -20,6 +20,6 @@ const void *resident_kernel(int cm, int stream_spec, int W, int small);
 cudaError_t launch_batch(int cm, int stream_spec, const BatchParams &B, const BatchTable &T, int n, int nthreads, size_t smem, cudaStream_t st);
 
 // k_cluster.cu
-const void *cluster_kernel(int cm, int stream_spec);
+const void *cluster_kernel(int cm, int stream_spec, int nthreads);   // nthreads: block size (register budget)
 
 }  // namespace potts

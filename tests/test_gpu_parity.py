@@ -259,7 +259,9 @@ def test_ladder_protocol_matches_oracle_and_call_sequence(pb):
 
 
 # ---- replica batch: lattice r of a batch == a single handle with (seed_r, T_r) ---------------------------
-@pytest.mark.parametrize("L,q,n", [(64, 9, 5), (32, 2, 3), (128, 24, 4), (96, 200, 2), (256, 6, 3)])
+@pytest.mark.parametrize("L,q,n", [(64, 9, 5), (32, 2, 3), (128, 24, 4), (96, 200, 2), (256, 6, 3),
+                                   (160, 12, 2),      # 1024 / (L/8) thread rows would be odd: made even (one parity per thread)
+                                   (416, 9, 2)])      # the largest lattice a CTA holds beside the 32 KB accept table: 18 thread rows over 416 rows, uneven
 def test_batch_replicas_match_oracle(pb, L, q, n):
     seeds = [1000 + 7 * r + (r << 40) for r in range(n)]
     Ts = [(0.9 + 0.1 * r) * workloads.t_c(q) for r in range(n)]
