@@ -123,12 +123,13 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
 
     const uint32_t tid = threadIdx.x, nthreads = blockDim.x;
     const int cpr = pitch / (4 * W);                                // compute threads per plane row
-    const int ccomm = pitch >> 3;                                   // comm threads: always one 8-site chunk (2 packets) each
+    const int ccomm = pitch >> 3;                                   // 8-site chunks (2 packets each) of a halo row; the comm threads share them
     const int tyc = P.tyc;
     const int ncompute = cpr * tyc;
     const int nbar = (ncompute + 31) & ~31;                         // compute warps, in threads
     const bool is_compute = (int)tid < ncompute;
     const int ctx = (int)tid - nbar;                                // comm thread index
+    const int ncomm = (int)nthreads - nbar;                         // comm threads: chunk ctx, ctx + ncomm, ... each
     const bool is_comm = ctx >= 0 && ctx < ccomm;
     const int ty = is_compute ? (int)tid / cpr : 0;
     const int cx = is_compute ? (int)tid - ty * cpr : 0;
@@ -181,7 +182,7 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
     auto inbox = [&](uint32_t x, uint32_t c, uint32_t s) { return P.inbox + ((size_t)(x * 2 + c) * 2 + s) * wpr + (col >> 2); };
     uint2 *const send_up0 = inbox(up_cta, 0, 1);     // my first row -> the row below the last row of the CTA above
     uint2 *const send_dn0 = inbox(dn_cta, 0, 0);     // my last row  -> the row above the first row of the CTA below
-    const uint2 *const recv0 = inbox(b, 0, 0);       // colour c: + c * 2 * wpr, side s: + s * wpr
+    const uint2 *const recv0 = inbox(b, 0, 0);       // colour c: + c * 2 * wpr, side s: + s * wpr, chunk ch beyond mine: + 2 (ch - ctx)
     const uint32_t cstride = 2u * wpr;
     const int halo_bar = 32 * nbw + ((int)nthreads - nbar);         // boundary warps + comm warps, in threads
 
@@ -292,18 +293,22 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
                 // comm warps: receive the rows the neighbours sent at the end of the PREVIOUS half-sweep (plane 1-c,
                 // tag seq-1) into the halo rows of plane 1-c, which only the boundary phase of this half-sweep reads
                 if (is_comm && seq > 1) {
-                    uint8_t *const halo = s_raw + (1u - c) * plane_stride + col;
 #pragma unroll 1
-                    for (int s = 0; s < 2; ++s) {
-                        const uint2 *src = recv0 + (1u - c) * cstride + (uint32_t)s * wpr;
-                        uint4 v = ld_packet2(src);
-                        long long spins = 0;
-                        while (v.y != seq - 1 || v.w != seq - 1) {
-                            if (++spins > RESIDENT_SPIN_LIMIT) { atomicExch(P.error, 1); break; }
-                            __nanosleep(40);
-                            v = ld_packet2(src);
+                    for (int ch = ctx; ch < ccomm; ch += ncomm) {
+                        const uint32_t more = (uint32_t)(ch - ctx);                            // chunks beyond my first one
+                        uint8_t *const halo = s_raw + (1u - c) * plane_stride + col + 8u * more;
+#pragma unroll 1
+                        for (int s = 0; s < 2; ++s) {
+                            const uint2 *src = recv0 + (1u - c) * cstride + (uint32_t)s * wpr + 2u * more;
+                            uint4 v = ld_packet2(src);
+                            long long spins = 0;
+                            while (v.y != seq - 1 || v.w != seq - 1) {
+                                if (++spins > RESIDENT_SPIN_LIMIT) { atomicExch(P.error, 1); break; }
+                                __nanosleep(40);
+                                v = ld_packet2(src);
+                            }
+                            *reinterpret_cast<uint2 *>(halo + (s == 0 ? 0u : (uint32_t)((rows + 1) * pitch))) = make_uint2(v.x, v.z);
                         }
-                        *reinterpret_cast<uint2 *>(halo + (s == 0 ? 0u : (uint32_t)((rows + 1) * pitch))) = make_uint2(v.x, v.z);
                     }
                 }
                 named_barrier_arrive(1, halo_bar);
@@ -312,9 +317,11 @@ __device__ __forceinline__ void resident_run(const ResidentParams &P, const Resi
             if (G == 1) {
                 // a single CTA is its own neighbour: wrap the rows inside shared memory
                 if (is_comm) {
-                    uint8_t *const mine = s_raw + c * plane_stride + col;
-                    *reinterpret_cast<uint2 *>(mine) = *reinterpret_cast<const uint2 *>(mine + (uint32_t)(rows * pitch));
-                    *reinterpret_cast<uint2 *>(mine + (uint32_t)((rows + 1) * pitch)) = *reinterpret_cast<const uint2 *>(mine + pitch);
+                    for (int ch = ctx; ch < ccomm; ch += ncomm) {
+                        uint8_t *const mine = s_raw + c * plane_stride + col + 8u * (uint32_t)(ch - ctx);
+                        *reinterpret_cast<uint2 *>(mine) = *reinterpret_cast<const uint2 *>(mine + (uint32_t)(rows * pitch));
+                        *reinterpret_cast<uint2 *>(mine + (uint32_t)((rows + 1) * pitch)) = *reinterpret_cast<const uint2 *>(mine + pitch);
+                    }
                 }
                 __syncthreads();
             }
