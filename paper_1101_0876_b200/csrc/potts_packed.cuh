@@ -78,7 +78,10 @@ struct PackedSweepParams {
     uint32_t *tile_counter;      // device word, 0 at launch and again after it (see k_sweep_rows_u8)
 };
 
-constexpr int PK_WARPS = 4;
+// 8 warps share a block's 48 KB of tables (ColKeys + accept table), three blocks per SM (80 registers): 24 warps per SM.
+// With 4 warps per block the shared memory held an SM to 4 blocks = 16 warps: cfg4 3.02 -> 2.75 ps per update.
+constexpr int PK_WARPS = 8;
+constexpr int PK_MIN_BLOCKS = 3;
 constexpr int PK_SITES = 32;     // same-colour sites per lane and row: 16 bytes of nibbles (+ 4 bytes of high bits)
 
 // Half-sweep, packed layout, one launch per colour: k_sweep_rows_u8 (potts_kernels.cuh) on packed planes.  A block owns
@@ -86,11 +89,11 @@ constexpr int PK_SITES = 32;     // same-colour sites per lane and row: 16 bytes
 // updates one 32-site chunk per row.  The other-colour rows i-1, i, i+1 roll through registers UNPACKED (and doubled
 // for the nibble compare), so a loaded word is unpacked once instead of once per use (three rows use it); the column
 // part of Philox (ColKeys) of the tile's 2 x 1024 columns is computed once per block into 32 KB of shared memory.
-// grid = as many blocks as are resident at once (or fewer tiles), block = (32, PK_WARPS); tiles drawn dynamically.
+// grid = as many blocks as are resident at once (or fewer tiles), block = (32, PK_WARPS = 8); tiles drawn dynamically.
 // DELTA (potts_sweep_delta): instead of the energy, add the sum of the accepted moves'
 // d = n_old - n_new of this half-sweep to *P.E_out (two's-complement int64).
 template <bool FIVE, int ST, int COLOUR, bool MEASURE, bool HIST, bool DELTA, bool FAST>
-__global__ void __launch_bounds__(32 * PK_WARPS) k_sweep_rows_packed(const __grid_constant__ PackedSweepParams P)
+__global__ void __launch_bounds__(32 * PK_WARPS, PK_MIN_BLOCKS) k_sweep_rows_packed(const __grid_constant__ PackedSweepParams P)
 {
     constexpr bool EX = MEASURE || DELTA;
     static_assert(!(FAST && EX), "the sums need the exact form of the acceptance");
