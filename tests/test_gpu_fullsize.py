@@ -73,6 +73,29 @@ def test_cfg3_full_size_scan_start(pb):
     assert (g.potts_download() == o.spins()).all()
 
 
+@pytest.mark.parametrize("L,q,opts", [
+    (3072, 9, {"variant": 2}),                                       # 192 chunks per halo row over 64 comm threads: three each
+    (2304, 6, {"variant": 2, "resident_ctas": 37}),                  # 144 chunks: sixteen comm threads get three, the rest two
+    (4096, 24, {"variant": 2, "resident_ctas": 148, "resident_rows": 1}),
+    (2560, 200, {"variant": 2, "resident_words": 2, "resident_ctas": 100}),
+])
+def test_resident_comm_threads_share_the_halo_chunks(pb, L, q, opts):
+    """Beyond L = 2048 the resident kernel's 64 comm threads each receive several 8-site chunks of a halo row
+    (potts_resident.cuh): every sweep of a short run against the oracle, on even and uneven chunk splits."""
+    g = pb.Potts(L, q, 31, workloads.INIT_RANDOM)
+    for k, v in opts.items():
+        g.potts_set_option(k, v)
+    assert g.potts_get_option("resident_active") > 1
+    o = oracle.OraclePotts(L, q, 31, workloads.INIT_RANDOM, threads=len(os.sched_getaffinity(0)))
+    T = 0.99 * workloads.t_c(q)
+    Eg, Hg = g.potts_sweep_measured(T, 4, 1, hist=True)
+    Eo, Ho = o.sweep_measured(T, 4, 1, hist=True)
+    assert (Eg == Eo).all() and (Hg == Ho).all()
+    g.potts_sweep(T, 3)
+    o.sweep(T, 3)
+    assert (g.potts_download() == o.spins()).all() and g.potts_energy() == o.energy()
+
+
 def test_cfg4_full_size_packed(pb):
     w = workloads.CONFIGS[4]
     T = w.temperatures[0]
