@@ -401,11 +401,12 @@ struct BatchParams {
 // to fill (the row above local row 1 IS local row L, read in place), one block barrier per half-sweep.  Block =
 // L/8 x tyc threads with tyc EVEN: thread row ty visits the rows 1+ty, 1+ty+tyc, ..., all of one parity, so the column
 // part of Philox (ColKeys) of its four columns is computed once per half-sweep into registers and serves every visit.
-#ifndef POTTS_BATCH_MINB
-#define POTTS_BATCH_MINB 3
-#endif
+// Register budget: blocks of up to 256 threads (L <= 64: two visits per thread) are compiled for three blocks per SM = 78
+// registers (measured at 888 cfg1 lattices: 3.44 ps per update; four blocks = 64 registers: 3.52; the 60 registers of the
+// shared resident body before: 4.37), up to 512 threads for one block = up to 128 registers, larger ones 64.
+constexpr int BATCH_MIN_BLOCKS = 3;
 template <int CM, int ST, int MAXT>
-__global__ void __launch_bounds__(MAXT, MAXT <= 256 ? POTTS_BATCH_MINB : 1) k_resident_batch_u8(const __grid_constant__ BatchParams B, const __grid_constant__ BatchTable T)
+__global__ void __launch_bounds__(MAXT, MAXT <= 256 ? BATCH_MIN_BLOCKS : 1) k_resident_batch_u8(const __grid_constant__ BatchParams B, const __grid_constant__ BatchTable T)
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
     __shared__ AcceptLutWide lut;

@@ -9,7 +9,7 @@ Both sides run the configuration's temperature ladder from its start state in ch
 chunk the energy (and histogram) series of the chunk are compared entry by entry, and every `spin_every` chunks the whole
 spin configuration.  The oracle runs in its row-parallel mode (same bits as serial, tests/test_oracle_pins.py).
 POTTS_FULL_LENGTH_LIMIT bounds the number of sweeps.  Records: profiles/r01d_full_length_parity.md (round 1),
-profiles/r02d_full_length_parity.md (round 2).
+profiles/r02d_full_length_parity.md and r02j_full_length_parity.md (round 2; r02j: all five complete).
 """
 import os
 import sys
