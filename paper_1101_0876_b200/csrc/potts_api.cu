@@ -422,7 +422,7 @@ ClusterPlan plan_cluster(const potts_t *h)
     R.nthreads = (wpr * tyc + 31) / 32 * 32;
     if ((R.rows_max + tyc - 1) / tyc > 60) { R.why = "too many rows per thread"; return R; }
     const size_t hist = 2 * (size_t)(h->q <= (int)potts::HIST_LANE_QMAX ? h->q * 32 : h->q) * 4;   // two tables
-    R.smem = 2 * (size_t)(R.rows_max + 2) * (L / 2) + hist;
+    R.smem = 2 * (size_t)(R.rows_max + 2) * (L / 2) + hist + 8 * (size_t)(L / 2);   // planes, histogram tables, packet inbox
     if (R.smem + STATIC_SMEM > h->smem_optin) { R.why = "lattice does not fit the shared memory of one cluster"; return R; }
     R.ok = true;
     return R;
