@@ -408,11 +408,11 @@ def test_persistent_kernels_are_deterministic_under_repetition(pb):
 
 
 @pytest.mark.parametrize("L,q,ctas", [(64, 9, 4), (64, 9, 1), (32, 6, 2), (128, 24, 16), (96, 3, 3), (64, 200, 8)])
-def test_cluster_kernel_mbarrier_phases_over_many_launches(pb, L, q, ctas):
-    """The cluster kernel's neighbour exchange (st.async into the neighbour's halo, completion counted by an mbarrier in
-    the receiver's shared memory, potts_cluster.cuh) keeps one phase per sweep and halo: launches of 1, 2, 3, ... sweeps
-    (odd and even phase counts, the wait-free first half-sweep, the drained last one), with every measurement form in
-    turn, must follow the oracle's chain bit for bit, and repeat it."""
+def test_cluster_kernel_exchange_over_many_launches(pb, L, q, ctas):
+    """The cluster kernel's neighbour exchange (8-byte packets {4 spins | half-sweep number} into the neighbour's inbox in
+    its shared memory, polled by the thread that needs them, potts_cluster.cuh) numbers its half-sweeps per launch:
+    launches of 1, 2, 3, ... sweeps (the packet-free first half-sweep, odd and even counts, an inbox that starts zeroed
+    every time), with every measurement form in turn, must follow the oracle's chain bit for bit, and repeat it."""
     seed = 21
     T = 0.99 * workloads.t_c(q)
     for rep in range(2):
