@@ -65,3 +65,63 @@ def test_random_case_matches_oracle(pb, case):
     o.sweep(T, 2)
     assert (g.potts_download() == o.spins()).all()
     assert g.potts_energy() == o.energy() and (g.potts_histogram() == o.histogram()).all()
+
+
+@pytest.mark.slow
+def test_cluster_kernel_soak(pb):
+    """Randomised soak of the cluster kernel's lock-free packet exchange (potts_cluster.cuh): for POTTS_SOAK_SECONDS
+    (default 60) seconds random (L <= 288, q, cluster size, stream definition, seed, temperature) runs of three calls of
+    random length and kind (measured, plain, energy-change series) against the oracle, each followed by a second handle
+    that repeats the chain in one call (determinism).  Collected but skipped unless POTTS_RUN_SLOW=1; record:
+    profiles/r02h_cluster_exchange.md."""
+    import os
+    import time
+    seconds = float(os.environ.get("POTTS_SOAK_SECONDS", "60"))
+    rng = np.random.default_rng(12345)
+    t0, n_ok = time.time(), 0
+    while time.time() - t0 < seconds:
+        L = int(rng.choice([32, 64, 96, 128, 160, 192, 256, 288]))
+        q = int(rng.choice([2, 3, 6, 9, 16, 17, 24, 128, 129, 256]))
+        G = int(rng.choice([0, 1, 2, 3, 4, 5, 7, 8, 12, 16]))
+        st = int(rng.choice([1, 2]))
+        seed = int(rng.integers(1, 2 ** 62))
+        T = float(rng.choice([0.5, 0.9, 0.99, 1.0, 1.05, 2.0])) * workloads.t_c(q)
+        case = (L, q, G, st, seed, T)
+
+        def handle():
+            g = pb.Potts(L, q, seed, workloads.INIT_RANDOM)
+            g.potts_set_option("variant", 3)
+            g.potts_set_option("cluster_ctas", G)
+            if st == 2:
+                g.potts_set_stream_spec(2)
+            return g
+        g = handle()
+        if g.potts_get_option("cluster_active") == 0:
+            g.close()
+            continue
+        o = oracle.OraclePotts(L, q, seed, workloads.INIT_RANDOM, stream=st, threads=8)
+        for _ in range(3):
+            n, kind = int(rng.integers(1, 40)), int(rng.integers(0, 3))
+            if kind == 0:
+                Eg, Hg = g.potts_sweep_measured(T, n, 1, hist=True)
+                Eo, Ho = o.sweep_measured(T, n, 1, hist=True)
+                assert (Eg == Eo).all() and (Hg == Ho).all(), case
+            elif kind == 1:
+                g.potts_sweep(T, n)
+                o.sweep(T, n)
+            else:
+                e0, es = o.energy(), []
+                d = g.potts_sweep_delta(T, n)
+                for _ in range(n):
+                    o.sweep(T, 1)
+                    es.append(o.energy())
+                assert (d == np.diff(np.array([e0] + es, dtype=np.int64))).all(), case
+            assert g.potts_energy() == o.energy(), case
+        assert (g.potts_download() == o.spins()).all(), case
+        g2 = handle()
+        g2.potts_sweep(T, int(o.t))
+        assert (g2.potts_download() == o.spins()).all(), case
+        g.close()
+        g2.close()
+        n_ok += 1
+    print(f"CLUSTER SOAK OK: {n_ok} random cases identical to the oracle and repeatable, {time.time() - t0:.0f} s", flush=True)
