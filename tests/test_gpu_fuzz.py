@@ -125,3 +125,44 @@ def test_cluster_kernel_soak(pb):
         g2.close()
         n_ok += 1
     print(f"CLUSTER SOAK OK: {n_ok} random cases identical to the oracle and repeatable, {time.time() - t0:.0f} s", flush=True)
+
+
+@pytest.mark.slow
+def test_resident_kernel_large_lattice_soak(pb):
+    """Randomised soak of the resident kernel beyond L = 2048, where 64 comm threads share the chunks of a halo row
+    (potts_resident.cuh): for POTTS_SOAK_SECONDS (default 60) seconds random (L, q, grid size, words per thread, thread
+    rows, stream definition, seed) runs of a few measured sweeps against the oracle.  Collected but skipped unless
+    POTTS_RUN_SLOW=1; record: profiles/r02i_occupancy.md."""
+    import os
+    import time
+    seconds = float(os.environ.get("POTTS_SOAK_SECONDS", "60"))
+    rng = np.random.default_rng(777)
+    threads = len(os.sched_getaffinity(0))
+    t0, n_ok = time.time(), 0
+    while time.time() - t0 < seconds:
+        L = int(rng.choice([2080, 2112, 2304, 2560, 3072, 3104, 3584, 4064, 4096]))
+        q = int(rng.choice([2, 6, 9, 16, 24, 129]))
+        G = int(rng.choice([0, 37, 64, 100, 111, 147, 148]))
+        W = int(rng.choice([0, 2]))
+        rows = int(rng.choice([0, 1, 2, 3]))
+        st = int(rng.choice([1, 2]))
+        seed = int(rng.integers(1, 2 ** 62))
+        T = float(rng.choice([0.9, 1.0, 1.1])) * workloads.t_c(q)
+        case = (L, q, G, W, rows, st, seed)
+        g = pb.Potts(L, q, seed, workloads.INIT_RANDOM)
+        for k, v in (("variant", 2), ("resident_ctas", G), ("resident_words", W), ("resident_rows", rows)):
+            g.potts_set_option(k, v)
+        if st == 2:
+            g.potts_set_stream_spec(2)
+        if g.potts_get_option("resident_active") == 0:
+            g.close()
+            continue
+        o = oracle.OraclePotts(L, q, seed, workloads.INIT_RANDOM, stream=st, threads=threads)
+        n = int(rng.integers(2, 5))
+        Eg, Hg = g.potts_sweep_measured(T, n, 1, hist=True)
+        Eo, Ho = o.sweep_measured(T, n, 1, hist=True)
+        assert (Eg == Eo).all() and (Hg == Ho).all(), case
+        assert (g.potts_download() == o.spins()).all(), case
+        g.close()
+        n_ok += 1
+    print(f"RESIDENT SOAK OK: {n_ok} random cases beyond L = 2048 identical to the oracle, {time.time() - t0:.0f} s", flush=True)
