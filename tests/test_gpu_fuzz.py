@@ -166,3 +166,43 @@ def test_resident_kernel_large_lattice_soak(pb):
         g.close()
         n_ok += 1
     print(f"RESIDENT SOAK OK: {n_ok} random cases beyond L = 2048 identical to the oracle, {time.time() - t0:.0f} s", flush=True)
+
+
+@pytest.mark.slow
+def test_batch_kernel_soak(pb):
+    """Randomised soak of the replica-batch kernel's own body (potts_resident.cuh, k_resident_batch_u8): for
+    POTTS_SOAK_SECONDS (default 60) seconds random (L <= 416, q, number of replicas, stream definition, seeds,
+    temperatures) batches, a measured call, an energy-change call and the final spins of every replica against the
+    oracle.  Collected but skipped unless POTTS_RUN_SLOW=1; record: profiles/r02i_occupancy.md."""
+    import os
+    import time
+    seconds = float(os.environ.get("POTTS_SOAK_SECONDS", "60"))
+    rng = np.random.default_rng(4242)
+    t0, n_ok = time.time(), 0
+    while time.time() - t0 < seconds:
+        L = int(rng.choice([32, 64, 96, 128, 160, 192, 224, 256, 320, 416]))
+        q = int(rng.choice([2, 3, 6, 9, 16, 17, 24, 129, 256]))
+        n = int(rng.integers(1, 7))
+        st = int(rng.choice([1, 2]))
+        seeds = [int(x) for x in rng.integers(1, 2 ** 62, size=n)]
+        Ts = [float(rng.choice([0.5, 0.99, 1.0, 1.05, 2.0])) * workloads.t_c(q) for _ in range(n)]
+        case = (L, q, n, st, seeds[0])
+        b = pb.PottsBatch(L, q, seeds, workloads.INIT_RANDOM)
+        if st == 2:
+            b.potts_batch_set_stream_spec(2)
+        ns, nd = int(rng.integers(1, 9)), int(rng.integers(1, 6))
+        E, H = b.potts_batch_sweep_measured(Ts, ns, 1)
+        dE = b.potts_batch_sweep_delta(Ts, nd)
+        for r in range(n):
+            o = oracle.OraclePotts(L, q, seeds[r], workloads.INIT_RANDOM, stream=st, threads=8)
+            Eo, Ho = o.sweep_measured(Ts[r], ns, 1, hist=True)
+            assert (E[r] == Eo).all() and (H[r] == Ho).all(), (case, r)
+            e0, es = o.energy(), []
+            for _ in range(nd):
+                o.sweep(Ts[r], 1)
+                es.append(o.energy())
+            assert (dE[r] == np.diff(np.array([e0] + es, dtype=np.int64))).all(), (case, r)
+            assert (b.potts_batch_download(r) == o.spins()).all(), (case, r)
+        b.close()
+        n_ok += 1
+    print(f"BATCH SOAK OK: {n_ok} random batches identical to the oracle, {time.time() - t0:.0f} s", flush=True)
